@@ -1,0 +1,211 @@
+"""ctypes front-end of the C oracle + the mu loop of Algorithm 1.
+
+TEST INFRASTRUCTURE, NOT PRODUCT CODE: importable only from tests/, __graft_entry__.smoke()
+and bench.py's cpu_baseline / --impl reference legs.  Shares nothing with the CUDA path; the
+only common module is the seeded input generator (paper_2004_10811_b200.workloads), which
+contains none of the method's arithmetic.
+
+All arithmetic of the method lives in submatrix_oracle.c; this file marshals arrays and runs
+the scalar mu loop:
+    n_elec(mu) = sum_i sum_{k in gen(i)} ( 1/2 - 1/2 sum_l Q_{k,l}^2 signum(lambda_l - mu) )
+               = sum_i ( |gen(i)|/2 - 1/2 sum_l w_{i,l} signum(lambda_{i,l} - mu) )   (Algorithm 1)
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.orc_index_count.restype = C.c_int64
+        _lib.orc_jacobi_eig.restype = C.c_int
+        _lib.orc_dense_sign.restype = C.c_int
+    return _lib
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _i64(a):
+    return np.ascontiguousarray(a, dtype=np.int64)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+class Index:
+    """Submatrix index of a pattern + grouping (step "index", L125/L199)."""
+
+    def __init__(self, m):
+        L = lib()
+        self.m = m
+        self.blk_size, self.colptr, self.rowidx = _i32(m.blk_size), _i64(m.colptr), _i32(m.rowidx)
+        self.grp_ptr, self.grp_cols = _i32(m.grp_ptr), _i32(m.grp_cols)
+        ng = len(self.grp_ptr) - 1
+        self.sub_ptr = np.zeros(ng + 1, dtype=np.int64)
+        tot = L.orc_index_count(C.c_int32(m.nb), _p(self.colptr, C.c_int64), _p(self.rowidx, C.c_int32),
+                                C.c_int32(ng), _p(self.grp_ptr, C.c_int32), _p(self.grp_cols, C.c_int32),
+                                _p(self.sub_ptr, C.c_int64))
+        self.sub_blocks = np.zeros(max(tot, 1), dtype=np.int32)[:tot]
+        self.sub_off = np.zeros(max(tot, 1), dtype=np.int32)[:tot]
+        self.sub_dim = np.zeros(ng, dtype=np.int32)
+        self.gen_pos = np.zeros(len(self.grp_cols), dtype=np.int32)
+        L.orc_index_fill(C.c_int32(m.nb), _p(self.blk_size, C.c_int32), _p(self.colptr, C.c_int64),
+                         _p(self.rowidx, C.c_int32), C.c_int32(ng), _p(self.grp_ptr, C.c_int32),
+                         _p(self.grp_cols, C.c_int32), _p(self.sub_ptr, C.c_int64),
+                         _p(self.sub_blocks, C.c_int32), _p(self.sub_off, C.c_int32),
+                         _p(self.sub_dim, C.c_int32), _p(self.gen_pos, C.c_int32))
+        self.val_off = _i64(m.val_off())
+        self.ngroups = ng
+        # number of generating basis functions per group (|gen(i)| in Algorithm 1)
+        self.gen_width = np.array([int(self.blk_size[self.grp_cols[self.grp_ptr[i]:self.grp_ptr[i + 1]]].sum())
+                                   for i in range(ng)], dtype=np.int64)
+
+
+def assemble(idx: Index, values, i: int) -> np.ndarray:
+    """Dense a_i (step "assemble", L125).  Returns an (n_i, n_i) array (symmetric)."""
+    n = int(idx.sub_dim[i])
+    a = np.zeros((n, n))
+    s, e = int(idx.sub_ptr[i]), int(idx.sub_ptr[i + 1])
+    S, So = _i32(idx.sub_blocks[s:e]), _i32(idx.sub_off[s:e])
+    v = _f64(values)
+    lib().orc_assemble(_p(idx.blk_size, C.c_int32), _p(idx.colptr, C.c_int64), _p(idx.rowidx, C.c_int32),
+                       _p(idx.val_off, C.c_int64), _p(v, C.c_double), C.c_int64(e - s),
+                       _p(S, C.c_int32), _p(So, C.c_int32), C.c_int32(n), _p(a, C.c_double))
+    return a.T  # column-major -> numpy view
+
+
+def jacobi_eig(a: np.ndarray):
+    """Cyclic Jacobi: returns (lam[n], Q[n,n]) with a = Q diag(lam) Q^T (Eq.(17))."""
+    n = a.shape[0]
+    w = _f64(a).copy()
+    qt = np.zeros((n, n))
+    lam = np.zeros(n)
+    lib().orc_jacobi_eig(C.c_int32(n), _p(w, C.c_double), _p(qt, C.c_double), _p(lam, C.c_double))
+    return lam, qt.T.copy()
+
+
+def dense_sign(a: np.ndarray, mu: float = 0.0) -> np.ndarray:
+    """sign(a - mu I) of one dense symmetric matrix via Jacobi (Eq.(17), Eq.(12))."""
+    n = a.shape[0]
+    aa = _f64(a)
+    s = np.zeros((n, n))
+    lib().orc_dense_sign(C.c_int32(n), _p(aa, C.c_double), C.c_double(mu), _p(s, C.c_double), None)
+    return s
+
+
+def _run_groups(idx: Index, values, groups, mu, do_extract, want_eig, nthreads):
+    groups = _i32(np.arange(idx.ngroups) if groups is None else groups)
+    v = _f64(values)
+    out = np.zeros_like(v) if do_extract else None
+    lw_ptr = np.zeros(len(groups) + 1, dtype=np.int64)
+    np.cumsum(idx.sub_dim[groups], out=lw_ptr[1:])
+    lam = np.zeros(int(lw_ptr[-1])) if want_eig else None
+    w = np.zeros(int(lw_ptr[-1])) if want_eig else None
+    lib().orc_submatrix_groups(
+        _p(idx.blk_size, C.c_int32), _p(idx.colptr, C.c_int64), _p(idx.rowidx, C.c_int32),
+        _p(idx.val_off, C.c_int64), _p(v, C.c_double), _p(idx.grp_ptr, C.c_int32),
+        _p(idx.grp_cols, C.c_int32), _p(idx.sub_ptr, C.c_int64), _p(idx.sub_blocks, C.c_int32),
+        _p(idx.sub_off, C.c_int32), _p(idx.sub_dim, C.c_int32), _p(idx.gen_pos, C.c_int32),
+        C.c_int32(len(groups)), _p(groups, C.c_int32), C.c_double(mu), C.c_int32(1 if do_extract else 0),
+        _p(out, C.c_double), _p(lw_ptr, C.c_int64), _p(lam, C.c_double), _p(w, C.c_double),
+        C.c_int32(nthreads))
+    return out, lam, w, lw_ptr, groups
+
+
+def density(idx: Index, values, mu: float, groups=None, nthreads: int = 0) -> np.ndarray:
+    """D~ = 1/2 (I - sign(K~ - mu I)) by the submatrix method on the input pattern (L123-127).
+    Only the block columns of the listed groups are filled (others stay 0)."""
+    return _run_groups(idx, values, groups, mu, True, False, nthreads)[0]
+
+
+def eig_groups(idx: Index, values, groups=None, nthreads: int = 0):
+    """Eigenvalues lambda_{i,l} and weights w_{i,l} of the listed groups (Algorithm 1).
+    Returns (lam, w, ptr, groups)."""
+    _, lam, w, ptr, g = _run_groups(idx, values, groups, 0.0, False, True, nthreads)
+    return lam, w, ptr, g
+
+
+def nelec(idx: Index, lam, w, groups, mu: float) -> float:
+    """Algorithm 1 inner loops for one mu."""
+    ngen = float(idx.gen_width[groups].sum())
+    return 0.5 * ngen - 0.5 * float(np.sum(w * np.sign(lam - mu)))
+
+
+def column_ids_of_groups(idx: Index, groups) -> np.ndarray:
+    return np.concatenate([idx.grp_cols[idx.grp_ptr[g]:idx.grp_ptr[g + 1]] for g in groups]).astype(np.int32)
+
+
+def traces(idx: Index, D, K, cols=None):
+    """(tr D, tr D K) (Eq.(18), Eq.(10)); restricted to block columns `cols` if given."""
+    td, tdk = C.c_double(0), C.c_double(0)
+    D, K = _f64(D), _f64(K)
+    cc = _i32(cols) if cols is not None else None
+    lib().orc_traces(C.c_int32(idx.m.nb), _p(idx.blk_size, C.c_int32), _p(idx.colptr, C.c_int64),
+                     _p(idx.rowidx, C.c_int32), _p(idx.val_off, C.c_int64), _p(D, C.c_double),
+                     _p(K, C.c_double), C.c_int32(-1 if cc is None else len(cc)), _p(cc, C.c_int32),
+                     C.byref(td), C.byref(tdk))
+    return td.value, tdk.value
+
+
+def gershgorin_interval(m) -> tuple[float, float]:
+    """Gershgorin interval of the whole block-sparse matrix: bracket for the mu loop (A11)."""
+    cols = m.block_cols()
+    voff = m.val_off()
+    boff = m.blk_off()
+    n = int(boff[-1])
+    diag = np.zeros(n)
+    rad = np.zeros(n)
+    for b in range(m.nnzb):
+        r, c = int(m.rowidx[b]), int(cols[b])
+        br, bc = int(m.blk_size[r]), int(m.blk_size[c])
+        blk = m.values[voff[b]:voff[b + 1]].reshape(bc, br)  # [q, e] column-major
+        colsum = np.abs(blk).sum(axis=1)
+        if r == c:
+            d = np.diagonal(blk).copy()
+            diag[boff[c]:boff[c] + bc] = d
+            colsum = colsum - np.abs(d)
+        rad[boff[c]:boff[c] + bc] += colsum
+    return float((diag - rad).min()), float((diag + rad).max())
+
+
+def bisect_mu(idx: Index, lam, w, groups, n_target: float, mu0: float, lo: float, hi: float,
+              tol_n: float, mu_tol: float = 1e-6, max_steps: int = 64):
+    """Algorithm 1 (L272-276) with the update rule of reading A11: evaluate mu0, then
+    midpoint bisection on g(mu) = n_elec(mu) - n_target inside [lo, hi] (raise mu if g < 0).
+    Stops on |g| <= tol_n, bracket width <= mu_tol, or max_steps; returns the evaluated mu with
+    the smallest |g| and the trace [(mu, n_elec), ...]."""
+    trace = []
+    mu = mu0
+    best = None
+    for _ in range(max_steps):
+        ne = nelec(idx, lam, w, groups, mu)
+        g = ne - n_target
+        trace.append((mu, ne))
+        if best is None or abs(g) < abs(best[1]):
+            best = (mu, g)
+        if abs(g) <= tol_n:
+            break
+        if g < 0:
+            lo = max(lo, mu)
+        else:
+            hi = min(hi, mu)
+        if hi - lo <= mu_tol:
+            break
+        mu = 0.5 * (lo + hi)
+    return best[0], best[1] + n_target, trace

@@ -1,0 +1,293 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (not against itself).
+
+Each test names the passage (PAPER.md line) or the textbook fact it rests on."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2004_10811_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _load(name):
+    return np.loadtxt(os.path.join(GOLD, name), comments="#")
+
+
+def _blocks_from_dense(a, bs, mask=None, groups=None):
+    """Pack a dense symmetric matrix into the block layout (data movement only)."""
+    bs = np.asarray(bs, dtype=np.int32)
+    nb = len(bs)
+    off = np.concatenate([[0], np.cumsum(bs)])
+    rows, cols, vals = [], [], []
+    for c in range(nb):
+        for r in range(nb):
+            blk = a[off[r]:off[r + 1], off[c]:off[c + 1]]
+            keep = (mask[r, c] if mask is not None else (np.any(blk != 0) or r == c))
+            if keep:
+                rows.append(r); cols.append(c); vals.append(blk.T.reshape(-1))
+    colptr = np.zeros(nb + 1, dtype=np.int64)
+    np.cumsum(np.bincount(cols, minlength=nb), out=colptr[1:])
+    if groups is None:
+        groups = [[c] for c in range(nb)]
+    grp_ptr = np.concatenate([[0], np.cumsum([len(g) for g in groups])]).astype(np.int32)
+    grp_cols = np.concatenate(groups).astype(np.int32)
+    return W.BlockSparseSym(nb, bs, colptr, np.array(rows, dtype=np.int32), np.concatenate(vals),
+                            grp_ptr, grp_cols)
+
+
+# ---------------------------------------------------------------- golden closed forms
+def test_golden_sign_2x2(oracle):
+    g = _load("sign_2x2.txt")
+    assert np.allclose(oracle.dense_sign(g[:2]), g[2:], atol=1e-15)
+
+
+def test_golden_zero_eigenvalue(oracle):
+    """Eq.(12): an eigenvalue exactly 0 maps to 0."""
+    g = _load("sign_zero_eig.txt")
+    assert np.allclose(oracle.dense_sign(g[:2]), g[2:], atol=1e-15)
+    # mu shifts the spectrum (Eq.16): A - 2I has eigenvalues -2, 0 -> sign = -v0 v0^T
+    assert np.allclose(oracle.dense_sign(g[:2], mu=2.0), [[-0.5, 0.5], [0.5, -0.5]], atol=1e-15)
+
+
+def test_golden_submatrix_3x3(oracle):
+    """Steps 1-3 (L125-127) worked by hand on a 3x3 tridiagonal matrix with 1x1 blocks."""
+    a = np.array([[3.0, 4, 0], [4, -3, 4], [0, 4, 3]])
+    m = _blocks_from_dense(a, [1, 1, 1])
+    idx = oracle.Index(m)
+    assert list(idx.sub_dim) == [2, 3, 2]
+    assert list(idx.sub_blocks) == [0, 1, 0, 1, 2, 1, 2]
+    assert list(idx.gen_pos) == [0, 1, 1]
+    d = m.to_dense(oracle.density(idx, m.values, 0.0))
+    sign_tilde = np.where(a != 0, np.eye(3) - 2 * d, 0.0)
+    assert np.allclose(sign_tilde, _load("submatrix_3x3.txt"), atol=1e-14)
+    assert d[0, 2] == 0 and d[2, 0] == 0  # pattern retained (L127)
+
+
+def test_ns_scalar_fixture_is_consistent_with_sign():
+    """Eq.(11): the scalar recursion converges to signum(x0); fixture values are exact rationals."""
+    g = _load("ns_scalar.txt")
+    x = 0.5
+    for k in range(3):
+        assert x == g[k]
+        x = 0.5 * x * (3 - x * x)
+
+
+# ---------------------------------------------------------------- Jacobi vs library / closed form
+@pytest.mark.parametrize("n", [1, 2, 7, 64])
+def test_jacobi_vs_lapack(oracle, n):
+    """Library pin: eigenvalues equal numpy.linalg.eigvalsh (LAPACK), a = Q L Q^T, Q orthogonal."""
+    rng = np.random.default_rng(n)
+    a = rng.standard_normal((n, n)); a = 0.5 * (a + a.T)
+    lam, q = oracle.jacobi_eig(a)
+    assert np.allclose(np.sort(lam), np.linalg.eigvalsh(a), atol=1e-13 * max(1, n))
+    assert np.allclose(q @ np.diag(lam) @ q.T, a, atol=1e-13 * max(1, n))
+    assert np.allclose(q.T @ q, np.eye(n), atol=1e-13)
+
+
+def test_sign_closed_form_haar(oracle):
+    """P1 (BASELINE config 1 recipe): A = Q diag(lam) Q^T  =>  sign(A) = Q diag(sgn lam) Q^T."""
+    a, q, lam = W.haar_spectrum_batch(3, 96, seed=5)
+    for b in range(3):
+        expect = (q[b] * np.sign(lam[b])) @ q[b].T
+        assert np.abs(oracle.dense_sign(a[b]) - expect).max() < 5e-13
+
+
+def test_sign_invariants(oracle, cfg0):
+    """P2: sign(a)^2 = I (Fig.13 involutority), commutes with a (Eq.8), symmetric; D_i idempotent,
+    tr D_i = number of eigenvalues below mu (Eq.6/7; count from LAPACK)."""
+    idx = oracle.Index(cfg0)
+    for i, mu in ((0, 0.0), (7, 0.1), (31, -0.9)):
+        a = oracle.assemble(idx, cfg0.values, i)
+        n = a.shape[0]
+        assert np.array_equal(a, a.T)
+        s = oracle.dense_sign(a, mu)
+        am = a - mu * np.eye(n)
+        assert np.abs(s @ s - np.eye(n)).max() < 1e-12
+        assert np.abs(s @ am - am @ s).max() < 1e-12
+        assert np.abs(s - s.T).max() < 1e-13
+        d = 0.5 * (np.eye(n) - s)
+        assert np.abs(d @ d - d).max() < 1e-12
+        assert abs(np.trace(d) - np.sum(np.linalg.eigvalsh(a) < mu)) < 1e-10
+
+
+def test_diagonal_and_2x2_family(oracle):
+    """P3: diagonal matrix -> elementwise signum; [[a,b],[b,-a]] -> A / sqrt(a^2+b^2)."""
+    dvals = np.array([-2.0, 0.5, 0.0, 3.0, -1e-3])
+    assert np.array_equal(oracle.dense_sign(np.diag(dvals)), np.diag(np.sign(dvals)))
+    rng = np.random.default_rng(3)
+    for _ in range(5):
+        a, b = rng.standard_normal(2)
+        m = np.array([[a, b], [b, -a]])
+        assert np.allclose(oracle.dense_sign(m), m / np.hypot(a, b), atol=1e-14)
+
+
+# ---------------------------------------------------------------- index: brute force
+@pytest.mark.parametrize("seed", range(6))
+def test_index_bruteforce(oracle, seed):
+    """P6: S_i = {r : any stored block (r,c), c in G_i}, from a dense boolean mask."""
+    m = W.random_block_pattern(nb=13 + seed, density=0.25, max_bs=4, seed=seed)
+    idx = oracle.Index(m)
+    mask = np.zeros((m.nb, m.nb), dtype=bool)
+    mask[m.rowidx, m.block_cols()] = True
+    for i in range(m.ngroups):
+        gc = m.grp_cols[m.grp_ptr[i]:m.grp_ptr[i + 1]]
+        S = np.nonzero(mask[:, gc].any(axis=1))[0]
+        got = idx.sub_blocks[idx.sub_ptr[i]:idx.sub_ptr[i + 1]]
+        assert np.array_equal(got, S)
+        assert idx.sub_dim[i] == m.blk_size[S].sum()
+        off = np.concatenate([[0], np.cumsum(m.blk_size[S])[:-1]])
+        assert np.array_equal(idx.sub_off[idx.sub_ptr[i]:idx.sub_ptr[i + 1]], off)
+        for g, c in zip(range(m.grp_ptr[i], m.grp_ptr[i + 1]), gc):
+            assert S[idx.gen_pos[g]] == c
+
+
+def test_assemble_is_principal_submatrix(oracle):
+    """L125: a_i equals the dense matrix restricted to the rows/columns of S_i."""
+    m = W.random_block_pattern(nb=11, density=0.3, max_bs=5, seed=42)
+    idx = oracle.Index(m)
+    k = m.to_dense()
+    off = m.blk_off()
+    for i in range(m.ngroups):
+        S = idx.sub_blocks[idx.sub_ptr[i]:idx.sub_ptr[i + 1]]
+        el = np.concatenate([np.arange(off[r], off[r + 1]) for r in S])
+        assert np.array_equal(oracle.assemble(idx, m.values, i), k[np.ix_(el, el)])
+
+
+# ---------------------------------------------------------------- whole pipeline: exactness cases
+def test_full_cutoff_equals_dense_sign(oracle):
+    """P5 (L125): if every column is full, every a_i is the whole matrix and the method is exact:
+    D~ = 1/2 (I - sign(K~)) computed with LAPACK eigh on the whole matrix; tr = N_occ exactly."""
+    m = W.water_like(8, "SZV", cutoff=1e9, seed=3)
+    assert m.nnzb == m.nb * m.nb
+    idx = oracle.Index(m)
+    assert np.all(idx.sub_dim == m.n_basis)
+    d = m.to_dense(oracle.density(idx, m.values, 0.0, nthreads=4))
+    k = m.to_dense()
+    ev, v = np.linalg.eigh(k)
+    dex = v[:, ev < 0] @ v[:, ev < 0].T
+    assert np.abs(d - dex).max() < 1e-12
+    td, tdk = oracle.traces(idx, oracle.density(idx, m.values, 0.0, nthreads=4), m.values)
+    assert abs(td - np.sum(ev < 0)) < 1e-11
+    assert abs(tdk - ev[ev < 0].sum()) < 1e-11  # Eq.(10): Tr(DK) = sum of occupied eigenvalues
+
+
+def test_block_diagonal_is_exact(oracle):
+    """P3: cutoff below the nearest neighbour -> K~ is its on-site diagonal -> D~ = diag(1 on the
+    N(-1,.) functions, 0 on the N(+1,.) ones)."""
+    m = W.water_like(8, "SZV", cutoff=0.1, seed=2)
+    assert m.nnzb == m.nb
+    idx = oracle.Index(m)
+    d = m.to_dense(oracle.density(idx, m.values, 0.0))
+    k = m.to_dense()
+    assert np.array_equal(d, np.diag((np.diag(k) < 0).astype(float)))
+    assert oracle.traces(idx, oracle.density(idx, m.values, 0.0), m.values)[0] == m.n_occ
+
+
+def test_symmetries(oracle, cfg0):
+    """P7: D~(-K,-mu) = I - D~(K,mu) on the pattern; D~(K,mu) = D~(K - mu I, 0); D~(cK, c mu) = D~(K, mu)."""
+    m = cfg0
+    idx = oracle.Index(m)
+    groups = [0, 5, 17]
+    mu = 0.07
+    d = oracle.density(idx, m.values, mu, groups)
+    cols = oracle.column_ids_of_groups(idx, groups)
+    sel = np.zeros(m.nnzb, dtype=bool)
+    bc = m.block_cols()
+    sel[np.isin(bc, cols)] = True
+    emask = np.repeat(sel, np.diff(idx.val_off))
+    # identity on the pattern
+    eye = np.zeros_like(m.values)
+    vo = idx.val_off
+    for b in np.nonzero(m.rowidx == bc)[0]:
+        n = m.blk_size[bc[b]]
+        eye[vo[b]:vo[b + 1]] = np.eye(n).reshape(-1)
+    d_neg = oracle.density(idx, -m.values, -mu, groups)
+    assert np.abs((eye - d)[emask] - d_neg[emask]).max() < 1e-12
+    d_shift = oracle.density(idx, m.values - mu * eye, 0.0, groups)
+    assert np.abs(d_shift - d)[emask].max() < 1e-12
+    d_scale = oracle.density(idx, 3.5 * m.values, 3.5 * mu, groups)
+    assert np.abs(d_scale - d)[emask].max() < 1e-12
+    assert np.all(d[~emask] == 0)  # nothing outside the listed groups' columns
+
+
+def test_atom_relabelling_permutes_result(oracle):
+    """P7: relabelling block columns permutes D~ (index maps carry no hidden order dependence)."""
+    m = W.random_block_pattern(nb=9, density=0.35, max_bs=3, seed=7, ngroups=9, contiguous_groups=True)
+    k = m.to_dense()
+    off = m.blk_off()
+    perm = np.random.default_rng(1).permutation(m.nb)
+    el = np.concatenate([np.arange(off[p], off[p + 1]) for p in perm])
+    kp = k[np.ix_(el, el)]
+    mask = np.zeros((m.nb, m.nb), dtype=bool); mask[m.rowidx, m.block_cols()] = True
+    mp = _blocks_from_dense(kp, m.blk_size[perm], mask=mask[np.ix_(perm, perm)])
+    m1 = _blocks_from_dense(k, m.blk_size, mask=mask)
+    d1 = m1.to_dense(oracle.density(oracle.Index(m1), m1.values, 0.1))
+    dp = mp.to_dense(oracle.density(oracle.Index(mp), mp.values, 0.1))
+    assert np.abs(dp - d1[np.ix_(el, el)]).max() < 1e-12
+
+
+def test_grouping_one_group_is_exact(oracle):
+    """L199: with all block columns in ONE group the single submatrix contains every row that has
+    any stored block, i.e. the whole matrix: result = dense sign restricted to the pattern."""
+    m = W.random_block_pattern(nb=10, density=0.3, max_bs=4, seed=11, ngroups=1)
+    idx = oracle.Index(m)
+    assert idx.sub_dim[0] == m.n_basis
+    d = m.to_dense(oracle.density(idx, m.values, 0.0))
+    k = m.to_dense()
+    ev, v = np.linalg.eigh(k)
+    dex = v[:, ev < 0] @ v[:, ev < 0].T
+    mask = np.zeros_like(k, dtype=bool)
+    off = m.blk_off()
+    for r, c in zip(m.rowidx, m.block_cols()):
+        mask[off[r]:off[r + 1], off[c]:off[c + 1]] = True
+    assert np.abs(d - dex)[mask].max() < 1e-12
+    assert np.all(d[~mask] == 0)
+
+
+# ---------------------------------------------------------------- Algorithm 1
+def test_nelec_matches_trace_and_is_monotone(oracle, cfg0):
+    """Algorithm 1 (L275) vs Eq.(18): n_elec(mu) from (lam, w) equals tr(D~(mu)) of the extracted
+    result; monotone non-decreasing, 0 below and n above the Gershgorin interval (P9)."""
+    m = cfg0
+    idx = oracle.Index(m)
+    groups = np.arange(m.ngroups)
+    lam, w, ptr, g = oracle.eig_groups(idx, m.values, groups, nthreads=8)
+    # weights of each submatrix sum to the generating width (rows of an orthogonal Q)
+    for j in range(len(g)):
+        assert abs(w[ptr[j]:ptr[j + 1]].sum() - idx.gen_width[g[j]]) < 1e-12
+    for mu in (0.0, -0.8):
+        d = oracle.density(idx, m.values, mu, nthreads=8)
+        assert abs(oracle.nelec(idx, lam, w, g, mu) - oracle.traces(idx, d, m.values)[0]) < 1e-10
+    lo, hi = oracle.gershgorin_interval(m)
+    kd = m.to_dense()
+    ev = np.linalg.eigvalsh(kd)
+    assert lo <= ev.min() and hi >= ev.max()
+    assert abs(oracle.nelec(idx, lam, w, g, lo - 1e-9)) < 1e-10
+    assert abs(oracle.nelec(idx, lam, w, g, hi + 1e-9) - m.n_basis) < 1e-10
+    mus = np.linspace(lo, hi, 200)
+    ne = np.array([oracle.nelec(idx, lam, w, g, x) for x in mus])
+    assert np.all(np.diff(ne) >= -1e-12)
+    # inside the gap the count is the occupied count up to the method's own error (A11)
+    assert abs(oracle.nelec(idx, lam, w, g, 0.0) - m.n_occ) < 1e-2
+
+
+def test_bisection_finds_gap_plateau(oracle, cfg0):
+    """A11: starting outside the gap, midpoint bisection ends on the plateau whose rounded count is
+    the target; with an unreachable tolerance it stops on the mu_tol / max_steps guards."""
+    m = cfg0
+    idx = oracle.Index(m)
+    groups = np.arange(m.ngroups)
+    lam, w, ptr, g = oracle.eig_groups(idx, m.values, groups, nthreads=8)
+    lo, hi = oracle.gershgorin_interval(m)
+    mu, ne, tr = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0=-1.0, lo=lo, hi=hi, tol_n=0.5)
+    kd = m.to_dense()
+    ev = np.linalg.eigvalsh(kd)
+    homo, lumo = ev[ev < 0].max(), ev[ev > 0].min()
+    assert abs(ne - m.n_occ) <= 0.5 and len(tr) > 1
+    assert homo - 0.2 < mu < lumo + 0.2
+    mu2, ne2, tr2 = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0=-1.0, lo=lo, hi=hi, tol_n=1e-8,
+                                     mu_tol=1e-6, max_steps=64)
+    assert abs(ne2 - m.n_occ) > 1e-8 and len(tr2) <= 64  # unreachable by construction
+    assert abs(ne2 - m.n_occ) < 1e-2
