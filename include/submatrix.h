@@ -1,0 +1,220 @@
+/*
+ * submatrix.h -- C-ABI of libsubmatrix_b200.so: the data-parallel hot path of the submatrix
+ * method for density-matrix linear-scaling DFT (Lass, Schade, Kuehne, Plessl, arXiv:2004.10811)
+ * on one NVIDIA B200 (sm_100a).
+ *
+ *     D~ = 1/2 ( I - sign( K~ - mu I ) )            (Eq.(16), inner factor)
+ *
+ * evaluated approximately by the submatrix method: for every generating group
+ * of block columns a dense principal submatrix is cut out of the block-sparse symmetric K~
+ * (step 1, L125/L196/L199), its matrix sign function is computed (step 2; here by Newton-Schulz
+ * iterations, Eq.(11), in FP64 on the tensor-core DMMA path), and the generating columns are
+ * copied back on the input sparsity pattern (step 3, L127).
+ *
+ * Conventions
+ *  - "host" / "device" says where a pointer must live.  The library never takes ownership of a
+ *    caller buffer; a plan owns only its own device index tables (freed by sm_plan_destroy).
+ *  - Block-sparse layout (DBCSR-like, L107; ordering of L180): nb block rows/columns with sizes
+ *    blk_size[nb]; pattern in block-CSC: colptr[nb+1] (int64), rowidx[nnzb] (int32, strictly
+ *    ascending inside a column).  The pattern must be structurally symmetric and contain every
+ *    diagonal block.  Values: blocks in pattern order, each block (r,c) dense COLUMN-major
+ *    blk_size[r] x blk_size[c]; the element offset of block b is the exclusive prefix sum of
+ *    blk_size[r]*blk_size[c].  K~ must be numerically symmetric.  The result D~ uses the same
+ *    pattern and layout; block (r,c) of column c comes from the submatrix of c's group (it is NOT
+ *    symmetrised, L127).
+ *  - Groups: grp_ptr[ngroups+1], grp_cols[nb] must be a partition of 0..nb-1 (every block column
+ *    in exactly one group), so every result block is written exactly once.
+ *  - Errors: no exceptions, no abort.  Status < 0: hard error, outputs unspecified.  Status > 0:
+ *    warning, outputs are written and sm_stats_t says what is suspect.  sm_strerror() names any
+ *    status.
+ *  - One plan may be used by one stream at a time.  Results are deterministic run to run for a
+ *    fixed plan and options (fixed reduction orders, no floating-point atomics).
+ */
+#ifndef SUBMATRIX_B200_H
+#define SUBMATRIX_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sm_plan sm_plan_t; /* opaque */
+typedef int32_t sm_status_t;
+
+enum {
+    SM_OK = 0,
+    SM_ERR_INVALID_ARG = -1,         /* NULL pointer, negative size, bad option value            */
+    SM_ERR_STRUCTURE = -2,           /* unsorted/duplicate rows, asymmetric pattern, missing     */
+                                     /* diagonal block, groups not a partition                   */
+    SM_ERR_ALLOC = -3,               /* host or device allocation failed                         */
+    SM_ERR_CUDA = -4,                /* a CUDA call or kernel failed (see sm_last_cuda_error)    */
+    SM_ERR_WORKSPACE_TOO_SMALL = -5, /* workspace_bytes < sm_plan_info_t.workspace_bytes         */
+    SM_WARN_SIGN_NOT_CONVERGED = 1,  /* >= 1 submatrix hit max_iter or stagnated                 */
+    SM_WARN_MU_NOT_CONVERGED = 2     /* bisection ended on mu_tol / max_steps, not on tol_n      */
+};
+
+/* Options fixed at plan creation.  Pass NULL for the defaults written beside each field. */
+typedef struct {
+    int32_t max_iter;    /* Newton-Schulz iteration cap per sign evaluation            [100] */
+    int32_t scaling;     /* spectral bound for X0 = (a - mu I)/s: 0 = Gershgorin row   [0]   */
+                         /* sums of the assembled submatrix (reading A8)                     */
+    int32_t precision;   /* 0 = FP64 DMMA (the parity path)                            [0]   */
+    int32_t check_every; /* host polls the "all converged" counter every this many     [1]   */
+                         /* iterations (>= 1)                                                */
+    int32_t max_mu_steps;/* bisection step cap of sm_density_matrix                    [64]  */
+    int32_t bisect_iter; /* iteration cap of the NON-final bisection evaluations        [0]  */
+                         /* (0 = max_iter). A capped evaluation is only used for the         */
+                         /* direction of the step, never for acceptance (A11).     */
+    double mu_tol;       /* bisection stops when the bracket is narrower than this     [1e-6]*/
+    int32_t reserved[8];
+} sm_options_t;
+
+/* Plan facts (all sizes in elements unless they say bytes). */
+typedef struct {
+    int32_t nb, ngroups;
+    int64_t nnzb;             /* stored blocks                                               */
+    int64_t nnz;              /* stored values = length of the value arrays                  */
+    int64_t n_basis;          /* sum of blk_size                                             */
+    int64_t sum_sub_blocks;   /* sum_i |S_i|                                                 */
+    int32_t dim_min, dim_max; /* min / max submatrix dimension n_i                           */
+    double dim_mean;
+    int64_t sum_n2, sum_n3;   /* sum n_i^2, sum n_i^3 (Eq.(14) cost model L201)              */
+    int64_t sum_ld2;          /* sum of padded ld_i^2 = doubles per workspace buffer         */
+    int64_t n_tiles;          /* CTA tiles per GEMM launch                                   */
+    int32_t n_buckets;        /* distinct padded sizes                                       */
+    int32_t reserved0;
+    size_t workspace_bytes;   /* what sm_sign_execute / sm_density_matrix need               */
+} sm_plan_info_t;
+
+/* Filled by sm_sign_execute / sm_density_matrix (may be NULL). Times are CUDA-event ms of the
+ * LAST sign evaluation when timing was requested with sm_set_timing(plan, 1), else 0. */
+typedef struct {
+    int32_t iterations;       /* Newton-Schulz iterations launched in the last evaluation    */
+    int32_t iter_min, iter_max; /* per-submatrix iteration counts at convergence             */
+    int32_t not_converged;    /* submatrices that hit max_iter / stagnated                   */
+    double max_residual;      /* max_i ||X^2 - I||_F / sqrt(n_i) at exit                     */
+    double n_elec;            /* sum_i sum_{k in gen(i)} 1/2 (1 - X_kk) (Algorithm 1)   */
+    double mu;                /* chemical potential of the returned result                   */
+    int32_t mu_steps;         /* sign evaluations done by sm_density_matrix                  */
+    int32_t gemm_launches;    /* GEMM kernel launches in the last evaluation                 */
+    int64_t sum_iter_n3;      /* sum_i (2*iters_i + 1) * n_i^3  (=> flop = 2x this)          */
+    float ms_gather, ms_sign, ms_scatter, ms_total;
+    double mu_trace[64];      /* bisection history: mu of step k                             */
+    double ne_trace[64];      /* n_elec of step k                                            */
+} sm_stats_t;
+
+/*
+ * sm_plan_create -- device BSR container + submatrix index builder ("a principal
+ * submatrix a_i is assembled by removing all rows and columns j where A_{j,i} = 0"; per block
+ * column L196; per group of block columns L199; global sorted pattern L180).
+ * For every group G_i it forms on the GPU S_i = ascending union of the row blocks of its columns,
+ * n_i = sum of their sizes, the local offsets, and the position of every generating column in
+ * S_i; then sizes the padded batched workspace and the GEMM tile lists.
+ *   nb, blk_size[nb], colptr[nb+1], rowidx[nnzb]   host, copied
+ *   ngroups, grp_ptr[ngroups+1], grp_cols[nb]       host, copied
+ *   opt                                             host or NULL
+ *   cuda_stream                                     cudaStream_t (NULL = default stream)
+ * Returns SM_OK and *plan, or <0 and *plan == NULL.
+ */
+sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_t* blk_size,
+                           const int64_t* colptr, const int32_t* rowidx, int32_t ngroups,
+                           const int32_t* grp_ptr, const int32_t* grp_cols, const sm_options_t* opt,
+                           void* cuda_stream);
+
+/* Plan facts, including the workspace size. */
+sm_status_t sm_plan_query(const sm_plan_t* plan, sm_plan_info_t* out);
+
+/*
+ * Host copies of the index the GPU built, for bit-exact parity checks (any pointer may be NULL):
+ *   sub_ptr[ngroups+1] (int64)   exclusive prefix sum of |S_i|
+ *   sub_blocks[sum|S_i|]         members of S_i, ascending
+ *   sub_off[sum|S_i|]            element offset of each member inside a_i
+ *   sub_dim[ngroups]             n_i
+ *   gen_pos[nb]                  for grp_cols[g]: its position inside S_i
+ */
+sm_status_t sm_plan_export_index(const sm_plan_t* plan, int64_t* sub_ptr, int32_t* sub_blocks,
+                                 int32_t* sub_off, int32_t* sub_dim, int32_t* gen_pos);
+
+/*
+ * sm_sign_execute -- the three steps of the method at a fixed mu (Eq.(16)):
+ * gather a_i - mu I into the batched dense workspace, X0 = (a_i - mu I)/s_i with a Gershgorin
+ * bound s_i, Newton-Schulz X <- 1/2 X (3I - X^2) (Eq.(11)) until ||X^2 - I||_F/sqrt(n_i) < eps
+ * (involutority criterion, L354/Fig.13), then D~[r,c] = 1/2 (delta_rc I - X[loc r, loc c]) for
+ * the generating columns.
+ *   d_vals_in [nnz]  device, K~ values            d_vals_out [nnz] device, D~ values (may be NULL:
+ *   mu, eps          scalars                                         only stats->n_elec is produced)
+ *   d_workspace      device, >= workspace_bytes, 256-byte aligned; contents are scratch
+ * Returns SM_OK, SM_WARN_SIGN_NOT_CONVERGED, or <0.
+ */
+sm_status_t sm_sign_execute(sm_plan_t* plan, const double* d_vals_in, double mu, double eps,
+                            double* d_vals_out, void* d_workspace, size_t workspace_bytes,
+                            sm_stats_t* stats, void* cuda_stream);
+
+/* Same with HOST value arrays (pageable or pinned): copies h_vals_in to the device, runs
+ * sm_sign_execute, copies D~ back.  The staging buffers are owned by the plan. */
+sm_status_t sm_sign_execute_host(sm_plan_t* plan, const double* h_vals_in, double mu, double eps,
+                                 double* h_vals_out, void* d_workspace, size_t workspace_bytes,
+                                 sm_stats_t* stats, void* cuda_stream);
+
+/*
+ * sm_density_matrix -- canonical ensemble (PAPER.md IV-G, L259-266, Algorithm 1):
+ * adjust mu until n_elec(mu) = sum_i sum_{k in gen(i)} 1/2 (1 - sign(a_i - mu I)_kk) matches
+ * n_target, "using a simple bisection" (L266).  Newton-Schulz keeps no eigendecomposition, so
+ * every step re-evaluates the sign function (the cost L266 warns about).
+ * Rule (reading A11): step 0 evaluates *mu_inout; then midpoint bisection inside the
+ * Gershgorin interval of K~ (n_elec = 0 below, = n_basis above), raising mu if n_elec < n_target.
+ * Stops when |n_elec - n_target| <= tol_n (SM_OK), or when the bracket is narrower than
+ * opt.mu_tol or after opt.max_mu_steps evaluations (SM_WARN_MU_NOT_CONVERGED); returns in
+ * *mu_inout the evaluated mu with the smallest |n_elec - n_target| and in d_vals_out D~ at that mu.
+ */
+sm_status_t sm_density_matrix(sm_plan_t* plan, const double* d_vals_in, double n_target,
+                              double tol_n, double eps, double* mu_inout, double* d_vals_out,
+                              void* d_workspace, size_t workspace_bytes, sm_stats_t* stats,
+                              void* cuda_stream);
+
+/* Host-buffer variant of sm_density_matrix (H2D of K~ and D2H of D~ inside the call). */
+sm_status_t sm_density_matrix_host(sm_plan_t* plan, const double* h_vals_in, double n_target,
+                                   double tol_n, double eps, double* mu_inout, double* h_vals_out,
+                                   void* d_workspace, size_t workspace_bytes, sm_stats_t* stats,
+                                   void* cuda_stream);
+
+/*
+ * sm_trace_dk -- tr(D) (Eq.(18)) and the band-structure energy tr(D K) (Eq.(10)) of two
+ * value arrays on the plan's pattern: tr(DK) = sum over stored elements D o K (K symmetric).
+ * d_D, d_K device [nnz]; tr_D, tr_DK host doubles.  Deterministic two-stage reduction.
+ */
+sm_status_t sm_trace_dk(sm_plan_t* plan, const double* d_D, const double* d_K, double* tr_D,
+                        double* tr_DK, void* cuda_stream);
+
+/*
+ * Phase entry points used by the tests and the roofline benchmark (same kernels as above):
+ *   sm_gather   : workspace X buffer <- a_i - mu I (identity-padded); also the Gershgorin bounds
+ *   sm_scatter  : d_vals_out <- 1/2 (delta - xscale_i * X) from the workspace X buffer written by
+ *                 the last sm_gather / sign evaluation; f = identity round trip when as_identity=1:
+ *                 d_vals_out <- X (i.e. gather then scatter returns K~ - mu I on the pattern)
+ *   sm_sign_iterate : run the Newton-Schulz loop on the gathered workspace
+ */
+sm_status_t sm_gather(sm_plan_t* plan, const double* d_vals_in, double mu, void* d_workspace,
+                      size_t workspace_bytes, void* cuda_stream);
+sm_status_t sm_sign_iterate(sm_plan_t* plan, double eps, void* d_workspace, size_t workspace_bytes,
+                            sm_stats_t* stats, void* cuda_stream);
+sm_status_t sm_scatter(sm_plan_t* plan, int32_t as_identity, double* d_vals_out, void* d_workspace,
+                       size_t workspace_bytes, void* cuda_stream);
+
+/* Enable (1) / disable (0) per-phase CUDA-event timing into sm_stats_t (adds stream syncs). */
+sm_status_t sm_set_timing(sm_plan_t* plan, int32_t enable);
+
+/* Number of kernels this plan has launched since creation (for bench.py's gpu_launches). */
+int64_t sm_launch_count(const sm_plan_t* plan);
+
+void sm_plan_destroy(sm_plan_t* plan);
+const char* sm_strerror(sm_status_t status);
+/* Text of the last CUDA error seen by this library in the calling process ("" if none). */
+const char* sm_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SUBMATRIX_B200_H */

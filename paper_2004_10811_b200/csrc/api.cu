@@ -1,0 +1,517 @@
+// C-ABI entry points (include/submatrix.h): argument checks, plan lifetime, the Newton-Schulz
+// host loop, the mu bisection (a8).  Every floating-point step of the path runs in the kernels of
+// plan.cu / gather_scatter.cu / ns_sign.cu; the host only sequences launches and compares scalars.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+namespace smb {
+static thread_local char g_cuda_err[512] = "";
+void set_cuda_error(cudaError_t e, const char* where) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    cudaGetLastError();  // clear the sticky-less error state
+}
+}  // namespace smb
+
+using namespace smb;
+
+static void default_options(sm_options_t* o) {
+    memset(o, 0, sizeof(*o));
+    o->max_iter = 100;
+    o->scaling = 0;
+    o->precision = 0;
+    o->check_every = 1;
+    o->max_mu_steps = 64;
+    o->bisect_iter = 0;
+    o->mu_tol = 1e-6;
+}
+
+static sm_status_t validate(int32_t nb, const int32_t* bs, const int64_t* colptr, const int32_t* rowidx,
+                            int32_t ng, const int32_t* gp, const int32_t* gc) {
+    if (nb < 0 || ng < 0 || (nb > 0 && (!bs || !colptr || !rowidx || !gp || !gc))) return SM_ERR_INVALID_ARG;
+    if (nb == 0) return ng == 0 ? SM_OK : SM_ERR_STRUCTURE;
+    if (colptr[0] != 0) return SM_ERR_STRUCTURE;
+    for (int c = 0; c < nb; ++c) {
+        if (bs[c] <= 0) return SM_ERR_INVALID_ARG;
+        if (colptr[c + 1] < colptr[c]) return SM_ERR_STRUCTURE;
+        bool diag = false;
+        for (int64_t p = colptr[c]; p < colptr[c + 1]; ++p) {
+            int r = rowidx[p];
+            if (r < 0 || r >= nb) return SM_ERR_STRUCTURE;
+            if (p > colptr[c] && rowidx[p - 1] >= r) return SM_ERR_STRUCTURE;  // unsorted / duplicate
+            if (r == c) diag = true;
+        }
+        if (!diag) return SM_ERR_STRUCTURE;  // reading A3
+    }
+    // structural symmetry: (r,c) stored => (c,r) stored
+    for (int c = 0; c < nb; ++c)
+        for (int64_t p = colptr[c]; p < colptr[c + 1]; ++p) {
+            int r = rowidx[p];
+            if (r == c) continue;
+            const int32_t* b = rowidx + colptr[r];
+            const int32_t* e = rowidx + colptr[r + 1];
+            if (!std::binary_search(b, e, c)) return SM_ERR_STRUCTURE;
+        }
+    // groups: a partition of 0..nb-1 (reading A6)
+    if (gp[0] != 0 || gp[ng] != nb) return SM_ERR_STRUCTURE;
+    std::vector<char> seen(nb, 0);
+    for (int g = 0; g < ng; ++g) {
+        if (gp[g + 1] <= gp[g]) return SM_ERR_STRUCTURE;  // empty group
+        for (int q = gp[g]; q < gp[g + 1]; ++q) {
+            int c = gc[q];
+            if (c < 0 || c >= nb || seen[c]) return SM_ERR_STRUCTURE;
+            seen[c] = 1;
+        }
+    }
+    return SM_OK;
+}
+
+extern "C" void sm_plan_destroy(sm_plan_t* p) {
+    if (!p) return;
+    void* ptrs[] = {p->d_blk_size, p->d_blk_off, p->d_rowidx, p->d_colptr, p->d_val_off, p->d_grp_ptr,
+                    p->d_grp_cols, p->d_col_grp, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off, p->d_sub_dim,
+                    p->d_gen_pos, p->d_gen_off, p->d_blk_loc, p->d_gen_width, p->d_ws_off, p->d_ld, p->d_tiles,
+                    p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
+                    p->d_partials, p->d_counters, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
+                    p->d_stage_out};
+    for (void* q : ptrs)
+        if (q) cudaFree(q);
+    if (p->h_pinned) cudaFreeHost(p->h_pinned);
+    if (p->h_pinned_d) cudaFreeHost(p->h_pinned_d);
+    for (auto& e : p->ev)
+        if (e) cudaEventDestroy(e);
+    for (auto& e : p->ev_iter)
+        if (e) cudaEventDestroy(e);
+    delete p;
+}
+
+extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_t* blk_size,
+                                      const int64_t* colptr, const int32_t* rowidx, int32_t ngroups,
+                                      const int32_t* grp_ptr, const int32_t* grp_cols,
+                                      const sm_options_t* opt, void* cuda_stream) {
+    if (!plan) return SM_ERR_INVALID_ARG;
+    *plan = nullptr;
+    sm_status_t s = validate(nb, blk_size, colptr, rowidx, ngroups, grp_ptr, grp_cols);
+    if (s) return s;
+    sm_plan* p = new (std::nothrow) sm_plan();
+    if (!p) return SM_ERR_ALLOC;
+    if (opt) p->opt = *opt; else default_options(&p->opt);
+    if (p->opt.max_iter <= 0) p->opt.max_iter = 100;
+    if (p->opt.check_every <= 0) p->opt.check_every = 1;
+    if (p->opt.max_mu_steps <= 0) p->opt.max_mu_steps = 64;
+    if (p->opt.max_mu_steps > 64) p->opt.max_mu_steps = 64;
+    if (!(p->opt.mu_tol > 0)) p->opt.mu_tol = 1e-6;
+    if (p->opt.precision != 0 || p->opt.scaling != 0) { delete p; return SM_ERR_INVALID_ARG; }
+    p->nb = nb; p->ngroups = ngroups; p->nnzb = nb ? colptr[nb] : 0;
+    p->h_blk_size.assign(blk_size, blk_size + nb);
+    p->h_colptr.assign(colptr, colptr + nb + 1);
+    p->h_rowidx.assign(rowidx, rowidx + p->nnzb);
+    p->h_grp_ptr.assign(grp_ptr, grp_ptr + ngroups + 1);
+    p->h_grp_cols.assign(grp_cols, grp_cols + nb);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        set_cuda_error(cudaGetLastError(), "cudaGetDevice");
+        delete p;
+        return SM_ERR_CUDA;
+    }
+    s = build_index_device(p, st);
+    if (s) { sm_plan_destroy(p); return s; }
+    // per-evaluation state
+    const int ng = std::max(ngroups, 1);
+    auto A = [&](void** d, size_t bytes) { return cudaMalloc(d, std::max<size_t>(bytes, 8)); };
+    cudaError_t e = cudaSuccess;
+    if (e == cudaSuccess) e = A((void**)&p->d_done_iter, (size_t)ng * 4);
+    if (e == cudaSuccess) e = A((void**)&p->d_flag, (size_t)ng * 4);
+    if (e == cudaSuccess) e = A((void**)&p->d_res, (size_t)ng * 16);
+    if (e == cudaSuccess) e = A((void**)&p->d_gersh, (size_t)ng * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_partials, (size_t)p->n_tiles * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_counters, (size_t)(p->opt.max_iter + 2) * 4);
+    if (e == cudaSuccess) e = A((void**)&p->d_ne_part, (size_t)ng * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_scalars, 8 * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_red, 4096 * 8);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned, (size_t)(p->opt.max_iter + 2) * 4);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned_d, 8 * 8);
+    for (auto& ev : p->ev)
+        if (e == cudaSuccess) e = cudaEventCreate(&ev);
+    for (auto& ev : p->ev_iter)
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+        set_cuda_error(e, "plan state allocation");
+        sm_plan_destroy(p);
+        return e == cudaErrorMemoryAllocation ? SM_ERR_ALLOC : SM_ERR_CUDA;
+    }
+    // gather launch shape: shared memory = row map + one source table per warp
+    {
+        const size_t rowmap = (((size_t)(p->info.dim_max + LD_ALIGN) * 4 + 15) / 16) * 16;
+        int warps = 8;
+        const size_t budget = 200 * 1024;
+        while (warps > 1 && rowmap + (size_t)warps * p->max_sub_blocks * 8 > budget) warps >>= 1;
+        p->gather_warps = warps;
+        p->gather_smem = rowmap + (size_t)warps * std::max(p->max_sub_blocks, 1) * 8;
+        if (p->gather_smem > budget) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }
+    }
+    *plan = p;
+    return SM_OK;
+}
+
+extern "C" sm_status_t sm_plan_query(const sm_plan_t* p, sm_plan_info_t* out) {
+    if (!p || !out) return SM_ERR_INVALID_ARG;
+    *out = p->info;
+    return SM_OK;
+}
+
+extern "C" sm_status_t sm_plan_export_index(const sm_plan_t* p, int64_t* sub_ptr, int32_t* sub_blocks,
+                                            int32_t* sub_off, int32_t* sub_dim, int32_t* gen_pos) {
+    if (!p) return SM_ERR_INVALID_ARG;
+    const int ng = p->ngroups;
+    const int64_t tot = p->info.sum_sub_blocks;
+    if (sub_ptr) memcpy(sub_ptr, p->h_sub_ptr.data(), (size_t)(ng + 1) * 8);
+    if (sub_blocks && tot) SM_CUDA(cudaMemcpy(sub_blocks, p->d_sub_blocks, (size_t)tot * 4, cudaMemcpyDeviceToHost));
+    if (sub_off && tot) SM_CUDA(cudaMemcpy(sub_off, p->d_sub_off, (size_t)tot * 4, cudaMemcpyDeviceToHost));
+    if (sub_dim && ng) SM_CUDA(cudaMemcpy(sub_dim, p->d_sub_dim, (size_t)ng * 4, cudaMemcpyDeviceToHost));
+    if (gen_pos && p->nb) SM_CUDA(cudaMemcpy(gen_pos, p->d_gen_pos, (size_t)p->nb * 4, cudaMemcpyDeviceToHost));
+    return SM_OK;
+}
+
+extern "C" sm_status_t sm_set_timing(sm_plan_t* p, int32_t enable) {
+    if (!p) return SM_ERR_INVALID_ARG;
+    p->timing = enable ? 1 : 0;
+    return SM_OK;
+}
+
+extern "C" int64_t sm_launch_count(const sm_plan_t* p) { return p ? p->launches : 0; }
+
+namespace {
+struct Bufs {
+    double *b0, *b1, *y;
+};
+sm_status_t carve(const sm_plan* p, void* ws, size_t bytes, Bufs* b) {
+    if (bytes < p->info.workspace_bytes) return SM_ERR_WORKSPACE_TOO_SMALL;
+    if (!ws && p->info.workspace_bytes) return SM_ERR_INVALID_ARG;
+    if (((uintptr_t)ws & 255) != 0) return SM_ERR_INVALID_ARG;
+    const size_t buf = p->info.workspace_bytes / 3;
+    b->b0 = (double*)ws;
+    b->b1 = (double*)((char*)ws + buf);
+    b->y = (double*)((char*)ws + 2 * buf);
+    return SM_OK;
+}
+
+sm_status_t reset_state(sm_plan* p, cudaStream_t st) {
+    const int ng = std::max(p->ngroups, 1);
+    SM_CUDA(cudaMemsetAsync(p->d_done_iter, 0xff, (size_t)ng * 4, st));
+    SM_CUDA(cudaMemsetAsync(p->d_flag, 0, (size_t)ng * 4, st));
+    SM_CUDA(cudaMemsetAsync(p->d_counters, 0, (size_t)(p->opt.max_iter + 2) * 4, st));
+    p->cur_k = 0;
+    return SM_OK;
+}
+
+// Newton-Schulz host loop: iterations k = k_begin .. k_end-1 (each = MODE 0 + MODE 1 launch).
+// Iteration k tests X_k and, if not converged, forms X_{k+1}.  At k == max_iter only the decision
+// is recorded.  Returns with *all_done = 1 if every submatrix has stopped.
+sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_done, int* launched,
+                    cudaStream_t st) {
+    *all_done = 0;
+    if (p->ngroups == 0) { *all_done = 1; return SM_OK; }
+    const int max_iter = p->opt.max_iter;
+    int k = p->cur_k;
+    int pending = -1;  // iteration whose counter copy is in flight
+    for (; k < k_end && k <= max_iter; ++k) {
+        sm_status_t s = launch_ns_pair(p, k, eps, k == max_iter ? 1 : 0, b.b0, b.b1, b.y, st);
+        if (s) return s;
+        (*launched) += 2;
+        if (pending >= 0) {
+            SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
+            if (p->h_pinned[pending] == 0) { *all_done = 1; p->cur_k = pending; return SM_OK; }
+            pending = -1;
+        }
+        if ((k % p->opt.check_every) == 0 || k == max_iter || k == k_end - 1) {
+            SM_CUDA(cudaMemcpyAsync(p->h_pinned + k, p->d_counters + k, 4, cudaMemcpyDeviceToHost, st));
+            SM_CUDA(cudaEventRecord(p->ev_iter[k & 1], st));
+            pending = k;
+        }
+    }
+    if (pending >= 0) {
+        SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
+        if (p->h_pinned[pending] == 0) { *all_done = 1; p->cur_k = pending; return SM_OK; }
+    }
+    // active submatrices have received k updates: their X lives in buf[k & 1]
+    p->cur_k = std::min(k, max_iter);
+    if (k > max_iter) *all_done = 1;
+    return SM_OK;
+}
+
+sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStream_t st) {
+    const int ng = p->ngroups;
+    std::vector<int32_t> di(ng), fl(ng);
+    std::vector<double> res((size_t)2 * ng);
+    if (ng) {
+        SM_CUDA(cudaMemcpyAsync(di.data(), p->d_done_iter, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
+        SM_CUDA(cudaMemcpyAsync(fl.data(), p->d_flag, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
+        SM_CUDA(cudaMemcpyAsync(res.data(), p->d_res, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+    }
+    SM_CUDA(cudaMemcpyAsync(p->h_pinned_d, p->d_scalars, 8, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    int imin = INT32_MAX, imax = 0, nc = 0;
+    double rmax = 0.0;
+    int64_t sin3 = 0;
+    for (int i = 0; i < ng; ++i) {
+        int it = di[i] >= 0 ? di[i] : p->cur_k;
+        if (di[i] < 0 || fl[i]) ++nc;
+        imin = std::min(imin, it);
+        imax = std::max(imax, it);
+        int slot = di[i] >= 0 ? (di[i] & 1) : ((std::max(p->cur_k, 1) - 1) & 1);
+        double r = res[(size_t)slot * ng + i];
+        if (r == r) rmax = std::max(rmax, r); else rmax = INFINITY;
+        int64_t n = p->h_sub_dim[i];
+        // executed GEMMs: one X^2 per tested iterate (it + 1) and one update per iteration (it)
+        sin3 += (int64_t)(2 * it + 1) * n * n * n;
+    }
+    *not_conv = nc;
+    if (stats) {
+        stats->iter_min = ng ? imin : 0;
+        stats->iter_max = imax;
+        stats->not_converged = nc;
+        stats->max_residual = rmax;
+        stats->n_elec = p->h_pinned_d[0];
+        stats->sum_iter_n3 = sin3;
+    }
+    return SM_OK;
+}
+
+// One sign evaluation at fixed mu: gather -> NS loop (up to iter_cap iterations) -> n_elec.
+sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, const Bufs& b, int iter_cap,
+                     sm_stats_t* stats, int* not_conv, cudaStream_t st) {
+    sm_status_t s;
+    int launched = 0, all_done = 0;
+    if (p->timing) SM_CUDA(cudaEventRecord(p->ev[0], st));
+    if ((s = reset_state(p, st))) return s;
+    if ((s = launch_gather(p, d_in, mu, b.b0, st))) return s;
+    if (p->timing) SM_CUDA(cudaEventRecord(p->ev[1], st));
+    if ((s = ns_loop(p, b, eps, iter_cap, &all_done, &launched, st))) return s;
+    if (p->timing) SM_CUDA(cudaEventRecord(p->ev[2], st));
+    if ((s = launch_nelec(p, b.b0, b.b1, st))) return s;
+    if ((s = collect_stats(p, stats, not_conv, st))) return s;
+    if (stats) {
+        stats->iterations = launched / 2;
+        stats->gemm_launches = launched;
+        stats->mu = mu;
+        if (p->timing) {
+            cudaEventElapsedTime(&stats->ms_gather, p->ev[0], p->ev[1]);
+            cudaEventElapsedTime(&stats->ms_sign, p->ev[1], p->ev[2]);
+        }
+    }
+    return SM_OK;
+}
+
+sm_status_t do_scatter(sm_plan* p, const Bufs& b, double* d_out, sm_stats_t* stats, cudaStream_t st) {
+    if (p->timing) SM_CUDA(cudaEventRecord(p->ev[3], st));
+    sm_status_t s = launch_scatter(p, 0, b.b0, b.b1, d_out, st);
+    if (s) return s;
+    if (p->timing) {
+        SM_CUDA(cudaEventRecord(p->ev[4], st));
+        SM_CUDA(cudaEventSynchronize(p->ev[4]));
+        if (stats) {
+            cudaEventElapsedTime(&stats->ms_scatter, p->ev[3], p->ev[4]);
+            cudaEventElapsedTime(&stats->ms_total, p->ev[0], p->ev[4]);
+        }
+    }
+    return SM_OK;
+}
+
+sm_status_t ensure_stage(sm_plan* p) {
+    const size_t bytes = std::max<size_t>((size_t)p->nnz * 8, 8);
+    if (!p->d_stage_in) SM_CUDA(cudaMalloc((void**)&p->d_stage_in, bytes));
+    if (!p->d_stage_out) SM_CUDA(cudaMalloc((void**)&p->d_stage_out, bytes));
+    return SM_OK;
+}
+}  // namespace
+
+extern "C" sm_status_t sm_sign_execute(sm_plan_t* p, const double* d_vals_in, double mu, double eps,
+                                       double* d_vals_out, void* d_workspace, size_t workspace_bytes,
+                                       sm_stats_t* stats, void* cuda_stream) {
+    if (!p || (!d_vals_in && p->nnz) || !(eps > 0.0) || !(mu == mu)) return SM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    Bufs b;
+    sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
+    if (s) return s;
+    if (stats) memset(stats, 0, sizeof(*stats));
+    int nc = 0;
+    if ((s = evaluate(p, d_vals_in, mu, eps, b, p->opt.max_iter + 1, stats, &nc, st))) return s;
+    if (d_vals_out && (s = do_scatter(p, b, d_vals_out, stats, st))) return s;
+    if (stats) stats->mu_steps = 1;
+    return nc ? SM_WARN_SIGN_NOT_CONVERGED : SM_OK;
+}
+
+extern "C" sm_status_t sm_gather(sm_plan_t* p, const double* d_vals_in, double mu, void* d_workspace,
+                                 size_t workspace_bytes, void* cuda_stream) {
+    if (!p || (!d_vals_in && p->nnz)) return SM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    Bufs b;
+    sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
+    if (s) return s;
+    if ((s = reset_state(p, st))) return s;
+    return launch_gather(p, d_vals_in, mu, b.b0, st);
+}
+
+extern "C" sm_status_t sm_sign_iterate(sm_plan_t* p, double eps, void* d_workspace, size_t workspace_bytes,
+                                       sm_stats_t* stats, void* cuda_stream) {
+    if (!p || !(eps > 0.0)) return SM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    Bufs b;
+    sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
+    if (s) return s;
+    if (stats) memset(stats, 0, sizeof(*stats));
+    int launched = 0, all_done = 0, nc = 0;
+    if ((s = ns_loop(p, b, eps, p->opt.max_iter + 1, &all_done, &launched, st))) return s;
+    if ((s = launch_nelec(p, b.b0, b.b1, st))) return s;
+    if ((s = collect_stats(p, stats, &nc, st))) return s;
+    if (stats) { stats->iterations = launched / 2; stats->gemm_launches = launched; }
+    return nc ? SM_WARN_SIGN_NOT_CONVERGED : SM_OK;
+}
+
+extern "C" sm_status_t sm_scatter(sm_plan_t* p, int32_t as_identity, double* d_vals_out, void* d_workspace,
+                                  size_t workspace_bytes, void* cuda_stream) {
+    if (!p || (!d_vals_out && p->nnz)) return SM_ERR_INVALID_ARG;
+    Bufs b;
+    sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
+    if (s) return s;
+    return launch_scatter(p, as_identity ? 1 : 0, b.b0, b.b1, d_vals_out, (cudaStream_t)cuda_stream);
+}
+
+extern "C" sm_status_t sm_sign_execute_host(sm_plan_t* p, const double* h_vals_in, double mu, double eps,
+                                            double* h_vals_out, void* d_workspace, size_t workspace_bytes,
+                                            sm_stats_t* stats, void* cuda_stream) {
+    if (!p || (!h_vals_in && p->nnz)) return SM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    sm_status_t s = ensure_stage(p);
+    if (s) return s;
+    if (p->nnz) SM_CUDA(cudaMemcpyAsync(p->d_stage_in, h_vals_in, (size_t)p->nnz * 8, cudaMemcpyHostToDevice, st));
+    s = sm_sign_execute(p, p->d_stage_in, mu, eps, h_vals_out ? p->d_stage_out : nullptr, d_workspace,
+                        workspace_bytes, stats, cuda_stream);
+    if (s < 0) return s;
+    if (h_vals_out && p->nnz)
+        SM_CUDA(cudaMemcpyAsync(h_vals_out, p->d_stage_out, (size_t)p->nnz * 8, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    return s;
+}
+
+extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, double n_target, double tol_n,
+                                         double eps, double* mu_inout, double* d_vals_out, void* d_workspace,
+                                         size_t workspace_bytes, sm_stats_t* stats, void* cuda_stream) {
+    if (!p || (!d_vals_in && p->nnz) || !mu_inout || !(eps > 0.0) || !(tol_n >= 0.0) || !(*mu_inout == *mu_inout))
+        return SM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    Bufs b;
+    sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
+    if (s) return s;
+    sm_stats_t local;
+    sm_stats_t* S = stats ? stats : &local;
+    memset(S, 0, sizeof(*S));
+    // bracket: Gershgorin interval of the whole K~ (n_elec = 0 below, n_basis above)
+    if ((s = launch_gersh_global(p, d_vals_in, st))) return s;
+    SM_CUDA(cudaMemcpy(p->h_pinned_d + 4, p->d_scalars + 4, 16, cudaMemcpyDeviceToHost));
+    double lo = p->h_pinned_d[4], hi = p->h_pinned_d[5];
+    double mu = *mu_inout;
+    const int cap = (p->opt.bisect_iter > 0 && p->opt.bisect_iter < p->opt.max_iter) ? p->opt.bisect_iter
+                                                                                       : p->opt.max_iter + 1;
+    double best_mu = mu, best_g = INFINITY;
+    int best_step = -1, steps = 0, nc = 0, last_nc = 0;
+    bool accepted = false;
+    sm_stats_t ev;
+    for (; steps < p->opt.max_mu_steps;) {
+        memset(&ev, 0, sizeof(ev));
+        if ((s = evaluate(p, d_vals_in, mu, eps, b, cap, &ev, &nc, st))) return s;
+        double g = ev.n_elec - n_target;
+        if (nc > 0 && cap <= p->opt.max_iter && std::fabs(g) <= std::max(tol_n, 0.0) + 1e-300) {
+            // a capped evaluation may not accept: finish this one to convergence first
+            int launched = 0, all_done = 0;
+            if ((s = ns_loop(p, b, eps, p->opt.max_iter + 1, &all_done, &launched, st))) return s;
+            if ((s = launch_nelec(p, b.b0, b.b1, st))) return s;
+            if ((s = collect_stats(p, &ev, &nc, st))) return s;
+            ev.iterations += launched / 2;
+            g = ev.n_elec - n_target;
+        }
+        S->mu_trace[steps] = mu;
+        S->ne_trace[steps] = ev.n_elec;
+        last_nc = nc;
+        if (std::fabs(g) < std::fabs(best_g)) { best_g = g; best_mu = mu; best_step = steps; }
+        ++steps;
+        if (std::fabs(g) <= tol_n) { accepted = true; break; }
+        if (g < 0) lo = std::max(lo, mu); else hi = std::min(hi, mu);
+        if (hi - lo <= p->opt.mu_tol) break;
+        mu = 0.5 * (lo + hi);
+    }
+    // the workspace holds the last evaluated mu; re-evaluate if the best one was an earlier step
+    // or if the last evaluation was capped before convergence
+    if (best_step != steps - 1 || (last_nc > 0 && cap <= p->opt.max_iter)) {
+        memset(&ev, 0, sizeof(ev));
+        if ((s = evaluate(p, d_vals_in, best_mu, eps, b, p->opt.max_iter + 1, &ev, &nc, st))) return s;
+        last_nc = nc;
+    }
+    double tr_mu[64], tr_ne[64];
+    memcpy(tr_mu, S->mu_trace, sizeof(tr_mu));
+    memcpy(tr_ne, S->ne_trace, sizeof(tr_ne));
+    *S = ev;
+    memcpy(S->mu_trace, tr_mu, sizeof(tr_mu));
+    memcpy(S->ne_trace, tr_ne, sizeof(tr_ne));
+    S->mu = best_mu;
+    S->mu_steps = steps;
+    *mu_inout = best_mu;
+    if (d_vals_out && (s = do_scatter(p, b, d_vals_out, S, st))) return s;
+    SM_CUDA(cudaStreamSynchronize(st));
+    if (!accepted) return SM_WARN_MU_NOT_CONVERGED;
+    return last_nc ? SM_WARN_SIGN_NOT_CONVERGED : SM_OK;
+}
+
+extern "C" sm_status_t sm_density_matrix_host(sm_plan_t* p, const double* h_vals_in, double n_target,
+                                              double tol_n, double eps, double* mu_inout, double* h_vals_out,
+                                              void* d_workspace, size_t workspace_bytes, sm_stats_t* stats,
+                                              void* cuda_stream) {
+    if (!p || (!h_vals_in && p->nnz)) return SM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    sm_status_t s = ensure_stage(p);
+    if (s) return s;
+    if (p->nnz) SM_CUDA(cudaMemcpyAsync(p->d_stage_in, h_vals_in, (size_t)p->nnz * 8, cudaMemcpyHostToDevice, st));
+    s = sm_density_matrix(p, p->d_stage_in, n_target, tol_n, eps, mu_inout, h_vals_out ? p->d_stage_out : nullptr,
+                          d_workspace, workspace_bytes, stats, cuda_stream);
+    if (s < 0) return s;
+    if (h_vals_out && p->nnz)
+        SM_CUDA(cudaMemcpyAsync(h_vals_out, p->d_stage_out, (size_t)p->nnz * 8, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    return s;
+}
+
+extern "C" sm_status_t sm_trace_dk(sm_plan_t* p, const double* d_D, const double* d_K, double* tr_D,
+                                   double* tr_DK, void* cuda_stream) {
+    if (!p || (p->nnz && (!d_D || !d_K))) return SM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    sm_status_t s = launch_trace_dk(p, d_D, d_K, st);
+    if (s) return s;
+    SM_CUDA(cudaMemcpyAsync(p->h_pinned_d + 1, p->d_scalars + 1, 16, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    if (tr_D) *tr_D = p->h_pinned_d[1];
+    if (tr_DK) *tr_DK = p->h_pinned_d[2];
+    return SM_OK;
+}
+
+extern "C" const char* sm_strerror(sm_status_t s) {
+    switch (s) {
+        case SM_OK: return "ok";
+        case SM_ERR_INVALID_ARG: return "invalid argument";
+        case SM_ERR_STRUCTURE: return "invalid block-sparse structure or grouping";
+        case SM_ERR_ALLOC: return "allocation failed";
+        case SM_ERR_CUDA: return "CUDA error";
+        case SM_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+        case SM_WARN_SIGN_NOT_CONVERGED: return "warning: sign iteration not converged for at least one submatrix";
+        case SM_WARN_MU_NOT_CONVERGED: return "warning: mu bisection ended without meeting tol_n";
+        default: return "unknown status";
+    }
+}
+
+extern "C" const char* sm_last_cuda_error(void) { return smb::g_cuda_err; }

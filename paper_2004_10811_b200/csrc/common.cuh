@@ -1,0 +1,100 @@
+// Internal declarations of libsubmatrix_b200.so (sm_100a).  Not part of the C-ABI; the boundary
+// is include/submatrix.h.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "submatrix.h"
+
+namespace smb {
+
+constexpr int TILE = 64;        // CTA tile edge of the Newton-Schulz GEMMs
+constexpr int LD_ALIGN = 8;     // padded leading dimension granularity (one DMMA k-step pair)
+
+// One CTA tile of one submatrix: lower-triangular tile (ti >= tj) of a symmetric product.
+struct TileDesc {
+    int32_t grp;   // submatrix (= generating group) index
+    int32_t tij;   // ti | (tj << 16)
+};
+
+void set_cuda_error(cudaError_t e, const char* where);
+
+#define SM_CUDA(call)                                        \
+    do {                                                     \
+        cudaError_t e__ = (call);                            \
+        if (e__ != cudaSuccess) {                            \
+            smb::set_cuda_error(e__, #call);                 \
+            return SM_ERR_CUDA;                              \
+        }                                                    \
+    } while (0)
+
+}  // namespace smb
+
+// The plan: device BSR container (a1) + submatrix index (a2) + workspace/tile tables.
+struct sm_plan {
+    sm_options_t opt;
+    sm_plan_info_t info;
+    int32_t nb = 0, ngroups = 0;
+    int64_t nnzb = 0, nnz = 0;
+    int32_t max_sub_blocks = 0;  // max |S_i|
+    // --- host copies
+    std::vector<int32_t> h_blk_size, h_rowidx, h_grp_ptr, h_grp_cols, h_sub_dim, h_ld;
+    std::vector<int64_t> h_colptr, h_sub_ptr, h_ws_off;
+    std::vector<int32_t> h_tile_first, h_tile_count;
+    // --- device: pattern
+    int32_t *d_blk_size = nullptr, *d_blk_off = nullptr, *d_rowidx = nullptr;
+    int64_t *d_colptr = nullptr, *d_val_off = nullptr;
+    int32_t *d_grp_ptr = nullptr, *d_grp_cols = nullptr, *d_col_grp = nullptr;
+    // --- device: submatrix index
+    int64_t* d_sub_ptr = nullptr;
+    int32_t *d_sub_blocks = nullptr, *d_sub_off = nullptr, *d_sub_dim = nullptr, *d_gen_pos = nullptr;
+    int32_t *d_gen_off = nullptr;  // [nb]  element offset of column c inside its group's submatrix
+    int32_t *d_blk_loc = nullptr;  // [nnzb] element row offset of block (r,c) inside c's group's submatrix
+    int32_t *d_gen_width = nullptr;// [ngroups] generating basis functions per group
+    // --- device: workspace geometry and tiles
+    int64_t* d_ws_off = nullptr;   // [ngroups] offset (doubles) of submatrix i in each buffer
+    int32_t* d_ld = nullptr;       // [ngroups] padded leading dimension
+    smb::TileDesc* d_tiles = nullptr;
+    int32_t *d_tile_first = nullptr, *d_tile_count = nullptr;
+    int64_t n_tiles = 0, sum_ld2 = 0;
+    // --- device: per-evaluation state
+    int32_t* d_done_iter = nullptr;        // [ngroups] -1 = active, else iteration at which it stopped
+    int32_t* d_flag = nullptr;             // [ngroups] 0 converged, 1 stagnated / max_iter
+    double* d_res = nullptr;               // [2][ngroups] residual history (ping-pong)
+    unsigned long long* d_gersh = nullptr; // [ngroups] bits of the Gershgorin bound (atomicMax)
+    double* d_partials = nullptr;          // [n_tiles] per-tile residual partial sums
+    int32_t* d_counters = nullptr;         // [max_iter+2] still-active submatrices after iteration k
+    double* d_ne_part = nullptr;           // [ngroups] per-group electron-count partials
+    double* d_scalars = nullptr;           // [8] n_elec, tr D, tr DK, gersh lo/hi
+    double* d_red = nullptr;               // [2*4096] reduction scratch
+    int32_t* h_pinned = nullptr;           // pinned host mirror for counters
+    double* h_pinned_d = nullptr;          // pinned host scalars
+    int cur_k = 0;                         // completed Newton-Schulz updates of the last evaluation
+    // --- staging for the *_host entry points
+    double *d_stage_in = nullptr, *d_stage_out = nullptr;
+    // --- misc
+    int timing = 0;
+    int64_t launches = 0;
+    cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_iter[2] = {nullptr, nullptr};
+    int gather_warps = 8;
+    size_t gather_smem = 0;
+    int num_sms = 148;
+};
+
+namespace smb {
+// plan.cu
+sm_status_t build_index_device(sm_plan* p, cudaStream_t st);
+// gather_scatter.cu
+sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, cudaStream_t st);
+sm_status_t launch_scatter(sm_plan* p, int as_identity, const double* buf0, const double* buf1,
+                           double* out, cudaStream_t st);
+sm_status_t launch_nelec(sm_plan* p, const double* buf0, const double* buf1, cudaStream_t st);
+sm_status_t launch_trace_dk(sm_plan* p, const double* D, const double* K, cudaStream_t st);
+sm_status_t launch_gersh_global(sm_plan* p, const double* vals, cudaStream_t st);
+// ns_sign.cu
+sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
+                           double* bufY, cudaStream_t st);
+}  // namespace smb

@@ -1,0 +1,373 @@
+"""Parity of the CUDA path (through the C-ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerances (BASELINE.json north_star): indices bit-exact;
+max |D_gpu - D_oracle| <= 1e-9; |tr(DK)_gpu - tr(DK)_oracle| / |tr(DK)_oracle| <= 1e-10."""
+import numpy as np
+import pytest
+
+from paper_2004_10811_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_D = 1e-9
+TOL_E = 1e-10
+EPS = 1e-12
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2004_10811_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _run_sign(B, m, mu=0.0, eps=EPS, opt=None, values=None):
+    torch = _torch()
+    plan = B.plan_from_matrix(m, opt)
+    ws = B.alloc_workspace(plan)
+    vin = torch.from_numpy(m.values if values is None else values).cuda()
+    vout = torch.full_like(vin, float("nan"))
+    stats = B.sm_stats_t()
+    st = B.sm_sign_execute(plan, vin, mu, eps, vout, ws, stats)
+    torch.cuda.synchronize()
+    return plan, st, vout.cpu().numpy(), stats, ws, vin
+
+
+def _sample_groups(idx, k, seed=0):
+    """Seeded sample of groups that always contains the min-, median- and max-dimension ones."""
+    ng = idx.ngroups
+    order = np.argsort(idx.sub_dim, kind="stable")
+    must = {int(order[0]), int(order[ng // 2]), int(order[-1])}
+    rng = np.random.default_rng(seed)
+    rest = [int(g) for g in rng.permutation(ng) if int(g) not in must][: max(0, k - len(must))]
+    return np.array(sorted(must | set(rest)), dtype=np.int32)
+
+
+def _column_mask(idx, m, groups):
+    cols = np.concatenate([idx.grp_cols[idx.grp_ptr[g]:idx.grp_ptr[g + 1]] for g in groups])
+    sel = np.isin(m.block_cols(), cols)
+    return np.repeat(sel, np.diff(idx.val_off)), cols.astype(np.int32)
+
+
+def _check_index(B, oracle, m, plan=None):
+    own = plan is None
+    if own:
+        plan = B.plan_from_matrix(m)
+    sub_ptr, sub_blocks, sub_off, sub_dim, gen_pos = B.sm_plan_export_index(plan)
+    idx = oracle.Index(m)
+    assert np.array_equal(sub_ptr, idx.sub_ptr)
+    assert np.array_equal(sub_blocks, idx.sub_blocks)
+    assert np.array_equal(sub_off, idx.sub_off)
+    assert np.array_equal(sub_dim, idx.sub_dim)
+    assert np.array_equal(gen_pos, idx.gen_pos)
+    if own:
+        B.sm_plan_destroy(plan)
+    return idx
+
+
+# ------------------------------------------------------------------------------ a2 index
+@pytest.mark.parametrize("seed", range(4))
+def test_index_bit_exact_random(B, oracle, seed):
+    m = W.random_block_pattern(nb=40 + 17 * seed, density=0.15, max_bs=7, seed=seed)
+    _check_index(B, oracle, m)
+
+
+def test_index_bit_exact_water(B, oracle, cfg0):
+    _check_index(B, oracle, cfg0)
+    _check_index(B, oracle, W.make_config(2))
+    _check_index(B, oracle, W.water_like(64, "DZVP", 5.0, seed=2))
+    _check_index(B, oracle, W.water_like(32, "SZV", 6.0, seed=3, group="atom"))
+
+
+def test_index_bit_exact_full_size(B, oracle):
+    """BASELINE configs 3 and 4 at full size (integer work: the oracle index is cheap)."""
+    for c in (3, 4):
+        m = W.make_config(c)
+        plan = B.plan_from_matrix(m)
+        idx = _check_index(B, oracle, m, plan)
+        info = B.sm_plan_query(plan)
+        assert info.nnz == len(m.values) and info.ngroups == m.ngroups
+        assert info.sum_n3 == int((idx.sub_dim.astype(np.int64) ** 3).sum())
+        B.sm_plan_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ a3 + a6 round trip
+@pytest.mark.parametrize("mu", [0.0, 0.37])
+def test_gather_scatter_identity_roundtrip(B, cfg0, mu):
+    """P8: gather then scatter with f = identity returns K~ - mu I on the pattern, bit for bit."""
+    torch = _torch()
+    for m in (cfg0, W.random_block_pattern(nb=37, density=0.2, max_bs=9, seed=5)):
+        plan = B.plan_from_matrix(m)
+        ws = B.alloc_workspace(plan)
+        vin = torch.from_numpy(m.values).cuda()
+        vout = torch.full_like(vin, float("nan"))
+        B.sm_gather(plan, vin, mu, ws)
+        B.sm_scatter(plan, 1, vout, ws)
+        torch.cuda.synchronize()
+        expect = m.values.copy()
+        vo = m.val_off()
+        bc = m.block_cols()
+        for b in np.nonzero(m.rowidx == bc)[0]:
+            n = int(m.blk_size[bc[b]])
+            expect[vo[b]:vo[b + 1]] -= mu * np.eye(n).reshape(-1)
+        assert np.array_equal(vout.cpu().numpy(), expect)
+        B.sm_plan_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ a3-a6 sign parity
+def test_config0_full_parity(B, oracle, cfg0):
+    m = cfg0
+    plan, st, d_gpu, stats, ws, vin = _run_sign(B, m)
+    assert st == B.SM_OK and stats.not_converged == 0 and stats.max_residual < EPS
+    idx = oracle.Index(m)
+    d_or = oracle.density(idx, m.values, 0.0)
+    assert np.abs(d_gpu - d_or).max() <= TOL_D
+    td_o, tdk_o = oracle.traces(idx, d_or, m.values)
+    vout = _torch().from_numpy(d_gpu).cuda()
+    td_g, tdk_g = B.sm_trace_dk(plan, vout, vin)
+    assert abs(tdk_g - tdk_o) / abs(tdk_o) <= TOL_E
+    assert abs(td_g - td_o) <= 1e-9
+    assert abs(stats.n_elec - td_o) <= 1e-9  # a7: Algorithm-1 count == tr(D~)
+    # determinism: a second run is bitwise identical
+    plan2, st2, d_gpu2, _, _, _ = _run_sign(B, m)
+    assert np.array_equal(d_gpu, d_gpu2)
+    B.sm_plan_destroy(plan); B.sm_plan_destroy(plan2)
+
+
+@pytest.mark.parametrize("mu", [-0.9, 0.11])
+def test_config0_shifted_mu(B, oracle, cfg0, mu):
+    """mu inside the occupied band: slow convergence, still parity where eigenvalues are not at mu."""
+    m = cfg0
+    plan, st, d_gpu, stats, _, _ = _run_sign(B, m, mu=mu)
+    idx = oracle.Index(m)
+    d_or = oracle.density(idx, m.values, mu)
+    lam, w, ptr, g = oracle.eig_groups(idx, m.values)
+    gap = np.abs(lam - mu).min()
+    assert st in (B.SM_OK, B.SM_WARN_SIGN_NOT_CONVERGED)
+    if st == B.SM_OK:
+        assert np.abs(d_gpu - d_or).max() <= max(TOL_D, 1e-13 / gap)
+    B.sm_plan_destroy(plan)
+
+
+def test_config1_closed_form_and_oracle(B, oracle):
+    """BASELINE config 1: 512 dense n=256 matrices.  All 512 against the closed form
+    sign(A) = Q sgn(lam) Q^T (P1); a sample of 6 also against the Jacobi oracle."""
+    m = W.make_config(1)
+    q, lam = m.meta["Q"], m.meta["lam"]
+    plan, st, d_gpu, stats, _, _ = _run_sign(B, m)
+    assert st == B.SM_OK
+    info = B.sm_plan_query(plan)
+    assert info.dim_min == 256 and info.dim_max == 256 and info.ngroups == 512
+    d = d_gpu.reshape(512, 256, 256)
+    expect = 0.5 * (np.eye(256)[None] - np.einsum("bik,bk,bjk->bij", q, np.sign(lam), q))
+    assert np.abs(d - expect).max() <= TOL_D
+    idx = oracle.Index(m)
+    groups = np.array([0, 100, 255, 256, 400, 511], dtype=np.int32)
+    d_or = oracle.density(idx, m.values, 0.0, groups)
+    mask, _ = _column_mask(idx, m, groups)
+    assert np.abs(d_gpu - d_or)[mask].max() <= TOL_D
+    assert stats.iter_max <= 25
+    B.sm_plan_destroy(plan)
+
+
+def _sampled_parity(B, oracle, m, k, mu=0.0):
+    plan, st, d_gpu, stats, ws, vin = _run_sign(B, m, mu=mu)
+    assert st == B.SM_OK, (st, stats.not_converged, stats.max_residual)
+    idx = _check_index(B, oracle, m, plan)
+    groups = _sample_groups(idx, k)
+    d_or = oracle.density(idx, m.values, mu, groups)
+    mask, cols = _column_mask(idx, m, groups)
+    err = np.abs(d_gpu - d_or)[mask].max()
+    assert err <= TOL_D, err
+    td_o, tdk_o = oracle.traces(idx, d_or, m.values, cols)
+    td_g, tdk_g = oracle.traces(idx, d_gpu, m.values, cols)  # same reduction on the GPU output
+    assert abs(tdk_g - tdk_o) / abs(tdk_o) <= TOL_E
+    # properties that hold at any size, on the whole GPU output
+    assert np.all(np.isfinite(d_gpu))
+    td_all, tdk_all = B.sm_trace_dk(plan, _torch().from_numpy(d_gpu).cuda(), vin)
+    assert abs(td_all - m.n_occ) < 1e-5 * m.n_occ  # the method's own error band (A11)
+    assert abs(stats.n_elec - td_all) <= 1e-9 * max(1.0, abs(td_all))
+    B.sm_plan_destroy(plan)
+    return stats
+
+
+def test_config2_sampled_parity(B, oracle):
+    _sampled_parity(B, oracle, W.make_config(2), k=24)
+
+
+def test_config3_sampled_parity_full_size(B, oracle):
+    """DZVP, n ~ 500: the launch configuration bench.py would time; oracle on sampled groups."""
+    _sampled_parity(B, oracle, W.make_config(3), k=6)
+
+
+def test_config4_sampled_parity_full_size(B, oracle):
+    """BASELINE config 4 at full size (20736 submatrices) in bench.py's launch configuration."""
+    _sampled_parity(B, oracle, W.make_config(4), k=16)
+
+
+# ------------------------------------------------------------------------------ edge cases
+def test_ragged_blocks_and_scattered_groups(B, oracle):
+    for seed in range(3):
+        m = W.random_block_pattern(nb=30 + seed, density=0.2, max_bs=7, seed=10 + seed)
+        plan, st, d_gpu, stats, _, _ = _run_sign(B, m, mu=0.05)
+        idx = oracle.Index(m)
+        d_or = oracle.density(idx, m.values, 0.05)
+        lam, _, _, _ = oracle.eig_groups(idx, m.values)
+        gap = np.abs(lam - 0.05).min()
+        assert st == B.SM_OK
+        assert np.abs(d_gpu - d_or).max() <= max(TOL_D, 1e-13 / gap)
+        B.sm_plan_destroy(plan)
+
+
+def test_tiny_and_degenerate(B, oracle):
+    torch = _torch()
+    # 1x1 matrix, n < one DMMA tile
+    m = W.BlockSparseSym(1, np.array([1], np.int32), np.array([0, 1], np.int64), np.array([0], np.int32),
+                         np.array([-0.7]), np.array([0, 1], np.int32), np.array([0], np.int32))
+    plan, st, d, stats, _, _ = _run_sign(B, m)
+    assert st == B.SM_OK and d[0] == 1.0
+    B.sm_plan_destroy(plan)
+    # already-involutory input: converges at iteration 0 (scatter applies 1/s)
+    a = np.array([[3.0, 4.0], [4.0, -3.0]])
+    m = W.dense_batch_as_blocks(a[None])
+    plan, st, d, stats, _, _ = _run_sign(B, m)
+    assert st == B.SM_OK and stats.iter_max == 0
+    assert np.allclose(d.reshape(2, 2), 0.5 * (np.eye(2) - a / 5), atol=1e-15)
+    B.sm_plan_destroy(plan)
+    # diagonal matrix -> elementwise signum
+    dv = np.array([-2.0, 0.5, 3.0, -1e-3, 0.25, -0.5, 1.0, 2.0, -4.0])
+    m = W.dense_batch_as_blocks(np.diag(dv)[None])
+    plan, st, d, stats, _, _ = _run_sign(B, m)
+    assert st == B.SM_OK
+    assert np.allclose(d.reshape(9, 9), np.diag(dv < 0).astype(float), atol=1e-12)
+    B.sm_plan_destroy(plan)
+    # empty problem
+    e32, e64 = np.zeros(0, np.int32), np.zeros(1, np.int64)
+    plan = B.sm_plan_create(0, e32, e64, e32, 0, np.zeros(1, np.int32), e32)
+    ws = B.alloc_workspace(plan)
+    v = torch.zeros(0, dtype=torch.float64, device="cuda")
+    assert B.sm_sign_execute(plan, v, 0.0, EPS, v, ws) == B.SM_OK
+    B.sm_plan_destroy(plan)
+
+
+def test_zero_eigenvalue_is_flagged(B):
+    """Eq.(12) / reading A10: x = 0 is an unstable fixed point of Newton-Schulz; the library must
+    report it (warning status), not return silently."""
+    a = np.array([[1.0, 1.0], [1.0, 1.0]])
+    m = W.dense_batch_as_blocks(a[None])
+    opt = B.default_options(max_iter=60)
+    plan, st, d, stats, _, _ = _run_sign(B, m, opt=opt)
+    assert st == B.SM_WARN_SIGN_NOT_CONVERGED and stats.not_converged == 1
+    B.sm_plan_destroy(plan)
+
+
+def test_structure_errors(B):
+    m = W.random_block_pattern(nb=12, density=0.3, max_bs=3, seed=1)
+
+    def create(**kw):
+        a = dict(nb=m.nb, blk_size=m.blk_size, colptr=m.colptr, rowidx=m.rowidx, ngroups=m.ngroups,
+                 grp_ptr=m.grp_ptr, grp_cols=m.grp_cols)
+        a.update(kw)
+        return B.sm_plan_create(a["nb"], a["blk_size"], a["colptr"], a["rowidx"], a["ngroups"], a["grp_ptr"],
+                                a["grp_cols"])
+
+    def status_of(**kw):
+        try:
+            p = create(**kw)
+        except B.SubmatrixError as e:
+            return e.status
+        B.sm_plan_destroy(p)
+        return 0
+
+    assert status_of() == 0
+    r = m.rowidx.copy(); r[[0, 1]] = r[[1, 0]] if m.colptr[1] >= 2 else r[[0, 1]]
+    gc = m.grp_cols.copy(); gc[0] = gc[1]
+    assert status_of(grp_cols=gc) == B.SM_ERR_STRUCTURE  # not a partition
+    # asymmetric pattern: drop one off-diagonal block
+    cols = m.block_cols()
+    off = np.nonzero(m.rowidx != cols)[0]
+    if len(off):
+        k = off[0]
+        rowidx = np.delete(m.rowidx, k)
+        colptr = m.colptr.copy(); colptr[cols[k] + 1:] -= 1
+        assert status_of(rowidx=rowidx, colptr=colptr) == B.SM_ERR_STRUCTURE
+    # missing diagonal block
+    k = np.nonzero(m.rowidx == cols)[0][0]
+    rowidx = np.delete(m.rowidx, k)
+    colptr = m.colptr.copy(); colptr[cols[k] + 1:] -= 1
+    assert status_of(rowidx=rowidx, colptr=colptr) == B.SM_ERR_STRUCTURE
+    # workspace too small
+    plan = create()
+    torch = _torch()
+    v = torch.from_numpy(m.values).cuda()
+    small = torch.empty(32, dtype=torch.float64, device="cuda")
+    with pytest.raises(B.SubmatrixError) as ei:
+        B.sm_sign_execute(plan, v, 0.0, EPS, v.clone(), small)
+    assert ei.value.status == B.SM_ERR_WORKSPACE_TOO_SMALL
+    B.sm_plan_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ a7 + a8 bisection
+def test_density_matrix_bisection_config0(B, oracle, cfg0):
+    """Algorithm 1 / reading A11-A12: same bisection trace as the oracle's (which uses stored
+    eigendecompositions), same plateau; D~ parity at the GPU's final mu."""
+    torch = _torch()
+    m = cfg0
+    idx = oracle.Index(m)
+    lam, w, ptr, g = oracle.eig_groups(idx, m.values)
+    lo, hi = oracle.gershgorin_interval(m)
+    for mu0, tol_n in ((-1.0, 0.5), (1.2, 0.5)):
+        plan = B.plan_from_matrix(m)
+        ws = B.alloc_workspace(plan)
+        vin = torch.from_numpy(m.values).cuda()
+        vout = torch.empty_like(vin)
+        stats = B.sm_stats_t()
+        st, mu = B.sm_density_matrix(plan, vin, float(m.n_occ), tol_n, EPS, mu0, vout, ws, stats)
+        torch.cuda.synchronize()
+        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0, lo, hi, tol_n)
+        assert st == B.SM_OK
+        assert stats.mu_steps == len(trace_o)
+        for k, (mo, no) in enumerate(trace_o):
+            assert abs(stats.mu_trace[k] - mo) <= 1e-12 * max(1, abs(mo))  # same bracket (Gershgorin) and midpoints
+        assert abs(stats.n_elec - ne_o) <= 1e-9  # same plateau
+        d_or = oracle.density(idx, m.values, mu)
+        assert np.abs(vout.cpu().numpy() - d_or).max() <= TOL_D
+        B.sm_plan_destroy(plan)
+
+
+def test_density_matrix_unreachable_tolerance_is_guarded(B, cfg0):
+    """BASELINE config 4 asks for 1e-8 on tr(D); the method's own offset makes that unreachable
+    (A11): the call must stop on its guards with a warning and still return the best step."""
+    torch = _torch()
+    m = cfg0
+    plan = B.plan_from_matrix(m, B.default_options(max_mu_steps=12))
+    ws = B.alloc_workspace(plan)
+    vin = torch.from_numpy(m.values).cuda()
+    vout = torch.empty_like(vin)
+    stats = B.sm_stats_t()
+    st, mu = B.sm_density_matrix(plan, vin, float(m.n_occ), 1e-8, EPS, 0.0, vout, ws, stats)
+    assert st == B.SM_WARN_MU_NOT_CONVERGED and stats.mu_steps <= 12
+    assert abs(stats.n_elec - m.n_occ) < 1e-2
+    B.sm_plan_destroy(plan)
+
+
+def test_host_buffer_entry_point(B, oracle, cfg0):
+    torch = _torch()
+    m = cfg0
+    plan = B.plan_from_matrix(m)
+    ws = B.alloc_workspace(plan)
+    hin = torch.from_numpy(m.values).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    st = B.sm_sign_execute_host(plan, hin, 0.0, EPS, hout, ws)
+    assert st == B.SM_OK
+    idx = oracle.Index(m)
+    assert np.abs(hout.numpy() - oracle.density(idx, m.values, 0.0)).max() <= TOL_D
+    assert B.sm_launch_count(plan) > 4
+    B.sm_plan_destroy(plan)
