@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py -- density-matrix builds/s of the submatrix hot path on B200 (BASELINE.json metric).
+
+One "step" = one pass of the whole hot path over one synthetic input: sm_density_matrix on
+BASELINE config 4 (20736 water molecules, SZV, cutoff 6 A, one submatrix per molecule): Gershgorin
+bracket of K~, mu bisection from mu0 (each step = gather -> Newton-Schulz FP64 DMMA sign of all
+20736 submatrices -> electron count), final extract/scatter of D~.  The plan (device BSR container
++ submatrix index, built once per sparsity pattern) is created before the timed region, like the
+paper's initialisation phase (PAPER.md IV-A).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+Prints ONE JSON line (rank 0).  `value` = builds/s with K~ already resident in HBM; `e2e` = the
+same through the C-ABI host-buffer call (H2D of K~ and D2H of D~ inside the timed region);
+`roofline` = the Newton-Schulz GEMM kernel against the FP64 tensor peak; `cpu_baseline` = the CPU
+oracle timed on this box's cores on a bounded sample.  N > 1: N independent replicas (the path does
+not shard in this build), weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "density_matrix_builds_per_s"
+UNIT = "builds/s"
+EPS = 1e-12
+TOL_N = 0.5      # plateau acceptance (reading A11); 1e-8 is unreachable by construction
+MU0 = -1.0       # starting mu inside the occupied band: forces a genuine bisection
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of k_ns_gemm from the committed
+# `ncu --set full` capture (profiles/), or None when no capture matches the current kernel.
+NS_GEMM_DRAM_BYTES_PER_LAUNCH = None
+NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # guide: B200 FP64 tensor 45 TF/s, bf16 2250 TF/s (nominal)
+
+
+def fp64_peak_tflops():
+    """Roofline denominator for an FP64 contraction: measured bf16 peak x nominal FP64/bf16 ratio."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            pk = json.load(f)
+        return pk["bf16_tflops"] * NOMINAL_FP64_OVER_BF16, "measured bf16 burst x 45/2250 (MEASURED_PEAKS.json)"
+    return 1590.0 * NOMINAL_FP64_OVER_BF16, "fallback bf16 1.59 PF x 45/2250"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (profiling recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        os.unlink(self.f.name)
+        if sm:
+            # "under load": samples above 60% of the max power seen
+            thr = 0.6 * max(pw)
+            load = [s for s, w in zip(sm, pw) if w >= thr] or sm
+            out = {"sm_mhz": statistics.median(load), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                   "power_w_max": max(pw), "samples": len(sm)}
+        return out
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def max_over_ranks(ms: float, world: int, backend_device) -> float:
+    """MAX over ranks of a per-rank time (plumbing only; no data-path collective)."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=backend_device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def cpu_baseline(m, sample_groups=None, nthreads=0):
+    """The oracle as it stands, timed on this box's cores on a bounded sample of the workload:
+    Jacobi eigendecomposition + sign + extraction of `sample_groups` submatrices; the whole-job
+    time is extrapolated by sum n_i^3 (Eq.(14)).  One decomposition serves the whole mu loop
+    (Algorithm 1), so a build costs one pass."""
+    from oracle import oracle as O
+    cores = nthreads or os.cpu_count() or 1
+    idx = O.Index(m)
+    if sample_groups is None:
+        k = min(idx.ngroups, 4 * cores)
+        sample_groups = np.linspace(0, idx.ngroups - 1, k).astype(np.int32)
+    t0 = time.perf_counter()
+    _ = O._run_groups(idx, m.values, sample_groups, 0.0, True, True, cores)
+    dt = time.perf_counter() - t0
+    n3 = idx.sub_dim.astype(np.float64) ** 3
+    scale = n3.sum() / n3[sample_groups].sum()
+    t_full = dt * scale
+    return {"value": 1.0 / t_full, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{len(sample_groups)} of {idx.ngroups} submatrices (evenly spaced), {dt:.2f} s measured, "
+                      f"extrapolated x{scale:.1f} by sum n^3", "seconds_measured": dt}, t_full
+
+
+def run_reference(args, m, rank):
+    """--impl reference: the oracle on the host cores, each step a bounded sample."""
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    times = []
+    cb = None
+    for it in range(args.warmup + args.steps):
+        cb, t_full = cpu_baseline(m)
+        if it >= args.warmup:
+            times.append(t_full)
+    t = sum(times) / len(times)
+    line = {"impl": "reference", "metric": METRIC, "value": 1.0 / t, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(args, m), "cpu_baseline": dict(cb, value=1.0 / t),
+            "e2e": {"value": 1.0 / t, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(args, m):
+    from paper_2004_10811_b200 import workloads as W
+    c = W.CONFIGS[args.config]
+    return {"workload": f"BASELINE config {args.config}: " + (
+                f"{c['n_mol']} H2O {c['basis']} cutoff {c['cutoff']} A, one submatrix per molecule"
+                if c["kind"] == "water" else f"{c['batch']} dense n={c['n']} (block-diagonal plan)"),
+            "n_basis": int(m.n_basis), "nnzb": int(m.nnzb), "ngroups": int(m.ngroups),
+            "n_target": int(m.n_occ), "tol_n": TOL_N, "mu0": MU0, "eps": EPS,
+            "cache": "inputs larger than L2 (dense workspace >> 126 MB)" if args.config in (3, 4)
+                     else "L2 flushed between steps", "seed": args.seed}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, local_rank, world = dist_env()
+    from paper_2004_10811_b200 import workloads as W
+
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, W.make_config(args.config, args.seed), rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2004_10811_b200 import binding as B
+    B.lib()  # fail loudly if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    # replicas: rank r builds the same-size problem from seed + r
+    m = W.make_config(args.config, args.seed + rank)
+    plan = B.plan_from_matrix(m)
+    info = B.sm_plan_query(plan)
+    ws = B.alloc_workspace(plan)
+    d_in = torch.from_numpy(m.values).cuda()
+    d_out = torch.empty_like(d_in)
+    h_in = torch.from_numpy(m.values).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda") if args.config not in (3, 4) else None
+    stats = B.sm_stats_t()
+    B.sm_set_timing(plan, True)
+    n_target = float(m.n_occ)
+    stream = torch.cuda.current_stream()
+
+    def step_device():
+        if flush is not None:
+            flush.zero_()
+        return B.sm_density_matrix(plan, d_in, n_target, TOL_N, EPS, MU0, d_out, ws, stats)
+
+    def step_host():
+        if flush is not None:
+            flush.zero_()
+        return B.sm_density_matrix_host(plan, h_in, n_target, TOL_N, EPS, MU0, h_out, ws, stats)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        st, mu = step_device()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    launches0 = B.sm_launch_count(plan)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    gemm_ms = gemm_launches = sym_flop = n3 = evals = 0.0
+    gather_ms = 0.0
+    e0.record(stream)
+    for _ in range(args.steps):
+        st, mu = step_device()
+        gemm_ms += stats.tot_ms_sign; gemm_launches += stats.tot_gemm_launches
+        sym_flop += stats.tot_sym_flop; n3 += stats.tot_sum_iter_n3; evals += stats.tot_evaluations
+        gather_ms += stats.tot_ms_gather
+    e1.record(stream)
+    barrier()
+    launches = B.sm_launch_count(plan) - launches0
+    ms = max_over_ranks(e0.elapsed_time(e1), world, torch.device("cuda", local_rank))
+    clocks = sampler.stop() if sampler else None
+    last = stats.as_dict()
+
+    # end to end through the host-buffer C-ABI call
+    for _ in range(1):
+        step_host()
+    barrier()
+    k_e2e = max(1, min(args.steps, 3))
+    e0.record(stream)
+    for _ in range(k_e2e):
+        step_host()
+    e1.record(stream)
+    barrier()
+    ms_e2e = max_over_ranks(e0.elapsed_time(e1), world, torch.device("cuda", local_rank))
+
+    if rank == 0:
+        peak, peak_src = fp64_peak_tflops()
+        # dominant kernel: k_ns_gemm<0|1>.  Algorithmic flops of one symmetric n x n product:
+        # n(n+1)/2 outputs x 2n flop = n^2 (n+1); per launch = sum over the active submatrices.
+        ach = sym_flop / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
+        roofline = {"bound": "tensor", "kernel": "k_ns_gemm (FP64 DMMA Newton-Schulz, both modes)",
+                    "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                    "traffic": NS_GEMM_DRAM_BYTES_PER_LAUNCH, "peak_source": peak_src,
+                    "peak_dmma_issue_measured": 37.1, "frac_of_dmma_issue": ach / 37.1,
+                    "launches_timed": int(gemm_launches), "avg_launch_ms": gemm_ms / max(gemm_launches, 1),
+                    "alg_flop_per_launch": sym_flop / max(gemm_launches, 1),
+                    "full_gemm_equiv_tflops": 2.0 * n3 / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0,
+                    "sign_share_of_step": gemm_ms / ms if ms > 0 else None}
+        gather_bytes = (info.sum_ld2 + info.nnz) * 8.0
+        line = {"metric": METRIC, "value": world * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "data": "synthetic", "config": workload_config(args, m), "clocks": clocks,
+                "e2e": {"value": world * k_e2e / (ms_e2e * 1e-3), "unit": UNIT,
+                        "h2d_bytes_per_step": int(info.nnz * 8), "d2h_bytes_per_step": int(info.nnz * 8)},
+                "gpu_launches": int(launches), "roofline": roofline,
+                "detail": {"status": int(st), "mu": mu, "mu_steps": last["mu_steps"], "n_elec": last["n_elec"],
+                           "sign_evaluations_per_step": evals / args.steps,
+                           "ns_iterations_last_eval": last["iterations"], "iter_min": last["iter_min"],
+                           "iter_max": last["iter_max"], "max_residual": last["max_residual"],
+                           "dim_min": info.dim_min, "dim_mean": info.dim_mean, "dim_max": info.dim_max,
+                           "workspace_GB": info.workspace_bytes / 1e9, "n_tiles": info.n_tiles,
+                           "gather_GBps": gather_bytes * evals / (gather_ms * 1e-3) / 1e9 if gather_ms > 0 else None,
+                           "ms_scatter_last": last["ms_scatter"], "mu_trace": last["mu_trace"],
+                           "ne_trace": last["ne_trace"]}}
+        if not args.no_cpu_baseline:
+            cb, _ = cpu_baseline(m)
+            line["cpu_baseline"] = cb
+        print(json.dumps(line), flush=True)
+    B.sm_plan_destroy(plan)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

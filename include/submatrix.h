@@ -103,6 +103,12 @@ typedef struct {
     float ms_gather, ms_sign, ms_scatter, ms_total;
     double mu_trace[64];      /* bisection history: mu of step k                             */
     double ne_trace[64];      /* n_elec of step k                                            */
+    /* totals over ALL sign evaluations of the call (a bisection makes several) */
+    int64_t tot_sum_iter_n3;  /* sum over evaluations of sum_iter_n3                         */
+    int64_t tot_sym_flop;     /* sum over executed symmetric products of n_i^2 (n_i + 1)     */
+    int32_t tot_gemm_launches;
+    int32_t tot_evaluations;
+    float tot_ms_gather, tot_ms_sign;
 } sm_stats_t;
 
 /*

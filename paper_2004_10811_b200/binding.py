@@ -51,7 +51,9 @@ class sm_stats_t(C.Structure):
                 ("mu", C.c_double), ("mu_steps", C.c_int32), ("gemm_launches", C.c_int32),
                 ("sum_iter_n3", C.c_int64), ("ms_gather", C.c_float), ("ms_sign", C.c_float),
                 ("ms_scatter", C.c_float), ("ms_total", C.c_float), ("mu_trace", C.c_double * 64),
-                ("ne_trace", C.c_double * 64)]
+                ("ne_trace", C.c_double * 64), ("tot_sum_iter_n3", C.c_int64), ("tot_sym_flop", C.c_int64),
+                ("tot_gemm_launches", C.c_int32), ("tot_evaluations", C.c_int32),
+                ("tot_ms_gather", C.c_float), ("tot_ms_sign", C.c_float)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_ if k not in ("mu_trace", "ne_trace")}

@@ -259,7 +259,7 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
     SM_CUDA(cudaStreamSynchronize(st));
     int imin = INT32_MAX, imax = 0, nc = 0;
     double rmax = 0.0;
-    int64_t sin3 = 0;
+    int64_t sin3 = 0, symf = 0;
     for (int i = 0; i < ng; ++i) {
         int it = di[i] >= 0 ? di[i] : p->cur_k;
         if (di[i] < 0 || fl[i]) ++nc;
@@ -271,6 +271,7 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         int64_t n = p->h_sub_dim[i];
         // executed GEMMs: one X^2 per tested iterate (it + 1) and one update per iteration (it)
         sin3 += (int64_t)(2 * it + 1) * n * n * n;
+        symf += (int64_t)(2 * it + 1) * n * n * (n + 1);
     }
     *not_conv = nc;
     if (stats) {
@@ -280,6 +281,7 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         stats->max_residual = rmax;
         stats->n_elec = p->h_pinned_d[0];
         stats->sum_iter_n3 = sin3;
+        stats->tot_sym_flop = symf;  // per evaluation here; callers accumulate
     }
     return SM_OK;
 }
@@ -305,6 +307,11 @@ sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, cons
             cudaEventElapsedTime(&stats->ms_gather, p->ev[0], p->ev[1]);
             cudaEventElapsedTime(&stats->ms_sign, p->ev[1], p->ev[2]);
         }
+        stats->tot_sum_iter_n3 = stats->sum_iter_n3;
+        stats->tot_gemm_launches = launched;
+        stats->tot_evaluations = 1;
+        stats->tot_ms_gather = stats->ms_gather;
+        stats->tot_ms_sign = stats->ms_sign;
     }
     return SM_OK;
 }
@@ -424,6 +431,13 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     int best_step = -1, steps = 0, nc = 0, last_nc = 0;
     bool accepted = false;
     sm_stats_t ev;
+    int64_t acc_n3 = 0, acc_sym = 0;
+    int acc_launch = 0, acc_eval = 0;
+    float acc_g = 0.f, acc_s = 0.f;
+    auto accumulate = [&](const sm_stats_t& e) {
+        acc_n3 += e.tot_sum_iter_n3; acc_sym += e.tot_sym_flop; acc_launch += e.tot_gemm_launches;
+        acc_eval += 1; acc_g += e.tot_ms_gather; acc_s += e.tot_ms_sign;
+    };
     for (; steps < p->opt.max_mu_steps;) {
         memset(&ev, 0, sizeof(ev));
         if ((s = evaluate(p, d_vals_in, mu, eps, b, cap, &ev, &nc, st))) return s;
@@ -435,8 +449,11 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
             if ((s = launch_nelec(p, b.b0, b.b1, st))) return s;
             if ((s = collect_stats(p, &ev, &nc, st))) return s;
             ev.iterations += launched / 2;
+            ev.tot_gemm_launches += launched;
+            ev.tot_sum_iter_n3 = ev.sum_iter_n3;
             g = ev.n_elec - n_target;
         }
+        accumulate(ev);
         S->mu_trace[steps] = mu;
         S->ne_trace[steps] = ev.n_elec;
         last_nc = nc;
@@ -453,6 +470,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         memset(&ev, 0, sizeof(ev));
         if ((s = evaluate(p, d_vals_in, best_mu, eps, b, p->opt.max_iter + 1, &ev, &nc, st))) return s;
         last_nc = nc;
+        accumulate(ev);
     }
     double tr_mu[64], tr_ne[64];
     memcpy(tr_mu, S->mu_trace, sizeof(tr_mu));
@@ -462,6 +480,8 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     memcpy(S->ne_trace, tr_ne, sizeof(tr_ne));
     S->mu = best_mu;
     S->mu_steps = steps;
+    S->tot_sum_iter_n3 = acc_n3; S->tot_sym_flop = acc_sym; S->tot_gemm_launches = acc_launch;
+    S->tot_evaluations = acc_eval; S->tot_ms_gather = acc_g; S->tot_ms_sign = acc_s;
     *mu_inout = best_mu;
     if (d_vals_out && (s = do_scatter(p, b, d_vals_out, S, st))) return s;
     SM_CUDA(cudaStreamSynchronize(st));

@@ -188,9 +188,9 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
         SM_CUDA(cudaFuncSetAttribute(k_index_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bm_bytes));
     }
     int32_t* d_cnt = nullptr;
-    SM_CUDA(cudaMalloc((void**)&d_cnt, (size_t)ng * 4));
-    SM_CUDA(cudaMalloc((void**)&p->d_sub_dim, (size_t)ng * 4));
-    k_index_count<<<ng, 256, bm_bytes, st>>>(nb, p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr,
+    SM_CUDA(cudaMalloc((void**)&d_cnt, (size_t)std::max(ng, 1) * 4));
+    SM_CUDA(cudaMalloc((void**)&p->d_sub_dim, (size_t)std::max(ng, 1) * 4));
+    if (ng > 0) k_index_count<<<ng, 256, bm_bytes, st>>>(nb, p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr,
                                             p->d_grp_cols, d_cnt, p->d_sub_dim);
     p->launches++;
     std::vector<int32_t> cnt(ng);
@@ -213,12 +213,12 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMalloc((void**)&p->d_gen_off, (size_t)std::max(nb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_col_grp, (size_t)std::max(nb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_blk_loc, std::max<int64_t>(p->nnzb, 1) * 4));
-    SM_CUDA(cudaMalloc((void**)&p->d_gen_width, (size_t)ng * 4));
+    SM_CUDA(cudaMalloc((void**)&p->d_gen_width, (size_t)std::max(ng, 1) * 4));
     int32_t* d_err = nullptr;
     SM_CUDA(cudaMalloc((void**)&d_err, 4));
     SM_CUDA(cudaMemsetAsync(d_err, 0, 4, st));
     // pass 2
-    k_index_fill<<<ng, 256, bm_bytes, st>>>(nb, p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr,
+    if (ng > 0) k_index_fill<<<ng, 256, bm_bytes, st>>>(nb, p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr,
                                            p->d_grp_cols, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off,
                                            p->d_gen_pos, p->d_gen_off, p->d_blk_loc, p->d_col_grp,
                                            p->d_gen_width, d_err);

@@ -235,11 +235,17 @@ def test_tiny_and_degenerate(B, oracle):
     assert st == B.SM_OK and d[0] == 1.0
     B.sm_plan_destroy(plan)
     # already-involutory input: converges at iteration 0 (scatter applies 1/s)
-    a = np.array([[3.0, 4.0], [4.0, -3.0]])
+    a = np.array([[0.0, 2.0], [2.0, 0.0]])  # Gershgorin bound 2 = spectral radius: X0 = A/2 is involutory
     m = W.dense_batch_as_blocks(a[None])
     plan, st, d, stats, _, _ = _run_sign(B, m)
     assert st == B.SM_OK and stats.iter_max == 0
-    assert np.allclose(d.reshape(2, 2), 0.5 * (np.eye(2) - a / 5), atol=1e-15)
+    assert np.allclose(d.reshape(2, 2), 0.5 * (np.eye(2) - a / 2), atol=1e-15)
+    B.sm_plan_destroy(plan)
+    a = np.array([[3.0, 4.0], [4.0, -3.0]])  # Eq.(8): sign(A) = A/5
+    m = W.dense_batch_as_blocks(a[None])
+    plan, st, d, stats, _, _ = _run_sign(B, m)
+    assert st == B.SM_OK
+    assert np.allclose(d.reshape(2, 2), 0.5 * (np.eye(2) - a / 5), atol=1e-14)
     B.sm_plan_destroy(plan)
     # diagonal matrix -> elementwise signum
     dv = np.array([-2.0, 0.5, 3.0, -1e-3, 0.25, -0.5, 1.0, 2.0, -4.0])
