@@ -17,7 +17,10 @@
 namespace smb {
 
 constexpr int BM = TILE, BN = TILE, BK = 16, STAGES = 3;
-constexpr int LDS_ROW = BK + 4;  // 20 doubles: row stride = 4 (mod 16) doubles -> conflict-free LDS.64
+// Row stride of the staged operand tiles: 24 doubles = 192 B.  Fragments are read with 16-byte
+// loads (two consecutive k per lane); consecutive rows then start 64 B apart modulo 128 B, so the
+// eight lanes of a quarter-warp (2 rows x 4 lanes x 16 B) hit all 32 banks once: conflict-free.
+constexpr int LDS_ROW = BK + 8;
 constexpr int NTHREADS = 128;    // 4 warps as 2 x 2, warp tile 32 x 32 = 4 x 4 DMMA tiles
 constexpr size_t NS_SMEM = (size_t)STAGES * (BM + BN) * LDS_ROW * sizeof(double);
 
@@ -34,6 +37,31 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
+
+// One staged k-tile (BK = 16) of a warp's 32 x 32 tile: MT x NT DMMA sub-tiles (TRI: only nt <= mt).
+// The contraction index may be visited in any order as long as A and B agree: lane (lr, lk) loads
+// the two consecutive k = 8 j + 2 lk + {0,1} with one 16-byte load; the first DMMA of a pair
+// contracts the even k of the 8-wide group, the second the odd k.
+template <int MT, int NT, bool TRI>
+__device__ __forceinline__ void ktile_mma(double (&acc)[4][4][2], const double* __restrict__ Aw,
+                                          const double* __restrict__ Bw) {
+#pragma unroll
+    for (int j = 0; j < BK / 8; ++j) {
+        double2 af[MT], bf[NT];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) af[mt] = *reinterpret_cast<const double2*>(Aw + mt * 8 * LDS_ROW + j * 8);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) bf[nt] = *reinterpret_cast<const double2*>(Bw + nt * 8 * LDS_ROW + j * 8);
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt)
+                if (!TRI || nt <= mt) {
+                    dmma(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
+                    dmma(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
+                }
+    }
+}
 
 struct NsArgs {
     const TileDesc* tiles;
@@ -136,25 +164,19 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
     };
 
     const int wm = wid >> 1, wn = wid & 1;
-    // which 8x8 DMMA sub-tiles of this warp's 32x32 tile are needed: inside the padded matrix and,
-    // on diagonal tiles, not entirely above the diagonal
-    unsigned need = 0;
-#pragma unroll
-    for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) {
-            const int rm = row0 + wm * 32 + mt * 8, cn = col0 + wn * 32 + nt * 8;
-            bool ok = (rm < ld) && (cn < ld);
-            if (diag && (rm + 7 < cn)) ok = false;
-            if (ok) need |= 1u << (mt * 4 + nt);
-        }
-    unsigned need_m = 0, need_n = 0;
-#pragma unroll
-    for (int mt = 0; mt < 4; ++mt)
-        if (need & (0xfu << (mt * 4))) need_m |= 1u << mt;
-#pragma unroll
-    for (int nt = 0; nt < 4; ++nt)
-        if (need & (0x1111u << nt)) need_n |= 1u << nt;
+    // Work of this warp: number of valid 8-row sub-tile rows (the padded matrix ends inside the last
+    // tile) and, on diagonal tiles, only the sub-tiles that touch the lower triangle.  Off-diagonal
+    // tiles always have all 64 columns (tj < ti <= last).  Warp-uniform: dispatched once per k-tile.
+    const int rows_left = ld - (row0 + wm * 32), cols_left = ld - (col0 + wn * 32);
+    int mt_cnt = rows_left <= 0 ? 0 : (rows_left >= 32 ? 4 : rows_left >> 3);
+    int nt_cnt = cols_left <= 0 ? 0 : (cols_left >= 32 ? 4 : cols_left >> 3);
+    bool tri = false;
+    if (diag) {
+        if (wm < wn) mt_cnt = 0;          // entirely above the diagonal
+        else if (wm == wn) tri = true;    // mt_cnt == nt_cnt here
+    }
+    if (nt_cnt == 0) mt_cnt = 0;
+    const int variant = mt_cnt == 0 ? 0 : (tri ? 4 + mt_cnt : mt_cnt);  // 1..4 FULL<MT,nt>, 5..8 TRI<S>
 
     double acc[4][4][2];
 #pragma unroll
@@ -177,20 +199,24 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
             cp_async_commit();
         }
         const int stage = kt % STAGES;
-        const double* Aw = As + ((size_t)stage * BM + wm * 32 + lr) * LDS_ROW + lk;
-        const double* Bw = Bs + ((size_t)stage * BN + wn * 32 + lr) * LDS_ROW + lk;
-#pragma unroll
-        for (int ks = 0; ks < BK / 4; ++ks) {
-            double af[4], bf[4];
-#pragma unroll
-            for (int mt = 0; mt < 4; ++mt) af[mt] = (need_m >> mt & 1) ? Aw[mt * 8 * LDS_ROW + ks * 4] : 0.0;
-#pragma unroll
-            for (int nt = 0; nt < 4; ++nt) bf[nt] = (need_n >> nt & 1) ? Bw[nt * 8 * LDS_ROW + ks * 4] : 0.0;
-#pragma unroll
-            for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-                for (int nt = 0; nt < 4; ++nt)
-                    if (need >> (mt * 4 + nt) & 1) dmma(acc[mt][nt][0], acc[mt][nt][1], af[mt], bf[nt]);
+        const double* Aw = As + ((size_t)stage * BM + wm * 32 + lr) * LDS_ROW + 2 * lk;
+        const double* Bw = Bs + ((size_t)stage * BN + wn * 32 + lr) * LDS_ROW + 2 * lk;
+        if (nt_cnt == 4 || tri) {
+            switch (variant) {
+                case 4: ktile_mma<4, 4, false>(acc, Aw, Bw); break;
+                case 3: ktile_mma<3, 4, false>(acc, Aw, Bw); break;
+                case 2: ktile_mma<2, 4, false>(acc, Aw, Bw); break;
+                case 1: ktile_mma<1, 4, false>(acc, Aw, Bw); break;
+                case 8: ktile_mma<4, 4, true>(acc, Aw, Bw); break;
+                case 7: ktile_mma<3, 3, true>(acc, Aw, Bw); break;
+                case 6: ktile_mma<2, 2, true>(acc, Aw, Bw); break;
+                case 5: ktile_mma<1, 1, true>(acc, Aw, Bw); break;
+                default: break;
+            }
+        } else if (variant) {
+            // cannot happen for lower-triangular tiles (see above); kept for safety: full 4 x 4 on
+            // zero-filled operands is still correct
+            ktile_mma<4, 4, false>(acc, Aw, Bw);
         }
     }
     cp_async_wait<0>();
@@ -205,7 +231,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
     for (int mt = 0; mt < 4; ++mt)
 #pragma unroll
         for (int nt = 0; nt < 4; ++nt) {
-            if (!(need >> (mt * 4 + nt) & 1)) continue;
+            if (mt >= mt_cnt || nt >= nt_cnt || (tri && nt > mt)) continue;
             const int r = row0 + wm * 32 + mt * 8 + lr;
             const int c = col0 + wn * 32 + nt * 8 + 2 * lk;
             if (r >= ld || c >= ld) continue;  // ld is a multiple of 8: whole sub-tile in or out
