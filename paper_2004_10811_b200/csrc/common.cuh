@@ -13,10 +13,16 @@ namespace smb {
 constexpr int TILE = 64;        // CTA tile edge of the Newton-Schulz GEMMs
 constexpr int LD_ALIGN = 8;     // padded leading dimension granularity (one DMMA k-step pair)
 
-// One CTA tile of one submatrix: lower-triangular tile (ti >= tj) of a symmetric product.
-struct TileDesc {
-    int32_t grp;   // submatrix (= generating group) index
-    int32_t tij;   // ti | (tj << 16)
+// One CTA tile of one submatrix: lower-triangular tile (ti >= tj) of a symmetric product, with
+// the geometry of its submatrix inlined so that a CTA needs a single 32-byte load to start.
+struct __align__(16) TileDesc {
+    int64_t ws_off;      // offset (doubles) of the submatrix in each workspace buffer
+    int32_t grp;         // submatrix (= generating group) index
+    int32_t ld;          // padded leading dimension
+    int32_t n;           // true dimension
+    int32_t tij;         // ti | (tj << 16)
+    int32_t tile_first;  // first tile of this submatrix in the tile list
+    int32_t tile_count;  // number of tiles of this submatrix
 };
 
 void set_cuda_error(cudaError_t e, const char* where);

@@ -12,6 +12,14 @@
 // only FP64 MMA sm_100a has; tcgen05 has no f64 kind), fed from shared memory by a 3-stage
 // cp.async pipeline.  MODE 1 first reduces the per-tile partials of its submatrix in a fixed
 // order (deterministic, no atomics on doubles) and decides convergence per submatrix.
+//
+// Work split inside a CTA (4 warps).  The FP64 pipe is per SM sub-partition, so the four warps of
+// a CTA must carry equal work whatever the tile looks like:
+//   * rectangular tiles (off-diagonal, or the small last diagonal tile): warp w owns the two
+//     8-column sub-tiles 2w, 2w+1 and ALL valid 8-row sub-tiles (M = 1..8, the padded matrix may
+//     end inside the tile): M x 2 DMMA tiles per warp, identical for the four warps;
+//   * full diagonal tiles: only the 36 sub-tiles on or below the diagonal are needed; warp w owns
+//     the sub-tile rows w and 7-w, i.e. (w+1) + (8-w) = 9 sub-tiles for every warp.
 #include "common.cuh"
 
 namespace smb {
@@ -21,12 +29,12 @@ constexpr int BM = TILE, BN = TILE, BK = 16, STAGES = 3;
 // loads (two consecutive k per lane); consecutive rows then start 64 B apart modulo 128 B, so the
 // eight lanes of a quarter-warp (2 rows x 4 lanes x 16 B) hit all 32 banks once: conflict-free.
 constexpr int LDS_ROW = BK + 8;
-constexpr int NTHREADS = 128;    // 4 warps as 2 x 2, warp tile 32 x 32 = 4 x 4 DMMA tiles
+constexpr int NTHREADS = 128;
 constexpr size_t NS_SMEM = (size_t)STAGES * (BM + BN) * LDS_ROW * sizeof(double);
 
-__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
+__device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-        : "+d"(c0), "+d"(c1)
+        : "+d"(c[0]), "+d"(c[1])
         : "d"(a), "d"(b));
 }
 
@@ -38,38 +46,60 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
 
-// One staged k-tile (BK = 16) of a warp's 32 x 32 tile: MT x NT DMMA sub-tiles (TRI: only nt <= mt).
 // The contraction index may be visited in any order as long as A and B agree: lane (lr, lk) loads
 // the two consecutive k = 8 j + 2 lk + {0,1} with one 16-byte load; the first DMMA of a pair
 // contracts the even k of the 8-wide group, the second the odd k.
-template <int MT, int NT, bool TRI>
-__device__ __forceinline__ void ktile_mma(double (&acc)[4][4][2], const double* __restrict__ Aw,
-                                          const double* __restrict__ Bw) {
+//
+// Rectangular tile: M valid row sub-tiles x this warp's 2 column sub-tiles.  acc[2 mt + nt].
+// Ap = stage A + lr * LDS_ROW + 2 lk;  Bp = stage B + (16 w + lr) * LDS_ROW + 2 lk.
+template <int M>
+__device__ __forceinline__ void ktile_rect(double (&acc)[16][2], const double* __restrict__ Ap,
+                                           const double* __restrict__ Bp) {
 #pragma unroll
     for (int j = 0; j < BK / 8; ++j) {
-        double2 af[MT], bf[NT];
+        double2 bf[2], af[M];
 #pragma unroll
-        for (int mt = 0; mt < MT; ++mt) af[mt] = *reinterpret_cast<const double2*>(Aw + mt * 8 * LDS_ROW + j * 8);
+        for (int nt = 0; nt < 2; ++nt) bf[nt] = *reinterpret_cast<const double2*>(Bp + nt * 8 * LDS_ROW + j * 8);
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) bf[nt] = *reinterpret_cast<const double2*>(Bw + nt * 8 * LDS_ROW + j * 8);
+        for (int mt = 0; mt < M; ++mt) af[mt] = *reinterpret_cast<const double2*>(Ap + mt * 8 * LDS_ROW + j * 8);
 #pragma unroll
-        for (int mt = 0; mt < MT; ++mt)
+        for (int mt = 0; mt < M; ++mt)
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt)
-                if (!TRI || nt <= mt) {
-                    dmma(acc[mt][nt][0], acc[mt][nt][1], af[mt].x, bf[nt].x);
-                    dmma(acc[mt][nt][0], acc[mt][nt][1], af[mt].y, bf[nt].y);
-                }
+            for (int nt = 0; nt < 2; ++nt) dmma(acc[2 * mt + nt], af[mt].x, bf[nt].x);
+#pragma unroll
+        for (int mt = 0; mt < M; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) dmma(acc[2 * mt + nt], af[mt].y, bf[nt].y);
+    }
+}
+
+// Full diagonal tile, warp W: sub-tile row W with columns 0..W  -> acc[0..W],
+//                             sub-tile row 7-W with columns 0..7-W -> acc[W+1 .. 8].
+// Ap = stage A + lr * LDS_ROW + 2 lk;  Bp = stage B + lr * LDS_ROW + 2 lk.
+template <int W>
+__device__ __forceinline__ void ktile_diag(double (&acc)[16][2], const double* __restrict__ Ap,
+                                           const double* __restrict__ Bp) {
+    constexpr int RA = W, RB = 7 - W, NB = 8 - W;
+#pragma unroll
+    for (int j = 0; j < BK / 8; ++j) {
+        double2 bf[NB];
+        const double2 aa = *reinterpret_cast<const double2*>(Ap + RA * 8 * LDS_ROW + j * 8);
+        const double2 ab = *reinterpret_cast<const double2*>(Ap + RB * 8 * LDS_ROW + j * 8);
+#pragma unroll
+        for (int c = 0; c < NB; ++c) bf[c] = *reinterpret_cast<const double2*>(Bp + c * 8 * LDS_ROW + j * 8);
+#pragma unroll
+        for (int c = 0; c <= W; ++c) dmma(acc[c], aa.x, bf[c].x);
+#pragma unroll
+        for (int c = 0; c < NB; ++c) dmma(acc[W + 1 + c], ab.x, bf[c].x);
+#pragma unroll
+        for (int c = 0; c <= W; ++c) dmma(acc[c], aa.y, bf[c].y);
+#pragma unroll
+        for (int c = 0; c < NB; ++c) dmma(acc[W + 1 + c], ab.y, bf[c].y);
     }
 }
 
 struct NsArgs {
     const TileDesc* tiles;
-    const int64_t* ws_off;
-    const int32_t* ld;
-    const int32_t* dim;
-    const int32_t* tile_first;
-    const int32_t* tile_count;
     const unsigned long long* gersh;
     double* buf0;
     double* buf1;
@@ -90,50 +120,18 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
     extern __shared__ __align__(16) double smem[];
     __shared__ double s_red[4];
     __shared__ int s_stop;
-    const TileDesc td = a.tiles[blockIdx.x];
-    const int g = td.grp;
+    const int4* tdp = reinterpret_cast<const int4*>(a.tiles + blockIdx.x);
+    const int4 t0 = __ldg(tdp), t1 = __ldg(tdp + 1);
+    const int64_t ws_off = ((int64_t)(unsigned)t0.x) | ((int64_t)t0.y << 32);
+    const int g = t0.z, ld = t0.w, n = t1.x, tij = t1.y, tile_first = t1.z, tile_count = t1.w;
     if (a.done_iter[g] >= 0) return;
-    const int ti = td.tij & 0xffff, tj = td.tij >> 16;
-    const int ld = a.ld[g], n = a.dim[g];
+    const int ti = tij & 0xffff, tj = tij >> 16;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int k = a.k;
-    double s = __longlong_as_double((long long)a.gersh[g]);
-    if (!(s > 0.0)) s = 1.0;
 
-    if (MODE == 1) {
-        // residual of X_k from the partials MODE 0 just wrote; fixed summation order
-        if (wid == 0) {
-            const int t0 = a.tile_first[g], tc = a.tile_count[g];
-            double r2 = 0.0;
-            for (int t = lane; t < tc; t += 32) r2 += a.partials[t0 + t];
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
-            if (lane == 0) {
-                const double r = sqrt(r2 / (double)(n > 0 ? n : 1));
-                const double prev = k > 0 ? a.res[(size_t)((k - 1) & 1) * a.ngroups + g] : 1e300;
-                const bool conv = r < a.eps;
-                const bool stag = (k > 0) && (r >= prev) && (r < 1e-6);
-                const bool stop = conv || stag || a.decide_only || !(r == r);
-                s_stop = stop ? 1 : 0;
-                if (blockIdx.x == (unsigned)t0) {  // one CTA per submatrix records the decision
-                    a.res[(size_t)(k & 1) * a.ngroups + g] = r;
-                    if (stop) {
-                        a.done_iter[g] = k;
-                        a.flag[g] = conv ? 0 : 1;
-                        if (!conv) a.res[(size_t)((k + 1) & 1) * a.ngroups + g] = r;
-                    } else {
-                        atomicAdd(a.counters + k, 1);
-                    }
-                }
-            }
-        }
-        __syncthreads();
-        if (s_stop) return;
-    }
-
-    const double* X = ((k & 1) ? a.buf1 : a.buf0) + a.ws_off[g];
+    const double* X = ((k & 1) ? a.buf1 : a.buf0) + ws_off;
     const double* Aop = X;
-    const double* Bop = (MODE == 0) ? X : (a.bufY + a.ws_off[g]);
+    const double* Bop = (MODE == 0) ? X : (a.bufY + ws_off);
     const int row0 = ti * BM, col0 = tj * BN;
     const bool diag = (ti == tj);
 
@@ -163,32 +161,57 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
         }
     };
 
-    const int wm = wid >> 1, wn = wid & 1;
-    // Work of this warp: number of valid 8-row sub-tile rows (the padded matrix ends inside the last
-    // tile) and, on diagonal tiles, only the sub-tiles that touch the lower triangle.  Off-diagonal
-    // tiles always have all 64 columns (tj < ti <= last).  Warp-uniform: dispatched once per k-tile.
-    const int rows_left = ld - (row0 + wm * 32), cols_left = ld - (col0 + wn * 32);
-    int mt_cnt = rows_left <= 0 ? 0 : (rows_left >= 32 ? 4 : rows_left >> 3);
-    int nt_cnt = cols_left <= 0 ? 0 : (cols_left >= 32 ? 4 : cols_left >> 3);
-    bool tri = false;
-    if (diag) {
-        if (wm < wn) mt_cnt = 0;          // entirely above the diagonal
-        else if (wm == wn) tri = true;    // mt_cnt == nt_cnt here
-    }
-    if (nt_cnt == 0) mt_cnt = 0;
-    const int variant = mt_cnt == 0 ? 0 : (tri ? 4 + mt_cnt : mt_cnt);  // 1..4 FULL<MT,nt>, 5..8 TRI<S>
-
-    double acc[4][4][2];
-#pragma unroll
-    for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
-
+    // start filling the pipeline before anything else (MODE 1 decides convergence meanwhile)
 #pragma unroll
     for (int st = 0; st < STAGES - 1; ++st) {
         if (st < KT) load_stage(st, st);
         cp_async_commit();
     }
+
+    if (MODE == 1) {
+        // residual of X_k from the partials MODE 0 just wrote; fixed summation order
+        if (wid == 0) {
+            double r2 = 0.0;
+            for (int t = lane; t < tile_count; t += 32) r2 += a.partials[tile_first + t];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+            if (lane == 0) {
+                const double r = sqrt(r2 / (double)(n > 0 ? n : 1));
+                const double prev = k > 0 ? a.res[(size_t)((k - 1) & 1) * a.ngroups + g] : 1e300;
+                const bool conv = r < a.eps;
+                const bool stag = (k > 0) && (r >= prev) && (r < 1e-6);
+                const bool stop = conv || stag || a.decide_only || !(r == r);
+                s_stop = stop ? 1 : 0;
+                if (blockIdx.x == (unsigned)tile_first) {  // one CTA per submatrix records the decision
+                    a.res[(size_t)(k & 1) * a.ngroups + g] = r;
+                    if (stop) {
+                        a.done_iter[g] = k;
+                        a.flag[g] = conv ? 0 : 1;
+                    } else {
+                        atomicAdd(a.counters + k, 1);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        if (s_stop) {
+            cp_async_wait<0>();
+            return;
+        }
+    }
+
+    // Warp-uniform work selection (see the file header).
+    const int s_rows = min(8, (ld - row0) >> 3);  // valid 8-row sub-tile rows of this tile, 1..8
+    const bool full_diag = diag && s_rows == 8;
+    int variant;  // 0 idle, 1..8 rect<M>, 9..12 diag<W>
+    if (full_diag) variant = 9 + wid;
+    else if (diag) variant = (2 * wid < s_rows) ? s_rows : 0;  // columns past the matrix: nothing to do
+    else variant = s_rows;
+
+    double acc[16][2];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) acc[e][0] = acc[e][1] = 0.0;
+
     const int lr = lane >> 2, lk = lane & 3;
     for (int kt = 0; kt < KT; ++kt) {
         cp_async_wait<STAGES - 2>();
@@ -199,63 +222,71 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
             cp_async_commit();
         }
         const int stage = kt % STAGES;
-        const double* Aw = As + ((size_t)stage * BM + wm * 32 + lr) * LDS_ROW + 2 * lk;
-        const double* Bw = Bs + ((size_t)stage * BN + wn * 32 + lr) * LDS_ROW + 2 * lk;
-        if (nt_cnt == 4 || tri) {
-            switch (variant) {
-                case 4: ktile_mma<4, 4, false>(acc, Aw, Bw); break;
-                case 3: ktile_mma<3, 4, false>(acc, Aw, Bw); break;
-                case 2: ktile_mma<2, 4, false>(acc, Aw, Bw); break;
-                case 1: ktile_mma<1, 4, false>(acc, Aw, Bw); break;
-                case 8: ktile_mma<4, 4, true>(acc, Aw, Bw); break;
-                case 7: ktile_mma<3, 3, true>(acc, Aw, Bw); break;
-                case 6: ktile_mma<2, 2, true>(acc, Aw, Bw); break;
-                case 5: ktile_mma<1, 1, true>(acc, Aw, Bw); break;
-                default: break;
-            }
-        } else if (variant) {
-            // cannot happen for lower-triangular tiles (see above); kept for safety: full 4 x 4 on
-            // zero-filled operands is still correct
-            ktile_mma<4, 4, false>(acc, Aw, Bw);
+        const double* Ap = As + ((size_t)stage * BM + lr) * LDS_ROW + 2 * lk;
+        const double* Bp0 = Bs + ((size_t)stage * BN + lr) * LDS_ROW + 2 * lk;
+        const double* Bp = Bp0 + (size_t)wid * 16 * LDS_ROW;
+        switch (variant) {
+            case 8: ktile_rect<8>(acc, Ap, Bp); break;
+            case 7: ktile_rect<7>(acc, Ap, Bp); break;
+            case 6: ktile_rect<6>(acc, Ap, Bp); break;
+            case 5: ktile_rect<5>(acc, Ap, Bp); break;
+            case 4: ktile_rect<4>(acc, Ap, Bp); break;
+            case 3: ktile_rect<3>(acc, Ap, Bp); break;
+            case 2: ktile_rect<2>(acc, Ap, Bp); break;
+            case 1: ktile_rect<1>(acc, Ap, Bp); break;
+            case 9: ktile_diag<0>(acc, Ap, Bp0); break;
+            case 10: ktile_diag<1>(acc, Ap, Bp0); break;
+            case 11: ktile_diag<2>(acc, Ap, Bp0); break;
+            case 12: ktile_diag<3>(acc, Ap, Bp0); break;
+            default: break;
         }
     }
     cp_async_wait<0>();
 
     // ------------------------------------------------------------------ epilogue
+    double s = __longlong_as_double((long long)a.gersh[g]);
+    if (!(s > 0.0)) s = 1.0;
     double alpha, ca, cb;
     if (k == 0) { alpha = 1.0 / (s * s); ca = 1.5 / s; cb = -0.5 / s; }
     else { alpha = 1.0; ca = 1.5; cb = -0.5; }
-    double* Out = (MODE == 0) ? (a.bufY + a.ws_off[g]) : (((k & 1) ? a.buf0 : a.buf1) + a.ws_off[g]);
+    double* Out = (MODE == 0) ? (a.bufY + ws_off) : (((k & 1) ? a.buf0 : a.buf1) + ws_off);
     double part = 0.0;
 #pragma unroll
-    for (int mt = 0; mt < 4; ++mt)
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) {
-            if (mt >= mt_cnt || nt >= nt_cnt || (tri && nt > mt)) continue;
-            const int r = row0 + wm * 32 + mt * 8 + lr;
-            const int c = col0 + wn * 32 + nt * 8 + 2 * lk;
-            if (r >= ld || c >= ld) continue;  // ld is a multiple of 8: whole sub-tile in or out
-            double v0 = acc[mt][nt][0], v1 = acc[mt][nt][1];
-            if (MODE == 0) {
-                v0 *= alpha; v1 *= alpha;
-                if (r < n) {  // residual over the n x n part; strictly-lower elements count twice
-                    if (c < n && c <= r) { double d = v0 - (c == r ? 1.0 : 0.0); part += (c == r ? 1.0 : 2.0) * d * d; }
-                    if (c + 1 < n && c + 1 <= r) { double d = v1 - (c + 1 == r ? 1.0 : 0.0); part += (c + 1 == r ? 1.0 : 2.0) * d * d; }
-                }
-            } else {
-                const double2 x = *reinterpret_cast<const double2*>(X + (size_t)r * ld + c);
-                v0 = ca * x.x + cb * v0;
-                v1 = ca * x.y + cb * v1;
-            }
-            if (!diag) {
-                *reinterpret_cast<double2*>(Out + (size_t)r * ld + c) = make_double2(v0, v1);
-                Out[(size_t)c * ld + r] = v0;
-                Out[(size_t)(c + 1) * ld + r] = v1;
-            } else {  // diagonal tile: keep the lower triangle, mirror it
-                if (c <= r) { Out[(size_t)r * ld + c] = v0; if (c != r) Out[(size_t)c * ld + r] = v0; }
-                if (c + 1 <= r) { Out[(size_t)r * ld + c + 1] = v1; if (c + 1 != r) Out[(size_t)(c + 1) * ld + r] = v1; }
-            }
+    for (int e = 0; e < 16; ++e) {
+        int sr, sc;  // sub-tile row / column inside the CTA tile
+        bool valid;
+        if (full_diag) {
+            valid = e < 9;
+            if (e <= wid) { sr = wid; sc = e; } else { sr = 7 - wid; sc = e - wid - 1; }
+        } else {
+            sr = e >> 1; sc = 2 * wid + (e & 1);
+            valid = variant != 0 && sr < s_rows;
         }
+        if (!valid) continue;
+        const int r = row0 + sr * 8 + lr;
+        const int c = col0 + sc * 8 + 2 * lk;
+        if (r >= ld || c >= ld) continue;  // ld is a multiple of 8: whole sub-tile in or out
+        double v0 = acc[e][0], v1 = acc[e][1];
+        if (MODE == 0) {
+            v0 *= alpha; v1 *= alpha;
+            if (r < n) {  // residual over the n x n part; strictly-lower elements count twice
+                if (c < n && c <= r) { double d = v0 - (c == r ? 1.0 : 0.0); part += (c == r ? 1.0 : 2.0) * d * d; }
+                if (c + 1 < n && c + 1 <= r) { double d = v1 - (c + 1 == r ? 1.0 : 0.0); part += (c + 1 == r ? 1.0 : 2.0) * d * d; }
+            }
+        } else {
+            const double2 x = *reinterpret_cast<const double2*>(X + (size_t)r * ld + c);
+            v0 = ca * x.x + cb * v0;
+            v1 = ca * x.y + cb * v1;
+        }
+        if (!diag) {
+            *reinterpret_cast<double2*>(Out + (size_t)r * ld + c) = make_double2(v0, v1);
+            Out[(size_t)c * ld + r] = v0;
+            Out[(size_t)(c + 1) * ld + r] = v1;
+        } else {  // diagonal tile: keep the lower triangle, mirror it
+            if (c <= r) { Out[(size_t)r * ld + c] = v0; if (c != r) Out[(size_t)c * ld + r] = v0; }
+            if (c + 1 <= r) { Out[(size_t)r * ld + c + 1] = v1; if (c + 1 != r) Out[(size_t)(c + 1) * ld + r] = v1; }
+        }
+    }
     if (MODE == 0) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
@@ -275,8 +306,7 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
         attr_set = true;
     }
     NsArgs a;
-    a.tiles = p->d_tiles; a.ws_off = p->d_ws_off; a.ld = p->d_ld; a.dim = p->d_sub_dim;
-    a.tile_first = p->d_tile_first; a.tile_count = p->d_tile_count; a.gersh = p->d_gersh;
+    a.tiles = p->d_tiles; a.gersh = p->d_gersh;
     a.buf0 = buf0; a.buf1 = buf1; a.bufY = bufY; a.partials = p->d_partials;
     a.done_iter = p->d_done_iter; a.flag = p->d_flag; a.res = p->d_res; a.counters = p->d_counters;
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;

@@ -260,10 +260,17 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
         if (p->h_ld[i] != last_ld) { ++nbuckets; last_ld = p->h_ld[i]; }
         int nt = (p->h_ld[i] + TILE - 1) / TILE;
         p->h_tile_first[i] = (int32_t)tiles.size();
+        const int32_t first = (int32_t)tiles.size(), count = nt * (nt + 1) / 2;
+        auto push = [&](int ti, int tj) {
+            TileDesc t;
+            t.ws_off = p->h_ws_off[i]; t.grp = i; t.ld = p->h_ld[i]; t.n = p->h_sub_dim[i];
+            t.tij = ti | (tj << 16); t.tile_first = first; t.tile_count = count;
+            tiles.push_back(t);
+        };
         // off-diagonal (full) tiles first, diagonal (half-empty) tiles last
         for (int ti = 0; ti < nt; ++ti)
-            for (int tj = 0; tj < ti; ++tj) tiles.push_back({i, ti | (tj << 16)});
-        for (int ti = 0; ti < nt; ++ti) tiles.push_back({i, ti | (ti << 16)});
+            for (int tj = 0; tj < ti; ++tj) push(ti, tj);
+        for (int ti = 0; ti < nt; ++ti) push(ti, ti);
         p->h_tile_count[i] = (int32_t)tiles.size() - p->h_tile_first[i];
     }
     p->n_tiles = (int64_t)tiles.size();
