@@ -76,7 +76,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_grp_cols, p->d_col_grp, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off, p->d_sub_dim,
                     p->d_gen_pos, p->d_gen_off, p->d_blk_loc, p->d_gen_width, p->d_ws_off, p->d_ld, p->d_tiles,
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
-                    p->d_partials, p->d_counters, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
+                    p->d_partials, p->d_counters, p->d_sched, p->d_tile_done, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out};
     for (void* q : ptrs)
         if (q) cudaFree(q);
@@ -132,6 +132,8 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_gersh, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_partials, (size_t)p->n_tiles * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_counters, (size_t)(p->opt.max_iter + 2) * 4);
+    if (e == cudaSuccess) e = A((void**)&p->d_sched, (size_t)(p->opt.max_iter + 2) * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_tile_done, (size_t)ng * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_ne_part, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_scalars, 8 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_red, 4096 * 8);
@@ -207,6 +209,8 @@ sm_status_t reset_state(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMemsetAsync(p->d_done_iter, 0xff, (size_t)ng * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_flag, 0, (size_t)ng * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_counters, 0, (size_t)(p->opt.max_iter + 2) * 4, st));
+    SM_CUDA(cudaMemsetAsync(p->d_sched, 0, (size_t)(p->opt.max_iter + 2) * 8, st));
+    SM_CUDA(cudaMemsetAsync(p->d_tile_done, 0, (size_t)ng * 4, st));
     p->cur_k = 0;
     return SM_OK;
 }
@@ -224,7 +228,7 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
     for (; k < k_end && k <= max_iter; ++k) {
         sm_status_t s = launch_ns_pair(p, k, eps, k == max_iter ? 1 : 0, b.b0, b.b1, b.y, st);
         if (s) return s;
-        (*launched) += 2;
+        (*launched) += (k == max_iter) ? 1 : 2;
         if (pending >= 0) {
             SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
             if (p->h_pinned[pending] == 0) { *all_done = 1; p->cur_k = pending; return SM_OK; }

@@ -25,6 +25,19 @@ struct __align__(16) TileDesc {
     int32_t tile_count;  // number of tiles of this submatrix
 };
 
+// Workspace layout of one symmetric ld x ld matrix ("k8-panel" layout): rows are grouped in
+// row-tiles of 64 (the last one holds rows_t = ld - 64 t rows); inside a row-tile the data is a
+// sequence of panels, panel kp = the 8 consecutive columns 8 kp .. 8 kp + 7 of all rows_t rows,
+// row-major (64 bytes per row).  The operand slice (64 rows x 16 k) that one pipeline stage of the
+// Newton-Schulz GEMM needs is therefore ONE contiguous block of rows_t * 128 bytes -- a single
+// cp.async.bulk -- and its dense 64-byte rows are bank-conflict-free for the 16-byte fragment loads.
+// ld is a multiple of 8, the matrix occupies exactly ld * ld doubles.
+__host__ __device__ __forceinline__ size_t panel_off(int r, int c, int ld) {
+    const int t0 = r & ~63;
+    const int rows_t = (ld - t0) < 64 ? (ld - t0) : 64;
+    return (size_t)t0 * ld + (size_t)(c >> 3) * rows_t * 8 + (size_t)((r & 63) * 8 + (c & 7));
+}
+
 void set_cuda_error(cudaError_t e, const char* where);
 
 #define SM_CUDA(call)                                        \
@@ -72,6 +85,8 @@ struct sm_plan {
     unsigned long long* d_gersh = nullptr; // [ngroups] bits of the Gershgorin bound (atomicMax)
     double* d_partials = nullptr;          // [n_tiles] per-tile residual partial sums
     int32_t* d_counters = nullptr;         // [max_iter+2] still-active submatrices after iteration k
+    int32_t* d_sched = nullptr;            // [2*(max_iter+2)] work counters of the persistent GEMM launches
+    int32_t* d_tile_done = nullptr;        // [ngroups] finished tiles of a submatrix in the current launch
     double* d_ne_part = nullptr;           // [ngroups] per-group electron-count partials
     double* d_scalars = nullptr;           // [8] n_elec, tr D, tr DK, gersh lo/hi
     double* d_red = nullptr;               // [2*4096] reduction scratch

@@ -69,7 +69,7 @@ __global__ void k_gather(const int32_t* __restrict__ blk_size, const int64_t* __
         __syncwarp();
         const int coff = So[tc];
         for (int q = 0; q < bc; ++q) {
-            double* col = Xg + (size_t)(coff + q) * ld;
+            const int xrow = coff + q;  // symmetric: dense column q of a_i is stored as row q
             double asum = 0.0;
             for (int p = 2 * lane; p < ld; p += 64) {
                 double v[2];
@@ -90,7 +90,7 @@ __global__ void k_gather(const int32_t* __restrict__ blk_size, const int64_t* __
                     v[u] = x;
                     asum += fabs(x);
                 }
-                *reinterpret_cast<double2*>(col + p) = make_double2(v[0], v[1]);
+                *reinterpret_cast<double2*>(Xg + panel_off(xrow, p, ld)) = make_double2(v[0], v[1]);
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) asum += __shfl_xor_sync(0xffffffffu, asum, o);
@@ -101,8 +101,8 @@ __global__ void k_gather(const int32_t* __restrict__ blk_size, const int64_t* __
     // zero padding columns n..ld-1 (last chunk only)
     if ((int)blockIdx.y == nchunks - 1) {
         for (int qq = n + wid; qq < ld; qq += nw) {
-            double* col = Xg + (size_t)qq * ld;
-            for (int p = 2 * lane; p < ld; p += 64) *reinterpret_cast<double2*>(col + p) = make_double2(0.0, 0.0);
+            for (int p = 2 * lane; p < ld; p += 64)
+                *reinterpret_cast<double2*>(Xg + panel_off(qq, p, ld)) = make_double2(0.0, 0.0);
         }
     }
     if (lane == 0 && cmax > 0.0) atomicMax(gersh + g, (unsigned long long)__double_as_longlong(cmax));
@@ -167,7 +167,7 @@ __global__ void k_scatter(const int32_t* __restrict__ blk_size, const int64_t* _
         const int br = blk_size[r];
         const int w = (int)(e - val_off[b]);
         const int q = w / br, el = w - q * br;
-        double x = Xg[(size_t)(go + q) * ld + blk_loc[b] + el];
+        double x = Xg[panel_off(go + q, blk_loc[b] + el, ld)];
         double d;
         if (as_identity) d = x;
         else d = 0.5 * (((r == c && q == el) ? 1.0 : 0.0) - xs * x);
@@ -228,8 +228,8 @@ __global__ void k_nelec_part(int ngroups, const int32_t* __restrict__ grp_ptr, c
         int c = grp_cols[gc];
         int o = gen_off[c], b = blk_size[c];
         for (int e = lane; e < b; e += 32) {
-            size_t d = (size_t)(o + e);
-            a += 0.5 * (1.0 - xs * Xg[d * ld + d]);
+            const int d = o + e;
+            a += 0.5 * (1.0 - xs * Xg[panel_off(d, d, ld)]);
         }
     }
 #pragma unroll
