@@ -36,7 +36,7 @@ static sm_status_t validate(int32_t nb, const int32_t* bs, const int64_t* colptr
     if (nb == 0) return ng == 0 ? SM_OK : SM_ERR_STRUCTURE;
     if (colptr[0] != 0) return SM_ERR_STRUCTURE;
     for (int c = 0; c < nb; ++c) {
-        if (bs[c] <= 0) return SM_ERR_INVALID_ARG;
+        if (bs[c] <= 0 || bs[c] > 4095) return SM_ERR_INVALID_ARG;  // 12-bit block heights (scatter records)
         if (colptr[c + 1] < colptr[c]) return SM_ERR_STRUCTURE;
         bool diag = false;
         for (int64_t p = colptr[c]; p < colptr[c + 1]; ++p) {
@@ -74,7 +74,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
     if (!p) return;
     void* ptrs[] = {p->d_blk_size, p->d_blk_off, p->d_rowidx, p->d_colptr, p->d_val_off, p->d_grp_ptr,
                     p->d_grp_cols, p->d_col_grp, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off, p->d_sub_dim,
-                    p->d_gen_pos, p->d_gen_off, p->d_blk_loc, p->d_gen_width, p->d_ws_off, p->d_ld, p->d_tiles,
+                    p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_gen_width, p->d_ws_off, p->d_ld, p->d_tiles,
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
                     p->d_partials, p->d_counters, p->d_sched, p->d_tile_done, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out};
@@ -148,14 +148,21 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
         sm_plan_destroy(p);
         return e == cudaErrorMemoryAllocation ? SM_ERR_ALLOC : SM_ERR_CUDA;
     }
-    // gather launch shape: shared memory = row map + one source table per warp
+    // gather launch shape: per-warp source tables + row records + hash table + S_i / offsets
     {
-        const size_t rowmap = (((size_t)(p->info.dim_max + LD_ALIGN) * 4 + 15) / 16) * 16;
+        const int msb = (std::max(p->max_sub_blocks, 1) + 1) & ~1;
+        const int max_ld = p->info.dim_max + LD_ALIGN;
+        int hs = 32, shift = 27;
+        while (hs < 2 * msb) { hs <<= 1; --shift; }
+        auto bytes = [&](int warps) {
+            return (size_t)warps * msb * 8 + (size_t)max_ld * 8 + (size_t)hs * 8 + (size_t)(2 * msb + 2) * 4;
+        };
         int warps = 8;
         const size_t budget = 200 * 1024;
-        while (warps > 1 && rowmap + (size_t)warps * p->max_sub_blocks * 8 > budget) warps >>= 1;
-        p->gather_warps = warps;
-        p->gather_smem = rowmap + (size_t)warps * std::max(p->max_sub_blocks, 1) * 8;
+        while (warps > 1 && bytes(warps) > budget) warps >>= 1;
+        p->gather_warps = warps; p->gather_msb = msb; p->gather_max_ld = max_ld;
+        p->gather_hash_size = hs; p->gather_hash_shift = shift;
+        p->gather_smem = bytes(warps);
         if (p->gather_smem > budget) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }
     }
     *plan = p;

@@ -70,7 +70,8 @@ struct sm_plan {
     int64_t* d_sub_ptr = nullptr;
     int32_t *d_sub_blocks = nullptr, *d_sub_off = nullptr, *d_sub_dim = nullptr, *d_gen_pos = nullptr;
     int32_t *d_gen_off = nullptr;  // [nb]  element offset of column c inside its group's submatrix
-    int32_t *d_blk_loc = nullptr;  // [nnzb] element row offset of block (r,c) inside c's group's submatrix
+    uint32_t *d_blk_pack = nullptr;// [nnzb] block (r,c): element row offset inside c's group's submatrix (low 20
+                                   //        bits) | height blk_size[r] (high 12 bits)
     int32_t *d_gen_width = nullptr;// [ngroups] generating basis functions per group
     // --- device: workspace geometry and tiles
     int64_t* d_ws_off = nullptr;   // [ngroups] offset (doubles) of submatrix i in each buffer
@@ -100,7 +101,7 @@ struct sm_plan {
     int64_t launches = 0;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_iter[2] = {nullptr, nullptr};
-    int gather_warps = 8;
+    int gather_warps = 8, gather_msb = 0, gather_max_ld = 0, gather_hash_size = 32, gather_hash_shift = 27;
     size_t gather_smem = 0;
     int num_sms = 148;
 };

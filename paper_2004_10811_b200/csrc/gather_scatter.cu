@@ -17,84 +17,140 @@ __device__ __forceinline__ int find_sorted64(const int32_t* __restrict__ a, int 
 
 // ---------------------------------------------------------------------------------------------
 // Gather (PAPER.md L125 step 1; L187 "submatrix assembly becomes a purely local operation").
-// grid = (ngroups, chunks of CB column blocks); one warp assembles one block column of a_i at a
-// time: (1) lanes look up, for every member r of S_i, the stored block (r,c) of column c
-// (binary search in the CSC column; -1 if absent -> zero fill, reading A4), (2) for each dense
-// column the lanes sweep the ld rows two at a time and store 16 bytes each (coalesced), taking
-// the values from the stored blocks, subtracting mu on the diagonal (Eq.(16)) and zero-padding
-// rows/columns n..ld-1.  The column abs-sums give the Gershgorin bound s_i = max_q sum_p |a_pq|
-// (symmetric: column sums = row sums), combined by atomicMax on the bits of a non-negative double.
+// grid = (ngroups, chunks of GATHER_CB column blocks).  Per CTA, once: S_i and its element
+// offsets go to shared memory together with a hash table block-row -> member index and a
+// per-dense-row record (member, row inside the member, member height).  Then one warp assembles
+// one block column c = S_i[tc] of a_i at a time:
+//  (1) the lanes walk the stored blocks (r,c) of column c (coalesced reads of rowidx / val_off),
+//      look r up in the hash table and note the value offset of the block for member r;
+//      members without a stored block stay -1 -> zero fill (reading A4);
+//  (2) for up to four dense columns of the block column at once the lanes sweep the ld rows two
+//      at a time and store 16 bytes each, taking the values from the stored blocks, subtracting
+//      mu on the diagonal (Eq.(16)) and zero-padding rows/columns n..ld-1.
+// The column abs-sums give the Gershgorin bound s_i = max_q sum_p |a_pq| (symmetric: column sums
+// = row sums), combined by atomicMax on the bits of a non-negative double.
 // ---------------------------------------------------------------------------------------------
-constexpr int GATHER_CB = 8;  // column blocks per CTA
+constexpr int GATHER_CB = 16;  // column blocks per CTA
 
-__global__ void k_gather(const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
-                         const int32_t* __restrict__ rowidx, const int64_t* __restrict__ val_off,
-                         const double* __restrict__ vals, const int64_t* __restrict__ sub_ptr,
-                         const int32_t* __restrict__ sub_blocks, const int32_t* __restrict__ sub_off,
-                         const int32_t* __restrict__ sub_dim, const int32_t* __restrict__ ldv,
-                         const int64_t* __restrict__ ws_off, double mu, double* __restrict__ X,
-                         unsigned long long* __restrict__ gersh, int max_sub_blocks, int max_ld) {
-    extern __shared__ unsigned char smem_raw[];
+__device__ __forceinline__ unsigned gather_hash(int key, int shift) {
+    return ((unsigned)key * 2654435761u) >> shift;
+}
+
+__global__ void __launch_bounds__(256)
+k_gather(const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx,
+         const int64_t* __restrict__ val_off, const double* __restrict__ vals,
+         const int64_t* __restrict__ sub_ptr, const int32_t* __restrict__ sub_blocks,
+         const int32_t* __restrict__ sub_off, const int32_t* __restrict__ sub_dim,
+         const int32_t* __restrict__ ldv, const int64_t* __restrict__ ws_off, double mu,
+         double* __restrict__ X, unsigned long long* __restrict__ gersh, int max_sub_blocks, int max_ld,
+         int hash_size, int hash_shift) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
     const int g = blockIdx.x;
     const int m = (int)(sub_ptr[g + 1] - sub_ptr[g]);
     const int cb0 = blockIdx.y * GATHER_CB;
-    const int n = sub_dim[g], ld = ldv[g];
     // column chunks past |S_i| only have padding columns to write (handled by the last chunk)
     const int nchunks = (m + GATHER_CB - 1) / GATHER_CB;
     if ((int)blockIdx.y >= nchunks) return;
-    const int32_t* S = sub_blocks + sub_ptr[g];
-    const int32_t* So = sub_off + sub_ptr[g];
-    int32_t* row2blk = reinterpret_cast<int32_t*>(smem_raw);                       // [max_ld]
-    int64_t* src_all = reinterpret_cast<int64_t*>(smem_raw + (((size_t)max_ld * 4 + 15) / 16) * 16);
+    const int n = sub_dim[g], ld = ldv[g];
+    // shared-memory carve-up (all 8-byte aligned)
+    int64_t* src_all = reinterpret_cast<int64_t*>(smem_raw);                  // [warps][max_sub_blocks]
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    int64_t* src = src_all + (size_t)wid * max_sub_blocks;                         // [m] per warp
-    // row -> member map
+    int2* rinfo = reinterpret_cast<int2*>(src_all + (size_t)nw * max_sub_blocks);  // [max_ld]
+    int32_t* hk = reinterpret_cast<int32_t*>(rinfo + max_ld);                 // [hash_size] keys
+    int32_t* hv = hk + hash_size;                                             // [hash_size] member index
+    int32_t* S = hv + hash_size;                                              // [max_sub_blocks]
+    int32_t* So = S + max_sub_blocks;                                         // [max_sub_blocks + 1]
+    for (int h = threadIdx.x; h < hash_size; h += blockDim.x) hk[h] = -1;
     for (int t = threadIdx.x; t < m; t += blockDim.x) {
-        int o = So[t], b = blk_size[S[t]];
-        for (int e = 0; e < b; ++e) row2blk[o + e] = t;
+        S[t] = sub_blocks[sub_ptr[g] + t];
+        So[t] = sub_off[sub_ptr[g] + t];
     }
+    if (threadIdx.x == 0) So[m] = n;
     __syncthreads();
+    const unsigned hmask = (unsigned)hash_size - 1u;
+    for (int t = threadIdx.x; t < m; t += blockDim.x) {
+        const int key = S[t];
+        unsigned h = gather_hash(key, hash_shift);
+        while (atomicCAS(&hk[h], -1, key) != -1) h = (h + 1) & hmask;
+        hv[h] = t;
+        const int o = So[t], b = So[t + 1] - o;
+        for (int e = 0; e < b; ++e) rinfo[o + e] = make_int2(t, e | (b << 16));
+    }
+    for (int p = n + threadIdx.x; p < ld; p += blockDim.x) rinfo[p] = make_int2(-1, 0);
+    __syncthreads();
+    int64_t* src = src_all + (size_t)wid * max_sub_blocks;                    // [m] per warp
     double* Xg = X + ws_off[g];
     double cmax = 0.0;
     const int cb1 = min(cb0 + GATHER_CB, m);
     for (int tc = cb0 + wid; tc < cb1; tc += nw) {
         const int c = S[tc];
-        const int bc = blk_size[c];
+        const int coff = So[tc], bc = So[tc + 1] - coff;
+        for (int t = lane; t < m; t += 32) src[t] = -1;
+        __syncwarp();
         const int64_t p0 = colptr[c];
         const int clen = (int)(colptr[c + 1] - p0);
-        for (int t = lane; t < m; t += 32) {
-            int f = find_sorted64(rowidx + p0, clen, S[t]);
-            src[t] = f >= 0 ? val_off[p0 + f] : (int64_t)-1;
+        for (int j = lane; j < clen; j += 32) {
+            const int r = __ldg(rowidx + p0 + j);
+            unsigned h = gather_hash(r, hash_shift);
+            for (;;) {
+                const int k = hk[h];
+                if (k == r) { src[hv[h]] = __ldg(val_off + p0 + j); break; }
+                if (k < 0) break;
+                h = (h + 1) & hmask;
+            }
         }
         __syncwarp();
-        const int coff = So[tc];
-        for (int q = 0; q < bc; ++q) {
-            const int xrow = coff + q;  // symmetric: dense column q of a_i is stored as row q
-            double asum = 0.0;
+        for (int q0 = 0; q0 < bc; q0 += 4) {
+            const int nq = min(4, bc - q0);
+            double asum[4] = {0.0, 0.0, 0.0, 0.0};
+            // dense column q of a_i is stored as row coff+q of the symmetric X (k8-panel layout)
+            size_t rbase[4];
+            int rstride[4];
+#pragma unroll
+            for (int qq = 0; qq < 4; ++qq) {
+                const int xrow = coff + q0 + (qq < nq ? qq : 0);
+                const int t0 = xrow & ~63;
+                const int rows_t = min(64, ld - t0);
+                rbase[qq] = (size_t)t0 * ld + (size_t)(xrow & 63) * 8;
+                rstride[qq] = rows_t * 8;
+            }
+            const int dq = coff + q0;  // diagonal position of dense column q0
             for (int p = 2 * lane; p < ld; p += 64) {
-                double v[2];
+                double v[4][2];
+#pragma unroll
+                for (int qq = 0; qq < 4; ++qq) v[qq][0] = v[qq][1] = 0.0;
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
-                    int pp = p + u;
-                    double x = 0.0;
-                    if (pp < n) {
-                        int t = row2blk[pp];
-                        int64_t s0 = src[t];
+                    const int2 ri = rinfo[p + u];
+                    if (ri.x >= 0) {
+                        const int64_t s0 = src[ri.x];
                         if (s0 >= 0) {
-                            int o = So[t];
-                            int br = (t + 1 < m ? So[t + 1] : n) - o;
-                            x = __ldg(vals + s0 + (int64_t)q * br + (pp - o));
+                            const int br = ri.y >> 16;
+                            const double* vp = vals + s0 + (int64_t)q0 * br + (ri.y & 0xffff);
+#pragma unroll
+                            for (int qq = 0; qq < 4; ++qq)
+                                if (qq < nq) v[qq][u] = __ldg(vp + qq * br);
                         }
-                        if (pp == coff + q) x -= mu;
                     }
-                    v[u] = x;
-                    asum += fabs(x);
                 }
-                *reinterpret_cast<double2*>(Xg + panel_off(xrow, p, ld)) = make_double2(v[0], v[1]);
+#pragma unroll
+                for (int qq = 0; qq < 4; ++qq) {
+                    if (qq < nq) {
+                        if (dq + qq == p) v[qq][0] -= mu;
+                        else if (dq + qq == p + 1) v[qq][1] -= mu;
+                        asum[qq] += fabs(v[qq][0]) + fabs(v[qq][1]);
+                        *reinterpret_cast<double2*>(Xg + rbase[qq] + (size_t)(p >> 3) * rstride[qq] + (p & 7)) =
+                            make_double2(v[qq][0], v[qq][1]);
+                    }
+                }
             }
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) asum += __shfl_xor_sync(0xffffffffu, asum, o);
-            cmax = fmax(cmax, asum);
+            for (int qq = 0; qq < 4; ++qq) {
+                double a = asum[qq];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                cmax = fmax(cmax, a);
+            }
         }
         __syncwarp();
     }
@@ -116,34 +172,40 @@ sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, 
     if (p->gather_smem > 48 * 1024)
         SM_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
     k_gather<<<grid, p->gather_warps * 32, p->gather_smem, st>>>(
-        p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_val_off, vals, p->d_sub_ptr, p->d_sub_blocks,
-        p->d_sub_off, p->d_sub_dim, p->d_ld, p->d_ws_off, mu, X, p->d_gersh, p->max_sub_blocks,
-        p->info.dim_max + LD_ALIGN);
+        p->d_colptr, p->d_rowidx, p->d_val_off, vals, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off,
+        p->d_sub_dim, p->d_ld, p->d_ws_off, mu, X, p->d_gersh, p->gather_msb, p->gather_max_ld,
+        p->gather_hash_size, p->gather_hash_shift);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
-// Scatter (PAPER.md L127 step 3 + Eq.(16) inner factor): one CTA per block column c; threads
-// sweep the column's contiguous value range (coalesced stores); element (e,q) of block (r,c)
-// reads X_i[blk_loc(r) + e, gen_off(c) + q] of c's group i (X symmetric, so the read walks a
-// contiguous column segment).  D = 1/2 (delta - xs * X), xs = 1/s_i if the submatrix converged at
-// iteration 0 (the buffer then still holds the unscaled a_i - mu I), else 1.
+// Scatter (PAPER.md L127 step 3 + Eq.(16) inner factor): one warp per block column c.  The values
+// of a block column are one contiguous range of the result; the warp takes 32 of its blocks at a
+// time (one packed record each: row offset inside the submatrix | block height), prefix-sums
+// their sizes and then sweeps the contiguous output range with one element per lane (coalesced
+// stores), finding the block of an element by a shuffle binary search over the prefix sums.
+// Element (el,q) of block (r,c) reads X_i[gen_off(c) + q, blk_loc(r) + el] of c's group i
+// (X symmetric, so the read walks a contiguous row segment).  D = 1/2 (delta - xs * X), xs = 1/s_i
+// if the submatrix converged at iteration 0 (the buffer then still holds the unscaled
+// a_i - mu I), else 1.
 // ---------------------------------------------------------------------------------------------
-__global__ void k_scatter(const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
-                          const int32_t* __restrict__ rowidx, const int64_t* __restrict__ val_off,
-                          const int32_t* __restrict__ col_grp, const int32_t* __restrict__ gen_off,
-                          const int32_t* __restrict__ blk_loc, const int32_t* __restrict__ ldv,
-                          const int64_t* __restrict__ ws_off, const int32_t* __restrict__ done_iter,
-                          const unsigned long long* __restrict__ gersh, int cur_k,
-                          const double* __restrict__ buf0, const double* __restrict__ buf1,
-                          double* __restrict__ out, int as_identity) {
-    const int c = blockIdx.x;
+__global__ void __launch_bounds__(256)
+k_scatter(int nb, const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
+          const int64_t* __restrict__ val_off, const int32_t* __restrict__ col_grp,
+          const int32_t* __restrict__ gen_off, const uint32_t* __restrict__ blk_pack,
+          const int32_t* __restrict__ ldv, const int64_t* __restrict__ ws_off,
+          const int32_t* __restrict__ done_iter, const unsigned long long* __restrict__ gersh, int cur_k,
+          const double* __restrict__ buf0, const double* __restrict__ buf1, double* __restrict__ out,
+          int as_identity) {
+    const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (c >= nb) return;
+    const int lane = threadIdx.x & 31;
     const int g = col_grp[c];
     const int bc = blk_size[c];
-    const int64_t p0 = colptr[c], p1 = colptr[c + 1];
-    const int64_t v0 = val_off[p0], v1 = val_off[p1];
+    const int64_t p0 = colptr[c];
+    const int nblk = (int)(colptr[c + 1] - p0);
     const int di = done_iter[g];
     const int kb = di >= 0 ? di : cur_k;
     const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];
@@ -154,34 +216,48 @@ __global__ void k_scatter(const int32_t* __restrict__ blk_size, const int64_t* _
         xs = s > 0.0 ? 1.0 / s : 1.0;
     }
     const int go = gen_off[c];
-    const int nblk = (int)(p1 - p0);
-    for (int64_t e = v0 + threadIdx.x; e < v1; e += blockDim.x) {
-        // block containing element e: largest b with val_off[b] <= e
-        int lo = 0, hi = nblk - 1;
-        while (lo < hi) {
-            int mid = (lo + hi + 1) >> 1;
-            if (__ldg(val_off + p0 + mid) <= e) lo = mid; else hi = mid - 1;
+    double* o = out + val_off[p0];
+    for (int base = 0; base < nblk; base += 32) {
+        const int b = base + lane;
+        const uint32_t pk = b < nblk ? __ldg(blk_pack + p0 + b) : 0u;
+        const int sz = (int)(pk >> 20) * bc;
+        int incl = sz;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
         }
-        const int64_t b = p0 + lo;
-        const int r = rowidx[b];
-        const int br = blk_size[r];
-        const int w = (int)(e - val_off[b]);
-        const int q = w / br, el = w - q * br;
-        double x = Xg[panel_off(go + q, blk_loc[b] + el, ld)];
-        double d;
-        if (as_identity) d = x;
-        else d = 0.5 * (((r == c && q == el) ? 1.0 : 0.0) - xs * x);
-        out[e] = d;
+        const int excl = incl - sz;
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        for (int e0 = 0; e0 < total; e0 += 32) {
+            const int e = e0 + lane;
+            int k = 0;  // number of blocks that end at or before element e
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                const int v = __shfl_sync(0xffffffffu, incl, k + d - 1);
+                if (v <= e) k += d;
+            }
+            const uint32_t pkk = __shfl_sync(0xffffffffu, pk, k & 31);
+            const int ex = __shfl_sync(0xffffffffu, excl, k & 31);
+            if (e < total) {
+                const int br = (int)(pkk >> 20), loc = (int)(pkk & 0xfffffu);
+                const int w = e - ex;
+                const int q = w / br, el = w - q * br;
+                const double x = Xg[panel_off(go + q, loc + el, ld)];
+                o[e] = as_identity ? x : 0.5 * (((loc + el == go + q) ? 1.0 : 0.0) - xs * x);
+            }
+        }
+        o += total;
     }
-    (void)bc;
 }
 
 sm_status_t launch_scatter(sm_plan* p, int as_identity, const double* buf0, const double* buf1,
                            double* out, cudaStream_t st) {
     if (p->nb == 0) return SM_OK;
-    k_scatter<<<p->nb, 128, 0, st>>>(p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_val_off, p->d_col_grp,
-                                     p->d_gen_off, p->d_blk_loc, p->d_ld, p->d_ws_off, p->d_done_iter,
-                                     p->d_gersh, p->cur_k, buf0, buf1, out, as_identity);
+    k_scatter<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_blk_size, p->d_colptr, p->d_val_off, p->d_col_grp,
+                                               p->d_gen_off, p->d_blk_pack, p->d_ld, p->d_ws_off,
+                                               p->d_done_iter, p->d_gersh, p->cur_k, buf0, buf1, out,
+                                               as_identity);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;

@@ -99,7 +99,7 @@ __global__ void k_index_fill(int nb, const int32_t* __restrict__ blk_size, const
                              const int32_t* __restrict__ grp_cols, const int64_t* __restrict__ sub_ptr,
                              int32_t* __restrict__ sub_blocks, int32_t* __restrict__ sub_off,
                              int32_t* __restrict__ gen_pos, int32_t* __restrict__ gen_off,
-                             int32_t* __restrict__ blk_loc, int32_t* __restrict__ col_grp,
+                             uint32_t* __restrict__ blk_pack, int32_t* __restrict__ col_grp,
                              int32_t* __restrict__ gen_width, int32_t* __restrict__ err) {
     extern __shared__ uint32_t bitmap[];
     __shared__ int s_w[64];
@@ -147,8 +147,9 @@ __global__ void k_index_fill(int nb, const int32_t* __restrict__ blk_size, const
             if (pos < 0) atomicExch(err, 1); else gen_off[c] = So[pos];
         }
         for (int64_t p = colptr[c] + threadIdx.x; p < colptr[c + 1]; p += blockDim.x) {
-            int t = find_sorted(S, m, rowidx[p]);
-            blk_loc[p] = t >= 0 ? So[t] : -1;
+            const int r = rowidx[p];
+            const int t = find_sorted(S, m, r);  // always found: S_i contains the rows of its own columns
+            blk_pack[p] = (t >= 0 ? (uint32_t)So[t] : 0xfffffu) | ((uint32_t)blk_size[r] << 20);
         }
     }
     if (threadIdx.x == 0) gen_width[g] = gw;
@@ -212,7 +213,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMalloc((void**)&p->d_gen_pos, (size_t)std::max(nb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_gen_off, (size_t)std::max(nb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_col_grp, (size_t)std::max(nb, 1) * 4));
-    SM_CUDA(cudaMalloc((void**)&p->d_blk_loc, std::max<int64_t>(p->nnzb, 1) * 4));
+    SM_CUDA(cudaMalloc((void**)&p->d_blk_pack, std::max<int64_t>(p->nnzb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_gen_width, (size_t)std::max(ng, 1) * 4));
     int32_t* d_err = nullptr;
     SM_CUDA(cudaMalloc((void**)&d_err, 4));
@@ -220,7 +221,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     // pass 2
     if (ng > 0) k_index_fill<<<ng, 256, bm_bytes, st>>>(nb, p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr,
                                            p->d_grp_cols, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off,
-                                           p->d_gen_pos, p->d_gen_off, p->d_blk_loc, p->d_col_grp,
+                                           p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_col_grp,
                                            p->d_gen_width, d_err);
     p->launches++;
     int32_t herr = 0;
@@ -248,6 +249,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
         dmax = std::max(dmax, n);
     }
     p->sum_ld2 = off;
+    if (dmax >= (1 << 20) - LD_ALIGN) return SM_ERR_INVALID_ARG;  // packed block records hold 20-bit offsets
     std::vector<int32_t> order(ng);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return p->h_ld[a] > p->h_ld[b]; });
