@@ -148,22 +148,30 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
         sm_plan_destroy(p);
         return e == cudaErrorMemoryAllocation ? SM_ERR_ALLOC : SM_ERR_CUDA;
     }
-    // gather launch shape: per-warp source tables + row records + hash table + S_i / offsets
+    // gather launch shape: per-warp tile (qt dense columns x tile_ld) + two per-warp buffers of block
+    // records + member tables + hash table of S_i.  qt and the warp count shrink until the CTA fits.
     {
         const int msb = (std::max(p->max_sub_blocks, 1) + 1) & ~1;
-        const int max_ld = p->info.dim_max + LD_ALIGN;
+        const int tile_ld = (p->info.dim_max + LD_ALIGN + 1) & ~1;
         int hs = 32, shift = 27;
         while (hs < 2 * msb) { hs <<= 1; --shift; }
-        auto bytes = [&](int warps) {
-            return (size_t)warps * msb * 8 + (size_t)max_ld * 8 + (size_t)hs * 8 + (size_t)(2 * msb + 2) * 4;
+        auto bytes = [&](int warps, int qt) {
+            return (size_t)warps * 2 * qt * tile_ld * 8 + (size_t)msb * 16 + (size_t)warps * tile_ld * 8 +
+                   (size_t)hs * 8 + (size_t)(2 * msb + 2) * 4;
         };
-        int warps = 8;
-        const size_t budget = 200 * 1024;
-        while (warps > 1 && bytes(warps) > budget) warps >>= 1;
-        p->gather_warps = warps; p->gather_msb = msb; p->gather_max_ld = max_ld;
-        p->gather_hash_size = hs; p->gather_hash_shift = shift;
-        p->gather_smem = bytes(warps);
-        if (p->gather_smem > budget) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }
+        int warps = 8, qt = 4;
+        const size_t want = 60 * 1024, budget = 200 * 1024;  // measured: 3-4 CTAs per SM beat wider tiles
+        while (qt > 1 && bytes(warps, qt) > want) qt >>= 1;
+        while (warps > 1 && bytes(warps, qt) > want) warps >>= 1;
+        if (bytes(warps, qt) > budget) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }  // n_i > ~25000
+        p->gather_warps = warps; p->gather_qt = qt; p->gather_tile_ld = tile_ld;
+        p->gather_msb = msb; p->gather_hash_size = hs; p->gather_hash_shift = shift;
+        p->gather_smem = bytes(warps, qt);
+        // CTAs per submatrix: enough CTAs to fill the GPU a few times over, at least 2 block columns per warp
+        int split = 1;
+        const int64_t want_ctas = (int64_t)p->num_sms * 12;
+        while ((int64_t)ngroups * split < want_ctas && split * warps * 2 < p->max_sub_blocks) ++split;
+        p->gather_split = std::max(split, 1);
     }
     *plan = p;
     return SM_OK;

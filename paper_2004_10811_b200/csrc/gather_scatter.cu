@@ -17,164 +17,250 @@ __device__ __forceinline__ int find_sorted64(const int32_t* __restrict__ a, int 
 
 // ---------------------------------------------------------------------------------------------
 // Gather (PAPER.md L125 step 1; L187 "submatrix assembly becomes a purely local operation").
-// grid = (ngroups, chunks of GATHER_CB column blocks).  Per CTA, once: S_i and its element
-// offsets go to shared memory together with a hash table block-row -> member index and a
-// per-dense-row record (member, row inside the member, member height).  Then one warp assembles
-// one block column c = S_i[tc] of a_i at a time:
-//  (1) the lanes walk the stored blocks (r,c) of column c (coalesced reads of rowidx / val_off),
-//      look r up in the hash table and note the value offset of the block for member r;
-//      members without a stored block stay -1 -> zero fill (reading A4);
-//  (2) for up to four dense columns of the block column at once the lanes sweep the ld rows two
-//      at a time and store 16 bytes each, taking the values from the stored blocks, subtracting
-//      mu on the diagonal (Eq.(16)) and zero-padding rows/columns n..ld-1.
-// The column abs-sums give the Gershgorin bound s_i = max_q sum_p |a_pq| (symmetric: column sums
-// = row sums), combined by atomicMax on the bits of a non-negative double.
+// grid = (ngroups, split): the CTAs of a submatrix share its block columns round-robin by warp.
+// Per CTA, once, in shared memory: the members of S_i with their element offsets, for each the
+// extent of its stored block column (colptr, first value offset), and a hash table
+// block row -> (element offset inside a_i | block height).  All later global reads are then one
+// dependent hop deep.  One warp assembles one block column c = S_i[tc] of a_i at a time, through
+// two zeroed per-warp shared-memory tiles of qt dense columns x ld rows (software pipeline):
+//  (1) row list: the lanes take the stored blocks (r,c) of column c (rowidx / val_off, loaded
+//      one block column ahead into registers), probe the hash table, and a warp prefix sum over
+//      the heights of the blocks found expands them into a compact list of the stored dense rows
+//      (source offset, destination row | height); blocks whose row is not in S_i are dropped,
+//      members without a stored block stay zero in the tile (reading A4);
+//  (2) fill: lanes <-> consecutive entries of the row list, one 8-byte cp.async per dense column
+//      (no register round trip, every load of the pass in flight at once, consecutive lanes hit
+//      consecutive tile addresses); mu is subtracted on the diagonal (Eq.(16));
+//  (3) flush: the lanes sweep the tile rows two elements at a time: 16-byte coalesced stores into
+//      the k8-panel workspace (dense column q of a_i = row q of the symmetric X), abs-sums for
+//      the Gershgorin bound s_i = max_q sum_p |a_pq|, and the tile is zeroed again behind them.
+// Rows n..ld-1 of the tile are never filled, so padding comes out as zeros.
 // ---------------------------------------------------------------------------------------------
-constexpr int GATHER_CB = 16;  // column blocks per CTA
+constexpr int GATHER_PF = 3;  // block-column entries prefetched per lane (columns up to 96 blocks)
 
 __device__ __forceinline__ unsigned gather_hash(int key, int shift) {
     return ((unsigned)key * 2654435761u) >> shift;
 }
+__device__ __forceinline__ void cp_async8(unsigned smem_dst, const void* gsrc) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_dst), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-__global__ void __launch_bounds__(256)
-k_gather(const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx,
-         const int64_t* __restrict__ val_off, const double* __restrict__ vals,
-         const int64_t* __restrict__ sub_ptr, const int32_t* __restrict__ sub_blocks,
-         const int32_t* __restrict__ sub_off, const int32_t* __restrict__ sub_dim,
-         const int32_t* __restrict__ ldv, const int64_t* __restrict__ ws_off, double mu,
-         double* __restrict__ X, unsigned long long* __restrict__ gersh, int max_sub_blocks, int max_ld,
-         int hash_size, int hash_shift) {
+struct GatherArgs {
+    const int64_t* colptr;
+    const int32_t* rowidx;
+    const int64_t* val_off;
+    const double* vals;
+    const int64_t* sub_ptr;
+    const int32_t* sub_blocks;
+    const int32_t* sub_off;
+    const int32_t* sub_dim;
+    const int32_t* ldv;
+    const int64_t* ws_off;
+    double* X;
+    unsigned long long* gersh;
+    double mu;
+    int qt, tile_ld, msb, hash_size, hash_shift;
+};
+
+__global__ void __launch_bounds__(256, 3) k_gather(const GatherArgs A) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int g = blockIdx.x;
-    const int m = (int)(sub_ptr[g + 1] - sub_ptr[g]);
-    const int cb0 = blockIdx.y * GATHER_CB;
-    // column chunks past |S_i| only have padding columns to write (handled by the last chunk)
-    const int nchunks = (m + GATHER_CB - 1) / GATHER_CB;
-    if ((int)blockIdx.y >= nchunks) return;
-    const int n = sub_dim[g], ld = ldv[g];
-    // shared-memory carve-up (all 8-byte aligned)
-    int64_t* src_all = reinterpret_cast<int64_t*>(smem_raw);                  // [warps][max_sub_blocks]
+    const int64_t sp = A.sub_ptr[g];
+    const int m = (int)(A.sub_ptr[g + 1] - sp);
+    const int n = A.sub_dim[g], ld = A.ldv[g];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    int2* rinfo = reinterpret_cast<int2*>(src_all + (size_t)nw * max_sub_blocks);  // [max_ld]
-    int32_t* hk = reinterpret_cast<int32_t*>(rinfo + max_ld);                 // [hash_size] keys
-    int32_t* hv = hk + hash_size;                                             // [hash_size] member index
-    int32_t* S = hv + hash_size;                                              // [max_sub_blocks]
-    int32_t* So = S + max_sub_blocks;                                         // [max_sub_blocks + 1]
-    for (int h = threadIdx.x; h < hash_size; h += blockDim.x) hk[h] = -1;
-    for (int t = threadIdx.x; t < m; t += blockDim.x) {
-        S[t] = sub_blocks[sub_ptr[g] + t];
-        So[t] = sub_off[sub_ptr[g] + t];
-    }
-    if (threadIdx.x == 0) So[m] = n;
+    const int qt = A.qt, tile_ld = A.tile_ld, msb = A.msb;
+    // shared-memory carve-up
+    double* tiles = reinterpret_cast<double*>(smem_raw);                        // [nw][2][qt][tile_ld]
+    int64_t* mP0 = reinterpret_cast<int64_t*>(tiles + (size_t)nw * 2 * qt * tile_ld);   // [msb] colptr of member
+    int64_t* mVb = mP0 + msb;                                                   // [msb] first value offset
+    int2* rows_all = reinterpret_cast<int2*>(mVb + msb);                        // [nw][tile_ld]
+    int32_t* hk = reinterpret_cast<int32_t*>(rows_all + (size_t)nw * tile_ld);  // [hash_size] keys
+    uint32_t* hv = reinterpret_cast<uint32_t*>(hk + A.hash_size);               // [hash_size] offset | height << 20
+    int32_t* mLen = reinterpret_cast<int32_t*>(hv + A.hash_size);               // [msb] blocks in the column
+    int32_t* mSo = mLen + msb;                                                  // [msb + 1] element offsets
+    for (int h = threadIdx.x; h < A.hash_size; h += blockDim.x) hk[h] = -1;
+    for (int e = threadIdx.x; e < nw * 2 * qt * tile_ld; e += blockDim.x) tiles[e] = 0.0;
+    for (int t = threadIdx.x; t < m; t += blockDim.x) mSo[t] = A.sub_off[sp + t];
+    if (threadIdx.x == 0) mSo[m] = n;
     __syncthreads();
-    const unsigned hmask = (unsigned)hash_size - 1u;
+    const unsigned hmask = (unsigned)A.hash_size - 1u;
     for (int t = threadIdx.x; t < m; t += blockDim.x) {
-        const int key = S[t];
-        unsigned h = gather_hash(key, hash_shift);
+        const int key = A.sub_blocks[sp + t];
+        const int64_t p0 = A.colptr[key];
+        mP0[t] = p0;
+        mLen[t] = (int)(A.colptr[key + 1] - p0);
+        mVb[t] = A.val_off[p0];
+        unsigned h = gather_hash(key, A.hash_shift);
         while (atomicCAS(&hk[h], -1, key) != -1) h = (h + 1) & hmask;
-        hv[h] = t;
-        const int o = So[t], b = So[t + 1] - o;
-        for (int e = 0; e < b; ++e) rinfo[o + e] = make_int2(t, e | (b << 16));
+        hv[h] = (uint32_t)mSo[t] | ((uint32_t)(mSo[t + 1] - mSo[t]) << 20);
     }
-    for (int p = n + threadIdx.x; p < ld; p += blockDim.x) rinfo[p] = make_int2(-1, 0);
     __syncthreads();
-    int64_t* src = src_all + (size_t)wid * max_sub_blocks;                    // [m] per warp
-    double* Xg = X + ws_off[g];
+    double* tile = tiles + (size_t)wid * 2 * qt * tile_ld;
+    const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
+    int2* rows = rows_all + (size_t)wid * tile_ld;
+    double* Xg = A.X + A.ws_off[g];
     double cmax = 0.0;
-    const int cb1 = min(cb0 + GATHER_CB, m);
-    for (int tc = cb0 + wid; tc < cb1; tc += nw) {
-        const int c = S[tc];
-        const int coff = So[tc], bc = So[tc + 1] - coff;
-        for (int t = lane; t < m; t += 32) src[t] = -1;
-        __syncwarp();
-        const int64_t p0 = colptr[c];
-        const int clen = (int)(colptr[c + 1] - p0);
-        for (int j = lane; j < clen; j += 32) {
-            const int r = __ldg(rowidx + p0 + j);
-            unsigned h = gather_hash(r, hash_shift);
+
+    // (1) one stored block (row r, value offset vo relative to the column's first value): append
+    // its dense rows to the row list.  All 32 lanes call this together (ok = lane has a block).
+    int nrows = 0;
+    auto append = [&](bool ok, int r, int rel) {
+        uint32_t pk = 0;
+        if (ok) {
+            unsigned h = gather_hash(r, A.hash_shift);
             for (;;) {
                 const int k = hk[h];
-                if (k == r) { src[hv[h]] = __ldg(val_off + p0 + j); break; }
+                if (k == r) { pk = hv[h]; break; }
                 if (k < 0) break;
                 h = (h + 1) & hmask;
             }
         }
-        __syncwarp();
-        for (int q0 = 0; q0 < bc; q0 += 4) {
-            const int nq = min(4, bc - q0);
-            double asum[4] = {0.0, 0.0, 0.0, 0.0};
-            // dense column q of a_i is stored as row coff+q of the symmetric X (k8-panel layout)
-            size_t rbase[4];
-            int rstride[4];
+        const int br = (int)(pk >> 20);
+        int incl = br;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        int2* dst = rows + nrows + incl - br;
+        const int so = (int)(pk & 0xfffffu);
+        for (int el = 0; el < br; ++el) dst[el] = make_int2(rel + el, (so + el) | (br << 20));
+        nrows += __shfl_sync(0xffffffffu, incl, 31);
+    };
+    // (2) asynchronous copies of dense columns q0 .. q0+nq-1 of the listed rows into the tile
+    auto fill = [&](unsigned ts, const double* vcol, int q0, int nq) {
+        for (int k = lane; k < nrows; k += 32) {
+            const int2 en = rows[k];
+            const int br = (int)((uint32_t)en.y >> 20);
+            const double* vp = vcol + en.x + (int64_t)q0 * br;
+            unsigned d = ts + (unsigned)(en.y & 0xfffff) * 8u;
 #pragma unroll
             for (int qq = 0; qq < 4; ++qq) {
-                const int xrow = coff + q0 + (qq < nq ? qq : 0);
-                const int t0 = xrow & ~63;
-                const int rows_t = min(64, ld - t0);
-                rbase[qq] = (size_t)t0 * ld + (size_t)(xrow & 63) * 8;
-                rstride[qq] = rows_t * 8;
-            }
-            const int dq = coff + q0;  // diagonal position of dense column q0
-            for (int p = 2 * lane; p < ld; p += 64) {
-                double v[4][2];
-#pragma unroll
-                for (int qq = 0; qq < 4; ++qq) v[qq][0] = v[qq][1] = 0.0;
-#pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int2 ri = rinfo[p + u];
-                    if (ri.x >= 0) {
-                        const int64_t s0 = src[ri.x];
-                        if (s0 >= 0) {
-                            const int br = ri.y >> 16;
-                            const double* vp = vals + s0 + (int64_t)q0 * br + (ri.y & 0xffff);
-#pragma unroll
-                            for (int qq = 0; qq < 4; ++qq)
-                                if (qq < nq) v[qq][u] = __ldg(vp + qq * br);
-                        }
-                    }
-                }
-#pragma unroll
-                for (int qq = 0; qq < 4; ++qq) {
-                    if (qq < nq) {
-                        if (dq + qq == p) v[qq][0] -= mu;
-                        else if (dq + qq == p + 1) v[qq][1] -= mu;
-                        asum[qq] += fabs(v[qq][0]) + fabs(v[qq][1]);
-                        *reinterpret_cast<double2*>(Xg + rbase[qq] + (size_t)(p >> 3) * rstride[qq] + (p & 7)) =
-                            make_double2(v[qq][0], v[qq][1]);
-                    }
-                }
-            }
-#pragma unroll
-            for (int qq = 0; qq < 4; ++qq) {
-                double a = asum[qq];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-                cmax = fmax(cmax, a);
+                if (qq < nq) cp_async8(d, vp);
+                vp += br;
+                d += (unsigned)tile_ld * 8u;
             }
         }
+    };
+
+    const int stride = nw * gridDim.y;
+    // register prefetch of a block column's entries, one block column ahead of the row list
+    int pr[GATHER_PF];
+    int64_t pv[GATHER_PF];
+    auto prefetch = [&](int t) {
+        if (t >= m) return;
+        const int64_t p0 = mP0[t];
+        const int clen = mLen[t];
+        if (clen > 32 * GATHER_PF) return;
+#pragma unroll
+        for (int i = 0; i < GATHER_PF; ++i) {
+            const int j = lane + 32 * i;
+            if (j < clen) { pr[i] = __ldg(A.rowidx + p0 + j); pv[i] = __ldg(A.val_off + p0 + j); }
+        }
+    };
+    // Software pipeline over passes (block column tc, dense columns q0..q0+nq-1) with two tiles per
+    // warp: the copies of pass k+1 are issued before pass k is flushed, so the global-load latency
+    // of a fill hides behind the row list of the next pass and the flush of the previous one.
+    int tc_f = blockIdx.y * nw + wid, q0_f = 0;  // next pass to issue
+    prefetch(tc_f);
+    int is_coff = 0, is_q0 = 0, is_nq = 0;  // what the flush needs to know about the pass just issued
+    auto issue = [&](int buf) -> bool {
+        if (tc_f >= m) return false;
+        const int coff = mSo[tc_f], bc = mSo[tc_f + 1] - coff;
+        const int64_t p0 = mP0[tc_f], vb = mVb[tc_f];
+        const int clen = mLen[tc_f];
+        const double* vcol = A.vals + vb;
+        const int nq = min(qt, bc - q0_f);
+        const unsigned ts = tile_s + (unsigned)(buf * qt * tile_ld) * 8u;
+        if (clen <= 32 * GATHER_PF) {
+            if (q0_f == 0) {  // the row list of a short column is built once and serves all its passes
+                nrows = 0;
+#pragma unroll
+                for (int i = 0; i < GATHER_PF; ++i)
+                    if (32 * i < clen) append(lane + 32 * i < clen, pr[i], (int)(pv[i] - vb));
+                __syncwarp();
+                prefetch(tc_f + stride);
+            }
+            fill(ts, vcol, q0_f, nq);
+        } else {  // long column: list and fill 32 blocks at a time (cp.async has read its list entry at issue)
+            for (int jb = 0; jb < clen; jb += 32) {
+                const bool ok = jb + lane < clen;
+                nrows = 0;
+                append(ok, ok ? __ldg(A.rowidx + p0 + jb + lane) : 0,
+                       ok ? (int)(__ldg(A.val_off + p0 + jb + lane) - vb) : 0);
+                __syncwarp();
+                fill(ts, vcol, q0_f, nq);
+                __syncwarp();
+            }
+            if (q0_f + qt >= bc) prefetch(tc_f + stride);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        is_coff = coff; is_q0 = q0_f; is_nq = nq;
+        q0_f += qt;
+        if (q0_f >= bc) { tc_f += stride; q0_f = 0; }
+        return true;
+    };
+    int buf = 0;
+    bool have = issue(0);
+    while (have) {
+        const int coff = is_coff, q0 = is_q0, nq = is_nq;
+        const bool have_next = issue(buf ^ 1);
+        if (have_next) asm volatile("cp.async.wait_group 1;" ::: "memory");
+        else asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
+        double* tl = tile + buf * qt * tile_ld;
+        if (lane < nq) tl[lane * tile_ld + coff + q0 + lane] -= A.mu;
+        __syncwarp();
+        // (3) flush.  Lane covers columns p = 2 lane + 64 i: panel (lane >> 2) + 8 i, offset
+        // 2 (lane & 3) inside it.  Offsets inside one submatrix fit 32 bits (ld <= 25600).
+        for (int qq = 0; qq < nq; ++qq) {
+            const int xrow = coff + q0 + qq;
+            const int t0 = xrow & ~63;
+            const unsigned rstride = (unsigned)min(64, ld - t0) * 8u;
+            unsigned xo = (unsigned)t0 * (unsigned)ld + (unsigned)(xrow & 63) * 8u +
+                          (unsigned)(lane >> 2) * rstride + 2u * (lane & 3);
+            double* tp = tl + qq * tile_ld + 2 * lane;
+            const unsigned xstep = rstride * 8u;
+            double a = 0.0;
+#pragma unroll 4
+            for (int p = 2 * lane; p < ld; p += 64, tp += 64, xo += xstep) {
+                const double2 v = *reinterpret_cast<const double2*>(tp);
+                *reinterpret_cast<double2*>(tp) = make_double2(0.0, 0.0);
+                a += fabs(v.x) + fabs(v.y);
+                *reinterpret_cast<double2*>(Xg + xo) = v;
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+            cmax = fmax(cmax, a);
+        }
+        __syncwarp();
+        buf ^= 1;
+        have = have_next;
     }
-    // zero padding columns n..ld-1 (last chunk only)
-    if ((int)blockIdx.y == nchunks - 1) {
+    // zero padding columns n..ld-1 (first CTA of the submatrix)
+    if (blockIdx.y == 0) {
         for (int qq = n + wid; qq < ld; qq += nw) {
             for (int p = 2 * lane; p < ld; p += 64)
                 *reinterpret_cast<double2*>(Xg + panel_off(qq, p, ld)) = make_double2(0.0, 0.0);
         }
     }
-    if (lane == 0 && cmax > 0.0) atomicMax(gersh + g, (unsigned long long)__double_as_longlong(cmax));
+    if (lane == 0 && cmax > 0.0) atomicMax(A.gersh + g, (unsigned long long)__double_as_longlong(cmax));
 }
 
 sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, cudaStream_t st) {
     if (p->ngroups == 0) return SM_OK;
     SM_CUDA(cudaMemsetAsync(p->d_gersh, 0, (size_t)p->ngroups * 8, st));
-    int chunks = (p->max_sub_blocks + GATHER_CB - 1) / GATHER_CB;
-    dim3 grid(p->ngroups, chunks > 0 ? chunks : 1);
     if (p->gather_smem > 48 * 1024)
         SM_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
-    k_gather<<<grid, p->gather_warps * 32, p->gather_smem, st>>>(
-        p->d_colptr, p->d_rowidx, p->d_val_off, vals, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off,
-        p->d_sub_dim, p->d_ld, p->d_ws_off, mu, X, p->d_gersh, p->gather_msb, p->gather_max_ld,
-        p->gather_hash_size, p->gather_hash_shift);
+    GatherArgs a;
+    a.colptr = p->d_colptr; a.rowidx = p->d_rowidx; a.val_off = p->d_val_off; a.vals = vals;
+    a.sub_ptr = p->d_sub_ptr; a.sub_blocks = p->d_sub_blocks; a.sub_off = p->d_sub_off; a.sub_dim = p->d_sub_dim;
+    a.ldv = p->d_ld; a.ws_off = p->d_ws_off; a.X = X; a.gersh = p->d_gersh; a.mu = mu;
+    a.qt = p->gather_qt; a.tile_ld = p->gather_tile_ld; a.msb = p->gather_msb;
+    a.hash_size = p->gather_hash_size; a.hash_shift = p->gather_hash_shift;
+    k_gather<<<dim3(p->ngroups, p->gather_split), p->gather_warps * 32, p->gather_smem, st>>>(a);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;

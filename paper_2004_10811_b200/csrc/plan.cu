@@ -173,6 +173,9 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
         for (int64_t q = p->h_colptr[c]; q < p->h_colptr[c + 1]; ++q)
             val_off[q + 1] = val_off[q] + (int64_t)p->h_blk_size[p->h_rowidx[q]] * p->h_blk_size[c];
     p->nnz = val_off[p->nnzb];
+    p->max_col_blocks = 0;
+    for (int c = 0; c < nb; ++c)
+        p->max_col_blocks = std::max<int32_t>(p->max_col_blocks, (int32_t)(p->h_colptr[c + 1] - p->h_colptr[c]));
     if ((s = upload(&p->d_blk_size, p->h_blk_size.data(), nb, st))) return s;
     if ((s = upload(&p->d_blk_off, blk_off.data(), nb + 1, st))) return s;
     if ((s = upload(&p->d_colptr, p->h_colptr.data(), nb + 1, st))) return s;
