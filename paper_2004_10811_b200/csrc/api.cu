@@ -130,7 +130,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_flag, (size_t)ng * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_res, (size_t)ng * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_gersh, (size_t)ng * 8);
-    if (e == cudaSuccess) e = A((void**)&p->d_partials, (size_t)p->n_tiles * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_partials, (size_t)p->n_tiles * 4 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_counters, (size_t)(p->opt.max_iter + 2) * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_sched, (size_t)(p->opt.max_iter + 2) * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_tile_done, (size_t)ng * 4);

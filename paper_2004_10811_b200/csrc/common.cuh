@@ -84,7 +84,7 @@ struct sm_plan {
     int32_t* d_flag = nullptr;             // [ngroups] 0 converged, 1 stagnated / max_iter
     double* d_res = nullptr;               // [2][ngroups] residual history (ping-pong)
     unsigned long long* d_gersh = nullptr; // [ngroups] bits of the Gershgorin bound (atomicMax)
-    double* d_partials = nullptr;          // [n_tiles] per-tile residual partial sums
+    double* d_partials = nullptr;          // [n_tiles][4] per-tile, per-consumer-warp residual partials
     int32_t* d_counters = nullptr;         // [max_iter+2] still-active submatrices after iteration k
     int32_t* d_sched = nullptr;            // [2*(max_iter+2)] work counters of the persistent GEMM launches
     int32_t* d_tile_done = nullptr;        // [ngroups] finished tiles of a submatrix in the current launch
