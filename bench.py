@@ -159,6 +159,53 @@ def run_reference(args, m, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_phases(args, m, B, torch):
+    """--phases: CUDA-event timing of the HBM-bound phases (a3 gather + a4 bound, a6 scatter) and of
+    one fixed-mu sign evaluation, each against its roofline.  One JSON line."""
+    plan = B.plan_from_matrix(m)
+    info = B.sm_plan_query(plan)
+    ws = B.alloc_workspace(plan)
+    vin = torch.from_numpy(m.values).cuda()
+    vout = torch.empty_like(vin)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    hbm = 6544.3
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            hbm = json.load(f)["hbm_gbs"]
+
+    def timeit(f, reps=10):
+        for _ in range(3):
+            f()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            e0.record(); f(); e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return min(ts), float(np.median(ts))
+
+    out = {"phases": True, "config": workload_config(args, m), "hbm_peak_GBps": hbm}
+    gb = (info.sum_ld2 + info.nnz) * 8 / 1e9
+    tmin, tmed = timeit(lambda: B.sm_gather(plan, vin, 0.0, ws))
+    out["gather"] = {"ms_min": tmin, "ms_med": tmed, "alg_GB": gb, "GBps": gb / tmed * 1e3, "frac": gb / tmed * 1e3 / hbm}
+    _, _, _, sub_dim, _ = B.sm_plan_export_index(plan)
+    gw = np.zeros(m.ngroups, np.int64)
+    np.add.at(gw, np.repeat(np.arange(m.ngroups), np.diff(m.grp_ptr)), m.blk_size[m.grp_cols])
+    sb = ((sub_dim.astype(np.int64) * gw).sum() + info.nnz) * 8 / 1e9
+    tmin, tmed = timeit(lambda: B.sm_scatter(plan, 1, vout, ws))
+    out["scatter"] = {"ms_min": tmin, "ms_med": tmed, "alg_GB": sb, "GBps": sb / tmed * 1e3, "frac": sb / tmed * 1e3 / hbm}
+    st = B.sm_stats_t()
+    B.sm_set_timing(plan, True)
+    for _ in range(2):
+        B.sm_sign_execute(plan, vin, 0.0, EPS, vout, ws, st)
+    d = st.as_dict()
+    out["sign"] = {"ms_sign": d["ms_sign"], "iter_min": d["iter_min"], "iter_max": d["iter_max"],
+                   "gemm_launches": d["gemm_launches"], "alg_TFLOPs": d["tot_sym_flop"] / d["ms_sign"] / 1e9,
+                   "ms_gather": d["ms_gather"], "ms_scatter": d["ms_scatter"], "ms_total": d["ms_total"]}
+    print(json.dumps(out), flush=True)
+    B.sm_plan_destroy(plan)
+
+
 def workload_config(args, m):
     from paper_2004_10811_b200 import workloads as W
     c = W.CONFIGS[args.config]
@@ -180,6 +227,8 @@ def main():
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--phases", action="store_true",
+                    help="time gather / scatter / one sign evaluation separately (phase rooflines) and exit")
     args = ap.parse_args()
     rank, local_rank, world = dist_env()
     from paper_2004_10811_b200 import workloads as W
@@ -202,6 +251,10 @@ def main():
 
     # replicas: rank r builds the same-size problem from seed + r
     m = W.make_config(args.config, args.seed + rank)
+    if args.phases:
+        if rank == 0:
+            run_phases(args, m, B, torch)
+        return
     plan = B.plan_from_matrix(m)
     info = B.sm_plan_query(plan)
     ws = B.alloc_workspace(plan)
