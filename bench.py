@@ -346,7 +346,8 @@ def main():
                            "workspace_GB": info.workspace_bytes / 1e9, "n_tiles": info.n_tiles,
                            "gather_GBps": gather_bytes * evals / (gather_ms * 1e-3) / 1e9 if gather_ms > 0 else None,
                            "ms_scatter_last": last["ms_scatter"], "mu_trace": last["mu_trace"],
-                           "ne_trace": last["ne_trace"]}}
+                           "ne_trace": last["ne_trace"], "ne_err_trace": last["ne_err_trace"],
+                           "iter_trace": last["iter_trace"], "spec_lo": last["spec_lo"], "spec_hi": last["spec_hi"]}}
         if not args.no_cpu_baseline:
             cb, _ = cpu_baseline(m)
             line["cpu_baseline"] = cb

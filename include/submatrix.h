@@ -58,8 +58,11 @@ enum {
 /* Options fixed at plan creation.  Pass NULL for the defaults written beside each field. */
 typedef struct {
     int32_t max_iter;    /* Newton-Schulz iteration cap per sign evaluation            [100] */
-    int32_t scaling;     /* spectral bound for X0 = (a - mu I)/s: 0 = Gershgorin row   [0]   */
-                         /* sums of the assembled submatrix (reading A8)                     */
+    int32_t scaling;     /* spectral bound for X0 = (a - mu I)/s (reading A8):          [1]  */
+                         /* 0 = Gershgorin row sums of the assembled submatrix;              */
+                         /* 1 = min(that, interlacing bound): a_i is a principal submatrix   */
+                         /*     of K~, so rho(a_i - mu I) <= max|lambda_minmax(K~) - mu|,    */
+                         /*     extremes of K~ by a short Lanczos run per call, then / overshoot */
     int32_t precision;   /* 0 = FP64 DMMA (the parity path)                            [0]   */
     int32_t check_every; /* host polls the "all converged" counter every this many     [1]   */
                          /* iterations (>= 1)                                                */
@@ -68,7 +71,14 @@ typedef struct {
                          /* (0 = max_iter). A capped evaluation is only used for the         */
                          /* direction of the step, never for acceptance (A11).     */
     double mu_tol;       /* bisection stops when the bracket is narrower than this     [1e-6]*/
-    int32_t reserved[8];
+    int32_t early_out;   /* 1: a bisection evaluation stops as soon as the bound           [1]  */
+                         /* |n_elec(final) - n_elec(X_k)| <= 1/2 sum_gen (1 - (X_k^2)_kk)     */
+                         /* proves the sign of n_elec - n_target (reading A11c); such a step */
+                         /* only steers, it is never accepted.  0: every evaluation converges*/
+    int32_t reserved_i;
+    double overshoot;    /* scaling = 1 only: s = bound / overshoot, 1 <= overshoot <= 1.5 [1.25]*/
+                         /* (eigenvalues of X0 in (1, 1.5] map back into [0.56, 1))          */
+    int32_t reserved[4];
 } sm_options_t;
 
 /* Plan facts (all sizes in elements unless they say bytes). */
@@ -102,13 +112,17 @@ typedef struct {
     int64_t sum_iter_n3;      /* sum_i (2*iters_i + 1) * n_i^3  (=> flop = 2x this)          */
     float ms_gather, ms_sign, ms_scatter, ms_total;
     double mu_trace[64];      /* bisection history: mu of step k                             */
-    double ne_trace[64];      /* n_elec of step k                                            */
+    double ne_trace[64];      /* n_elec of step k (of the last iterate if the step ended early) */
+    double ne_err_trace[64];  /* bound on |n_elec(converged) - ne_trace[k]| (0: converged)    */
+    int32_t iter_trace[64];   /* Newton-Schulz iterations spent on step k                    */
     /* totals over ALL sign evaluations of the call (a bisection makes several) */
     int64_t tot_sum_iter_n3;  /* sum over evaluations of sum_iter_n3                         */
     int64_t tot_sym_flop;     /* sum over executed symmetric products of n_i^2 (n_i + 1)     */
     int32_t tot_gemm_launches;
     int32_t tot_evaluations;
     float tot_ms_gather, tot_ms_sign;
+    double spec_lo, spec_hi;  /* scaling = 1: the widened Lanczos estimate of [lambda_min, lambda_max] */
+                              /* of K~ the interlacing bound was taken from (else 0, 0)       */
 } sm_stats_t;
 
 /*

@@ -34,7 +34,8 @@ EXPORTS = [
 class sm_options_t(C.Structure):
     _fields_ = [("max_iter", C.c_int32), ("scaling", C.c_int32), ("precision", C.c_int32),
                 ("check_every", C.c_int32), ("max_mu_steps", C.c_int32), ("bisect_iter", C.c_int32),
-                ("mu_tol", C.c_double), ("reserved", C.c_int32 * 8)]
+                ("mu_tol", C.c_double), ("early_out", C.c_int32), ("reserved_i", C.c_int32),
+                ("overshoot", C.c_double), ("reserved", C.c_int32 * 4)]
 
 
 class sm_plan_info_t(C.Structure):
@@ -51,21 +52,25 @@ class sm_stats_t(C.Structure):
                 ("mu", C.c_double), ("mu_steps", C.c_int32), ("gemm_launches", C.c_int32),
                 ("sum_iter_n3", C.c_int64), ("ms_gather", C.c_float), ("ms_sign", C.c_float),
                 ("ms_scatter", C.c_float), ("ms_total", C.c_float), ("mu_trace", C.c_double * 64),
-                ("ne_trace", C.c_double * 64), ("tot_sum_iter_n3", C.c_int64), ("tot_sym_flop", C.c_int64),
+                ("ne_trace", C.c_double * 64), ("ne_err_trace", C.c_double * 64), ("iter_trace", C.c_int32 * 64),
+                ("tot_sum_iter_n3", C.c_int64), ("tot_sym_flop", C.c_int64),
                 ("tot_gemm_launches", C.c_int32), ("tot_evaluations", C.c_int32),
-                ("tot_ms_gather", C.c_float), ("tot_ms_sign", C.c_float)]
+                ("tot_ms_gather", C.c_float), ("tot_ms_sign", C.c_float),
+                ("spec_lo", C.c_double), ("spec_hi", C.c_double)]
 
     def as_dict(self):
-        d = {k: getattr(self, k) for k, _ in self._fields_ if k not in ("mu_trace", "ne_trace")}
+        d = {k: getattr(self, k) for k, _ in self._fields_ if k not in ("mu_trace", "ne_trace", "ne_err_trace", "iter_trace")}
         n = max(int(self.mu_steps), 0)
         d["mu_trace"] = list(self.mu_trace[:n])
         d["ne_trace"] = list(self.ne_trace[:n])
+        d["ne_err_trace"] = list(self.ne_err_trace[:n])
+        d["iter_trace"] = list(self.iter_trace[:n])
         return d
 
 
 def default_options(**kw) -> sm_options_t:
-    o = sm_options_t(max_iter=100, scaling=0, precision=0, check_every=1, max_mu_steps=64, bisect_iter=0,
-                     mu_tol=1e-6)
+    o = sm_options_t(max_iter=100, scaling=1, precision=0, check_every=1, max_mu_steps=64, bisect_iter=0,
+                     mu_tol=1e-6, early_out=1, overshoot=1.25)
     for k, v in kw.items():
         setattr(o, k, v)
     return o

@@ -22,7 +22,9 @@ using namespace smb;
 static void default_options(sm_options_t* o) {
     memset(o, 0, sizeof(*o));
     o->max_iter = 100;
-    o->scaling = 0;
+    o->scaling = 1;
+    o->early_out = 1;
+    o->overshoot = 1.25;
     o->precision = 0;
     o->check_every = 1;
     o->max_mu_steps = 64;
@@ -77,11 +79,12 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_gen_width, p->d_ws_off, p->d_ld, p->d_tiles,
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
                     p->d_partials, p->d_counters, p->d_sched, p->d_tile_done, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
-                    p->d_stage_out};
+                    p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     if (p->h_pinned) cudaFreeHost(p->h_pinned);
     if (p->h_pinned_d) cudaFreeHost(p->h_pinned_d);
+    if (p->h_bound) cudaFreeHost(p->h_bound);
     for (auto& e : p->ev)
         if (e) cudaEventDestroy(e);
     for (auto& e : p->ev_iter)
@@ -105,7 +108,9 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (p->opt.max_mu_steps <= 0) p->opt.max_mu_steps = 64;
     if (p->opt.max_mu_steps > 64) p->opt.max_mu_steps = 64;
     if (!(p->opt.mu_tol > 0)) p->opt.mu_tol = 1e-6;
-    if (p->opt.precision != 0 || p->opt.scaling != 0) { delete p; return SM_ERR_INVALID_ARG; }
+    if (!(p->opt.overshoot >= 1.0)) p->opt.overshoot = 1.0;     // zero-initialised struct: no overshoot
+    if (p->opt.overshoot > 1.5) p->opt.overshoot = 1.5;         // f(x) = x(3 - x^2)/2 keeps [1, 1.5] inside [0.56, 1]
+    if (p->opt.precision != 0 || p->opt.scaling < 0 || p->opt.scaling > 1) { delete p; return SM_ERR_INVALID_ARG; }
     p->nb = nb; p->ngroups = ngroups; p->nnzb = nb ? colptr[nb] : 0;
     p->h_blk_size.assign(blk_size, blk_size + nb);
     p->h_colptr.assign(colptr, colptr + nb + 1);
@@ -137,6 +142,9 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_ne_part, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_scalars, 8 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_red, 4096 * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_bound, (size_t)(p->opt.max_iter + 2) * 16);
+    if (e == cudaSuccess) e = A((void**)&p->d_bound_part, (size_t)ng * 16);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_bound, (size_t)(p->opt.max_iter + 2) * 16);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned, (size_t)(p->opt.max_iter + 2) * 4);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned_d, 8 * 8);
     for (auto& ev : p->ev)
@@ -230,34 +238,65 @@ sm_status_t reset_state(sm_plan* p, cudaStream_t st) {
     return SM_OK;
 }
 
-// Newton-Schulz host loop: iterations k = k_begin .. k_end-1 (each = MODE 0 + MODE 1 launch).
+// Steering of one bisection evaluation (reading A11c): the loop may stop as soon as the bound of
+// k_nelec_bound proves on which side of n_target the converged n_elec lies.
+struct Steer {
+    double n_target = 0.0, tol_n = 0.0, slack = 0.0;
+    int decided = 0;        // out: +1 n_elec > n_target + tol_n proven, -1 the opposite, 0 not decided
+    int k = -1;             // out: iterate the decision was taken on
+    double ne = 0.0, err = 0.0;  // out: n_elec(X_k) and its bound
+};
+
+// Newton-Schulz host loop: iterations k = cur_k .. k_end-1 (each = MODE 0 + MODE 1 launch).
 // Iteration k tests X_k and, if not converged, forms X_{k+1}.  At k == max_iter only the decision
-// is recorded.  Returns with *all_done = 1 if every submatrix has stopped.
+// is recorded.  Returns with *all_done = 1 if every submatrix has stopped.  The host reads the
+// "still active" counter (and the steering bound) one iteration behind, so it never stalls the GPU.
 sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_done, int* launched,
-                    cudaStream_t st) {
+                    cudaStream_t st, Steer* steer = nullptr) {
     *all_done = 0;
     if (p->ngroups == 0) { *all_done = 1; return SM_OK; }
     const int max_iter = p->opt.max_iter;
     int k = p->cur_k;
     int pending = -1;  // iteration whose counter copy is in flight
+    auto poll = [&](int q) -> int {  // 1 = all converged, 2 = steering decision, 0 = go on
+        if (p->h_pinned[q] == 0) { *all_done = 1; p->cur_k = q; return 1; }
+        if (steer && q >= 1) {
+            const double ne = p->h_bound[2 * q], err = p->h_bound[2 * q + 1];
+            if (ne == ne && err == err && err >= 0.0) {
+                const double g = ne - steer->n_target, m = err + steer->slack + steer->tol_n;
+                if (g > m || g < -m) {
+                    steer->decided = g > 0 ? 1 : -1; steer->k = q; steer->ne = ne; steer->err = err;
+                    return 2;
+                }
+            }
+        }
+        return 0;
+    };
     for (; k < k_end && k <= max_iter; ++k) {
         sm_status_t s = launch_ns_pair(p, k, eps, k == max_iter ? 1 : 0, b.b0, b.b1, b.y, st);
         if (s) return s;
         (*launched) += (k == max_iter) ? 1 : 2;
+        if (steer && k >= 1 && (s = launch_nelec_bound(p, k, b.b0, b.b1, b.y, st))) return s;
         if (pending >= 0) {
             SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
-            if (p->h_pinned[pending] == 0) { *all_done = 1; p->cur_k = pending; return SM_OK; }
+            const int r = poll(pending);
+            if (r == 1) return SM_OK;
+            if (r == 2) { p->cur_k = std::min(k + 1, max_iter); return SM_OK; }
             pending = -1;
         }
         if ((k % p->opt.check_every) == 0 || k == max_iter || k == k_end - 1) {
             SM_CUDA(cudaMemcpyAsync(p->h_pinned + k, p->d_counters + k, 4, cudaMemcpyDeviceToHost, st));
+            if (steer && k >= 1)
+                SM_CUDA(cudaMemcpyAsync(p->h_bound + 2 * k, p->d_bound + 2 * k, 16, cudaMemcpyDeviceToHost, st));
             SM_CUDA(cudaEventRecord(p->ev_iter[k & 1], st));
             pending = k;
         }
     }
     if (pending >= 0) {
         SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
-        if (p->h_pinned[pending] == 0) { *all_done = 1; p->cur_k = pending; return SM_OK; }
+        const int r = poll(pending);
+        if (r == 1) return SM_OK;
+        if (r == 2) { p->cur_k = std::min(k, max_iter); return SM_OK; }
     }
     // active submatrices have received k updates: their X lives in buf[k & 1]
     p->cur_k = std::min(k, max_iter);
@@ -288,9 +327,11 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         double r = res[(size_t)slot * ng + i];
         if (r == r) rmax = std::max(rmax, r); else rmax = INFINITY;
         int64_t n = p->h_sub_dim[i];
-        // executed GEMMs: one X^2 per tested iterate (it + 1) and one update per iteration (it)
-        sin3 += (int64_t)(2 * it + 1) * n * n * n;
-        symf += (int64_t)(2 * it + 1) * n * n * (n + 1);
+        // executed symmetric products: stopped at iteration it: one X^2 per tested iterate (it + 1)
+        // and one update per iteration (it); still active after cur_k launch pairs: 2 cur_k
+        const int64_t prods = di[i] >= 0 ? 2 * it + 1 : 2 * (int64_t)p->cur_k;
+        sin3 += prods * n * n * n;
+        symf += prods * n * n * (n + 1);
     }
     *not_conv = nc;
     if (stats) {
@@ -305,20 +346,39 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
     return SM_OK;
 }
 
+// Spectral scale of the evaluation at mu (option scaling = 1): s_i = min(Gershgorin_i, cap(mu)) / overshoot.
+sm_status_t ensure_bounds(sm_plan* p, const double* d_in, cudaStream_t st) {
+    if (p->opt.scaling != 1 || p->lz_valid) return SM_OK;
+    sm_status_t s = launch_lanczos_bounds(p, d_in, st);
+    if (s) return s;
+    p->lz_valid = 1;
+    return SM_OK;
+}
+sm_status_t apply_scaling(sm_plan* p, double mu, cudaStream_t st) {
+    if (p->opt.scaling != 1) return SM_OK;
+    const double cap = std::max(std::fabs(p->lz_hi - mu), std::fabs(p->lz_lo - mu));
+    return launch_apply_scale(p, cap, p->opt.overshoot, st);
+}
+
 // One sign evaluation at fixed mu: gather -> NS loop (up to iter_cap iterations) -> n_elec.
+// With `steer` the loop may end early on a proven direction (steer->decided != 0): the workspace
+// is then NOT converged and stats->n_elec is the last iterate's count.
 sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, const Bufs& b, int iter_cap,
-                     sm_stats_t* stats, int* not_conv, cudaStream_t st) {
+                     sm_stats_t* stats, int* not_conv, cudaStream_t st, Steer* steer = nullptr) {
     sm_status_t s;
     int launched = 0, all_done = 0;
+    if ((s = ensure_bounds(p, d_in, st))) return s;  // once per call, outside the gather timing
     if (p->timing) SM_CUDA(cudaEventRecord(p->ev[0], st));
     if ((s = reset_state(p, st))) return s;
     if ((s = launch_gather(p, d_in, mu, b.b0, st))) return s;
+    if ((s = apply_scaling(p, mu, st))) return s;
     if (p->timing) SM_CUDA(cudaEventRecord(p->ev[1], st));
-    if ((s = ns_loop(p, b, eps, iter_cap, &all_done, &launched, st))) return s;
+    if ((s = ns_loop(p, b, eps, iter_cap, &all_done, &launched, st, steer))) return s;
     if (p->timing) SM_CUDA(cudaEventRecord(p->ev[2], st));
     if ((s = launch_nelec(p, b.b0, b.b1, st))) return s;
     if ((s = collect_stats(p, stats, not_conv, st))) return s;
     if (stats) {
+        if (steer && steer->decided) stats->n_elec = steer->ne;
         stats->iterations = launched / 2;
         stats->gemm_launches = launched;
         stats->mu = mu;
@@ -331,6 +391,7 @@ sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, cons
         stats->tot_evaluations = 1;
         stats->tot_ms_gather = stats->ms_gather;
         stats->tot_ms_sign = stats->ms_sign;
+        if (p->opt.scaling == 1) { stats->spec_lo = p->lz_lo; stats->spec_hi = p->lz_hi; }
     }
     return SM_OK;
 }
@@ -368,6 +429,7 @@ extern "C" sm_status_t sm_sign_execute(sm_plan_t* p, const double* d_vals_in, do
     if (s) return s;
     if (stats) memset(stats, 0, sizeof(*stats));
     int nc = 0;
+    p->lz_valid = 0;  // the values may have changed since the last call
     if ((s = evaluate(p, d_vals_in, mu, eps, b, p->opt.max_iter + 1, stats, &nc, st))) return s;
     if (d_vals_out && (s = do_scatter(p, b, d_vals_out, stats, st))) return s;
     if (stats) stats->mu_steps = 1;
@@ -448,7 +510,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
                                                                                        : p->opt.max_iter + 1;
     double best_mu = mu, best_g = INFINITY;
     int best_step = -1, steps = 0, nc = 0, last_nc = 0;
-    bool accepted = false;
+    bool accepted = false, last_partial = false;
     sm_stats_t ev;
     int64_t acc_n3 = 0, acc_sym = 0;
     int acc_launch = 0, acc_eval = 0;
@@ -457,11 +519,17 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         acc_n3 += e.tot_sum_iter_n3; acc_sym += e.tot_sym_flop; acc_launch += e.tot_gemm_launches;
         acc_eval += 1; acc_g += e.tot_ms_gather; acc_s += e.tot_ms_sign;
     };
+    p->lz_valid = 0;  // one Lanczos run serves every mu of this call
+    const bool early = p->opt.early_out != 0;
     for (; steps < p->opt.max_mu_steps;) {
         memset(&ev, 0, sizeof(ev));
-        if ((s = evaluate(p, d_vals_in, mu, eps, b, cap, &ev, &nc, st))) return s;
+        Steer steer;
+        steer.n_target = n_target; steer.tol_n = tol_n;
+        steer.slack = 1e-10 * (double)std::max<int64_t>(p->info.n_basis, 1);
+        if ((s = evaluate(p, d_vals_in, mu, eps, b, cap, &ev, &nc, st, early ? &steer : nullptr))) return s;
         double g = ev.n_elec - n_target;
-        if (nc > 0 && cap <= p->opt.max_iter && std::fabs(g) <= std::max(tol_n, 0.0) + 1e-300) {
+        const bool partial = steer.decided != 0;  // direction proven, sign function not converged
+        if (!partial && nc > 0 && cap <= p->opt.max_iter && std::fabs(g) <= std::max(tol_n, 0.0) + 1e-300) {
             // a capped evaluation may not accept: finish this one to convergence first
             int launched = 0, all_done = 0;
             if ((s = ns_loop(p, b, eps, p->opt.max_iter + 1, &all_done, &launched, st))) return s;
@@ -475,28 +543,38 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         accumulate(ev);
         S->mu_trace[steps] = mu;
         S->ne_trace[steps] = ev.n_elec;
+        S->ne_err_trace[steps] = partial ? steer.err : 0.0;
+        S->iter_trace[steps] = ev.iterations;
         last_nc = nc;
-        if (std::fabs(g) < std::fabs(best_g)) { best_g = g; best_mu = mu; best_step = steps; }
+        last_partial = partial;
+        // |g| of a partial step is only known up to its bound: rank it by the pessimistic end
+        const double g_rank = std::fabs(g) + (partial ? steer.err : 0.0);
+        if (g_rank < std::fabs(best_g)) { best_g = g_rank; best_mu = mu; best_step = steps; }
         ++steps;
-        if (std::fabs(g) <= tol_n) { accepted = true; break; }
+        if (!partial && std::fabs(g) <= tol_n) { accepted = true; break; }
         if (g < 0) lo = std::max(lo, mu); else hi = std::min(hi, mu);
         if (hi - lo <= p->opt.mu_tol) break;
         mu = 0.5 * (lo + hi);
     }
     // the workspace holds the last evaluated mu; re-evaluate if the best one was an earlier step
-    // or if the last evaluation was capped before convergence
-    if (best_step != steps - 1 || (last_nc > 0 && cap <= p->opt.max_iter)) {
+    // or if the last evaluation ended before convergence (capped or steering-only)
+    if (best_step != steps - 1 || last_partial || (last_nc > 0 && cap <= p->opt.max_iter)) {
         memset(&ev, 0, sizeof(ev));
         if ((s = evaluate(p, d_vals_in, best_mu, eps, b, p->opt.max_iter + 1, &ev, &nc, st))) return s;
         last_nc = nc;
         accumulate(ev);
     }
-    double tr_mu[64], tr_ne[64];
+    double tr_mu[64], tr_ne[64], tr_err[64];
+    int32_t tr_it[64];
     memcpy(tr_mu, S->mu_trace, sizeof(tr_mu));
     memcpy(tr_ne, S->ne_trace, sizeof(tr_ne));
+    memcpy(tr_err, S->ne_err_trace, sizeof(tr_err));
+    memcpy(tr_it, S->iter_trace, sizeof(tr_it));
     *S = ev;
     memcpy(S->mu_trace, tr_mu, sizeof(tr_mu));
     memcpy(S->ne_trace, tr_ne, sizeof(tr_ne));
+    memcpy(S->ne_err_trace, tr_err, sizeof(tr_err));
+    memcpy(S->iter_trace, tr_it, sizeof(tr_it));
     S->mu = best_mu;
     S->mu_steps = steps;
     S->tot_sum_iter_n3 = acc_n3; S->tot_sym_flop = acc_sym; S->tot_gemm_launches = acc_launch;

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "submatrix.h"
@@ -94,6 +95,12 @@ struct sm_plan {
     int32_t* h_pinned = nullptr;           // pinned host mirror for counters
     double* h_pinned_d = nullptr;          // pinned host scalars
     int cur_k = 0;                         // completed Newton-Schulz updates of the last evaluation
+    double* d_bound = nullptr;             // [max_iter+2][2] per iteration: n_elec(X_k), its error bound
+    double* d_bound_part = nullptr;        // [2][ngroups] per-group partials of the two
+    double* h_bound = nullptr;             // pinned mirror of d_bound
+    double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
+    double lz_lo = 0.0, lz_hi = 0.0;       // estimated [lambda_min, lambda_max] of K~ (widened)
+    int lz_valid = 0;                      // lz_lo / lz_hi belong to the current call's values
     // --- staging for the *_host entry points
     double *d_stage_in = nullptr, *d_stage_out = nullptr;
     // --- misc
@@ -118,6 +125,11 @@ sm_status_t launch_scatter(sm_plan* p, int as_identity, const double* buf0, cons
 sm_status_t launch_nelec(sm_plan* p, const double* buf0, const double* buf1, cudaStream_t st);
 sm_status_t launch_trace_dk(sm_plan* p, const double* D, const double* K, cudaStream_t st);
 sm_status_t launch_gersh_global(sm_plan* p, const double* vals, cudaStream_t st);
+sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const double* buf1, const double* bufY,
+                               cudaStream_t st);
+// spectral.cu
+sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st);
+sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStream_t st);
 // ns_sign.cu
 sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
                            double* bufY, cudaStream_t st);

@@ -410,6 +410,63 @@ sm_status_t launch_nelec(sm_plan* p, const double* buf0, const double* buf1, cud
     return SM_OK;
 }
 
+// Steering bound of the mu bisection (reading A11c).  After MODE 0 of iteration k >= 1 the
+// workspace holds X_k and Y_k = X_k^2, all eigenvalues x_l of X_k lie in [-1,1] and move monotonically
+// towards +-1, so with w_l = sum_{k in gen} Q_kl^2 (Algorithm 1)
+//   |n_elec(final) - n_elec(X_k)| <= 1/2 sum_l w_l (1 - |x_l|) <= 1/2 sum_l w_l (1 - x_l^2)
+//                                   = 1/2 sum_{k in gen} (1 - (Y_k)_kk).
+// part[g] = n_elec partial of X_k, part[ngroups + g] = bound partial; one warp per group.
+__global__ void k_nelec_bound(int ngroups, const int32_t* __restrict__ grp_ptr, const int32_t* __restrict__ grp_cols,
+                              const int32_t* __restrict__ blk_size, const int32_t* __restrict__ gen_off,
+                              const int32_t* __restrict__ ldv, const int64_t* __restrict__ ws_off,
+                              const int32_t* __restrict__ done_iter, const unsigned long long* __restrict__ gersh,
+                              int k, const double* __restrict__ buf0, const double* __restrict__ buf1,
+                              const double* __restrict__ bufY, double* __restrict__ part) {
+    const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (g >= ngroups) return;
+    const int lane = threadIdx.x & 31;
+    const int di = done_iter[g];
+    const int kb = di >= 0 ? di : k;
+    const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];
+    const double* Yg = bufY + ws_off[g];
+    const int ld = ldv[g];
+    double xs = 1.0;
+    if (kb == 0) {  // stopped at iteration 0: the buffer still holds the unscaled a_i - mu I
+        const double s = __longlong_as_double((long long)gersh[g]);
+        xs = s > 0.0 ? 1.0 / s : 1.0;
+    }
+    double a = 0.0, d = 0.0;
+    for (int gc = grp_ptr[g]; gc < grp_ptr[g + 1]; ++gc) {
+        const int c = grp_cols[gc];
+        const int o = gen_off[c], b = blk_size[c];
+        for (int e = lane; e < b; e += 32) {
+            const size_t off = panel_off(o + e, o + e, ld);
+            a += 0.5 * (1.0 - xs * Xg[off]);
+            d += 0.5 * fmax(1.0 - Yg[off], 0.0);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        d += __shfl_xor_sync(0xffffffffu, d, o);
+    }
+    if (lane == 0) { part[g] = a; part[ngroups + g] = d; }
+}
+
+// Called after the launch pair of iteration k >= 1 (MODE 1 touches neither X_k nor Y_k).
+sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const double* buf1, const double* bufY,
+                               cudaStream_t st) {
+    if (p->ngroups == 0) return SM_OK;
+    k_nelec_bound<<<(p->ngroups + 7) / 8, 256, 0, st>>>(p->ngroups, p->d_grp_ptr, p->d_grp_cols, p->d_blk_size,
+                                                        p->d_gen_off, p->d_ld, p->d_ws_off, p->d_done_iter, p->d_gersh,
+                                                        k, buf0, buf1, bufY, p->d_bound_part);
+    k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part, p->ngroups, p->d_bound + 2 * k);
+    k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part + p->ngroups, p->ngroups, p->d_bound + 2 * k + 1);
+    p->launches += 3;
+    SM_CUDA(cudaGetLastError());
+    return SM_OK;
+}
+
 // tr(D) and tr(D K) (Eq.(18), Eq.(10)).  Stage 1: each CTA reduces a fixed contiguous
 // slice of the value arrays (and the diagonal entries of the diagonal blocks it owns by block
 // column); stage 2: k_sum_fixed.

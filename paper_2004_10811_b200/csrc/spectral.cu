@@ -1,0 +1,198 @@
+// a4 spectral bound, option scaling = 1 ("interlacing"): every a_i is a PRINCIPAL submatrix of the
+// symmetric K~, so by Cauchy interlacing  lambda_min(K~) <= lambda(a_i) <= lambda_max(K~)
+// and  rho(a_i - mu I) <= max(|lambda_max(K~) - mu|, |lambda_min(K~) - mu|)  for EVERY submatrix and
+// EVERY mu of the bisection.  The two extreme eigenvalues of the block-sparse K~ are estimated once
+// per call by a short Lanczos run (block-CSC mat-vec, deterministic reductions) and widened by a
+// safety margin; Newton-Schulz converges for any rho/s < sqrt(3), so the margin guards iteration
+// counts, not correctness (reading A8).  All arithmetic runs on the device; the host
+// only sequences the launches and reads the two resulting doubles.
+#include "common.cuh"
+
+namespace smb {
+
+constexpr int LZ_STEPS = 32;
+
+// y = K x for the symmetric block-CSC K~: y_c = sum_{(r,c) stored} K[r,c]^T x_r, one warp per block
+// column (no atomics); lane b takes every 32nd block of the column.  part[c] = y_c . x_c.
+__global__ void __launch_bounds__(256)
+k_lz_spmv(int nb, const int32_t* __restrict__ blk_size, const int32_t* __restrict__ blk_off,
+          const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx,
+          const int64_t* __restrict__ val_off, const double* __restrict__ vals, const double* __restrict__ x,
+          double* __restrict__ y, double* __restrict__ part) {
+    const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (c >= nb) return;
+    const int lane = threadIdx.x & 31;
+    const int bc = blk_size[c], oc = blk_off[c];
+    const int64_t p0 = colptr[c], p1 = colptr[c + 1];
+    double dot = 0.0;
+    for (int q = 0; q < bc; ++q) {
+        double a = 0.0;
+        for (int64_t b = p0 + lane; b < p1; b += 32) {
+            const int r = rowidx[b];
+            const int br = blk_size[r];
+            const double* col = vals + val_off[b] + (size_t)q * br;
+            const double* xr = x + blk_off[r];
+            for (int e = 0; e < br; ++e) a = fma(col[e], xr[e], a);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+        if (lane == 0) y[oc + q] = a;
+        dot = fma(a, x[oc + q], dot);
+    }
+    if (lane == 0) part[c] = dot;
+}
+
+// Deterministic 1-CTA sum; mode 0: out = sum, mode 1: out = sqrt(sum).
+__global__ void k_lz_reduce(const double* __restrict__ in, int n, double* __restrict__ out, int mode) {
+    __shared__ double s[1024];
+    double a = 0.0;
+    for (int i = threadIdx.x; i < n; i += 1024) a += in[i];
+    s[threadIdx.x] = a;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = mode ? sqrt(s[0]) : s[0];
+}
+
+// w = w - alpha v - beta_prev v_prev; part[block] = partial ||w||^2 (fixed order inside the CTA).
+__global__ void __launch_bounds__(256)
+k_lz_axpy(int64_t n, double* __restrict__ w, const double* __restrict__ v, const double* __restrict__ vprev,
+          const double* __restrict__ alpha, const double* __restrict__ beta_prev, double* __restrict__ part) {
+    __shared__ double s[256];
+    const double al = *alpha, be = beta_prev ? *beta_prev : 0.0;
+    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t b = (int64_t)blockIdx.x * per, e = min(b + per, n);
+    double a = 0.0;
+    for (int64_t i = b + threadIdx.x; i < e; i += 256) {
+        const double t = w[i] - al * v[i] - be * vprev[i];
+        w[i] = t;
+        a = fma(t, t, a);
+    }
+    s[threadIdx.x] = a;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[blockIdx.x] = s[0];
+}
+
+// vnext = w / beta (zero vector after a breakdown: the run then appends decoupled zeros to T,
+// which can only widen the interval).
+__global__ void k_lz_scale(int64_t n, const double* __restrict__ w, const double* __restrict__ beta,
+                           double* __restrict__ vnext) {
+    const double be = *beta;
+    const double inv = be > 1e-300 ? 1.0 / be : 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        vnext[i] = w[i] * inv;
+}
+
+// Start vector: +-1/sqrt(n) by an integer hash of the index (deterministic, not orthogonal to
+// anything in particular).
+__global__ void k_lz_start(int64_t n, double* __restrict__ v, double* __restrict__ vprev) {
+    const double a = rsqrt((double)n);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        unsigned h = (unsigned)i * 2654435761u;
+        h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
+        v[i] = (h & 1u) ? a : -a;
+        vprev[i] = 0.0;
+    }
+}
+
+// Extreme eigenvalues of the k x k Lanczos tridiagonal T (diag alpha, off-diagonal beta) by
+// bisection on Sturm counts, widened by margin * spread.  One thread; k <= LZ_STEPS.
+__global__ void k_lz_extremes(int k, const double* __restrict__ alpha, const double* __restrict__ beta,
+                              double margin, double* __restrict__ out) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double glo = 1e300, ghi = -1e300;
+    for (int i = 0; i < k; ++i) {
+        const double r = (i > 0 ? fabs(beta[i - 1]) : 0.0) + (i + 1 < k ? fabs(beta[i]) : 0.0);
+        glo = fmin(glo, alpha[i] - r);
+        ghi = fmax(ghi, alpha[i] + r);
+    }
+    auto count_below = [&](double x) {  // eigenvalues of T smaller than x
+        int cnt = 0;
+        double d = 1.0;
+        for (int i = 0; i < k; ++i) {
+            const double b2 = i > 0 ? beta[i - 1] * beta[i - 1] : 0.0;
+            d = alpha[i] - x - (i > 0 ? b2 / d : 0.0);
+            if (d == 0.0) d = -1e-300;
+            if (d < 0.0) ++cnt;
+        }
+        return cnt;
+    };
+    double lo = glo, hi = ghi;  // smallest eigenvalue: first x with count_below(x) >= 1
+    for (int it = 0; it < 200; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (count_below(mid) >= 1) hi = mid; else lo = mid;
+    }
+    const double emin = lo;
+    lo = glo; hi = ghi;         // largest eigenvalue: first x with count_below(x) >= k
+    for (int it = 0; it < 200; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (count_below(mid) >= k) hi = mid; else lo = mid;
+    }
+    const double emax = hi;
+    const double spread = emax - emin;
+    out[0] = emin - margin * spread;
+    out[1] = emax + margin * spread;
+}
+
+// s_g <- min(Gershgorin_g, cap) / overshoot  (in place, bits of a double as written by k_gather).
+__global__ void k_apply_scale(int ng, unsigned long long* __restrict__ gersh, double cap, double inv_overshoot) {
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ng) return;
+    double s = __longlong_as_double((long long)gersh[g]);
+    if (cap > 0.0 && cap < s) s = cap;
+    s *= inv_overshoot;
+    gersh[g] = (unsigned long long)__double_as_longlong(s);
+}
+
+sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStream_t st) {
+    if (p->ngroups == 0) return SM_OK;
+    k_apply_scale<<<(p->ngroups + 255) / 256, 256, 0, st>>>(p->ngroups, p->d_gersh, cap, 1.0 / overshoot);
+    p->launches++;
+    SM_CUDA(cudaGetLastError());
+    return SM_OK;
+}
+
+// Lanczos estimate of [lambda_min, lambda_max] of K~ -> p->lz_lo / p->lz_hi (host), widened by 3 %
+// of the spread.  ~5 small launches per step, LZ_STEPS steps.
+sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st) {
+    const int64_t n = p->info.n_basis;
+    if (n == 0 || p->nb == 0) { p->lz_lo = p->lz_hi = 0.0; return SM_OK; }
+    if (!p->d_lz) SM_CUDA(cudaMalloc((void**)&p->d_lz, (size_t)(3 * n + 2 * LZ_STEPS + 8 + std::max<int64_t>(p->nb, 1024)) * 8));
+    double* vb[3] = {p->d_lz, p->d_lz + n, p->d_lz + 2 * n};
+    double* alpha = p->d_lz + 3 * n;
+    double* beta = alpha + LZ_STEPS;
+    double* outp = beta + LZ_STEPS;
+    double* part = outp + 8;
+    const int steps = (int)std::min<int64_t>(LZ_STEPS, n);
+    const int ew = (int)std::min<int64_t>((n + 255) / 256, 592);
+    const int nred = 296;
+    double *vprev = vb[0], *v = vb[1], *w = vb[2];
+    k_lz_start<<<ew, 256, 0, st>>>(n, v, vprev);
+    p->launches++;
+    for (int j = 0; j < steps; ++j) {
+        k_lz_spmv<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_blk_size, p->d_blk_off, p->d_colptr, p->d_rowidx,
+                                                   p->d_val_off, vals, v, w, part);
+        k_lz_reduce<<<1, 1024, 0, st>>>(part, p->nb, alpha + j, 0);
+        k_lz_axpy<<<nred, 256, 0, st>>>(n, w, v, vprev, alpha + j, j > 0 ? beta + j - 1 : nullptr, part);
+        k_lz_reduce<<<1, 1024, 0, st>>>(part, nred, beta + j, 1);
+        k_lz_scale<<<ew, 256, 0, st>>>(n, w, beta + j, vprev);
+        p->launches += 5;
+        double* t = vprev; vprev = v; v = t;  // v_{j+1} was written over v_{j-1}
+    }
+    k_lz_extremes<<<1, 32, 0, st>>>(steps, alpha, beta, 0.03, outp);
+    p->launches++;
+    SM_CUDA(cudaGetLastError());
+    SM_CUDA(cudaMemcpyAsync(p->h_pinned_d + 6, outp, 16, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    p->lz_lo = p->h_pinned_d[6];
+    p->lz_hi = p->h_pinned_d[7];
+    return SM_OK;
+}
+
+}  // namespace smb

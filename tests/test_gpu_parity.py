@@ -232,12 +232,12 @@ def test_tiny_and_degenerate(B, oracle):
     m = W.BlockSparseSym(1, np.array([1], np.int32), np.array([0, 1], np.int64), np.array([0], np.int32),
                          np.array([-0.7]), np.array([0, 1], np.int32), np.array([0], np.int32))
     plan, st, d, stats, _, _ = _run_sign(B, m)
-    assert st == B.SM_OK and d[0] == 1.0
+    assert st == B.SM_OK and abs(d[0] - 1.0) <= 1e-12  # converged to eps = 1e-12, any scale
     B.sm_plan_destroy(plan)
     # already-involutory input: converges at iteration 0 (scatter applies 1/s)
     a = np.array([[0.0, 2.0], [2.0, 0.0]])  # Gershgorin bound 2 = spectral radius: X0 = A/2 is involutory
     m = W.dense_batch_as_blocks(a[None])
-    plan, st, d, stats, _, _ = _run_sign(B, m)
+    plan, st, d, stats, _, _ = _run_sign(B, m, opt=B.default_options(scaling=0))
     assert st == B.SM_OK and stats.iter_max == 0
     assert np.allclose(d.reshape(2, 2), 0.5 * (np.eye(2) - a / 2), atol=1e-15)
     B.sm_plan_destroy(plan)
@@ -321,16 +321,20 @@ def test_structure_errors(B):
 
 
 # ------------------------------------------------------------------------------ a7 + a8 bisection
-def test_density_matrix_bisection_config0(B, oracle, cfg0):
-    """Algorithm 1 / reading A11-A12: same bisection trace as the oracle's (which uses stored
-    eigendecompositions), same plateau; D~ parity at the GPU's final mu."""
+@pytest.mark.parametrize("early_out", [1, 0])
+@pytest.mark.parametrize("scaling", [1, 0])
+def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling):
+    """Algorithm 1 / readings A11-A12: same bisection trace as the oracle's (which uses stored
+    eigendecompositions), same plateau; D~ parity at the GPU's final mu.  With early_out (A11c) a
+    steering step reports the count of its last iterate and a bound: the oracle's converged count
+    must lie inside it, on the same side of the target, and the mu trace must not change."""
     torch = _torch()
     m = cfg0
     idx = oracle.Index(m)
     lam, w, ptr, g = oracle.eig_groups(idx, m.values)
     lo, hi = oracle.gershgorin_interval(m)
     for mu0, tol_n in ((-1.0, 0.5), (1.2, 0.5)):
-        plan = B.plan_from_matrix(m)
+        plan = B.plan_from_matrix(m, B.default_options(early_out=early_out, scaling=scaling))
         ws = B.alloc_workspace(plan)
         vin = torch.from_numpy(m.values).cuda()
         vout = torch.empty_like(vin)
@@ -340,12 +344,59 @@ def test_density_matrix_bisection_config0(B, oracle, cfg0):
         mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0, lo, hi, tol_n)
         assert st == B.SM_OK
         assert stats.mu_steps == len(trace_o)
+        n_partial = 0
         for k, (mo, no) in enumerate(trace_o):
             assert abs(stats.mu_trace[k] - mo) <= 1e-12 * max(1, abs(mo))  # same bracket (Gershgorin) and midpoints
+            err = stats.ne_err_trace[k]
+            if err > 0.0:  # steering step: proven side, converged count inside the bound
+                n_partial += 1
+                assert early_out == 1
+                assert abs(stats.ne_trace[k] - no) <= err + 1e-9
+                assert abs(stats.ne_trace[k] - m.n_occ) > err + tol_n
+                assert (stats.ne_trace[k] > m.n_occ) == (no > m.n_occ)
+            else:
+                assert abs(stats.ne_trace[k] - no) <= 1e-9
+        if early_out:
+            assert n_partial >= 1 and stats.ne_err_trace[stats.mu_steps - 1] == 0.0
+            assert stats.iter_trace[0] < stats.iter_trace[stats.mu_steps - 1]  # mu0 inside a band: decided early
         assert abs(stats.n_elec - ne_o) <= 1e-9  # same plateau
         d_or = oracle.density(idx, m.values, mu)
         assert np.abs(vout.cpu().numpy() - d_or).max() <= TOL_D
         B.sm_plan_destroy(plan)
+
+
+def test_interlacing_bound_encloses_spectrum(B, cfg0):
+    """scaling = 1: the widened Lanczos estimate must enclose LAPACK's spectrum of the dense K~
+    (so that, by Cauchy interlacing, it bounds every principal submatrix) without being loose."""
+    for m in (cfg0, W.water_like(64, "DZVP", 5.0, seed=3), W.random_block_pattern(40, 0.2, 7, seed=5)):
+        lam = np.linalg.eigvalsh(m.to_dense())
+        plan, st, d, stats, ws, vin = _run_sign(B, m, mu=0.0, opt=B.default_options(scaling=1))
+        spread = lam[-1] - lam[0]
+        assert stats.spec_lo <= lam[0] and stats.spec_hi >= lam[-1]
+        assert lam[0] - stats.spec_lo <= 0.08 * spread and stats.spec_hi - lam[-1] <= 0.08 * spread
+        B.sm_plan_destroy(plan)
+
+
+@pytest.mark.parametrize("scaling", [0, 1])
+def test_scaling_modes_agree(B, oracle, cfg0, scaling):
+    """Reading A8: the sign function is scale invariant; the interlacing bound (scaling = 1, with
+    overshoot) must give the oracle's D~ like the Gershgorin bound, in fewer iterations."""
+    m = cfg0
+    idx = oracle.Index(m)
+    d_or = oracle.density(idx, m.values, 0.1)
+    its = {}
+    for ov in (1.0, 1.25, 1.5):
+        plan, st, d, stats, ws, vin = _run_sign(B, m, mu=0.1, opt=B.default_options(scaling=scaling, overshoot=ov))
+        assert st == B.SM_OK
+        assert np.abs(d - d_or).max() <= TOL_D
+        its[ov] = stats.iter_max
+        B.sm_plan_destroy(plan)
+    if scaling == 0:
+        assert its[1.0] == its[1.25] == its[1.5]  # overshoot only applies to scaling = 1
+    test_scaling_modes_agree.its = getattr(test_scaling_modes_agree, "its", {})
+    test_scaling_modes_agree.its[scaling] = its
+    if scaling == 1 and 0 in test_scaling_modes_agree.its:
+        assert its[1.25] < test_scaling_modes_agree.its[0][1.0]
 
 
 def test_density_matrix_unreachable_tolerance_is_guarded(B, cfg0):
