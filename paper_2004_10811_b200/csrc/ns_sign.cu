@@ -71,6 +71,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+// Producer-side wait: back off between polls so that the single producer thread does not take issue
+// slots from the consumer warp that shares its SM sub-partition.
+#ifndef SM_PROD_SLEEP
+#define SM_PROD_SLEEP 0
+#endif
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, unsigned parity) {
+    const unsigned a = smem_u32(bar);
+    for (;;) {
+        unsigned ok;
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        if (ok) return;
+        if (SM_PROD_SLEEP > 0) __nanosleep(SM_PROD_SLEEP);
+    }
+}
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
                      smem_u32(dst)),
@@ -110,14 +129,26 @@ __device__ __forceinline__ void mbar_arrive_a(unsigned bar) {
 //
 // Rectangular tile: M valid row sub-tiles x this warp's 2 column sub-tiles, acc[2 mt + nt].
 // fold >= 0: this panel holds the tile's own column sub-tile `fold` (MODE 1: acc += -3 x).
+#ifndef SM_VLOAD
+#define SM_VLOAD 0
+#endif
+__device__ __forceinline__ double2 lds2(const double* p) {
+#if SM_VLOAD
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(smem_u32(p)));
+    return v;
+#else
+    return *reinterpret_cast<const double2*>(p);
+#endif
+}
 template <int M>
 __device__ __forceinline__ void panel_rect(double (&acc)[16][2], const double* __restrict__ Ap,
                                            const double* __restrict__ Bp) {
     double2 bf[2], af[M];
 #pragma unroll
-    for (int nt = 0; nt < 2; ++nt) bf[nt] = *reinterpret_cast<const double2*>(Bp + nt * 64);
+    for (int nt = 0; nt < 2; ++nt) bf[nt] = lds2(Bp + nt * 64);
 #pragma unroll
-    for (int mt = 0; mt < M; ++mt) af[mt] = *reinterpret_cast<const double2*>(Ap + mt * 64);
+    for (int mt = 0; mt < M; ++mt) af[mt] = lds2(Ap + mt * 64);
 #pragma unroll
     for (int mt = 0; mt < M; ++mt)
 #pragma unroll
@@ -211,49 +242,36 @@ __device__ __forceinline__ void fold_diag(double (&acc)[16][2], const double* __
     }
 }
 
-// k loop of one tile for one consumer warp.  `variant` is the warp's work shape for this tile
-// (0 idle, 1..8 rect<M>, 9..12 diag<W>); per stage: wait, its k panels (two, or one in the last
-// stage of an odd panel count), release.  One panel body per shape, dispatched by a warp-uniform
-// switch, keeps the kernel within the instruction cache.  The first stage of the tile has already
-// been waited for by the caller (it carries the TileInfo).
-template <int MODE>
-__device__ __forceinline__ void k_loop(double (&acc)[16][2], const double* smem, unsigned full0, unsigned empty0,
-                                       int& stage, unsigned& phase, int KP, int ja, int jb, bool b_is_a,
-                                       int frag_off, int wid, int lane, int kp_col0, int s_rows, int variant) {
+// k loop of one tile for one consumer warp, specialised per work shape VAR (1..8 rect<M>, 9..12
+// diag<W>, 0 idle): the shape is dispatched ONCE per tile, so the loop over the k panels carries
+// only its own panel body, the stage hand-over every second panel and (MODE 1) the fold test.
+// Per stage: wait "full", its k panels (two, or one in the last stage of an odd panel count),
+// release "empty".  The first stage of the tile has already been waited for by the caller (it
+// carries the TileInfo).
+template <int MODE, int VAR>
+__device__ __forceinline__ void k_loop_var(double (&acc)[16][2], const double* smem, unsigned full0, unsigned empty0,
+                                           int& stage, unsigned& phase, int KP, int ja, int jb, bool b_is_a,
+                                           int frag_off, int wid, int lane, int kp_col0, int s_rows) {
     const int KT = (KP + 1) >> 1;
-    const int boff = frag_off + (variant <= 8 ? wid * 128 : 0);
+    const int boff = frag_off + ((VAR <= 8 || VAR == 13) ? wid * 128 : 0);
 #pragma unroll 1
     for (int kt = 0; kt < KT; ++kt) {
         if (kt > 0) mbar_wait_a(full0 + 8u * stage, phase);
-        if (variant != 0) {
+        if (VAR != 0) {
             const double* sa = smem + (size_t)stage * STAGE_DOUBLES;
             const double* Ap = sa + frag_off;
             const double* Bp = (b_is_a ? sa : sa + BM * BK) + boff;
             const int nj = min(2, KP - 2 * kt);
 #pragma unroll 1
             for (int j = 0; j < nj; ++j, Ap += ja, Bp += jb) {
-                switch (variant) {
-                    case 8: panel_rect<8>(acc, Ap, Bp); break;
-                    case 7: panel_rect<7>(acc, Ap, Bp); break;
-                    case 6: panel_rect<6>(acc, Ap, Bp); break;
-                    case 5: panel_rect<5>(acc, Ap, Bp); break;
-                    case 4: panel_rect<4>(acc, Ap, Bp); break;
-                    case 3: panel_rect<3>(acc, Ap, Bp); break;
-                    case 2: panel_rect<2>(acc, Ap, Bp); break;
-                    case 1: panel_rect<1>(acc, Ap, Bp); break;
-                    case 9: panel_diag<0>(acc, Ap, Bp); break;
-                    case 10: panel_diag<1>(acc, Ap, Bp); break;
-                    case 11: panel_diag<2>(acc, Ap, Bp); break;
-                    default: panel_diag<3>(acc, Ap, Bp); break;
-                }
+                if (VAR >= 1 && VAR <= 8) panel_rect<(VAR >= 1 && VAR <= 8) ? VAR : 1>(acc, Ap, Bp);
+                else if (VAR == 13) panel_rect_dyn(acc, Ap, Bp, s_rows);
+                else panel_diag<(VAR >= 9 && VAR <= 12) ? VAR - 9 : 0>(acc, Ap, Bp);
                 if (MODE == 1) {
                     const int sc = 2 * kt + j - kp_col0;
                     if ((unsigned)sc < 8u) {
-                        if (variant <= 8) fold_rect(acc, Ap, s_rows, wid, sc);
-                        else if (variant == 9) fold_diag<0>(acc, Ap, sc);
-                        else if (variant == 10) fold_diag<1>(acc, Ap, sc);
-                        else if (variant == 11) fold_diag<2>(acc, Ap, sc);
-                        else fold_diag<3>(acc, Ap, sc);
+                        if (VAR <= 8 || VAR == 13) fold_rect(acc, Ap, VAR <= 8 ? VAR : s_rows, wid, sc);
+                        else fold_diag<(VAR >= 9 && VAR <= 12) ? VAR - 9 : 0>(acc, Ap, sc);
                     }
                 }
             }
@@ -261,6 +279,107 @@ __device__ __forceinline__ void k_loop(double (&acc)[16][2], const double* smem,
         __syncwarp();
         if (lane == 0) mbar_arrive_a(empty0 + 8u * stage);
         if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    }
+}
+
+// ---- epilogue of one tile.  k8-panel offsets of this thread's elements (common.cuh): all rows of
+// the tile sit in one row-tile, all its columns (as mirror rows) in another, so an element of
+// sub-tile (sr, sc) is at  base_d + sc * pd + sr * 64  and its mirror at  base_m + sr * pm + sc * 64
+// (+8 for the next column).
+struct EpiCtx {
+    double* Out;
+    double scale;  // MODE 0: alpha; MODE 1: b (acc = X Y - 3 X -> X' = b acc)
+    int base_d, base_m, pd, pm;
+    int rlim;      // n - row0 - lr: rows sr*8 < rlim count for the residual (n x n part only)
+};
+// sub-tile strictly below the matrix diagonal: both elements stored, mirrored, counted twice
+template <int MODE>
+__device__ __forceinline__ void store_below(const EpiCtx& c, const double (&a)[2], int sr, int sc, double& part) {
+    const double v0 = a[0] * c.scale, v1 = a[1] * c.scale;
+    *reinterpret_cast<double2*>(c.Out + (c.base_d + sc * c.pd + sr * 64)) = make_double2(v0, v1);
+    double* pm_ = c.Out + (c.base_m + sr * c.pm + sc * 64);
+    pm_[0] = v0;
+    pm_[8] = v1;
+    if (MODE == 0 && sr * 8 < c.rlim) part = fma(2.0 * v0, v0, fma(2.0 * v1, v1, part));
+}
+// sub-tile on the matrix diagonal (sr == sc of a diagonal tile): lower triangle only
+template <int MODE>
+__device__ __forceinline__ void store_ondiag(const EpiCtx& c, const double (&a)[2], int sr, int lr, int lk,
+                                             double& part) {
+    double* pd_ = c.Out + (c.base_d + sr * c.pd + sr * 64);
+    double* pm_ = c.Out + (c.base_m + sr * c.pm + sr * 64);
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const int cq = 2 * lk + q;
+        if (cq > lr) continue;  // upper triangle: its mirror image is stored
+        const double v = a[q] * c.scale;
+        pd_[q] = v;
+        if (cq != lr) pm_[q * 8] = v;
+        if (MODE == 0 && sr * 8 < c.rlim) {
+            const double d = v - (cq == lr ? 1.0 : 0.0);
+            part = fma((cq == lr ? 1.0 : 2.0) * d, d, part);
+        }
+    }
+}
+
+struct TileGeo {
+    int64_t ws_off;
+    double* out;
+    const unsigned long long* gersh;
+    int ld, n, row0, col0, grp, k;
+};
+
+// One tile for one consumer warp: k loop + epilogue, specialised per work shape
+//   VAR 1..8  rect<M> of an OFF-diagonal tile (no triangle tests in the epilogue)
+//   VAR 9..12 diag<W> of a full diagonal tile
+//   VAR 13    the small last diagonal tile (s_rows < 8 at run time; warps past the matrix idle)
+//   VAR 0     idle warp of a small diagonal tile (takes part in the stage hand-over only)
+template <int MODE, int VAR>
+__device__ __forceinline__ void tile_var(double (&acc)[16][2], const double* smem, unsigned full0, unsigned empty0,
+                                         int& stage, unsigned& phase, int KP, int ja, int jb, bool b_is_a,
+                                         int frag_off, int wid, int lane, int kp_col0, int s_rows,
+                                         const TileGeo& t, double& part) {
+    k_loop_var<MODE, VAR>(acc, smem, full0, empty0, stage, phase, KP, ja, jb, b_is_a, frag_off, wid, lane, kp_col0,
+                          s_rows);
+    if (VAR == 0) return;
+    const int lr = lane >> 2, lk = lane & 3;
+    EpiCtx c;  // built after the k loop: only the tile geometry stays live across it
+    c.scale = (MODE == 0) ? 1.0 : -0.5;
+    if (t.k == 0) {  // iteration 0 folds the spectral scale 1/s_i into the coefficients
+        double sg = __longlong_as_double((long long)t.gersh[t.grp]);
+        if (!(sg > 0.0)) sg = 1.0;
+        c.scale = (MODE == 0) ? 1.0 / (sg * sg) : -0.5 / sg;
+    }
+    c.Out = t.out + t.ws_off;
+    c.pd = min(BM, t.ld - t.row0) * 8;
+    c.pm = min(BN, t.ld - t.col0) * 8;
+    c.base_d = t.row0 * t.ld + kp_col0 * c.pd + lr * 8 + 2 * lk;
+    c.base_m = t.col0 * t.ld + (t.row0 >> 3) * c.pm + 2 * lk * 8 + lr;
+    c.rlim = t.n - t.row0 - lr;
+    if (VAR >= 1 && VAR <= 8) {
+#pragma unroll
+        for (int mt = 0; mt < (VAR <= 8 ? VAR : 0); ++mt)
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) store_below<MODE>(c, acc[2 * mt + nt], mt, 2 * wid + nt, part);
+    } else if (VAR >= 9 && VAR <= 12) {
+        constexpr int W = VAR >= 9 ? VAR - 9 : 0;
+#pragma unroll
+        for (int sc = 0; sc < W; ++sc) store_below<MODE>(c, acc[sc], W, sc, part);
+        store_ondiag<MODE>(c, acc[W], W, lr, lk, part);
+#pragma unroll
+        for (int sc = 0; sc < 7 - W; ++sc) store_below<MODE>(c, acc[W + 1 + sc], 7 - W, sc, part);
+        store_ondiag<MODE>(c, acc[8], 7 - W, lr, lk, part);
+    } else if (VAR == 13) {
+#pragma unroll
+        for (int mt = 0; mt < 7; ++mt) {
+            if (mt >= s_rows) break;
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) {
+                const int sc = 2 * wid + nt;
+                if (sc < mt) store_below<MODE>(c, acc[2 * mt + nt], mt, sc, part);
+                else if (sc == mt) store_ondiag<MODE>(c, acc[2 * mt + nt], mt, lr, lk, part);
+            }
+        }
     }
 }
 
@@ -341,7 +460,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
                 const double* Asrc = Xbase + ws_off + (size_t)row0 * ld;
                 const double* Bsrc = Bbase + ws_off + (size_t)col0 * ld;
                 for (int kt = 0; kt < KT; ++kt) {
-                    mbar_wait(&s_empty[stage], phase ^ 1);
+                    mbar_wait_backoff(&s_empty[stage], phase ^ 1);
                     const int nj = min(2, KP - 2 * kt);
                     if (kt == 0) {
                         TileInfo& ti_ = s_info[stage];
@@ -386,98 +505,66 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
         const bool full_diag = diag && s_rows == 8;
         const int rows_a = min(BM, si.ld - row0), rows_b = min(BN, si.ld - col0);
         const bool b_is_a = (MODE == 0) && diag;
-        // 0 idle, 1..8 rect<M>, 9..12 diag<W>
+        // work shape of this warp for this tile (see tile_var)
         int variant;
         if (full_diag) variant = 9 + wid;
-        else if (diag) variant = (2 * wid < s_rows) ? s_rows : 0;  // columns past the matrix
+        else if (diag) variant = (2 * wid < s_rows) ? 13 : 0;  // columns past the matrix: idle
         else variant = s_rows;
 #pragma unroll
         for (int e = 0; e < 16; ++e) acc[e][0] = acc[e][1] = 0.0;
-        {
-            const int KP = si.ld >> 3;
-            const int ja = rows_a * 8, jb = (b_is_a ? rows_a : rows_b) * 8;  // panel strides (doubles)
-            k_loop<MODE>(acc, smem, full0, empty0, stage, phase, KP, ja, jb, b_is_a, frag_off, wid, lane, kp_col0,
-                         s_rows, variant);
-        }
-
-        // ------------------------------------------------------------------ epilogue of the tile
-        const int g = si.grp, ld = si.ld, n = si.n;
-        double s = __longlong_as_double((long long)a.gersh[g]);
-        if (!(s > 0.0)) s = 1.0;
-        double alpha, cb;
-        if (k == 0) { alpha = 1.0 / (s * s); cb = -0.5 / s; }
-        else { alpha = 1.0; cb = -0.5; }
-        double* Out = ((MODE == 0) ? a.bufY : ((k & 1) ? a.buf0 : a.buf1)) + si.ws_off;
+        const int ld = si.ld;
+        TileGeo c;
+        c.ws_off = si.ws_off; c.out = (MODE == 0) ? a.bufY : ((k & 1) ? a.buf0 : a.buf1); c.gersh = a.gersh;
+        c.ld = ld; c.n = si.n; c.row0 = row0; c.col0 = col0; c.grp = si.grp; c.k = k;
         double part = 0.0;
-        // k8-panel offsets of this thread's elements (common.cuh): all rows of the tile sit in one
-        // row-tile, all its columns (as mirror rows) in another, so an element of sub-tile (sr, sc)
-        // is at  base_d + sc * pd + sr * 64  and its mirror at  base_m + sr * pm + sc * 64 (+8 for c+1).
-        const int pd = rows_a * 8, pm = min(BN, ld - col0) * 8;
-        const int base_d = row0 * ld + kp_col0 * pd + lr * 8 + 2 * lk;
-        const int base_m = col0 * ld + (row0 >> 3) * pm + 2 * lk * 8 + lr;
-        const double scale = (MODE == 0) ? alpha : cb;  // MODE 1: acc = X Y - 3 X -> X' = b acc
-#pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            int sr, sc;  // sub-tile row / column inside the CTA tile
-            bool valid;
-            if (full_diag) {
-                valid = e < 9;
-                if (e <= wid) { sr = wid; sc = e; } else { sr = 7 - wid; sc = e - wid - 1; }
-            } else {
-                sr = e >> 1; sc = 2 * wid + (e & 1);
-                valid = variant != 0 && sr < s_rows && (col0 + sc * 8) < ld;
+        {
+            const int KP = ld >> 3;
+            const int ja = rows_a * 8, jb = (b_is_a ? rows_a : rows_b) * 8;  // panel strides (doubles)
+#define SM_TV(V) case V: tile_var<MODE, V>(acc, smem, full0, empty0, stage, phase, KP, ja, jb, b_is_a, frag_off, wid, \
+                                          lane, kp_col0, s_rows, c, part); break;
+            switch (variant) {
+                SM_TV(1) SM_TV(2) SM_TV(3) SM_TV(4) SM_TV(5) SM_TV(6) SM_TV(7) SM_TV(8)
+                SM_TV(9) SM_TV(10) SM_TV(11) SM_TV(12) SM_TV(13)
+                default: tile_var<MODE, 0>(acc, smem, full0, empty0, stage, phase, KP, ja, jb, b_is_a, frag_off, wid,
+                                           lane, kp_col0, s_rows, c, part); break;
             }
-            if (!valid) continue;
-            const int r = row0 + sr * 8 + lr;
-            const int c = col0 + sc * 8 + 2 * lk;
-            double* pd_ = Out + (base_d + sc * pd + sr * 64);
-            double* pm_ = Out + (base_m + sr * pm + sc * 64);
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                const int cc = c + q;
-                if (cc > r) continue;  // upper triangle of a diagonal tile: its mirror image is stored
-                const double v = acc[e][q] * scale;
-                pd_[q] = v;
-                if (cc != r) pm_[q * 8] = v;
-                if (MODE == 0 && r < n) {  // residual over the n x n part; strictly-lower elements count twice
-                    const double d = v - (cc == r ? 1.0 : 0.0);
-                    part = fma((cc == r ? 1.0 : 2.0) * d, d, part);
-                }
-            }
+#undef SM_TV
         }
         if (MODE == 0) {
-            // Residual: every consumer warp publishes its partial of the tile; the warp that brings
-            // the submatrix's count to 4 x tile_count sums all partials in a fixed order and records
-            // the decision (deterministic; no CTA-wide barrier, no floating-point atomics).
+            // Residual: every consumer warp publishes its partial of the tile (plain store, no fence,
+            // no atomics); k_ns_decide sums them per submatrix in a fixed order after the launch.
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-            int is_last = 0;
-            if (lane == 0) {
-                a.partials[(size_t)si.tile * 4 + wid] = part;
-                __threadfence();
-                is_last = (atomicAdd(a.tile_done + g, 1) == 4 * si.tile_count - 1) ? 1 : 0;
-            }
-            is_last = __shfl_sync(0xffffffffu, is_last, 0);
-            if (is_last) {
-                __threadfence();
-                double r2 = 0.0;
-                const double* pp = a.partials + (size_t)si.tile_first * 4;
-                for (int t = lane; t < 4 * si.tile_count; t += 32) r2 += __ldcg(pp + t);
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
-                if (lane == 0) {
-                    const double r = sqrt(r2 / (double)(n > 0 ? n : 1));
-                    const double prev = k > 0 ? a.res[(size_t)((k - 1) & 1) * a.ngroups + g] : 1e300;
-                    const bool conv = r < a.eps;
-                    const bool stag = (k > 0) && (r >= prev) && (r < 1e-6);
-                    const bool stop = conv || stag || a.decide_only || !(r == r);
-                    a.res[(size_t)(k & 1) * a.ngroups + g] = r;
-                    a.tile_done[g] = 0;
-                    if (stop) { a.flag[g] = conv ? 0 : 1; a.done_iter[g] = k; }
-                    else atomicAdd(a.counters + k, 1);
-                }
-            }
+            if (lane == 0) a.partials[(size_t)si.tile * 4 + wid] = part;
         }
+    }
+}
+
+// Convergence decision of iteration k (reading A9), one warp per still-active submatrix: residual
+// r = sqrt(sum of its tile partials / n) in a fixed order (deterministic), then stop on r < eps,
+// on stagnation (r not decreasing below 1e-6), at max_iter, or on NaN.
+__global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __restrict__ tile_first,
+                                                   const int32_t* __restrict__ tile_count,
+                                                   const int32_t* __restrict__ sub_dim) {
+    const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (g >= a.ngroups) return;
+    if (a.done_iter[g] >= 0) return;
+    const int lane = threadIdx.x & 31, k = a.k;
+    const int cnt = 4 * tile_count[g], n = sub_dim[g];
+    const double* pp = a.partials + (size_t)tile_first[g] * 4;
+    double r2 = 0.0;
+    for (int t = lane; t < cnt; t += 32) r2 += pp[t];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+    if (lane == 0) {
+        const double r = sqrt(r2 / (double)(n > 0 ? n : 1));
+        const double prev = k > 0 ? a.res[(size_t)((k - 1) & 1) * a.ngroups + g] : 1e300;
+        const bool conv = r < a.eps;
+        const bool stag = (k > 0) && (r >= prev) && (r < 1e-6);
+        const bool stop = conv || stag || a.decide_only || !(r == r);
+        a.res[(size_t)(k & 1) * a.ngroups + g] = r;
+        if (stop) { a.flag[g] = conv ? 0 : 1; a.done_iter[g] = k; }
+        else atomicAdd(a.counters + k, 1);
     }
 }
 
@@ -499,7 +586,8 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * 3);
     a.sched = p->d_sched + 2 * k;
     k_ns_gemm<0><<<grid, NTHREADS, NS_SMEM, st>>>(a);
-    p->launches += 1;
+    k_ns_decide<<<(p->ngroups + 7) / 8, 256, 0, st>>>(a, p->d_tile_first, p->d_tile_count, p->d_sub_dim);
+    p->launches += 2;
     if (!decide_only) {
         a.sched = p->d_sched + 2 * k + 1;
         k_ns_gemm<1><<<grid, NTHREADS, NS_SMEM, st>>>(a);
