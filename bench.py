@@ -288,6 +288,9 @@ def main():
         st, mu = step_device()
     barrier()
     sampler = ClockSampler(local_rank) if rank == 0 else None
+    if sampler is not None:
+        time.sleep(1.5)  # let nvidia-smi finish attaching (its start-up stalls synchronous CUDA calls)
+        barrier()
     launches0 = B.sm_launch_count(plan)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     gemm_ms = gemm_launches = sym_flop = n3 = evals = 0.0

@@ -257,6 +257,7 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
     if (p->ngroups == 0) { *all_done = 1; return SM_OK; }
     const int max_iter = p->opt.max_iter;
     int k = p->cur_k;
+    p->half_iter = 0;
     int pending = -1;  // iteration whose counter copy is in flight
     auto poll = [&](int q) -> int {  // 1 = all converged, 2 = steering decision, 0 = go on
         if (p->h_pinned[q] == 0) { *all_done = 1; p->cur_k = q; return 1; }
@@ -272,31 +273,50 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
         }
         return 0;
     };
+    if (steer) {
+        // Steering evaluation: poll synchronously between MODE 0 and MODE 1 of every iteration k >= 1
+        // (a ~20 us bubble against a multi-ms launch), so that a proven direction stops the
+        // evaluation before the next update is even launched.
+        for (; k < k_end && k <= max_iter; ++k) {
+            const int last = k == max_iter ? 1 : 0;
+            sm_status_t s = launch_ns_pair(p, k, eps, last, b.b0, b.b1, b.y, st, 1);
+            if (s) return s;
+            (*launched) += 1;
+            SM_CUDA(cudaMemcpyAsync(p->h_pinned + k, p->d_counters + k, 4, cudaMemcpyDeviceToHost, st));
+            if (k >= 1) {
+                if ((s = launch_nelec_bound(p, k, b.b0, b.b1, b.y, st))) return s;
+                SM_CUDA(cudaMemcpyAsync(p->h_bound + 2 * k, p->d_bound + 2 * k, 16, cudaMemcpyDeviceToHost, st));
+            }
+            SM_CUDA(cudaStreamSynchronize(st));
+            const int r = poll(k);
+            if (r == 1) return SM_OK;                       // all converged: X_k is the result (cur_k = k)
+            if (r == 2) { p->cur_k = k; p->half_iter = 1; return SM_OK; }  // X_k in buf[k & 1], not converged
+            if (last) break;
+            if ((s = launch_ns_pair(p, k, eps, 0, b.b0, b.b1, b.y, st, 2))) return s;
+            (*launched) += 1;
+        }
+        p->cur_k = std::min(k, max_iter);
+        if (k >= max_iter) *all_done = 1;
+        return SM_OK;
+    }
     for (; k < k_end && k <= max_iter; ++k) {
         sm_status_t s = launch_ns_pair(p, k, eps, k == max_iter ? 1 : 0, b.b0, b.b1, b.y, st);
         if (s) return s;
         (*launched) += (k == max_iter) ? 1 : 2;
-        if (steer && k >= 1 && (s = launch_nelec_bound(p, k, b.b0, b.b1, b.y, st))) return s;
         if (pending >= 0) {
             SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
-            const int r = poll(pending);
-            if (r == 1) return SM_OK;
-            if (r == 2) { p->cur_k = std::min(k + 1, max_iter); return SM_OK; }
+            if (poll(pending) == 1) return SM_OK;
             pending = -1;
         }
         if ((k % p->opt.check_every) == 0 || k == max_iter || k == k_end - 1) {
             SM_CUDA(cudaMemcpyAsync(p->h_pinned + k, p->d_counters + k, 4, cudaMemcpyDeviceToHost, st));
-            if (steer && k >= 1)
-                SM_CUDA(cudaMemcpyAsync(p->h_bound + 2 * k, p->d_bound + 2 * k, 16, cudaMemcpyDeviceToHost, st));
             SM_CUDA(cudaEventRecord(p->ev_iter[k & 1], st));
             pending = k;
         }
     }
     if (pending >= 0) {
         SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
-        const int r = poll(pending);
-        if (r == 1) return SM_OK;
-        if (r == 2) { p->cur_k = std::min(k, max_iter); return SM_OK; }
+        if (poll(pending) == 1) return SM_OK;
     }
     // active submatrices have received k updates: their X lives in buf[k & 1]
     p->cur_k = std::min(k, max_iter);
@@ -328,8 +348,8 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         if (r == r) rmax = std::max(rmax, r); else rmax = INFINITY;
         int64_t n = p->h_sub_dim[i];
         // executed symmetric products: stopped at iteration it: one X^2 per tested iterate (it + 1)
-        // and one update per iteration (it); still active after cur_k launch pairs: 2 cur_k
-        const int64_t prods = di[i] >= 0 ? 2 * it + 1 : 2 * (int64_t)p->cur_k;
+        // and one update per iteration (it); still active after cur_k launch pairs: 2 cur_k (+1 if a steering decision came between the two modes)
+        const int64_t prods = di[i] >= 0 ? 2 * it + 1 : 2 * (int64_t)p->cur_k + p->half_iter;
         sin3 += prods * n * n * n;
         symf += prods * n * n * (n + 1);
     }

@@ -95,6 +95,7 @@ struct sm_plan {
     int32_t* h_pinned = nullptr;           // pinned host mirror for counters
     double* h_pinned_d = nullptr;          // pinned host scalars
     int cur_k = 0;                         // completed Newton-Schulz updates of the last evaluation
+    int half_iter = 0;                     // 1: MODE 0 of iteration cur_k ran, its MODE 1 did not (steering stop)
     double* d_bound = nullptr;             // [max_iter+2][2] per iteration: n_elec(X_k), its error bound
     double* d_bound_part = nullptr;        // [2][ngroups] per-group partials of the two
     double* h_bound = nullptr;             // pinned mirror of d_bound
@@ -132,5 +133,5 @@ sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t s
 sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStream_t st);
 // ns_sign.cu
 sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
-                           double* bufY, cudaStream_t st);
+                           double* bufY, cudaStream_t st, int which = 3);
 }  // namespace smb

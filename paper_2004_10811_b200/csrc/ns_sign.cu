@@ -568,8 +568,9 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
     }
 }
 
+// which: bit 0 = MODE 0 + decision of iteration k, bit 1 = MODE 1 (update) of iteration k.
 sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
-                           double* bufY, cudaStream_t st) {
+                           double* bufY, cudaStream_t st, int which) {
     if (p->n_tiles == 0) return SM_OK;
     static bool attr_set = false;
     if (!attr_set) {
@@ -585,10 +586,12 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * 3);
     a.sched = p->d_sched + 2 * k;
-    k_ns_gemm<0><<<grid, NTHREADS, NS_SMEM, st>>>(a);
-    k_ns_decide<<<(p->ngroups + 7) / 8, 256, 0, st>>>(a, p->d_tile_first, p->d_tile_count, p->d_sub_dim);
-    p->launches += 2;
-    if (!decide_only) {
+    if (which & 1) {
+        k_ns_gemm<0><<<grid, NTHREADS, NS_SMEM, st>>>(a);
+        k_ns_decide<<<(p->ngroups + 7) / 8, 256, 0, st>>>(a, p->d_tile_first, p->d_tile_count, p->d_sub_dim);
+        p->launches += 2;
+    }
+    if ((which & 2) && !decide_only) {
         a.sched = p->d_sched + 2 * k + 1;
         k_ns_gemm<1><<<grid, NTHREADS, NS_SMEM, st>>>(a);
         p->launches += 1;
