@@ -156,29 +156,41 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
         sm_plan_destroy(p);
         return e == cudaErrorMemoryAllocation ? SM_ERR_ALLOC : SM_ERR_CUDA;
     }
-    // gather launch shape: per-warp tile (qt dense columns x tile_ld) + two per-warp buffers of block
-    // records + member tables + hash table of S_i.  qt and the warp count shrink until the CTA fits.
+    // gather launch shape: member tables + hash table of S_i + position map + block map of a chunk
+    // of mc member columns (all of them when it fits ~72 KB, so that 3 CTAs share an SM)
     {
         const int msb = (std::max(p->max_sub_blocks, 1) + 1) & ~1;
-        const int tile_ld = (p->info.dim_max + LD_ALIGN + 1) & ~1;
+        const int tile_ld = (p->info.dim_max + LD_ALIGN + 3) & ~3;
+        const int mpad = (msb + 2 + 15) & ~15;  // + the "no member" column of padding positions; 32-byte rows
         int hs = 32, shift = 27;
         while (hs < 2 * msb) { hs <<= 1; --shift; }
-        auto bytes = [&](int warps, int qt) {
-            return (size_t)warps * 2 * qt * tile_ld * 8 + (size_t)msb * 16 + (size_t)warps * tile_ld * 8 +
-                   (size_t)hs * 8 + (size_t)(2 * msb + 2) * 4;
-        };
-        int warps = 8, qt = 4;
-        const size_t want = 60 * 1024, budget = 200 * 1024;  // measured: 3-4 CTAs per SM beat wider tiles
-        while (qt > 1 && bytes(warps, qt) > want) qt >>= 1;
-        while (warps > 1 && bytes(warps, qt) > want) warps >>= 1;
-        if (bytes(warps, qt) > budget) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }  // n_i > ~25000
-        p->gather_warps = warps; p->gather_qt = qt; p->gather_tile_ld = tile_ld;
+        const size_t fixed = (size_t)msb * 8 + (size_t)tile_ld * 8 + (size_t)hs * 8 + (size_t)(msb + 2) * 4 +
+                             (size_t)msb * 4;
+        // a block-map entry is the value offset of a block inside its block column: 16 bits when
+        // every block column holds fewer than 65535 values (halves the table), else 32 bits
+        int64_t max_col_elems = 0;
+        for (int c = 0; c < nb; ++c) {
+            int64_t elems = 0;
+            for (int64_t q = colptr[c]; q < colptr[c + 1]; ++q) elems += blk_size[rowidx[q]];
+            max_col_elems = std::max(max_col_elems, elems * blk_size[c]);
+        }
+        if (max_col_elems >= (int64_t)UINT32_MAX) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }
+        const int esz = max_col_elems < 65535 ? 2 : 4;
+        p->gather_map16 = esz == 2;
+        auto bytes = [&](int mc) { return fixed + (((size_t)mc * mpad * esz + 15) & ~(size_t)15); };
+        int mc = msb;
+        const size_t want = 44 * 1024, budget = 200 * 1024;
+        if (bytes(mc) > want) mc = (int)std::max<int64_t>(((int64_t)want - (int64_t)fixed) / (mpad * esz), 16);
+        mc = std::min(mc, msb);
+        while (mc > 1 && bytes(mc) > budget) mc >>= 1;
+        if (bytes(mc) > budget) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }
+        p->gather_warps = 8; p->gather_tile_ld = tile_ld; p->gather_mpad = mpad; p->gather_mc = mc;
         p->gather_msb = msb; p->gather_hash_size = hs; p->gather_hash_shift = shift;
-        p->gather_smem = bytes(warps, qt);
-        // CTAs per submatrix: enough CTAs to fill the GPU a few times over, at least 2 block columns per warp
+        p->gather_smem = bytes(mc);
+        // CTAs per submatrix: enough CTAs to fill the GPU a few times over
         int split = 1;
         const int64_t want_ctas = (int64_t)p->num_sms * 12;
-        while ((int64_t)ngroups * split < want_ctas && split * warps * 2 < p->max_sub_blocks) ++split;
+        while ((int64_t)ngroups * split < want_ctas && split * 8 * 4 < p->info.dim_max) ++split;
         p->gather_split = std::max(split, 1);
     }
     *plan = p;

@@ -110,7 +110,7 @@ struct sm_plan {
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_iter[2] = {nullptr, nullptr};
     int gather_warps = 8, gather_qt = 4, gather_tile_ld = 0, gather_chunk = 32, gather_msb = 2, gather_split = 1;
-    int gather_hash_size = 32, gather_hash_shift = 27;
+    int gather_hash_size = 32, gather_hash_shift = 27, gather_mpad = 4, gather_mc = 2, gather_map16 = 0;
     int32_t max_col_blocks = 0;  // longest block column
     size_t gather_smem = 0;
     int num_sms = 148;

@@ -17,34 +17,25 @@ __device__ __forceinline__ int find_sorted64(const int32_t* __restrict__ a, int 
 
 // ---------------------------------------------------------------------------------------------
 // Gather (PAPER.md L125 step 1; L187 "submatrix assembly becomes a purely local operation").
-// grid = (ngroups, split): the CTAs of a submatrix share its block columns round-robin by warp.
-// Per CTA, once, in shared memory: the members of S_i with their element offsets, for each the
-// extent of its stored block column (colptr, first value offset), and a hash table
-// block row -> (element offset inside a_i | block height).  All later global reads are then one
-// dependent hop deep.  One warp assembles one block column c = S_i[tc] of a_i at a time, through
-// two zeroed per-warp shared-memory tiles of qt dense columns x ld rows (software pipeline):
-//  (1) row list: the lanes take the stored blocks (r,c) of column c (rowidx / val_off, loaded
-//      one block column ahead into registers), probe the hash table, and a warp prefix sum over
-//      the heights of the blocks found expands them into a compact list of the stored dense rows
-//      (source offset, destination row | height); blocks whose row is not in S_i are dropped,
-//      members without a stored block stay zero in the tile (reading A4);
-//  (2) fill: lanes <-> consecutive entries of the row list, one 8-byte cp.async per dense column
-//      (no register round trip, every load of the pass in flight at once, consecutive lanes hit
-//      consecutive tile addresses); mu is subtracted on the diagonal (Eq.(16));
-//  (3) flush: the lanes sweep the tile rows two elements at a time: 16-byte coalesced stores into
-//      the k8-panel workspace (dense column q of a_i = row q of the symmetric X), abs-sums for
-//      the Gershgorin bound s_i = max_q sum_p |a_pq|, and the tile is zeroed again behind them.
-// Rows n..ld-1 of the tile are never filled, so padding comes out as zeros.
+// grid = (ngroups, split); one CTA (or `split` CTAs sharing the dense rows) per submatrix, NO matrix
+// data staged in shared memory.  Per CTA, in shared memory:
+//   * a hash table  block row -> member index t of S_i,
+//   * posmap[p] for every dense row p of a_i: its member t, the row el inside the block, the block
+//     height (p >= n: the "no member" column of the block map),
+//   * the BLOCK MAP of a chunk of member columns:  bmap[tc][t] = offset of the stored block
+//     (S_i[t], S_i[tc]) inside the values of block column S_i[tc], (16 bits when every block column holds fewer than 65535 values), or all-ones if it is not stored
+//     (reading A4: zero fill).  It is built by walking the stored block columns once (coalesced
+//     reads of rowidx / val_off, one hash probe per stored block; blocks whose row is not in S_i
+//     are dropped).
+// Sweep: dense column q of a_i is row q of the symmetric X; one warp per row, lanes two positions
+// at a time: posmap (one 16-byte read), two block-map reads, predicated 8-byte loads of the stored
+// values straight from global memory (L2-resident: every value is used by ~|S_i| submatrices), mu
+// subtracted on the diagonal (Eq.(16)), one coalesced 16-byte store into the k8-panel workspace,
+// abs-sums for the Gershgorin bound s_i = max_q sum_p |a_pq|.
 // ---------------------------------------------------------------------------------------------
-constexpr int GATHER_PF = 3;  // block-column entries prefetched per lane (columns up to 96 blocks)
-
 __device__ __forceinline__ unsigned gather_hash(int key, int shift) {
     return ((unsigned)key * 2654435761u) >> shift;
 }
-__device__ __forceinline__ void cp_async8(unsigned smem_dst, const void* gsrc) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_dst), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 struct GatherArgs {
     const int64_t* colptr;
@@ -60,184 +51,99 @@ struct GatherArgs {
     double* X;
     unsigned long long* gersh;
     double mu;
-    int qt, tile_ld, msb, hash_size, hash_shift;
+    int tile_ld, msb, mpad, mc, hash_size, hash_shift;
 };
 
-__global__ void __launch_bounds__(256, 3) k_gather(const GatherArgs A) {
+template <typename MapT>
+__global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
+    constexpr MapT NONE = (MapT)~(MapT)0;  // block (S_i[t], S_i[tc]) not stored
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int g = blockIdx.x;
     const int64_t sp = A.sub_ptr[g];
     const int m = (int)(A.sub_ptr[g + 1] - sp);
     const int n = A.sub_dim[g], ld = A.ldv[g];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    const int qt = A.qt, tile_ld = A.tile_ld, msb = A.msb;
+    const int tile_ld = A.tile_ld, msb = A.msb, mpad = A.mpad, mc = A.mc;
     // shared-memory carve-up
-    double* tiles = reinterpret_cast<double*>(smem_raw);                        // [nw][2][qt][tile_ld]
-    int64_t* mP0 = reinterpret_cast<int64_t*>(tiles + (size_t)nw * 2 * qt * tile_ld);   // [msb] colptr of member
-    int64_t* mVb = mP0 + msb;                                                   // [msb] first value offset
-    int2* rows_all = reinterpret_cast<int2*>(mVb + msb);                        // [nw][tile_ld]
-    int32_t* hk = reinterpret_cast<int32_t*>(rows_all + (size_t)nw * tile_ld);  // [hash_size] keys
-    uint32_t* hv = reinterpret_cast<uint32_t*>(hk + A.hash_size);               // [hash_size] offset | height << 20
-    int32_t* mLen = reinterpret_cast<int32_t*>(hv + A.hash_size);               // [msb] blocks in the column
-    int32_t* mSo = mLen + msb;                                                  // [msb + 1] element offsets
+    int64_t* mVb = reinterpret_cast<int64_t*>(smem_raw);                        // [msb] first value offset of the member's column
+    uint2* posmap = reinterpret_cast<uint2*>(mVb + msb);                        // [tile_ld] member | (el | height << 16)
+    MapT* bmap = reinterpret_cast<MapT*>(posmap + tile_ld);                     // [mc][mpad]
+    int32_t* hk = reinterpret_cast<int32_t*>(bmap + (size_t)mc * mpad);                                    // [hash_size] keys
+    int32_t* hv = hk + A.hash_size;                                             // [hash_size] member index
+    int32_t* mSo = hv + A.hash_size;                                            // [msb + 1] element offsets
+    int32_t* mKey = mSo + msb + 2;                                              // [msb] global block index of the member
     for (int h = threadIdx.x; h < A.hash_size; h += blockDim.x) hk[h] = -1;
-    for (int e = threadIdx.x; e < nw * 2 * qt * tile_ld; e += blockDim.x) tiles[e] = 0.0;
     for (int t = threadIdx.x; t < m; t += blockDim.x) mSo[t] = A.sub_off[sp + t];
     if (threadIdx.x == 0) mSo[m] = n;
     __syncthreads();
     const unsigned hmask = (unsigned)A.hash_size - 1u;
     for (int t = threadIdx.x; t < m; t += blockDim.x) {
         const int key = A.sub_blocks[sp + t];
-        const int64_t p0 = A.colptr[key];
-        mP0[t] = p0;
-        mLen[t] = (int)(A.colptr[key + 1] - p0);
-        mVb[t] = A.val_off[p0];
+        mKey[t] = key;
+        mVb[t] = A.val_off[A.colptr[key]];
         unsigned h = gather_hash(key, A.hash_shift);
         while (atomicCAS(&hk[h], -1, key) != -1) h = (h + 1) & hmask;
-        hv[h] = (uint32_t)mSo[t] | ((uint32_t)(mSo[t + 1] - mSo[t]) << 20);
+        hv[h] = t;
+        const int so = mSo[t], br = mSo[t + 1] - so;
+        for (int el = 0; el < br; ++el) posmap[so + el] = make_uint2((unsigned)t, (unsigned)el | ((unsigned)br << 16));
     }
-    __syncthreads();
-    double* tile = tiles + (size_t)wid * 2 * qt * tile_ld;
-    const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
-    int2* rows = rows_all + (size_t)wid * tile_ld;
+    for (int p = n + threadIdx.x; p < tile_ld; p += blockDim.x) posmap[p] = make_uint2((unsigned)m, 1u << 16);
     double* Xg = A.X + A.ws_off[g];
     double cmax = 0.0;
+    const int gw = blockIdx.y * nw + wid, gstride = nw * gridDim.y;
 
-    // (1) one stored block (row r, value offset vo relative to the column's first value): append
-    // its dense rows to the row list.  All 32 lanes call this together (ok = lane has a block).
-    int nrows = 0;
-    auto append = [&](bool ok, int r, int rel) {
-        uint32_t pk = 0;
-        if (ok) {
-            unsigned h = gather_hash(r, A.hash_shift);
-            for (;;) {
-                const int k = hk[h];
-                if (k == r) { pk = hv[h]; break; }
-                if (k < 0) break;
-                h = (h + 1) & hmask;
+    for (int c0 = 0; c0 < m; c0 += mc) {
+        const int c1 = min(m, c0 + mc);
+        __syncthreads();  // tables ready / previous chunk swept
+        for (int e = threadIdx.x; e < (c1 - c0) * mpad; e += blockDim.x) bmap[e] = NONE;
+        __syncthreads();
+        // block map of member columns c0..c1-1: one warp per column, lanes over its stored blocks
+        for (int tc = c0 + wid; tc < c1; tc += nw) {
+            const int key = mKey[tc];
+            const int64_t p0 = A.colptr[key], p1 = A.colptr[key + 1], vb = mVb[tc];
+            MapT* row = bmap + (size_t)(tc - c0) * mpad;
+            for (int64_t j = p0 + lane; j < p1; j += 32) {
+                const int r = __ldg(A.rowidx + j);
+                const int rel = (int)(__ldg(A.val_off + j) - vb);
+                unsigned h = gather_hash(r, A.hash_shift);
+                for (;;) {
+                    const int k = hk[h];
+                    if (k == r) { row[hv[h]] = (MapT)rel; break; }
+                    if (k < 0) break;
+                    h = (h + 1) & hmask;
+                }
             }
         }
-        const int br = (int)(pk >> 20);
-        int incl = br;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += t;
-        }
-        int2* dst = rows + nrows + incl - br;
-        const int so = (int)(pk & 0xfffffu);
-        for (int el = 0; el < br; ++el) dst[el] = make_int2(rel + el, (so + el) | (br << 20));
-        nrows += __shfl_sync(0xffffffffu, incl, 31);
-    };
-    // (2) asynchronous copies of dense columns q0 .. q0+nq-1 of the listed rows into the tile
-    auto fill = [&](unsigned ts, const double* vcol, int q0, int nq) {
-        for (int k = lane; k < nrows; k += 32) {
-            const int2 en = rows[k];
-            const int br = (int)((uint32_t)en.y >> 20);
-            const double* vp = vcol + en.x + (int64_t)q0 * br;
-            unsigned d = ts + (unsigned)(en.y & 0xfffff) * 8u;
-#pragma unroll
-            for (int qq = 0; qq < 4; ++qq) {
-                if (qq < nq) cp_async8(d, vp);
-                vp += br;
-                d += (unsigned)tile_ld * 8u;
-            }
-        }
-    };
-
-    const int stride = nw * gridDim.y;
-    // register prefetch of a block column's entries, one block column ahead of the row list
-    int pr[GATHER_PF];
-    int64_t pv[GATHER_PF];
-    auto prefetch = [&](int t) {
-        if (t >= m) return;
-        const int64_t p0 = mP0[t];
-        const int clen = mLen[t];
-        if (clen > 32 * GATHER_PF) return;
-#pragma unroll
-        for (int i = 0; i < GATHER_PF; ++i) {
-            const int j = lane + 32 * i;
-            if (j < clen) { pr[i] = __ldg(A.rowidx + p0 + j); pv[i] = __ldg(A.val_off + p0 + j); }
-        }
-    };
-    // Software pipeline over passes (block column tc, dense columns q0..q0+nq-1) with two tiles per
-    // warp: the copies of pass k+1 are issued before pass k is flushed, so the global-load latency
-    // of a fill hides behind the row list of the next pass and the flush of the previous one.
-    int tc_f = blockIdx.y * nw + wid, q0_f = 0;  // next pass to issue
-    prefetch(tc_f);
-    int is_coff = 0, is_q0 = 0, is_nq = 0;  // what the flush needs to know about the pass just issued
-    auto issue = [&](int buf) -> bool {
-        if (tc_f >= m) return false;
-        const int coff = mSo[tc_f], bc = mSo[tc_f + 1] - coff;
-        const int64_t p0 = mP0[tc_f], vb = mVb[tc_f];
-        const int clen = mLen[tc_f];
-        const double* vcol = A.vals + vb;
-        const int nq = min(qt, bc - q0_f);
-        const unsigned ts = tile_s + (unsigned)(buf * qt * tile_ld) * 8u;
-        if (clen <= 32 * GATHER_PF) {
-            if (q0_f == 0) {  // the row list of a short column is built once and serves all its passes
-                nrows = 0;
-#pragma unroll
-                for (int i = 0; i < GATHER_PF; ++i)
-                    if (32 * i < clen) append(lane + 32 * i < clen, pr[i], (int)(pv[i] - vb));
-                __syncwarp();
-                prefetch(tc_f + stride);
-            }
-            fill(ts, vcol, q0_f, nq);
-        } else {  // long column: list and fill 32 blocks at a time (cp.async has read its list entry at issue)
-            for (int jb = 0; jb < clen; jb += 32) {
-                const bool ok = jb + lane < clen;
-                nrows = 0;
-                append(ok, ok ? __ldg(A.rowidx + p0 + jb + lane) : 0,
-                       ok ? (int)(__ldg(A.val_off + p0 + jb + lane) - vb) : 0);
-                __syncwarp();
-                fill(ts, vcol, q0_f, nq);
-                __syncwarp();
-            }
-            if (q0_f + qt >= bc) prefetch(tc_f + stride);
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        is_coff = coff; is_q0 = q0_f; is_nq = nq;
-        q0_f += qt;
-        if (q0_f >= bc) { tc_f += stride; q0_f = 0; }
-        return true;
-    };
-    int buf = 0;
-    bool have = issue(0);
-    while (have) {
-        const int coff = is_coff, q0 = is_q0, nq = is_nq;
-        const bool have_next = issue(buf ^ 1);
-        if (have_next) asm volatile("cp.async.wait_group 1;" ::: "memory");
-        else asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncwarp();
-        double* tl = tile + buf * qt * tile_ld;
-        if (lane < nq) tl[lane * tile_ld + coff + q0 + lane] -= A.mu;
-        __syncwarp();
-        // (3) flush.  Lane covers columns p = 2 lane + 64 i: panel (lane >> 2) + 8 i, offset
-        // 2 (lane & 3) inside it.  Offsets inside one submatrix fit 32 bits (ld <= 25600).
-        for (int qq = 0; qq < nq; ++qq) {
-            const int xrow = coff + q0 + qq;
-            const int t0 = xrow & ~63;
-            const unsigned rstride = (unsigned)min(64, ld - t0) * 8u;
-            unsigned xo = (unsigned)t0 * (unsigned)ld + (unsigned)(xrow & 63) * 8u +
-                          (unsigned)(lane >> 2) * rstride + 2u * (lane & 3);
-            double* tp = tl + qq * tile_ld + 2 * lane;
-            const unsigned xstep = rstride * 8u;
-            double a = 0.0;
+        __syncthreads();
+        // sweep the dense rows of this chunk's members
+        const int q_begin = mSo[c0], q_end = mSo[c1];
+        for (int q = q_begin + gw; q < q_end; q += gstride) {
+            const uint2 me = posmap[q];
+            const int tc = (int)me.x, qq = (int)(me.y & 0xffffu);
+            const MapT* row = bmap + (size_t)(tc - c0) * mpad;
+            const double* vcol = A.vals + mVb[tc];
+            const int t0 = q & ~63;
+            const unsigned rows_t = (unsigned)min(64, ld - t0);
+            unsigned xo = (unsigned)t0 * (unsigned)ld + (unsigned)(q & 63) * 8u + (unsigned)(lane >> 2) * rows_t * 8u +
+                          2u * (lane & 3);
+            const unsigned xstep = rows_t * 64u;
+            double asum = 0.0;
 #pragma unroll 4
-            for (int p = 2 * lane; p < ld; p += 64, tp += 64, xo += xstep) {
-                const double2 v = *reinterpret_cast<const double2*>(tp);
-                *reinterpret_cast<double2*>(tp) = make_double2(0.0, 0.0);
-                a += fabs(v.x) + fabs(v.y);
+            for (int p = 2 * lane; p < ld; p += 64, xo += xstep) {
+                const uint4 pm = *reinterpret_cast<const uint4*>(posmap + p);
+                const MapT r0 = row[pm.x], r1 = row[pm.z];
+                double2 v = make_double2(0.0, 0.0);
+                if (r0 != NONE) v.x = __ldg(vcol + (int)r0 + (int)(pm.y & 0xffffu) + qq * (int)(pm.y >> 16));
+                if (r1 != NONE) v.y = __ldg(vcol + (int)r1 + (int)(pm.w & 0xffffu) + qq * (int)(pm.w >> 16));
+                if (p == q) v.x -= A.mu;
+                if (p + 1 == q) v.y -= A.mu;
+                asum += fabs(v.x) + fabs(v.y);
                 *reinterpret_cast<double2*>(Xg + xo) = v;
             }
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-            cmax = fmax(cmax, a);
+            for (int o = 16; o > 0; o >>= 1) asum += __shfl_xor_sync(0xffffffffu, asum, o);
+            cmax = fmax(cmax, asum);
         }
-        __syncwarp();
-        buf ^= 1;
-        have = have_next;
     }
     // zero padding columns n..ld-1 (first CTA of the submatrix)
     if (blockIdx.y == 0) {
@@ -252,15 +158,18 @@ __global__ void __launch_bounds__(256, 3) k_gather(const GatherArgs A) {
 sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, cudaStream_t st) {
     if (p->ngroups == 0) return SM_OK;
     SM_CUDA(cudaMemsetAsync(p->d_gersh, 0, (size_t)p->ngroups * 8, st));
-    if (p->gather_smem > 48 * 1024)
-        SM_CUDA(cudaFuncSetAttribute(k_gather, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
+    if (p->gather_smem > 48 * 1024) {
+        SM_CUDA(cudaFuncSetAttribute(k_gather<uint16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
+        SM_CUDA(cudaFuncSetAttribute(k_gather<uint32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
+    }
     GatherArgs a;
     a.colptr = p->d_colptr; a.rowidx = p->d_rowidx; a.val_off = p->d_val_off; a.vals = vals;
     a.sub_ptr = p->d_sub_ptr; a.sub_blocks = p->d_sub_blocks; a.sub_off = p->d_sub_off; a.sub_dim = p->d_sub_dim;
     a.ldv = p->d_ld; a.ws_off = p->d_ws_off; a.X = X; a.gersh = p->d_gersh; a.mu = mu;
-    a.qt = p->gather_qt; a.tile_ld = p->gather_tile_ld; a.msb = p->gather_msb;
+    a.tile_ld = p->gather_tile_ld; a.msb = p->gather_msb; a.mpad = p->gather_mpad; a.mc = p->gather_mc;
     a.hash_size = p->gather_hash_size; a.hash_shift = p->gather_hash_shift;
-    k_gather<<<dim3(p->ngroups, p->gather_split), p->gather_warps * 32, p->gather_smem, st>>>(a);
+    if (p->gather_map16) k_gather<uint16_t><<<dim3(p->ngroups, p->gather_split), p->gather_warps * 32, p->gather_smem, st>>>(a);
+    else k_gather<uint32_t><<<dim3(p->ngroups, p->gather_split), p->gather_warps * 32, p->gather_smem, st>>>(a);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
