@@ -39,7 +39,7 @@ TOL_N = 0.5      # plateau acceptance (reading A11); 1e-8 is unreachab
 MU0 = -1.0       # starting mu inside the occupied band: forces a genuine bisection
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_ns_gemm from the committed
 # `ncu --set full` capture (profiles/), or None when no capture matches the current kernel.
-NS_GEMM_DRAM_BYTES_PER_LAUNCH = None
+NS_GEMM_DRAM_BYTES_PER_LAUNCH = 20.3e9  # all-active launch, mean of MODE 0 (15.8 GB) and MODE 1 (24.8 GB): profiles/r01_v6_ns_gemm_full.md
 NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # guide: B200 FP64 tensor 45 TF/s, bf16 2250 TF/s (nominal)
 
 

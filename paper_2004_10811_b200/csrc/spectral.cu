@@ -124,13 +124,13 @@ __global__ void k_lz_extremes(int k, const double* __restrict__ alpha, const dou
         return cnt;
     };
     double lo = glo, hi = ghi;  // smallest eigenvalue: first x with count_below(x) >= 1
-    for (int it = 0; it < 200; ++it) {
+    for (int it = 0; it < 64; ++it) {
         const double mid = 0.5 * (lo + hi);
         if (count_below(mid) >= 1) hi = mid; else lo = mid;
     }
     const double emin = lo;
     lo = glo; hi = ghi;         // largest eigenvalue: first x with count_below(x) >= k
-    for (int it = 0; it < 200; ++it) {
+    for (int it = 0; it < 64; ++it) {
         const double mid = 0.5 * (lo + hi);
         if (count_below(mid) >= k) hi = mid; else lo = mid;
     }
