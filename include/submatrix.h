@@ -63,7 +63,13 @@ typedef struct {
                          /* 1 = min(that, interlacing bound): a_i is a principal submatrix   */
                          /*     of K~, so rho(a_i - mu I) <= max|lambda_minmax(K~) - mu|,    */
                          /*     extremes of K~ by a short Lanczos run per call, then / overshoot */
-    int32_t precision;   /* 0 = FP64 DMMA (the parity path)                            [0]   */
+    int32_t precision;   /* 0 = FP64 DMMA (the parity path);                           [0]   */
+                         /* opt-in reduced precision on the tcgen05 tensor cores (FP32       */
+                         /* accumulators in tensor memory; accuracy reported separately; no  */
+                         /* steering early-out):                                             */
+                         /* 1 = FP32 storage, plain TF32 products (error ~2e-3 class);       */
+                         /* 2 = "3xTF32": operands stored as hi + lo TF32 pairs, products    */
+                         /*     hi hi + hi lo + lo hi (FP32-class, <= 1e-3 bar)              */
     int32_t check_every; /* host polls the "all converged" counter every this many     [1]   */
                          /* iterations (>= 1)                                                */
     int32_t max_mu_steps;/* bisection step cap of sm_density_matrix                    [64]  */

@@ -79,7 +79,8 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_gen_width, p->d_ws_off, p->d_ld, p->d_tiles,
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
                     p->d_partials, p->d_counters, p->d_sched, p->d_tile_done, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
-                    p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz};
+                    p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
+                    p->d_tile_first32, p->d_tile_count32, p->d_partials32};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     if (p->h_pinned) cudaFreeHost(p->h_pinned);
@@ -110,7 +111,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (!(p->opt.mu_tol > 0)) p->opt.mu_tol = 1e-6;
     if (!(p->opt.overshoot >= 1.0)) p->opt.overshoot = 1.0;     // zero-initialised struct: no overshoot
     if (p->opt.overshoot > 1.5) p->opt.overshoot = 1.5;         // f(x) = x(3 - x^2)/2 keeps [1, 1.5] inside [0.56, 1]
-    if (p->opt.precision != 0 || p->opt.scaling < 0 || p->opt.scaling > 1) { delete p; return SM_ERR_INVALID_ARG; }
+    if (p->opt.precision < 0 || p->opt.precision > 2 || p->opt.scaling < 0 || p->opt.scaling > 1) { delete p; return SM_ERR_INVALID_ARG; }
     p->nb = nb; p->ngroups = ngroups; p->nnzb = nb ? colptr[nb] : 0;
     p->h_blk_size.assign(blk_size, blk_size + nb);
     p->h_colptr.assign(colptr, colptr + nb + 1);
@@ -127,6 +128,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     }
     s = build_index_device(p, st);
     if (s) { sm_plan_destroy(p); return s; }
+    if (p->opt.precision != 0 && (s = build_tf32_tables(p, st))) { sm_plan_destroy(p); return s; }
     // per-evaluation state
     const int ng = std::max(ngroups, 1);
     auto A = [&](void** d, size_t bytes) { return cudaMalloc(d, std::max<size_t>(bytes, 8)); };
@@ -259,6 +261,12 @@ struct Steer {
     double ne = 0.0, err = 0.0;  // out: n_elec(X_k) and its bound
 };
 
+// One iteration's launches on the path the plan was created for (FP64 DMMA, or TF32 tcgen05).
+sm_status_t launch_pair(sm_plan* p, int k, double eps, int last, const Bufs& b, cudaStream_t st, int which) {
+    if (p->opt.precision != 0) return launch_ns_pair_tf32(p, k, eps, last, b.b0, b.b1, b.y, st, which);
+    return launch_ns_pair(p, k, eps, last, b.b0, b.b1, b.y, st, which);
+}
+
 // Newton-Schulz host loop: iterations k = cur_k .. k_end-1 (each = MODE 0 + MODE 1 launch).
 // Iteration k tests X_k and, if not converged, forms X_{k+1}.  At k == max_iter only the decision
 // is recorded.  Returns with *all_done = 1 if every submatrix has stopped.  The host reads the
@@ -291,7 +299,7 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
         // evaluation before the next update is even launched.
         for (; k < k_end && k <= max_iter; ++k) {
             const int last = k == max_iter ? 1 : 0;
-            sm_status_t s = launch_ns_pair(p, k, eps, last, b.b0, b.b1, b.y, st, 1);
+            sm_status_t s = launch_pair(p, k, eps, last, b, st, 1);
             if (s) return s;
             (*launched) += 1;
             SM_CUDA(cudaMemcpyAsync(p->h_pinned + k, p->d_counters + k, 4, cudaMemcpyDeviceToHost, st));
@@ -304,7 +312,7 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
             if (r == 1) return SM_OK;                       // all converged: X_k is the result (cur_k = k)
             if (r == 2) { p->cur_k = k; p->half_iter = 1; return SM_OK; }  // X_k in buf[k & 1], not converged
             if (last) break;
-            if ((s = launch_ns_pair(p, k, eps, 0, b.b0, b.b1, b.y, st, 2))) return s;
+            if ((s = launch_pair(p, k, eps, 0, b, st, 2))) return s;
             (*launched) += 1;
         }
         p->cur_k = std::min(k, max_iter);
@@ -312,7 +320,7 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
         return SM_OK;
     }
     for (; k < k_end && k <= max_iter; ++k) {
-        sm_status_t s = launch_ns_pair(p, k, eps, k == max_iter ? 1 : 0, b.b0, b.b1, b.y, st);
+        sm_status_t s = launch_pair(p, k, eps, k == max_iter ? 1 : 0, b, st, 3);
         if (s) return s;
         (*launched) += (k == max_iter) ? 1 : 2;
         if (pending >= 0) {
@@ -405,9 +413,12 @@ sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, cons
     if ((s = launch_gather(p, d_in, mu, b.b0, st))) return s;
     if ((s = apply_scaling(p, mu, st))) return s;
     if (p->timing) SM_CUDA(cudaEventRecord(p->ev[1], st));
-    if ((s = ns_loop(p, b, eps, iter_cap, &all_done, &launched, st, steer))) return s;
+    const bool reduced = p->opt.precision != 0;
+    if (reduced && (s = launch_to_f32(p, b.b0, b.b1, st))) return s;  // X0 = (a_i - mu I)/s_i in FP32
+    if ((s = ns_loop(p, b, eps, iter_cap, &all_done, &launched, st, reduced ? nullptr : steer))) return s;
+    if (reduced && (s = launch_to_f64(p, b.b0, b.b1, b.y, st))) return s;  // result back in buf0, FP64 layout
     if (p->timing) SM_CUDA(cudaEventRecord(p->ev[2], st));
-    if ((s = launch_nelec(p, b.b0, b.b1, st))) return s;
+    if ((s = launch_nelec(p, b.b0, reduced ? b.b0 : b.b1, st))) return s;
     if ((s = collect_stats(p, stats, not_conv, st))) return s;
     if (stats) {
         if (steer && steer->decided) stats->n_elec = steer->ne;
@@ -430,7 +441,7 @@ sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, cons
 
 sm_status_t do_scatter(sm_plan* p, const Bufs& b, double* d_out, sm_stats_t* stats, cudaStream_t st) {
     if (p->timing) SM_CUDA(cudaEventRecord(p->ev[3], st));
-    sm_status_t s = launch_scatter(p, 0, b.b0, b.b1, d_out, st);
+    sm_status_t s = launch_scatter(p, 0, b.b0, p->opt.precision != 0 ? b.b0 : b.b1, d_out, st);
     if (s) return s;
     if (p->timing) {
         SM_CUDA(cudaEventRecord(p->ev[4], st));
@@ -481,7 +492,7 @@ extern "C" sm_status_t sm_gather(sm_plan_t* p, const double* d_vals_in, double m
 
 extern "C" sm_status_t sm_sign_iterate(sm_plan_t* p, double eps, void* d_workspace, size_t workspace_bytes,
                                        sm_stats_t* stats, void* cuda_stream) {
-    if (!p || !(eps > 0.0)) return SM_ERR_INVALID_ARG;
+    if (!p || !(eps > 0.0) || p->opt.precision != 0) return SM_ERR_INVALID_ARG;  // phase entry: FP64 path only
     cudaStream_t st = (cudaStream_t)cuda_stream;
     Bufs b;
     sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
@@ -538,8 +549,8 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     SM_CUDA(cudaMemcpy(p->h_pinned_d + 4, p->d_scalars + 4, 16, cudaMemcpyDeviceToHost));
     double lo = p->h_pinned_d[4], hi = p->h_pinned_d[5];
     double mu = *mu_inout;
-    const int cap = (p->opt.bisect_iter > 0 && p->opt.bisect_iter < p->opt.max_iter) ? p->opt.bisect_iter
-                                                                                       : p->opt.max_iter + 1;
+    const int cap = (p->opt.precision == 0 && p->opt.bisect_iter > 0 && p->opt.bisect_iter < p->opt.max_iter)
+                        ? p->opt.bisect_iter : p->opt.max_iter + 1;
     double best_mu = mu, best_g = INFINITY;
     int best_step = -1, steps = 0, nc = 0, last_nc = 0;
     bool accepted = false, last_partial = false;
@@ -552,7 +563,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         acc_eval += 1; acc_g += e.tot_ms_gather; acc_s += e.tot_ms_sign;
     };
     p->lz_valid = 0;  // one Lanczos run serves every mu of this call
-    const bool early = p->opt.early_out != 0;
+    const bool early = p->opt.early_out != 0 && p->opt.precision == 0;
     for (; steps < p->opt.max_mu_steps;) {
         memset(&ev, 0, sizeof(ev));
         Steer steer;

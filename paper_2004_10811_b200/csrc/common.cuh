@@ -99,6 +99,12 @@ struct sm_plan {
     double* d_bound = nullptr;             // [max_iter+2][2] per iteration: n_elec(X_k), its error bound
     double* d_bound_part = nullptr;        // [2][ngroups] per-group partials of the two
     double* h_bound = nullptr;             // pinned mirror of d_bound
+    // --- reduced-precision path (precision = 1, ns_tf32.cu)
+    void* d_tiles32 = nullptr;
+    int64_t* d_ws_off32 = nullptr;
+    int32_t *d_tile_first32 = nullptr, *d_tile_count32 = nullptr;
+    double* d_partials32 = nullptr;
+    int64_t n_tiles32 = 0, sum_ldp2 = 0;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
     double lz_lo = 0.0, lz_hi = 0.0;       // estimated [lambda_min, lambda_max] of K~ (widened)
     int lz_valid = 0;                      // lz_lo / lz_hi belong to the current call's values
@@ -128,6 +134,12 @@ sm_status_t launch_trace_dk(sm_plan* p, const double* D, const double* K, cudaSt
 sm_status_t launch_gersh_global(sm_plan* p, const double* vals, cudaStream_t st);
 sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const double* buf1, const double* bufY,
                                cudaStream_t st);
+// ns_tf32.cu
+sm_status_t build_tf32_tables(sm_plan* p, cudaStream_t st);
+sm_status_t launch_to_f32(sm_plan* p, const double* buf0, double* buf1, cudaStream_t st);
+sm_status_t launch_to_f64(sm_plan* p, double* buf0, const double* buf1, const double* bufY, cudaStream_t st);
+sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
+                                double* bufY, cudaStream_t st, int which);
 // spectral.cu
 sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st);
 sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStream_t st);

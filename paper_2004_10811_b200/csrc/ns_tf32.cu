@@ -1,0 +1,552 @@
+// a5, opt-in reduced-precision variant (options.precision = 1): the same Newton-Schulz iteration
+// (Eq.(11)) with FP32 storage and TF32 products on the 5th-generation tensor cores
+// (tcgen05.mma kind::tf32, FP32 accumulators in tensor memory) -- the B200 counterpart of the
+// paper's FP16 / FP32 cuBLAS experiment (L346-360, Table I).  Its accuracy is reported
+// separately (north_star: <= 1e-3 elementwise); the FP64 DMMA path of ns_sign.cu stays the parity
+// path.  NS never re-reads A, so the result carries the precision of the products.
+//
+// Data layout ("k4-panel/128", FP32): ldp = n rounded up to 16; rows in row-tiles of 128; inside a
+// row-tile, chunk kc = the 4 consecutive columns 4 kc .. 4 kc + 3 of all its rows, row-major (16 B
+// per row).  This IS the canonical K-major no-swizzle operand layout of tcgen05.mma (core matrix =
+// 8 rows x 16 B contiguous, SBO = 128 B between row groups, LBO = rows_t * 16 B between chunks), so
+// a pipeline stage (128 rows x 32 k) is one contiguous block in global memory: one cp.async.bulk,
+// no tensor map, and the tensor core reads it as it landed.  It also makes the epilogue coalesced:
+// thread r of a warp owns TMEM lane (row) r and writes 16 B per chunk next to its neighbours.
+//
+// Kernel: persistent, one CTA per SM, warp-specialised:
+//   warp 0 (one thread)  producer: cp.async.bulk of the A / B slices into a 4-stage ring (mbarrier tx)
+//   warp 1 (one thread)  issues tcgen05.mma (M = 128, N = rows of the B half, K = 8 per instruction),
+//                        tcgen05.commit releases the stage / hands the accumulator to the epilogue
+//   warps 2..5           epilogue: tcgen05.ld of their 32 TMEM lanes, MODE 0: Y = X X and residual
+//                        partials; MODE 1: X' = 3/2 X - 1/2 X Y; two 256-column accumulators in
+//                        TMEM, so the epilogue of one tile overlaps the MMAs of the next.
+// Work unit: (submatrix, 128-row tile, 256-column tile on or below the diagonal), static round-robin
+// over the CTAs.  Only the lower triangle is computed; every element is stored together with its
+// mirror image, so X and Y are bitwise symmetric and B can be read as k-contiguous rows.
+#include <algorithm>
+
+#include "common.cuh"
+
+namespace smb {
+
+constexpr int R_BM = 128, R_BN = 256, R_BK = 32, R_STAGES = 4;
+constexpr int R_STAGE_FLOATS = (R_BM + R_BN) * R_BK;  // 48 KB
+constexpr size_t R_SMEM = (size_t)R_STAGES * R_STAGE_FLOATS * sizeof(float);
+constexpr int R_THREADS = 192;
+
+__host__ __device__ __forceinline__ size_t panel32_off(int r, int c, int ldp) {
+    const int t0 = r & ~127;
+    const int rows_t = (ldp - t0) < 128 ? (ldp - t0) : 128;
+    return (size_t)t0 * ldp + (size_t)(c >> 2) * rows_t * 4 + (size_t)((r - t0) * 4 + (c & 3));
+}
+
+__device__ __forceinline__ unsigned r_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void r_mbar_init(uint64_t* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(r_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void r_mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(r_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void r_mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(r_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void r_mbar_wait(uint64_t* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(r_smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void r_bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     r_smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(r_smem_u32(bar))
+                 : "memory");
+}
+// Shared-memory matrix descriptor, K-major, no swizzle (bit layout as in the sm_100 UMMA descriptor:
+// start address >> 4 in [0,14), leading byte offset >> 4 in [16,30), stride byte offset >> 4 in
+// [32,46), version 1 in [46,48), layout type 0 in [61,64)).
+__device__ __forceinline__ uint64_t r_desc(unsigned addr, unsigned lbo_bytes) {
+    uint64_t d = (uint64_t)((addr & 0x3ffffu) >> 4);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3fffu) << 16;
+    d |= (uint64_t)(128u >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
+// Instruction descriptor: D = F32 ([4,6) = 1), A = B = TF32 ([7,10) = [10,13) = 2), both K-major,
+// N >> 3 in [17,23), M >> 4 in [24,29).
+__device__ __forceinline__ uint32_t r_idesc(int n_cols) {
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)(n_cols >> 3) << 17) | ((unsigned)(R_BM >> 4) << 24);
+}
+__device__ __forceinline__ void r_mma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void r_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(r_smem_u32(bar))
+                 : "memory");
+}
+
+// Round to nearest TF32 (10-bit mantissa): kind::tf32 ignores the low 13 mantissa bits of its FP32
+// operands, so values are rounded when they are stored instead of truncated when they are read.
+__device__ __forceinline__ float r_tf32(float x) {
+    uint32_t u;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(x));
+    return __uint_as_float(u);
+}
+
+// One work unit of the reduced-precision GEMMs.
+struct __align__(16) Tile32 {
+    int64_t off32;   // offset (floats) of the submatrix in each FP32 buffer
+    int32_t grp, ldp, n;
+    int32_t ti, tj;  // 128-row tile, 256-column tile
+    int32_t tile;    // index in the list (slot of the residual partials)
+};
+
+// FP64 k8-panel a_i - mu I  ->  FP32 k4-panel/128 X0 = (a_i - mu I) / s_i (padding written as zeros).
+__global__ void __launch_bounds__(256)
+k_to_f32(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __restrict__ ldv,
+         const int64_t* __restrict__ ws_off, const int64_t* __restrict__ ws_off32,
+         const unsigned long long* __restrict__ gersh, const double* __restrict__ X64, float* __restrict__ X32,
+         int64_t lo_plane) {  // 0: single FP32 plane; else offset (floats) of the "lo" plane of the hi/lo split
+    const int g = blockIdx.x;
+    const int n = sub_dim[g], ld = ldv[g], ldp = (n + 15) & ~15;
+    double s = __longlong_as_double((long long)gersh[g]);
+    const double inv = s > 0.0 ? 1.0 / s : 1.0;
+    const double* src = X64 + ws_off[g];
+    float* dst = X32 + ws_off32[g];
+    const int chunks = ldp >> 2;
+    for (int e = blockIdx.y * blockDim.x + threadIdx.x; e < ldp * chunks; e += gridDim.y * blockDim.x) {
+        // consecutive threads -> consecutive rows of one chunk: coalesced 16-byte stores
+        const int t = e / (128 * chunks);                 // row tile (all full tiles hold 128 * chunks units)
+        const int rows_t = min(128, ldp - 128 * t);
+        const int w = e - t * 128 * chunks;
+        const int kc = w / rows_t, r = 128 * t + (w - kc * rows_t);
+        double x[4] = {0.0, 0.0, 0.0, 0.0};
+        if (r < n) {
+            const int c = 4 * kc;
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (c + j < n) x[j] = src[panel_off(r, c + j, ld)] * inv;
+        }
+        float* d = dst + panel32_off(r, 4 * kc, ldp);
+        if (lo_plane == 0) {
+            *reinterpret_cast<float4*>(d) = make_float4((float)x[0], (float)x[1], (float)x[2], (float)x[3]);
+        } else {
+            float4 hi, lo;
+            hi.x = r_tf32((float)x[0]); hi.y = r_tf32((float)x[1]); hi.z = r_tf32((float)x[2]); hi.w = r_tf32((float)x[3]);
+            lo.x = (float)(x[0] - hi.x); lo.y = (float)(x[1] - hi.y); lo.z = (float)(x[2] - hi.z); lo.w = (float)(x[3] - hi.w);
+            *reinterpret_cast<float4*>(d) = hi;
+            *reinterpret_cast<float4*>(d + lo_plane) = lo;
+        }
+    }
+}
+
+// FP32 result -> FP64 k8-panel buffer (the layout scatter / trace kernels read).  A submatrix that
+// stopped at iteration 0 is written back unscaled (x s_i), as the FP64 path leaves it.
+__global__ void __launch_bounds__(256)
+k_to_f64(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __restrict__ ldv,
+         const int64_t* __restrict__ ws_off, const int64_t* __restrict__ ws_off32,
+         const unsigned long long* __restrict__ gersh, const int32_t* __restrict__ done_iter, int cur_k,
+         const float* __restrict__ Xa, const float* __restrict__ Xb, double* __restrict__ X64, int64_t lo_plane) {
+    const int g = blockIdx.x;
+    const int n = sub_dim[g], ld = ldv[g], ldp = (n + 15) & ~15;
+    const int di = done_iter[g];
+    const int kb = di >= 0 ? di : cur_k;
+    const float* src = ((kb & 1) ? Xb : Xa) + ws_off32[g];
+    double mul = 1.0;
+    if (kb == 0) {
+        const double s = __longlong_as_double((long long)gersh[g]);
+        mul = s > 0.0 ? s : 1.0;
+    }
+    double* dst = X64 + ws_off[g];
+    for (int e = blockIdx.y * blockDim.x + threadIdx.x; e < ld * ld; e += gridDim.y * blockDim.x) {
+        const int r = e / ld, c = e - r * ld;
+        double v = 0.0;
+        if (r < n && c < n) {
+            const size_t o = panel32_off(r, c, ldp);
+            v = (double)src[o];
+            if (lo_plane) v += (double)src[o + lo_plane];
+            v *= mul;
+        }
+        dst[panel_off(r, c, ld)] = v;
+    }
+}
+
+struct Ns32Args {
+    const Tile32* tiles;
+    const float* A;        // X_k
+    const float* B;        // MODE 0: X_k, MODE 1: Y_k
+    float* Out;            // MODE 0: Y_k, MODE 1: X_{k+1}
+    double* partials;      // [n_tiles][4]
+    const int32_t* done_iter;
+    int64_t lo_plane;      // SPLIT: offset (floats) of the lo plane inside A, B, Out
+    int32_t n_tiles;
+};
+
+// SPLIT = 0: plain TF32 (operands truncated to 10 mantissa bits by the tensor core).
+// SPLIT = 1: "3xTF32": every operand is stored as hi + lo with hi = tf32(x), lo = x - hi, and a
+//            product is hi hi + hi lo + lo hi accumulated in the same FP32 TMEM tile (FP32-class
+//            accuracy, three MMAs per k step, 16-wide k slices so that a stage stays 48 KB).
+template <int MODE, int SPLIT>
+__global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
+    constexpr int BK = SPLIT ? R_BK / 2 : R_BK;     // k columns per stage
+    constexpr int PL = SPLIT ? 2 : 1;               // operand planes
+    constexpr int SA = R_BM * BK;                   // floats of one 128-row operand plane in a stage
+    extern __shared__ __align__(128) float rsm[];
+    __shared__ __align__(8) uint64_t s_full[R_STAGES], s_empty[R_STAGES], s_tfull[2], s_tempty[2];
+    __shared__ uint32_t s_tmem;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) {
+        for (int s = 0; s < R_STAGES; ++s) { r_mbar_init(&s_full[s], 1); r_mbar_init(&s_empty[s], 1); }
+        for (int b = 0; b < 2; ++b) { r_mbar_init(&s_tfull[b], 1); r_mbar_init(&s_tempty[b], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (wid == 1) {  // tensor memory: all 512 columns (one CTA per SM), two 256-column accumulators
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(r_smem_u32(&s_tmem)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem = s_tmem;
+
+    if (wid == 0) {
+        // ================================================================ producer (one thread)
+        if (lane == 0) {
+            int stage = 0;
+            unsigned phase = 0;
+            for (int t = blockIdx.x; t < a.n_tiles; t += gridDim.x) {
+                const Tile32 T = a.tiles[t];
+                if (a.done_iter[T.grp] >= 0) continue;
+                const int ldp = T.ldp;
+                const int row0 = T.ti * R_BM, rows_a = min(R_BM, ldp - row0);
+                const int col0 = T.tj * R_BN, ncols = min(R_BN, min(ldp, row0 + R_BM) - col0);  // lower triangle only
+                const int rows_b0 = min(128, ncols), rows_b1 = max(0, ncols - 128);
+                const float* Asrc = a.A + T.off32 + (size_t)row0 * ldp;
+                const float* B0 = a.B + T.off32 + (size_t)col0 * ldp;
+                const float* B1 = a.B + T.off32 + (size_t)(col0 + 128) * ldp;
+                for (int k0 = 0; k0 < ldp; k0 += BK) {
+                    const int chunks = min(BK, ldp - k0) >> 2;
+                    r_mbar_wait(&s_empty[stage], phase ^ 1);
+                    float* sa = rsm + (size_t)stage * R_STAGE_FLOATS;
+                    const unsigned ba = (unsigned)(chunks * rows_a * 16), bb0 = (unsigned)(chunks * rows_b0 * 16),
+                                   bb1 = (unsigned)(chunks * rows_b1 * 16);
+                    r_mbar_expect_tx(&s_full[stage], PL * (ba + bb0 + bb1));
+#pragma unroll
+                    for (int pl = 0; pl < PL; ++pl) {  // stage layout: [A planes][B0 planes][B1 planes]
+                        const size_t po = (size_t)pl * a.lo_plane;
+                        r_bulk_g2s(sa + pl * SA, Asrc + po + (size_t)(k0 >> 2) * rows_a * 4, ba, &s_full[stage]);
+                        r_bulk_g2s(sa + (PL + pl) * SA, B0 + po + (size_t)(k0 >> 2) * rows_b0 * 4, bb0, &s_full[stage]);
+                        if (rows_b1 > 0)
+                            r_bulk_g2s(sa + (2 * PL + pl) * SA, B1 + po + (size_t)(k0 >> 2) * rows_b1 * 4, bb1,
+                                       &s_full[stage]);
+                    }
+                    if (++stage == R_STAGES) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (wid == 1) {
+        // ================================================================ MMA issuer (one thread)
+        if (lane == 0) {
+            int stage = 0, buf = 0;
+            unsigned phase = 0, tphase[2] = {0, 0};
+            for (int t = blockIdx.x; t < a.n_tiles; t += gridDim.x) {
+                const Tile32 T = a.tiles[t];
+                if (a.done_iter[T.grp] >= 0) continue;
+                const int ldp = T.ldp;
+                const int row0 = T.ti * R_BM, rows_a = min(R_BM, ldp - row0);
+                const int col0 = T.tj * R_BN, ncols = min(R_BN, min(ldp, row0 + R_BM) - col0);
+                const int rows_b0 = min(128, ncols), rows_b1 = max(0, ncols - 128);
+                r_mbar_wait(&s_tempty[buf], tphase[buf] ^ 1);  // epilogue has drained this accumulator
+                asm volatile("tcgen05.fence::after_thread_sync;");
+                const uint32_t d0 = tmem + (uint32_t)(buf * R_BN);
+                const uint32_t id0 = r_idesc(rows_b0), id1 = r_idesc(rows_b1 > 0 ? rows_b1 : 16);
+                for (int k0 = 0; k0 < ldp; k0 += BK) {
+                    const int ksteps = min(BK, ldp - k0) >> 3;
+                    r_mbar_wait(&s_full[stage], phase);
+                    asm volatile("tcgen05.fence::after_thread_sync;");
+                    const unsigned sa = r_smem_u32(rsm + (size_t)stage * R_STAGE_FLOATS);
+                    const unsigned sb0 = sa + PL * SA * 4, sb1 = sa + 2 * PL * SA * 4;
+                    for (int ks = 0; ks < ksteps; ++ks) {
+                        const uint32_t acc = (k0 > 0 || ks > 0) ? 1u : 0u;
+                        const unsigned oa = (unsigned)(ks * 2 * rows_a * 16), ob0 = (unsigned)(ks * 2 * rows_b0 * 16),
+                                       ob1 = (unsigned)(ks * 2 * rows_b1 * 16);
+                        const unsigned la = (unsigned)(rows_a * 16), lb0 = (unsigned)(rows_b0 * 16), lb1 = (unsigned)(rows_b1 * 16);
+                        const uint64_t da = r_desc(sa + oa, la);
+                        r_mma(d0, da, r_desc(sb0 + ob0, lb0), id0, acc);                                  // hi hi
+                        if (SPLIT) {
+                            r_mma(d0, da, r_desc(sb0 + SA * 4 + ob0, lb0), id0, 1u);                      // hi lo
+                            r_mma(d0, r_desc(sa + SA * 4 + oa, la), r_desc(sb0 + ob0, lb0), id0, 1u);      // lo hi
+                        }
+                        if (rows_b1 > 0) {
+                            r_mma(d0 + 128, da, r_desc(sb1 + ob1, lb1), id1, acc);
+                            if (SPLIT) {
+                                r_mma(d0 + 128, da, r_desc(sb1 + SA * 4 + ob1, lb1), id1, 1u);
+                                r_mma(d0 + 128, r_desc(sa + SA * 4 + oa, la), r_desc(sb1 + ob1, lb1), id1, 1u);
+                            }
+                        }
+                    }
+                    r_commit(&s_empty[stage]);  // the stage is free once these MMAs have read it
+                    if (++stage == R_STAGES) { stage = 0; phase ^= 1; }
+                }
+                r_commit(&s_tfull[buf]);        // accumulator complete
+                tphase[buf] ^= 1;
+                buf ^= 1;
+            }
+        }
+    } else {
+        // ================================================================ epilogue warps 2..5
+        const int q = wid & 3;  // TMEM lane quarter this warp may access
+        int buf = 0;
+        unsigned tphase[2] = {0, 0};
+        for (int t = blockIdx.x; t < a.n_tiles; t += gridDim.x) {
+            const Tile32 T = a.tiles[t];
+            if (a.done_iter[T.grp] >= 0) continue;
+            const int ldp = T.ldp, n = T.n;
+            const int row0 = T.ti * R_BM, rows_a = min(R_BM, ldp - row0);
+            const int col0 = T.tj * R_BN, ncols = min(R_BN, min(ldp, row0 + R_BM) - col0);
+            const int rl = q * 32 + lane, r = row0 + rl;
+            r_mbar_wait(&s_tfull[buf], tphase[buf]);
+            tphase[buf] ^= 1;
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * R_BN);
+            float* orow = a.Out + T.off32 + (size_t)row0 * ldp + (size_t)rl * 4;
+            const float* xrow = a.A + T.off32 + (size_t)row0 * ldp + (size_t)rl * 4;
+            double part = 0.0;
+            for (int c0 = 0; c0 < ncols; c0 += 16) {
+                uint32_t v[16];
+                asm volatile(
+                    "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                    : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                      "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                    : "r"(taddr + (uint32_t)c0));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (rl < rows_a) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int c = col0 + c0 + 4 * j;
+                        if (c > r) continue;  // upper triangle: the mirror image of (c, r) is stored instead
+                        const size_t o = (size_t)(c >> 2) * rows_a * 4;
+                        float w[4] = {__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
+                                      __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3])};
+                        if (MODE == 0) {
+                            if (r < n) {  // residual over the n x n part; strictly-lower elements count twice
+                                float p = 0.f;
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) {
+                                    const float d = w[e] - (c + e == r ? 1.f : 0.f);
+                                    if (c + e < r) p += 2.f * d * d;
+                                    else if (c + e == r) p += d * d;
+                                }
+                                part += (double)p;
+                            }
+                        } else {
+                            float4 x = *reinterpret_cast<const float4*>(xrow + o);
+                            if (SPLIT) {
+                                const float4 xl = *reinterpret_cast<const float4*>(xrow + o + a.lo_plane);
+                                x.x += xl.x; x.y += xl.y; x.z += xl.z; x.w += xl.w;
+                            }
+                            w[0] = 1.5f * x.x - 0.5f * w[0]; w[1] = 1.5f * x.y - 0.5f * w[1];
+                            w[2] = 1.5f * x.z - 0.5f * w[2]; w[3] = 1.5f * x.w - 0.5f * w[3];
+                        }
+                        float hi[4], lo[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            hi[e] = SPLIT ? r_tf32(w[e]) : w[e];
+                            lo[e] = w[e] - hi[e];
+                        }
+                        // direct elements (r, c + e), c + e <= r: one 16-byte store when the whole group is
+                        // on or below the diagonal; mirror elements (c + e, r), c + e < r: 4-byte stores.
+                        // Every stored element has exactly one writer, so X and Y stay bitwise symmetric,
+                        // which is what lets B be read as rows (and keeps the iteration stable: the
+                        // X X^T form amplifies any antisymmetric rounding noise).
+                        if (c + 3 <= r) {
+                            *reinterpret_cast<float4*>(orow + o) = make_float4(hi[0], hi[1], hi[2], hi[3]);
+                            if (SPLIT) *reinterpret_cast<float4*>(orow + o + a.lo_plane) = make_float4(lo[0], lo[1], lo[2], lo[3]);
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < 4; ++e)
+                                if (c + e <= r) {
+                                    orow[o + e] = hi[e];
+                                    if (SPLIT) orow[o + e + a.lo_plane] = lo[e];
+                                }
+                        }
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (c + e < r) {
+                                float* mp = a.Out + T.off32 + panel32_off(c + e, r, ldp);
+                                *mp = hi[e];
+                                if (SPLIT) mp[a.lo_plane] = lo[e];
+                            }
+                    }
+                }
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            __syncwarp();
+            if (lane == 0) r_mbar_arrive(&s_tempty[buf]);
+            if (MODE == 0) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+                if (lane == 0) a.partials[(size_t)T.tile * 4 + q] = part;
+            }
+            buf ^= 1;
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (wid == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+}
+
+// Residual decision of the reduced-precision iteration: like k_ns_decide, but the residual has a
+// precision floor.  r < 1/(2 sqrt(n)) means every eigenvalue satisfies |1 - x^2| < 1/2, i.e. the
+// exact iteration at least halves r from there on; "two consecutive residuals inside that zone and
+// no halving" is therefore the precision floor: the submatrix stops as converged-to-the-floor, and
+// the floor is reported in sm_stats_t.max_residual.  Hard cap of 40 iterations (noise cannot be
+// iterated away).
+__global__ void __launch_bounds__(256)
+k_ns_decide32(int ngroups, int k, int decide_only, double eps, double floor_zone,
+              const int32_t* __restrict__ tile_first,
+              const int32_t* __restrict__ tile_count, const int32_t* __restrict__ sub_dim,
+              const double* __restrict__ partials, double* __restrict__ res, int32_t* __restrict__ done_iter,
+              int32_t* __restrict__ flag, int32_t* __restrict__ counters) {
+    const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (g >= ngroups) return;
+    if (done_iter[g] >= 0) return;
+    const int lane = threadIdx.x & 31;
+    const int cnt = 4 * tile_count[g], n = sub_dim[g];
+    const double* pp = partials + (size_t)tile_first[g] * 4;
+    double r2 = 0.0;
+    for (int t = lane; t < cnt; t += 32) r2 += pp[t];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+    if (lane == 0) {
+        const double r = sqrt(r2 / (double)(n > 0 ? n : 1));
+        const double prev = k > 0 ? res[(size_t)((k - 1) & 1) * ngroups + g] : 1e300;
+        const bool conv = r < eps;
+        const double zone = floor_zone / sqrt((double)(n > 0 ? n : 1));
+        const bool floor_hit = (k > 0) && (prev < zone) && (r < zone) && (r >= 0.5 * prev);
+        const bool stop = conv || floor_hit || decide_only || k >= 40 || !(r == r);
+        res[(size_t)(k & 1) * ngroups + g] = r;
+        if (stop) { flag[g] = (conv || floor_hit) ? 0 : 1; done_iter[g] = k; }
+        else atomicAdd(counters + k, 1);
+    }
+}
+
+// Tile list and FP32 offsets of the reduced-precision path (plan creation, precision = 1).
+sm_status_t build_tf32_tables(sm_plan* p, cudaStream_t st) {
+    const int ng = p->ngroups;
+    std::vector<int64_t> off32(ng);
+    std::vector<int32_t> first(ng), count(ng);
+    std::vector<Tile32> tiles;
+    int64_t off = 0;
+    for (int g = 0; g < ng; ++g) {
+        const int n = p->h_sub_dim[g], ldp = (n + 15) & ~15;
+        off32[g] = off;
+        off += (int64_t)ldp * ldp;
+        first[g] = (int32_t)tiles.size();
+        for (int ti = 0; ti * R_BM < ldp; ++ti)
+            for (int tj = 0; tj * R_BN < std::min(ldp, (ti + 1) * R_BM); ++tj) {  // lower triangle only
+                Tile32 t;
+                t.off32 = off32[g]; t.grp = g; t.ldp = ldp; t.n = n; t.ti = ti; t.tj = tj; t.tile = (int32_t)tiles.size();
+                tiles.push_back(t);
+            }
+        count[g] = (int32_t)tiles.size() - first[g];
+    }
+    p->sum_ldp2 = off;
+    const int planes = p->opt.precision == 2 ? 2 : 1;
+    p->n_tiles32 = (int64_t)tiles.size();
+    auto up = [&](void** d, const void* h, size_t bytes) -> sm_status_t {
+        SM_CUDA(cudaMalloc(d, std::max<size_t>(bytes, 16)));
+        if (bytes) SM_CUDA(cudaMemcpyAsync(*d, h, bytes, cudaMemcpyHostToDevice, st));
+        return SM_OK;
+    };
+    sm_status_t s;
+    if ((s = up((void**)&p->d_ws_off32, off32.data(), (size_t)ng * 8))) return s;
+    if ((s = up((void**)&p->d_tile_first32, first.data(), (size_t)ng * 4))) return s;
+    if ((s = up((void**)&p->d_tile_count32, count.data(), (size_t)ng * 4))) return s;
+    if ((s = up((void**)&p->d_tiles32, tiles.data(), tiles.size() * sizeof(Tile32)))) return s;
+    SM_CUDA(cudaMalloc((void**)&p->d_partials32, std::max<size_t>((size_t)tiles.size() * 32, 16)));
+    SM_CUDA(cudaStreamSynchronize(st));
+    // each of the three workspace buffers must hold the FP64 matrices and the FP32 ones
+    const size_t need = std::max((size_t)p->sum_ld2 * 8, (size_t)p->sum_ldp2 * 4 * planes);
+    const size_t buf = (need + 255) / 256 * 256;
+    p->info.workspace_bytes = 3 * buf;
+    return SM_OK;
+}
+
+// buf0: gathered FP64 a_i - mu I (in), afterwards Y (FP32) during the iteration and the FP64 result
+// at the end; buf1 / bufY: X ping / pong (FP32).
+sm_status_t launch_to_f32(sm_plan* p, const double* buf0, double* buf1, cudaStream_t st) {
+    if (p->ngroups == 0) return SM_OK;
+    const int split = (int)std::min<int64_t>(8, std::max<int64_t>(1, (int64_t)p->num_sms * 8 / p->ngroups));
+    k_to_f32<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
+                                                       p->d_gersh, buf0, reinterpret_cast<float*>(buf1),
+                                                       p->opt.precision == 2 ? p->sum_ldp2 : 0);
+    p->launches++;
+    SM_CUDA(cudaGetLastError());
+    return SM_OK;
+}
+
+sm_status_t launch_to_f64(sm_plan* p, double* buf0, const double* buf1, const double* bufY, cudaStream_t st) {
+    if (p->ngroups == 0) return SM_OK;
+    const int split = (int)std::min<int64_t>(8, std::max<int64_t>(1, (int64_t)p->num_sms * 8 / p->ngroups));
+    k_to_f64<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
+                                                       p->d_gersh, p->d_done_iter, p->cur_k,
+                                                       reinterpret_cast<const float*>(buf1),
+                                                       reinterpret_cast<const float*>(bufY), buf0,
+                                                       p->opt.precision == 2 ? p->sum_ldp2 : 0);
+    p->launches++;
+    SM_CUDA(cudaGetLastError());
+    return SM_OK;
+}
+
+sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
+                                double* bufY, cudaStream_t st, int which) {
+    if (p->n_tiles32 == 0) return SM_OK;
+    static bool attr_set = false;
+    if (!attr_set) {
+        SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
+        attr_set = true;
+    }
+    float* X[2] = {reinterpret_cast<float*>(buf1), reinterpret_cast<float*>(bufY)};
+    float* Y = reinterpret_cast<float*>(buf0);
+    Ns32Args a;
+    a.tiles = reinterpret_cast<const Tile32*>(p->d_tiles32); a.partials = p->d_partials32; a.done_iter = p->d_done_iter;
+    a.n_tiles = (int32_t)p->n_tiles32;
+    const bool split = p->opt.precision == 2;
+    a.lo_plane = split ? p->sum_ldp2 : 0;
+    const int grid = (int)std::min<int64_t>(p->n_tiles32, p->num_sms);
+    if (which & 1) {
+        a.A = X[k & 1]; a.B = X[k & 1]; a.Out = Y;
+        if (split) k_ns_tf32<0, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        else k_ns_tf32<0, 0><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        k_ns_decide32<<<(p->ngroups + 7) / 8, 256, 0, st>>>(p->ngroups, k, decide_only, eps, 0.5,
+                                                            p->d_tile_first32,
+                                                            p->d_tile_count32, p->d_sub_dim, p->d_partials32, p->d_res,
+                                                            p->d_done_iter, p->d_flag, p->d_counters);
+        p->launches += 2;
+    }
+    if ((which & 2) && !decide_only) {
+        a.A = X[k & 1]; a.B = Y; a.Out = X[(k + 1) & 1];
+        if (split) k_ns_tf32<1, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        else k_ns_tf32<1, 0><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        p->launches += 1;
+    }
+    SM_CUDA(cudaGetLastError());
+    return SM_OK;
+}
+
+}  // namespace smb

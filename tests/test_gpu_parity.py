@@ -415,6 +415,52 @@ def test_density_matrix_unreachable_tolerance_is_guarded(B, cfg0):
     B.sm_plan_destroy(plan)
 
 
+# ------------------------------------------------------------------------------ reduced precision
+@pytest.mark.parametrize("precision,tol_d,tol_e", [(2, 1e-4, 1e-5), (1, 5e-3, 2e-3)])
+def test_reduced_precision_variants(B, oracle, cfg0, precision, tol_d, tol_e):
+    """Opt-in tcgen05 variants (north_star: <= 1e-3 elementwise, energy error reported): precision 2
+    ("3xTF32", FP32-class) must be far inside the bar, precision 1 (plain TF32) is the ~2e-3 class the
+    survey predicts (A16).  Cases: config 0; dense n = 256 (two B halves, closed form); DZVP blocks with
+    n > 256 (several column tiles); ragged blocks with tiny submatrices (n < 16)."""
+    cases = [cfg0, W.dense_batch_as_blocks(W.haar_spectrum_batch(6, 256, seed=3)[0]),
+             W.water_like(16, "DZVP", 6.0, seed=3), W.random_block_pattern(nb=30, density=0.2, max_bs=5, seed=11)]
+    for m in cases:
+        idx = oracle.Index(m)
+        lam, w, ptr, g = oracle.eig_groups(idx, m.values)
+        mu = 0.0
+        if np.abs(lam - mu).min() < 0.05:  # keep the test away from (near-)singular submatrices
+            srt = np.sort(lam)
+            k = int(np.argmax(np.diff(srt)))
+            mu = 0.5 * (srt[k] + srt[k + 1])
+        d_or = oracle.density(idx, m.values, mu)
+        eps = 2e-6 if precision == 2 else 1e-5
+        plan, st, d, stats, ws, vin = _run_sign(B, m, mu=mu, eps=eps, opt=B.default_options(precision=precision))
+        assert st == B.SM_OK, (st, stats.not_converged, stats.max_residual)
+        gap = np.abs(lam - mu).min()
+        err = np.abs(d - d_or).max()
+        assert err <= tol_d / min(1.0, gap / 0.3), (err, gap, idx.sub_dim.max())
+        _, tdk_o = oracle.traces(idx, d_or, m.values)
+        _, tdk_g = B.sm_trace_dk(plan, _torch().from_numpy(d).cuda(), vin)
+        assert abs(tdk_g - tdk_o) <= tol_e * max(abs(tdk_o), 1.0) / min(1.0, gap / 0.3)
+        B.sm_plan_destroy(plan)
+
+
+def test_reduced_precision_bisection(B, oracle, cfg0):
+    """sm_density_matrix on the 3xTF32 path lands on the same plateau (no steering early-out there)."""
+    torch = _torch()
+    m = cfg0
+    plan = B.plan_from_matrix(m, B.default_options(precision=2))
+    ws = B.alloc_workspace(plan)
+    vin = torch.from_numpy(m.values).cuda()
+    vout = torch.empty_like(vin)
+    stats = B.sm_stats_t()
+    st, mu = B.sm_density_matrix(plan, vin, float(m.n_occ), 0.5, 2e-6, -1.0, vout, ws, stats)
+    assert st == B.SM_OK and abs(stats.n_elec - m.n_occ) < 1e-2
+    idx = oracle.Index(m)
+    assert np.abs(vout.cpu().numpy() - oracle.density(idx, m.values, mu)).max() <= 1e-4
+    B.sm_plan_destroy(plan)
+
+
 def test_host_buffer_entry_point(B, oracle, cfg0):
     torch = _torch()
     m = cfg0
