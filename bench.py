@@ -202,8 +202,28 @@ def run_phases(args, m, B, torch):
     out["sign"] = {"ms_sign": d["ms_sign"], "iter_min": d["iter_min"], "iter_max": d["iter_max"],
                    "gemm_launches": d["gemm_launches"], "alg_TFLOPs": d["tot_sym_flop"] / d["ms_sign"] / 1e9,
                    "ms_gather": d["ms_gather"], "ms_scatter": d["ms_scatter"], "ms_total": d["ms_total"]}
-    print(json.dumps(out), flush=True)
+    # opt-in reduced-precision variants (tcgen05): accuracy against the FP64 result, reported separately
+    d64 = vout.clone()
+    _, tdk64 = B.sm_trace_dk(plan, d64, vin)
     B.sm_plan_destroy(plan)
+    del ws
+    out["reduced_precision"] = {}
+    for prec, name, eps in ((2, "3xTF32 (hi/lo split)", 2e-6), (1, "TF32", 1e-5)):
+        plan = B.plan_from_matrix(m, B.default_options(precision=prec))
+        ws = B.alloc_workspace(plan)
+        B.sm_set_timing(plan, True)
+        for _ in range(2):
+            rc = B.sm_sign_execute(plan, vin, 0.0, eps, vout, ws, st)
+        torch.cuda.synchronize()
+        d = st.as_dict()
+        _, tdk = B.sm_trace_dk(plan, vout, vin)
+        out["reduced_precision"][name] = {
+            "status": int(rc), "ms_sign": d["ms_sign"], "iter_min": d["iter_min"], "iter_max": d["iter_max"],
+            "residual_floor": d["max_residual"], "max_abs_err_vs_fp64": float((vout - d64).abs().max().item()),
+            "rel_band_energy_err_vs_fp64": abs(tdk - tdk64) / abs(tdk64), "n_elec": d["n_elec"]}
+        B.sm_plan_destroy(plan)
+        del ws
+    print(json.dumps(out), flush=True)
 
 
 def workload_config(args, m):
