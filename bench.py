@@ -68,6 +68,13 @@ class ClockSampler:
         except OSError:
             self.p = None
 
+    def mark(self):
+        """Samples written before this call (warm-up) are ignored by stop()."""
+        try:
+            self.skip = os.path.getsize(self.f.name)
+        except OSError:
+            self.skip = 0
+
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
         if self.p is None:
@@ -78,7 +85,8 @@ class ClockSampler:
         except subprocess.TimeoutExpired:
             self.p.kill()
         self.f.flush()
-        self.f.seek(0)
+        self.f.seek(getattr(self, "skip", 0))
+        self.f.readline()  # the (possibly partial) line the mark fell into
         sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f.read().splitlines():
@@ -304,13 +312,14 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # the clock sampler attaches BEFORE the warm-up (nvidia-smi's start-up stalls synchronous CUDA calls
+    # for a while); only the samples taken during the timed region are kept
+    sampler = ClockSampler(local_rank) if rank == 0 else None
     for _ in range(args.warmup):
         st, mu = step_device()
     barrier()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
     if sampler is not None:
-        time.sleep(1.5)  # let nvidia-smi finish attaching (its start-up stalls synchronous CUDA calls)
-        barrier()
+        sampler.mark()
     launches0 = B.sm_launch_count(plan)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     gemm_ms = gemm_launches = sym_flop = n3 = evals = 0.0

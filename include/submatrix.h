@@ -82,8 +82,9 @@ typedef struct {
                          /* proves the sign of n_elec - n_target (reading A11c); such a step */
                          /* only steers, it is never accepted.  0: every evaluation converges*/
     int32_t reserved_i;
-    double overshoot;    /* scaling = 1 only: s = bound / overshoot, 1 <= overshoot <= 1.5 [1.25]*/
-                         /* (eigenvalues of X0 in (1, 1.5] map back into [0.56, 1))          */
+    double overshoot;    /* scaling = 1 only: s = bound / overshoot, 1 <= overshoot <= 1.5 [1.45]*/
+                         /* (eigenvalues of X0 in (1, 1.5] map back into [0.56, 1); 1.45 is   */
+                         /* where the top and the bottom of the water-like spectra balance)  */
     int32_t reserved[4];
 } sm_options_t;
 

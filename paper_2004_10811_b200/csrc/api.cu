@@ -24,7 +24,7 @@ static void default_options(sm_options_t* o) {
     o->max_iter = 100;
     o->scaling = 1;
     o->early_out = 1;
-    o->overshoot = 1.25;
+    o->overshoot = 1.45;
     o->precision = 0;
     o->check_every = 1;
     o->max_mu_steps = 64;
