@@ -103,6 +103,11 @@ typedef struct {
     int32_t n_buckets;        /* distinct padded sizes                                       */
     int32_t reserved0;
     size_t workspace_bytes;   /* what sm_sign_execute / sm_density_matrix need               */
+    int64_t sum_n3_columns;   /* sum over single block columns c of n~_c^3, n~_c = rows of the */
+                              /* submatrix generated by column c alone (numerator of Eq.(15))  */
+    double est_speedup;       /* Eq.(15): S = sum_c n~_c^3 / sum_i n_i^3, the estimated    */
+                              /* additional speed-up of this grouping over per-column          */
+                              /* submatrices under the O(n^3) cost model of Eq.(14)       */
 } sm_plan_info_t;
 
 /* Filled by sm_sign_execute / sm_density_matrix (may be NULL). Times are CUDA-event ms of the

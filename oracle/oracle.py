@@ -163,6 +163,18 @@ def traces(idx: Index, D, K, cols=None):
     return td.value, tdk.value
 
 
+def flop_model(m, idx: "Index"):
+    """PAPER.md Eq.(14) L201 and Eq.(15), written out: operations ~ sum_i n_i^3 for the given
+    grouping; S = sum over single block columns c of n~_c^3 (n~_c = dimension of the submatrix that
+    column c alone generates = total height of its stored blocks) divided by that."""
+    ops = sum(int(n) ** 3 for n in idx.sub_dim)
+    ops_cols = 0
+    for c in range(m.nb):
+        rows = m.rowidx[m.colptr[c]:m.colptr[c + 1]]
+        ops_cols += int(m.blk_size[rows].sum()) ** 3
+    return ops, ops_cols, (ops_cols / ops if ops else 0.0)
+
+
 def gershgorin_interval(m) -> tuple[float, float]:
     """Gershgorin interval of the whole block-sparse matrix: bracket for the mu loop (A11)."""
     cols = m.block_cols()

@@ -43,7 +43,8 @@ class sm_plan_info_t(C.Structure):
                 ("n_basis", C.c_int64), ("sum_sub_blocks", C.c_int64), ("dim_min", C.c_int32),
                 ("dim_max", C.c_int32), ("dim_mean", C.c_double), ("sum_n2", C.c_int64), ("sum_n3", C.c_int64),
                 ("sum_ld2", C.c_int64), ("n_tiles", C.c_int64), ("n_buckets", C.c_int32),
-                ("reserved0", C.c_int32), ("workspace_bytes", C.c_size_t)]
+                ("reserved0", C.c_int32), ("workspace_bytes", C.c_size_t), ("sum_n3_columns", C.c_int64),
+                ("est_speedup", C.c_double)]
 
 
 class sm_stats_t(C.Structure):

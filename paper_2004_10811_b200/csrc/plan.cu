@@ -294,6 +294,15 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     I.sum_n2 = n2; I.sum_n3 = n3; I.sum_ld2 = p->sum_ld2; I.n_tiles = p->n_tiles; I.n_buckets = nbuckets;
     const size_t buf = ((size_t)p->sum_ld2 * 8 + 255) / 256 * 256;
     I.workspace_bytes = 3 * buf;
+    // cost model of the grouping (Eq.(14), Eq.(15)): integer sums on the host
+    int64_t n3c = 0;
+    for (int c = 0; c < nb; ++c) {
+        int64_t nc = 0;
+        for (int64_t q = p->h_colptr[c]; q < p->h_colptr[c + 1]; ++q) nc += p->h_blk_size[p->h_rowidx[q]];
+        n3c += nc * nc * nc;
+    }
+    I.sum_n3_columns = n3c;
+    I.est_speedup = n3 > 0 ? (double)n3c / (double)n3 : 0.0;
     return SM_OK;
 }
 

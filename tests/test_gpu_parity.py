@@ -95,6 +95,8 @@ def test_index_bit_exact_full_size(B, oracle):
         info = B.sm_plan_query(plan)
         assert info.nnz == len(m.values) and info.ngroups == m.ngroups
         assert info.sum_n3 == int((idx.sub_dim.astype(np.int64) ** 3).sum())
+        ops, ops_cols, S = oracle.flop_model(m, idx)  # Eq.(14)/(15): integer sums, exact
+        assert (info.sum_n3, info.sum_n3_columns) == (ops, ops_cols) and abs(info.est_speedup - S) <= 1e-12 * S
         B.sm_plan_destroy(plan)
 
 
@@ -213,6 +215,13 @@ def test_config4_sampled_parity_full_size(B, oracle):
 
 
 # ------------------------------------------------------------------------------ edge cases
+def test_large_member_count_chunked_block_map(B, oracle):
+    """|S_i| = 288 members: the gather's block map does not fit its shared-memory budget and is
+    built in chunks of member columns; n = 576 also spans nine row tiles of the GEMM."""
+    m = W.water_like(96, "SZV", 9.0, seed=5)
+    _sampled_parity(B, oracle, m, 4)
+
+
 def test_ragged_blocks_and_scattered_groups(B, oracle):
     for seed in range(3):
         m = W.random_block_pattern(nb=30 + seed, density=0.2, max_bs=7, seed=10 + seed)

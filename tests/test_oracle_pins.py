@@ -291,3 +291,24 @@ def test_bisection_finds_gap_plateau(oracle, cfg0):
                                      mu_tol=1e-6, max_steps=64)
     assert abs(ne2 - m.n_occ) > 1e-8 and len(tr2) <= 64  # unreachable by construction
     assert abs(ne2 - m.n_occ) < 1e-2
+
+
+def test_flop_model_eq14_eq15(oracle):
+    """Eq.(14)/(15): with one group per block column the estimated speed-up is exactly 1; merging all
+    columns into one group gives S = sum_c n~_c^3 / n_basis^3; a hand-worked 3-column case."""
+    from paper_2004_10811_b200 import workloads as W
+    import dataclasses
+    m = W.random_block_pattern(nb=12, density=0.3, max_bs=4, seed=2)
+    per_col = dataclasses.replace(m, grp_ptr=np.arange(m.nb + 1, dtype=np.int32), grp_cols=np.arange(m.nb, dtype=np.int32))
+    ops, ops_cols, S = oracle.flop_model(per_col, oracle.Index(per_col))
+    assert ops == ops_cols and S == 1.0
+    one = dataclasses.replace(m, grp_ptr=np.array([0, m.nb], np.int32), grp_cols=np.arange(m.nb, dtype=np.int32))
+    idx1 = oracle.Index(one)
+    ops1, ops_cols1, S1 = oracle.flop_model(one, idx1)
+    assert ops_cols1 == ops_cols and ops1 == int(idx1.sub_dim[0]) ** 3
+    # tridiagonal block pattern, sizes 2,3,1: columns generate n~ = 5, 6, 4; groups {0,1},{2}: n = 6, 4
+    tri = W.BlockSparseSym(3, np.array([2, 3, 1], np.int32), np.array([0, 2, 5, 7], np.int64),
+                           np.array([0, 1, 0, 1, 2, 1, 2], np.int32), np.zeros(4 + 6 + 6 + 9 + 3 + 3 + 1),
+                           np.array([0, 2, 3], np.int32), np.array([0, 1, 2], np.int32))
+    ops, ops_cols, S = oracle.flop_model(tri, oracle.Index(tri))
+    assert (ops, ops_cols) == (6 ** 3 + 4 ** 3, 5 ** 3 + 6 ** 3 + 4 ** 3) and abs(S - 405 / 280) < 1e-15
