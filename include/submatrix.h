@@ -81,7 +81,10 @@ typedef struct {
                          /* |n_elec(final) - n_elec(X_k)| <= 1/2 sum_gen (1 - (X_k^2)_kk)     */
                          /* proves the sign of n_elec - n_target (reading A11c); such a step */
                          /* only steers, it is never accepted.  0: every evaluation converges*/
-    int32_t reserved_i;
+    int32_t order;       /* 2: Newton-Schulz X <- 1/2 X (3I - X^2), Eq.(11) L97          [2]  */
+                         /* 3: the paper's GPU iteration X <- 1/8 X (15I - 10X^2 + 3X^4),     */
+                         /*    Eq.(19) L348 (three products per iteration, one more          */
+                         /*    workspace buffer, FP64 only, overshoot forced to 1)           */
     double overshoot;    /* scaling = 1 only: s = bound / overshoot, 1 <= overshoot <= 1.5 [1.45]*/
                          /* (eigenvalues of X0 in (1, 1.5] map back into [0.56, 1); 1.45 is   */
                          /* where the top and the bottom of the water-like spectra balance)  */

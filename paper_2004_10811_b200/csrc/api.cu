@@ -25,6 +25,7 @@ static void default_options(sm_options_t* o) {
     o->scaling = 1;
     o->early_out = 1;
     o->overshoot = 1.45;
+    o->order = 2;
     o->precision = 0;
     o->check_every = 1;
     o->max_mu_steps = 64;
@@ -111,6 +112,12 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (!(p->opt.mu_tol > 0)) p->opt.mu_tol = 1e-6;
     if (!(p->opt.overshoot >= 1.0)) p->opt.overshoot = 1.0;     // zero-initialised struct: no overshoot
     if (p->opt.overshoot > 1.5) p->opt.overshoot = 1.5;         // f(x) = x(3 - x^2)/2 keeps [1, 1.5] inside [0.56, 1]
+    if (p->opt.order == 0) p->opt.order = 2;                    // zero-initialised struct: Eq.(11)
+    if (p->opt.order != 2 && p->opt.order != 3) { delete p; return SM_ERR_INVALID_ARG; }
+    if (p->opt.order == 3) {
+        if (p->opt.precision != 0) { delete p; return SM_ERR_INVALID_ARG; }
+        p->opt.overshoot = 1.0;  // Eq.(19)'s map is increasing beyond 1: eigenvalues of X0 must not exceed 1
+    }
     if (p->opt.precision < 0 || p->opt.precision > 2 || p->opt.scaling < 0 || p->opt.scaling > 1) { delete p; return SM_ERR_INVALID_ARG; }
     p->nb = nb; p->ngroups = ngroups; p->nnzb = nb ? colptr[nb] : 0;
     p->h_blk_size.assign(blk_size, blk_size + nb);
@@ -129,6 +136,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     s = build_index_device(p, st);
     if (s) { sm_plan_destroy(p); return s; }
     if (p->opt.precision != 0 && (s = build_tf32_tables(p, st))) { sm_plan_destroy(p); return s; }
+    if (p->opt.order == 3) p->info.workspace_bytes = p->info.workspace_bytes / 3 * 4;  // + W of Eq.(19)
     // per-evaluation state
     const int ng = std::max(ngroups, 1);
     auto A = [&](void** d, size_t bytes) { return cudaMalloc(d, std::max<size_t>(bytes, 8)); };
@@ -139,7 +147,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_gersh, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_partials, (size_t)p->n_tiles * 4 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_counters, (size_t)(p->opt.max_iter + 2) * 4);
-    if (e == cudaSuccess) e = A((void**)&p->d_sched, (size_t)(p->opt.max_iter + 2) * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_sched, (size_t)(p->opt.max_iter + 2) * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_tile_done, (size_t)ng * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_ne_part, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_scalars, 8 * 8);
@@ -228,16 +236,17 @@ extern "C" int64_t sm_launch_count(const sm_plan_t* p) { return p ? p->launches 
 
 namespace {
 struct Bufs {
-    double *b0, *b1, *y;
+    double *b0, *b1, *y, *w;
 };
 sm_status_t carve(const sm_plan* p, void* ws, size_t bytes, Bufs* b) {
     if (bytes < p->info.workspace_bytes) return SM_ERR_WORKSPACE_TOO_SMALL;
     if (!ws && p->info.workspace_bytes) return SM_ERR_INVALID_ARG;
     if (((uintptr_t)ws & 255) != 0) return SM_ERR_INVALID_ARG;
-    const size_t buf = p->info.workspace_bytes / 3;
+    const size_t buf = p->info.workspace_bytes / (p->opt.order == 3 ? 4 : 3);
     b->b0 = (double*)ws;
     b->b1 = (double*)((char*)ws + buf);
     b->y = (double*)((char*)ws + 2 * buf);
+    b->w = p->opt.order == 3 ? (double*)((char*)ws + 3 * buf) : nullptr;
     return SM_OK;
 }
 
@@ -246,7 +255,7 @@ sm_status_t reset_state(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMemsetAsync(p->d_done_iter, 0xff, (size_t)ng * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_flag, 0, (size_t)ng * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_counters, 0, (size_t)(p->opt.max_iter + 2) * 4, st));
-    SM_CUDA(cudaMemsetAsync(p->d_sched, 0, (size_t)(p->opt.max_iter + 2) * 8, st));
+    SM_CUDA(cudaMemsetAsync(p->d_sched, 0, (size_t)(p->opt.max_iter + 2) * 16, st));
     SM_CUDA(cudaMemsetAsync(p->d_tile_done, 0, (size_t)ng * 4, st));
     p->cur_k = 0;
     return SM_OK;
@@ -264,7 +273,7 @@ struct Steer {
 // One iteration's launches on the path the plan was created for (FP64 DMMA, or TF32 tcgen05).
 sm_status_t launch_pair(sm_plan* p, int k, double eps, int last, const Bufs& b, cudaStream_t st, int which) {
     if (p->opt.precision != 0) return launch_ns_pair_tf32(p, k, eps, last, b.b0, b.b1, b.y, st, which);
-    return launch_ns_pair(p, k, eps, last, b.b0, b.b1, b.y, st, which);
+    return launch_ns_pair(p, k, eps, last, b.b0, b.b1, b.y, st, which, b.w);
 }
 
 // Newton-Schulz host loop: iterations k = cur_k .. k_end-1 (each = MODE 0 + MODE 1 launch).
@@ -313,7 +322,7 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
             if (r == 2) { p->cur_k = k; p->half_iter = 1; return SM_OK; }  // X_k in buf[k & 1], not converged
             if (last) break;
             if ((s = launch_pair(p, k, eps, 0, b, st, 2))) return s;
-            (*launched) += 1;
+            (*launched) += p->opt.order == 3 ? 2 : 1;
         }
         p->cur_k = std::min(k, max_iter);
         if (k >= max_iter) *all_done = 1;
@@ -322,7 +331,7 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
     for (; k < k_end && k <= max_iter; ++k) {
         sm_status_t s = launch_pair(p, k, eps, k == max_iter ? 1 : 0, b, st, 3);
         if (s) return s;
-        (*launched) += (k == max_iter) ? 1 : 2;
+        (*launched) += (k == max_iter) ? 1 : (p->opt.order == 3 ? 3 : 2);
         if (pending >= 0) {
             SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
             if (poll(pending) == 1) return SM_OK;
@@ -369,7 +378,8 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         int64_t n = p->h_sub_dim[i];
         // executed symmetric products: stopped at iteration it: one X^2 per tested iterate (it + 1)
         // and one update per iteration (it); still active after cur_k launch pairs: 2 cur_k (+1 if a steering decision came between the two modes)
-        const int64_t prods = di[i] >= 0 ? 2 * it + 1 : 2 * (int64_t)p->cur_k + p->half_iter;
+        const int64_t ppi = p->opt.order == 3 ? 3 : 2;  // products per iteration (Eq.(11): 2, Eq.(19): 3)
+        const int64_t prods = di[i] >= 0 ? ppi * it + 1 : ppi * (int64_t)p->cur_k + p->half_iter;
         sin3 += prods * n * n * n;
         symf += prods * n * n * (n + 1);
     }
@@ -422,7 +432,7 @@ sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, cons
     if ((s = collect_stats(p, stats, not_conv, st))) return s;
     if (stats) {
         if (steer && steer->decided) stats->n_elec = steer->ne;
-        stats->iterations = launched / 2;
+        stats->iterations = launched / (p->opt.order == 3 ? 3 : 2);
         stats->gemm_launches = launched;
         stats->mu = mu;
         if (p->timing) {
@@ -502,7 +512,7 @@ extern "C" sm_status_t sm_sign_iterate(sm_plan_t* p, double eps, void* d_workspa
     if ((s = ns_loop(p, b, eps, p->opt.max_iter + 1, &all_done, &launched, st))) return s;
     if ((s = launch_nelec(p, b.b0, b.b1, st))) return s;
     if ((s = collect_stats(p, stats, &nc, st))) return s;
-    if (stats) { stats->iterations = launched / 2; stats->gemm_launches = launched; }
+    if (stats) { stats->iterations = launched / (p->opt.order == 3 ? 3 : 2); stats->gemm_launches = launched; }
     return nc ? SM_WARN_SIGN_NOT_CONVERGED : SM_OK;
 }
 
@@ -578,7 +588,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
             if ((s = ns_loop(p, b, eps, p->opt.max_iter + 1, &all_done, &launched, st))) return s;
             if ((s = launch_nelec(p, b.b0, b.b1, st))) return s;
             if ((s = collect_stats(p, &ev, &nc, st))) return s;
-            ev.iterations += launched / 2;
+            ev.iterations += launched / (p->opt.order == 3 ? 3 : 2);
             ev.tot_gemm_launches += launched;
             ev.tot_sum_iter_n3 = ev.sum_iter_n3;
             g = ev.n_elec - n_target;

@@ -145,5 +145,5 @@ sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t s
 sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStream_t st);
 // ns_sign.cu
 sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
-                           double* bufY, cudaStream_t st, int which = 3);
+                           double* bufY, cudaStream_t st, int which = 3, double* bufW = nullptr);
 }  // namespace smb

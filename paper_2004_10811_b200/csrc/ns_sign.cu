@@ -39,6 +39,17 @@
 namespace smb {
 
 constexpr int BM = TILE, BN = TILE, BK = 16, STAGES = 4;
+
+// Kernel modes.  Update modes compute  Out = cb (A B + fold A)  on symmetric operands:
+//   MODE 0   Y  = alpha X X (+ residual partials)                          Eq.(11), Eq.(19)
+//   MODE 1   X' = -1/2 (X Y - 3 X)          = 1/2 X (3 I - X^2)            Eq.(11)
+//   MODE 2   W  = 3/8 (Y Y - 10/3 Y)        = 1/8 (3 X^4 - 10 X^2)         Eq.(19), first half
+//   MODE 3   X' = X W + 15/8 X              = 1/8 X (15 I - 10 X^2 + 3 X^4) Eq.(19), second half
+template <int MODE> struct ModeTraits;
+template <> struct ModeTraits<0> { static constexpr double fold = 0.0, cb = 1.0; static constexpr bool scale_k0 = true; };
+template <> struct ModeTraits<1> { static constexpr double fold = -3.0, cb = -0.5; static constexpr bool scale_k0 = true; };
+template <> struct ModeTraits<2> { static constexpr double fold = -10.0 / 3.0, cb = 0.375; static constexpr bool scale_k0 = false; };
+template <> struct ModeTraits<3> { static constexpr double fold = 1.875, cb = 1.0; static constexpr bool scale_k0 = true; };
 constexpr int NCONSUMER = 128, NTHREADS = NCONSUMER + 32;
 constexpr int STAGE_DOUBLES = (BM + BN) * BK;  // A slice then B slice, dense
 constexpr size_t NS_SMEM = (size_t)STAGES * STAGE_DOUBLES * sizeof(double);
@@ -212,31 +223,31 @@ __device__ __forceinline__ void panel_diag(double (&acc)[16][2], const double* _
 // (X' = b (X Y - 3 X)).  Runs on 8 of the K/8 panels of a tile; specialised per work shape so that
 // each k loop carries only its own few instructions.
 __device__ __forceinline__ void fold_rect(double (&acc)[16][2], const double* __restrict__ Ap, int s_rows, int wid,
-                                          int sc) {
+                                          int sc, const double f) {
     if ((sc >> 1) != wid) return;
     const bool odd = sc & 1;
 #pragma unroll
     for (int mt = 0; mt < 8; ++mt) {
         if (mt < s_rows) {
             const double2 x = *reinterpret_cast<const double2*>(Ap + mt * 64);
-            if (odd) { acc[2 * mt + 1][0] = fma(-3.0, x.x, acc[2 * mt + 1][0]); acc[2 * mt + 1][1] = fma(-3.0, x.y, acc[2 * mt + 1][1]); }
-            else { acc[2 * mt][0] = fma(-3.0, x.x, acc[2 * mt][0]); acc[2 * mt][1] = fma(-3.0, x.y, acc[2 * mt][1]); }
+            if (odd) { acc[2 * mt + 1][0] = fma(f, x.x, acc[2 * mt + 1][0]); acc[2 * mt + 1][1] = fma(f, x.y, acc[2 * mt + 1][1]); }
+            else { acc[2 * mt][0] = fma(f, x.x, acc[2 * mt][0]); acc[2 * mt][1] = fma(f, x.y, acc[2 * mt][1]); }
         }
     }
 }
 template <int W>
-__device__ __forceinline__ void fold_diag(double (&acc)[16][2], const double* __restrict__ Ap, int sc) {
+__device__ __forceinline__ void fold_diag(double (&acc)[16][2], const double* __restrict__ Ap, int sc, const double f) {
     // sub-tile row W holds columns 0..W in acc[0..W]; row 7-W holds columns 0..7-W in acc[W+1..8]
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         if (c == sc) {
             if (c <= W) {
                 const double2 x = *reinterpret_cast<const double2*>(Ap + W * 64);
-                acc[c][0] = fma(-3.0, x.x, acc[c][0]); acc[c][1] = fma(-3.0, x.y, acc[c][1]);
+                acc[c][0] = fma(f, x.x, acc[c][0]); acc[c][1] = fma(f, x.y, acc[c][1]);
             }
             if (c <= 7 - W) {
                 const double2 x = *reinterpret_cast<const double2*>(Ap + (7 - W) * 64);
-                acc[W + 1 + c][0] = fma(-3.0, x.x, acc[W + 1 + c][0]); acc[W + 1 + c][1] = fma(-3.0, x.y, acc[W + 1 + c][1]);
+                acc[W + 1 + c][0] = fma(f, x.x, acc[W + 1 + c][0]); acc[W + 1 + c][1] = fma(f, x.y, acc[W + 1 + c][1]);
             }
         }
     }
@@ -267,11 +278,11 @@ __device__ __forceinline__ void k_loop_var(double (&acc)[16][2], const double* s
                 if (VAR >= 1 && VAR <= 8) panel_rect<(VAR >= 1 && VAR <= 8) ? VAR : 1>(acc, Ap, Bp);
                 else if (VAR == 13) panel_rect_dyn(acc, Ap, Bp, s_rows);
                 else panel_diag<(VAR >= 9 && VAR <= 12) ? VAR - 9 : 0>(acc, Ap, Bp);
-                if (MODE == 1) {
+                if (MODE >= 1) {
                     const int sc = 2 * kt + j - kp_col0;
                     if ((unsigned)sc < 8u) {
-                        if (VAR <= 8 || VAR == 13) fold_rect(acc, Ap, VAR <= 8 ? VAR : s_rows, wid, sc);
-                        else fold_diag<(VAR >= 9 && VAR <= 12) ? VAR - 9 : 0>(acc, Ap, sc);
+                        if (VAR <= 8 || VAR == 13) fold_rect(acc, Ap, VAR <= 8 ? VAR : s_rows, wid, sc, ModeTraits<MODE>::fold);
+                        else fold_diag<(VAR >= 9 && VAR <= 12) ? VAR - 9 : 0>(acc, Ap, sc, ModeTraits<MODE>::fold);
                     }
                 }
             }
@@ -344,11 +355,11 @@ __device__ __forceinline__ void tile_var(double (&acc)[16][2], const double* sme
     if (VAR == 0) return;
     const int lr = lane >> 2, lk = lane & 3;
     EpiCtx c;  // built after the k loop: only the tile geometry stays live across it
-    c.scale = (MODE == 0) ? 1.0 : -0.5;
-    if (t.k == 0) {  // iteration 0 folds the spectral scale 1/s_i into the coefficients
+    c.scale = ModeTraits<MODE>::cb;
+    if (t.k == 0 && ModeTraits<MODE>::scale_k0) {  // iteration 0 folds the spectral scale 1/s_i into the coefficients
         double sg = __longlong_as_double((long long)t.gersh[t.grp]);
         if (!(sg > 0.0)) sg = 1.0;
-        c.scale = (MODE == 0) ? 1.0 / (sg * sg) : -0.5 / sg;
+        c.scale = (MODE == 0) ? 1.0 / (sg * sg) : ModeTraits<MODE>::cb / sg;
     }
     c.Out = t.out + t.ws_off;
     c.pd = min(BM, t.ld - t.row0) * 8;
@@ -389,6 +400,7 @@ struct NsArgs {
     double* buf0;
     double* buf1;
     double* bufY;
+    double* bufW;        // order 3 only (Eq.(19)): W = 1/8 (3 X^4 - 10 X^2)
     double* partials;
     int32_t* done_iter;
     int32_t* flag;
@@ -418,8 +430,9 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
     }
     __syncthreads();
 
-    const double* Xbase = (k & 1) ? a.buf1 : a.buf0;
-    const double* Bbase = (MODE == 0) ? Xbase : a.bufY;
+    const double* Xk = (k & 1) ? a.buf1 : a.buf0;
+    const double* Xbase = (MODE == 2) ? a.bufY : Xk;                                  // A operand
+    const double* Bbase = (MODE == 0) ? Xk : (MODE == 3 ? a.bufW : a.bufY);           // B operand
 
     if (wid == 4) {
         // ============================================================ producer (one thread)
@@ -454,7 +467,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
                 const int ti = tij & 0xffff, tj = tij >> 16;
                 const int row0 = ti * BM, col0 = tj * BN;
                 const int rows_a = min(BM, ld - row0), rows_b = min(BN, ld - col0);
-                const bool b_is_a = (MODE == 0) && (ti == tj);
+                const bool b_is_a = (MODE == 0 || MODE == 2) && (ti == tj);
                 const int KP = ld >> 3;            // 8-wide k panels
                 const int KT = (KP + 1) >> 1;      // stages of two panels
                 const double* Asrc = Xbase + ws_off + (size_t)row0 * ld;
@@ -504,7 +517,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
         const int s_rows = min(8, (si.ld - row0) >> 3);  // valid 8-row sub-tile rows of this tile, 1..8
         const bool full_diag = diag && s_rows == 8;
         const int rows_a = min(BM, si.ld - row0), rows_b = min(BN, si.ld - col0);
-        const bool b_is_a = (MODE == 0) && diag;
+        const bool b_is_a = (MODE == 0 || MODE == 2) && diag;
         // work shape of this warp for this tile (see tile_var)
         int variant;
         if (full_diag) variant = 9 + wid;
@@ -514,7 +527,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
         for (int e = 0; e < 16; ++e) acc[e][0] = acc[e][1] = 0.0;
         const int ld = si.ld;
         TileGeo c;
-        c.ws_off = si.ws_off; c.out = (MODE == 0) ? a.bufY : ((k & 1) ? a.buf0 : a.buf1); c.gersh = a.gersh;
+        c.ws_off = si.ws_off; c.out = (MODE == 0) ? a.bufY : (MODE == 2 ? a.bufW : ((k & 1) ? a.buf0 : a.buf1)); c.gersh = a.gersh;
         c.ld = ld; c.n = si.n; c.row0 = row0; c.col0 = col0; c.grp = si.grp; c.k = k;
         double part = 0.0;
         {
@@ -570,31 +583,41 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
 
 // which: bit 0 = MODE 0 + decision of iteration k, bit 1 = MODE 1 (update) of iteration k.
 sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
-                           double* bufY, cudaStream_t st, int which) {
+                           double* bufY, cudaStream_t st, int which, double* bufW) {
     if (p->n_tiles == 0) return SM_OK;
     static bool attr_set = false;
     if (!attr_set) {
         SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
         attr_set = true;
     }
     NsArgs a;
     a.tiles = p->d_tiles; a.gersh = p->d_gersh;
-    a.buf0 = buf0; a.buf1 = buf1; a.bufY = bufY; a.partials = p->d_partials;
+    a.buf0 = buf0; a.buf1 = buf1; a.bufY = bufY; a.bufW = bufW; a.partials = p->d_partials;
     a.done_iter = p->d_done_iter; a.flag = p->d_flag; a.tile_done = p->d_tile_done; a.res = p->d_res;
     a.counters = p->d_counters; a.n_tiles = (int32_t)p->n_tiles;
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * 3);
-    a.sched = p->d_sched + 2 * k;
+    a.sched = p->d_sched + 4 * k;
     if (which & 1) {
         k_ns_gemm<0><<<grid, NTHREADS, NS_SMEM, st>>>(a);
         k_ns_decide<<<(p->ngroups + 7) / 8, 256, 0, st>>>(a, p->d_tile_first, p->d_tile_count, p->d_sub_dim);
         p->launches += 2;
     }
     if ((which & 2) && !decide_only) {
-        a.sched = p->d_sched + 2 * k + 1;
-        k_ns_gemm<1><<<grid, NTHREADS, NS_SMEM, st>>>(a);
-        p->launches += 1;
+        if (p->opt.order == 3 && bufW) {  // Eq.(19): two products per update
+            a.sched = p->d_sched + 4 * k + 1;
+            k_ns_gemm<2><<<grid, NTHREADS, NS_SMEM, st>>>(a);
+            a.sched = p->d_sched + 4 * k + 2;
+            k_ns_gemm<3><<<grid, NTHREADS, NS_SMEM, st>>>(a);
+            p->launches += 2;
+        } else {
+            a.sched = p->d_sched + 4 * k + 1;
+            k_ns_gemm<1><<<grid, NTHREADS, NS_SMEM, st>>>(a);
+            p->launches += 1;
+        }
     }
     SM_CUDA(cudaGetLastError());
     return SM_OK;

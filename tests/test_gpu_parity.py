@@ -424,6 +424,42 @@ def test_density_matrix_unreachable_tolerance_is_guarded(B, cfg0):
     B.sm_plan_destroy(plan)
 
 
+# ------------------------------------------------------------------------------ Eq.(19)
+def test_third_order_iteration_eq19(B, oracle, cfg0):
+    """order = 3: the paper's GPU iteration X <- 1/8 X (15 I - 10 X^2 + 3 X^4) (Eq.(19)) reaches
+    the same sign function (oracle parity) in fewer iterations than Eq.(11); scalar pin: its
+    iteration count equals the one of the scalar map on the oracle's eigenvalues."""
+    m = cfg0
+    idx = oracle.Index(m)
+    d_or = oracle.density(idx, m.values, 0.0)
+    plan2, st2, d2, stats2, _, _ = _run_sign(B, m, opt=B.default_options(order=2, overshoot=1.0))
+    plan3, st3, d3, stats3, ws, vin = _run_sign(B, m, opt=B.default_options(order=3))
+    assert st2 == B.SM_OK and st3 == B.SM_OK
+    assert np.abs(d3 - d_or).max() <= TOL_D
+    assert stats3.iter_max < stats2.iter_max
+    # scalar recursion on the eigenvalues of the largest-iteration submatrix bound
+    lam, w, ptr, g = oracle.eig_groups(idx, m.values)
+    s = max(abs(stats3.spec_lo), abs(stats3.spec_hi))
+    worst = 0
+    for i in range(idx.ngroups):
+        x = lam[ptr[i]:ptr[i + 1]] / s
+        n = len(x)
+        for k in range(60):
+            if np.sqrt(((x * x - 1.0) ** 2).sum() / n) < EPS:
+                break
+            x = x * (15.0 - 10.0 * x ** 2 + 3.0 * x ** 4) / 8.0
+        worst = max(worst, k)
+    assert abs(stats3.iter_max - worst) <= 1  # Gershgorin can be the tighter bound for a submatrix
+    # bisection with the steering bound works unchanged on this path
+    torch = _torch()
+    vout = torch.empty_like(vin)
+    stats = B.sm_stats_t()
+    st, mu = B.sm_density_matrix(plan3, vin, float(m.n_occ), 0.5, EPS, -1.0, vout, ws, stats)
+    assert st == B.SM_OK
+    assert np.abs(vout.cpu().numpy() - oracle.density(idx, m.values, mu)).max() <= TOL_D
+    B.sm_plan_destroy(plan2); B.sm_plan_destroy(plan3)
+
+
 # ------------------------------------------------------------------------------ reduced precision
 @pytest.mark.parametrize("precision,tol_d,tol_e", [(2, 1e-4, 1e-5), (1, 5e-3, 2e-3)])
 def test_reduced_precision_variants(B, oracle, cfg0, precision, tol_d, tol_e):
