@@ -128,17 +128,24 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
                           2u * (lane & 3);
             const unsigned xstep = rows_t * 64u;
             double asum = 0.0;
-#pragma unroll 4
-            for (int p = 2 * lane; p < ld; p += 64, xo += xstep) {
-                const uint4 pm = *reinterpret_cast<const uint4*>(posmap + p);
-                const MapT r0 = row[pm.x], r1 = row[pm.z];
-                double2 v = make_double2(0.0, 0.0);
-                if (r0 != NONE) v.x = __ldg(vcol + (int)r0 + (int)(pm.y & 0xffffu) + qq * (int)(pm.y >> 16));
-                if (r1 != NONE) v.y = __ldg(vcol + (int)r1 + (int)(pm.w & 0xffffu) + qq * (int)(pm.w >> 16));
-                if (p == q) v.x -= A.mu;
-                if (p + 1 == q) v.y -= A.mu;
-                asum += fabs(v.x) + fabs(v.y);
-                *reinterpret_cast<double2*>(Xg + xo) = v;
+            // warp-uniform trip count (groups of four 64-wide steps, predicated inside): one loop body,
+            // no divergent remainder loop; all look-ups and loads of a group are in flight together
+            for (int base = 0, p0 = 2 * lane; base < ld; base += 256, p0 += 256, xo += 4 * xstep) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int p = p0 + 64 * u;
+                    if (p < ld) {
+                        const uint4 pm = *reinterpret_cast<const uint4*>(posmap + p);
+                        const MapT r0 = row[pm.x], r1 = row[pm.z];
+                        double2 v = make_double2(0.0, 0.0);
+                        if (r0 != NONE) v.x = __ldg(vcol + (int)r0 + (int)(pm.y & 0xffffu) + qq * (int)(pm.y >> 16));
+                        if (r1 != NONE) v.y = __ldg(vcol + (int)r1 + (int)(pm.w & 0xffffu) + qq * (int)(pm.w >> 16));
+                        if (p == q) v.x -= A.mu;
+                        if (p + 1 == q) v.y -= A.mu;
+                        asum += fabs(v.x) + fabs(v.y);
+                        *reinterpret_cast<double2*>(Xg + xo + u * xstep) = v;
+                    }
+                }
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) asum += __shfl_xor_sync(0xffffffffu, asum, o);
