@@ -105,6 +105,8 @@ struct sm_plan {
     int32_t *d_tile_first32 = nullptr, *d_tile_count32 = nullptr;
     double* d_partials32 = nullptr;
     int64_t n_tiles32 = 0, sum_ldp2 = 0;
+    uint32_t* d_src_map = nullptr;         // [nnz] scatter source map (built by the first scatter)
+    int scatter_chunks = 1;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
     double lz_lo = 0.0, lz_hi = 0.0;       // estimated [lambda_min, lambda_max] of K~ (widened)
     int lz_valid = 0;                      // lz_lo / lz_hi belong to the current call's values

@@ -183,24 +183,22 @@ sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, 
 }
 
 // ---------------------------------------------------------------------------------------------
-// Scatter (PAPER.md L127 step 3 + Eq.(16) inner factor): one warp per block column c.  The values
-// of a block column are one contiguous range of the result; the warp takes 32 of its blocks at a
-// time (one packed record each: row offset inside the submatrix | block height), prefix-sums
-// their sizes and then sweeps the contiguous output range with one element per lane (coalesced
-// stores), finding the block of an element by a shuffle binary search over the prefix sums.
-// Element (el,q) of block (r,c) reads X_i[gen_off(c) + q, blk_loc(r) + el] of c's group i
-// (X symmetric, so the read walks a contiguous row segment).  D = 1/2 (delta - xs * X), xs = 1/s_i
-// if the submatrix converged at iteration 0 (the buffer then still holds the unscaled
-// a_i - mu I), else 1.
+// Scatter (PAPER.md L127 step 3 + Eq.(16) inner factor).  Element (el,q) of result block (r,c) is
+// X_i[gen_off(c) + q, blk_loc(r) + el] of c's group i (X symmetric, so the read walks a row).
+// Where each stored value comes from depends on the pattern only, so the first scatter of a plan
+// builds a SOURCE MAP: one 32-bit entry per stored value = its offset inside the submatrix's
+// workspace matrix (k8-panel layout) | "diagonal element" in bit 31.  k_scatter_map_build walks
+// the block columns once (one warp per block column: 32 packed block records at a time, prefix
+// sums of their sizes, shuffle binary search of an element's block); k_scatter is then a plain
+// parallel sweep over the values of a block column, any block size, any number of groups:
+//     D = 1/2 (delta - xs * X),  xs = 1/s_i if the submatrix stopped at iteration 0 (the buffer
+// then still holds the unscaled a_i - mu I), else 1.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_scatter(int nb, const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
-          const int64_t* __restrict__ val_off, const int32_t* __restrict__ col_grp,
-          const int32_t* __restrict__ gen_off, const uint32_t* __restrict__ blk_pack,
-          const int32_t* __restrict__ ldv, const int64_t* __restrict__ ws_off,
-          const int32_t* __restrict__ done_iter, const unsigned long long* __restrict__ gersh, int cur_k,
-          const double* __restrict__ buf0, const double* __restrict__ buf1, double* __restrict__ out,
-          int as_identity) {
+k_scatter_map_build(int nb, const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
+                    const int64_t* __restrict__ val_off, const int32_t* __restrict__ col_grp,
+                    const int32_t* __restrict__ gen_off, const uint32_t* __restrict__ blk_pack,
+                    const int32_t* __restrict__ ldv, uint32_t* __restrict__ src_map) {
     const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (c >= nb) return;
     const int lane = threadIdx.x & 31;
@@ -208,17 +206,9 @@ k_scatter(int nb, const int32_t* __restrict__ blk_size, const int64_t* __restric
     const int bc = blk_size[c];
     const int64_t p0 = colptr[c];
     const int nblk = (int)(colptr[c + 1] - p0);
-    const int di = done_iter[g];
-    const int kb = di >= 0 ? di : cur_k;
-    const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];
     const int ld = ldv[g];
-    double xs = 1.0;
-    if (kb == 0 && !as_identity) {
-        double s = __longlong_as_double((long long)gersh[g]);
-        xs = s > 0.0 ? 1.0 / s : 1.0;
-    }
     const int go = gen_off[c];
-    double* o = out + val_off[p0];
+    uint32_t* o = src_map + val_off[p0];
     for (int base = 0; base < nblk; base += 32) {
         const int b = base + lane;
         const uint32_t pk = b < nblk ? __ldg(blk_pack + p0 + b) : 0u;
@@ -245,21 +235,63 @@ k_scatter(int nb, const int32_t* __restrict__ blk_size, const int64_t* __restric
                 const int br = (int)(pkk >> 20), loc = (int)(pkk & 0xfffffu);
                 const int w = e - ex;
                 const int q = w / br, el = w - q * br;
-                const double x = Xg[panel_off(go + q, loc + el, ld)];
-                o[e] = as_identity ? x : 0.5 * (((loc + el == go + q) ? 1.0 : 0.0) - xs * x);
+                o[e] = (uint32_t)panel_off(go + q, loc + el, ld) | ((loc + el == go + q) ? 0x80000000u : 0u);
             }
         }
         o += total;
     }
 }
 
+constexpr int SCATTER_THREADS = 128, SCATTER_CHUNK = 1024;  // values per CTA (8 per thread)
+
+__global__ void __launch_bounds__(SCATTER_THREADS)
+k_scatter(const int64_t* __restrict__ colptr, const int64_t* __restrict__ val_off,
+          const int32_t* __restrict__ col_grp, const int64_t* __restrict__ ws_off,
+          const int32_t* __restrict__ done_iter, const unsigned long long* __restrict__ gersh, int cur_k,
+          const uint32_t* __restrict__ src_map, const double* __restrict__ buf0, const double* __restrict__ buf1,
+          double* __restrict__ out, int as_identity) {
+    const int c = blockIdx.x;
+    const int64_t v0 = val_off[colptr[c]], v1 = val_off[colptr[c + 1]];
+    const int64_t b = v0 + (int64_t)blockIdx.y * SCATTER_CHUNK;
+    if (b >= v1) return;
+    const int64_t e1 = min(v1, b + SCATTER_CHUNK);
+    const int g = col_grp[c];
+    const int di = done_iter[g];
+    const int kb = di >= 0 ? di : cur_k;
+    const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];
+    double xs = 1.0;
+    if (kb == 0 && !as_identity) {
+        const double s = __longlong_as_double((long long)gersh[g]);
+        xs = s > 0.0 ? 1.0 / s : 1.0;
+    }
+#pragma unroll 4
+    for (int64_t e = b + threadIdx.x; e < e1; e += SCATTER_THREADS) {
+        const uint32_t m = __ldg(src_map + e);
+        const double x = Xg[m & 0x7fffffffu];
+        out[e] = as_identity ? x : 0.5 * ((double)(m >> 31) - xs * x);
+    }
+}
+
 sm_status_t launch_scatter(sm_plan* p, int as_identity, const double* buf0, const double* buf1,
                            double* out, cudaStream_t st) {
-    if (p->nb == 0) return SM_OK;
-    k_scatter<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_blk_size, p->d_colptr, p->d_val_off, p->d_col_grp,
-                                               p->d_gen_off, p->d_blk_pack, p->d_ld, p->d_ws_off,
-                                               p->d_done_iter, p->d_gersh, p->cur_k, buf0, buf1, out,
-                                               as_identity);
+    if (p->nb == 0 || p->nnz == 0) return SM_OK;
+    if (!p->d_src_map) {  // once per plan (pattern only)
+        SM_CUDA(cudaMalloc((void**)&p->d_src_map, (size_t)p->nnz * 4));
+        k_scatter_map_build<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_blk_size, p->d_colptr, p->d_val_off,
+                                                             p->d_col_grp, p->d_gen_off, p->d_blk_pack, p->d_ld,
+                                                             p->d_src_map);
+        p->launches++;
+        int64_t mx = 0;
+        for (int c = 0; c < p->nb; ++c) {
+            int64_t rows = 0;
+            for (int64_t q = p->h_colptr[c]; q < p->h_colptr[c + 1]; ++q) rows += p->h_blk_size[p->h_rowidx[q]];
+            mx = std::max(mx, rows * p->h_blk_size[c]);
+        }
+        p->scatter_chunks = (int)std::max<int64_t>(1, (mx + SCATTER_CHUNK - 1) / SCATTER_CHUNK);
+    }
+    k_scatter<<<dim3(p->nb, p->scatter_chunks), SCATTER_THREADS, 0, st>>>(
+        p->d_colptr, p->d_val_off, p->d_col_grp, p->d_ws_off, p->d_done_iter, p->d_gersh, p->cur_k, p->d_src_map, buf0,
+        buf1, out, as_identity);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;

@@ -253,6 +253,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     }
     p->sum_ld2 = off;
     if (dmax >= (1 << 20) - LD_ALIGN) return SM_ERR_INVALID_ARG;  // packed block records hold 20-bit offsets
+    if ((int64_t)(dmax + LD_ALIGN) * (dmax + LD_ALIGN) >= (1LL << 31)) return SM_ERR_INVALID_ARG;  // 31-bit scatter map / tile offsets
     std::vector<int32_t> order(ng);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return p->h_ld[a] > p->h_ld[b]; });
