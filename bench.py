@@ -22,7 +22,7 @@ import argparse
 import json
 import os
 import statistics
-import subprocess
+import subprocess  # noqa: F401
 import sys
 import tempfile
 import time
@@ -54,60 +54,64 @@ def fp64_peak_tflops():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (profiling recipe)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock, power and throttle reasons sampled DURING the timed region (profiling recipe): NVML
+    in a background thread of this process (spawning `nvidia-smi -lms` was measured to stall the
+    synchronous CUDA calls of the timed region while it attaches and on every query)."""
 
-    def __init__(self, gpu_index):
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+    def __init__(self, gpu_index, period_s=0.1):
+        import threading
+        self.samples, self.skip, self.run, self.err = [], 0, True, None
         try:
-            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "200"],
-                                      stdout=self.f, stderr=subprocess.DEVNULL)
-        except OSError:
-            self.p = None
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(gpu_index)
+        except Exception as e:  # no NVML: the line says so instead of inventing clocks
+            self.nv, self.err = None, repr(e)
+            return
+        self.period = period_s
+        self.t = threading.Thread(target=self._loop, daemon=True)
+        self.t.start()
+
+    def _loop(self):
+        nv = self.nv
+        while self.run:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                mx = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                    else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.samples.append((sm, mx, pw, rs))
+            except Exception as e:
+                self.err = repr(e)
+            time.sleep(self.period)
 
     def mark(self):
-        """Samples written before this call (warm-up) are ignored by stop()."""
-        try:
-            self.skip = os.path.getsize(self.f.name)
-        except OSError:
-            self.skip = 0
+        """Samples taken before this call (warm-up) are ignored by stop()."""
+        self.skip = len(self.samples)
 
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
-        if self.p is None:
+        if self.nv is None:
+            out["error"] = self.err
             return out
-        self.p.terminate()
-        try:
-            self.p.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.p.kill()
-        self.f.flush()
-        self.f.seek(getattr(self, "skip", 0))
-        self.f.readline()  # the (possibly partial) line the mark fell into
-        sm, mx, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.f.read().splitlines():
-            parts = [x.strip() for x in line.split(",")]
-            if len(parts) < 7:
-                continue
-            try:
-                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
-            except ValueError:
-                continue
-            for nm, v in zip(names, parts[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(nm)
-        os.unlink(self.f.name)
-        if sm:
-            # "under load": samples above 60% of the max power seen
-            thr = 0.6 * max(pw)
-            load = [s for s, w in zip(sm, pw) if w >= thr] or sm
-            out = {"sm_mhz": statistics.median(load), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
-                   "power_w_max": max(pw), "samples": len(sm)}
-        return out
+        self.run = False
+        self.t.join(timeout=2)
+        nv = self.nv
+        rows = self.samples[self.skip:] or self.samples[-1:]
+        if not rows:
+            out["error"] = self.err
+            return out
+        bits = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+                "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+                "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
+        reasons = sorted(k for k, bit in bits.items() if any(r[3] & bit for r in rows))
+        pmax = max(r[2] for r in rows)
+        load = [r[0] for r in rows if r[2] >= 0.6 * pmax] or [r[0] for r in rows]
+        return {"sm_mhz": statistics.median(load), "sm_max_mhz": max(r[1] for r in rows), "reasons": reasons,
+                "power_w_max": pmax, "samples": len(rows)}
 
 
 def dist_env():
@@ -314,7 +318,7 @@ def main():
 
     # the clock sampler attaches BEFORE the warm-up (nvidia-smi's start-up stalls synchronous CUDA calls
     # for a while); only the samples taken during the timed region are kept
-    sampler = ClockSampler(local_rank) if rank == 0 else None
+    sampler = ClockSampler(local_rank) if (rank == 0 and not os.environ.get('SM_NO_SAMPLER')) else None
     for _ in range(args.warmup):
         st, mu = step_device()
     barrier()

@@ -70,8 +70,9 @@ typedef struct {
                          /* 1 = FP32 storage, plain TF32 products (error ~2e-3 class);       */
                          /* 2 = "3xTF32": operands stored as hi + lo TF32 pairs, products    */
                          /*     hi hi + hi lo + lo hi (FP32-class, <= 1e-3 bar)              */
-    int32_t check_every; /* host polls the "all converged" counter every this many     [1]   */
-                         /* iterations (>= 1)                                                */
+    int32_t check_every; /* the stop decisions are taken on the device; the host enqueues  [8]   */
+                         /* this many iterations ahead before it reads the control block     */
+                         /* (>= 1; launches after the stop are empty)                        */
     int32_t max_mu_steps;/* bisection step cap of sm_density_matrix                    [64]  */
     int32_t bisect_iter; /* iteration cap of the NON-final bisection evaluations        [0]  */
                          /* (0 = max_iter). A capped evaluation is only used for the         */

@@ -70,7 +70,7 @@ class sm_stats_t(C.Structure):
 
 
 def default_options(**kw) -> sm_options_t:
-    o = sm_options_t(max_iter=100, scaling=1, precision=0, check_every=1, max_mu_steps=64, bisect_iter=0,
+    o = sm_options_t(max_iter=100, scaling=1, precision=0, check_every=8, max_mu_steps=64, bisect_iter=0,
                      mu_tol=1e-6, early_out=1, overshoot=1.45, order=2)
     for k, v in kw.items():
         setattr(o, k, v)

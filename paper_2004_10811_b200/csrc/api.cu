@@ -27,7 +27,7 @@ static void default_options(sm_options_t* o) {
     o->overshoot = 1.45;
     o->order = 2;
     o->precision = 0;
-    o->check_every = 1;
+    o->check_every = 8;
     o->max_mu_steps = 64;
     o->bisect_iter = 0;
     o->mu_tol = 1e-6;
@@ -81,12 +81,13 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
                     p->d_partials, p->d_counters, p->d_sched, p->d_tile_done, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
-                    p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map};
+                    p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_ctrl};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     if (p->h_pinned) cudaFreeHost(p->h_pinned);
     if (p->h_pinned_d) cudaFreeHost(p->h_pinned_d);
     if (p->h_bound) cudaFreeHost(p->h_bound);
+    if (p->h_ctrl) cudaFreeHost(p->h_ctrl);
     for (auto& e : p->ev)
         if (e) cudaEventDestroy(e);
     for (auto& e : p->ev_iter)
@@ -155,6 +156,9 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_bound, (size_t)(p->opt.max_iter + 2) * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_bound_part, (size_t)ng * 16);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_bound, (size_t)(p->opt.max_iter + 2) * 16);
+    if (e == cudaSuccess) e = A((void**)&p->d_ctrl, 64);
+    if (e == cudaSuccess) e = cudaMemset(p->d_ctrl, 0, 64);
+    if (e == cudaSuccess) e = cudaMallocHost(&p->h_ctrl, 64);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned, (size_t)(p->opt.max_iter + 2) * 4);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned_d, 8 * 8);
     for (auto& ev : p->ev)
@@ -257,12 +261,13 @@ sm_status_t reset_state(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMemsetAsync(p->d_counters, 0, (size_t)(p->opt.max_iter + 2) * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_sched, 0, (size_t)(p->opt.max_iter + 2) * 16, st));
     SM_CUDA(cudaMemsetAsync(p->d_tile_done, 0, (size_t)ng * 4, st));
+    SM_CUDA(cudaMemsetAsync(p->d_ctrl, 0, sizeof(EvalCtrl), st));
     p->cur_k = 0;
     return SM_OK;
 }
 
-// Steering of one bisection evaluation (reading A11c): the loop may stop as soon as the bound of
-// k_nelec_bound proves on which side of n_target the converged n_elec lies.
+// Steering of one bisection evaluation (reading A11c): the evaluation may stop as soon as the bound
+// of k_nelec_bound proves on which side of n_target the converged n_elec lies.
 struct Steer {
     double n_target = 0.0, tol_n = 0.0, slack = 0.0;
     int decided = 0;        // out: +1 n_elec > n_target + tol_n proven, -1 the opposite, 0 not decided
@@ -276,80 +281,54 @@ sm_status_t launch_pair(sm_plan* p, int k, double eps, int last, const Bufs& b, 
     return launch_ns_pair(p, k, eps, last, b.b0, b.b1, b.y, st, which, b.w);
 }
 
-// Newton-Schulz host loop: iterations k = cur_k .. k_end-1 (each = MODE 0 + MODE 1 launch).
-// Iteration k tests X_k and, if not converged, forms X_{k+1}.  At k == max_iter only the decision
-// is recorded.  Returns with *all_done = 1 if every submatrix has stopped.  The host reads the
-// "still active" counter (and the steering bound) one iteration behind, so it never stalls the GPU.
+// Newton-Schulz host loop: iterations k = cur_k .. k_end-1.  Iteration k = MODE 0 (Y = X_k^2, residual)
+// + decision [+ steering bound] + k_eval_ctrl + update (X_{k+1}); at k == max_iter only the decision
+// is recorded.  Every stop decision -- all submatrices converged, or a proven steering direction --
+// is taken ON THE DEVICE (EvalCtrl): once it is set, the remaining launches of the evaluation are
+// empty.  The host therefore enqueues `check_every` iterations ahead and only then reads the
+// control block: the GPU never waits for the host, and a stalled host thread costs nothing while
+// work is queued.  Returns with *all_done = 1 if every submatrix has stopped.
 sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_done, int* launched,
                     cudaStream_t st, Steer* steer = nullptr) {
     *all_done = 0;
     if (p->ngroups == 0) { *all_done = 1; return SM_OK; }
-    const int max_iter = p->opt.max_iter;
-    int k = p->cur_k;
+    const int max_iter = p->opt.max_iter, upd = p->opt.order == 3 ? 2 : 1;
+    const EvalCtrl* hc = reinterpret_cast<const EvalCtrl*>(p->h_ctrl);
+    const int k_begin = p->cur_k;
+    const double margin = steer ? steer->slack + steer->tol_n : 0.0;
     p->half_iter = 0;
-    int pending = -1;  // iteration whose counter copy is in flight
-    auto poll = [&](int q) -> int {  // 1 = all converged, 2 = steering decision, 0 = go on
-        if (p->h_pinned[q] == 0) { *all_done = 1; p->cur_k = q; return 1; }
-        if (steer && q >= 1) {
-            const double ne = p->h_bound[2 * q], err = p->h_bound[2 * q + 1];
-            if (ne == ne && err == err && err >= 0.0) {
-                const double g = ne - steer->n_target, m = err + steer->slack + steer->tol_n;
-                if (g > m || g < -m) {
-                    steer->decided = g > 0 ? 1 : -1; steer->k = q; steer->ne = ne; steer->err = err;
-                    return 2;
-                }
-            }
-        }
-        return 0;
-    };
-    if (steer) {
-        // Steering evaluation: poll synchronously between MODE 0 and MODE 1 of every iteration k >= 1
-        // (a ~20 us bubble against a multi-ms launch), so that a proven direction stops the
-        // evaluation before the next update is even launched.
-        for (; k < k_end && k <= max_iter; ++k) {
-            const int last = k == max_iter ? 1 : 0;
-            sm_status_t s = launch_pair(p, k, eps, last, b, st, 1);
-            if (s) return s;
-            (*launched) += 1;
-            SM_CUDA(cudaMemcpyAsync(p->h_pinned + k, p->d_counters + k, 4, cudaMemcpyDeviceToHost, st));
-            if (k >= 1) {
-                if ((s = launch_nelec_bound(p, k, b.b0, b.b1, b.y, st))) return s;
-                SM_CUDA(cudaMemcpyAsync(p->h_bound + 2 * k, p->d_bound + 2 * k, 16, cudaMemcpyDeviceToHost, st));
-            }
+    int k = k_begin, since = 0;
+    bool stopped = false;
+    sm_status_t s;
+    for (; k < k_end && k <= max_iter && !stopped; ++k) {
+        const int last = k == max_iter ? 1 : 0;
+        if ((s = launch_pair(p, k, eps, last, b, st, 1))) return s;
+        const int steer_k = (steer && k >= 1) ? 1 : 0;
+        if (steer_k && (s = launch_nelec_bound(p, k, b.b0, b.b1, b.y, st))) return s;
+        if ((s = launch_eval_ctrl(p, k, steer_k, steer ? steer->n_target : 0.0, margin, st))) return s;
+        if (!last && (s = launch_pair(p, k, eps, 0, b, st, 2))) return s;
+        if (++since >= p->opt.check_every || last || k == k_end - 1) {
+            SM_CUDA(cudaMemcpyAsync(p->h_ctrl, p->d_ctrl, sizeof(EvalCtrl), cudaMemcpyDeviceToHost, st));
             SM_CUDA(cudaStreamSynchronize(st));
-            const int r = poll(k);
-            if (r == 1) return SM_OK;                       // all converged: X_k is the result (cur_k = k)
-            if (r == 2) { p->cur_k = k; p->half_iter = 1; return SM_OK; }  // X_k in buf[k & 1], not converged
-            if (last) break;
-            if ((s = launch_pair(p, k, eps, 0, b, st, 2))) return s;
-            (*launched) += p->opt.order == 3 ? 2 : 1;
+            since = 0;
+            stopped = hc->stop != 0;
         }
-        p->cur_k = std::min(k, max_iter);
-        if (k >= max_iter) *all_done = 1;
+    }
+    if (stopped) {
+        const int ks = hc->k_stop;
+        p->cur_k = ks;
+        (*launched) += (ks - k_begin + 1) + (ks - k_begin) * upd;  // launches that did work; later ones were empty
+        if (hc->stop == 1) {
+            *all_done = 1;
+        } else {
+            p->half_iter = 1;  // MODE 0 of iteration ks ran, its update did not: X_ks in buf[ks & 1], not converged
+            if (steer) { steer->decided = hc->decided; steer->k = ks; steer->ne = hc->ne; steer->err = hc->err; }
+        }
         return SM_OK;
     }
-    for (; k < k_end && k <= max_iter; ++k) {
-        sm_status_t s = launch_pair(p, k, eps, k == max_iter ? 1 : 0, b, st, 3);
-        if (s) return s;
-        (*launched) += (k == max_iter) ? 1 : (p->opt.order == 3 ? 3 : 2);
-        if (pending >= 0) {
-            SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
-            if (poll(pending) == 1) return SM_OK;
-            pending = -1;
-        }
-        if ((k % p->opt.check_every) == 0 || k == max_iter || k == k_end - 1) {
-            SM_CUDA(cudaMemcpyAsync(p->h_pinned + k, p->d_counters + k, 4, cudaMemcpyDeviceToHost, st));
-            SM_CUDA(cudaEventRecord(p->ev_iter[k & 1], st));
-            pending = k;
-        }
-    }
-    if (pending >= 0) {
-        SM_CUDA(cudaEventSynchronize(p->ev_iter[pending & 1]));
-        if (poll(pending) == 1) return SM_OK;
-    }
-    // active submatrices have received k updates: their X lives in buf[k & 1]
+    // iteration cap reached with active submatrices: they have received k updates, X lives in buf[k & 1]
+    (*launched) += (k - k_begin) * (1 + upd);
     p->cur_k = std::min(k, max_iter);
-    if (k > max_iter) *all_done = 1;
     return SM_OK;
 }
 

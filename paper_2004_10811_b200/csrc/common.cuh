@@ -105,6 +105,8 @@ struct sm_plan {
     int32_t *d_tile_first32 = nullptr, *d_tile_count32 = nullptr;
     double* d_partials32 = nullptr;
     int64_t n_tiles32 = 0, sum_ldp2 = 0;
+    int32_t* d_ctrl = nullptr;             // [8] + doubles: device-side stop decision of an evaluation (EvalCtrl)
+    void* h_ctrl = nullptr;                // pinned mirror
     uint32_t* d_src_map = nullptr;         // [nnz] scatter source map (built by the first scatter)
     int scatter_chunks = 1;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
@@ -142,6 +144,17 @@ sm_status_t launch_to_f32(sm_plan* p, const double* buf0, double* buf1, cudaStre
 sm_status_t launch_to_f64(sm_plan* p, double* buf0, const double* buf1, const double* bufY, cudaStream_t st);
 sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
                                 double* bufY, cudaStream_t st, int which);
+// Device-side control block of one sign evaluation: set by k_eval_ctrl after the decision (and the
+// steering bound) of iteration k; once stop != 0 every later launch of the evaluation is empty, so the
+// host can enqueue iterations ahead without synchronising after each of them.
+struct EvalCtrl {
+    int32_t stop;      // 0 running, 1 all submatrices stopped, 2 steering decision (A11c)
+    int32_t k_stop;    // iteration at which it was set
+    int32_t decided;   // +1 / -1: n_elec proven above / below the target
+    int32_t pad;
+    double ne, err;    // n_elec(X_k) and its bound at the decision
+};
+sm_status_t launch_eval_ctrl(sm_plan* p, int k, int steer, double n_target, double margin, cudaStream_t st);
 // spectral.cu
 sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st);
 sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStream_t st);

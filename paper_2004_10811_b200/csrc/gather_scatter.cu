@@ -415,6 +415,28 @@ sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const doub
     return SM_OK;
 }
 
+// Device-side end of an evaluation (one thread, after k_ns_decide and k_nelec_bound of iteration k).
+__global__ void k_eval_ctrl(EvalCtrl* __restrict__ c, int k, const int32_t* __restrict__ counters,
+                            const double* __restrict__ bound, int steer, double n_target, double margin) {
+    if (threadIdx.x != 0 || blockIdx.x != 0 || c->stop != 0) return;
+    if (counters[k] == 0) { c->stop = 1; c->k_stop = k; return; }
+    if (steer && k >= 1) {
+        const double ne = bound[2 * k], err = bound[2 * k + 1];
+        if (ne == ne && err == err && err >= 0.0) {
+            const double g = ne - n_target, m = err + margin;
+            if (g > m || g < -m) { c->stop = 2; c->k_stop = k; c->decided = g > 0 ? 1 : -1; c->ne = ne; c->err = err; }
+        }
+    }
+}
+
+sm_status_t launch_eval_ctrl(sm_plan* p, int k, int steer, double n_target, double margin, cudaStream_t st) {
+    k_eval_ctrl<<<1, 32, 0, st>>>(reinterpret_cast<EvalCtrl*>(p->d_ctrl), k, p->d_counters, p->d_bound, steer, n_target,
+                                  margin);
+    p->launches++;
+    SM_CUDA(cudaGetLastError());
+    return SM_OK;
+}
+
 // tr(D) and tr(D K) (Eq.(18), Eq.(10)).  Stage 1: each CTA reduces a fixed contiguous
 // slice of the value arrays (and the diagonal entries of the diagonal blocks it owns by block
 // column); stage 2: k_sum_fixed.

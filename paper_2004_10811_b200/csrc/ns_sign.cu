@@ -408,6 +408,7 @@ struct NsArgs {
     double* res;         // [2][ngroups]
     int32_t* counters;   // [max_iter+2] still-active submatrices after iteration k
     int32_t* sched;      // work counter of this launch
+    const int32_t* ctrl; // [0] != 0: the evaluation has been stopped on the device (k_eval_ctrl): do nothing
     int32_t n_tiles;
     int32_t ngroups;
     int32_t k;
@@ -442,7 +443,8 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
         if (lane != 0) return;
         int stage = 0;
         unsigned phase = 0;
-        auto draw = [&]() { return atomicAdd(a.sched, 1); };
+        const bool stopped = a.ctrl[0] != 0;  // decided / all converged earlier in the stream: empty launch
+        auto draw = [&]() { return stopped ? a.n_tiles : atomicAdd(a.sched, 1); };
         auto load_desc = [&](int tile, int4& t0, int4& t1, int& done) {
             if (tile < a.n_tiles) {
                 const int4* tdp = reinterpret_cast<const int4*>(a.tiles + tile);
@@ -560,7 +562,7 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
                                                    const int32_t* __restrict__ tile_count,
                                                    const int32_t* __restrict__ sub_dim) {
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (g >= a.ngroups) return;
+    if (g >= a.ngroups || a.ctrl[0] != 0) return;
     if (a.done_iter[g] >= 0) return;
     const int lane = threadIdx.x & 31, k = a.k;
     const int cnt = 4 * tile_count[g], n = sub_dim[g];
@@ -597,7 +599,7 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     a.tiles = p->d_tiles; a.gersh = p->d_gersh;
     a.buf0 = buf0; a.buf1 = buf1; a.bufY = bufY; a.bufW = bufW; a.partials = p->d_partials;
     a.done_iter = p->d_done_iter; a.flag = p->d_flag; a.tile_done = p->d_tile_done; a.res = p->d_res;
-    a.counters = p->d_counters; a.n_tiles = (int32_t)p->n_tiles;
+    a.counters = p->d_counters; a.n_tiles = (int32_t)p->n_tiles; a.ctrl = p->d_ctrl;
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * 3);
     a.sched = p->d_sched + 4 * k;

@@ -190,6 +190,7 @@ struct Ns32Args {
     double* partials;      // [n_tiles][4]
     const int32_t* done_iter;
     int64_t lo_plane;      // SPLIT: offset (floats) of the lo plane inside A, B, Out
+    const int32_t* ctrl;   // [0] != 0: evaluation stopped on the device: empty launch
     int32_t n_tiles;
 };
 
@@ -219,13 +220,14 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tmem = s_tmem;
+    const int n_tiles = a.ctrl[0] != 0 ? 0 : a.n_tiles;
 
     if (wid == 0) {
         // ================================================================ producer (one thread)
         if (lane == 0) {
             int stage = 0;
             unsigned phase = 0;
-            for (int t = blockIdx.x; t < a.n_tiles; t += gridDim.x) {
+            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
                 const Tile32 T = a.tiles[t];
                 if (a.done_iter[T.grp] >= 0) continue;
                 const int ldp = T.ldp;
@@ -260,7 +262,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
         if (lane == 0) {
             int stage = 0, buf = 0;
             unsigned phase = 0, tphase[2] = {0, 0};
-            for (int t = blockIdx.x; t < a.n_tiles; t += gridDim.x) {
+            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
                 const Tile32 T = a.tiles[t];
                 if (a.done_iter[T.grp] >= 0) continue;
                 const int ldp = T.ldp;
@@ -309,7 +311,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
         const int q = wid & 3;  // TMEM lane quarter this warp may access
         int buf = 0;
         unsigned tphase[2] = {0, 0};
-        for (int t = blockIdx.x; t < a.n_tiles; t += gridDim.x) {
+        for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
             const Tile32 T = a.tiles[t];
             if (a.done_iter[T.grp] >= 0) continue;
             const int ldp = T.ldp, n = T.n;
@@ -418,9 +420,9 @@ k_ns_decide32(int ngroups, int k, int decide_only, double eps, double floor_zone
               const int32_t* __restrict__ tile_first,
               const int32_t* __restrict__ tile_count, const int32_t* __restrict__ sub_dim,
               const double* __restrict__ partials, double* __restrict__ res, int32_t* __restrict__ done_iter,
-              int32_t* __restrict__ flag, int32_t* __restrict__ counters) {
+              int32_t* __restrict__ flag, int32_t* __restrict__ counters, const int32_t* __restrict__ ctrl) {
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (g >= ngroups) return;
+    if (g >= ngroups || ctrl[0] != 0) return;
     if (done_iter[g] >= 0) return;
     const int lane = threadIdx.x & 31;
     const int cnt = 4 * tile_count[g], n = sub_dim[g];
@@ -525,7 +527,7 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
     float* Y = reinterpret_cast<float*>(buf0);
     Ns32Args a;
     a.tiles = reinterpret_cast<const Tile32*>(p->d_tiles32); a.partials = p->d_partials32; a.done_iter = p->d_done_iter;
-    a.n_tiles = (int32_t)p->n_tiles32;
+    a.n_tiles = (int32_t)p->n_tiles32; a.ctrl = p->d_ctrl;
     const bool split = p->opt.precision == 2;
     a.lo_plane = split ? p->sum_ldp2 : 0;
     const int grid = (int)std::min<int64_t>(p->n_tiles32, p->num_sms);
@@ -536,7 +538,7 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
         k_ns_decide32<<<(p->ngroups + 7) / 8, 256, 0, st>>>(p->ngroups, k, decide_only, eps, 0.5,
                                                             p->d_tile_first32,
                                                             p->d_tile_count32, p->d_sub_dim, p->d_partials32, p->d_res,
-                                                            p->d_done_iter, p->d_flag, p->d_counters);
+                                                            p->d_done_iter, p->d_flag, p->d_counters, p->d_ctrl);
         p->launches += 2;
     }
     if ((which & 2) && !decide_only) {
