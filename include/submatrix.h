@@ -89,7 +89,10 @@ typedef struct {
     double overshoot;    /* scaling = 1 only: s = bound / overshoot, 1 <= overshoot <= 1.5 [1.45]*/
                          /* (eigenvalues of X0 in (1, 1.5] map back into [0.56, 1); 1.45 is   */
                          /* where the top and the bottom of the water-like spectra balance)  */
-    int32_t reserved[4];
+    int32_t predict;     /* 1: predicted exit (reading A9): a submatrix whose next residual  [1]  */
+                         /* is bounded a factor 10 below eps by ||E'|| <= 3/4||E||^2+1/4||E||^3 */
+                         /* stops after its update, without the confirming X^2 product       */
+    int32_t reserved[3];
 } sm_options_t;
 
 /* Plan facts (all sizes in elements unless they say bytes). */

@@ -26,6 +26,7 @@ static void default_options(sm_options_t* o) {
     o->early_out = 1;
     o->overshoot = 1.45;
     o->order = 2;
+    o->predict = 1;
     o->precision = 0;
     o->check_every = 8;
     o->max_mu_steps = 64;
@@ -348,7 +349,7 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
     int64_t sin3 = 0, symf = 0;
     for (int i = 0; i < ng; ++i) {
         int it = di[i] >= 0 ? di[i] : p->cur_k;
-        if (di[i] < 0 || fl[i]) ++nc;
+        if (di[i] < 0 || fl[i] == 1) ++nc;  // flag 2 = converged by the predicted exit
         imin = std::min(imin, it);
         imax = std::max(imax, it);
         int slot = di[i] >= 0 ? (di[i] & 1) : ((std::max(p->cur_k, 1) - 1) & 1);
@@ -358,7 +359,7 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         // executed symmetric products: stopped at iteration it: one X^2 per tested iterate (it + 1)
         // and one update per iteration (it); still active after cur_k launch pairs: 2 cur_k (+1 if a steering decision came between the two modes)
         const int64_t ppi = p->opt.order == 3 ? 3 : 2;  // products per iteration (Eq.(11): 2, Eq.(19): 3)
-        const int64_t prods = di[i] >= 0 ? ppi * it + 1 : ppi * (int64_t)p->cur_k + p->half_iter;
+        const int64_t prods = di[i] >= 0 ? ppi * it + (fl[i] == 2 ? 0 : 1) : ppi * (int64_t)p->cur_k + p->half_iter;
         sin3 += prods * n * n * n;
         symf += prods * n * n * (n + 1);
     }

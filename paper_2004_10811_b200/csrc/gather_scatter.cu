@@ -374,7 +374,7 @@ __global__ void k_nelec_bound(int ngroups, const int32_t* __restrict__ grp_ptr, 
     if (g >= ngroups) return;
     const int lane = threadIdx.x & 31;
     const int di = done_iter[g];
-    const int kb = di >= 0 ? di : k;
+    const int kb = (di >= 0 && di <= k) ? di : k;  // di = k + 1: predicted exit, its last update has not run yet
     const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];
     const double* Yg = bufY + ws_off[g];
     const int ld = ldv[g];

@@ -413,6 +413,8 @@ struct NsArgs {
     int32_t ngroups;
     int32_t k;
     int32_t decide_only;  // k == max_iter: stop whatever the residual is
+    int32_t predict;      // 1: predicted exit allowed (Eq.(11) path, eps well above the FP64 floor)
+    int32_t max_iter;
     double eps;
 };
 
@@ -462,7 +464,7 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
         while (tile < a.n_tiles) {
             load_desc(tile_n, n0, n1, done_n);  // in flight while this tile streams
             const int tile_nn = draw();
-            if (done < 0) {
+            if (done < 0 || done > k) {  // active (done > k: stops after the update of iteration k, see k_ns_decide)
                 const int g = t0.z;
                 const int64_t ws_off = ((int64_t)(unsigned)t0.x) | ((int64_t)t0.y << 32);
                 const int ld = t0.w, tij = t1.y;
@@ -579,7 +581,22 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
         const bool stop = conv || stag || a.decide_only || !(r == r);
         a.res[(size_t)(k & 1) * a.ngroups + g] = r;
         if (stop) { a.flag[g] = conv ? 0 : 1; a.done_iter[g] = k; }
-        else atomicAdd(a.counters + k, 1);
+        else {
+            atomicAdd(a.counters + k, 1);
+            // Predicted exit (reading A9): with E_k = X_k^2 - I symmetric, E_{k+1} = -3/4 E_k^2 - 1/4 E_k^3, so
+            // ||E_{k+1}||_F <= 3/4 ||E_k||_F^2 + 1/4 ||E_k||_F^3.  If that bound is already a factor 10 below
+            // eps, X_{k+1} is accepted without the product that would only confirm it: the submatrix takes part
+            // in the update of this iteration (done_iter = k + 1 > k) and in nothing after it.
+            if (a.predict && k + 1 < a.max_iter) {
+                const double sn = sqrt((double)(n > 0 ? n : 1)), f = r * sn;
+                const double next = (0.75 * f * f + 0.25 * f * f * f) / sn;
+                if (next < 0.1 * a.eps) {
+                    a.done_iter[g] = k + 1;
+                    a.flag[g] = 2;
+                    a.res[(size_t)((k + 1) & 1) * a.ngroups + g] = next;
+                }
+            }
+        }
     }
 }
 
@@ -601,6 +618,7 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     a.done_iter = p->d_done_iter; a.flag = p->d_flag; a.tile_done = p->d_tile_done; a.res = p->d_res;
     a.counters = p->d_counters; a.n_tiles = (int32_t)p->n_tiles; a.ctrl = p->d_ctrl;
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;
+    a.predict = (p->opt.predict != 0 && p->opt.order == 2 && eps >= 1e-13) ? 1 : 0; a.max_iter = p->opt.max_iter;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * 3);
     a.sched = p->d_sched + 4 * k;
     if (which & 1) {

@@ -424,6 +424,25 @@ def test_density_matrix_unreachable_tolerance_is_guarded(B, cfg0):
     B.sm_plan_destroy(plan)
 
 
+def test_predicted_exit_same_result_fewer_products(B, oracle, cfg0):
+    """Reading A9: with predict = 1 a submatrix whose next residual is bounded below eps / 10 stops after
+    its update without the confirming product: same iteration counts, same D~ within the parity bar,
+    fewer products executed than with predict = 0."""
+    m = cfg0
+    idx = oracle.Index(m)
+    d_or = oracle.density(idx, m.values, 0.0)
+    out = {}
+    for pr in (0, 1):
+        plan, st, d, stats, _, _ = _run_sign(B, m, opt=B.default_options(predict=pr))
+        assert st == B.SM_OK and stats.not_converged == 0
+        assert np.abs(d - d_or).max() <= TOL_D
+        out[pr] = (stats.iter_min, stats.iter_max, stats.sum_iter_n3, stats.max_residual)
+        B.sm_plan_destroy(plan)
+    assert out[0][:2] == out[1][:2]
+    assert out[1][2] < out[0][2]
+    assert out[1][3] < EPS  # measured or predicted, every residual is below eps
+
+
 # ------------------------------------------------------------------------------ Eq.(19)
 def test_third_order_iteration_eq19(B, oracle, cfg0):
     """order = 3: the paper's GPU iteration X <- 1/8 X (15 I - 10 X^2 + 3 X^4) (Eq.(19)) reaches
