@@ -361,8 +361,12 @@ sm_status_t launch_nelec(sm_plan* p, const double* buf0, const double* buf1, cud
 // Steering bound of the mu bisection (reading A11c).  After MODE 0 of iteration k >= 1 the
 // workspace holds X_k and Y_k = X_k^2, all eigenvalues x_l of X_k lie in [-1,1] and move monotonically
 // towards +-1, so with w_l = sum_{k in gen} Q_kl^2 (Algorithm 1)
-//   |n_elec(final) - n_elec(X_k)| <= 1/2 sum_l w_l (1 - |x_l|) <= 1/2 sum_l w_l (1 - x_l^2)
-//                                   = 1/2 sum_{k in gen} (1 - (Y_k)_kk).
+//   |n_elec(final) - n_elec(X_k)| <= 1/2 sum_l w_l (1 - |x_l|).
+// With u_l = 1 - x_l^2 in [0,1]:  1 - |x_l| = 1 - sqrt(1 - u_l) <= min(u_l, u_l/2 + u_l^2/2)  (the second
+// is tangent at u = 0 and exact at u = 1), and per generating row k (weights Q_kl^2, summing to 1)
+//   sum_l Q_kl^2 u_l = 1 - (Y_k)_kk =: S1,   sum_l Q_kl^2 u_l^2 = ((I - Y_k)^2)_kk = sum_j (delta_kj - Y_kj)^2 =: S2,
+// so row k contributes at most 1/2 min(S1, (S1 + S2)/2): half of the first-order bound once the
+// iteration is close to convergence.  The rows of Y_k for the generating functions are read in full.
 // part[g] = n_elec partial of X_k, part[ngroups + g] = bound partial; one warp per group.
 __global__ void k_nelec_bound(int ngroups, const int32_t* __restrict__ grp_ptr, const int32_t* __restrict__ grp_cols,
                               const int32_t* __restrict__ blk_size, const int32_t* __restrict__ gen_off,
@@ -387,16 +391,29 @@ __global__ void k_nelec_bound(int ngroups, const int32_t* __restrict__ grp_ptr, 
     for (int gc = grp_ptr[g]; gc < grp_ptr[g + 1]; ++gc) {
         const int c = grp_cols[gc];
         const int o = gen_off[c], b = blk_size[c];
-        for (int e = lane; e < b; e += 32) {
-            const size_t off = panel_off(o + e, o + e, ld);
-            a += 0.5 * (1.0 - xs * Xg[off]);
-            d += 0.5 * fmax(1.0 - Yg[off], 0.0);
-        }
-    }
+        for (int e = 0; e < b; ++e) {      // generating function (row) o + e: the lanes sweep its row of Y
+            const int row = o + e;
+            const int t0 = row & ~63;
+            const double* yr = Yg + (size_t)t0 * ld + (size_t)(row & 63) * 8;
+            const size_t pstride = (size_t)min(64, ld - t0) * 8;
+            double s2 = 0.0, ykk = 0.0;
+            for (int j = lane; j < ld; j += 32) {
+                const double y = yr[(size_t)(j >> 3) * pstride + (j & 7)];
+                const double t = (j == row ? 1.0 : 0.0) - y;
+                s2 = fma(t, t, s2);
+                if (j == row) ykk = y;
+            }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        a += __shfl_xor_sync(0xffffffffu, a, o);
-        d += __shfl_xor_sync(0xffffffffu, d, o);
+            for (int w = 16; w > 0; w >>= 1) {
+                s2 += __shfl_xor_sync(0xffffffffu, s2, w);
+                ykk += __shfl_xor_sync(0xffffffffu, ykk, w);
+            }
+            if (lane == 0) {
+                const double s1 = fmax(1.0 - ykk, 0.0);
+                a += 0.5 * (1.0 - xs * Xg[panel_off(row, row, ld)]);
+                d += 0.5 * fmin(s1, 0.5 * (s1 + s2));
+            }
+        }
     }
     if (lane == 0) { part[g] = a; part[ngroups + g] = d; }
 }
