@@ -70,7 +70,7 @@ typedef struct {
                          /* 1 = FP32 storage, plain TF32 products (error ~2e-3 class);       */
                          /* 2 = "3xTF32": operands stored as hi + lo TF32 pairs, products    */
                          /*     hi hi + hi lo + lo hi (FP32-class, <= 1e-3 bar)              */
-    int32_t check_every; /* the stop decisions are taken on the device; the host enqueues  [8]   */
+    int32_t check_every; /* the stop decisions are taken on the device; the host enqueues  [16]  */
                          /* this many iterations ahead before it reads the control block     */
                          /* (>= 1; launches after the stop are empty)                        */
     int32_t max_mu_steps;/* bisection step cap of sm_density_matrix                    [64]  */
@@ -142,6 +142,7 @@ typedef struct {
     float tot_ms_gather, tot_ms_sign;
     double spec_lo, spec_hi;  /* scaling = 1: the widened Lanczos estimate of [lambda_min, lambda_max] */
                               /* of K~ the interlacing bound was taken from (else 0, 0)       */
+    double bracket_lo, bracket_hi; /* sm_density_matrix: the initial bisection bracket        */
 } sm_stats_t;
 
 /*
@@ -203,7 +204,9 @@ sm_status_t sm_sign_execute_host(sm_plan_t* plan, const double* h_vals_in, doubl
  * n_target, "using a simple bisection" (L266).  Newton-Schulz keeps no eigendecomposition, so
  * every step re-evaluates the sign function (the cost L266 warns about).
  * Rule (reading A11): step 0 evaluates *mu_inout; then midpoint bisection inside the
- * Gershgorin interval of K~ (n_elec = 0 below, = n_basis above), raising mu if n_elec < n_target.
+ * Gershgorin interval of K~ (n_elec = 0 below, = n_basis above; intersected with the interlacing
+ * interval of K~'s extreme eigenvalues when scaling = 1; reported in stats->bracket_lo/hi), raising
+ * mu if n_elec < n_target.
  * Stops when |n_elec - n_target| <= tol_n (SM_OK), or when the bracket is narrower than
  * opt.mu_tol or after opt.max_mu_steps evaluations (SM_WARN_MU_NOT_CONVERGED); returns in
  * *mu_inout the evaluated mu with the smallest |n_elec - n_target| and in d_vals_out D~ at that mu.

@@ -28,7 +28,7 @@ static void default_options(sm_options_t* o) {
     o->order = 2;
     o->predict = 1;
     o->precision = 0;
-    o->check_every = 8;
+    o->check_every = 16;
     o->max_mu_steps = 64;
     o->bisect_iter = 0;
     o->mu_tol = 1e-6;
@@ -534,10 +534,19 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     sm_stats_t local;
     sm_stats_t* S = stats ? stats : &local;
     memset(S, 0, sizeof(*S));
-    // bracket: Gershgorin interval of the whole K~ (n_elec = 0 below, n_basis above)
+    // bracket (n_elec = 0 below, n_basis above): the Gershgorin interval of the whole K~, intersected with
+    // the interlacing interval [lambda_min, lambda_max](K~) of the Lanczos run when scaling = 1 has it
+    // (every submatrix eigenvalue lies inside both, reading A11)
     if ((s = launch_gersh_global(p, d_vals_in, st))) return s;
     SM_CUDA(cudaMemcpy(p->h_pinned_d + 4, p->d_scalars + 4, 16, cudaMemcpyDeviceToHost));
     double lo = p->h_pinned_d[4], hi = p->h_pinned_d[5];
+    p->lz_valid = 0;  // one Lanczos run serves every mu of this call
+    if (p->opt.scaling == 1) {
+        if ((s = ensure_bounds(p, d_vals_in, st))) return s;
+        lo = std::max(lo, p->lz_lo);
+        hi = std::min(hi, p->lz_hi);
+    }
+    S->bracket_lo = lo; S->bracket_hi = hi;
     double mu = *mu_inout;
     const int cap = (p->opt.precision == 0 && p->opt.bisect_iter > 0 && p->opt.bisect_iter < p->opt.max_iter)
                         ? p->opt.bisect_iter : p->opt.max_iter + 1;
@@ -552,7 +561,6 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         acc_n3 += e.tot_sum_iter_n3; acc_sym += e.tot_sym_flop; acc_launch += e.tot_gemm_launches;
         acc_eval += 1; acc_g += e.tot_ms_gather; acc_s += e.tot_ms_sign;
     };
-    p->lz_valid = 0;  // one Lanczos run serves every mu of this call
     const bool early = p->opt.early_out != 0 && p->opt.precision == 0;
     for (; steps < p->opt.max_mu_steps;) {
         memset(&ev, 0, sizeof(ev));
@@ -603,7 +611,9 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     memcpy(tr_ne, S->ne_trace, sizeof(tr_ne));
     memcpy(tr_err, S->ne_err_trace, sizeof(tr_err));
     memcpy(tr_it, S->iter_trace, sizeof(tr_it));
+    const double br_lo = S->bracket_lo, br_hi = S->bracket_hi;
     *S = ev;
+    S->bracket_lo = br_lo; S->bracket_hi = br_hi;
     memcpy(S->mu_trace, tr_mu, sizeof(tr_mu));
     memcpy(S->ne_trace, tr_ne, sizeof(tr_ne));
     memcpy(S->ne_err_trace, tr_err, sizeof(tr_err));

@@ -350,7 +350,13 @@ def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling):
         stats = B.sm_stats_t()
         st, mu = B.sm_density_matrix(plan, vin, float(m.n_occ), tol_n, EPS, mu0, vout, ws, stats)
         torch.cuda.synchronize()
-        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0, lo, hi, tol_n)
+        # the oracle bisects in the bracket the library reports: the Gershgorin interval (scaling = 0),
+        # intersected with the interlacing interval of K~ (scaling = 1); both enclose every submatrix spectrum
+        assert lo <= stats.bracket_lo + 1e-12 and stats.bracket_hi <= hi + 1e-12
+        if scaling == 0:
+            assert abs(stats.bracket_lo - lo) <= 1e-12 * abs(lo) and abs(stats.bracket_hi - hi) <= 1e-12 * abs(hi)
+        assert stats.bracket_lo <= lam.min() and lam.max() <= stats.bracket_hi
+        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0, stats.bracket_lo, stats.bracket_hi, tol_n)
         assert st == B.SM_OK
         assert stats.mu_steps == len(trace_o)
         n_partial = 0
