@@ -107,6 +107,9 @@ struct sm_plan {
     int64_t n_tiles32 = 0, sum_ldp2 = 0;
     int32_t* d_ctrl = nullptr;             // [8] + doubles: device-side stop decision of an evaluation (EvalCtrl)
     void* h_ctrl = nullptr;                // pinned mirror
+    int64_t* d_gl_ptr = nullptr;           // gather list (built by the first gather): extents per member column
+    uint32_t* d_gl = nullptr;              //   entries: member index << 16 | value offset inside the block column
+    int gather_no_list = 0;
     uint32_t* d_src_map = nullptr;         // [nnz] scatter source map (built by the first scatter)
     int scatter_chunks = 1;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated

@@ -52,9 +52,11 @@ struct GatherArgs {
     unsigned long long* gersh;
     double mu;
     int tile_ld, msb, mpad, mc, hash_size, hash_shift;
+    const int64_t* gl_ptr;   // LIST: per (submatrix, member column) extent in gl
+    const uint32_t* gl;      // LIST: member index t << 16 | value offset of block (S_i[t], S_i[tc]) in its column
 };
 
-template <typename MapT>
+template <typename MapT, bool LIST>
 __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
     constexpr MapT NONE = (MapT)~(MapT)0;  // block (S_i[t], S_i[tc]) not stored
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -72,7 +74,8 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
     int32_t* hv = hk + A.hash_size;                                             // [hash_size] member index
     int32_t* mSo = hv + A.hash_size;                                            // [msb + 1] element offsets
     int32_t* mKey = mSo + msb + 2;                                              // [msb] global block index of the member
-    for (int h = threadIdx.x; h < A.hash_size; h += blockDim.x) hk[h] = -1;
+    if (!LIST)
+        for (int h = threadIdx.x; h < A.hash_size; h += blockDim.x) hk[h] = -1;
     for (int t = threadIdx.x; t < m; t += blockDim.x) mSo[t] = A.sub_off[sp + t];
     if (threadIdx.x == 0) mSo[m] = n;
     __syncthreads();
@@ -81,9 +84,11 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
         const int key = A.sub_blocks[sp + t];
         mKey[t] = key;
         mVb[t] = A.val_off[A.colptr[key]];
-        unsigned h = gather_hash(key, A.hash_shift);
-        while (atomicCAS(&hk[h], -1, key) != -1) h = (h + 1) & hmask;
-        hv[h] = t;
+        if (!LIST) {
+            unsigned h = gather_hash(key, A.hash_shift);
+            while (atomicCAS(&hk[h], -1, key) != -1) h = (h + 1) & hmask;
+            hv[h] = t;
+        }
         const int so = mSo[t], br = mSo[t + 1] - so;
         for (int el = 0; el < br; ++el) posmap[so + el] = make_uint2((unsigned)t, (unsigned)el | ((unsigned)br << 16));
     }
@@ -99,9 +104,17 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
         __syncthreads();
         // block map of member columns c0..c1-1: one warp per column, lanes over its stored blocks
         for (int tc = c0 + wid; tc < c1; tc += nw) {
+            MapT* row = bmap + (size_t)(tc - c0) * mpad;
+            if (LIST) {  // the pairs (member, value offset) were listed when the plan first gathered
+                const int64_t e1 = A.gl_ptr[sp + tc + 1];
+                for (int64_t e = A.gl_ptr[sp + tc] + lane; e < e1; e += 32) {
+                    const uint32_t v = __ldg(A.gl + e);
+                    row[v >> 16] = (MapT)(v & 0xffffu);
+                }
+                continue;
+            }
             const int key = mKey[tc];
             const int64_t p0 = A.colptr[key], p1 = A.colptr[key + 1], vb = mVb[tc];
-            MapT* row = bmap + (size_t)(tc - c0) * mpad;
             for (int64_t j = p0 + lane; j < p1; j += 32) {
                 const int r = __ldg(A.rowidx + j);
                 const int rel = (int)(__ldg(A.val_off + j) - vb);
@@ -162,12 +175,100 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
     if (lane == 0 && cmax > 0.0) atomicMax(A.gersh + g, (unsigned long long)__double_as_longlong(cmax));
 }
 
+// Gather list (pattern only, built by the first gather of a plan when 16-bit entries suffice): for every
+// submatrix i and member column tc the pairs (t, value offset) of the stored blocks (S_i[t], S_i[tc]).
+// One CTA per submatrix, hash table of S_i in shared memory, one warp per member column; FILL = false
+// counts, FILL = true writes (order inside a column: ascending stored position, by ballot ranks).
+template <bool FILL>
+__global__ void __launch_bounds__(256)
+k_glist(const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx, const int64_t* __restrict__ val_off,
+        const int64_t* __restrict__ sub_ptr, const int32_t* __restrict__ sub_blocks, int hash_size, int hash_shift,
+        int32_t* __restrict__ cnt, const int64_t* __restrict__ gl_ptr, uint32_t* __restrict__ gl) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    int32_t* hk = reinterpret_cast<int32_t*>(smem_raw);
+    int32_t* hv = hk + hash_size;
+    const int g = blockIdx.x;
+    const int64_t sp = sub_ptr[g];
+    const int m = (int)(sub_ptr[g + 1] - sp);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int h = threadIdx.x; h < hash_size; h += blockDim.x) hk[h] = -1;
+    __syncthreads();
+    const unsigned hmask = (unsigned)hash_size - 1u;
+    for (int t = threadIdx.x; t < m; t += blockDim.x) {
+        const int key = sub_blocks[sp + t];
+        unsigned h = gather_hash(key, hash_shift);
+        while (atomicCAS(&hk[h], -1, key) != -1) h = (h + 1) & hmask;
+        hv[h] = t;
+    }
+    __syncthreads();
+    for (int tc = wid; tc < m; tc += nw) {
+        const int key = sub_blocks[sp + tc];
+        const int64_t p0 = colptr[key], p1 = colptr[key + 1], vb = val_off[p0];
+        int64_t out = FILL ? gl_ptr[sp + tc] : 0;
+        int total = 0;
+        for (int64_t j0 = p0; j0 < p1; j0 += 32) {
+            const int64_t j = j0 + lane;
+            int t = -1;
+            if (j < p1) {
+                const int r = __ldg(rowidx + j);
+                unsigned h = gather_hash(r, hash_shift);
+                for (;;) {
+                    const int k = hk[h];
+                    if (k == r) { t = hv[h]; break; }
+                    if (k < 0) break;
+                    h = (h + 1) & hmask;
+                }
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, t >= 0);
+            if (FILL && t >= 0)
+                gl[out + __popc(mask & ((1u << lane) - 1u))] = ((uint32_t)t << 16) | (uint32_t)(__ldg(val_off + j) - vb);
+            out += __popc(mask);
+            total += __popc(mask);
+        }
+        if (!FILL && lane == 0) cnt[sp + tc] = total;
+    }
+}
+
+static sm_status_t build_gather_list(sm_plan* p, cudaStream_t st) {
+    const int64_t tot = p->info.sum_sub_blocks;
+    const size_t hbytes = (size_t)p->gather_hash_size * 8;
+    if (hbytes > 48 * 1024) {
+        SM_CUDA(cudaFuncSetAttribute(k_glist<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hbytes));
+        SM_CUDA(cudaFuncSetAttribute(k_glist<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hbytes));
+    }
+    int32_t* d_cnt = nullptr;
+    SM_CUDA(cudaMalloc((void**)&d_cnt, (size_t)std::max<int64_t>(tot, 1) * 4));
+    k_glist<false><<<p->ngroups, 256, hbytes, st>>>(p->d_colptr, p->d_rowidx, p->d_val_off, p->d_sub_ptr, p->d_sub_blocks,
+                                                    p->gather_hash_size, p->gather_hash_shift, d_cnt, nullptr, nullptr);
+    std::vector<int32_t> cnt((size_t)tot);
+    SM_CUDA(cudaMemcpyAsync(cnt.data(), d_cnt, (size_t)tot * 4, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    cudaFree(d_cnt);
+    std::vector<int64_t> ptr((size_t)tot + 1, 0);
+    for (int64_t i = 0; i < tot; ++i) ptr[i + 1] = ptr[i] + cnt[i];
+    SM_CUDA(cudaMalloc((void**)&p->d_gl_ptr, ((size_t)tot + 1) * 8));
+    SM_CUDA(cudaMemcpyAsync(p->d_gl_ptr, ptr.data(), ((size_t)tot + 1) * 8, cudaMemcpyHostToDevice, st));
+    SM_CUDA(cudaMalloc((void**)&p->d_gl, (size_t)std::max<int64_t>(ptr[tot], 1) * 4));
+    k_glist<true><<<p->ngroups, 256, hbytes, st>>>(p->d_colptr, p->d_rowidx, p->d_val_off, p->d_sub_ptr, p->d_sub_blocks,
+                                                   p->gather_hash_size, p->gather_hash_shift, nullptr, p->d_gl_ptr, p->d_gl);
+    p->launches += 2;
+    SM_CUDA(cudaStreamSynchronize(st));  // ptr[] is read by the copy above
+    SM_CUDA(cudaGetLastError());
+    return SM_OK;
+}
+
 sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, cudaStream_t st) {
     if (p->ngroups == 0) return SM_OK;
+    const bool list = p->gather_map16 && p->gather_msb < 65536 && !p->gather_no_list;
+    if (list && !p->d_gl) {
+        sm_status_t s = build_gather_list(p, st);
+        if (s) return s;
+    }
     SM_CUDA(cudaMemsetAsync(p->d_gersh, 0, (size_t)p->ngroups * 8, st));
     if (p->gather_smem > 48 * 1024) {
-        SM_CUDA(cudaFuncSetAttribute(k_gather<uint16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
-        SM_CUDA(cudaFuncSetAttribute(k_gather<uint32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
+        SM_CUDA(cudaFuncSetAttribute(k_gather<uint16_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
+        SM_CUDA(cudaFuncSetAttribute(k_gather<uint16_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
+        SM_CUDA(cudaFuncSetAttribute(k_gather<uint32_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
     }
     GatherArgs a;
     a.colptr = p->d_colptr; a.rowidx = p->d_rowidx; a.val_off = p->d_val_off; a.vals = vals;
@@ -175,8 +276,11 @@ sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, 
     a.ldv = p->d_ld; a.ws_off = p->d_ws_off; a.X = X; a.gersh = p->d_gersh; a.mu = mu;
     a.tile_ld = p->gather_tile_ld; a.msb = p->gather_msb; a.mpad = p->gather_mpad; a.mc = p->gather_mc;
     a.hash_size = p->gather_hash_size; a.hash_shift = p->gather_hash_shift;
-    if (p->gather_map16) k_gather<uint16_t><<<dim3(p->ngroups, p->gather_split), p->gather_warps * 32, p->gather_smem, st>>>(a);
-    else k_gather<uint32_t><<<dim3(p->ngroups, p->gather_split), p->gather_warps * 32, p->gather_smem, st>>>(a);
+    a.gl_ptr = p->d_gl_ptr; a.gl = p->d_gl;
+    const dim3 grid(p->ngroups, p->gather_split);
+    if (list) k_gather<uint16_t, true><<<grid, p->gather_warps * 32, p->gather_smem, st>>>(a);
+    else if (p->gather_map16) k_gather<uint16_t, false><<<grid, p->gather_warps * 32, p->gather_smem, st>>>(a);
+    else k_gather<uint32_t, false><<<grid, p->gather_warps * 32, p->gather_smem, st>>>(a);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
