@@ -477,9 +477,10 @@ __global__ void k_nelec_bound(int ngroups, const int32_t* __restrict__ grp_ptr, 
                               const int32_t* __restrict__ ldv, const int64_t* __restrict__ ws_off,
                               const int32_t* __restrict__ done_iter, const unsigned long long* __restrict__ gersh,
                               int k, const double* __restrict__ buf0, const double* __restrict__ buf1,
-                              const double* __restrict__ bufY, double* __restrict__ part) {
+                              const double* __restrict__ bufY, double* __restrict__ part,
+                              const int32_t* __restrict__ ctrl) {
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (g >= ngroups) return;
+    if (g >= ngroups || ctrl[0] != 0) return;  // evaluation already stopped: empty launch
     const int lane = threadIdx.x & 31;
     const int di = done_iter[g];
     const int kb = (di >= 0 && di <= k) ? di : k;  // di = k + 1: predicted exit, its last update has not run yet
@@ -528,7 +529,7 @@ sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const doub
     if (p->ngroups == 0) return SM_OK;
     k_nelec_bound<<<(p->ngroups + 7) / 8, 256, 0, st>>>(p->ngroups, p->d_grp_ptr, p->d_grp_cols, p->d_blk_size,
                                                         p->d_gen_off, p->d_ld, p->d_ws_off, p->d_done_iter, p->d_gersh,
-                                                        k, buf0, buf1, bufY, p->d_bound_part);
+                                                        k, buf0, buf1, bufY, p->d_bound_part, p->d_ctrl);
     k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part, p->ngroups, p->d_bound + 2 * k);
     k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part + p->ngroups, p->ngroups, p->d_bound + 2 * k + 1);
     p->launches += 3;
