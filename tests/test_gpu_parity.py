@@ -214,6 +214,50 @@ def test_config4_sampled_parity_full_size(B, oracle):
     _sampled_parity(B, oracle, W.make_config(4), k=16)
 
 
+def test_config4_density_matrix_as_benchmarked(B, oracle):
+    """BASELINE config 4 exactly as bench.py runs it: sm_density_matrix from mu0 = -1 with plateau
+    acceptance (tol_n = 0.5, reading A11), default options.  Sampled parity of D~ at the returned mu
+    (oracle's fixed-mu path, reading A12), plus what holds at any size: the accepted count lies on the
+    gap plateau, steering steps report a bound that separates them from the target, the trace is a
+    bisection inside the reported bracket."""
+    torch = _torch()
+    m = W.make_config(4)
+    plan = B.plan_from_matrix(m)
+    ws = B.alloc_workspace(plan)
+    vin = torch.from_numpy(m.values).cuda()
+    vout = torch.full_like(vin, float("nan"))
+    stats = B.sm_stats_t()
+    st, mu = B.sm_density_matrix(plan, vin, float(m.n_occ), 0.5, EPS, -1.0, vout, ws, stats)
+    torch.cuda.synchronize()
+    assert st == B.SM_OK
+    d_gpu = vout.cpu().numpy()
+    assert np.all(np.isfinite(d_gpu))
+    assert abs(stats.n_elec - m.n_occ) <= 0.5 and stats.not_converged == 0 and stats.max_residual < EPS
+    n = stats.mu_steps
+    lo, hi = stats.bracket_lo, stats.bracket_hi
+    for k in range(n):
+        muk, nek, errk = stats.mu_trace[k], stats.ne_trace[k], stats.ne_err_trace[k]
+        assert lo <= muk <= hi or k == 0
+        if k < n - 1:  # a steering or rejected step: on a proven side of the target
+            assert abs(nek - m.n_occ) > errk + 0.5
+            if k >= 1:
+                assert abs(muk - 0.5 * (lo + hi)) <= 1e-12 * max(1.0, abs(muk))  # midpoint of the current bracket
+            if nek < m.n_occ: lo = max(lo, muk)
+            else: hi = min(hi, muk)
+    assert stats.ne_err_trace[n - 1] == 0.0 and abs(stats.mu_trace[n - 1] - mu) == 0.0
+    idx = oracle.Index(m)
+    groups = _sample_groups(idx, 8, seed=1)
+    d_or = oracle.density(idx, m.values, mu, groups)
+    mask, cols = _column_mask(idx, m, groups)
+    assert np.abs(d_gpu - d_or)[mask].max() <= TOL_D
+    td_o, tdk_o = oracle.traces(idx, d_or, m.values, cols)
+    td_g, tdk_g = oracle.traces(idx, d_gpu, m.values, cols)
+    assert abs(tdk_g - tdk_o) / abs(tdk_o) <= TOL_E
+    td_all, _ = B.sm_trace_dk(plan, vout, vin)
+    assert abs(td_all - stats.n_elec) <= 1e-9 * td_all
+    B.sm_plan_destroy(plan)
+
+
 # ------------------------------------------------------------------------------ edge cases
 def test_large_member_count_chunked_block_map(B, oracle):
     """|S_i| = 288 members: the gather's block map does not fit its shared-memory budget and is
