@@ -138,8 +138,10 @@ def cpu_baseline(m, sample_groups=None, nthreads=0):
     cores = nthreads or os.cpu_count() or 1
     idx = O.Index(m)
     if sample_groups is None:
-        k = min(idx.ngroups, 4 * cores)
-        sample_groups = np.linspace(0, idx.ngroups - 1, k).astype(np.int32)
+        # bounded sample: ~10-20 s of CPU work (the Jacobi oracle runs ~1.2e9 n^3-units per core in that time)
+        mean_n3 = float((idx.sub_dim.astype(np.float64) ** 3).mean())
+        k = int(max(min(cores, idx.ngroups), min(idx.ngroups, 1.2e9 * cores / mean_n3)))
+        sample_groups = np.unique(np.linspace(0, idx.ngroups - 1, k).astype(np.int32))
     t0 = time.perf_counter()
     _ = O._run_groups(idx, m.values, sample_groups, 0.0, True, True, cores)
     dt = time.perf_counter() - t0
