@@ -88,7 +88,6 @@ struct sm_plan {
     double* d_partials = nullptr;          // [n_tiles][4] per-tile, per-consumer-warp residual partials
     int32_t* d_counters = nullptr;         // [max_iter+2] still-active submatrices after iteration k
     int32_t* d_sched = nullptr;            // [2*(max_iter+2)] work counters of the persistent GEMM launches
-    int32_t* d_tile_done = nullptr;        // [ngroups] finished tiles of a submatrix in the current launch
     double* d_ne_part = nullptr;           // [ngroups] per-group electron-count partials
     double* d_scalars = nullptr;           // [8] n_elec, tr D, tr DK, gersh lo/hi
     double* d_red = nullptr;               // [2*4096] reduction scratch
@@ -122,7 +121,7 @@ struct sm_plan {
     int64_t launches = 0;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_iter[2] = {nullptr, nullptr};
-    int gather_warps = 8, gather_qt = 4, gather_tile_ld = 0, gather_chunk = 32, gather_msb = 2, gather_split = 1;
+    int gather_warps = 8, gather_tile_ld = 0, gather_msb = 2, gather_split = 1;
     int gather_hash_size = 32, gather_hash_shift = 27, gather_mpad = 4, gather_mc = 2, gather_map16 = 0;
     int32_t max_col_blocks = 0;  // longest block column
     size_t gather_smem = 0;

@@ -19,19 +19,21 @@ __device__ __forceinline__ int find_sorted64(const int32_t* __restrict__ a, int 
 // Gather (PAPER.md L125 step 1; L187 "submatrix assembly becomes a purely local operation").
 // grid = (ngroups, split); one CTA (or `split` CTAs sharing the dense rows) per submatrix, NO matrix
 // data staged in shared memory.  Per CTA, in shared memory:
-//   * a hash table  block row -> member index t of S_i,
 //   * posmap[p] for every dense row p of a_i: its member t, the row el inside the block, the block
 //     height (p >= n: the "no member" column of the block map),
 //   * the BLOCK MAP of a chunk of member columns:  bmap[tc][t] = offset of the stored block
-//     (S_i[t], S_i[tc]) inside the values of block column S_i[tc], (16 bits when every block column holds fewer than 65535 values), or all-ones if it is not stored
-//     (reading A4: zero fill).  It is built by walking the stored block columns once (coalesced
-//     reads of rowidx / val_off, one hash probe per stored block; blocks whose row is not in S_i
-//     are dropped).
+//     (S_i[t], S_i[tc]) inside the values of block column S_i[tc] (16 bits when every block column
+//     holds fewer than 65535 values), or all-ones if it is not stored (reading A4: zero fill).
+//     LIST = true: filled from the plan's gather list -- the (t, offset) pairs of every submatrix
+//     column, listed once per plan by k_glist (pattern only).  LIST = false (32-bit entries): built
+//     in place by walking the stored block columns (coalesced reads of rowidx / val_off, one probe
+//     of a hash table  block row -> member  per stored block; rows outside S_i are dropped).
 // Sweep: dense column q of a_i is row q of the symmetric X; one warp per row, lanes two positions
-// at a time: posmap (one 16-byte read), two block-map reads, predicated 8-byte loads of the stored
-// values straight from global memory (L2-resident: every value is used by ~|S_i| submatrices), mu
-// subtracted on the diagonal (Eq.(16)), one coalesced 16-byte store into the k8-panel workspace,
-// abs-sums for the Gershgorin bound s_i = max_q sum_p |a_pq|.
+// at a time in groups of four 64-wide steps (warp-uniform trip count): posmap (one 16-byte read),
+// two block-map reads, predicated 8-byte loads of the stored values straight from global memory
+// (L2-resident: every value is used by ~|S_i| submatrices), mu subtracted on the diagonal
+// (Eq.(16)), one coalesced 16-byte store into the k8-panel workspace, abs-sums for the Gershgorin
+// bound s_i = max_q sum_p |a_pq|.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned gather_hash(int key, int shift) {
     return ((unsigned)key * 2654435761u) >> shift;

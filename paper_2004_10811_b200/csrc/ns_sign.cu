@@ -3,11 +3,13 @@
 //
 // Two persistent kernels per iteration over ALL submatrices at once; the unit of work is one 64x64
 // lower-triangular tile of one submatrix, handed out by an atomic counter:
-//   MODE 0:  Y  = alpha * X X          + ||Y - I||_F^2 per tile; the CTA that finishes the last
-//                                        tile of a submatrix sums the partials in a fixed order and
-//                                        records the convergence decision (deterministic)
-//   MODE 1:  X' = a X + b (X Y)        (a = 3/2, b = -1/2; iteration 0 folds the spectral scale
-//                                        1/s_i into alpha, a, b so that no scaling pass is needed)
+//   MODE 0:  Y  = alpha * X X          + per-warp partials of ||Y - I||_F^2 (plain stores);
+//                                        k_ns_decide then sums them per submatrix in a fixed order
+//                                        and records the convergence decision (deterministic)
+//   MODE 1:  X' = -1/2 (X Y - 3 X)     (iteration 0 folds the spectral scale 1/s_i into the
+//                                        coefficients, so that no scaling pass is needed)
+//   MODE 2/3: the two products of the third-order iteration Eq.(19) L348 (option order = 3).
+// A launch issued after the evaluation was stopped on the device (EvalCtrl, common.cuh) is empty.
 // X, Y and X' are symmetric polynomials of the same matrix, so only tiles on or below the diagonal
 // are computed and every element is stored together with its mirror image: the stored matrices are
 // bitwise symmetric, which also lets both GEMM operands be read as k-contiguous rows
@@ -404,7 +406,6 @@ struct NsArgs {
     double* partials;
     int32_t* done_iter;
     int32_t* flag;
-    int32_t* tile_done;  // [ngroups] tiles of the submatrix finished in this MODE 0 launch
     double* res;         // [2][ngroups]
     int32_t* counters;   // [max_iter+2] still-active submatrices after iteration k
     int32_t* sched;      // work counter of this launch
@@ -615,7 +616,7 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     NsArgs a;
     a.tiles = p->d_tiles; a.gersh = p->d_gersh;
     a.buf0 = buf0; a.buf1 = buf1; a.bufY = bufY; a.bufW = bufW; a.partials = p->d_partials;
-    a.done_iter = p->d_done_iter; a.flag = p->d_flag; a.tile_done = p->d_tile_done; a.res = p->d_res;
+    a.done_iter = p->d_done_iter; a.flag = p->d_flag; a.res = p->d_res;
     a.counters = p->d_counters; a.n_tiles = (int32_t)p->n_tiles; a.ctrl = p->d_ctrl;
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;
     a.predict = (p->opt.predict != 0 && p->opt.order == 2 && eps >= 1e-13) ? 1 : 0; a.max_iter = p->opt.max_iter;
