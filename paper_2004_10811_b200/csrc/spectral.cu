@@ -14,6 +14,39 @@ constexpr int LZ_STEPS = 24;  // extreme Ritz values within ~1 % of the spread (
 
 // y = K x for the symmetric block-CSC K~: y_c = sum_{(r,c) stored} K[r,c]^T x_r, one warp per block
 // column (no atomics); lane b takes every 32nd block of the column.  part[c] = y_c . x_c.
+// For the common block widths (1, 4, 5, 13: H and O in SZV / DZVP) the lane keeps the partial sums of
+// all dense columns of the block column in registers, so index and values of a block are read once.
+template <int BC>
+__device__ __forceinline__ double lz_col(int lane, int oc, int64_t p0, int64_t p1, const int32_t* __restrict__ blk_size,
+                                         const int32_t* __restrict__ blk_off, const int32_t* __restrict__ rowidx,
+                                         const int64_t* __restrict__ val_off, const double* __restrict__ vals,
+                                         const double* __restrict__ x, double* __restrict__ y) {
+    double a[BC];
+#pragma unroll
+    for (int q = 0; q < BC; ++q) a[q] = 0.0;
+    for (int64_t b = p0 + lane; b < p1; b += 32) {
+        const int r = __ldg(rowidx + b);
+        const int br = __ldg(blk_size + r);
+        const double* blk = vals + __ldg(val_off + b);
+        const double* xr = x + __ldg(blk_off + r);
+        for (int e = 0; e < br; ++e) {
+            const double xe = xr[e];
+#pragma unroll
+            for (int q = 0; q < BC; ++q) a[q] = fma(blk[q * br + e], xe, a[q]);
+        }
+    }
+    double dot = 0.0;
+#pragma unroll
+    for (int q = 0; q < BC; ++q) {
+        double v = a[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) y[oc + q] = v;
+        dot = fma(v, x[oc + q], dot);
+    }
+    return dot;
+}
+
 __global__ void __launch_bounds__(256)
 k_lz_spmv(int nb, const int32_t* __restrict__ blk_size, const int32_t* __restrict__ blk_off,
           const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx,
@@ -25,19 +58,26 @@ k_lz_spmv(int nb, const int32_t* __restrict__ blk_size, const int32_t* __restric
     const int bc = blk_size[c], oc = blk_off[c];
     const int64_t p0 = colptr[c], p1 = colptr[c + 1];
     double dot = 0.0;
-    for (int q = 0; q < bc; ++q) {
-        double a = 0.0;
-        for (int64_t b = p0 + lane; b < p1; b += 32) {
-            const int r = rowidx[b];
-            const int br = blk_size[r];
-            const double* col = vals + val_off[b] + (size_t)q * br;
-            const double* xr = x + blk_off[r];
-            for (int e = 0; e < br; ++e) a = fma(col[e], xr[e], a);
-        }
+    switch (bc) {
+        case 1: dot = lz_col<1>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, x, y); break;
+        case 4: dot = lz_col<4>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, x, y); break;
+        case 5: dot = lz_col<5>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, x, y); break;
+        case 13: dot = lz_col<13>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, x, y); break;
+        default:
+            for (int q = 0; q < bc; ++q) {
+                double a = 0.0;
+                for (int64_t b = p0 + lane; b < p1; b += 32) {
+                    const int r = rowidx[b];
+                    const int br = blk_size[r];
+                    const double* col = vals + val_off[b] + (size_t)q * br;
+                    const double* xr = x + blk_off[r];
+                    for (int e = 0; e < br; ++e) a = fma(col[e], xr[e], a);
+                }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-        if (lane == 0) y[oc + q] = a;
-        dot = fma(a, x[oc + q], dot);
+                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                if (lane == 0) y[oc + q] = a;
+                dot = fma(a, x[oc + q], dot);
+            }
     }
     if (lane == 0) part[c] = dot;
 }
