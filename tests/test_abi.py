@@ -47,3 +47,44 @@ def test_strerror_and_missing_library_is_loud(monkeypatch):
         assert "no CPU fallback" in str(e)
     else:
         raise AssertionError("missing library must raise")
+
+
+def test_plan_validation_is_host_logic():
+    """Structure errors (readings A1, A3, A6) are detected on the host before any CUDA call, so the
+    validation of sm_plan_create can be exercised without a GPU: every malformed input must come back
+    as its documented status with *plan == NULL."""
+    import numpy as np
+    from paper_2004_10811_b200 import binding as B, workloads as W
+    L = B.lib()
+    m = W.random_block_pattern(nb=12, density=0.3, max_bs=3, seed=1)
+
+    def status(nb=None, blk_size=None, colptr=None, rowidx=None, ngroups=None, grp_ptr=None, grp_cols=None, opt=None):
+        a = [np.ascontiguousarray(x) for x in (
+            m.blk_size if blk_size is None else blk_size, m.colptr if colptr is None else colptr,
+            m.rowidx if rowidx is None else rowidx, m.grp_ptr if grp_ptr is None else grp_ptr,
+            m.grp_cols if grp_cols is None else grp_cols)]
+        plan = ctypes.c_void_p(0xdead)
+        st = L.sm_plan_create(ctypes.byref(plan), m.nb if nb is None else nb, a[0].ctypes.data, a[1].ctypes.data,
+                              a[2].ctypes.data, m.ngroups if ngroups is None else ngroups, a[3].ctypes.data,
+                              a[4].ctypes.data, opt, None)
+        assert st < 0 and not plan.value  # every case below is an error: *plan is reset to NULL
+        return st
+
+    cols = m.block_cols()
+    gc = m.grp_cols.copy(); gc[0] = gc[1]
+    assert status(grp_cols=gc) == B.SM_ERR_STRUCTURE                      # groups not a partition (A6)
+    gp = m.grp_ptr.copy(); gp[-1] -= 1
+    assert status(grp_ptr=gp) == B.SM_ERR_STRUCTURE                       # groups do not cover all columns
+    k = np.nonzero(m.rowidx != cols)[0][0]                                # drop one off-diagonal block: asymmetric (A1)
+    cp = m.colptr.copy(); cp[cols[k] + 1:] -= 1
+    assert status(rowidx=np.delete(m.rowidx, k), colptr=cp) == B.SM_ERR_STRUCTURE
+    k = np.nonzero(m.rowidx == cols)[0][0]                                # drop a diagonal block (A3)
+    cp = m.colptr.copy(); cp[cols[k] + 1:] -= 1
+    assert status(rowidx=np.delete(m.rowidx, k), colptr=cp) == B.SM_ERR_STRUCTURE
+    c = int(np.argmax(np.diff(m.colptr) >= 2))                            # unsorted rows inside a column
+    r = m.rowidx.copy(); p0 = m.colptr[c]; r[[p0, p0 + 1]] = r[[p0 + 1, p0]]
+    assert status(rowidx=r) == B.SM_ERR_STRUCTURE
+    bs = m.blk_size.copy(); bs[3] = 0
+    assert status(blk_size=bs) == B.SM_ERR_INVALID_ARG                    # non-positive block size
+    assert status(nb=-1) == B.SM_ERR_INVALID_ARG
+    assert L.sm_plan_create(None, m.nb, None, None, None, 0, None, None, None, None) == B.SM_ERR_INVALID_ARG
