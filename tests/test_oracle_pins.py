@@ -312,3 +312,55 @@ def test_flop_model_eq14_eq15(oracle):
                            np.array([0, 2, 3], np.int32), np.array([0, 1, 2], np.int32))
     ops, ops_cols, S = oracle.flop_model(tri, oracle.Index(tri))
     assert (ops, ops_cols) == (6 ** 3 + 4 ** 3, 5 ** 3 + 6 ** 3 + 4 ** 3) and abs(S - 405 / 280) < 1e-15
+
+
+def test_steering_bound_inequality(oracle, cfg0):
+    """DESIGN.md reading A11c, checked with the oracle's eigendecompositions (no CUDA): for the
+    Newton-Schulz iterate x_k of every eigenvalue (scalar map of Eq.(11)) and Algorithm 1's weights
+    w_l = sum_{k in gen} Q_kl^2, the distance of the running count to the final count is bounded by
+    1/2 sum_k min(S1_k, (S1_k + S2_k)/2), S1 = 1 - (X^2)_kk, S2 = sum_j (delta_kj - (X^2)_kj)^2 over the
+    generating rows k -- and the bound tightens monotonically."""
+    m = cfg0
+    idx = oracle.Index(m)
+    for g in (0, 7, 19):
+        a = oracle.assemble(idx, m.values, g) - (-0.9) * np.eye(idx.sub_dim[g])  # mu inside the occupied band
+        lam, q = np.linalg.eigh(a)
+        gen = []
+        for c in idx.grp_cols[idx.grp_ptr[g]:idx.grp_ptr[g + 1]]:
+            t = int(np.searchsorted(idx.sub_blocks[idx.sub_ptr[g]:idx.sub_ptr[g + 1]], c))
+            o = int(idx.sub_off[idx.sub_ptr[g] + t])
+            gen.extend(range(o, o + int(m.blk_size[c])))
+        w = (q[gen, :] ** 2).sum(0)
+        n_final = (w * 0.5 * (1.0 - np.sign(lam))).sum()
+        x = lam / (np.abs(lam).max() * 1.02)
+        prev = np.inf
+        for k in range(1, 25):
+            x = 0.5 * x * (3.0 - x * x)
+            xm = (q * x) @ q.T
+            y = xm @ xm
+            n_k = (0.5 * (1.0 - np.diag(xm)[gen])).sum()
+            s1 = np.maximum(1.0 - np.diag(y)[gen], 0.0)
+            s2 = ((np.eye(len(lam))[gen] - y[gen]) ** 2).sum(1)
+            bound = (0.5 * np.minimum(s1, 0.5 * (s1 + s2))).sum()
+            assert abs(n_final - n_k) <= bound + 1e-10
+            assert bound <= prev + 1e-10
+            prev = bound
+        assert prev < 1e-2
+
+
+def test_predicted_residual_bound(oracle, cfg0):
+    """DESIGN.md reading A9b: for a symmetric iterate, E_{k+1} = X_{k+1}^2 - I = -3/4 E_k^2 - 1/4 E_k^3 with
+    E_k = X_k^2 - I (Eq.(11) L97 squared), hence ||E_{k+1}||_F <= 3/4 ||E_k||_F^2 + 1/4 ||E_k||_F^3."""
+    m = cfg0
+    idx = oracle.Index(m)
+    a = oracle.assemble(idx, m.values, 3)
+    x = a / (np.abs(np.linalg.eigvalsh(a)).max() * 1.01)
+    eye = np.eye(len(a))
+    for k in range(12):
+        e = x @ x - eye
+        xn = 0.5 * x @ (3.0 * eye - x @ x)
+        en = xn @ xn - eye
+        assert np.abs(en - (-0.75 * e @ e - 0.25 * e @ e @ e)).max() <= 1e-12
+        f = np.linalg.norm(e)
+        assert np.linalg.norm(en) <= 0.75 * f * f + 0.25 * f ** 3 + 1e-13
+        x = xn
