@@ -584,7 +584,7 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
         if (stop) { a.flag[g] = conv ? 0 : 1; a.done_iter[g] = k; }
         else {
             atomicAdd(a.counters + k, 1);
-            // Predicted exit (reading A9): with E_k = X_k^2 - I symmetric, E_{k+1} = -3/4 E_k^2 - 1/4 E_k^3, so
+            // Predicted exit (reading A9): with E_k = X_k^2 - I symmetric, E_{k+1} = -3/4 E_k^2 + 1/4 E_k^3, so
             // ||E_{k+1}||_F <= 3/4 ||E_k||_F^2 + 1/4 ||E_k||_F^3.  If that bound is already a factor 10 below
             // eps, X_{k+1} is accepted without the product that would only confirm it: the submatrix takes part
             // in the update of this iteration (done_iter = k + 1 > k) and in nothing after it.

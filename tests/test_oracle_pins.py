@@ -349,7 +349,7 @@ def test_steering_bound_inequality(oracle, cfg0):
 
 
 def test_predicted_residual_bound(oracle, cfg0):
-    """DESIGN.md reading A9b: for a symmetric iterate, E_{k+1} = X_{k+1}^2 - I = -3/4 E_k^2 - 1/4 E_k^3 with
+    """DESIGN.md reading A9b: for a symmetric iterate, E_{k+1} = X_{k+1}^2 - I = -3/4 E_k^2 + 1/4 E_k^3 with
     E_k = X_k^2 - I (Eq.(11) L97 squared), hence ||E_{k+1}||_F <= 3/4 ||E_k||_F^2 + 1/4 ||E_k||_F^3."""
     m = cfg0
     idx = oracle.Index(m)
@@ -360,7 +360,7 @@ def test_predicted_residual_bound(oracle, cfg0):
         e = x @ x - eye
         xn = 0.5 * x @ (3.0 * eye - x @ x)
         en = xn @ xn - eye
-        assert np.abs(en - (-0.75 * e @ e - 0.25 * e @ e @ e)).max() <= 1e-12
+        assert np.abs(en - (-0.75 * e @ e + 0.25 * e @ e @ e)).max() <= 1e-12
         f = np.linalg.norm(e)
         assert np.linalg.norm(en) <= 0.75 * f * f + 0.25 * f ** 3 + 1e-13
         x = xn
