@@ -359,6 +359,10 @@ def main():
         peak, peak_src = fp64_peak_tflops()
         # dominant kernel: k_ns_gemm<0|1>.  Algorithmic flops of one symmetric n x n product:
         # n(n+1)/2 outputs x 2n flop = n^2 (n+1); per launch = sum over the active submatrices.
+        # gemm_ms = CUDA-event time of the Newton-Schulz phases (event pairs recorded by the library on its
+        # stream around every evaluation's iteration loop): the GEMM launches plus the decision / bound /
+        # control kernels and the empty launches behind a device-side stop (~2 % of it), so `achieved` is a
+        # slight under-estimate of the GEMM kernels' own rate (profiles/: 26.4 TFLOP/s in isolation).
         ach = sym_flop / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
         roofline = {"bound": "tensor", "kernel": "k_ns_gemm (FP64 DMMA Newton-Schulz, both modes)",
                     "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
