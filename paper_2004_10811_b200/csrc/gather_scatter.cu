@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
             if (LIST) {  // the pairs (member, value offset) were listed when the plan first gathered
                 const int64_t e1 = A.gl_ptr[sp + tc + 1];
                 for (int64_t e = A.gl_ptr[sp + tc] + lane; e < e1; e += 32) {
-                    const uint32_t v = __ldg(A.gl + e);
+                    const uint32_t v = __ldcs(A.gl + e);  // read once per gather: do not displace the values in L2
                     row[v >> 16] = (MapT)(v & 0xffffu);
                 }
                 continue;
@@ -158,7 +158,7 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
                         if (p == q) v.x -= A.mu;
                         if (p + 1 == q) v.y -= A.mu;
                         asum += fabs(v.x) + fabs(v.y);
-                        *reinterpret_cast<double2*>(Xg + xo + u * xstep) = v;
+                        __stcs(reinterpret_cast<double2*>(Xg + xo + u * xstep), v);  // streaming: the workspace is far larger than L2
                     }
                 }
             }
