@@ -171,7 +171,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
         return e == cudaErrorMemoryAllocation ? SM_ERR_ALLOC : SM_ERR_CUDA;
     }
     // gather launch shape: member tables + hash table of S_i + position map + block map of a chunk
-    // of mc member columns (all of them when it fits ~72 KB, so that 3 CTAs share an SM)
+    // of mc member columns (as many as fit ~24 KB: measured best, occupancy beats fewer chunks)
     {
         const int msb = (std::max(p->max_sub_blocks, 1) + 1) & ~1;
         const int tile_ld = (p->info.dim_max + LD_ALIGN + 3) & ~3;
@@ -193,7 +193,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
         p->gather_map16 = esz == 2;
         auto bytes = [&](int mc) { return fixed + (((size_t)mc * mpad * esz + 15) & ~(size_t)15); };
         int mc = msb;
-        const size_t want = 44 * 1024, budget = 200 * 1024;
+        const size_t want = 24 * 1024, budget = 200 * 1024;
         if (bytes(mc) > want) mc = (int)std::max<int64_t>(((int64_t)want - (int64_t)fixed) / (mpad * esz), 16);
         mc = std::min(mc, msb);
         while (mc > 1 && bytes(mc) > budget) mc >>= 1;
