@@ -296,7 +296,7 @@ sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, 
 // workspace matrix (k8-panel layout) | "diagonal element" in bit 31.  k_scatter_map_build walks
 // the block columns once (one warp per block column: 32 packed block records at a time, prefix
 // sums of their sizes, shuffle binary search of an element's block); k_scatter is then a plain
-// parallel sweep over the values of a block column, any block size, any number of groups:
+// parallel sweep (one warp per block column and chunk of 1024 values), any block size:
 //     D = 1/2 (delta - xs * X),  xs = 1/s_i if the submatrix stopped at iteration 0 (the buffer
 // then still holds the unscaled a_i - mu I), else 1.
 // ---------------------------------------------------------------------------------------------
@@ -348,15 +348,17 @@ k_scatter_map_build(int nb, const int32_t* __restrict__ blk_size, const int64_t*
     }
 }
 
-constexpr int SCATTER_THREADS = 128, SCATTER_CHUNK = 1024;  // values per CTA (8 per thread)
+constexpr int SCATTER_THREADS = 256, SCATTER_CHUNK = 1024;  // one warp per (block column, chunk of values)
 
 __global__ void __launch_bounds__(SCATTER_THREADS)
-k_scatter(const int64_t* __restrict__ colptr, const int64_t* __restrict__ val_off,
+k_scatter(int nb, const int64_t* __restrict__ colptr, const int64_t* __restrict__ val_off,
           const int32_t* __restrict__ col_grp, const int64_t* __restrict__ ws_off,
           const int32_t* __restrict__ done_iter, const unsigned long long* __restrict__ gersh, int cur_k,
           const uint32_t* __restrict__ src_map, const double* __restrict__ buf0, const double* __restrict__ buf1,
           double* __restrict__ out, int as_identity) {
-    const int c = blockIdx.x;
+    const int c = blockIdx.x * (SCATTER_THREADS >> 5) + (threadIdx.x >> 5);
+    if (c >= nb) return;
+    const int lane = threadIdx.x & 31;
     const int64_t v0 = val_off[colptr[c]], v1 = val_off[colptr[c + 1]];
     const int64_t b = v0 + (int64_t)blockIdx.y * SCATTER_CHUNK;
     if (b >= v1) return;
@@ -371,7 +373,7 @@ k_scatter(const int64_t* __restrict__ colptr, const int64_t* __restrict__ val_of
         xs = s > 0.0 ? 1.0 / s : 1.0;
     }
 #pragma unroll 4
-    for (int64_t e = b + threadIdx.x; e < e1; e += SCATTER_THREADS) {
+    for (int64_t e = b + lane; e < e1; e += 32) {
         const uint32_t m = __ldg(src_map + e);
         const double x = Xg[m & 0x7fffffffu];
         out[e] = as_identity ? x : 0.5 * ((double)(m >> 31) - xs * x);
@@ -395,8 +397,8 @@ sm_status_t launch_scatter(sm_plan* p, int as_identity, const double* buf0, cons
         }
         p->scatter_chunks = (int)std::max<int64_t>(1, (mx + SCATTER_CHUNK - 1) / SCATTER_CHUNK);
     }
-    k_scatter<<<dim3(p->nb, p->scatter_chunks), SCATTER_THREADS, 0, st>>>(
-        p->d_colptr, p->d_val_off, p->d_col_grp, p->d_ws_off, p->d_done_iter, p->d_gersh, p->cur_k, p->d_src_map, buf0,
+    k_scatter<<<dim3((p->nb + 7) / 8, p->scatter_chunks), SCATTER_THREADS, 0, st>>>(
+        p->nb, p->d_colptr, p->d_val_off, p->d_col_grp, p->d_ws_off, p->d_done_iter, p->d_gersh, p->cur_k, p->d_src_map, buf0,
         buf1, out, as_identity);
     p->launches++;
     SM_CUDA(cudaGetLastError());
