@@ -154,7 +154,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_scalars, 8 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_red, 4096 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_bound, (size_t)(p->opt.max_iter + 2) * 16);
-    if (e == cudaSuccess) e = A((void**)&p->d_bound_part, (size_t)ng * 16);
+    if (e == cudaSuccess) e = A((void**)&p->d_bound_part, (size_t)std::max(nb, 1) * 16);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_bound, (size_t)(p->opt.max_iter + 2) * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_ctrl, 64);
     if (e == cudaSuccess) e = cudaMemset(p->d_ctrl, 0, 64);

@@ -96,7 +96,7 @@ struct sm_plan {
     int cur_k = 0;                         // completed Newton-Schulz updates of the last evaluation
     int half_iter = 0;                     // 1: MODE 0 of iteration cur_k ran, its MODE 1 did not (steering stop)
     double* d_bound = nullptr;             // [max_iter+2][2] per iteration: n_elec(X_k), its error bound
-    double* d_bound_part = nullptr;        // [2][ngroups] per-group partials of the two
+    double* d_bound_part = nullptr;        // [2][nb] per-block-column partials of the two
     double* h_bound = nullptr;             // pinned mirror of d_bound
     // --- reduced-precision path (precision = 1, ns_tf32.cu)
     void* d_tiles32 = nullptr;

@@ -475,17 +475,18 @@ sm_status_t launch_nelec(sm_plan* p, const double* buf0, const double* buf1, cud
 //   sum_l Q_kl^2 u_l = 1 - (Y_k)_kk =: S1,   sum_l Q_kl^2 u_l^2 = ((I - Y_k)^2)_kk = sum_j (delta_kj - Y_kj)^2 =: S2,
 // so row k contributes at most 1/2 min(S1, (S1 + S2)/2): half of the first-order bound once the
 // iteration is close to convergence.  The rows of Y_k for the generating functions are read in full.
-// part[g] = n_elec partial of X_k, part[ngroups + g] = bound partial; one warp per group.
-__global__ void k_nelec_bound(int ngroups, const int32_t* __restrict__ grp_ptr, const int32_t* __restrict__ grp_cols,
-                              const int32_t* __restrict__ blk_size, const int32_t* __restrict__ gen_off,
-                              const int32_t* __restrict__ ldv, const int64_t* __restrict__ ws_off,
-                              const int32_t* __restrict__ done_iter, const unsigned long long* __restrict__ gersh,
-                              int k, const double* __restrict__ buf0, const double* __restrict__ buf1,
-                              const double* __restrict__ bufY, double* __restrict__ part,
-                              const int32_t* __restrict__ ctrl) {
-    const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (g >= ngroups || ctrl[0] != 0) return;  // evaluation already stopped: empty launch
+// part[c] = n_elec partial of X_k, part[nb + c] = bound partial of block column c.
+__global__ void k_nelec_bound(int nb, const int32_t* __restrict__ col_grp, const int32_t* __restrict__ blk_size,
+                              const int32_t* __restrict__ gen_off, const int32_t* __restrict__ ldv,
+                              const int64_t* __restrict__ ws_off, const int32_t* __restrict__ done_iter,
+                              const unsigned long long* __restrict__ gersh, int k, const double* __restrict__ buf0,
+                              const double* __restrict__ buf1, const double* __restrict__ bufY,
+                              double* __restrict__ part, const int32_t* __restrict__ ctrl) {
+    // one warp per generating block column c (partials per block column: more warps in flight than one per group)
+    const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (c >= nb || ctrl[0] != 0) return;  // evaluation already stopped: empty launch
     const int lane = threadIdx.x & 31;
+    const int g = col_grp[c];
     const int di = done_iter[g];
     const int kb = (di >= 0 && di <= k) ? di : k;  // di = k + 1: predicted exit, its last update has not run yet
     const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];
@@ -497,45 +498,42 @@ __global__ void k_nelec_bound(int ngroups, const int32_t* __restrict__ grp_ptr, 
         xs = s > 0.0 ? 1.0 / s : 1.0;
     }
     double a = 0.0, d = 0.0;
-    for (int gc = grp_ptr[g]; gc < grp_ptr[g + 1]; ++gc) {
-        const int c = grp_cols[gc];
-        const int o = gen_off[c], b = blk_size[c];
-        for (int e = 0; e < b; ++e) {      // generating function (row) o + e: the lanes sweep its row of Y
-            const int row = o + e;
-            const int t0 = row & ~63;
-            const double* yr = Yg + (size_t)t0 * ld + (size_t)(row & 63) * 8;
-            const size_t pstride = (size_t)min(64, ld - t0) * 8;
-            double s2 = 0.0, ykk = 0.0;
-            for (int j = lane; j < ld; j += 32) {
-                const double y = yr[(size_t)(j >> 3) * pstride + (j & 7)];
-                const double t = (j == row ? 1.0 : 0.0) - y;
-                s2 = fma(t, t, s2);
-                if (j == row) ykk = y;
-            }
+    const int o = gen_off[c], b = blk_size[c];
+    for (int e = 0; e < b; ++e) {      // generating function (row) o + e: the lanes sweep its row of Y
+        const int row = o + e;
+        const int t0 = row & ~63;
+        const double* yr = Yg + (size_t)t0 * ld + (size_t)(row & 63) * 8;
+        const size_t pstride = (size_t)min(64, ld - t0) * 8;
+        double s2 = 0.0, ykk = 0.0;
+        for (int j = lane; j < ld; j += 32) {
+            const double y = yr[(size_t)(j >> 3) * pstride + (j & 7)];
+            const double t = (j == row ? 1.0 : 0.0) - y;
+            s2 = fma(t, t, s2);
+            if (j == row) ykk = y;
+        }
 #pragma unroll
-            for (int w = 16; w > 0; w >>= 1) {
-                s2 += __shfl_xor_sync(0xffffffffu, s2, w);
-                ykk += __shfl_xor_sync(0xffffffffu, ykk, w);
-            }
-            if (lane == 0) {
-                const double s1 = fmax(1.0 - ykk, 0.0);
-                a += 0.5 * (1.0 - xs * Xg[panel_off(row, row, ld)]);
-                d += 0.5 * fmin(s1, 0.5 * (s1 + s2));
-            }
+        for (int w = 16; w > 0; w >>= 1) {
+            s2 += __shfl_xor_sync(0xffffffffu, s2, w);
+            ykk += __shfl_xor_sync(0xffffffffu, ykk, w);
+        }
+        if (lane == 0) {
+            const double s1 = fmax(1.0 - ykk, 0.0);
+            a += 0.5 * (1.0 - xs * Xg[panel_off(row, row, ld)]);
+            d += 0.5 * fmin(s1, 0.5 * (s1 + s2));
         }
     }
-    if (lane == 0) { part[g] = a; part[ngroups + g] = d; }
+    if (lane == 0) { part[c] = a; part[nb + c] = d; }
 }
 
-// Called after the launch pair of iteration k >= 1 (MODE 1 touches neither X_k nor Y_k).
+// Called after MODE 0 + decision of iteration k >= 1 (the update touches neither X_k nor Y_k).
 sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const double* buf1, const double* bufY,
                                cudaStream_t st) {
-    if (p->ngroups == 0) return SM_OK;
-    k_nelec_bound<<<(p->ngroups + 7) / 8, 256, 0, st>>>(p->ngroups, p->d_grp_ptr, p->d_grp_cols, p->d_blk_size,
-                                                        p->d_gen_off, p->d_ld, p->d_ws_off, p->d_done_iter, p->d_gersh,
-                                                        k, buf0, buf1, bufY, p->d_bound_part, p->d_ctrl);
-    k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part, p->ngroups, p->d_bound + 2 * k);
-    k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part + p->ngroups, p->ngroups, p->d_bound + 2 * k + 1);
+    if (p->ngroups == 0 || p->nb == 0) return SM_OK;
+    k_nelec_bound<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_col_grp, p->d_blk_size, p->d_gen_off, p->d_ld, p->d_ws_off,
+                                                   p->d_done_iter, p->d_gersh, k, buf0, buf1, bufY, p->d_bound_part,
+                                                   p->d_ctrl);
+    k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part, p->nb, p->d_bound + 2 * k);
+    k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part + p->nb, p->nb, p->d_bound + 2 * k + 1);
     p->launches += 3;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
