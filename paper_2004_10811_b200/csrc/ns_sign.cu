@@ -40,7 +40,13 @@
 
 namespace smb {
 
-constexpr int BM = TILE, BN = TILE, BK = 16, STAGES = 4;
+#ifndef SM_BK
+#define SM_BK 16
+#endif
+#ifndef SM_STAGES
+#define SM_STAGES 4
+#endif
+constexpr int BM = TILE, BN = TILE, BK = SM_BK, STAGES = SM_STAGES, PPS = BK / 8;  // PPS: k panels per stage
 
 // Kernel modes.  Update modes compute  Out = cb (A B + fold A)  on symmetric operands:
 //   MODE 0   Y  = alpha X X (+ residual partials)                          Eq.(11), Eq.(19)
@@ -265,7 +271,7 @@ template <int MODE, int VAR>
 __device__ __forceinline__ void k_loop_var(double (&acc)[16][2], const double* smem, unsigned full0, unsigned empty0,
                                            int& stage, unsigned& phase, int KP, int ja, int jb, bool b_is_a,
                                            int frag_off, int wid, int lane, int kp_col0, int s_rows) {
-    const int KT = (KP + 1) >> 1;
+    const int KT = (KP + PPS - 1) / PPS;
     const int boff = frag_off + ((VAR <= 8 || VAR == 13) ? wid * 128 : 0);
 #pragma unroll 1
     for (int kt = 0; kt < KT; ++kt) {
@@ -274,14 +280,14 @@ __device__ __forceinline__ void k_loop_var(double (&acc)[16][2], const double* s
             const double* sa = smem + (size_t)stage * STAGE_DOUBLES;
             const double* Ap = sa + frag_off;
             const double* Bp = (b_is_a ? sa : sa + BM * BK) + boff;
-            const int nj = min(2, KP - 2 * kt);
+            const int nj = min(PPS, KP - PPS * kt);
 #pragma unroll 1
             for (int j = 0; j < nj; ++j, Ap += ja, Bp += jb) {
                 if (VAR >= 1 && VAR <= 8) panel_rect<(VAR >= 1 && VAR <= 8) ? VAR : 1>(acc, Ap, Bp);
                 else if (VAR == 13) panel_rect_dyn(acc, Ap, Bp, s_rows);
                 else panel_diag<(VAR >= 9 && VAR <= 12) ? VAR - 9 : 0>(acc, Ap, Bp);
                 if (MODE >= 1) {
-                    const int sc = 2 * kt + j - kp_col0;
+                    const int sc = PPS * kt + j - kp_col0;
                     if ((unsigned)sc < 8u) {
                         if (VAR <= 8 || VAR == 13) fold_rect(acc, Ap, VAR <= 8 ? VAR : s_rows, wid, sc, ModeTraits<MODE>::fold);
                         else fold_diag<(VAR >= 9 && VAR <= 12) ? VAR - 9 : 0>(acc, Ap, sc, ModeTraits<MODE>::fold);
@@ -474,12 +480,12 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
                 const int rows_a = min(BM, ld - row0), rows_b = min(BN, ld - col0);
                 const bool b_is_a = (MODE == 0 || MODE == 2) && (ti == tj);
                 const int KP = ld >> 3;            // 8-wide k panels
-                const int KT = (KP + 1) >> 1;      // stages of two panels
+                const int KT = (KP + PPS - 1) / PPS;  // stages of PPS panels
                 const double* Asrc = Xbase + ws_off + (size_t)row0 * ld;
                 const double* Bsrc = Bbase + ws_off + (size_t)col0 * ld;
                 for (int kt = 0; kt < KT; ++kt) {
                     mbar_wait_backoff(&s_empty[stage], phase ^ 1);
-                    const int nj = min(2, KP - 2 * kt);
+                    const int nj = min(PPS, KP - PPS * kt);
                     if (kt == 0) {
                         TileInfo& ti_ = s_info[stage];
                         ti_.ws_off = ws_off; ti_.grp = g; ti_.ld = ld; ti_.n = t1.x; ti_.tij = tij;
@@ -489,9 +495,9 @@ __global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
                     const unsigned bytes_b = b_is_a ? 0u : (unsigned)(rows_b * 8 * nj) * 8u;
                     mbar_arrive_expect_tx(&s_full[stage], bytes_a + bytes_b);
                     double* sa = smem + (size_t)stage * STAGE_DOUBLES;
-                    bulk_g2s(sa, Asrc + (size_t)(2 * kt) * rows_a * 8, bytes_a, &s_full[stage]);
+                    bulk_g2s(sa, Asrc + (size_t)(PPS * kt) * rows_a * 8, bytes_a, &s_full[stage]);
                     if (!b_is_a)
-                        bulk_g2s(sa + BM * BK, Bsrc + (size_t)(2 * kt) * rows_b * 8, bytes_b, &s_full[stage]);
+                        bulk_g2s(sa + BM * BK, Bsrc + (size_t)(PPS * kt) * rows_b * 8, bytes_b, &s_full[stage]);
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
             }
