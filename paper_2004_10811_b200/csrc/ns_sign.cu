@@ -426,7 +426,10 @@ struct NsArgs {
 };
 
 template <int MODE>
-__global__ void __launch_bounds__(NTHREADS, 3) k_ns_gemm(NsArgs a) {
+#ifndef SM_MINB
+#define SM_MINB 3
+#endif
+__global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
     extern __shared__ __align__(128) double smem[];
     __shared__ __align__(16) TileInfo s_info[STAGES];
     __shared__ __align__(8) uint64_t s_full[STAGES], s_empty[STAGES];
@@ -626,7 +629,7 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     a.counters = p->d_counters; a.n_tiles = (int32_t)p->n_tiles; a.ctrl = p->d_ctrl;
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;
     a.predict = (p->opt.predict != 0 && p->opt.order == 2 && eps >= 1e-13) ? 1 : 0; a.max_iter = p->opt.max_iter;
-    const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * 3);
+    const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * SM_MINB);
     a.sched = p->d_sched + 4 * k;
     if (which & 1) {
         k_ns_gemm<0><<<grid, NTHREADS, NS_SMEM, st>>>(a);
