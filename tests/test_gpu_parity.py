@@ -200,18 +200,18 @@ def _sampled_parity(B, oracle, m, k, mu=0.0):
     return stats
 
 
-def test_config2_sampled_parity(B, oracle):
-    _sampled_parity(B, oracle, W.make_config(2), k=24)
+def test_config2_sampled_parity(B, oracle):  # all 1024 submatrices: the "sample" is the whole config
+    _sampled_parity(B, oracle, W.make_config(2), k=1024)  # every submatrix
 
 
 def test_config3_sampled_parity_full_size(B, oracle):
     """DZVP, n ~ 500: the launch configuration bench.py would time; oracle on sampled groups."""
-    _sampled_parity(B, oracle, W.make_config(3), k=6)
+    _sampled_parity(B, oracle, W.make_config(3), k=64)
 
 
 def test_config4_sampled_parity_full_size(B, oracle):
     """BASELINE config 4 at full size (20736 submatrices) in bench.py's launch configuration."""
-    _sampled_parity(B, oracle, W.make_config(4), k=16)
+    _sampled_parity(B, oracle, W.make_config(4), k=64)
 
 
 def test_config4_density_matrix_as_benchmarked(B, oracle):
