@@ -176,7 +176,7 @@ def run_reference(args, m, rank):
 def run_phases(args, m, B, torch):
     """--phases: CUDA-event timing of the HBM-bound phases (a3 gather + a4 bound, a6 scatter) and of
     one fixed-mu sign evaluation, each against its roofline.  One JSON line."""
-    plan = B.plan_from_matrix(m)
+    plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess))
     info = B.sm_plan_query(plan)
     ws = B.alloc_workspace(plan)
     vin = torch.from_numpy(m.values).cuda()
@@ -248,6 +248,8 @@ def workload_config(args, m):
                 if c["kind"] == "water" else f"{c['batch']} dense n={c['n']} (block-diagonal plan)"),
             "n_basis": int(m.n_basis), "nnzb": int(m.nnzb), "ngroups": int(m.ngroups),
             "n_target": int(m.n_occ), "tol_n": TOL_N, "mu0": MU0, "eps": EPS,
+            "mu_search": "bisection, first interior step from the Lanczos quadrature (A11d)"
+                         if getattr(args, "mu_guess", 1) else "midpoint bisection (A11)",
             "cache": "inputs larger than L2 (dense workspace >> 126 MB)" if args.config in (3, 4, 5)
                      else "L2 flushed between steps", "seed": args.seed}
 
@@ -261,6 +263,9 @@ def main():
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mu-guess", type=int, default=1, choices=[0, 1],
+                    help="1 (library default): first interior step of the mu search from the Lanczos quadrature "
+                         "(DESIGN.md reading A11d); 0: pure midpoint bisection (reading A11)")
     ap.add_argument("--phases", action="store_true",
                     help="time gather / scatter / one sign evaluation separately (phase rooflines) and exit")
     args = ap.parse_args()
@@ -289,7 +294,7 @@ def main():
         if rank == 0:
             run_phases(args, m, B, torch)
         return
-    plan = B.plan_from_matrix(m)
+    plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess))
     info = B.sm_plan_query(plan)
     ws = B.alloc_workspace(plan)
     d_in = torch.from_numpy(m.values).cuda()
@@ -389,7 +394,8 @@ def main():
                            "gather_GBps": gather_bytes * evals / (gather_ms * 1e-3) / 1e9 if gather_ms > 0 else None,
                            "ms_scatter_last": last["ms_scatter"], "mu_trace": last["mu_trace"],
                            "ne_trace": last["ne_trace"], "ne_err_trace": last["ne_err_trace"],
-                           "iter_trace": last["iter_trace"], "spec_lo": last["spec_lo"], "spec_hi": last["spec_hi"]}}
+                           "iter_trace": last["iter_trace"], "spec_lo": last["spec_lo"], "spec_hi": last["spec_hi"],
+                           "bracket": [last["bracket_lo"], last["bracket_hi"]], "mu_guess": last["mu_guess"] if last["mu_guess"] == last["mu_guess"] else None}}
         if not args.no_cpu_baseline:
             cb, _ = cpu_baseline(m)
             line["cpu_baseline"] = cb

@@ -92,7 +92,11 @@ typedef struct {
     int32_t predict;     /* 1: predicted exit (reading A9): a submatrix whose next residual  [1]  */
                          /* is bounded a factor 10 below eps by ||E'|| <= 3/4||E||^2+1/4||E||^3 */
                          /* stops after its update, without the confirming X^2 product       */
-    int32_t reserved[3];
+    int32_t mu_guess;    /* sm_density_matrix, scaling = 1 only: the first interior step of the   [1]  */
+                         /* mu search goes to the estimate the Gauss quadrature of the Lanczos     */
+                         /* run gives for the target filling (reading A11d) if that lies inside    */
+                         /* the bracket; 0 = pure midpoint bisection (reading A11)                 */
+    int32_t reserved[2];
 } sm_options_t;
 
 /* Plan facts (all sizes in elements unless they say bytes). */
@@ -143,6 +147,7 @@ typedef struct {
     double spec_lo, spec_hi;  /* scaling = 1: the widened Lanczos estimate of [lambda_min, lambda_max] */
                               /* of K~ the interlacing bound was taken from (else 0, 0)       */
     double bracket_lo, bracket_hi; /* sm_density_matrix: the initial bisection bracket        */
+    double mu_guess;          /* sm_density_matrix: the quadrature estimate (NaN if not computed) */
 } sm_stats_t;
 
 /*
@@ -206,7 +211,8 @@ sm_status_t sm_sign_execute_host(sm_plan_t* plan, const double* h_vals_in, doubl
  * Rule (reading A11): step 0 evaluates *mu_inout; then midpoint bisection inside the
  * Gershgorin interval of K~ (n_elec = 0 below, = n_basis above; intersected with the interlacing
  * interval of K~'s extreme eigenvalues when scaling = 1; reported in stats->bracket_lo/hi), raising
- * mu if n_elec < n_target.
+ * mu if n_elec < n_target.  With opt.mu_guess (reading A11d) the step after step 0 goes to
+ * stats->mu_guess instead of the midpoint when that lies strictly inside the bracket.
  * Stops when |n_elec - n_target| <= tol_n (SM_OK), or when the bracket is narrower than
  * opt.mu_tol or after opt.max_mu_steps evaluations (SM_WARN_MU_NOT_CONVERGED); returns in
  * *mu_inout the evaluated mu with the smallest |n_elec - n_target| and in d_vals_out D~ at that mu.

@@ -196,12 +196,91 @@ def gershgorin_interval(m) -> tuple[float, float]:
     return float((diag - rad).min()), float((diag + rad).max())
 
 
+def sparse_matrix(m):
+    """The block-sparse K~ as a scipy CSC matrix (block (r, c) stored column-major, bs[c] columns of
+    bs[r] values each)."""
+    import scipy.sparse as sp
+    cols = m.block_cols()
+    voff = m.val_off()
+    boff = m.blk_off()
+    n = int(boff[-1])
+    ri, ci = [], []
+    for b in range(m.nnzb):
+        r, c = int(m.rowidx[b]), int(cols[b])
+        br, bc = int(m.blk_size[r]), int(m.blk_size[c])
+        ri.append(np.tile(np.arange(boff[r], boff[r] + br), bc))
+        ci.append(np.repeat(np.arange(boff[c], boff[c] + bc), br))
+    ri = np.concatenate(ri) if ri else np.zeros(0, dtype=np.int64)
+    ci = np.concatenate(ci) if ci else np.zeros(0, dtype=np.int64)
+    return sp.csc_matrix((np.asarray(m.values[:len(ri)], dtype=np.float64), (ri, ci)), shape=(n, n))
+
+
+def lanczos_quadrature(m, steps: int = 24):
+    """Reading A11d: `steps` steps of the plain Lanczos recurrence on K~ (no
+    re-orthogonalisation) from the counter-based start vector v_i = +-1/sqrt(n) (sign = bit 0 of the
+    integer hash h = i * 2654435761; h ^= h >> 15; h *= 2246822519; h ^= h >> 13 in 32-bit unsigned
+    arithmetic).  Returns the Ritz values theta_j (eigenvalues of the tridiagonal T, ascending) and the
+    Gauss quadrature weights w_j = (first component of T's j-th eigenvector)^2, for which
+    v^T f(K~) v ~ sum_j w_j f(theta_j), exact for polynomials of degree < 2 steps."""
+    A = sparse_matrix(m)
+    n = A.shape[0]
+    v = v_start_of(n)
+    vp = np.zeros(n)
+    al, be = [], []
+    b = 0.0
+    for _ in range(min(steps, n)):
+        w = A @ v
+        a = float(w @ v)
+        w = w - a * v - b * vp
+        b = float(np.sqrt(w @ w))
+        al.append(a)
+        be.append(b)
+        if not b > 1e-300:
+            break
+        vp, v = v, w / b
+    T = np.diag(al) + np.diag(be[:len(al) - 1], 1) + np.diag(be[:len(al) - 1], -1)
+    th, U = np.linalg.eigh(T)
+    return th, U[0] ** 2
+
+
+def v_start_of(n: int) -> np.ndarray:
+    """The start vector of lanczos_quadrature (for the moment pins)."""
+    i = np.arange(n, dtype=np.uint64)
+    h = (i * 2654435761) & 0xFFFFFFFF
+    h ^= h >> 15
+    h = (h * 2246822519) & 0xFFFFFFFF
+    h ^= h >> 13
+    return np.where(h & 1, 1.0, -1.0) / np.sqrt(n)
+
+
+def lanczos_interval(th, margin: float = 0.03):
+    """Reading A8: the extreme Ritz values widened by margin * spread (the interlacing interval)."""
+    spread = float(th[-1] - th[0])
+    return float(th[0]) - margin * spread, float(th[-1]) + margin * spread
+
+
+def mu_guess(th, w, frac: float) -> float:
+    """Reading A11d: cum_j = sum_{l <= j} w_l estimates the fraction of eigenvalues of K~ at or below
+    theta_j.  m = the node (last excluded) whose cum is nearest to the target filling `frac`; among the
+    Ritz intervals (theta_i, theta_i+1), m-2 <= i <= m+2, the widest one is taken for the gap and its
+    midpoint returned."""
+    k = len(th)
+    cum = np.cumsum(w) / np.sum(w)
+    m = int(np.argmin(np.abs(cum[:k - 1] - frac)))
+    best = max(0, m - 2)
+    for i in range(best + 1, min(k - 2, m + 2) + 1):
+        if th[i + 1] - th[i] > th[best + 1] - th[best]:
+            best = i
+    return 0.5 * float(th[best] + th[best + 1])
+
+
 def bisect_mu(idx: Index, lam, w, groups, n_target: float, mu0: float, lo: float, hi: float,
-              tol_n: float, mu_tol: float = 1e-6, max_steps: int = 64):
+              tol_n: float, mu_tol: float = 1e-6, max_steps: int = 64, mu_first: float | None = None):
     """Algorithm 1 (L272-276) with the update rule of reading A11: evaluate mu0, then
     midpoint bisection on g(mu) = n_elec(mu) - n_target inside [lo, hi] (raise mu if g < 0).
     Stops on |g| <= tol_n, bracket width <= mu_tol, or max_steps; returns the evaluated mu with
-    the smallest |g| and the trace [(mu, n_elec), ...]."""
+    the smallest |g| and the trace [(mu, n_elec), ...].  Reading A11d: if mu_first is given and lies
+    strictly inside the bracket after step 0, step 1 evaluates it instead of the midpoint."""
     trace = []
     mu = mu0
     best = None
@@ -220,4 +299,6 @@ def bisect_mu(idx: Index, lam, w, groups, n_target: float, mu0: float, lo: float
         if hi - lo <= mu_tol:
             break
         mu = 0.5 * (lo + hi)
+        if len(trace) == 1 and mu_first is not None and lo < mu_first < hi:
+            mu = mu_first
     return best[0], best[1] + n_target, trace

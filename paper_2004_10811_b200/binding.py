@@ -35,7 +35,7 @@ class sm_options_t(C.Structure):
     _fields_ = [("max_iter", C.c_int32), ("scaling", C.c_int32), ("precision", C.c_int32),
                 ("check_every", C.c_int32), ("max_mu_steps", C.c_int32), ("bisect_iter", C.c_int32),
                 ("mu_tol", C.c_double), ("early_out", C.c_int32), ("order", C.c_int32),
-                ("overshoot", C.c_double), ("predict", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("overshoot", C.c_double), ("predict", C.c_int32), ("mu_guess", C.c_int32), ("reserved", C.c_int32 * 2)]
 
 
 class sm_plan_info_t(C.Structure):
@@ -58,7 +58,7 @@ class sm_stats_t(C.Structure):
                 ("tot_gemm_launches", C.c_int32), ("tot_evaluations", C.c_int32),
                 ("tot_ms_gather", C.c_float), ("tot_ms_sign", C.c_float),
                 ("spec_lo", C.c_double), ("spec_hi", C.c_double), ("bracket_lo", C.c_double),
-                ("bracket_hi", C.c_double)]
+                ("bracket_hi", C.c_double), ("mu_guess", C.c_double)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_ if k not in ("mu_trace", "ne_trace", "ne_err_trace", "iter_trace")}
@@ -72,7 +72,7 @@ class sm_stats_t(C.Structure):
 
 def default_options(**kw) -> sm_options_t:
     o = sm_options_t(max_iter=100, scaling=1, precision=0, check_every=16, max_mu_steps=64, bisect_iter=0,
-                     mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=1)
+                     mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=1, mu_guess=1)
     for k, v in kw.items():
         setattr(o, k, v)
     return o

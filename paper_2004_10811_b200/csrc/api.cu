@@ -27,6 +27,7 @@ static void default_options(sm_options_t* o) {
     o->overshoot = 1.45;
     o->order = 2;
     o->predict = 1;
+    o->mu_guess = 1;
     o->precision = 0;
     o->check_every = 16;
     o->max_mu_steps = 64;
@@ -89,6 +90,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
     if (p->h_pinned_d) cudaFreeHost(p->h_pinned_d);
     if (p->h_bound) cudaFreeHost(p->h_bound);
     if (p->h_ctrl) cudaFreeHost(p->h_ctrl);
+    if (p->h_lz) cudaFreeHost(p->h_lz);
     for (auto& e : p->ev)
         if (e) cudaEventDestroy(e);
     for (auto& e : p->ev_iter)
@@ -159,6 +161,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_ctrl, 64);
     if (e == cudaSuccess) e = cudaMemset(p->d_ctrl, 0, 64);
     if (e == cudaSuccess) e = cudaMallocHost(&p->h_ctrl, 64);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_lz, 66 * 8);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned, (size_t)(p->opt.max_iter + 2) * 4);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned_d, 8 * 8);
     for (auto& ev : p->ev)
@@ -545,6 +548,24 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         hi = std::min(hi, p->lz_hi);
     }
     S->bracket_lo = lo; S->bracket_hi = hi;
+    // reading A11d: the Gauss quadrature of the same Lanczos run estimates the fraction of eigenvalues of
+    // K~ below each Ritz value; the first interior step goes to the middle of the widest Ritz interval
+    // near the target filling instead of the bracket midpoint (a guess only: the bracket logic is unchanged)
+    double guess = NAN;
+    if (p->opt.mu_guess && p->opt.scaling == 1 && p->lz_nodes >= 2 && p->info.n_basis > 0) {
+        const int k = p->lz_nodes;
+        const double* th = p->h_lz + 2;
+        const double* cum = p->h_lz + 34;
+        const double frac = n_target / (double)p->info.n_basis;
+        int m = 0;
+        for (int i = 1; i + 1 < k; ++i)
+            if (std::fabs(cum[i] - frac) < std::fabs(cum[m] - frac)) m = i;
+        int gi = std::max(0, m - 2);
+        for (int i = gi + 1; i <= std::min(k - 2, m + 2); ++i)
+            if (th[i + 1] - th[i] > th[gi + 1] - th[gi]) gi = i;
+        guess = 0.5 * (th[gi] + th[gi + 1]);
+    }
+    S->mu_guess = guess;
     double mu = *mu_inout;
     const int cap = (p->opt.precision == 0 && p->opt.bisect_iter > 0 && p->opt.bisect_iter < p->opt.max_iter)
                         ? p->opt.bisect_iter : p->opt.max_iter + 1;
@@ -593,7 +614,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         if (!partial && std::fabs(g) <= tol_n) { accepted = true; break; }
         if (g < 0) lo = std::max(lo, mu); else hi = std::min(hi, mu);
         if (hi - lo <= p->opt.mu_tol) break;
-        mu = 0.5 * (lo + hi);
+        mu = (steps == 1 && guess > lo && guess < hi) ? guess : 0.5 * (lo + hi);
     }
     // the workspace holds the last evaluated mu; re-evaluate if the best one was an earlier step
     // or if the last evaluation ended before convergence (capped or steering-only)
@@ -609,9 +630,9 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     memcpy(tr_ne, S->ne_trace, sizeof(tr_ne));
     memcpy(tr_err, S->ne_err_trace, sizeof(tr_err));
     memcpy(tr_it, S->iter_trace, sizeof(tr_it));
-    const double br_lo = S->bracket_lo, br_hi = S->bracket_hi;
+    const double br_lo = S->bracket_lo, br_hi = S->bracket_hi, br_guess = S->mu_guess;
     *S = ev;
-    S->bracket_lo = br_lo; S->bracket_hi = br_hi;
+    S->bracket_lo = br_lo; S->bracket_hi = br_hi; S->mu_guess = br_guess;
     memcpy(S->mu_trace, tr_mu, sizeof(tr_mu));
     memcpy(S->ne_trace, tr_ne, sizeof(tr_ne));
     memcpy(S->ne_err_trace, tr_err, sizeof(tr_err));

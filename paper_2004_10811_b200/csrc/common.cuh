@@ -113,6 +113,8 @@ struct sm_plan {
     int scatter_chunks = 1;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
     double lz_lo = 0.0, lz_hi = 0.0;       // estimated [lambda_min, lambda_max] of K~ (widened)
+    double* h_lz = nullptr;                // pinned [66]: lo, hi, Ritz values [32], cumulative quadrature weights [32]
+    int lz_nodes = 0;
     int lz_valid = 0;                      // lz_lo / lz_hi belong to the current call's values
     // --- staging for the *_host entry points
     double *d_stage_in = nullptr, *d_stage_out = nullptr;

@@ -141,11 +141,17 @@ __global__ void k_lz_start(int64_t n, double* __restrict__ v, double* __restrict
     }
 }
 
-// Extreme eigenvalues of the k x k Lanczos tridiagonal T (diag alpha, off-diagonal beta) by
-// bisection on Sturm counts, widened by margin * spread.  One thread; k <= LZ_STEPS.
-__global__ void k_lz_extremes(int k, const double* __restrict__ alpha, const double* __restrict__ beta,
-                              double margin, double* __restrict__ out) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+// Gauss quadrature of the k x k Lanczos tridiagonal T (diag alpha, off-diagonal beta): thread j finds
+// the j-th Ritz value by bisection on Sturm counts and its weight = squared first component of the
+// eigenvector (1 / sum_i p_i(theta)^2 with the normalised Lanczos polynomials p_i).  out[0], out[1]:
+// extreme Ritz values widened by margin * spread (interlacing bound, bisection bracket); out[2 + j]:
+// Ritz values ascending; out[2 + 32 + j]: cumulative weights = the start vector's estimate of the
+// fraction of eigenvalues of K~ below the node (used for the first interior step of the mu search,
+// DESIGN.md reading A11d).  One warp; k <= 32.
+__global__ void k_lz_quadrature(int k, const double* __restrict__ alpha, const double* __restrict__ beta,
+                                double margin, double* __restrict__ out) {
+    __shared__ double th[32], wt[32];
+    const int j = threadIdx.x;
     double glo = 1e300, ghi = -1e300;
     for (int i = 0; i < k; ++i) {
         const double r = (i > 0 ? fabs(beta[i - 1]) : 0.0) + (i + 1 < k ? fabs(beta[i]) : 0.0);
@@ -163,21 +169,39 @@ __global__ void k_lz_extremes(int k, const double* __restrict__ alpha, const dou
         }
         return cnt;
     };
-    double lo = glo, hi = ghi;  // smallest eigenvalue: first x with count_below(x) >= 1
-    for (int it = 0; it < 64; ++it) {
-        const double mid = 0.5 * (lo + hi);
-        if (count_below(mid) >= 1) hi = mid; else lo = mid;
+    if (j < k) {
+        double lo = glo, hi = ghi;  // j-th smallest eigenvalue: first x with count_below(x) >= j + 1
+        for (int it = 0; it < 64; ++it) {
+            const double mid = 0.5 * (lo + hi);
+            if (count_below(mid) >= j + 1) hi = mid; else lo = mid;
+        }
+        const double t = 0.5 * (lo + hi);
+        double pm = 0.0, pc = 1.0, sum = 1.0;  // p_{-1}, p_0
+        for (int i = 0; i + 1 < k; ++i) {
+            const double bi = beta[i];
+            if (!(fabs(bi) > 1e-300)) break;   // breakdown: the rest of T is decoupled
+            const double pn = ((t - alpha[i]) * pc - (i > 0 ? beta[i - 1] * pm : 0.0)) / bi;
+            pm = pc; pc = pn;
+            sum = fma(pn, pn, sum);
+            if (!(sum < 1e280)) break;
+        }
+        th[j] = t;
+        wt[j] = 1.0 / sum;
     }
-    const double emin = lo;
-    lo = glo; hi = ghi;         // largest eigenvalue: first x with count_below(x) >= k
-    for (int it = 0; it < 64; ++it) {
-        const double mid = 0.5 * (lo + hi);
-        if (count_below(mid) >= k) hi = mid; else lo = mid;
+    __syncwarp();
+    if (j == 0) {
+        const double emin = th[0], emax = th[k - 1], spread = emax - emin;
+        out[0] = emin - margin * spread;
+        out[1] = emax + margin * spread;
+        double tot = 0.0;
+        for (int i = 0; i < k; ++i) tot += wt[i];
+        double cum = 0.0;
+        for (int i = 0; i < 32; ++i) {
+            if (i < k) cum += wt[i] / tot;
+            out[2 + i] = i < k ? th[i] : th[k - 1];
+            out[2 + 32 + i] = i < k ? cum : 1.0;
+        }
     }
-    const double emax = hi;
-    const double spread = emax - emin;
-    out[0] = emin - margin * spread;
-    out[1] = emax + margin * spread;
 }
 
 // s_g <- min(Gershgorin_g, cap) / overshoot  (in place, bits of a double as written by k_gather).
@@ -203,12 +227,12 @@ sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStr
 sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st) {
     const int64_t n = p->info.n_basis;
     if (n == 0 || p->nb == 0) { p->lz_lo = p->lz_hi = 0.0; return SM_OK; }
-    if (!p->d_lz) SM_CUDA(cudaMalloc((void**)&p->d_lz, (size_t)(3 * n + 2 * LZ_STEPS + 8 + std::max<int64_t>(p->nb, 1024)) * 8));
+    if (!p->d_lz) SM_CUDA(cudaMalloc((void**)&p->d_lz, (size_t)(3 * n + 2 * LZ_STEPS + 72 + std::max<int64_t>(p->nb, 1024)) * 8));
     double* vb[3] = {p->d_lz, p->d_lz + n, p->d_lz + 2 * n};
     double* alpha = p->d_lz + 3 * n;
     double* beta = alpha + LZ_STEPS;
     double* outp = beta + LZ_STEPS;
-    double* part = outp + 8;
+    double* part = outp + 72;
     const int steps = (int)std::min<int64_t>(LZ_STEPS, n);
     const int ew = (int)std::min<int64_t>((n + 255) / 256, 592);
     const int nred = 296;
@@ -225,13 +249,14 @@ sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t s
         p->launches += 5;
         double* t = vprev; vprev = v; v = t;  // v_{j+1} was written over v_{j-1}
     }
-    k_lz_extremes<<<1, 32, 0, st>>>(steps, alpha, beta, 0.03, outp);
+    k_lz_quadrature<<<1, 32, 0, st>>>(steps, alpha, beta, 0.03, outp);
     p->launches++;
     SM_CUDA(cudaGetLastError());
-    SM_CUDA(cudaMemcpyAsync(p->h_pinned_d + 6, outp, 16, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaMemcpyAsync(p->h_lz, outp, 66 * 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));
-    p->lz_lo = p->h_pinned_d[6];
-    p->lz_hi = p->h_pinned_d[7];
+    p->lz_lo = p->h_lz[0];
+    p->lz_hi = p->h_lz[1];
+    p->lz_nodes = steps;
     return SM_OK;
 }
 

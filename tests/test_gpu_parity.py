@@ -240,8 +240,9 @@ def test_config4_density_matrix_as_benchmarked(B, oracle):
         assert lo <= muk <= hi or k == 0
         if k < n - 1:  # a steering or rejected step: on a proven side of the target
             assert abs(nek - m.n_occ) > errk + 0.5
-            if k >= 1:
-                assert abs(muk - 0.5 * (lo + hi)) <= 1e-12 * max(1.0, abs(muk))  # midpoint of the current bracket
+            if k >= 1:  # midpoint of the current bracket, or (step 1 only, reading A11d) the quadrature guess
+                want = stats.mu_guess if (k == 1 and lo < stats.mu_guess < hi) else 0.5 * (lo + hi)
+                assert abs(muk - want) <= 1e-12 * max(1.0, abs(muk))
             if nek < m.n_occ: lo = max(lo, muk)
             else: hi = min(hi, muk)
     assert stats.ne_err_trace[n - 1] == 0.0 and abs(stats.mu_trace[n - 1] - mu) == 0.0
@@ -375,19 +376,23 @@ def test_structure_errors(B):
 
 # ------------------------------------------------------------------------------ a7 + a8 bisection
 @pytest.mark.parametrize("early_out", [1, 0])
-@pytest.mark.parametrize("scaling", [1, 0])
-def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling):
+@pytest.mark.parametrize("scaling,mu_guess", [(1, 1), (1, 0), (0, 0)])
+def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling, mu_guess):
     """Algorithm 1 / readings A11-A12: same bisection trace as the oracle's (which uses stored
     eigendecompositions), same plateau; D~ parity at the GPU's final mu.  With early_out (A11c) a
     steering step reports the count of its last iterate and a bound: the oracle's converged count
-    must lie inside it, on the same side of the target, and the mu trace must not change."""
+    must lie inside it, on the same side of the target, and the mu trace must not change.  With
+    mu_guess (A11d) step 1 is the oracle's own Lanczos quadrature estimate."""
     torch = _torch()
     m = cfg0
     idx = oracle.Index(m)
     lam, w, ptr, g = oracle.eig_groups(idx, m.values)
     lo, hi = oracle.gershgorin_interval(m)
+    th, wq = oracle.lanczos_quadrature(m, steps=24)
+    guess_o = oracle.mu_guess(th, wq, m.n_occ / m.n_basis) if mu_guess else None
+    llo, lhi = oracle.lanczos_interval(th)
     for mu0, tol_n in ((-1.0, 0.5), (1.2, 0.5)):
-        plan = B.plan_from_matrix(m, B.default_options(early_out=early_out, scaling=scaling))
+        plan = B.plan_from_matrix(m, B.default_options(early_out=early_out, scaling=scaling, mu_guess=mu_guess))
         ws = B.alloc_workspace(plan)
         vin = torch.from_numpy(m.values).cuda()
         vout = torch.empty_like(vin)
@@ -400,12 +405,22 @@ def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling):
         if scaling == 0:
             assert abs(stats.bracket_lo - lo) <= 1e-12 * abs(lo) and abs(stats.bracket_hi - hi) <= 1e-12 * abs(hi)
         assert stats.bracket_lo <= lam.min() and lam.max() <= stats.bracket_hi
-        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0, stats.bracket_lo, stats.bracket_hi, tol_n)
+        if scaling == 1:  # the device's Lanczos run against the oracle's: same interval, same estimate
+            assert abs(stats.bracket_lo - max(lo, llo)) <= 1e-8 and abs(stats.bracket_hi - min(hi, lhi)) <= 1e-8
+        if mu_guess:
+            assert abs(stats.mu_guess - guess_o) <= 1e-8
+        else:
+            assert stats.mu_guess != stats.mu_guess  # NaN: not computed
+        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0, stats.bracket_lo, stats.bracket_hi, tol_n,
+                                               mu_first=guess_o)
         assert st == B.SM_OK
         assert stats.mu_steps == len(trace_o)
+        if mu_guess:
+            assert stats.mu_steps == 2  # the guess lies in the gap of this workload
         n_partial = 0
         for k, (mo, no) in enumerate(trace_o):
-            assert abs(stats.mu_trace[k] - mo) <= 1e-12 * max(1, abs(mo))  # same bracket (Gershgorin) and midpoints
+            # same bracket and midpoints; the guess agrees to the rounding of two Lanczos runs
+            assert abs(stats.mu_trace[k] - mo) <= (1e-8 if mu_guess and k >= 1 else 1e-12 * max(1, abs(mo)))
             err = stats.ne_err_trace[k]
             if err > 0.0:  # steering step: proven side, converged count inside the bound
                 n_partial += 1

@@ -364,3 +364,70 @@ def test_predicted_residual_bound(oracle, cfg0):
         f = np.linalg.norm(e)
         assert np.linalg.norm(en) <= 0.75 * f * f + 0.25 * f ** 3 + 1e-13
         x = xn
+
+
+def test_lanczos_quadrature_is_gauss_quadrature(oracle):
+    """A11d pins: (1) the sparse assembly equals the dense one; (2) with as many steps as rows the Ritz
+    values are the eigenvalues and the weights the squared projections of the start vector (textbook);
+    (3) with k < n steps the rule integrates the moments v^T K^j v exactly for j <= 2k - 1, the weights
+    sum to 1 and the Ritz values lie inside the spectrum."""
+    m = W.random_block_pattern(nb=10, density=0.4, max_bs=3, seed=5)
+    kd = m.to_dense()
+    A = oracle.sparse_matrix(m)
+    assert np.array_equal(A.toarray(), kd)
+    n = kd.shape[0]
+    lam, Q = np.linalg.eigh(kd)
+    v = oracle.v_start_of(n)
+    assert abs(v @ v - 1.0) < 1e-14 and set(np.round(np.abs(v) * np.sqrt(n), 12)) == {1.0}
+    k = 6
+    th, w = oracle.lanczos_quadrature(m, steps=k)
+    assert len(th) == k and abs(w.sum() - 1.0) < 1e-13
+    assert lam[0] - 1e-12 <= th[0] and th[-1] <= lam[-1] + 1e-12
+    scale = max(abs(lam[0]), abs(lam[-1]))
+    for j in range(2 * k):
+        exact = v @ np.linalg.matrix_power(kd / scale, j) @ v
+        assert abs(np.sum(w * (th / scale) ** j) - exact) < 1e-11, j
+    j = 2 * k  # the first moment the k-point rule does NOT reproduce
+    assert abs(np.sum(w * (th / scale) ** j) - v @ np.linalg.matrix_power(kd / scale, j) @ v) > 1e-9
+    small = W.random_block_pattern(nb=3, density=1.0, max_bs=3, seed=2)
+    ks = small.to_dense()
+    ns = ks.shape[0]
+    th, w = oracle.lanczos_quadrature(small, steps=ns)
+    lam, Q = np.linalg.eigh(ks)
+    assert np.allclose(th, lam, atol=1e-10)
+    assert np.allclose(w, (Q.T @ oracle.v_start_of(ns)) ** 2, atol=1e-9)
+    lo, hi = oracle.lanczos_interval(th)
+    assert lo < lam[0] and hi > lam[-1]
+
+
+def test_mu_guess_rule(oracle, cfg0):
+    """A11d: a hand-worked case of the widest-interval rule; on the water-like workload the guess lands
+    inside the HOMO-LUMO gap, and the search with that first step ends on the same plateau in fewer
+    evaluations than the midpoint search; a guess outside the bracket is ignored."""
+    th = np.array([0.0, 1.0, 2.0, 10.0, 11.0])
+    w = np.full(5, 0.2)
+    assert oracle.mu_guess(th, w, 0.6) == 6.0      # cum = .2 .4 .6 .8: m = 2, window 0..3, widest (2, 10)
+    assert oracle.mu_guess(th, w, 0.05) == 6.0     # m = 0, window 0..2 still holds (2, 10)
+    th2 = np.array([0.0, 1.0, 2.0, 2.5, 3.0, 3.5, 12.0])
+    assert oracle.mu_guess(th2, np.full(7, 1 / 7), 0.1) == 0.5  # m = 0, window 0..2: first of the widest
+    m = cfg0
+    kd = m.to_dense()
+    ev = np.linalg.eigvalsh(kd)
+    homo, lumo = ev[m.n_occ - 1], ev[m.n_occ]
+    th, w = oracle.lanczos_quadrature(m, steps=24)
+    guess = oracle.mu_guess(th, w, m.n_occ / kd.shape[0])
+    assert homo < guess < lumo
+    idx = oracle.Index(m)
+    lam, wq, ptr, g = oracle.eig_groups(idx, m.values, np.arange(m.ngroups), nthreads=8)
+    lo, hi = oracle.gershgorin_interval(m)
+    llo, lhi = oracle.lanczos_interval(th)
+    lo, hi = max(lo, llo), min(hi, lhi)
+    mu_a, ne_a, tr_a = oracle.bisect_mu(idx, lam, wq, g, m.n_occ, mu0=-1.0, lo=lo, hi=hi, tol_n=0.5)
+    mu_b, ne_b, tr_b = oracle.bisect_mu(idx, lam, wq, g, m.n_occ, mu0=-1.0, lo=lo, hi=hi, tol_n=0.5,
+                                        mu_first=guess)
+    assert len(tr_b) == 2 and tr_b[1][0] == guess and len(tr_a) >= len(tr_b)
+    assert abs(ne_a - m.n_occ) <= 0.5 and abs(ne_b - m.n_occ) <= 0.5
+    _, _, tr_c = oracle.bisect_mu(idx, lam, wq, g, m.n_occ, mu0=-1.0, lo=lo, hi=hi, tol_n=0.5, mu_first=hi + 1.0)
+    assert tr_c == tr_a
+    _, _, tr_d = oracle.bisect_mu(idx, lam, wq, g, m.n_occ, mu0=-1.0, lo=lo, hi=hi, tol_n=0.5, mu_first=-2.0)
+    assert tr_d == tr_a  # below the evaluated mu0: outside the bracket after step 0
