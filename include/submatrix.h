@@ -96,7 +96,11 @@ typedef struct {
                          /* mu search goes to the estimate the Gauss quadrature of the Lanczos     */
                          /* run gives for the target filling (reading A11d) if that lies inside    */
                          /* the bracket; 0 = pure midpoint bisection (reading A11)                 */
-    int32_t reserved[2];
+    int32_t rescale;     /* scaling = 1, order = 2, precision = 0 only (reading A8b): every          [1]  */
+                         /* iteration applies Eq.(11) to al_k X_k, al_k = sqrt(3/(1 + l_k + l_k^2)), */
+                         /* l_k the tracked lower bound of the eigenvalue moduli (l_0 from the Ritz  */
+                         /* values of the Lanczos run), al_k = 1 once l_k >= 0.9; replaces overshoot */
+    int32_t reserved[1];
 } sm_options_t;
 
 /* Plan facts (all sizes in elements unless they say bytes). */

@@ -3,6 +3,7 @@
 // plan.cu / gather_scatter.cu / ns_sign.cu; the host only sequences launches and compares scalars.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -28,6 +29,7 @@ static void default_options(sm_options_t* o) {
     o->order = 2;
     o->predict = 1;
     o->mu_guess = 1;
+    o->rescale = 1;
     o->precision = 0;
     o->check_every = 16;
     o->max_mu_steps = 64;
@@ -83,7 +85,8 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
                     p->d_partials, p->d_counters, p->d_sched, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
-                    p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_ctrl, p->d_gl_ptr, p->d_gl};
+                    p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_ctrl, p->d_gl_ptr, p->d_gl,
+                    p->d_alpha, p->d_lmin};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     if (p->h_pinned) cudaFreeHost(p->h_pinned);
@@ -149,6 +152,8 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_flag, (size_t)ng * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_res, (size_t)ng * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_gersh, (size_t)ng * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_alpha, (size_t)ng * 16);
+    if (e == cudaSuccess) e = A((void**)&p->d_lmin, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_partials, (size_t)p->n_tiles * 4 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_counters, (size_t)(p->opt.max_iter + 2) * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_sched, (size_t)(p->opt.max_iter + 2) * 16);
@@ -386,9 +391,21 @@ sm_status_t ensure_bounds(sm_plan* p, const double* d_in, cudaStream_t st) {
     return SM_OK;
 }
 sm_status_t apply_scaling(sm_plan* p, double mu, cudaStream_t st) {
+    p->resc_eval = 0;
     if (p->opt.scaling != 1) return SM_OK;
     const double cap = std::max(std::fabs(p->lz_hi - mu), std::fabs(p->lz_lo - mu));
-    return launch_apply_scale(p, cap, p->opt.overshoot, st);
+    // reading A8b: distance from mu to the nearest Ritz value of the Lanczos run = estimate of the smallest
+    // eigenvalue modulus of K~ - mu I (Ritz values sit inside the bands, so it errs on the large side)
+    // Only where mu sits in a hole of the Ritz spectrum (l_0 >= 0.05): inside a band the evaluation is most
+    // likely a steering one, and there the rescaling, which folds the top of the spectrum down onto l_k,
+    // loosens the bound of reading A11c (measured: 4 instead of 2 iterations until the side is proven).
+    double ell = 0.0;
+    if (p->opt.rescale != 0 && p->opt.order == 2 && p->opt.precision == 0 && p->lz_nodes > 0 && cap > 0.0) {
+        ell = INFINITY;
+        for (int j = 0; j < p->lz_nodes; ++j) ell = std::min(ell, std::fabs(p->h_lz[2 + j] - mu));
+        p->resc_eval = (ell >= 0.05 * cap) ? 1 : 0;
+    }
+    return launch_apply_scale(p, cap, p->opt.overshoot, ell, st);
 }
 
 // One sign evaluation at fixed mu: gather -> NS loop (up to iter_cap iterations) -> n_elec.

@@ -113,6 +113,9 @@ struct sm_plan {
     int scatter_chunks = 1;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
     double lz_lo = 0.0, lz_hi = 0.0;       // estimated [lambda_min, lambda_max] of K~ (widened)
+    double* d_alpha = nullptr;             // [2][ngroups] rescaling factor alpha_k of iteration k (slot k & 1), reading A8b
+    int resc_eval = 0;                     // this evaluation runs the rescaled iteration (A8b)
+    double* d_lmin = nullptr;              // [ngroups] tracked lower bound l_k of the schedule
     double* h_lz = nullptr;                // pinned [66]: lo, hi, Ritz values [32], cumulative quadrature weights [32]
     int lz_nodes = 0;
     int lz_valid = 0;                      // lz_lo / lz_hi belong to the current call's values
@@ -161,7 +164,8 @@ struct EvalCtrl {
 sm_status_t launch_eval_ctrl(sm_plan* p, int k, int steer, double n_target, double margin, cudaStream_t st);
 // spectral.cu
 sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st);
-sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStream_t st);
+sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, double ell_abs, cudaStream_t st);
+inline bool rescale_on(const sm_plan* p) { return p->resc_eval != 0; }  // set per evaluation by apply_scaling
 // ns_sign.cu
 sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
                            double* bufY, cudaStream_t st, int which = 3, double* bufW = nullptr);

@@ -481,7 +481,8 @@ __global__ void k_nelec_bound(int nb, const int32_t* __restrict__ col_grp, const
                               const int64_t* __restrict__ ws_off, const int32_t* __restrict__ done_iter,
                               const unsigned long long* __restrict__ gersh, int k, const double* __restrict__ buf0,
                               const double* __restrict__ buf1, const double* __restrict__ bufY,
-                              double* __restrict__ part, const int32_t* __restrict__ ctrl) {
+                              double* __restrict__ part, const int32_t* __restrict__ ctrl,
+                              const double* __restrict__ alpha, int ngroups) {
     // one warp per generating block column c (partials per block column: more warps in flight than one per group)
     const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (c >= nb || ctrl[0] != 0) return;  // evaluation already stopped: empty launch
@@ -497,6 +498,8 @@ __global__ void k_nelec_bound(int nb, const int32_t* __restrict__ col_grp, const
         const double s = __longlong_as_double((long long)gersh[g]);
         xs = s > 0.0 ? 1.0 / s : 1.0;
     }
+    double rinv = 1.0;  // reading A8b: the stored Y is al^2 X^2
+    if (alpha) { const double al = alpha[(size_t)(kb & 1) * ngroups + g]; rinv = 1.0 / (al * al); }
     double a = 0.0, d = 0.0;
     const int o = gen_off[c], b = blk_size[c];
     for (int e = 0; e < b; ++e) {      // generating function (row) o + e: the lanes sweep its row of Y
@@ -506,7 +509,7 @@ __global__ void k_nelec_bound(int nb, const int32_t* __restrict__ col_grp, const
         const size_t pstride = (size_t)min(64, ld - t0) * 8;
         double s2 = 0.0, ykk = 0.0;
         for (int j = lane; j < ld; j += 32) {
-            const double y = yr[(size_t)(j >> 3) * pstride + (j & 7)];
+            const double y = yr[(size_t)(j >> 3) * pstride + (j & 7)] * rinv;
             const double t = (j == row ? 1.0 : 0.0) - y;
             s2 = fma(t, t, s2);
             if (j == row) ykk = y;
@@ -531,7 +534,7 @@ sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const doub
     if (p->ngroups == 0 || p->nb == 0) return SM_OK;
     k_nelec_bound<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_col_grp, p->d_blk_size, p->d_gen_off, p->d_ld, p->d_ws_off,
                                                    p->d_done_iter, p->d_gersh, k, buf0, buf1, bufY, p->d_bound_part,
-                                                   p->d_ctrl);
+                                                   p->d_ctrl, rescale_on(p) ? p->d_alpha : nullptr, p->ngroups);
     k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part, p->nb, p->d_bound + 2 * k);
     k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part + p->nb, p->nb, p->d_bound + 2 * k + 1);
     p->launches += 3;

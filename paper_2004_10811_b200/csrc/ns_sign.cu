@@ -308,6 +308,7 @@ __device__ __forceinline__ void k_loop_var(double (&acc)[16][2], const double* s
 struct EpiCtx {
     double* Out;
     double scale;  // MODE 0: alpha; MODE 1: b (acc = X Y - 3 X -> X' = b acc)
+    double rinv;   // MODE 0 with rescaling (A8b): stored Y = al^2 X^2, the residual is taken of Y * rinv = X^2
     int base_d, base_m, pd, pm;
     int rlim;      // n - row0 - lr: rows sr*8 < rlim count for the residual (n x n part only)
 };
@@ -319,7 +320,10 @@ __device__ __forceinline__ void store_below(const EpiCtx& c, const double (&a)[2
     double* pm_ = c.Out + (c.base_m + sr * c.pm + sc * 64);
     pm_[0] = v0;
     pm_[8] = v1;
-    if (MODE == 0 && sr * 8 < c.rlim) part = fma(2.0 * v0, v0, fma(2.0 * v1, v1, part));
+    if (MODE == 0 && sr * 8 < c.rlim) {
+        const double w0 = v0 * c.rinv, w1 = v1 * c.rinv;
+        part = fma(2.0 * w0, w0, fma(2.0 * w1, w1, part));
+    }
 }
 // sub-tile on the matrix diagonal (sr == sc of a diagonal tile): lower triangle only
 template <int MODE>
@@ -335,7 +339,7 @@ __device__ __forceinline__ void store_ondiag(const EpiCtx& c, const double (&a)[
         pd_[q] = v;
         if (cq != lr) pm_[q * 8] = v;
         if (MODE == 0 && sr * 8 < c.rlim) {
-            const double d = v - (cq == lr ? 1.0 : 0.0);
+            const double d = v * c.rinv - (cq == lr ? 1.0 : 0.0);
             part = fma((cq == lr ? 1.0 : 2.0) * d, d, part);
         }
     }
@@ -345,6 +349,7 @@ struct TileGeo {
     int64_t ws_off;
     double* out;
     const unsigned long long* gersh;
+    const double* alpha;  // null, or the rescaling factors of this iteration (one per submatrix)
     int ld, n, row0, col0, grp, k;
 };
 
@@ -368,6 +373,12 @@ __device__ __forceinline__ void tile_var(double (&acc)[16][2], const double* sme
         double sg = __longlong_as_double((long long)t.gersh[t.grp]);
         if (!(sg > 0.0)) sg = 1.0;
         c.scale = (MODE == 0) ? 1.0 / (sg * sg) : ModeTraits<MODE>::cb / sg;
+    }
+    c.rinv = 1.0;
+    if ((MODE == 0 || MODE == 1) && t.alpha) {  // reading A8b: this iteration works on al X_k
+        const double al = t.alpha[t.grp];
+        if (MODE == 0) { c.scale *= al * al; c.rinv = 1.0 / (al * al); }
+        else c.scale *= al;
     }
     c.Out = t.out + t.ws_off;
     c.pd = min(BM, t.ld - t.row0) * 8;
@@ -416,6 +427,8 @@ struct NsArgs {
     int32_t* counters;   // [max_iter+2] still-active submatrices after iteration k
     int32_t* sched;      // work counter of this launch
     const int32_t* ctrl; // [0] != 0: the evaluation has been stopped on the device (k_eval_ctrl): do nothing
+    double* alpha;       // null, or [2][ngroups] rescaling factors (slot k & 1 = iteration k), reading A8b
+    double* lmin;        // [ngroups] lower bound l_k the schedule tracks
     int32_t n_tiles;
     int32_t ngroups;
     int32_t k;
@@ -542,6 +555,7 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
         const int ld = si.ld;
         TileGeo c;
         c.ws_off = si.ws_off; c.out = (MODE == 0) ? a.bufY : (MODE == 2 ? a.bufW : ((k & 1) ? a.buf0 : a.buf1)); c.gersh = a.gersh;
+        c.alpha = a.alpha ? a.alpha + (size_t)(k & 1) * a.ngroups : nullptr;
         c.ld = ld; c.n = si.n; c.row0 = row0; c.col0 = col0; c.grp = si.grp; c.k = k;
         double part = 0.0;
         {
@@ -590,6 +604,20 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
         const bool stag = (k > 0) && (r >= prev) && (r < 1e-6);
         const bool stop = conv || stag || a.decide_only || !(r == r);
         a.res[(size_t)(k & 1) * a.ngroups + g] = r;
+        bool unscaled = true;
+        if (a.alpha && !stop) {
+            // Reading A8b: iteration k maps the eigenvalue moduli [l_k, 1] of X_k onto [l_{k+1}, 1] with
+            // l_{k+1} = f(l_k) = f(1), f(x) = 1/2 al x (3 - al^2 x^2); al_{k+1} = sqrt(3 / (1 + l + l^2)) is the
+            // factor that equalises both ends again; exactly 1 once l >= 0.9 (plain Eq.(11) from there on).
+            // l is an estimate: eigenvalues below it just converge later, the stop test is the residual.
+            const double al = a.alpha[(size_t)(k & 1) * a.ngroups + g], l = a.lmin[g];
+            unscaled = (al == 1.0);
+            const double fl = 0.5 * al * l * (3.0 - al * al * l * l), f1 = 0.5 * al * (3.0 - al * al);
+            const double ln = fmin(fmin(fl, f1), 1.0);  // f peaks (= 1) at x = 1/al inside [l, 1]: the ends bound it
+            a.lmin[g] = ln;
+            // al <= 1.7 keeps al |x| < sqrt(3) (no sign change) with |x| <= 1 + rounding
+            a.alpha[(size_t)((k + 1) & 1) * a.ngroups + g] = ln < 0.9 ? fmin(sqrt(3.0 / (1.0 + ln + ln * ln)), 1.7) : 1.0;
+        }
         if (stop) { a.flag[g] = conv ? 0 : 1; a.done_iter[g] = k; }
         else {
             atomicAdd(a.counters + k, 1);
@@ -597,7 +625,7 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
             // ||E_{k+1}||_F <= 3/4 ||E_k||_F^2 + 1/4 ||E_k||_F^3.  If that bound is already a factor 10 below
             // eps, X_{k+1} is accepted without the product that would only confirm it: the submatrix takes part
             // in the update of this iteration (done_iter = k + 1 > k) and in nothing after it.
-            if (a.predict && k + 1 < a.max_iter) {
+            if (a.predict && unscaled && k + 1 < a.max_iter) {
                 const double sn = sqrt((double)(n > 0 ? n : 1)), f = r * sn;
                 const double next = (0.75 * f * f + 0.25 * f * f * f) / sn;
                 if (next < 0.1 * a.eps) {
@@ -628,6 +656,8 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     a.done_iter = p->d_done_iter; a.flag = p->d_flag; a.res = p->d_res;
     a.counters = p->d_counters; a.n_tiles = (int32_t)p->n_tiles; a.ctrl = p->d_ctrl;
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;
+    const bool resc = rescale_on(p);
+    a.alpha = resc ? p->d_alpha : nullptr; a.lmin = resc ? p->d_lmin : nullptr;
     a.predict = (p->opt.predict != 0 && p->opt.order == 2 && eps >= 1e-13) ? 1 : 0; a.max_iter = p->opt.max_iter;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * SM_MINB);
     a.sched = p->d_sched + 4 * k;

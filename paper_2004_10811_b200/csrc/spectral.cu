@@ -205,18 +205,31 @@ __global__ void k_lz_quadrature(int k, const double* __restrict__ alpha, const d
 }
 
 // s_g <- min(Gershgorin_g, cap) / overshoot  (in place, bits of a double as written by k_gather).
-__global__ void k_apply_scale(int ng, unsigned long long* __restrict__ gersh, double cap, double inv_overshoot) {
+// With alpha != null (reading A8b) the overshoot is not applied; instead iteration 0 works on al_0 X_0 with
+// al_0 = min(sqrt(3 / (1 + l + l^2)), 1.5), l = ell_abs / s_g the estimated smallest eigenvalue modulus of X_0
+// (1.5: the same safety against an underestimated bound as the overshoot limit of reading A8).
+__global__ void k_apply_scale(int ng, unsigned long long* __restrict__ gersh, double cap, double inv_overshoot,
+                              double ell_abs, double* __restrict__ alpha, double* __restrict__ lmin) {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ng) return;
     double s = __longlong_as_double((long long)gersh[g]);
     if (cap > 0.0 && cap < s) s = cap;
-    s *= inv_overshoot;
+    if (alpha) {
+        double l = s > 0.0 ? ell_abs / s : 1.0;
+        l = fmin(fmax(l, 1e-4), 1.0);
+        alpha[g] = l < 0.9 ? fmin(sqrt(3.0 / (1.0 + l + l * l)), 1.5) : 1.0;
+        lmin[g] = l;
+    } else {
+        s *= inv_overshoot;
+    }
     gersh[g] = (unsigned long long)__double_as_longlong(s);
 }
 
-sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, cudaStream_t st) {
+sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, double ell_abs, cudaStream_t st) {
     if (p->ngroups == 0) return SM_OK;
-    k_apply_scale<<<(p->ngroups + 255) / 256, 256, 0, st>>>(p->ngroups, p->d_gersh, cap, 1.0 / overshoot);
+    const bool resc = rescale_on(p);
+    k_apply_scale<<<(p->ngroups + 255) / 256, 256, 0, st>>>(p->ngroups, p->d_gersh, cap, 1.0 / overshoot, ell_abs,
+                                                            resc ? p->d_alpha : nullptr, resc ? p->d_lmin : nullptr);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;

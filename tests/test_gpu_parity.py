@@ -460,7 +460,7 @@ def test_scaling_modes_agree(B, oracle, cfg0, scaling):
     d_or = oracle.density(idx, m.values, 0.1)
     its = {}
     for ov in (1.0, 1.25, 1.5):
-        plan, st, d, stats, ws, vin = _run_sign(B, m, mu=0.1, opt=B.default_options(scaling=scaling, overshoot=ov))
+        plan, st, d, stats, ws, vin = _run_sign(B, m, mu=0.1, opt=B.default_options(scaling=scaling, overshoot=ov, rescale=0))
         assert st == B.SM_OK
         assert np.abs(d - d_or).max() <= TOL_D
         its[ov] = stats.iter_max
@@ -471,6 +471,24 @@ def test_scaling_modes_agree(B, oracle, cfg0, scaling):
     test_scaling_modes_agree.its[scaling] = its
     if scaling == 1 and 0 in test_scaling_modes_agree.its:
         assert its[1.25] < test_scaling_modes_agree.its[0][1.0]
+
+
+@pytest.mark.parametrize("mu", [0.0, -0.9, 0.6])
+def test_rescaled_iteration_a8b(B, oracle, cfg0, mu):
+    """Reading A8b: Eq.(11) applied to al_k X_k with the tracked lower bound l_k (l_0 from the Ritz values)
+    gives the oracle's D~ at a gap mu and at in-band mus (where l_0 overestimates: the residual test
+    decides, not the schedule), with no more products than the overshoot scaling of reading A8."""
+    m = cfg0
+    idx = oracle.Index(m)
+    d_or = oracle.density(idx, m.values, mu)
+    work = {}
+    for rs in (0, 1):
+        plan, st, d, stats, ws, vin = _run_sign(B, m, mu=mu, opt=B.default_options(rescale=rs))
+        assert st == B.SM_OK and stats.not_converged == 0 and stats.max_residual < EPS
+        assert np.abs(d - d_or).max() <= TOL_D
+        work[rs] = stats.sum_iter_n3
+        B.sm_plan_destroy(plan)
+    assert work[1] <= work[0]
 
 
 def test_density_matrix_unreachable_tolerance_is_guarded(B, cfg0):

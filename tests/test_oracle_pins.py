@@ -431,3 +431,32 @@ def test_mu_guess_rule(oracle, cfg0):
     assert tr_c == tr_a
     _, _, tr_d = oracle.bisect_mu(idx, lam, wq, g, m.n_occ, mu0=-1.0, lo=lo, hi=hi, tol_n=0.5, mu_first=-2.0)
     assert tr_d == tr_a  # below the evaluated mu0: outside the bracket after step 0
+
+
+def test_rescaled_newton_schulz_scalar_properties():
+    """Reading A8b, the properties the schedule relies on, checked numerically on the scalar map
+    f(x) = 1/2 al x (3 - al^2 x^2): with al = sqrt(3 / (1 + l + l^2)) both ends of [l, 1] map to the same
+    value, the image of [l, 1] is [f(l), 1], signs are kept for al <= 1.7 and |x| <= 1, and the iteration
+    count to |1 - x| < 1e-13 over [l0, 1] is smaller than that of the plain map."""
+    xs = np.linspace(0.0, 1.0, 20001)
+    for l in (1e-4, 0.01, 0.08, 0.3, 0.7, 0.89):
+        al = np.sqrt(3.0 / (1.0 + l + l * l))
+        f = lambda x: 0.5 * al * x * (3.0 - al * al * x * x)
+        assert abs(f(l) - f(1.0)) < 1e-14
+        img = f(xs[xs >= l])
+        assert img.min() >= f(l) - 1e-14 and img.max() <= 1.0 + 1e-14 and img.max() > 1.0 - 1e-6
+        assert f(l) > 0.5 * l * (3.0 - l * l)  # the lower end moves faster than under the plain map
+    for al in (1.5, 1.7):
+        assert np.all(0.5 * al * xs[1:] * (3.0 - al * al * xs[1:] ** 2) > 0.0)
+    def count(l0, rescale):
+        x = np.linspace(l0, 1.0, 4001)
+        l = l0
+        for k in range(200):
+            if np.abs(1.0 - x).max() < 1e-13:
+                return k
+            al = min(np.sqrt(3.0 / (1.0 + l + l * l)), 1.5 if k == 0 else 1.7) if (rescale and l < 0.9) else 1.0
+            g = lambda t: 0.5 * al * t * (3.0 - al * al * t * t)
+            x, l = g(x), min(g(l), g(1.0), 1.0)
+        return 200
+    for l0 in (0.01, 0.08, 0.2):
+        assert count(l0, True) < count(l0, False)
