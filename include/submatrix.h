@@ -99,7 +99,7 @@ typedef struct {
     int32_t rescale;     /* scaling = 1, order = 2, precision = 0 only (reading A8b): every          [1]  */
                          /* iteration applies Eq.(11) to al_k X_k, al_k = sqrt(3/(1 + l_k + l_k^2)), */
                          /* l_k the tracked lower bound of the eigenvalue moduli (l_0 from the Ritz  */
-                         /* values of the Lanczos run), al_k = 1 once l_k >= 0.9; replaces overshoot */
+                         /* values of the Lanczos run), al_k = 1 once l_k >= 0.9999; replaces overshoot */
     int32_t reserved[1];
 } sm_options_t;
 

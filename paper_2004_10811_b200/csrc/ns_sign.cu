@@ -608,7 +608,8 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
         if (a.alpha && !stop) {
             // Reading A8b: iteration k maps the eigenvalue moduli [l_k, 1] of X_k onto [l_{k+1}, 1] with
             // l_{k+1} = f(l_k) = f(1), f(x) = 1/2 al x (3 - al^2 x^2); al_{k+1} = sqrt(3 / (1 + l + l^2)) is the
-            // factor that equalises both ends again; exactly 1 once l >= 0.9 (plain Eq.(11) from there on).
+            // factor that equalises both ends again; exactly 1 once l >= 0.9999 (plain Eq.(11) from there on,
+            // which the predicted exit needs for the last two iterations).
             // l is an estimate: eigenvalues below it just converge later, the stop test is the residual.
             const double al = a.alpha[(size_t)(k & 1) * a.ngroups + g], l = a.lmin[g];
             unscaled = (al == 1.0);
@@ -616,7 +617,7 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
             const double ln = fmin(fmin(fl, f1), 1.0);  // f peaks (= 1) at x = 1/al inside [l, 1]: the ends bound it
             a.lmin[g] = ln;
             // al <= 1.7 keeps al |x| < sqrt(3) (no sign change) with |x| <= 1 + rounding
-            a.alpha[(size_t)((k + 1) & 1) * a.ngroups + g] = ln < 0.9 ? fmin(sqrt(3.0 / (1.0 + ln + ln * ln)), 1.7) : 1.0;
+            a.alpha[(size_t)((k + 1) & 1) * a.ngroups + g] = ln < 0.9999 ? fmin(sqrt(3.0 / (1.0 + ln + ln * ln)), 1.7) : 1.0;
         }
         if (stop) { a.flag[g] = conv ? 0 : 1; a.done_iter[g] = k; }
         else {

@@ -217,7 +217,7 @@ __global__ void k_apply_scale(int ng, unsigned long long* __restrict__ gersh, do
     if (alpha) {
         double l = s > 0.0 ? ell_abs / s : 1.0;
         l = fmin(fmax(l, 1e-4), 1.0);
-        alpha[g] = l < 0.9 ? fmin(sqrt(3.0 / (1.0 + l + l * l)), 1.5) : 1.0;
+        alpha[g] = l < 0.9999 ? fmin(sqrt(3.0 / (1.0 + l + l * l)), 1.5) : 1.0;
         lmin[g] = l;
     } else {
         s *= inv_overshoot;

@@ -454,7 +454,7 @@ def test_rescaled_newton_schulz_scalar_properties():
         for k in range(200):
             if np.abs(1.0 - x).max() < 1e-13:
                 return k
-            al = min(np.sqrt(3.0 / (1.0 + l + l * l)), 1.5 if k == 0 else 1.7) if (rescale and l < 0.9) else 1.0
+            al = min(np.sqrt(3.0 / (1.0 + l + l * l)), 1.5 if k == 0 else 1.7) if (rescale and l < 0.9999) else 1.0
             g = lambda t: 0.5 * al * t * (3.0 - al * al * t * t)
             x, l = g(x), min(g(l), g(1.0), 1.0)
         return 200
