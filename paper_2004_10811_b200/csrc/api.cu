@@ -85,7 +85,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
                     p->d_partials, p->d_counters, p->d_sched, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
-                    p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_ctrl, p->d_gl_ptr, p->d_gl,
+                    p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_col_rec, p->d_ctrl, p->d_gl_ptr, p->d_gl,
                     p->d_alpha, p->d_lmin};
     for (void* q : ptrs)
         if (q) cudaFree(q);

@@ -110,6 +110,7 @@ struct sm_plan {
     uint32_t* d_gl = nullptr;              //   entries: member index << 16 | value offset inside the block column
     int gather_no_list = 0;
     uint32_t* d_src_map = nullptr;         // [nnz] scatter source map (built by the first scatter)
+    int4* d_col_rec = nullptr;             // [nb] scatter column records (first value lo/hi, value count, group)
     int scatter_chunks = 1;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
     double lz_lo = 0.0, lz_hi = 0.0;       // estimated [lambda_min, lambda_max] of K~ (widened)

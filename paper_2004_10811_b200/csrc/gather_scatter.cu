@@ -304,13 +304,17 @@ __global__ void __launch_bounds__(256)
 k_scatter_map_build(int nb, const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
                     const int64_t* __restrict__ val_off, const int32_t* __restrict__ col_grp,
                     const int32_t* __restrict__ gen_off, const uint32_t* __restrict__ blk_pack,
-                    const int32_t* __restrict__ ldv, uint32_t* __restrict__ src_map) {
+                    const int32_t* __restrict__ ldv, uint32_t* __restrict__ src_map, int4* __restrict__ col_rec) {
     const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (c >= nb) return;
     const int lane = threadIdx.x & 31;
     const int g = col_grp[c];
     const int bc = blk_size[c];
     const int64_t p0 = colptr[c];
+    if (lane == 0) {  // column record of k_scatter: first value, value count, group -- one 16-byte load
+        const int64_t v0 = val_off[p0];
+        col_rec[c] = make_int4((int)(v0 & 0xffffffffll), (int)(v0 >> 32), (int)(val_off[colptr[c + 1]] - v0), g);
+    }
     const int nblk = (int)(colptr[c + 1] - p0);
     const int ld = ldv[g];
     const int go = gen_off[c];
@@ -349,21 +353,28 @@ k_scatter_map_build(int nb, const int32_t* __restrict__ blk_size, const int64_t*
 }
 
 constexpr int SCATTER_THREADS = 256, SCATTER_CHUNK = 1024;  // one warp per (block column, chunk of values)
+constexpr int SCATTER_U = 12;  // values per lane in flight (384 per warp: a typical SZV block column in one pass)
 
 __global__ void __launch_bounds__(SCATTER_THREADS)
-k_scatter(int nb, const int64_t* __restrict__ colptr, const int64_t* __restrict__ val_off,
-          const int32_t* __restrict__ col_grp, const int64_t* __restrict__ ws_off,
+k_scatter(int nb, const int4* __restrict__ col_rec, const int64_t* __restrict__ ws_off,
           const int32_t* __restrict__ done_iter, const unsigned long long* __restrict__ gersh, int cur_k,
           const uint32_t* __restrict__ src_map, const double* __restrict__ buf0, const double* __restrict__ buf1,
           double* __restrict__ out, int as_identity) {
     const int c = blockIdx.x * (SCATTER_THREADS >> 5) + (threadIdx.x >> 5);
     if (c >= nb) return;
     const int lane = threadIdx.x & 31;
-    const int64_t v0 = val_off[colptr[c]], v1 = val_off[colptr[c + 1]];
-    const int64_t b = v0 + (int64_t)blockIdx.y * SCATTER_CHUNK;
-    if (b >= v1) return;
-    const int64_t e1 = min(v1, b + SCATTER_CHUNK);
-    const int g = col_grp[c];
+    const int4 rec = __ldg(col_rec + c);
+    const int nv = rec.z - (int)blockIdx.y * SCATTER_CHUNK;  // values of this chunk
+    if (nv <= 0) return;
+    const int cnt = min(nv, SCATTER_CHUNK);
+    const int64_t b = (((int64_t)rec.y << 32) | (int64_t)(uint32_t)rec.x) + (int64_t)blockIdx.y * SCATTER_CHUNK;
+    const uint32_t* sm = src_map + b;
+    double* o = out + b;
+    const int g = rec.w;
+    // the source-map entries of the first pass do not depend on the group: in flight with its scalars
+    uint32_t m[SCATTER_U];
+#pragma unroll
+    for (int u = 0; u < SCATTER_U; ++u) m[u] = (lane + 32 * u < cnt) ? __ldcs(sm + lane + 32 * u) : 0u;
     const int di = done_iter[g];
     const int kb = di >= 0 ? di : cur_k;
     const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];
@@ -372,11 +383,18 @@ k_scatter(int nb, const int64_t* __restrict__ colptr, const int64_t* __restrict_
         const double s = __longlong_as_double((long long)gersh[g]);
         xs = s > 0.0 ? 1.0 / s : 1.0;
     }
-#pragma unroll 4
-    for (int64_t e = b + lane; e < e1; e += 32) {
-        const uint32_t m = __ldg(src_map + e);
-        const double x = Xg[m & 0x7fffffffu];
-        out[e] = as_identity ? x : 0.5 * ((double)(m >> 31) - xs * x);
+    for (int e0 = 0;;) {
+        double x[SCATTER_U];
+#pragma unroll
+        for (int u = 0; u < SCATTER_U; ++u) x[u] = (e0 + lane + 32 * u < cnt) ? __ldcs(Xg + (m[u] & 0x7fffffffu)) : 0.0;
+#pragma unroll
+        for (int u = 0; u < SCATTER_U; ++u)
+            if (e0 + lane + 32 * u < cnt)
+                __stcs(o + e0 + lane + 32 * u, as_identity ? x[u] : 0.5 * ((double)(m[u] >> 31) - xs * x[u]));
+        e0 += 32 * SCATTER_U;
+        if (e0 >= cnt) break;
+#pragma unroll
+        for (int u = 0; u < SCATTER_U; ++u) m[u] = (e0 + lane + 32 * u < cnt) ? __ldcs(sm + e0 + lane + 32 * u) : 0u;
     }
 }
 
@@ -385,9 +403,10 @@ sm_status_t launch_scatter(sm_plan* p, int as_identity, const double* buf0, cons
     if (p->nb == 0 || p->nnz == 0) return SM_OK;
     if (!p->d_src_map) {  // once per plan (pattern only)
         SM_CUDA(cudaMalloc((void**)&p->d_src_map, (size_t)p->nnz * 4));
+        SM_CUDA(cudaMalloc((void**)&p->d_col_rec, (size_t)p->nb * 16));
         k_scatter_map_build<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_blk_size, p->d_colptr, p->d_val_off,
                                                              p->d_col_grp, p->d_gen_off, p->d_blk_pack, p->d_ld,
-                                                             p->d_src_map);
+                                                             p->d_src_map, p->d_col_rec);
         p->launches++;
         int64_t mx = 0;
         for (int c = 0; c < p->nb; ++c) {
@@ -398,8 +417,7 @@ sm_status_t launch_scatter(sm_plan* p, int as_identity, const double* buf0, cons
         p->scatter_chunks = (int)std::max<int64_t>(1, (mx + SCATTER_CHUNK - 1) / SCATTER_CHUNK);
     }
     k_scatter<<<dim3((p->nb + 7) / 8, p->scatter_chunks), SCATTER_THREADS, 0, st>>>(
-        p->nb, p->d_colptr, p->d_val_off, p->d_col_grp, p->d_ws_off, p->d_done_iter, p->d_gersh, p->cur_k, p->d_src_map, buf0,
-        buf1, out, as_identity);
+        p->nb, p->d_col_rec, p->d_ws_off, p->d_done_iter, p->d_gersh, p->cur_k, p->d_src_map, buf0, buf1, out, as_identity);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
