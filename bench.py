@@ -176,7 +176,7 @@ def run_reference(args, m, rank):
 def run_phases(args, m, B, torch):
     """--phases: CUDA-event timing of the HBM-bound phases (a3 gather + a4 bound, a6 scatter) and of
     one fixed-mu sign evaluation, each against its roofline.  One JSON line."""
-    plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess))
+    plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess, mu_start=args.mu_start))
     info = B.sm_plan_query(plan)
     ws = B.alloc_workspace(plan)
     vin = torch.from_numpy(m.values).cuda()
@@ -248,8 +248,10 @@ def workload_config(args, m):
                 if c["kind"] == "water" else f"{c['batch']} dense n={c['n']} (block-diagonal plan)"),
             "n_basis": int(m.n_basis), "nnzb": int(m.nnzb), "ngroups": int(m.ngroups),
             "n_target": int(m.n_occ), "tol_n": TOL_N, "mu0": MU0, "eps": EPS,
-            "mu_search": "bisection, first interior step from the Lanczos quadrature (A11d)"
-                         if getattr(args, "mu_guess", 1) else "midpoint bisection (A11)",
+            "mu_search": ("bisection started at the Lanczos quadrature estimate (A11d, A11e: mu0 lies outside the "
+                          "Ritz interval taken for the gap)" if getattr(args, "mu_start", 1) else
+                          "bisection from mu0, first interior step from the Lanczos quadrature (A11d)")
+                         if getattr(args, "mu_guess", 1) else "midpoint bisection from mu0 (A11)",
             "cache": "inputs larger than L2 (dense workspace >> 126 MB)" if args.config in (3, 4, 5)
                      else "L2 flushed between steps", "seed": args.seed}
 
@@ -266,6 +268,9 @@ def main():
     ap.add_argument("--mu-guess", type=int, default=1, choices=[0, 1],
                     help="1 (library default): first interior step of the mu search from the Lanczos quadrature "
                          "(DESIGN.md reading A11d); 0: pure midpoint bisection (reading A11)")
+    ap.add_argument("--mu-start", type=int, default=1, dest="mu_start",
+                    help="1 (library default): step 0 of the mu search evaluates the quadrature estimate when mu0 lies "
+                         "outside the Ritz interval taken for the gap (reading A11e); 0: step 0 always evaluates mu0")
     ap.add_argument("--phases", action="store_true",
                     help="time gather / scatter / one sign evaluation separately (phase rooflines) and exit")
     args = ap.parse_args()
@@ -294,7 +299,7 @@ def main():
         if rank == 0:
             run_phases(args, m, B, torch)
         return
-    plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess))
+    plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess, mu_start=args.mu_start))
     info = B.sm_plan_query(plan)
     ws = B.alloc_workspace(plan)
     d_in = torch.from_numpy(m.values).cuda()

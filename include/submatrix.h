@@ -100,7 +100,11 @@ typedef struct {
                          /* iteration applies Eq.(11) to al_k X_k, al_k = sqrt(3/(1 + l_k + l_k^2)), */
                          /* l_k the tracked lower bound of the eigenvalue moduli (l_0 from the Ritz  */
                          /* values of the Lanczos run), al_k = 1 once l_k >= 0.9999; replaces overshoot */
-    int32_t reserved[1];
+    int32_t mu_start;    /* sm_density_matrix with mu_guess (reading A11e): 1 = step 0 evaluates the      [1]  */
+                         /* quadrature estimate instead of *mu_inout when *mu_inout lies outside the    */
+                         /* Ritz interval the estimate is the middle of (a caller's mu inside it, e.g.  */
+                         /* the previous SCF step's, is evaluated first); 0 = step 0 always evaluates   */
+                         /* *mu_inout (reading A11)                                                      */
 } sm_options_t;
 
 /* Plan facts (all sizes in elements unless they say bytes). */
@@ -216,7 +220,9 @@ sm_status_t sm_sign_execute_host(sm_plan_t* plan, const double* h_vals_in, doubl
  * Gershgorin interval of K~ (n_elec = 0 below, = n_basis above; intersected with the interlacing
  * interval of K~'s extreme eigenvalues when scaling = 1; reported in stats->bracket_lo/hi), raising
  * mu if n_elec < n_target.  With opt.mu_guess (reading A11d) the step after step 0 goes to
- * stats->mu_guess instead of the midpoint when that lies strictly inside the bracket.
+ * stats->mu_guess instead of the midpoint when that lies strictly inside the bracket; with
+ * opt.mu_start (reading A11e) step 0 itself goes there unless *mu_inout lies inside the Ritz
+ * interval the estimate was taken from.
  * Stops when |n_elec - n_target| <= tol_n (SM_OK), or when the bracket is narrower than
  * opt.mu_tol or after opt.max_mu_steps evaluations (SM_WARN_MU_NOT_CONVERGED); returns in
  * *mu_inout the evaluated mu with the smallest |n_elec - n_target| and in d_vals_out D~ at that mu.

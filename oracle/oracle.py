@@ -259,11 +259,10 @@ def lanczos_interval(th, margin: float = 0.03):
     return float(th[0]) - margin * spread, float(th[-1]) + margin * spread
 
 
-def mu_guess(th, w, frac: float) -> float:
+def mu_guess_interval(th, w, frac: float):
     """Reading A11d: cum_j = sum_{l <= j} w_l estimates the fraction of eigenvalues of K~ at or below
     theta_j.  m = the node (last excluded) whose cum is nearest to the target filling `frac`; among the
-    Ritz intervals (theta_i, theta_i+1), m-2 <= i <= m+2, the widest one is taken for the gap and its
-    midpoint returned."""
+    Ritz intervals (theta_i, theta_i+1), m-2 <= i <= m+2, the widest one is taken for the gap."""
     k = len(th)
     cum = np.cumsum(w) / np.sum(w)
     m = int(np.argmin(np.abs(cum[:k - 1] - frac)))
@@ -271,7 +270,24 @@ def mu_guess(th, w, frac: float) -> float:
     for i in range(best + 1, min(k - 2, m + 2) + 1):
         if th[i + 1] - th[i] > th[best + 1] - th[best]:
             best = i
-    return 0.5 * float(th[best] + th[best + 1])
+    return float(th[best]), float(th[best + 1])
+
+
+def mu_guess(th, w, frac: float) -> float:
+    """Reading A11d: the midpoint of the Ritz interval taken for the gap."""
+    a, b = mu_guess_interval(th, w, frac)
+    return 0.5 * (a + b)
+
+
+def mu_start(th, w, frac: float, mu0: float, lo: float, hi: float) -> float:
+    """Reading A11e: the mu of step 0.  The caller's mu0 if it lies strictly inside the Ritz interval taken
+    for the gap (it is then as good as the estimate), or if the estimate is not strictly inside the
+    bracket [lo, hi]; otherwise the estimate of reading A11d."""
+    a, b = mu_guess_interval(th, w, frac)
+    guess = 0.5 * (a + b)
+    if lo < guess < hi and not (a < mu0 < b):
+        return guess
+    return mu0
 
 
 def bisect_mu(idx: Index, lam, w, groups, n_target: float, mu0: float, lo: float, hi: float,

@@ -35,7 +35,7 @@ class sm_options_t(C.Structure):
     _fields_ = [("max_iter", C.c_int32), ("scaling", C.c_int32), ("precision", C.c_int32),
                 ("check_every", C.c_int32), ("max_mu_steps", C.c_int32), ("bisect_iter", C.c_int32),
                 ("mu_tol", C.c_double), ("early_out", C.c_int32), ("order", C.c_int32),
-                ("overshoot", C.c_double), ("predict", C.c_int32), ("mu_guess", C.c_int32), ("rescale", C.c_int32), ("reserved", C.c_int32 * 1)]
+                ("overshoot", C.c_double), ("predict", C.c_int32), ("mu_guess", C.c_int32), ("rescale", C.c_int32), ("mu_start", C.c_int32)]
 
 
 class sm_plan_info_t(C.Structure):
@@ -72,7 +72,7 @@ class sm_stats_t(C.Structure):
 
 def default_options(**kw) -> sm_options_t:
     o = sm_options_t(max_iter=100, scaling=1, precision=0, check_every=16, max_mu_steps=64, bisect_iter=0,
-                     mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=1, mu_guess=1, rescale=1)
+                     mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=1, mu_guess=1, rescale=1, mu_start=1)
     for k, v in kw.items():
         setattr(o, k, v)
     return o

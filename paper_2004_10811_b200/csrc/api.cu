@@ -29,6 +29,7 @@ static void default_options(sm_options_t* o) {
     o->order = 2;
     o->predict = 1;
     o->mu_guess = 1;
+    o->mu_start = 1;
     o->rescale = 1;
     o->precision = 0;
     o->check_every = 16;
@@ -568,7 +569,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     // reading A11d: the Gauss quadrature of the same Lanczos run estimates the fraction of eigenvalues of
     // K~ below each Ritz value; the first interior step goes to the middle of the widest Ritz interval
     // near the target filling instead of the bracket midpoint (a guess only: the bracket logic is unchanged)
-    double guess = NAN;
+    double guess = NAN, guess_a = NAN, guess_b = NAN;  // the estimate and the Ritz interval it is the middle of
     if (p->opt.mu_guess && p->opt.scaling == 1 && p->lz_nodes >= 2 && p->info.n_basis > 0) {
         const int k = p->lz_nodes;
         const double* th = p->h_lz + 2;
@@ -581,9 +582,15 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         for (int i = gi + 1; i <= std::min(k - 2, m + 2); ++i)
             if (th[i + 1] - th[i] > th[gi + 1] - th[gi]) gi = i;
         guess = 0.5 * (th[gi] + th[gi + 1]);
+        guess_a = th[gi]; guess_b = th[gi + 1];
     }
     S->mu_guess = guess;
     double mu = *mu_inout;
+    // reading A11e: a caller's mu outside the Ritz interval the quadrature takes for the gap is not worth an
+    // evaluation of its own -- step 0 goes to the estimate (the bracket alone keeps the search correct: every
+    // accepted mu is verified by a converged evaluation); a caller's mu inside that interval (e.g. the mu of
+    // the previous SCF step) is as good as the estimate and is evaluated first, as in reading A11
+    if (p->opt.mu_start && guess > lo && guess < hi && !(mu > guess_a && mu < guess_b)) mu = guess;
     const int cap = (p->opt.precision == 0 && p->opt.bisect_iter > 0 && p->opt.bisect_iter < p->opt.max_iter)
                         ? p->opt.bisect_iter : p->opt.max_iter + 1;
     double best_mu = mu, best_g = INFINITY;

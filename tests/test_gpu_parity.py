@@ -376,13 +376,14 @@ def test_structure_errors(B):
 
 # ------------------------------------------------------------------------------ a7 + a8 bisection
 @pytest.mark.parametrize("early_out", [1, 0])
-@pytest.mark.parametrize("scaling,mu_guess", [(1, 1), (1, 0), (0, 0)])
-def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling, mu_guess):
+@pytest.mark.parametrize("scaling,mu_guess,mu_start", [(1, 1, 1), (1, 1, 0), (1, 0, 1), (0, 0, 1)])
+def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling, mu_guess, mu_start):
     """Algorithm 1 / readings A11-A12: same bisection trace as the oracle's (which uses stored
     eigendecompositions), same plateau; D~ parity at the GPU's final mu.  With early_out (A11c) a
     steering step reports the count of its last iterate and a bound: the oracle's converged count
     must lie inside it, on the same side of the target, and the mu trace must not change.  With
-    mu_guess (A11d) step 1 is the oracle's own Lanczos quadrature estimate."""
+    mu_guess (A11d) step 1 is the oracle's own Lanczos quadrature estimate; with mu_start (A11e) step 0
+    already is, because both start values lie outside the Ritz interval taken for the gap."""
     torch = _torch()
     m = cfg0
     idx = oracle.Index(m)
@@ -392,7 +393,8 @@ def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling, m
     guess_o = oracle.mu_guess(th, wq, m.n_occ / m.n_basis) if mu_guess else None
     llo, lhi = oracle.lanczos_interval(th)
     for mu0, tol_n in ((-1.0, 0.5), (1.2, 0.5)):
-        plan = B.plan_from_matrix(m, B.default_options(early_out=early_out, scaling=scaling, mu_guess=mu_guess))
+        plan = B.plan_from_matrix(m, B.default_options(early_out=early_out, scaling=scaling, mu_guess=mu_guess,
+                                                       mu_start=mu_start))
         ws = B.alloc_workspace(plan)
         vin = torch.from_numpy(m.values).cuda()
         vout = torch.empty_like(vin)
@@ -411,16 +413,21 @@ def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling, m
             assert abs(stats.mu_guess - guess_o) <= 1e-8
         else:
             assert stats.mu_guess != stats.mu_guess  # NaN: not computed
-        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu0, stats.bracket_lo, stats.bracket_hi, tol_n,
-                                               mu_first=guess_o)
+        start_o = mu0
+        if mu_guess and mu_start:  # A11e: the oracle's own rule, in the bracket the library reports
+            start_o = oracle.mu_start(th, wq, m.n_occ / m.n_basis, mu0, stats.bracket_lo, stats.bracket_hi)
+            assert start_o == guess_o
+        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, start_o, stats.bracket_lo, stats.bracket_hi,
+                                               tol_n, mu_first=guess_o)
         assert st == B.SM_OK
         assert stats.mu_steps == len(trace_o)
         if mu_guess:
-            assert stats.mu_steps == 2  # the guess lies in the gap of this workload
+            assert stats.mu_steps == (1 if mu_start else 2)  # the guess lies in the gap of this workload
         n_partial = 0
         for k, (mo, no) in enumerate(trace_o):
             # same bracket and midpoints; the guess agrees to the rounding of two Lanczos runs
-            assert abs(stats.mu_trace[k] - mo) <= (1e-8 if mu_guess and k >= 1 else 1e-12 * max(1, abs(mo)))
+            from_guess = mu_guess and (k >= 1 or mu_start)
+            assert abs(stats.mu_trace[k] - mo) <= (1e-8 if from_guess else 1e-12 * max(1, abs(mo)))
             err = stats.ne_err_trace[k]
             if err > 0.0:  # steering step: proven side, converged count inside the bound
                 n_partial += 1
@@ -430,12 +437,30 @@ def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling, m
                 assert (stats.ne_trace[k] > m.n_occ) == (no > m.n_occ)
             else:
                 assert abs(stats.ne_trace[k] - no) <= 1e-9
-        if early_out:
+        if early_out and stats.mu_steps > 1:
             assert n_partial >= 1 and stats.ne_err_trace[stats.mu_steps - 1] == 0.0
             assert stats.iter_trace[0] < stats.iter_trace[stats.mu_steps - 1]  # mu0 inside a band: decided early
+        if stats.mu_steps == 1:
+            assert n_partial == 0
         assert abs(stats.n_elec - ne_o) <= 1e-9  # same plateau
         d_or = oracle.density(idx, m.values, mu)
         assert np.abs(vout.cpu().numpy() - d_or).max() <= TOL_D
+        B.sm_plan_destroy(plan)
+    if mu_guess and mu_start:  # A11e: a caller's mu inside the Ritz interval taken for the gap is evaluated first
+        a, b = oracle.mu_guess_interval(th, wq, m.n_occ / m.n_basis)
+        mu_in = 0.25 * a + 0.75 * b
+        plan = B.plan_from_matrix(m, B.default_options(early_out=early_out, scaling=scaling))
+        ws = B.alloc_workspace(plan)
+        vin = torch.from_numpy(m.values).cuda()
+        vout = torch.empty_like(vin)
+        stats = B.sm_stats_t()
+        st, mu = B.sm_density_matrix(plan, vin, float(m.n_occ), 0.5, EPS, mu_in, vout, ws, stats)
+        torch.cuda.synchronize()
+        assert stats.mu_trace[0] == mu_in
+        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu_in, stats.bracket_lo, stats.bracket_hi, 0.5,
+                                               mu_first=guess_o)
+        assert st == B.SM_OK and stats.mu_steps == len(trace_o) and abs(stats.n_elec - ne_o) <= 1e-9
+        assert np.abs(vout.cpu().numpy() - oracle.density(idx, m.values, mu)).max() <= TOL_D
         B.sm_plan_destroy(plan)
 
 
@@ -535,7 +560,7 @@ def test_third_order_iteration_eq19(B, oracle, cfg0):
     idx = oracle.Index(m)
     d_or = oracle.density(idx, m.values, 0.0)
     plan2, st2, d2, stats2, _, _ = _run_sign(B, m, opt=B.default_options(order=2, overshoot=1.0))
-    plan3, st3, d3, stats3, ws, vin = _run_sign(B, m, opt=B.default_options(order=3))
+    plan3, st3, d3, stats3, ws, vin = _run_sign(B, m, opt=B.default_options(order=3, mu_start=0))
     assert st2 == B.SM_OK and st3 == B.SM_OK
     assert np.abs(d3 - d_or).max() <= TOL_D
     assert stats3.iter_max < stats2.iter_max

@@ -400,6 +400,40 @@ def test_lanczos_quadrature_is_gauss_quadrature(oracle):
     assert lo < lam[0] and hi > lam[-1]
 
 
+def test_mu_start_rule(oracle, cfg0):
+    """A11e: hand-worked cases of the step-0 rule (the caller's mu is kept only inside the Ritz interval taken for
+    the gap, the estimate must lie strictly inside the bracket); on the water-like workload a start from mu0 = -1
+    goes straight to the estimate and the search ends after ONE evaluation on the plateau of the target, the same
+    plateau the search of reading A11 (which spends an evaluation on mu0) ends on."""
+    th = np.array([0.0, 1.0, 2.0, 10.0, 11.0])
+    w = np.full(5, 0.2)
+    assert oracle.mu_guess_interval(th, w, 0.6) == (2.0, 10.0)
+    assert oracle.mu_start(th, w, 0.6, mu0=-1.0, lo=-3.0, hi=12.0) == 6.0   # mu0 outside (2, 10): the estimate
+    assert oracle.mu_start(th, w, 0.6, mu0=10.5, lo=-3.0, hi=12.0) == 6.0
+    assert oracle.mu_start(th, w, 0.6, mu0=2.0, lo=-3.0, hi=12.0) == 6.0    # the interval is open
+    assert oracle.mu_start(th, w, 0.6, mu0=3.0, lo=-3.0, hi=12.0) == 3.0    # inside: the caller knows better
+    assert oracle.mu_start(th, w, 0.6, mu0=9.9, lo=-3.0, hi=12.0) == 9.9
+    assert oracle.mu_start(th, w, 0.6, mu0=-1.0, lo=-3.0, hi=6.0) == -1.0   # estimate not strictly inside the bracket
+    assert oracle.mu_start(th, w, 0.6, mu0=-1.0, lo=6.0, hi=12.0) == -1.0
+    m = cfg0
+    th, w = oracle.lanczos_quadrature(m, steps=24)
+    frac = m.n_occ / m.n_basis
+    idx = oracle.Index(m)
+    lam, wq, ptr, g = oracle.eig_groups(idx, m.values, np.arange(m.ngroups), nthreads=8)
+    lo, hi = oracle.gershgorin_interval(m)
+    llo, lhi = oracle.lanczos_interval(th)
+    lo, hi = max(lo, llo), min(hi, lhi)
+    guess = oracle.mu_guess(th, w, frac)
+    start = oracle.mu_start(th, w, frac, -1.0, lo, hi)
+    assert start == guess
+    mu_e, ne_e, tr_e = oracle.bisect_mu(idx, lam, wq, g, m.n_occ, mu0=start, lo=lo, hi=hi, tol_n=0.5, mu_first=guess)
+    mu_d, ne_d, tr_d = oracle.bisect_mu(idx, lam, wq, g, m.n_occ, mu0=-1.0, lo=lo, hi=hi, tol_n=0.5, mu_first=guess)
+    assert len(tr_e) == 1 and len(tr_d) == 2 and mu_e == mu_d and ne_e == ne_d
+    a, b = oracle.mu_guess_interval(th, w, frac)
+    inside = 0.25 * a + 0.75 * b
+    assert oracle.mu_start(th, w, frac, inside, lo, hi) == inside
+
+
 def test_mu_guess_rule(oracle, cfg0):
     """A11d: a hand-worked case of the widest-interval rule; on the water-like workload the guess lands
     inside the HOMO-LUMO gap, and the search with that first step ends on the same plateau in fewer
