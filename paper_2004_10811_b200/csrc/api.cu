@@ -86,12 +86,13 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
                     p->d_partials, p->d_counters, p->d_sched, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
-                    p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_col_rec, p->d_ctrl, p->d_gl_ptr, p->d_gl,
+                    p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_col_rec, p->d_gg, p->d_ctrl, p->d_gl_ptr, p->d_gl,
                     p->d_alpha, p->d_lmin};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     if (p->h_pinned) cudaFreeHost(p->h_pinned);
     if (p->h_pinned_d) cudaFreeHost(p->h_pinned_d);
+    if (p->h_stats) cudaFreeHost(p->h_stats);
     if (p->h_bound) cudaFreeHost(p->h_bound);
     if (p->h_ctrl) cudaFreeHost(p->h_ctrl);
     if (p->h_lz) cudaFreeHost(p->h_lz);
@@ -342,12 +343,14 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
 
 sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStream_t st) {
     const int ng = p->ngroups;
-    std::vector<int32_t> di(ng), fl(ng);
-    std::vector<double> res((size_t)2 * ng);
+    if (!p->h_stats) SM_CUDA(cudaMallocHost((void**)&p->h_stats, (size_t)std::max(ng, 1) * 24));
+    const double* res = reinterpret_cast<const double*>(p->h_stats);                       // [2 ng]
+    const int32_t* di = reinterpret_cast<const int32_t*>(p->h_stats + (size_t)ng * 16);   // [ng]
+    const int32_t* fl = di + ng;                                                           // [ng]
     if (ng) {
-        SM_CUDA(cudaMemcpyAsync(di.data(), p->d_done_iter, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
-        SM_CUDA(cudaMemcpyAsync(fl.data(), p->d_flag, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
-        SM_CUDA(cudaMemcpyAsync(res.data(), p->d_res, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
+        SM_CUDA(cudaMemcpyAsync((void*)di, p->d_done_iter, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
+        SM_CUDA(cudaMemcpyAsync((void*)fl, p->d_flag, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
+        SM_CUDA(cudaMemcpyAsync((void*)res, p->d_res, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
     }
     SM_CUDA(cudaMemcpyAsync(p->h_pinned_d, p->d_scalars, 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));
@@ -556,12 +559,12 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     // bracket (n_elec = 0 below, n_basis above): the Gershgorin interval of the whole K~, intersected with
     // the interlacing interval [lambda_min, lambda_max](K~) of the Lanczos run when scaling = 1 has it
     // (every submatrix eigenvalue lies inside both, reading A11)
-    if ((s = launch_gersh_global(p, d_vals_in, st))) return s;
-    SM_CUDA(cudaMemcpy(p->h_pinned_d + 4, p->d_scalars + 4, 16, cudaMemcpyDeviceToHost));
-    double lo = p->h_pinned_d[4], hi = p->h_pinned_d[5];
+    if ((s = launch_gersh_global(p, d_vals_in, st))) return s;  // result read after the next synchronisation
     p->lz_valid = 0;  // one Lanczos run serves every mu of this call
+    if (p->opt.scaling == 1 && (s = ensure_bounds(p, d_vals_in, st))) return s;  // ends with a synchronisation
+    SM_CUDA(cudaStreamSynchronize(st));  // no-op after the Lanczos run
+    double lo = p->h_pinned_d[4], hi = p->h_pinned_d[5];
     if (p->opt.scaling == 1) {
-        if ((s = ensure_bounds(p, d_vals_in, st))) return s;
         lo = std::max(lo, p->lz_lo);
         hi = std::min(hi, p->lz_hi);
     }

@@ -93,6 +93,8 @@ struct sm_plan {
     double* d_red = nullptr;               // [2*4096] reduction scratch
     int32_t* h_pinned = nullptr;           // pinned host mirror for counters
     double* h_pinned_d = nullptr;          // pinned host scalars
+    double* d_gg = nullptr;                // [2 nb] per-column Gershgorin ends of k_gersh_global (allocated on first use)
+    unsigned char* h_stats = nullptr;      // pinned mirror of done_iter / flag / res for collect_stats (first use)
     int cur_k = 0;                         // completed Newton-Schulz updates of the last evaluation
     int half_iter = 0;                     // 1: MODE 0 of iteration cur_k ran, its MODE 1 did not (steering stop)
     double* d_bound = nullptr;             // [max_iter+2][2] per iteration: n_elec(X_k), its error bound

@@ -688,18 +688,17 @@ __global__ void k_minmax_fixed(const double* __restrict__ lo, const double* __re
     if (threadIdx.x == 0) { out[0] = s0[0]; out[1] = s1[0]; }
 }
 
+// Enqueues the Gershgorin interval of the whole K~ into d_scalars[4..5] and its copy into h_pinned_d[4..5];
+// the caller synchronises the stream before reading them (no allocation, no synchronisation here).
 sm_status_t launch_gersh_global(sm_plan* p, const double* vals, cudaStream_t st) {
-    double *lo = nullptr, *hi = nullptr;
-    SM_CUDA(cudaMalloc((void**)&lo, (size_t)p->nb * 8));
-    SM_CUDA(cudaMalloc((void**)&hi, (size_t)p->nb * 8));
+    if (!p->d_gg) SM_CUDA(cudaMalloc((void**)&p->d_gg, (size_t)std::max(p->nb, 1) * 16));
+    double *lo = p->d_gg, *hi = p->d_gg + p->nb;
     k_gersh_global<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_val_off,
                                                     vals, lo, hi);
     k_minmax_fixed<<<1, 1024, 0, st>>>(lo, hi, p->nb, p->d_scalars + 4);
     p->launches += 2;
     SM_CUDA(cudaGetLastError());
-    SM_CUDA(cudaStreamSynchronize(st));
-    cudaFree(lo);
-    cudaFree(hi);
+    SM_CUDA(cudaMemcpyAsync(p->h_pinned_d + 4, p->d_scalars + 4, 16, cudaMemcpyDeviceToHost, st));
     return SM_OK;
 }
 
