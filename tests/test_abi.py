@@ -21,10 +21,12 @@ def test_library_exports_header_symbols():
 
 
 def test_struct_sizes_match_header():
-    """ctypes mirrors must have the C layout (sizes checked against a tiny C program)."""
+    """ctypes mirrors must have the C layout (sizes and a few field offsets checked against a tiny C program)."""
     import subprocess, tempfile
     from paper_2004_10811_b200 import binding as B
-    src = '#include <stdio.h>\n#include "submatrix.h"\nint main(){printf("%zu %zu %zu\\n", sizeof(sm_options_t), sizeof(sm_plan_info_t), sizeof(sm_stats_t));return 0;}\n'
+    src = ('#include <stdio.h>\n#include <stddef.h>\n#include "submatrix.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu\\n", '
+           'sizeof(sm_options_t), sizeof(sm_plan_info_t), sizeof(sm_stats_t), offsetof(sm_options_t, overshoot), '
+           'offsetof(sm_options_t, mu_guess), offsetof(sm_options_t, mu_start), offsetof(sm_stats_t, mu_guess));return 0;}\n')
     with tempfile.TemporaryDirectory() as d:
         c = os.path.join(d, "s.c")
         open(c, "w").write(src)
@@ -32,7 +34,9 @@ def test_struct_sizes_match_header():
         subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), c, "-o", exe], check=True)
         out = subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()
     assert [int(x) for x in out] == [ctypes.sizeof(B.sm_options_t), ctypes.sizeof(B.sm_plan_info_t),
-                                     ctypes.sizeof(B.sm_stats_t)]
+                                     ctypes.sizeof(B.sm_stats_t), B.sm_options_t.overshoot.offset,
+                                     B.sm_options_t.mu_guess.offset, B.sm_options_t.mu_start.offset,
+                                     B.sm_stats_t.mu_guess.offset]
 
 
 def test_strerror_and_missing_library_is_loud(monkeypatch):
