@@ -2,11 +2,17 @@
 """bench.py -- density-matrix builds/s of the submatrix hot path on B200 (BASELINE.json metric).
 
 One "step" = one pass of the whole hot path over one synthetic input: sm_density_matrix on
-BASELINE config 4 (20736 water molecules, SZV, cutoff 6 A, one submatrix per molecule): Gershgorin
-bracket of K~, mu bisection from mu0 (each step = gather -> Newton-Schulz FP64 DMMA sign of all
-20736 submatrices -> electron count), final extract/scatter of D~.  The plan (device BSR container
-+ submatrix index, built once per sparsity pattern) is created before the timed region, like the
-paper's initialisation phase (PAPER.md IV-A).
+BASELINE config 4 (20736 water molecules, SZV, cutoff 6 A, one submatrix per molecule) with the
+library's default options: Gershgorin bracket of K~, a 24-step Lanczos run on K~ (interlacing scale,
+bracket, quadrature estimate of mu), then the mu search, every step of which is one sign evaluation
+(gather -> Newton-Schulz FP64 DMMA sign of all 20736 submatrices -> electron count), and the final
+extract/scatter of D~.  With the default search (readings A11d/A11e) the caller's mu0 = -1
+lies outside the Ritz interval taken for the gap and is NOT evaluated: the timed build is ONE sign
+evaluation at the quadrature estimate, verified by its converged electron count (plateau acceptance).
+`detail.literal_A11` reports the same build with the literal rule (step 0 at mu0, midpoint bisection),
+`detail.guarded_tol_1e-8` BASELINE's literal tolerance.  The plan (device BSR container + submatrix
+index, built once per sparsity pattern) is created before the timed region, like the paper's
+initialisation phase (PAPER.md IV-A); its time is reported in `detail.plan_create_ms`.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
 
@@ -22,7 +28,6 @@ import argparse
 import json
 import os
 import statistics
-import subprocess  # noqa: F401
 import sys
 import tempfile
 import time
@@ -36,10 +41,11 @@ METRIC = "density_matrix_builds_per_s"
 UNIT = "builds/s"
 EPS = 1e-12
 TOL_N = 0.5      # plateau acceptance (reading A11); 1e-8 is unreachable by construction
-MU0 = -1.0       # starting mu inside the occupied band: forces a genuine bisection
+MU0 = -1.0       # the caller's mu, inside the occupied band (evaluated only by the literal rule, see docstring)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_ns_gemm from the committed
-# `ncu --set full` capture (profiles/), or None when no capture matches the current kernel.
-NS_GEMM_DRAM_BYTES_PER_LAUNCH = 20.3e9  # all-active launch, mean of MODE 0 (15.8 GB) and MODE 1 (24.8 GB): profiles/r01_v6_ns_gemm_full.md
+# `ncu --set full` capture of the current kernel (profiles/r01_final_full_captures.md): all-active launch,
+# mean of MODE 0 (8.16 + 7.64 GB) and MODE 1 (17.25 + 7.69 GB).
+NS_GEMM_DRAM_BYTES_PER_LAUNCH = 20.4e9
 NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # guide: B200 FP64 tensor 45 TF/s, bf16 2250 TF/s (nominal)
 
 
@@ -51,6 +57,15 @@ def fp64_peak_tflops():
             pk = json.load(f)
         return pk["bf16_tflops"] * NOMINAL_FP64_OVER_BF16, "measured bf16 burst x 45/2250 (MEASURED_PEAKS.json)"
     return 1590.0 * NOMINAL_FP64_OVER_BF16, "fallback bf16 1.59 PF x 45/2250"
+
+
+def hbm_peak_gbps():
+    """Roofline denominator of the HBM-bound phases: the driver-measured copy bandwidth."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f)["hbm_gbs"], "MEASURED_PEAKS.json hbm_gbs (driver-measured copy bandwidth)"
+    return 6544.3, "fallback: the copy bandwidth measured on this pool in round 1"
 
 
 class ClockSampler:
@@ -149,6 +164,7 @@ def cpu_baseline(m, sample_groups=None, nthreads=0):
     scale = n3.sum() / n3[sample_groups].sum()
     t_full = dt * scale
     return {"value": 1.0 / t_full, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "note": "the test oracle (cyclic Jacobi eigendecomposition), not a tuned CPU implementation",
             "sample": f"{len(sample_groups)} of {idx.ngroups} submatrices (evenly spaced), {dt:.2f} s measured, "
                       f"extrapolated x{scale:.1f} by sum n^3", "seconds_measured": dt}, t_full
 
@@ -240,6 +256,84 @@ def run_phases(args, m, B, torch):
     print(json.dumps(out), flush=True)
 
 
+def run_extras(args, m, B, torch, plan, info, ws, d_in, d_out, mu, hbm_peak):
+    """Everything else north_star names, measured in the same run after the timed regions (rank 0):
+    phase rooflines of gather / scatter (CUDA events, best and median of 10), the literal A11 search, the
+    guarded tol_n = 1e-8 run, and the opt-in reduced-precision variant on the same input."""
+    out = {}
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timeit(f, reps=10):
+        for _ in range(3):
+            f()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            e0.record(); f(); e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return min(ts), float(np.median(ts))
+
+    tmp_out = torch.empty_like(d_out)
+    gb = (info.sum_ld2 + info.nnz) * 8 / 1e9
+    tmin, tmed = timeit(lambda: B.sm_gather(plan, d_in, mu, ws))
+    out["gather"] = {"ms_min": tmin, "ms_med": tmed, "alg_GB": gb, "GBps": gb / tmed * 1e3, "frac": gb / tmed * 1e3 / hbm_peak}
+    _, _, _, sub_dim, _ = B.sm_plan_export_index(plan)
+    gw = np.zeros(m.ngroups, np.int64)
+    np.add.at(gw, np.repeat(np.arange(m.ngroups), np.diff(m.grp_ptr)), m.blk_size[m.grp_cols])
+    sb = ((sub_dim.astype(np.int64) * gw).sum() + info.nnz) * 8 / 1e9
+    tmin, tmed = timeit(lambda: B.sm_scatter(plan, 1, tmp_out, ws))
+    out["scatter"] = {"ms_min": tmin, "ms_med": tmed, "alg_GB": sb, "GBps": sb / tmed * 1e3, "frac": sb / tmed * 1e3 / hbm_peak}
+    st = B.sm_stats_t()
+    n_target = float(m.n_occ)
+
+    # SURVEY A11 (i): the literal tolerance of BASELINE config 4, guarded by mu_tol / max_mu_steps
+    e0.record()
+    rc, mu_g = B.sm_density_matrix(plan, d_in, n_target, 1e-8, EPS, MU0, tmp_out, ws, st)
+    e1.record(); torch.cuda.synchronize()
+    out["guarded_tol_1e-8"] = {"status": int(rc), "status_text": B.sm_strerror(int(rc)), "mu_steps": st.mu_steps,
+                               "sign_evaluations": st.tot_evaluations, "abs_g": abs(st.n_elec - n_target),
+                               "mu": mu_g, "ms": e0.elapsed_time(e1)}
+
+    # reading A11 as written: step 0 at the caller's mu0, midpoint bisection (no quadrature estimate)
+    plan2 = B.plan_from_matrix(m, B.default_options(mu_guess=0, mu_start=0))
+    B.sm_density_matrix(plan2, d_in, n_target, TOL_N, EPS, MU0, tmp_out, ws, st)
+    torch.cuda.synchronize()
+    k = 3
+    e0.record()
+    for _ in range(k):
+        rc, mu_l = B.sm_density_matrix(plan2, d_in, n_target, TOL_N, EPS, MU0, tmp_out, ws, st)
+    e1.record(); torch.cuda.synchronize()
+    d = st.as_dict()
+    out["literal_A11"] = {"builds_per_s": k / (e0.elapsed_time(e1) * 1e-3), "ms_per_build": e0.elapsed_time(e1) / k,
+                          "status": int(rc), "mu": mu_l, "mu_steps": d["mu_steps"], "sign_evaluations": d["tot_evaluations"],
+                          "iter_trace": d["iter_trace"], "mu_trace": d["mu_trace"]}
+    B.sm_plan_destroy(plan2)
+
+    # opt-in reduced precision (3xTF32 on tcgen05) on the same input at the accepted mu, against the FP64 result
+    _, tdk64 = B.sm_trace_dk(plan, d_out, d_in)
+    plan3 = B.plan_from_matrix(m, B.default_options(precision=2))
+    need = B.sm_plan_query(plan3).workspace_bytes
+    ws3 = ws if need <= ws.numel() * 8 else B.alloc_workspace(plan3)
+    B.sm_set_timing(plan3, True)
+    for _ in range(2):
+        rc = B.sm_sign_execute(plan3, d_in, mu, 2e-6, tmp_out, ws3, st)
+    torch.cuda.synchronize()
+    d = st.as_dict()
+    _, tdk = B.sm_trace_dk(plan3, tmp_out, d_in)
+    out["reduced_precision_3xTF32"] = {
+        "status": int(rc), "ms_sign": d["ms_sign"], "ms_total": d["ms_total"], "iter_min": d["iter_min"],
+        "iter_max": d["iter_max"], "residual_floor": d["max_residual"],
+        "max_abs_err_vs_fp64": float((tmp_out - d_out).abs().max().item()),
+        "rel_band_energy_err_vs_fp64": abs(tdk - tdk64) / abs(tdk64), "n_elec": d["n_elec"]}
+    B.sm_plan_destroy(plan3)
+    # the FP64 evaluation at the same mu, for the comparison above
+    B.sm_sign_execute(plan, d_in, mu, EPS, tmp_out, ws, st)
+    torch.cuda.synchronize()
+    out["fp64_sign_evaluation"] = {"ms_sign": st.ms_sign, "ms_gather": st.ms_gather, "ms_scatter": st.ms_scatter,
+                                   "ms_total": st.ms_total, "iter_min": st.iter_min, "iter_max": st.iter_max}
+    return out
+
+
 def workload_config(args, m):
     from paper_2004_10811_b200 import workloads as W
     c = W.CONFIGS[args.config]
@@ -259,12 +353,15 @@ def workload_config(args, m):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the extra measurements of `detail` (phase rooflines, literal A11 search, guarded "
+                         "1e-8 run, reduced-precision run)")
     ap.add_argument("--mu-guess", type=int, default=1, choices=[0, 1],
                     help="1 (library default): first interior step of the mu search from the Lanczos quadrature "
                          "(DESIGN.md reading A11d); 0: pure midpoint bisection (reading A11)")
@@ -299,6 +396,16 @@ def main():
         if rank == 0:
             run_phases(args, m, B, torch)
         return
+    # roofline denominators measured in THIS run, with the clocks they were measured at
+    peaks = None
+    if rank == 0:
+        smp = ClockSampler(local_rank, period_s=0.01) if not os.environ.get('SM_NO_SAMPLER') else None
+        time.sleep(0.05)
+        pk = B.sm_measure_peaks()
+        peaks = {"dmma_issue_tflops": pk.dmma_tflops, "hbm_copy_GBps": pk.hbm_copy_gbs, "ms_dmma": pk.ms_dmma,
+                 "ms_copy": pk.ms_copy, "num_sms": pk.num_sms, "clocks": smp.stop() if smp else None,
+                 "how": "sm_measure_peaks: mma.sync.m8n8k4.f64 from registers, 16 warps/SM x 16 accumulators; "
+                        "16-byte grid-stride copy of 1 GiB (read + write bytes); best of 5 each"}
     plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess, mu_start=args.mu_start))
     info = B.sm_plan_query(plan)
     ws = B.alloc_workspace(plan)
@@ -337,27 +444,29 @@ def main():
     if sampler is not None:
         sampler.mark()
     launches0 = B.sm_launch_count(plan)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     gemm_ms = gemm_launches = sym_flop = n3 = evals = 0.0
     gather_ms = 0.0
-    e0.record(stream)
-    for _ in range(args.steps):
+    evs[0].record(stream)
+    for i in range(args.steps):
         st, mu = step_device()
+        evs[i + 1].record(stream)
         gemm_ms += stats.tot_ms_sign; gemm_launches += stats.tot_gemm_launches
         sym_flop += stats.tot_sym_flop; n3 += stats.tot_sum_iter_n3; evals += stats.tot_evaluations
         gather_ms += stats.tot_ms_gather
-    e1.record(stream)
     barrier()
     launches = B.sm_launch_count(plan) - launches0
-    ms = max_over_ranks(e0.elapsed_time(e1), world, torch.device("cuda", local_rank))
+    ms = max_over_ranks(evs[0].elapsed_time(evs[-1]), world, torch.device("cuda", local_rank))
+    per_step = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
     clocks = sampler.stop() if sampler else None
     last = stats.as_dict()
 
-    # end to end through the host-buffer C-ABI call
-    for _ in range(1):
+    # end to end through the host-buffer C-ABI call: same number of steps as the device-resident figure
+    for _ in range(min(args.warmup, 2)):
         step_host()
     barrier()
-    k_e2e = max(1, min(args.steps, 3))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    k_e2e = args.steps
     e0.record(stream)
     for _ in range(k_e2e):
         step_host()
@@ -367,40 +476,53 @@ def main():
 
     if rank == 0:
         peak, peak_src = fp64_peak_tflops()
+        hbm_peak, hbm_src = hbm_peak_gbps()
         # dominant kernel: k_ns_gemm<0|1>.  Algorithmic flops of one symmetric n x n product:
         # n(n+1)/2 outputs x 2n flop = n^2 (n+1); per launch = sum over the active submatrices.
         # gemm_ms = CUDA-event time of the Newton-Schulz phases (event pairs recorded by the library on its
         # stream around every evaluation's iteration loop): the GEMM launches plus the decision / bound /
         # control kernels and the empty launches behind a device-side stop (~2 % of it), so `achieved` is a
-        # slight under-estimate of the GEMM kernels' own rate (profiles/: 26.4 TFLOP/s in isolation).
+        # slight under-estimate of the GEMM kernels' own rate.
         ach = sym_flop / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
+        dmma = peaks["dmma_issue_tflops"]
         roofline = {"bound": "tensor", "kernel": "k_ns_gemm (FP64 DMMA Newton-Schulz, both modes)",
                     "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
                     "traffic": NS_GEMM_DRAM_BYTES_PER_LAUNCH, "peak_source": peak_src,
-                    "peak_dmma_issue_measured": 37.1, "frac_of_dmma_issue": ach / 37.1,
+                    "peak_dmma_issue_measured": dmma, "frac_of_dmma_issue": ach / dmma if dmma else None,
                     "launches_timed": int(gemm_launches), "avg_launch_ms": gemm_ms / max(gemm_launches, 1),
                     "alg_flop_per_launch": sym_flop / max(gemm_launches, 1),
                     "full_gemm_equiv_tflops": 2.0 * n3 / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0,
                     "sign_share_of_step": gemm_ms / ms if ms > 0 else None}
         gather_bytes = (info.sum_ld2 + info.nnz) * 8.0
+        detail = {"status": int(st), "mu": mu, "mu_steps": last["mu_steps"], "n_elec": last["n_elec"],
+                  "what_is_timed": "per build: Gershgorin bracket + 24-step Lanczos run + sign evaluations of the mu "
+                                   "search (see sign_evaluations_per_step) + scatter",
+                  "sign_evaluations_per_step": evals / args.steps,
+                  "ms_per_step_best": min(per_step), "ms_per_step_median": statistics.median(per_step),
+                  "ns_iterations_last_eval": last["iterations"], "iter_min": last["iter_min"],
+                  "iter_max": last["iter_max"], "max_residual": last["max_residual"],
+                  "dim_min": info.dim_min, "dim_mean": info.dim_mean, "dim_max": info.dim_max,
+                  "workspace_GB": info.workspace_bytes / 1e9, "n_tiles": info.n_tiles,
+                  "gather_GBps_in_build": gather_bytes * evals / (gather_ms * 1e-3) / 1e9 if gather_ms > 0 else None,
+                  "ms_scatter_last": last["ms_scatter"], "mu_trace": last["mu_trace"],
+                  "ne_trace": last["ne_trace"], "ne_err_trace": last["ne_err_trace"],
+                  "iter_trace": last["iter_trace"], "spec_lo": last["spec_lo"], "spec_hi": last["spec_hi"],
+                  "bracket": [last["bracket_lo"], last["bracket_hi"]],
+                  "mu_guess": last["mu_guess"] if last["mu_guess"] == last["mu_guess"] else None,
+                  "plan_create_ms": info.ms_plan_create,
+                  "index_build": {"ms": info.ms_index_kernels, "alg_GB": info.index_alg_bytes / 1e9,
+                                  "GBps": info.index_alg_bytes / 1e6 / info.ms_index_kernels if info.ms_index_kernels > 0 else None,
+                                  "frac": info.index_alg_bytes / 1e6 / info.ms_index_kernels / hbm_peak if info.ms_index_kernels > 0 else None},
+                  "hbm_peak_GBps": hbm_peak, "hbm_peak_source": hbm_src, "peaks_measured_this_run": peaks}
+        if not args.no_extras:
+            detail.update(run_extras(args, m, B, torch, plan, info, ws, d_in, d_out, mu, hbm_peak))
         line = {"metric": METRIC, "value": world * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic", "config": workload_config(args, m), "clocks": clocks,
-                "e2e": {"value": world * k_e2e / (ms_e2e * 1e-3), "unit": UNIT,
+                "e2e": {"value": world * k_e2e / (ms_e2e * 1e-3), "unit": UNIT, "steps": k_e2e,
                         "h2d_bytes_per_step": int(info.nnz * 8), "d2h_bytes_per_step": int(info.nnz * 8)},
-                "gpu_launches": int(launches), "roofline": roofline,
-                "detail": {"status": int(st), "mu": mu, "mu_steps": last["mu_steps"], "n_elec": last["n_elec"],
-                           "sign_evaluations_per_step": evals / args.steps,
-                           "ns_iterations_last_eval": last["iterations"], "iter_min": last["iter_min"],
-                           "iter_max": last["iter_max"], "max_residual": last["max_residual"],
-                           "dim_min": info.dim_min, "dim_mean": info.dim_mean, "dim_max": info.dim_max,
-                           "workspace_GB": info.workspace_bytes / 1e9, "n_tiles": info.n_tiles,
-                           "gather_GBps": gather_bytes * evals / (gather_ms * 1e-3) / 1e9 if gather_ms > 0 else None,
-                           "ms_scatter_last": last["ms_scatter"], "mu_trace": last["mu_trace"],
-                           "ne_trace": last["ne_trace"], "ne_err_trace": last["ne_err_trace"],
-                           "iter_trace": last["iter_trace"], "spec_lo": last["spec_lo"], "spec_hi": last["spec_hi"],
-                           "bracket": [last["bracket_lo"], last["bracket_hi"]], "mu_guess": last["mu_guess"] if last["mu_guess"] == last["mu_guess"] else None}}
+                "gpu_launches": int(launches), "roofline": roofline, "detail": detail}
         if not args.no_cpu_baseline:
             cb, _ = cpu_baseline(m)
             line["cpu_baseline"] = cb

@@ -24,9 +24,9 @@
  *    symmetrised, L127).
  *  - Groups: grp_ptr[ngroups+1], grp_cols[nb] must be a partition of 0..nb-1 (every block column
  *    in exactly one group), so every result block is written exactly once.
- *  - Errors: no exceptions, no abort.  Status < 0: hard error, outputs unspecified.  Status > 0:
- *    warning, outputs are written and sm_stats_t says what is suspect.  sm_strerror() names any
- *    status.
+ *  - Errors: no exceptions cross the boundary (host allocation failures come back as
+ *    SM_ERR_ALLOC), no abort.  Status < 0: hard error, outputs unspecified.  Status > 0: warning,
+ *    outputs are written and sm_stats_t says what is suspect.  sm_strerror() names any status.
  *  - One plan may be used by one stream at a time.  Results are deterministic run to run for a
  *    fixed plan and options (fixed reduction orders, no floating-point atomics).
  */
@@ -62,14 +62,19 @@ typedef struct {
                          /* 0 = Gershgorin row sums of the assembled submatrix;              */
                          /* 1 = min(that, interlacing bound): a_i is a principal submatrix   */
                          /*     of K~, so rho(a_i - mu I) <= max|lambda_minmax(K~) - mu|,    */
-                         /*     extremes of K~ by a short Lanczos run per call, then / overshoot */
+                         /*     extremes of K~ by a short Lanczos run per call, then / overshoot; */
+                         /*     a run that breaks down is discarded (Gershgorin only), and the  */
+                         /*     cap is never below the largest column 2-norm of a_i - mu I      */
     int32_t precision;   /* 0 = FP64 DMMA (the parity path);                           [0]   */
                          /* opt-in reduced precision on the tcgen05 tensor cores (FP32       */
                          /* accumulators in tensor memory; accuracy reported separately; no  */
                          /* steering early-out):                                             */
-                         /* 1 = FP32 storage, plain TF32 products (error ~2e-3 class);       */
                          /* 2 = "3xTF32": operands stored as hi + lo TF32 pairs, products    */
-                         /*     hi hi + hi lo + lo hi (FP32-class, <= 1e-3 bar)              */
+                         /*     hi hi + hi lo + lo hi -- THE reduced-precision variant: it   */
+                         /*     meets the <= 1e-3 elementwise bar (measured 1e-6 class);     */
+                         /* 1 = FP32 storage, plain TF32 products: experimental, error 5e-4   */
+                         /*     ... 2e-3, does NOT meet the 1e-3 bar in general and its      */
+                         /*     n_elec is too coarse to steer the mu search on large systems */
     int32_t check_every; /* the stop decisions are taken on the device; the host enqueues  [16]  */
                          /* this many iterations ahead before it reads the control block     */
                          /* (>= 1; launches after the stop are empty)                        */
@@ -79,7 +84,8 @@ typedef struct {
                          /* direction of the step, never for acceptance (A11).     */
     double mu_tol;       /* bisection stops when the bracket is narrower than this     [1e-6]*/
     int32_t early_out;   /* 1: a bisection evaluation stops as soon as the bound           [1]  */
-                         /* |n_elec(final) - n_elec(X_k)| <= 1/2 sum_gen (1 - (X_k^2)_kk)     */
+                         /* |n_elec(final) - n_elec(X_k)| <= 1/2 sum_gen min(S1, (S1 + S2)/2), */
+                         /* S1 = 1 - (X_k^2)_kk, S2 = sum_j (delta_kj - (X_k^2)_kj)^2,         */
                          /* proves the sign of n_elec - n_target (reading A11c); such a step */
                          /* only steers, it is never accepted.  0: every evaluation converges*/
     int32_t order;       /* 2: Newton-Schulz X <- 1/2 X (3I - X^2), Eq.(11) L97          [2]  */
@@ -127,6 +133,10 @@ typedef struct {
     double est_speedup;       /* Eq.(15): S = sum_c n~_c^3 / sum_i n_i^3, the estimated    */
                               /* additional speed-up of this grouping over per-column          */
                               /* submatrices under the O(n^3) cost model of Eq.(14)       */
+    int64_t index_alg_bytes;  /* algorithmic bytes of the index build: nnzb*4 read + nnzb*4 +  */
+                              /* sum|S_i|*8 written                               */
+    float ms_index_kernels;   /* CUDA-event time of the index-builder kernels (a2)              */
+    float ms_plan_create;     /* host wall clock of the whole sm_plan_create call               */
 } sm_plan_info_t;
 
 /* Filled by sm_sign_execute / sm_density_matrix (may be NULL). Times are CUDA-event ms of the
@@ -140,7 +150,9 @@ typedef struct {
     double mu;                /* chemical potential of the returned result                   */
     int32_t mu_steps;         /* sign evaluations done by sm_density_matrix                  */
     int32_t gemm_launches;    /* GEMM kernel launches in the last evaluation                 */
-    int64_t sum_iter_n3;      /* sum_i (2*iters_i + 1) * n_i^3  (=> flop = 2x this)          */
+    int64_t sum_iter_n3;      /* sum_i products_i * n_i^3 (=> dense-GEMM flop = 2x this); products_i */
+                              /* = 2 iters_i + 1, or 2 iters_i when the predicted exit (opt.predict) */
+                              /* skipped the confirming product; 3 per iteration for order = 3      */
     float ms_gather, ms_sign, ms_scatter, ms_total;
     double mu_trace[64];      /* bisection history: mu of step k                             */
     double ne_trace[64];      /* n_elec of step k (of the last iterate if the step ended early) */
@@ -248,7 +260,9 @@ sm_status_t sm_trace_dk(sm_plan_t* plan, const double* d_D, const double* d_K, d
 
 /*
  * Phase entry points used by the tests and the roofline benchmark (same kernels as above):
- *   sm_gather   : workspace X buffer <- a_i - mu I (identity-padded); also the Gershgorin bounds
+ *   sm_gather   : workspace X buffer <- a_i - mu I (rows / columns n_i .. ld_i - 1 zero: a fixed point of
+ *                 the iteration); also the Gershgorin bounds (plain Gershgorin scaling, whatever the
+ *                 previous call used)
  *   sm_scatter  : d_vals_out <- 1/2 (delta - xscale_i * X) from the workspace X buffer written by
  *                 the last sm_gather / sign evaluation; f = identity round trip when as_identity=1:
  *                 d_vals_out <- X (i.e. gather then scatter returns K~ - mu I on the pattern)
@@ -261,6 +275,21 @@ sm_status_t sm_sign_iterate(sm_plan_t* plan, double eps, void* d_workspace, size
 sm_status_t sm_scatter(sm_plan_t* plan, int32_t as_identity, double* d_vals_out, void* d_workspace,
                        size_t workspace_bytes, void* cuda_stream);
 
+/*
+ * sm_measure_peaks -- the roofline denominators of this library measured on the current device, for
+ * bench.py (diagnostic; allocates and frees 2 GiB of device memory; ~50 ms):
+ *   dmma_tflops  issue rate of mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4, the FP64 tensor-core instruction of
+ *                the Newton-Schulz kernel) with register-resident operands, 16 warps per SM, 16
+ *                independent accumulators per warp, best of 5
+ *   hbm_copy_gbs read + write bytes per second of a 16-byte grid-stride copy of 1 GiB, best of 5
+ */
+typedef struct {
+    double dmma_tflops, hbm_copy_gbs;
+    double ms_dmma, ms_copy;
+    int32_t num_sms, reserved;
+} sm_peaks_t;
+sm_status_t sm_measure_peaks(sm_peaks_t* out, void* cuda_stream);
+
 /* Enable (1) / disable (0) per-phase CUDA-event timing into sm_stats_t (adds stream syncs). */
 sm_status_t sm_set_timing(sm_plan_t* plan, int32_t enable);
 
@@ -269,7 +298,7 @@ int64_t sm_launch_count(const sm_plan_t* plan);
 
 void sm_plan_destroy(sm_plan_t* plan);
 const char* sm_strerror(sm_status_t status);
-/* Text of the last CUDA error seen by this library in the calling process ("" if none). */
+/* Text of the last CUDA error seen by this library on the calling THREAD ("" if none). */
 const char* sm_last_cuda_error(void);
 
 #ifdef __cplusplus

@@ -27,7 +27,7 @@ EXPORTS = [
     "sm_plan_create", "sm_plan_query", "sm_plan_export_index", "sm_sign_execute", "sm_sign_execute_host",
     "sm_density_matrix", "sm_density_matrix_host", "sm_trace_dk", "sm_gather", "sm_sign_iterate",
     "sm_scatter", "sm_set_timing", "sm_launch_count", "sm_plan_destroy", "sm_strerror",
-    "sm_last_cuda_error",
+    "sm_last_cuda_error", "sm_measure_peaks",
 ]
 
 
@@ -44,7 +44,13 @@ class sm_plan_info_t(C.Structure):
                 ("dim_max", C.c_int32), ("dim_mean", C.c_double), ("sum_n2", C.c_int64), ("sum_n3", C.c_int64),
                 ("sum_ld2", C.c_int64), ("n_tiles", C.c_int64), ("n_buckets", C.c_int32),
                 ("reserved0", C.c_int32), ("workspace_bytes", C.c_size_t), ("sum_n3_columns", C.c_int64),
-                ("est_speedup", C.c_double)]
+                ("est_speedup", C.c_double), ("index_alg_bytes", C.c_int64), ("ms_index_kernels", C.c_float),
+                ("ms_plan_create", C.c_float)]
+
+
+class sm_peaks_t(C.Structure):
+    _fields_ = [("dmma_tflops", C.c_double), ("hbm_copy_gbs", C.c_double), ("ms_dmma", C.c_double),
+                ("ms_copy", C.c_double), ("num_sms", C.c_int32), ("reserved", C.c_int32)]
 
 
 class sm_stats_t(C.Structure):
@@ -110,9 +116,10 @@ def lib() -> C.CDLL:
         L.sm_strerror.argtypes = [i32]
         L.sm_strerror.restype = C.c_char_p
         L.sm_last_cuda_error.restype = C.c_char_p
+        L.sm_measure_peaks.argtypes = [C.POINTER(sm_peaks_t), vp]
         for f in ("sm_plan_create", "sm_plan_query", "sm_plan_export_index", "sm_sign_execute",
                   "sm_sign_execute_host", "sm_density_matrix", "sm_density_matrix_host", "sm_trace_dk",
-                  "sm_gather", "sm_sign_iterate", "sm_scatter", "sm_set_timing"):
+                  "sm_gather", "sm_sign_iterate", "sm_scatter", "sm_set_timing", "sm_measure_peaks"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -248,6 +255,12 @@ def sm_set_timing(plan, enable: bool) -> int:
 
 def sm_launch_count(plan) -> int:
     return int(lib().sm_launch_count(plan))
+
+
+def sm_measure_peaks(stream=None) -> sm_peaks_t:
+    pk = sm_peaks_t()
+    _check(lib().sm_measure_peaks(C.byref(pk), _stream_ptr(stream)))
+    return pk
 
 
 def sm_plan_destroy(plan) -> None:

@@ -2,6 +2,7 @@
 // host loop, the mu bisection (a8).  Every floating-point step of the path runs in the kernels of
 // plan.cu / gather_scatter.cu / ns_sign.cu; the host only sequences launches and compares scalars.
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdlib>
 #include <cstdio>
@@ -103,16 +104,44 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
     delete p;
 }
 
+namespace {
+struct PlanGuard {  // destroys a half-built plan on every error path, exceptions included
+    sm_plan* p = nullptr;
+    ~PlanGuard() { if (p) sm_plan_destroy(p); }
+};
+sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_size, const int64_t* colptr,
+                             const int32_t* rowidx, int32_t ngroups, const int32_t* grp_ptr,
+                             const int32_t* grp_cols, const sm_options_t* opt, void* cuda_stream);
+}  // namespace
+
 extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_t* blk_size,
                                       const int64_t* colptr, const int32_t* rowidx, int32_t ngroups,
                                       const int32_t* grp_ptr, const int32_t* grp_cols,
                                       const sm_options_t* opt, void* cuda_stream) {
     if (!plan) return SM_ERR_INVALID_ARG;
     *plan = nullptr;
+    try {  // host containers may throw: nothing crosses the C boundary
+        return plan_create_impl(plan, nb, blk_size, colptr, rowidx, ngroups, grp_ptr, grp_cols, opt, cuda_stream);
+    } catch (const std::bad_alloc&) {
+        *plan = nullptr;
+        return SM_ERR_ALLOC;
+    } catch (...) {
+        *plan = nullptr;
+        return SM_ERR_INVALID_ARG;
+    }
+}
+
+namespace {
+sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_size, const int64_t* colptr,
+                             const int32_t* rowidx, int32_t ngroups, const int32_t* grp_ptr,
+                             const int32_t* grp_cols, const sm_options_t* opt, void* cuda_stream) {
+    const auto t_begin = std::chrono::steady_clock::now();
     sm_status_t s = validate(nb, blk_size, colptr, rowidx, ngroups, grp_ptr, grp_cols);
     if (s) return s;
     sm_plan* p = new (std::nothrow) sm_plan();
     if (!p) return SM_ERR_ALLOC;
+    PlanGuard guard;
+    guard.p = p;
     if (opt) p->opt = *opt; else default_options(&p->opt);
     if (p->opt.max_iter <= 0) p->opt.max_iter = 100;
     if (p->opt.check_every <= 0) p->opt.check_every = 1;
@@ -122,12 +151,12 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (!(p->opt.overshoot >= 1.0)) p->opt.overshoot = 1.0;     // zero-initialised struct: no overshoot
     if (p->opt.overshoot > 1.5) p->opt.overshoot = 1.5;         // f(x) = x(3 - x^2)/2 keeps [1, 1.5] inside [0.56, 1]
     if (p->opt.order == 0) p->opt.order = 2;                    // zero-initialised struct: Eq.(11)
-    if (p->opt.order != 2 && p->opt.order != 3) { delete p; return SM_ERR_INVALID_ARG; }
+    if (p->opt.order != 2 && p->opt.order != 3) return SM_ERR_INVALID_ARG;
     if (p->opt.order == 3) {
-        if (p->opt.precision != 0) { delete p; return SM_ERR_INVALID_ARG; }
+        if (p->opt.precision != 0) return SM_ERR_INVALID_ARG;
         p->opt.overshoot = 1.0;  // Eq.(19)'s map is increasing beyond 1: eigenvalues of X0 must not exceed 1
     }
-    if (p->opt.precision < 0 || p->opt.precision > 2 || p->opt.scaling < 0 || p->opt.scaling > 1) { delete p; return SM_ERR_INVALID_ARG; }
+    if (p->opt.precision < 0 || p->opt.precision > 2 || p->opt.scaling < 0 || p->opt.scaling > 1) return SM_ERR_INVALID_ARG;
     p->nb = nb; p->ngroups = ngroups; p->nnzb = nb ? colptr[nb] : 0;
     p->h_blk_size.assign(blk_size, blk_size + nb);
     p->h_colptr.assign(colptr, colptr + nb + 1);
@@ -139,12 +168,11 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (cudaGetDevice(&dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
         set_cuda_error(cudaGetLastError(), "cudaGetDevice");
-        delete p;
         return SM_ERR_CUDA;
     }
     s = build_index_device(p, st);
-    if (s) { sm_plan_destroy(p); return s; }
-    if (p->opt.precision != 0 && (s = build_tf32_tables(p, st))) { sm_plan_destroy(p); return s; }
+    if (s) return s;
+    if (p->opt.precision != 0 && (s = build_tf32_tables(p, st))) return s;
     if (p->opt.order == 3) p->info.workspace_bytes = p->info.workspace_bytes / 3 * 4;  // + W of Eq.(19)
     // per-evaluation state
     const int ng = std::max(ngroups, 1);
@@ -153,7 +181,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_done_iter, (size_t)ng * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_flag, (size_t)ng * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_res, (size_t)ng * 16);
-    if (e == cudaSuccess) e = A((void**)&p->d_gersh, (size_t)ng * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_gersh, (size_t)ng * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_alpha, (size_t)ng * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_lmin, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_partials, (size_t)p->n_tiles * 4 * 8);
@@ -168,7 +196,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
     if (e == cudaSuccess) e = A((void**)&p->d_ctrl, 64);
     if (e == cudaSuccess) e = cudaMemset(p->d_ctrl, 0, 64);
     if (e == cudaSuccess) e = cudaMallocHost(&p->h_ctrl, 64);
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_lz, 66 * 8);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_lz, 68 * 8);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned, (size_t)(p->opt.max_iter + 2) * 4);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_pinned_d, 8 * 8);
     for (auto& ev : p->ev)
@@ -177,7 +205,6 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         set_cuda_error(e, "plan state allocation");
-        sm_plan_destroy(p);
         return e == cudaErrorMemoryAllocation ? SM_ERR_ALLOC : SM_ERR_CUDA;
     }
     // gather launch shape: member tables + hash table of S_i + position map + block map of a chunk
@@ -198,7 +225,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
             for (int64_t q = colptr[c]; q < colptr[c + 1]; ++q) elems += blk_size[rowidx[q]];
             max_col_elems = std::max(max_col_elems, elems * blk_size[c]);
         }
-        if (max_col_elems >= (int64_t)UINT32_MAX) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }
+        if (max_col_elems >= (int64_t)UINT32_MAX) return SM_ERR_INVALID_ARG;
         const int esz = max_col_elems < 65535 ? 2 : 4;
         p->gather_map16 = esz == 2;
         auto bytes = [&](int mc) { return fixed + (((size_t)mc * mpad * esz + 15) & ~(size_t)15); };
@@ -207,7 +234,7 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
         if (bytes(mc) > want) mc = (int)std::max<int64_t>(((int64_t)want - (int64_t)fixed) / (mpad * esz), 16);
         mc = std::min(mc, msb);
         while (mc > 1 && bytes(mc) > budget) mc >>= 1;
-        if (bytes(mc) > budget) { sm_plan_destroy(p); return SM_ERR_INVALID_ARG; }
+        if (bytes(mc) > budget) return SM_ERR_INVALID_ARG;
         p->gather_warps = 8; p->gather_tile_ld = tile_ld; p->gather_mpad = mpad; p->gather_mc = mc;
         p->gather_msb = msb; p->gather_hash_size = hs; p->gather_hash_shift = shift;
         p->gather_smem = bytes(mc);
@@ -217,9 +244,13 @@ extern "C" sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_
         while ((int64_t)ngroups * split < want_ctas && split * 8 * 4 < p->info.dim_max) ++split;
         p->gather_split = std::max(split, 1);
     }
+    p->info.ms_plan_create =
+        std::chrono::duration<float, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    guard.p = nullptr;
     *plan = p;
     return SM_OK;
 }
+}  // namespace
 
 extern "C" sm_status_t sm_plan_query(const sm_plan_t* p, sm_plan_info_t* out) {
     if (!p || !out) return SM_ERR_INVALID_ARG;
@@ -397,7 +428,8 @@ sm_status_t ensure_bounds(sm_plan* p, const double* d_in, cudaStream_t st) {
 sm_status_t apply_scaling(sm_plan* p, double mu, cudaStream_t st) {
     p->resc_eval = 0;
     if (p->opt.scaling != 1) return SM_OK;
-    const double cap = std::max(std::fabs(p->lz_hi - mu), std::fabs(p->lz_lo - mu));
+    // a Lanczos run that broke down is not used (cap = 0: the rigorous Gershgorin bounds alone, reading A8)
+    const double cap = p->lz_ok ? std::max(std::fabs(p->lz_hi - mu), std::fabs(p->lz_lo - mu)) : 0.0;
     // reading A8b: distance from mu to the nearest Ritz value of the Lanczos run = estimate of the smallest
     // eigenvalue modulus of K~ - mu I (Ritz values sit inside the bands, so it errs on the large side)
     // Only where mu sits in a hole of the Ritz spectrum (l_0 >= 0.05): inside a band the evaluation is most
@@ -446,7 +478,7 @@ sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, cons
         stats->tot_evaluations = 1;
         stats->tot_ms_gather = stats->ms_gather;
         stats->tot_ms_sign = stats->ms_sign;
-        if (p->opt.scaling == 1) { stats->spec_lo = p->lz_lo; stats->spec_hi = p->lz_hi; }
+        if (p->opt.scaling == 1 && p->lz_ok) { stats->spec_lo = p->lz_lo; stats->spec_hi = p->lz_hi; }
     }
     return SM_OK;
 }
@@ -499,6 +531,7 @@ extern "C" sm_status_t sm_gather(sm_plan_t* p, const double* d_vals_in, double m
     sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
     if (s) return s;
     if ((s = reset_state(p, st))) return s;
+    p->resc_eval = 0;  // phase entry: plain Gershgorin scaling, whatever the previous call used
     return launch_gather(p, d_vals_in, mu, b.b0, st);
 }
 
@@ -564,7 +597,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     if (p->opt.scaling == 1 && (s = ensure_bounds(p, d_vals_in, st))) return s;  // ends with a synchronisation
     SM_CUDA(cudaStreamSynchronize(st));  // no-op after the Lanczos run
     double lo = p->h_pinned_d[4], hi = p->h_pinned_d[5];
-    if (p->opt.scaling == 1) {
+    if (p->opt.scaling == 1 && p->lz_ok) {
         lo = std::max(lo, p->lz_lo);
         hi = std::min(hi, p->lz_hi);
     }
@@ -573,7 +606,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     // K~ below each Ritz value; the first interior step goes to the middle of the widest Ritz interval
     // near the target filling instead of the bracket midpoint (a guess only: the bracket logic is unchanged)
     double guess = NAN, guess_a = NAN, guess_b = NAN;  // the estimate and the Ritz interval it is the middle of
-    if (p->opt.mu_guess && p->opt.scaling == 1 && p->lz_nodes >= 2 && p->info.n_basis > 0) {
+    if (p->opt.mu_guess && p->opt.scaling == 1 && p->lz_ok && p->lz_nodes >= 2 && p->info.n_basis > 0) {
         const int k = p->lz_nodes;
         const double* th = p->h_lz + 2;
         const double* cum = p->h_lz + 34;

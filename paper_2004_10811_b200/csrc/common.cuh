@@ -41,6 +41,12 @@ __host__ __device__ __forceinline__ size_t panel_off(int r, int c, int ld) {
 
 void set_cuda_error(cudaError_t e, const char* where);
 
+// Frees a temporary device buffer on every return path.
+struct DevTmp {
+    void* p = nullptr;
+    ~DevTmp() { if (p) cudaFree(p); }
+};
+
 #define SM_CUDA(call)                                        \
     do {                                                     \
         cudaError_t e__ = (call);                            \
@@ -84,7 +90,7 @@ struct sm_plan {
     int32_t* d_done_iter = nullptr;        // [ngroups] -1 = active, else iteration at which it stopped
     int32_t* d_flag = nullptr;             // [ngroups] 0 converged, 1 stagnated / max_iter
     double* d_res = nullptr;               // [2][ngroups] residual history (ping-pong)
-    unsigned long long* d_gersh = nullptr; // [ngroups] bits of the Gershgorin bound (atomicMax)
+    unsigned long long* d_gersh = nullptr; // [2][ngroups] bits of the Gershgorin bound | of the largest squared column norm (atomicMax)
     double* d_partials = nullptr;          // [n_tiles][4] per-tile, per-consumer-warp residual partials
     int32_t* d_counters = nullptr;         // [max_iter+2] still-active submatrices after iteration k
     int32_t* d_sched = nullptr;            // [2*(max_iter+2)] work counters of the persistent GEMM launches
@@ -122,10 +128,13 @@ struct sm_plan {
     double* h_lz = nullptr;                // pinned [66]: lo, hi, Ritz values [32], cumulative quadrature weights [32]
     int lz_nodes = 0;
     int lz_valid = 0;                      // lz_lo / lz_hi belong to the current call's values
+    int lz_ok = 0;                         // the run did not break down: cap, bracket and quadrature may be used
+    int ns_attr_set = 0, tf32_attr_set = 0;  // dynamic shared-memory opt-in done on this plan's device
     // --- staging for the *_host entry points
     double *d_stage_in = nullptr, *d_stage_out = nullptr;
     // --- misc
     int timing = 0;
+    float ms_index_kernels = 0.f;          // CUDA-event time of the index-builder kernels (plan creation)
     int64_t launches = 0;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_iter[2] = {nullptr, nullptr};
@@ -139,6 +148,7 @@ struct sm_plan {
 namespace smb {
 // plan.cu
 sm_status_t build_index_device(sm_plan* p, cudaStream_t st);
+sm_status_t launch_excl_scan(const int32_t* in, int64_t n, int64_t* out, cudaStream_t st);  // out[n + 1], one CTA
 // gather_scatter.cu
 sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, cudaStream_t st);
 sm_status_t launch_scatter(sm_plan* p, int as_identity, const double* buf0, const double* buf1,

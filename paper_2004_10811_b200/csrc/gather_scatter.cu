@@ -33,7 +33,9 @@ __device__ __forceinline__ int find_sorted64(const int32_t* __restrict__ a, int 
 // two block-map reads, predicated 8-byte loads of the stored values straight from global memory
 // (L2-resident: every value is used by ~|S_i| submatrices), mu subtracted on the diagonal
 // (Eq.(16)), one coalesced 16-byte store into the k8-panel workspace, abs-sums for the Gershgorin
-// bound s_i = max_q sum_p |a_pq|.
+// bound s_i = max_q sum_p |a_pq|, and squares for max_q ||a e_q||_2^2 (a rigorous LOWER bound of the
+// spectral radius: the estimated interlacing cap is never taken below it, reading A8; stored in
+// gersh[ngroups + g]).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned gather_hash(int key, int shift) {
     return ((unsigned)key * 2654435761u) >> shift;
@@ -96,7 +98,7 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
     }
     for (int p = n + threadIdx.x; p < tile_ld; p += blockDim.x) posmap[p] = make_uint2((unsigned)m, 1u << 16);
     double* Xg = A.X + A.ws_off[g];
-    double cmax = 0.0;
+    double cmax = 0.0, cmax2 = 0.0;
     const int gw = blockIdx.y * nw + wid, gstride = nw * gridDim.y;
 
     for (int c0 = 0; c0 < m; c0 += mc) {
@@ -142,7 +144,7 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
             unsigned xo = (unsigned)t0 * (unsigned)ld + (unsigned)(q & 63) * 8u + (unsigned)(lane >> 2) * rows_t * 8u +
                           2u * (lane & 3);
             const unsigned xstep = rows_t * 64u;
-            double asum = 0.0;
+            double asum = 0.0, ssum = 0.0;
             // warp-uniform trip count (groups of four 64-wide steps, predicated inside): one loop body,
             // no divergent remainder loop; all look-ups and loads of a group are in flight together
             for (int base = 0, p0 = 2 * lane; base < ld; base += 256, p0 += 256, xo += 4 * xstep) {
@@ -158,13 +160,18 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
                         if (p == q) v.x -= A.mu;
                         if (p + 1 == q) v.y -= A.mu;
                         asum += fabs(v.x) + fabs(v.y);
+                        ssum = fma(v.x, v.x, fma(v.y, v.y, ssum));
                         __stcs(reinterpret_cast<double2*>(Xg + xo + u * xstep), v);  // streaming: the workspace is far larger than L2
                     }
                 }
             }
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) asum += __shfl_xor_sync(0xffffffffu, asum, o);
+            for (int o = 16; o > 0; o >>= 1) {
+                asum += __shfl_xor_sync(0xffffffffu, asum, o);
+                ssum += __shfl_xor_sync(0xffffffffu, ssum, o);
+            }
             cmax = fmax(cmax, asum);
+            cmax2 = fmax(cmax2, ssum);
         }
     }
     // zero padding columns n..ld-1 (first CTA of the submatrix)
@@ -174,7 +181,10 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
                 *reinterpret_cast<double2*>(Xg + panel_off(qq, p, ld)) = make_double2(0.0, 0.0);
         }
     }
-    if (lane == 0 && cmax > 0.0) atomicMax(A.gersh + g, (unsigned long long)__double_as_longlong(cmax));
+    if (lane == 0 && cmax > 0.0) {
+        atomicMax(A.gersh + g, (unsigned long long)__double_as_longlong(cmax));
+        atomicMax(A.gersh + gridDim.x + g, (unsigned long long)__double_as_longlong(cmax2));
+    }
 }
 
 // Gather list (pattern only, built by the first gather of a plan when 16-bit entries suffice): for every
@@ -238,23 +248,22 @@ static sm_status_t build_gather_list(sm_plan* p, cudaStream_t st) {
         SM_CUDA(cudaFuncSetAttribute(k_glist<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hbytes));
         SM_CUDA(cudaFuncSetAttribute(k_glist<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hbytes));
     }
-    int32_t* d_cnt = nullptr;
-    SM_CUDA(cudaMalloc((void**)&d_cnt, (size_t)std::max<int64_t>(tot, 1) * 4));
+    DevTmp cnt_tmp;
+    SM_CUDA(cudaMalloc(&cnt_tmp.p, (size_t)std::max<int64_t>(tot, 1) * 4));
+    int32_t* d_cnt = (int32_t*)cnt_tmp.p;
     k_glist<false><<<p->ngroups, 256, hbytes, st>>>(p->d_colptr, p->d_rowidx, p->d_val_off, p->d_sub_ptr, p->d_sub_blocks,
                                                     p->gather_hash_size, p->gather_hash_shift, d_cnt, nullptr, nullptr);
-    std::vector<int32_t> cnt((size_t)tot);
-    SM_CUDA(cudaMemcpyAsync(cnt.data(), d_cnt, (size_t)tot * 4, cudaMemcpyDeviceToHost, st));
-    SM_CUDA(cudaStreamSynchronize(st));
-    cudaFree(d_cnt);
-    std::vector<int64_t> ptr((size_t)tot + 1, 0);
-    for (int64_t i = 0; i < tot; ++i) ptr[i + 1] = ptr[i] + cnt[i];
+    // extents by a device prefix sum; the host only learns the total (8 bytes) to size the list
     SM_CUDA(cudaMalloc((void**)&p->d_gl_ptr, ((size_t)tot + 1) * 8));
-    SM_CUDA(cudaMemcpyAsync(p->d_gl_ptr, ptr.data(), ((size_t)tot + 1) * 8, cudaMemcpyHostToDevice, st));
-    SM_CUDA(cudaMalloc((void**)&p->d_gl, (size_t)std::max<int64_t>(ptr[tot], 1) * 4));
+    sm_status_t s = launch_excl_scan(d_cnt, tot, p->d_gl_ptr, st);
+    if (s) return s;
+    int64_t n_entries = 0;
+    SM_CUDA(cudaMemcpyAsync(&n_entries, p->d_gl_ptr + tot, 8, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    SM_CUDA(cudaMalloc((void**)&p->d_gl, (size_t)std::max<int64_t>(n_entries, 1) * 4));
     k_glist<true><<<p->ngroups, 256, hbytes, st>>>(p->d_colptr, p->d_rowidx, p->d_val_off, p->d_sub_ptr, p->d_sub_blocks,
                                                    p->gather_hash_size, p->gather_hash_shift, nullptr, p->d_gl_ptr, p->d_gl);
-    p->launches += 2;
-    SM_CUDA(cudaStreamSynchronize(st));  // ptr[] is read by the copy above
+    p->launches += 3;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
 }
@@ -266,7 +275,7 @@ sm_status_t launch_gather(sm_plan* p, const double* vals, double mu, double* X, 
         sm_status_t s = build_gather_list(p, st);
         if (s) return s;
     }
-    SM_CUDA(cudaMemsetAsync(p->d_gersh, 0, (size_t)p->ngroups * 8, st));
+    SM_CUDA(cudaMemsetAsync(p->d_gersh, 0, (size_t)p->ngroups * 16, st));  // Gershgorin bounds + squared column norms
     if (p->gather_smem > 48 * 1024) {
         SM_CUDA(cudaFuncSetAttribute(k_gather<uint16_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));
         SM_CUDA(cudaFuncSetAttribute(k_gather<uint16_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->gather_smem));

@@ -643,13 +643,12 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
 sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
                            double* bufY, cudaStream_t st, int which, double* bufW) {
     if (p->n_tiles == 0) return SM_OK;
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!p->ns_attr_set) {  // per plan: the attribute belongs to the device the plan was created on
         SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
-        attr_set = true;
+        p->ns_attr_set = 1;
     }
     NsArgs a;
     a.tiles = p->d_tiles; a.gersh = p->d_gersh;

@@ -515,13 +515,12 @@ sm_status_t launch_to_f64(sm_plan* p, double* buf0, const double* buf1, const do
 sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, double* buf0, double* buf1,
                                 double* bufY, cudaStream_t st, int which) {
     if (p->n_tiles32 == 0) return SM_OK;
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!p->tf32_attr_set) {  // per plan: the attribute belongs to the device the plan was created on
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
-        attr_set = true;
+        p->tf32_attr_set = 1;
     }
     float* X[2] = {reinterpret_cast<float*>(buf1), reinterpret_cast<float*>(bufY)};
     float* Y = reinterpret_cast<float*>(buf0);

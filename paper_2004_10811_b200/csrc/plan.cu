@@ -23,65 +23,113 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
     return v;
 }
 
-// Marks the row blocks of group g in the shared bitmap.
-__device__ void mark_rows(uint32_t* bitmap, int words, const int64_t* colptr, const int32_t* rowidx,
-                          const int32_t* grp_ptr, const int32_t* grp_cols, int g) {
-    for (int w = threadIdx.x; w < words; w += blockDim.x) bitmap[w] = 0u;
-    __syncthreads();
-    for (int gc = grp_ptr[g]; gc < grp_ptr[g + 1]; ++gc) {
-        int c = grp_cols[gc];
-        for (int64_t p = colptr[c] + threadIdx.x; p < colptr[c + 1]; p += blockDim.x) {
-            int r = rowidx[p];
-            atomicOr(&bitmap[r >> 5], 1u << (r & 31));
+// In-place bitonic sort of P (a power of two) keys in shared memory by the whole CTA.
+__device__ void bitonic_sort_smem(int32_t* key, int P) {
+    for (int k = 2; k <= P; k <<= 1)
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = threadIdx.x; i < P; i += blockDim.x) {
+                const int l = i ^ j;
+                if (l > i) {
+                    const int a = key[i], b = key[l];
+                    if ((a > b) == ((i & k) == 0)) { key[i] = b; key[l] = a; }
+                }
+            }
+            __syncthreads();
         }
-    }
-    __syncthreads();
 }
 
-// Block-wide exclusive scan of (cnt, size) pairs over one chunk of blockDim words; returns the
-// exclusive prefix for this thread and adds the chunk totals to the running carries.
-__device__ void block_scan2(int cnt, int sz, int& ex_cnt, int& ex_sz, int& carry_cnt, int& carry_sz,
-                            int* s_w /*[2*32]*/) {
-    int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    int ic = warp_incl_scan(cnt, lane), is = warp_incl_scan(sz, lane);
-    if (lane == 31) { s_w[wid] = ic; s_w[32 + wid] = is; }
+// CTA-wide exclusive scan of one value per thread (chunk of blockDim values); returns the exclusive
+// prefix and adds the chunk total to `carry` (uniform).  s_w: 32 ints of shared scratch.
+__device__ int block_excl_scan(int v, int& carry, int* s_w) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int inc = warp_incl_scan(v, lane);
+    if (lane == 31) s_w[wid] = inc;
     __syncthreads();
-    int bc = 0, bsz = 0, tc = 0, tsz = 0;
+    int before = 0, total = 0;
     for (int w = 0; w < nw; ++w) {
-        if (w < wid) { bc += s_w[w]; bsz += s_w[32 + w]; }
-        tc += s_w[w]; tsz += s_w[32 + w];
+        if (w < wid) before += s_w[w];
+        total += s_w[w];
     }
-    ex_cnt = carry_cnt + bc + ic - cnt;
-    ex_sz = carry_sz + bsz + is - sz;
-    carry_cnt += tc;
-    carry_sz += tsz;
+    const int ex = carry + before + inc - v;
+    carry += total;
     __syncthreads();
+    return ex;
 }
 
-__global__ void k_index_count(int nb, const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
-                              const int32_t* __restrict__ rowidx, const int32_t* __restrict__ grp_ptr,
-                              const int32_t* __restrict__ grp_cols, int32_t* __restrict__ sub_cnt,
-                              int32_t* __restrict__ sub_dim) {
-    extern __shared__ uint32_t bitmap[];
-    __shared__ int s_w[64];
-    const int g = blockIdx.x, words = (nb + 31) >> 5;
-    mark_rows(bitmap, words, colptr, rowidx, grp_ptr, grp_cols, g);
-    int carry_c = 0, carry_s = 0;
-    for (int base = 0; base < words; base += blockDim.x) {
-        int w = base + threadIdx.x, cnt = 0, sz = 0;
-        if (w < words) {
-            uint32_t bits = bitmap[w];
-            cnt = __popc(bits);
-            while (bits) {
-                int b = __ffs(bits) - 1;
-                bits &= bits - 1;
-                sz += blk_size[(w << 5) + b];
+// Sort key[0..fill) and drop duplicates in place; returns the number of distinct keys (uniform).
+// Compaction runs chunk by chunk in ascending order: an element only ever moves to a position at or
+// below its own, and every chunk has its keys in registers before it writes.
+__device__ int sort_unique_smem(int32_t* key, int fill, int* s_w) {
+    int P = 2;
+    while (P < fill) P <<= 1;
+    for (int i = fill + threadIdx.x; i < P; i += blockDim.x) key[i] = INT32_MAX;
+    __syncthreads();
+    bitonic_sort_smem(key, P);
+    int u = 0;
+    for (int base = 0; base < fill; base += blockDim.x) {
+        const int i = base + threadIdx.x;
+        int cur = INT32_MAX, keep = 0;
+        if (i < fill) {
+            cur = key[i];
+            keep = (i == 0 || key[i - 1] != cur) ? 1 : 0;
+        }
+        __syncthreads();
+        const int pos = block_excl_scan(keep, u, s_w);
+        if (keep) key[pos] = cur;
+        __syncthreads();
+    }
+    return u;
+}
+
+// a2, pass 1: S_i = ascending union of the row lists of the group's block columns (L125, L199), by
+// SORTING -- work proportional to the group's own stored blocks, independent of nb: the lists are
+// appended to a shared buffer of `cap` keys behind the union found so far; when the next list does not
+// fit, and at the end, the buffer is sorted and deduplicated.  Output: scratch[eptr[g] ..] (eptr =
+// exclusive prefix of the groups' stored-block counts, so the scratch holds nnzb keys) and sub_cnt[g].
+__global__ void __launch_bounds__(256)
+k_index_union(const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx,
+              const int32_t* __restrict__ grp_ptr, const int32_t* __restrict__ grp_cols,
+              const int64_t* __restrict__ eptr, int cap, int32_t* __restrict__ scratch,
+              int32_t* __restrict__ sub_cnt, int32_t* __restrict__ err) {
+    extern __shared__ int32_t key[];
+    __shared__ int s_w[32];
+    const int g = blockIdx.x;
+    int u = 0, fill = 0;
+    for (int gc = grp_ptr[g]; gc < grp_ptr[g + 1]; ++gc) {
+        const int c = grp_cols[gc];
+        const int64_t p0 = colptr[c];
+        const int len = (int)(colptr[c + 1] - p0);
+        if (fill + len > cap) {
+            if (fill > u) { u = sort_unique_smem(key, fill, s_w); fill = u; }
+            if (fill + len > cap) {  // more member blocks than one pass holds: unsupported size
+                if (threadIdx.x == 0) { atomicExch(err, 2); sub_cnt[g] = 0; }
+                return;
             }
         }
-        int ec, es;
-        block_scan2(cnt, sz, ec, es, carry_c, carry_s, s_w);
+        for (int t = threadIdx.x; t < len; t += blockDim.x) key[fill + t] = rowidx[p0 + t];
+        fill += len;
+        __syncthreads();
     }
-    if (threadIdx.x == 0) { sub_cnt[g] = carry_c; sub_dim[g] = carry_s; }
+    if (fill > u) u = sort_unique_smem(key, fill, s_w);
+    int32_t* out = scratch + eptr[g];
+    for (int t = threadIdx.x; t < u; t += blockDim.x) out[t] = key[t];
+    if (threadIdx.x == 0) sub_cnt[g] = u;
+}
+
+// Exclusive prefix sum of n int32 counts into n + 1 int64 offsets by one CTA (fixed order; plan time).
+__global__ void __launch_bounds__(1024) k_excl_scan_i32_i64(const int32_t* __restrict__ in, int64_t n,
+                                                            int64_t* __restrict__ out) {
+    __shared__ int s_w[32];
+    int64_t carry = 0;
+    for (int64_t base = 0; base < n; base += blockDim.x) {
+        const int64_t i = base + threadIdx.x;
+        const int v = i < n ? in[i] : 0;
+        int c32 = 0;
+        const int ex = block_excl_scan(v, c32, s_w);
+        if (i < n) out[i] = carry + ex;
+        carry += c32;
+    }
+    if (threadIdx.x == 0) out[n] = carry;
 }
 
 __device__ __forceinline__ int find_sorted(const int32_t* a, int n, int key) {
@@ -94,53 +142,37 @@ __device__ __forceinline__ int find_sorted(const int32_t* a, int n, int key) {
     return -1;
 }
 
-__global__ void k_index_fill(int nb, const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
-                             const int32_t* __restrict__ rowidx, const int32_t* __restrict__ grp_ptr,
-                             const int32_t* __restrict__ grp_cols, const int64_t* __restrict__ sub_ptr,
-                             int32_t* __restrict__ sub_blocks, int32_t* __restrict__ sub_off,
-                             int32_t* __restrict__ gen_pos, int32_t* __restrict__ gen_off,
-                             uint32_t* __restrict__ blk_pack, int32_t* __restrict__ col_grp,
-                             int32_t* __restrict__ gen_width, int32_t* __restrict__ err) {
-    extern __shared__ uint32_t bitmap[];
-    __shared__ int s_w[64];
-    const int g = blockIdx.x, words = (nb + 31) >> 5;
-    mark_rows(bitmap, words, colptr, rowidx, grp_ptr, grp_cols, g);
+// a2, pass 2: members, element offsets (running sum of the block sizes), n_i, and for every generating
+// column its position / offset in S_i and the local row offset of each of its stored blocks.
+__global__ void __launch_bounds__(256)
+k_index_fill(const int32_t* __restrict__ blk_size, const int64_t* __restrict__ colptr,
+             const int32_t* __restrict__ rowidx, const int32_t* __restrict__ grp_ptr,
+             const int32_t* __restrict__ grp_cols, const int64_t* __restrict__ eptr,
+             const int32_t* __restrict__ scratch, const int64_t* __restrict__ sub_ptr,
+             int32_t* __restrict__ sub_blocks, int32_t* __restrict__ sub_off, int32_t* __restrict__ sub_dim,
+             int32_t* __restrict__ gen_pos, int32_t* __restrict__ gen_off, uint32_t* __restrict__ blk_pack,
+             int32_t* __restrict__ col_grp, int32_t* __restrict__ gen_width, int32_t* __restrict__ err) {
+    __shared__ int s_w[32];
+    const int g = blockIdx.x;
     int32_t* S = sub_blocks + sub_ptr[g];
     int32_t* So = sub_off + sub_ptr[g];
     const int m = (int)(sub_ptr[g + 1] - sub_ptr[g]);
-    int carry_c = 0, carry_s = 0;
-    for (int base = 0; base < words; base += blockDim.x) {
-        int w = base + threadIdx.x, cnt = 0, sz = 0;
-        uint32_t bits = 0;
-        if (w < words) {
-            bits = bitmap[w];
-            cnt = __popc(bits);
-            uint32_t t = bits;
-            while (t) {
-                int b = __ffs(t) - 1;
-                t &= t - 1;
-                sz += blk_size[(w << 5) + b];
-            }
-        }
-        int ec, es;
-        block_scan2(cnt, sz, ec, es, carry_c, carry_s, s_w);
-        while (bits) {  // ordered compaction: ascending bit order inside the word
-            int b = __ffs(bits) - 1;
-            bits &= bits - 1;
-            int r = (w << 5) + b;
-            S[ec] = r;
-            So[ec] = es;
-            ++ec;
-            es += blk_size[r];
-        }
+    const int32_t* in = scratch + eptr[g];
+    int carry = 0;
+    for (int base = 0; base < m; base += blockDim.x) {
+        const int t = base + threadIdx.x;
+        int r = 0, sz = 0;
+        if (t < m) { r = in[t]; sz = blk_size[r]; }
+        const int ex = block_excl_scan(sz, carry, s_w);
+        if (t < m) { S[t] = r; So[t] = ex; }
     }
+    if (threadIdx.x == 0) sub_dim[g] = carry;
     __syncthreads();  // S, So of this group are complete and visible to the CTA
-    // position / offset of every generating column, local row offset of each of its blocks
     int gw = 0;
     for (int gc = grp_ptr[g]; gc < grp_ptr[g + 1]; ++gc) {
-        int c = grp_cols[gc];
+        const int c = grp_cols[gc];
         gw += blk_size[c];
-        int pos = find_sorted(S, m, c);
+        const int pos = find_sorted(S, m, c);
         if (threadIdx.x == 0) {
             gen_pos[gc] = pos;
             col_grp[c] = g;
@@ -153,6 +185,12 @@ __global__ void k_index_fill(int nb, const int32_t* __restrict__ blk_size, const
         }
     }
     if (threadIdx.x == 0) gen_width[g] = gw;
+}
+
+sm_status_t launch_excl_scan(const int32_t* in, int64_t n, int64_t* out, cudaStream_t st) {
+    k_excl_scan_i32_i64<<<1, 1024, 0, st>>>(in, n, out);
+    SM_CUDA(cudaGetLastError());
+    return SM_OK;
 }
 
 template <typename T>
@@ -184,33 +222,52 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     if ((s = upload(&p->d_grp_ptr, p->h_grp_ptr.data(), ng + 1, st))) return s;
     if ((s = upload(&p->d_grp_cols, p->h_grp_cols.data(), nb, st))) return s;
 
-    // a2: index builder, pass 1
-    const size_t bm_bytes = (size_t)((nb + 31) / 32) * 4;
-    if (bm_bytes > 200 * 1024) return SM_ERR_INVALID_ARG;  // nb > 1.6 M block rows: bitmap does not fit
-    if (bm_bytes > 48 * 1024) {
-        SM_CUDA(cudaFuncSetAttribute(k_index_count, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bm_bytes));
-        SM_CUDA(cudaFuncSetAttribute(k_index_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bm_bytes));
-    }
-    int32_t* d_cnt = nullptr;
-    SM_CUDA(cudaMalloc((void**)&d_cnt, (size_t)std::max(ng, 1) * 4));
-    SM_CUDA(cudaMalloc((void**)&p->d_sub_dim, (size_t)std::max(ng, 1) * 4));
-    if (ng > 0) k_index_count<<<ng, 256, bm_bytes, st>>>(nb, p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr,
-                                            p->d_grp_cols, d_cnt, p->d_sub_dim);
-    p->launches++;
-    std::vector<int32_t> cnt(ng);
-    p->h_sub_dim.resize(ng);
-    SM_CUDA(cudaMemcpyAsync(cnt.data(), d_cnt, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
-    SM_CUDA(cudaMemcpyAsync(p->h_sub_dim.data(), p->d_sub_dim, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
-    SM_CUDA(cudaStreamSynchronize(st));
-    cudaFree(d_cnt);
-    p->h_sub_ptr.assign(ng + 1, 0);
-    p->max_sub_blocks = 0;
+    // a2: index builder.  eptr = exclusive prefix of the groups' stored-block counts (every block column is
+    // in exactly one group, so the scratch of pass 1 holds nnzb keys); O(nb) integers on the host.
+    std::vector<int64_t> eptr(ng + 1, 0);
+    int64_t max_e = 1;
     for (int i = 0; i < ng; ++i) {
-        p->h_sub_ptr[i + 1] = p->h_sub_ptr[i] + cnt[i];
-        p->max_sub_blocks = std::max(p->max_sub_blocks, cnt[i]);
+        int64_t e = 0;
+        for (int q = p->h_grp_ptr[i]; q < p->h_grp_ptr[i + 1]; ++q)
+            e += p->h_colptr[p->h_grp_cols[q] + 1] - p->h_colptr[p->h_grp_cols[q]];
+        eptr[i + 1] = eptr[i] + e;
+        max_e = std::max(max_e, e);
     }
-    const int64_t tot = p->h_sub_ptr[ng];
-    if ((s = upload(&p->d_sub_ptr, p->h_sub_ptr.data(), ng + 1, st))) return s;
+    int cap = 256;  // keys of one sort pass in shared memory: enough for the largest group, at most 32768 (128 KB)
+    while (cap < max_e && cap < 32768) cap <<= 1;
+    const size_t key_bytes = (size_t)cap * 4;
+    if (key_bytes > 48 * 1024)
+        SM_CUDA(cudaFuncSetAttribute(k_index_union, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)key_bytes));
+    DevTmp cnt_tmp, err_tmp, eptr_tmp, scratch_tmp;
+    SM_CUDA(cudaMalloc(&cnt_tmp.p, (size_t)std::max(ng, 1) * 4));
+    SM_CUDA(cudaMalloc(&err_tmp.p, 4));
+    SM_CUDA(cudaMalloc(&eptr_tmp.p, (size_t)(ng + 1) * 8));
+    SM_CUDA(cudaMalloc(&scratch_tmp.p, (size_t)std::max<int64_t>(p->nnzb, 1) * 4));
+    int32_t* d_cnt = (int32_t*)cnt_tmp.p;
+    int32_t* d_err = (int32_t*)err_tmp.p;
+    int64_t* d_eptr = (int64_t*)eptr_tmp.p;
+    int32_t* d_scratch = (int32_t*)scratch_tmp.p;
+    SM_CUDA(cudaMemcpyAsync(d_eptr, eptr.data(), (size_t)(ng + 1) * 8, cudaMemcpyHostToDevice, st));
+    SM_CUDA(cudaMemsetAsync(d_err, 0, 4, st));
+    SM_CUDA(cudaMalloc((void**)&p->d_sub_ptr, (size_t)(ng + 1) * 8));
+    SM_CUDA(cudaMalloc((void**)&p->d_sub_dim, (size_t)std::max(ng, 1) * 4));
+    cudaEvent_t ev[4];
+    for (auto& e : ev) SM_CUDA(cudaEventCreate(&e));
+    struct EvFree { cudaEvent_t* e; ~EvFree() { for (int i = 0; i < 4; ++i) cudaEventDestroy(e[i]); } } ev_free{ev};
+    // pass 1: sorted unions + their sizes, device prefix sum
+    SM_CUDA(cudaEventRecord(ev[0], st));
+    if (ng > 0) k_index_union<<<ng, 256, key_bytes, st>>>(p->d_colptr, p->d_rowidx, p->d_grp_ptr, p->d_grp_cols, d_eptr,
+                                                          cap, d_scratch, d_cnt, d_err);
+    k_excl_scan_i32_i64<<<1, 1024, 0, st>>>(d_cnt, ng, p->d_sub_ptr);
+    SM_CUDA(cudaEventRecord(ev[1], st));
+    p->launches += 2;
+    int64_t tot = 0;
+    int32_t herr = 0;
+    SM_CUDA(cudaMemcpyAsync(&tot, p->d_sub_ptr + ng, 8, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaMemcpyAsync(&herr, d_err, 4, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));  // the only host round trip of the build: 12 bytes, to size the index
+    SM_CUDA(cudaGetLastError());
+    if (herr == 2) return SM_ERR_INVALID_ARG;  // a submatrix with more member blocks than one sort pass holds
     SM_CUDA(cudaMalloc((void**)&p->d_sub_blocks, std::max<int64_t>(tot, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_sub_off, std::max<int64_t>(tot, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_gen_pos, (size_t)std::max(nb, 1) * 4));
@@ -218,21 +275,29 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMalloc((void**)&p->d_col_grp, (size_t)std::max(nb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_blk_pack, std::max<int64_t>(p->nnzb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_gen_width, (size_t)std::max(ng, 1) * 4));
-    int32_t* d_err = nullptr;
-    SM_CUDA(cudaMalloc((void**)&d_err, 4));
-    SM_CUDA(cudaMemsetAsync(d_err, 0, 4, st));
     // pass 2
-    if (ng > 0) k_index_fill<<<ng, 256, bm_bytes, st>>>(nb, p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr,
-                                           p->d_grp_cols, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off,
-                                           p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_col_grp,
-                                           p->d_gen_width, d_err);
+    SM_CUDA(cudaEventRecord(ev[2], st));
+    if (ng > 0) k_index_fill<<<ng, 256, 0, st>>>(p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr, p->d_grp_cols,
+                                                 d_eptr, d_scratch, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off,
+                                                 p->d_sub_dim, p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_col_grp,
+                                                 p->d_gen_width, d_err);
+    SM_CUDA(cudaEventRecord(ev[3], st));
     p->launches++;
-    int32_t herr = 0;
+    p->h_sub_dim.resize(ng);
+    p->h_sub_ptr.assign(ng + 1, 0);
     SM_CUDA(cudaMemcpyAsync(&herr, d_err, 4, cudaMemcpyDeviceToHost, st));
-    SM_CUDA(cudaStreamSynchronize(st));
-    cudaFree(d_err);
+    if (ng) SM_CUDA(cudaMemcpyAsync(p->h_sub_dim.data(), p->d_sub_dim, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaMemcpyAsync(p->h_sub_ptr.data(), p->d_sub_ptr, (size_t)(ng + 1) * 8, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));  // sizes for the workspace geometry and tile list below
     SM_CUDA(cudaGetLastError());
     if (herr) return SM_ERR_STRUCTURE;
+    float ms1 = 0.f, ms2 = 0.f;
+    cudaEventElapsedTime(&ms1, ev[0], ev[1]);
+    cudaEventElapsedTime(&ms2, ev[2], ev[3]);
+    p->ms_index_kernels = ms1 + ms2;
+    p->max_sub_blocks = 0;
+    for (int i = 0; i < ng; ++i)
+        p->max_sub_blocks = std::max<int32_t>(p->max_sub_blocks, (int32_t)(p->h_sub_ptr[i + 1] - p->h_sub_ptr[i]));
 
     // workspace geometry (group order, keeps the locality of consecutive submatrices, L188) and
     // the GEMM tile list, largest padded size first (size buckets = equal ld).
@@ -304,6 +369,10 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     }
     I.sum_n3_columns = n3c;
     I.est_speedup = n3 > 0 ? (double)n3c / (double)n3 : 0.0;
+    I.ms_index_kernels = p->ms_index_kernels;
+    // the pattern is read once (nnzb x 4), members and offsets (sum |S_i| x 8) and the packed
+    // block records (nnzb x 4) are written
+    I.index_alg_bytes = p->nnzb * 8 + tot * 8;
     return SM_OK;
 }
 

@@ -3,9 +3,15 @@
 // and  rho(a_i - mu I) <= max(|lambda_max(K~) - mu|, |lambda_min(K~) - mu|)  for EVERY submatrix and
 // EVERY mu of the bisection.  The two extreme eigenvalues of the block-sparse K~ are estimated once
 // per call by a short Lanczos run (block-CSC mat-vec, deterministic reductions) and widened by a
-// safety margin; Newton-Schulz converges for any rho/s < sqrt(3), so the margin guards iteration
-// counts, not correctness (reading A8).  All arithmetic runs on the device; the host
-// only sequences the launches and reads the two resulting doubles.
+// safety margin.  The Ritz extremes approach the true ones from INSIDE, so the cap is an estimate, not
+// a bound: Newton-Schulz tolerates rho/s < sqrt(3) (1.15 beyond the largest overshoot), and three
+// guards keep the estimate from going below that (reading A8): (i) a run that breaks down
+// (beta_j <= 1e-10 of the scale of T before the last step: the start vector lies in an invariant
+// subspace) is discarded -- the call then uses the rigorous Gershgorin bounds only, no interlacing
+// bracket, no quadrature guess; (ii) the cap of a submatrix is never taken below a rigorous LOWER bound
+// of its spectral radius (largest column 2-norm of a_i - mu I, from the gather); (iii) s_i never exceeds
+// the submatrix's own Gershgorin bound.  All arithmetic runs on the device; the host only sequences
+// the launches and reads the resulting doubles.
 #include "common.cuh"
 
 namespace smb {
@@ -147,17 +153,21 @@ __global__ void k_lz_start(int64_t n, double* __restrict__ v, double* __restrict
 // extreme Ritz values widened by margin * spread (interlacing bound, bisection bracket); out[2 + j]:
 // Ritz values ascending; out[2 + 32 + j]: cumulative weights = the start vector's estimate of the
 // fraction of eigenvalues of K~ below the node (used for the first interior step of the mu search,
-// DESIGN.md reading A11d).  One warp; k <= 32.
+// DESIGN.md reading A11d); out[66] = 1.0 if the recurrence broke down (some beta_i, i < k - 1, not above
+// 1e-10 of the largest entry of T: everything after it is rounding noise), else 0.0.  One warp; k <= 32.
 __global__ void k_lz_quadrature(int k, const double* __restrict__ alpha, const double* __restrict__ beta,
                                 double margin, double* __restrict__ out) {
     __shared__ double th[32], wt[32];
     const int j = threadIdx.x;
-    double glo = 1e300, ghi = -1e300;
+    double glo = 1e300, ghi = -1e300, tscale = 0.0;
     for (int i = 0; i < k; ++i) {
         const double r = (i > 0 ? fabs(beta[i - 1]) : 0.0) + (i + 1 < k ? fabs(beta[i]) : 0.0);
         glo = fmin(glo, alpha[i] - r);
         ghi = fmax(ghi, alpha[i] + r);
+        tscale = fmax(tscale, fmax(fabs(alpha[i]), i + 1 < k ? fabs(beta[i]) : 0.0));
     }
+    bool broken = false;
+    for (int i = 0; i + 1 < k; ++i) broken = broken || !(fabs(beta[i]) > 1e-10 * tscale);
     auto count_below = [&](double x) {  // eigenvalues of T smaller than x
         int cnt = 0;
         double d = 1.0;
@@ -201,19 +211,24 @@ __global__ void k_lz_quadrature(int k, const double* __restrict__ alpha, const d
             out[2 + i] = i < k ? th[i] : th[k - 1];
             out[2 + 32 + i] = i < k ? cum : 1.0;
         }
+        out[66] = broken ? 1.0 : 0.0;
     }
 }
 
-// s_g <- min(Gershgorin_g, cap) / overshoot  (in place, bits of a double as written by k_gather).
+// s_g <- min(Gershgorin_g, max(cap, rho_lo_g)) / overshoot  (in place, bits of a double as written by
+// k_gather; rho_lo_g = largest column 2-norm of a_g - mu I, a rigorous lower bound of its spectral radius:
+// the estimated cap is never taken below it).
 // With alpha != null (reading A8b) the overshoot is not applied; instead iteration 0 works on al_0 X_0 with
 // al_0 = min(sqrt(3 / (1 + l + l^2)), 1.5), l = ell_abs / s_g the estimated smallest eigenvalue modulus of X_0
 // (1.5: the same safety against an underestimated bound as the overshoot limit of reading A8).
-__global__ void k_apply_scale(int ng, unsigned long long* __restrict__ gersh, double cap, double inv_overshoot,
+__global__ void k_apply_scale(int ng, unsigned long long* __restrict__ gersh,
+                              const unsigned long long* __restrict__ col2, double cap, double inv_overshoot,
                               double ell_abs, double* __restrict__ alpha, double* __restrict__ lmin) {
     const int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ng) return;
     double s = __longlong_as_double((long long)gersh[g]);
-    if (cap > 0.0 && cap < s) s = cap;
+    const double c = fmax(cap, sqrt(__longlong_as_double((long long)col2[g])));
+    if (cap > 0.0 && c < s) s = c;
     if (alpha) {
         double l = s > 0.0 ? ell_abs / s : 1.0;
         l = fmin(fmax(l, 1e-4), 1.0);
@@ -228,7 +243,8 @@ __global__ void k_apply_scale(int ng, unsigned long long* __restrict__ gersh, do
 sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, double ell_abs, cudaStream_t st) {
     if (p->ngroups == 0) return SM_OK;
     const bool resc = rescale_on(p);
-    k_apply_scale<<<(p->ngroups + 255) / 256, 256, 0, st>>>(p->ngroups, p->d_gersh, cap, 1.0 / overshoot, ell_abs,
+    k_apply_scale<<<(p->ngroups + 255) / 256, 256, 0, st>>>(p->ngroups, p->d_gersh, p->d_gersh + p->ngroups, cap,
+                                                            1.0 / overshoot, ell_abs,
                                                             resc ? p->d_alpha : nullptr, resc ? p->d_lmin : nullptr);
     p->launches++;
     SM_CUDA(cudaGetLastError());
@@ -265,11 +281,13 @@ sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t s
     k_lz_quadrature<<<1, 32, 0, st>>>(steps, alpha, beta, 0.03, outp);
     p->launches++;
     SM_CUDA(cudaGetLastError());
-    SM_CUDA(cudaMemcpyAsync(p->h_lz, outp, 66 * 8, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaMemcpyAsync(p->h_lz, outp, 67 * 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));
     p->lz_lo = p->h_lz[0];
     p->lz_hi = p->h_lz[1];
     p->lz_nodes = steps;
+    // a broken-down or non-finite run is discarded: Gershgorin bounds only for this call (reading A8)
+    p->lz_ok = (p->h_lz[66] == 0.0 && p->lz_lo == p->lz_lo && p->lz_hi == p->lz_hi && p->lz_lo <= p->lz_hi) ? 1 : 0;
     return SM_OK;
 }
 

@@ -143,18 +143,41 @@ def test_config0_full_parity(B, oracle, cfg0):
     B.sm_plan_destroy(plan); B.sm_plan_destroy(plan2)
 
 
-@pytest.mark.parametrize("mu", [-0.9, 0.11])
+@pytest.mark.parametrize("mu", [-0.464, -1.6847, 0.11])
 def test_config0_shifted_mu(B, oracle, cfg0, mu):
-    """mu inside the occupied band: slow convergence, still parity where eigenvalues are not at mu."""
+    """mu inside the occupied band (in holes of the union of the submatrix spectra, half-width 0.013 and
+    0.008) and inside the gap: the library must converge (SM_OK) and meet the 1e-9 bar."""
     m = cfg0
     plan, st, d_gpu, stats, _, _ = _run_sign(B, m, mu=mu)
     idx = oracle.Index(m)
     d_or = oracle.density(idx, m.values, mu)
     lam, w, ptr, g = oracle.eig_groups(idx, m.values)
-    gap = np.abs(lam - mu).min()
-    assert st in (B.SM_OK, B.SM_WARN_SIGN_NOT_CONVERGED)
-    if st == B.SM_OK:
-        assert np.abs(d_gpu - d_or).max() <= max(TOL_D, 1e-13 / gap)
+    assert np.abs(lam - mu).min() > 5e-3  # the case is well conditioned: the plain bar applies
+    assert st == B.SM_OK and stats.not_converged == 0 and stats.max_residual < EPS
+    assert np.abs(d_gpu - d_or).max() <= TOL_D
+    B.sm_plan_destroy(plan)
+
+
+def test_config0_ill_conditioned_mu(B, oracle, cfg0):
+    """mu = -0.9 lies 4.7e-6 from an eigenvalue of one submatrix.  DESIGN.md reading A17: the sign function
+    has condition number ~ 1/min|lambda - mu| there, BOTH sides (Jacobi eigenvectors, Newton-Schulz) carry
+    rounding errors of that size, so the comparison bar is max(1e-9, 1e-13 / gap); what is asserted without
+    loosening: the status (converged inside max_iter: the eigenvalue is small, not zero), the residual, and
+    the plain 1e-9 bar on every block column whose own submatrix is well conditioned."""
+    m, mu = cfg0, -0.9
+    plan, st, d_gpu, stats, _, _ = _run_sign(B, m, mu=mu)
+    idx = oracle.Index(m)
+    d_or = oracle.density(idx, m.values, mu)
+    lam, w, ptr, g = oracle.eig_groups(idx, m.values)
+    gaps = np.array([np.abs(lam[ptr[i]:ptr[i + 1]] - mu).min() for i in range(idx.ngroups)])
+    assert gaps.min() < 1e-5
+    assert st == B.SM_OK and stats.not_converged == 0 and stats.max_residual < EPS
+    err = np.abs(d_gpu - d_or)
+    assert err.max() <= max(TOL_D, 1e-13 / gaps.min())
+    good = np.nonzero(gaps > 1e-3)[0].astype(np.int32)
+    assert len(good) >= idx.ngroups // 2
+    mask, _ = _column_mask(idx, m, good)
+    assert err[mask].max() <= TOL_D
     B.sm_plan_destroy(plan)
 
 
@@ -247,7 +270,7 @@ def test_config4_density_matrix_as_benchmarked(B, oracle):
             else: hi = min(hi, muk)
     assert stats.ne_err_trace[n - 1] == 0.0 and abs(stats.mu_trace[n - 1] - mu) == 0.0
     idx = oracle.Index(m)
-    groups = _sample_groups(idx, 8, seed=1)
+    groups = _sample_groups(idx, 64, seed=1)  # >= 64 groups incl. min / median / max dimension
     d_or = oracle.density(idx, m.values, mu, groups)
     mask, cols = _column_mask(idx, m, groups)
     assert np.abs(d_gpu - d_or)[mask].max() <= TOL_D
@@ -276,6 +299,8 @@ def test_ragged_blocks_and_scattered_groups(B, oracle):
         lam, _, _, _ = oracle.eig_groups(idx, m.values)
         gap = np.abs(lam - 0.05).min()
         assert st == B.SM_OK
+        # random patterns put eigenvalues of tiny submatrices anywhere: bar of reading A17 (conditioning of
+        # sign at min|lambda - mu|); it IS the plain 1e-9 bar whenever gap >= 1e-4
         assert np.abs(d_gpu - d_or).max() <= max(TOL_D, 1e-13 / gap)
         B.sm_plan_destroy(plan)
 
@@ -413,21 +438,22 @@ def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling, m
             assert abs(stats.mu_guess - guess_o) <= 1e-8
         else:
             assert stats.mu_guess != stats.mu_guess  # NaN: not computed
+        # the oracle runs in ITS OWN bracket (nothing the CUDA path reported enters an oracle call)
+        blo, bhi = (max(lo, llo), min(hi, lhi)) if scaling == 1 else (lo, hi)
         start_o = mu0
-        if mu_guess and mu_start:  # A11e: the oracle's own rule, in the bracket the library reports
-            start_o = oracle.mu_start(th, wq, m.n_occ / m.n_basis, mu0, stats.bracket_lo, stats.bracket_hi)
+        if mu_guess and mu_start:  # A11e: the oracle's own rule
+            start_o = oracle.mu_start(th, wq, m.n_occ / m.n_basis, mu0, blo, bhi)
             assert start_o == guess_o
-        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, start_o, stats.bracket_lo, stats.bracket_hi,
-                                               tol_n, mu_first=guess_o)
+        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, start_o, blo, bhi, tol_n, mu_first=guess_o)
         assert st == B.SM_OK
         assert stats.mu_steps == len(trace_o)
         if mu_guess:
             assert stats.mu_steps == (1 if mu_start else 2)  # the guess lies in the gap of this workload
         n_partial = 0
         for k, (mo, no) in enumerate(trace_o):
-            # same bracket and midpoints; the guess agrees to the rounding of two Lanczos runs
-            from_guess = mu_guess and (k >= 1 or mu_start)
-            assert abs(stats.mu_trace[k] - mo) <= (1e-8 if from_guess else 1e-12 * max(1, abs(mo)))
+            # two independent Lanczos runs (bracket ends, guess) agree to 1e-8; step 0 at the caller's mu is exact
+            exact = (k == 0 and not (mu_guess and mu_start))
+            assert abs(stats.mu_trace[k] - mo) <= (1e-12 * max(1, abs(mo)) if exact else 1e-8)
             err = stats.ne_err_trace[k]
             if err > 0.0:  # steering step: proven side, converged count inside the bound
                 n_partial += 1
@@ -457,8 +483,8 @@ def test_density_matrix_bisection_config0(B, oracle, cfg0, early_out, scaling, m
         st, mu = B.sm_density_matrix(plan, vin, float(m.n_occ), 0.5, EPS, mu_in, vout, ws, stats)
         torch.cuda.synchronize()
         assert stats.mu_trace[0] == mu_in
-        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu_in, stats.bracket_lo, stats.bracket_hi, 0.5,
-                                               mu_first=guess_o)
+        blo, bhi = (max(lo, llo), min(hi, lhi)) if scaling == 1 else (lo, hi)
+        mu_o, ne_o, trace_o = oracle.bisect_mu(idx, lam, w, g, m.n_occ, mu_in, blo, bhi, 0.5, mu_first=guess_o)
         assert st == B.SM_OK and stats.mu_steps == len(trace_o) and abs(stats.n_elec - ne_o) <= 1e-9
         assert np.abs(vout.cpu().numpy() - oracle.density(idx, m.values, mu)).max() <= TOL_D
         B.sm_plan_destroy(plan)
@@ -646,3 +672,83 @@ def test_host_buffer_entry_point(B, oracle, cfg0):
     assert np.abs(hout.numpy() - oracle.density(idx, m.values, 0.0)).max() <= TOL_D
     assert B.sm_launch_count(plan) > 4
     B.sm_plan_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ large submatrices
+def test_large_submatrix_parity_n1104(B, oracle):
+    """n > 1024 (verdict r1): 48 H2O DZVP with a cutoff of 10 A, above half the cell diagonal, so every
+    S_i holds all 144 atom blocks and every a_i is the whole 1104-dim K~ (P5): ld = 1104 means 18 x 18 tile
+    grids (171 tiles per matrix, the last row tile ragged with 16 rows), `tij` packing and large scatter
+    offsets at work.  Two witnesses: the Jacobi oracle on two groups (~1 core-minute each), and -- the
+    method being exact here (L125) -- LAPACK's spectral projector of the dense K~ on EVERY column."""
+    m = W.water_like(48, "DZVP", 10.0, seed=4)
+    plan, st, d_gpu, stats, ws, vin = _run_sign(B, m)
+    assert st == B.SM_OK and stats.not_converged == 0 and stats.max_residual < EPS
+    info = B.sm_plan_query(plan)
+    assert info.dim_min == 1104 and info.dim_max == 1104 and info.ngroups == 48
+    idx = _check_index(B, oracle, m, plan)
+    groups = np.array([0, 33], dtype=np.int32)
+    d_or = oracle.density(idx, m.values, 0.0, groups, nthreads=2)
+    mask, cols = _column_mask(idx, m, groups)
+    assert np.abs(d_gpu - d_or)[mask].max() <= TOL_D
+    td_o, tdk_o = oracle.traces(idx, d_or, m.values, cols)
+    td_g, tdk_g = oracle.traces(idx, d_gpu, m.values, cols)
+    assert abs(tdk_g - tdk_o) / abs(tdk_o) <= TOL_E
+    lam, U = np.linalg.eigh(m.to_dense())
+    occ = U[:, lam < 0.0]
+    assert np.abs(m.to_dense(d_gpu) - occ @ occ.T).max() <= TOL_D  # all 1104 columns, second witness
+    td_all, tdk_all = B.sm_trace_dk(plan, _torch().from_numpy(d_gpu).cuda(), vin)
+    assert abs(td_all - m.n_occ) <= 1e-9 and abs(tdk_all - lam[lam < 0.0].sum()) <= TOL_E * abs(tdk_all)
+    B.sm_plan_destroy(plan)
+
+
+def test_config4_reduced_precision_full_size(B, oracle):
+    """BASELINE config 4: "plus the reduced-precision tensor-core variant run on the same input".
+    precision = 2 (3xTF32 on tcgen05, THE reduced-precision variant of include/submatrix.h) at full size
+    against the ORACLE on 64 sampled groups: <= 1e-3 elementwise (north_star), its band-energy error
+    asserted and printed."""
+    m = W.make_config(4)
+    plan, st, d_gpu, stats, ws, vin = _run_sign(B, m, eps=2e-6, opt=B.default_options(precision=2))
+    assert st == B.SM_OK, (st, stats.not_converged, stats.max_residual)
+    idx = oracle.Index(m)
+    groups = _sample_groups(idx, 64, seed=2)
+    d_or = oracle.density(idx, m.values, 0.0, groups)
+    mask, cols = _column_mask(idx, m, groups)
+    err = np.abs(d_gpu - d_or)[mask].max()
+    td_o, tdk_o = oracle.traces(idx, d_or, m.values, cols)
+    td_g, tdk_g = oracle.traces(idx, d_gpu, m.values, cols)
+    e_rel = abs(tdk_g - tdk_o) / abs(tdk_o)
+    print(f"precision=2 config 4: max|D - D_oracle| = {err:.3e} on 64 groups, rel. band-energy error = {e_rel:.3e}, "
+          f"n_elec = {stats.n_elec:.4f}")
+    assert err <= 1e-3 and e_rel <= 1e-4
+    assert np.all(np.isfinite(d_gpu)) and abs(stats.n_elec - m.n_occ) < 1.0
+    B.sm_plan_destroy(plan)
+
+
+# ------------------------------------------------------------------------------ Lanczos breakdown
+def test_lanczos_breakdown_falls_back_to_gershgorin(B, oracle):
+    """Advisor finding r1: with default options the interlacing cap comes from a Lanczos run whose hashed
+    +-1 start vector can lie in an invariant subspace (K = [[0,1],[1,0]]: start (-,-)/sqrt2 is an
+    eigenvector, Ritz values {1,1}); an unguarded cap of 0.7 at mu = 0.3 is below rho = 1.3 and flips a sign.
+    The run must be discarded (no spec interval reported) and the result must be the oracle's."""
+    cases = [(np.array([[0.0, 1.0], [1.0, 0.0]]), 0.3), (np.array([[1.0, 2.0], [2.0, 1.0]]), 0.5),
+             (np.kron(np.eye(4), np.array([[0.0, 1.0], [1.0, 0.0]])), -0.2),
+             (np.diag([1.0, 1.0, 1.0, -1.0, -1.0, 2.0]), 0.4)]
+    for a, mu in cases:
+        m = W.dense_batch_as_blocks(a[None])
+        plan, st, d, stats, ws, vin = _run_sign(B, m, mu=mu)
+        n = a.shape[0]
+        lam, U = np.linalg.eigh(a)
+        expect = 0.5 * (np.eye(n) - (U * np.sign(lam - mu)) @ U.T)
+        assert st == B.SM_OK, (a, mu, st)
+        assert np.abs(d.reshape(n, n) - expect).max() <= TOL_D, (a, mu)
+        idx = oracle.Index(m)
+        assert np.abs(d - oracle.density(idx, m.values, mu)).max() <= TOL_D
+        # the bisection bracket must still enclose the spectrum
+        torch = _torch()
+        vout = torch.empty_like(vin)
+        n_t = float((lam < mu).sum())
+        st2, mu2 = B.sm_density_matrix(plan, vin, n_t, 0.25, EPS, mu, vout, ws, stats)
+        assert stats.bracket_lo <= lam.min() and lam.max() <= stats.bracket_hi
+        assert st2 == B.SM_OK and abs(stats.n_elec - n_t) <= 0.25
+        B.sm_plan_destroy(plan)
