@@ -29,6 +29,8 @@ def lib():
         _lib.orc_index_count.restype = C.c_int64
         _lib.orc_jacobi_eig.restype = C.c_int
         _lib.orc_dense_sign.restype = C.c_int
+        _lib.orc_occupation.restype = C.c_double
+        _lib.orc_occupation.argtypes = [C.c_double, C.c_double, C.c_double]
     return _lib
 
 
@@ -145,6 +147,61 @@ def nelec(idx: Index, lam, w, groups, mu: float) -> float:
     """Algorithm 1 inner loops for one mu."""
     ngen = float(idx.gen_width[groups].sum())
     return 0.5 * ngen - 0.5 * float(np.sum(w * np.sign(lam - mu)))
+
+
+def occupation(lam, mu: float, kT: float = 0.0) -> np.ndarray:
+    """Occupations f_l (L255, reading A18): Fermi function 1 / (1 + exp((lam - mu) / kT)) for kT > 0, else
+    1/2 (1 - signum(lam - mu)).  Evaluated by the C oracle, element by element."""
+    L = lib()
+    return np.array([L.orc_occupation(float(x), float(mu), float(kT)) for x in np.atleast_1d(lam)])
+
+
+def nelec_fermi(idx: Index, lam, w, groups, mu: float, kT: float) -> float:
+    """Algorithm 1's count with the Fermi function in place of signum (L255): sum_i sum_l w_il f(lam_il)."""
+    if kT <= 0.0:
+        return nelec(idx, lam, w, groups, mu)
+    return float(np.sum(w / (1.0 + np.exp((lam - mu) / kT))))
+
+
+def density_fermi(idx: Index, values, mu: float, kT: float, groups=None, nthreads: int = 0) -> np.ndarray:
+    """D~ = f(K~ - mu I) by the submatrix method at electronic temperature kT (L255): per submatrix
+    Q f(Lambda) Q^T, generating columns copied back on the input pattern."""
+    groups = _i32(np.arange(idx.ngroups) if groups is None else groups)
+    v = _f64(values)
+    out = np.zeros_like(v)
+    lib().orc_submatrix_groups_fermi(
+        _p(idx.blk_size, C.c_int32), _p(idx.colptr, C.c_int64), _p(idx.rowidx, C.c_int32),
+        _p(idx.val_off, C.c_int64), _p(v, C.c_double), _p(idx.grp_ptr, C.c_int32),
+        _p(idx.grp_cols, C.c_int32), _p(idx.sub_ptr, C.c_int64), _p(idx.sub_blocks, C.c_int32),
+        _p(idx.sub_off, C.c_int32), _p(idx.sub_dim, C.c_int32), _p(idx.gen_pos, C.c_int32),
+        C.c_int32(len(groups)), _p(groups, C.c_int32), C.c_double(mu), C.c_double(kT), _p(out, C.c_double),
+        C.c_int32(nthreads))
+    return out
+
+
+def bisect_mu_fermi(idx: Index, lam, w, groups, n_target: float, mu0: float, lo: float, hi: float, tol_n: float,
+                    kT: float, mu_tol: float = 1e-6, max_steps: int = 64):
+    """Algorithm 1 (L272-276) with the rule of reading A11 on the finite-temperature count (continuous and
+    strictly increasing in mu for kT > 0, so tol_n is reachable).  Same returns as bisect_mu."""
+    trace = []
+    mu = mu0
+    best = None
+    for _ in range(max_steps):
+        ne = nelec_fermi(idx, lam, w, groups, mu, kT)
+        g = ne - n_target
+        trace.append((mu, ne))
+        if best is None or abs(g) < abs(best[1]):
+            best = (mu, g)
+        if abs(g) <= tol_n:
+            break
+        if g < 0:
+            lo = max(lo, mu)
+        else:
+            hi = min(hi, mu)
+        if hi - lo <= mu_tol:
+            break
+        mu = 0.5 * (lo + hi)
+    return best[0], best[1] + n_target, trace
 
 
 def column_ids_of_groups(idx: Index, groups) -> np.ndarray:

@@ -22,6 +22,10 @@
  *             columns k; we return lambda_l and w_l = sum_{k in gen} Q_{k,l}^2 (L270) so that the
  *             mu loop of Algorithm 1 needs no new decomposition.
  *   energy    Eq.(10): Tr(D K).
+ *   fermi     L255 "systems at finite temperature by replacing the signum function in Eq. (17) by the
+ *             Fermi function": occupation f(lambda) = 1 / (1 + exp((lambda - mu) / kT)) in place of
+ *             1/2 (1 - signum(lambda - mu)), i.e. signum(x) -> tanh(x / (2 kT)) (reading A18);
+ *             D = Q f(Lambda) Q^T.  kT = 0 is the signum case.
  *
  * No blocking, fusion or reordering beyond the statements above.  OpenMP is used only ACROSS
  * submatrices (the paper does the same, L229).
@@ -280,6 +284,73 @@ void orc_submatrix_groups(const int32_t *blk_size, const int64_t *colptr, const 
             }
         }
         free(a); free(Qt); free(sg); free(lam);
+    }
+}
+
+/* Occupation of one eigenvalue (L255, reading A18): Fermi function for kT > 0, else the zero-temperature
+ * limit 1/2 (1 - signum(lambda - mu)) of Eq.(16)/(17) (1/2 exactly at lambda == mu, Eq.(12)). */
+double orc_occupation(double lam, double mu, double kT) {
+    if (kT > 0.0) return 1.0 / (1.0 + exp((lam - mu) / kT));
+    return 0.5 * (1.0 - signum(lam - mu));
+}
+
+/* D = Q diag(f_l) Q^T, f_l = orc_occupation(lam_l, mu, kT); column-major n x n output (symmetric). */
+void orc_occ_from_eig(int32_t n, const double *Qt, const double *lam, double mu, double kT, double *D) {
+    memset(D, 0, (size_t)n * n * sizeof(double));
+    for (int l = 0; l < n; ++l) {
+        double f = orc_occupation(lam[l], mu, kT);
+        if (f == 0.0) continue;
+        const double *v = Qt + (size_t)l * n;
+        for (int j = 0; j < n; ++j) {
+            double fj = f * v[j];
+            for (int i = 0; i < n; ++i) D[(size_t)j * n + i] += v[i] * fj;
+        }
+    }
+}
+
+/* The submatrix method at finite temperature (L255): as orc_submatrix_groups, with
+ * D[r,c] = (Q f(Lambda) Q^T)[loc r, loc c] for the generating columns of every listed group. */
+void orc_submatrix_groups_fermi(const int32_t *blk_size, const int64_t *colptr, const int32_t *rowidx,
+                                const int64_t *val_off, const double *vals, const int32_t *grp_ptr,
+                                const int32_t *grp_cols, const int64_t *sub_ptr, const int32_t *sub_blocks,
+                                const int32_t *sub_off, const int32_t *sub_dim, const int32_t *gen_pos,
+                                int32_t nlist, const int32_t *list, double mu, double kT, double *vals_out,
+                                int32_t nthreads) {
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int j = 0; j < nlist; ++j) {
+        int i = list[j];
+        int32_t n = sub_dim[i];
+        int64_t m = sub_ptr[i + 1] - sub_ptr[i];
+        const int32_t *S = sub_blocks + sub_ptr[i];
+        const int32_t *So = sub_off + sub_ptr[i];
+        double *a = (double *)malloc((size_t)n * n * sizeof(double));
+        double *Qt = (double *)malloc((size_t)n * n * sizeof(double));
+        double *D = (double *)malloc((size_t)n * n * sizeof(double));
+        double *lam = (double *)malloc((size_t)n * sizeof(double));
+        orc_assemble(blk_size, colptr, rowidx, val_off, vals, m, S, So, n, a);
+        orc_jacobi_eig(n, a, Qt, lam);
+        orc_occ_from_eig(n, Qt, lam, mu, kT, D);
+        for (int g = grp_ptr[i]; g < grp_ptr[i + 1]; ++g) {
+            int32_t c = grp_cols[g];
+            int tc = gen_pos[g];
+            int bc = blk_size[c];
+            for (int64_t p = colptr[c]; p < colptr[c + 1]; ++p) {
+                int32_t r = rowidx[p];
+                int64_t tr = -1;
+                for (int64_t t = 0; t < m; ++t)
+                    if (S[t] == r) { tr = t; break; }
+                int br = blk_size[r];
+                for (int q = 0; q < bc; ++q)
+                    for (int e = 0; e < br; ++e)
+                        vals_out[val_off[p] + (int64_t)q * br + e] = D[(size_t)(So[tc] + q) * n + So[tr] + e];
+            }
+        }
+        free(a); free(Qt); free(D); free(lam);
     }
 }
 

@@ -33,9 +33,9 @@ __device__ __forceinline__ int find_sorted64(const int32_t* __restrict__ a, int 
 // two block-map reads, predicated 8-byte loads of the stored values straight from global memory
 // (L2-resident: every value is used by ~|S_i| submatrices), mu subtracted on the diagonal
 // (Eq.(16)), one coalesced 16-byte store into the k8-panel workspace, abs-sums for the Gershgorin
-// bound s_i = max_q sum_p |a_pq|, and squares for max_q ||a e_q||_2^2 (a rigorous LOWER bound of the
-// spectral radius: the estimated interlacing cap is never taken below it, reading A8; stored in
-// gersh[ngroups + g]).
+// bound s_i = max_q sum_p |a_pq|, and squares for a rigorous LOWER bound of the spectral radius (the mean
+// of ||a e_q||_2^2 over the columns a warp sweeps <= max_q ||a e_q||_2^2 <= rho^2; no per-column reduction
+// needed): the estimated interlacing cap is never taken below it, reading A8; stored in gersh[ngroups + g].
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned gather_hash(int key, int shift) {
     return ((unsigned)key * 2654435761u) >> shift;
@@ -98,7 +98,8 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
     }
     for (int p = n + threadIdx.x; p < tile_ld; p += blockDim.x) posmap[p] = make_uint2((unsigned)m, 1u << 16);
     double* Xg = A.X + A.ws_off[g];
-    double cmax = 0.0, cmax2 = 0.0;
+    double cmax = 0.0, ssum = 0.0;
+    int swept = 0;
     const int gw = blockIdx.y * nw + wid, gstride = nw * gridDim.y;
 
     for (int c0 = 0; c0 < m; c0 += mc) {
@@ -144,7 +145,8 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
             unsigned xo = (unsigned)t0 * (unsigned)ld + (unsigned)(q & 63) * 8u + (unsigned)(lane >> 2) * rows_t * 8u +
                           2u * (lane & 3);
             const unsigned xstep = rows_t * 64u;
-            double asum = 0.0, ssum = 0.0;
+            double asum = 0.0;
+            ++swept;
             // warp-uniform trip count (groups of four 64-wide steps, predicated inside): one loop body,
             // no divergent remainder loop; all look-ups and loads of a group are in flight together
             for (int base = 0, p0 = 2 * lane; base < ld; base += 256, p0 += 256, xo += 4 * xstep) {
@@ -166,12 +168,8 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
                 }
             }
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                asum += __shfl_xor_sync(0xffffffffu, asum, o);
-                ssum += __shfl_xor_sync(0xffffffffu, ssum, o);
-            }
+            for (int o = 16; o > 0; o >>= 1) asum += __shfl_xor_sync(0xffffffffu, asum, o);
             cmax = fmax(cmax, asum);
-            cmax2 = fmax(cmax2, ssum);
         }
     }
     // zero padding columns n..ld-1 (first CTA of the submatrix)
@@ -181,9 +179,11 @@ __global__ void __launch_bounds__(256) k_gather(const GatherArgs A) {
                 *reinterpret_cast<double2*>(Xg + panel_off(qq, p, ld)) = make_double2(0.0, 0.0);
         }
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ssum += __shfl_xor_sync(0xffffffffu, ssum, o);
     if (lane == 0 && cmax > 0.0) {
         atomicMax(A.gersh + g, (unsigned long long)__double_as_longlong(cmax));
-        atomicMax(A.gersh + gridDim.x + g, (unsigned long long)__double_as_longlong(cmax2));
+        atomicMax(A.gersh + gridDim.x + g, (unsigned long long)__double_as_longlong(ssum / (double)max(swept, 1)));
     }
 }
 

@@ -494,3 +494,79 @@ def test_rescaled_newton_schulz_scalar_properties():
         return 200
     for l0 in (0.01, 0.08, 0.2):
         assert count(l0, True) < count(l0, False)
+
+
+# ---------------------------------------------------------------- finite temperature (L255)
+def test_golden_fermi_2x2(oracle):
+    """L255: signum of Eq.(17) replaced by the Fermi function; closed form on A^2 = 25 I (hand-derived)."""
+    g = _load("fermi_2x2.txt")
+    m = _blocks_from_dense(g[:2], [2])
+    idx = oracle.Index(m)
+    d = oracle.density_fermi(idx, m.values, 0.0, 2.0)
+    assert np.allclose(m.to_dense(d), g[2:], atol=1e-15)
+
+
+def test_fermi_diagonal_and_limits(oracle, cfg0):
+    """Diagonal matrix: elementwise Fermi function (scipy's logistic as the independent witness);
+    kT -> 0: the zero-temperature D~ (gap 0.3 >> kT); f(-x) = 1 - f(x): D~(-K, -mu, kT) = I - D~(K, mu, kT);
+    kT -> infinity: every occupation 1/2."""
+    from scipy.special import expit
+    dv = np.array([-2.0, 0.5, 3.0, -1e-3, 0.25, -0.5, 1.0, 2.0, -4.0])
+    m = W.dense_batch_as_blocks(np.diag(dv)[None])
+    idx = oracle.Index(m)
+    for mu, kT in ((0.0, 0.3), (0.4, 0.05), (-1.0, 2.0)):
+        d = m.to_dense(oracle.density_fermi(idx, m.values, mu, kT))
+        assert np.abs(d - np.diag(expit(-(dv - mu) / kT))).max() < 1e-15
+        assert np.abs(oracle.occupation(dv, mu, kT) - expit(-(dv - mu) / kT)).max() < 1e-15
+    assert np.array_equal(oracle.occupation([-1.0, 0.0, 2.0], 0.0, 0.0), [1.0, 0.5, 0.0])  # Eq.(12) at kT = 0
+    m = cfg0
+    idx = oracle.Index(m)
+    groups = np.array([0, 7, 19], dtype=np.int32)
+    d0 = oracle.density(idx, m.values, 0.0, groups)
+    dT = oracle.density_fermi(idx, m.values, 0.0, 1e-3, groups)
+    assert np.abs(dT - d0).max() < 1e-13
+    dp = oracle.density_fermi(idx, m.values, 0.2, 0.1, groups)
+    dm = oracle.density_fermi(idx, -m.values, -0.2, 0.1, groups)
+    eye = np.zeros_like(m.values)
+    vo, bc = m.val_off(), m.block_cols()
+    for b in np.nonzero(m.rowidx == bc)[0]:
+        n = int(m.blk_size[bc[b]])
+        eye[vo[b]:vo[b + 1]] = np.eye(n).reshape(-1)
+    cols = oracle.column_ids_of_groups(idx, groups)
+    mask = np.repeat(np.isin(bc, cols), np.diff(vo))
+    assert np.abs((dp + dm - eye)[mask]).max() < 1e-12
+    dh = oracle.density_fermi(idx, m.values, 0.0, 1e9, groups)
+    assert np.abs((dh - 0.5 * eye)[mask]).max() < 1e-8
+
+
+def test_fermi_full_cutoff_equals_lapack(oracle):
+    """P5 at finite temperature: with every a_i the whole matrix, D~ = U f(Lambda) U^T of LAPACK's eigh,
+    tr D~ = sum f(lambda), and Algorithm 1's count from (lambda, w) equals tr D~ (L275 with f for signum)."""
+    m = W.water_like(8, "SZV", cutoff=1e9, seed=3)
+    idx = oracle.Index(m)
+    mu, kT = 0.1, 0.05
+    dd = oracle.density_fermi(idx, m.values, mu, kT, nthreads=4)
+    ev, v = np.linalg.eigh(m.to_dense())
+    f = 1.0 / (1.0 + np.exp((ev - mu) / kT))
+    assert np.abs(m.to_dense(dd) - (v * f) @ v.T).max() < 1e-12
+    td, tdk = oracle.traces(idx, dd, m.values)
+    assert abs(td - f.sum()) < 1e-11 and abs(tdk - (f * ev).sum()) < 1e-11
+    lam, w, ptr, g = oracle.eig_groups(idx, m.values, nthreads=4)
+    assert abs(oracle.nelec_fermi(idx, lam, w, g, mu, kT) - td) < 1e-11
+
+
+def test_fermi_count_is_continuous_and_bisection_meets_1e8(oracle, cfg0):
+    """At kT > 0 the electron count is continuous and strictly increasing in mu (no plateau offset problem
+    of reading A11): the literal tolerance 1e-8 of BASELINE config 4 is reachable; nelec_fermi = tr D~."""
+    m = cfg0
+    idx = oracle.Index(m)
+    lam, w, ptr, g = oracle.eig_groups(idx, m.values, nthreads=4)
+    kT = 0.02
+    mus = np.linspace(-2.5, 2.5, 41)
+    ne = np.array([oracle.nelec_fermi(idx, lam, w, g, x, kT) for x in mus])
+    assert np.all(np.diff(ne) > 0) and ne[0] < 1e-6 and abs(ne[-1] - m.n_basis) < 1e-6
+    lo, hi = oracle.gershgorin_interval(m)
+    mu, ne_f, trace = oracle.bisect_mu_fermi(idx, lam, w, g, m.n_occ, -1.0, lo, hi, 1e-8, kT, mu_tol=1e-14)
+    assert abs(ne_f - m.n_occ) <= 1e-8 and len(trace) < 64
+    td, _ = oracle.traces(idx, oracle.density_fermi(idx, m.values, mu, kT, nthreads=4), m.values)
+    assert abs(td - ne_f) < 1e-9
