@@ -111,6 +111,18 @@ typedef struct {
                          /* Ritz interval the estimate is the middle of (a caller's mu inside it, e.g.  */
                          /* the previous SCF step's, is evaluated first); 0 = step 0 always evaluates   */
                          /* *mu_inout (reading A11)                                                      */
+    int32_t method;      /* how the function of a submatrix is evaluated:                        [0]  */
+                         /* 0 = Newton-Schulz iteration (Eq.(11)), every mu step re-evaluates it;     */
+                         /* 1 = eigendecomposition a_i = Q Lambda Q^T (Eq.(17)) once per     */
+                         /*     call and Algorithm 1 as written (L272-276): the mu loop runs on       */
+                         /*     (lambda, w) alone (L266), D~ = Q f(Lambda - mu) Q^T on the generating  */
+                         /*     columns.  FP64; literal midpoint bisection of reading A11 in the       */
+                         /*     Gershgorin bracket (no steering / quadrature options needed)           */
+    int32_t reserved1;
+    double kT;           /* method = 1 only: electronic temperature in the units of K~ (L255:    [0]  */
+                         /* signum of Eq.(17) replaced by the Fermi function, f(x) = 1 / (1 +          */
+                         /* exp(x / kT)) for the occupation 1/2 (1 - signum(x)), reading A18); 0 =      */
+                         /* zero temperature (signum)                                                  */
 } sm_options_t;
 
 /* Plan facts (all sizes in elements unless they say bytes). */
@@ -249,6 +261,28 @@ sm_status_t sm_density_matrix_host(sm_plan_t* plan, const double* h_vals_in, dou
                                    double tol_n, double eps, double* mu_inout, double* h_vals_out,
                                    void* d_workspace, size_t workspace_bytes, sm_stats_t* stats,
                                    void* cuda_stream);
+
+/*
+ * Eigendecomposition path, SURVEY 8(f)1 (PAPER.md IV-F Eq.(17), IV-G Algorithm 1; any plan, whatever
+ * opt.method says; sm_sign_execute / sm_density_matrix call these when opt.method = 1):
+ *   sm_eig_decompose  gathers a_i (mu = 0) and computes a_i = Q Lambda Q^T for every submatrix by one-sided
+ *                     Jacobi rotations on the GPU; Q stays in the workspace (second buffer), lambda_il and
+ *                     the weights w_il = sum_{k in gen(i)} Q_kl^2 of Algorithm 1 (L270, L275) in the plan.
+ *                     stats (may be NULL): iter_min / iter_max = Jacobi sweeps, not_converged.
+ *                     Returns SM_OK or SM_WARN_SIGN_NOT_CONVERGED (a submatrix hit the sweep cap).
+ *   sm_eig_export     host copies of what Algorithm 1 keeps: ptr[ngroups+1] (prefix of n_i), lam[sum n_i],
+ *                     w[sum n_i] (order inside a submatrix unspecified); any pointer may be NULL.
+ *   sm_eig_nelec      n_elec(mu) = sum_i sum_l w_il f(lambda_il - mu), f = 1/2 (1 - signum) for kT = 0 or the
+ *                     Fermi function (L255): one step of Algorithm 1's loop, no decomposition.
+ *   sm_eig_density    D~ = Q f(Lambda - mu) Q^T on the generating columns -> d_vals_out (same workspace as
+ *                     the sm_eig_decompose call, untouched in between).
+ */
+sm_status_t sm_eig_decompose(sm_plan_t* plan, const double* d_vals_in, void* d_workspace,
+                             size_t workspace_bytes, sm_stats_t* stats, void* cuda_stream);
+sm_status_t sm_eig_export(const sm_plan_t* plan, int64_t* ptr, double* lam, double* w);
+sm_status_t sm_eig_nelec(sm_plan_t* plan, double mu, double kT, double* n_elec, void* cuda_stream);
+sm_status_t sm_eig_density(sm_plan_t* plan, double mu, double kT, double* d_vals_out, void* d_workspace,
+                           size_t workspace_bytes, void* cuda_stream);
 
 /*
  * sm_trace_dk -- tr(D) (Eq.(18)) and the band-structure energy tr(D K) (Eq.(10)) of two

@@ -27,7 +27,7 @@ EXPORTS = [
     "sm_plan_create", "sm_plan_query", "sm_plan_export_index", "sm_sign_execute", "sm_sign_execute_host",
     "sm_density_matrix", "sm_density_matrix_host", "sm_trace_dk", "sm_gather", "sm_sign_iterate",
     "sm_scatter", "sm_set_timing", "sm_launch_count", "sm_plan_destroy", "sm_strerror",
-    "sm_last_cuda_error", "sm_measure_peaks",
+    "sm_last_cuda_error", "sm_measure_peaks", "sm_eig_decompose", "sm_eig_export", "sm_eig_nelec", "sm_eig_density",
 ]
 
 
@@ -35,7 +35,8 @@ class sm_options_t(C.Structure):
     _fields_ = [("max_iter", C.c_int32), ("scaling", C.c_int32), ("precision", C.c_int32),
                 ("check_every", C.c_int32), ("max_mu_steps", C.c_int32), ("bisect_iter", C.c_int32),
                 ("mu_tol", C.c_double), ("early_out", C.c_int32), ("order", C.c_int32),
-                ("overshoot", C.c_double), ("predict", C.c_int32), ("mu_guess", C.c_int32), ("rescale", C.c_int32), ("mu_start", C.c_int32)]
+                ("overshoot", C.c_double), ("predict", C.c_int32), ("mu_guess", C.c_int32), ("rescale", C.c_int32), ("mu_start", C.c_int32),
+                ("method", C.c_int32), ("reserved1", C.c_int32), ("kT", C.c_double)]
 
 
 class sm_plan_info_t(C.Structure):
@@ -78,7 +79,8 @@ class sm_stats_t(C.Structure):
 
 def default_options(**kw) -> sm_options_t:
     o = sm_options_t(max_iter=100, scaling=1, precision=0, check_every=16, max_mu_steps=64, bisect_iter=0,
-                     mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=1, mu_guess=1, rescale=1, mu_start=1)
+                     mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=1, mu_guess=1, rescale=1, mu_start=1,
+                     method=0, reserved1=0, kT=0.0)
     for k, v in kw.items():
         setattr(o, k, v)
     return o
@@ -117,9 +119,14 @@ def lib() -> C.CDLL:
         L.sm_strerror.restype = C.c_char_p
         L.sm_last_cuda_error.restype = C.c_char_p
         L.sm_measure_peaks.argtypes = [C.POINTER(sm_peaks_t), vp]
+        L.sm_eig_decompose.argtypes = [vp, vp, vp, C.c_size_t, C.POINTER(sm_stats_t), vp]
+        L.sm_eig_export.argtypes = [vp, vp, vp, vp]
+        L.sm_eig_nelec.argtypes = [vp, dbl, dbl, C.POINTER(dbl), vp]
+        L.sm_eig_density.argtypes = [vp, dbl, dbl, vp, vp, C.c_size_t, vp]
         for f in ("sm_plan_create", "sm_plan_query", "sm_plan_export_index", "sm_sign_execute",
                   "sm_sign_execute_host", "sm_density_matrix", "sm_density_matrix_host", "sm_trace_dk",
-                  "sm_gather", "sm_sign_iterate", "sm_scatter", "sm_set_timing", "sm_measure_peaks"):
+                  "sm_gather", "sm_sign_iterate", "sm_scatter", "sm_set_timing", "sm_measure_peaks", "sm_eig_decompose", "sm_eig_export",
+                  "sm_eig_nelec", "sm_eig_density"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -255,6 +262,34 @@ def sm_set_timing(plan, enable: bool) -> int:
 
 def sm_launch_count(plan) -> int:
     return int(lib().sm_launch_count(plan))
+
+
+def sm_eig_decompose(plan, d_vals_in, d_workspace, stats=None, stream=None) -> int:
+    return _check(lib().sm_eig_decompose(plan, _dev_ptr(d_vals_in), _dev_ptr(d_workspace),
+                                         d_workspace.numel() * d_workspace.element_size(),
+                                         C.byref(stats) if stats is not None else None, _stream_ptr(stream)))
+
+
+def sm_eig_export(plan):
+    """-> (ptr[ngroups+1], lam[sum n_i], w[sum n_i]) host copies of what Algorithm 1 keeps."""
+    info = sm_plan_query(plan)
+    ptr = np.zeros(info.ngroups + 1, dtype=np.int64)
+    _check(lib().sm_eig_export(plan, _np_ptr(ptr), None, None))
+    lam = np.zeros(int(ptr[-1]))
+    w = np.zeros(int(ptr[-1]))
+    _check(lib().sm_eig_export(plan, None, _np_ptr(lam), _np_ptr(w)))
+    return ptr, lam, w
+
+
+def sm_eig_nelec(plan, mu, kT=0.0, stream=None) -> float:
+    ne = C.c_double(0)
+    _check(lib().sm_eig_nelec(plan, mu, kT, C.byref(ne), _stream_ptr(stream)))
+    return ne.value
+
+
+def sm_eig_density(plan, mu, kT, d_vals_out, d_workspace, stream=None) -> int:
+    return _check(lib().sm_eig_density(plan, mu, kT, _dev_ptr(d_vals_out), _dev_ptr(d_workspace),
+                                       d_workspace.numel() * d_workspace.element_size(), _stream_ptr(stream)))
 
 
 def sm_measure_peaks(stream=None) -> sm_peaks_t:

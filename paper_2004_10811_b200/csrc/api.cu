@@ -37,6 +37,8 @@ static void default_options(sm_options_t* o) {
     o->max_mu_steps = 64;
     o->bisect_iter = 0;
     o->mu_tol = 1e-6;
+    o->method = 0;
+    o->kT = 0.0;
 }
 
 static sm_status_t validate(int32_t nb, const int32_t* bs, const int64_t* colptr, const int32_t* rowidx,
@@ -88,7 +90,8 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_partials, p->d_counters, p->d_sched, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
                     p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_col_rec, p->d_gg, p->d_ctrl, p->d_gl_ptr, p->d_gl,
-                    p->d_alpha, p->d_lmin};
+                    p->d_alpha, p->d_lmin, p->d_eig_ptr, p->d_eig_lam, p->d_eig_w, p->d_eig_sigma, p->d_eig_order,
+                    p->d_eig_state};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     if (p->h_pinned) cudaFreeHost(p->h_pinned);
@@ -157,6 +160,8 @@ sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_si
         p->opt.overshoot = 1.0;  // Eq.(19)'s map is increasing beyond 1: eigenvalues of X0 must not exceed 1
     }
     if (p->opt.precision < 0 || p->opt.precision > 2 || p->opt.scaling < 0 || p->opt.scaling > 1) return SM_ERR_INVALID_ARG;
+    if (p->opt.method < 0 || p->opt.method > 1 || !(p->opt.kT >= 0.0)) return SM_ERR_INVALID_ARG;
+    if (p->opt.method == 1 && (p->opt.precision != 0 || p->opt.order != 2)) return SM_ERR_INVALID_ARG;
     p->nb = nb; p->ngroups = ngroups; p->nnzb = nb ? colptr[nb] : 0;
     p->h_blk_size.assign(blk_size, blk_size + nb);
     p->h_colptr.assign(colptr, colptr + nb + 1);
@@ -498,6 +503,92 @@ sm_status_t do_scatter(sm_plan* p, const Bufs& b, double* d_out, sm_stats_t* sta
     return SM_OK;
 }
 
+// Eigendecomposition path (option method = 1, eig.cu): decomposition + its statistics.
+sm_status_t eig_decompose(sm_plan* p, const double* d_in, const Bufs& b, sm_stats_t* stats, int* not_conv,
+                          cudaStream_t st) {
+    sm_status_t s;
+    if (p->timing) SM_CUDA(cudaEventRecord(p->ev[0], st));
+    if ((s = reset_state(p, st))) return s;
+    if ((s = launch_eig_decompose(p, d_in, b.b0, b.b1, st))) return s;
+    if (p->timing) SM_CUDA(cudaEventRecord(p->ev[2], st));
+    const int ng = p->ngroups;
+    std::vector<int32_t> state((size_t)2 * ng + 2, 0);
+    if (ng) SM_CUDA(cudaMemcpyAsync(state.data(), p->d_eig_state, (size_t)2 * ng * 4, cudaMemcpyDeviceToHost, st));
+    SM_CUDA(cudaStreamSynchronize(st));
+    int smin = INT32_MAX, smax = 0, nc = 0;
+    for (int i = 0; i < ng; ++i) {
+        smin = std::min(smin, state[i]);
+        smax = std::max(smax, state[i]);
+        nc += state[ng + i] != 0;
+    }
+    *not_conv = nc;
+    if (stats) {
+        stats->iter_min = ng ? smin : 0;
+        stats->iter_max = smax;
+        stats->iterations = smax;
+        stats->not_converged = nc;
+        stats->tot_evaluations = 1;
+        if (p->timing) {
+            cudaEventElapsedTime(&stats->ms_sign, p->ev[0], p->ev[2]);
+            stats->tot_ms_sign = stats->ms_sign;
+        }
+    }
+    return SM_OK;
+}
+
+sm_status_t eig_count(sm_plan* p, double mu, double kT, double* ne, cudaStream_t st) {
+    if (p->eig_total == 0) { if (ne) *ne = 0.0; return SM_OK; }
+    sm_status_t s = launch_eig_nelec(p, mu, kT, st);
+    if (s) return s;
+    SM_CUDA(cudaStreamSynchronize(st));
+    if (ne) *ne = p->h_pinned_d[0];
+    return SM_OK;
+}
+
+// Algorithm 1 as written (L272-276) on the stored decompositions: the mu loop costs one reduction over
+// (lambda, w) per step and no sign evaluation (L266).  Update rule = reading A11: step 0 at the caller's mu,
+// midpoint bisection inside the Gershgorin interval of K~, same stopping rules as the Newton-Schulz path.
+sm_status_t density_matrix_eig(sm_plan* p, const double* d_in, double n_target, double tol_n, double* mu_inout,
+                               double* d_out, const Bufs& b, sm_stats_t* S, cudaStream_t st) {
+    sm_status_t s;
+    int nc = 0;
+    if ((s = launch_gersh_global(p, d_in, st))) return s;  // bracket; read after the next synchronisation
+    if ((s = eig_decompose(p, d_in, b, S, &nc, st))) return s;
+    double lo = p->h_pinned_d[4], hi = p->h_pinned_d[5];
+    S->bracket_lo = lo; S->bracket_hi = hi;
+    S->mu_guess = NAN;
+    const double kT = p->opt.kT;
+    double mu = *mu_inout, best_mu = mu, best_g = INFINITY, best_ne = 0.0;
+    int steps = 0;
+    bool accepted = false;
+    for (; steps < p->opt.max_mu_steps;) {
+        double ne = 0.0;
+        if ((s = eig_count(p, mu, kT, &ne, st))) return s;
+        const double g = ne - n_target;
+        S->mu_trace[steps] = mu;
+        S->ne_trace[steps] = ne;
+        S->ne_err_trace[steps] = 0.0;
+        S->iter_trace[steps] = 0;
+        if (std::fabs(g) < std::fabs(best_g)) { best_g = g; best_mu = mu; best_ne = ne; }
+        ++steps;
+        if (std::fabs(g) <= tol_n) { accepted = true; break; }
+        if (g < 0) lo = std::max(lo, mu); else hi = std::min(hi, mu);
+        if (hi - lo <= p->opt.mu_tol) break;
+        mu = 0.5 * (lo + hi);
+    }
+    S->mu = best_mu;
+    S->mu_steps = steps;
+    S->n_elec = best_ne;
+    *mu_inout = best_mu;
+    if (d_out) {
+        if ((s = launch_eig_density(p, best_mu, kT, b.b0, b.b1, st))) return s;
+        if ((s = do_scatter(p, b, d_out, S, st))) return s;
+    }
+    SM_CUDA(cudaStreamSynchronize(st));
+    if (!accepted) return SM_WARN_MU_NOT_CONVERGED;
+    return nc ? SM_WARN_SIGN_NOT_CONVERGED : SM_OK;
+}
+
 sm_status_t ensure_stage(sm_plan* p) {
     const size_t bytes = std::max<size_t>((size_t)p->nnz * 8, 8);
     if (!p->d_stage_in) SM_CUDA(cudaMalloc((void**)&p->d_stage_in, bytes));
@@ -516,6 +607,16 @@ extern "C" sm_status_t sm_sign_execute(sm_plan_t* p, const double* d_vals_in, do
     if (s) return s;
     if (stats) memset(stats, 0, sizeof(*stats));
     int nc = 0;
+    if (p->opt.method == 1) {  // Eq.(17): decomposition, then f(Lambda - mu)
+        if ((s = eig_decompose(p, d_vals_in, b, stats, &nc, st))) return s;
+        if ((s = eig_count(p, mu, p->opt.kT, stats ? &stats->n_elec : nullptr, st))) return s;
+        if (d_vals_out) {
+            if ((s = launch_eig_density(p, mu, p->opt.kT, b.b0, b.b1, st))) return s;
+            if ((s = do_scatter(p, b, d_vals_out, stats, st))) return s;
+        }
+        if (stats) { stats->mu = mu; stats->mu_steps = 1; }
+        return nc ? SM_WARN_SIGN_NOT_CONVERGED : SM_OK;
+    }
     p->lz_valid = 0;  // the values may have changed since the last call
     if ((s = evaluate(p, d_vals_in, mu, eps, b, p->opt.max_iter + 1, stats, &nc, st))) return s;
     if (d_vals_out && (s = do_scatter(p, b, d_vals_out, stats, st))) return s;
@@ -589,6 +690,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     sm_stats_t local;
     sm_stats_t* S = stats ? stats : &local;
     memset(S, 0, sizeof(*S));
+    if (p->opt.method == 1) return density_matrix_eig(p, d_vals_in, n_target, tol_n, mu_inout, d_vals_out, b, S, st);
     // bracket (n_elec = 0 below, n_basis above): the Gershgorin interval of the whole K~, intersected with
     // the interlacing interval [lambda_min, lambda_max](K~) of the Lanczos run when scaling = 1 has it
     // (every submatrix eigenvalue lies inside both, reading A11)
@@ -724,6 +826,46 @@ extern "C" sm_status_t sm_density_matrix_host(sm_plan_t* p, const double* h_vals
         SM_CUDA(cudaMemcpyAsync(h_vals_out, p->d_stage_out, (size_t)p->nnz * 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));
     return s;
+}
+
+extern "C" sm_status_t sm_eig_decompose(sm_plan_t* p, const double* d_vals_in, void* d_workspace,
+                                        size_t workspace_bytes, sm_stats_t* stats, void* cuda_stream) {
+    if (!p || (!d_vals_in && p->nnz) || p->opt.precision != 0 || p->opt.order != 2) return SM_ERR_INVALID_ARG;
+    Bufs b;
+    sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
+    if (s) return s;
+    if (stats) memset(stats, 0, sizeof(*stats));
+    int nc = 0;
+    if ((s = eig_decompose(p, d_vals_in, b, stats, &nc, (cudaStream_t)cuda_stream))) return s;
+    return nc ? SM_WARN_SIGN_NOT_CONVERGED : SM_OK;
+}
+
+extern "C" sm_status_t sm_eig_export(const sm_plan_t* p, int64_t* ptr, double* lam, double* w) {
+    if (!p || !p->eig_valid) return SM_ERR_INVALID_ARG;
+    const int ng = p->ngroups;
+    if (ptr) {
+        ptr[0] = 0;
+        for (int i = 0; i < ng; ++i) ptr[i + 1] = ptr[i] + p->h_sub_dim[i];
+    }
+    if (lam && p->eig_total) SM_CUDA(cudaMemcpy(lam, p->d_eig_lam, (size_t)p->eig_total * 8, cudaMemcpyDeviceToHost));
+    if (w && p->eig_total) SM_CUDA(cudaMemcpy(w, p->d_eig_w, (size_t)p->eig_total * 8, cudaMemcpyDeviceToHost));
+    return SM_OK;
+}
+
+extern "C" sm_status_t sm_eig_nelec(sm_plan_t* p, double mu, double kT, double* n_elec, void* cuda_stream) {
+    if (!p || !p->eig_valid || !n_elec || !(mu == mu) || !(kT >= 0.0)) return SM_ERR_INVALID_ARG;
+    return eig_count(p, mu, kT, n_elec, (cudaStream_t)cuda_stream);
+}
+
+extern "C" sm_status_t sm_eig_density(sm_plan_t* p, double mu, double kT, double* d_vals_out, void* d_workspace,
+                                      size_t workspace_bytes, void* cuda_stream) {
+    if (!p || !p->eig_valid || (!d_vals_out && p->nnz) || !(mu == mu) || !(kT >= 0.0)) return SM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    Bufs b;
+    sm_status_t s = carve(p, d_workspace, workspace_bytes, &b);
+    if (s) return s;
+    if ((s = launch_eig_density(p, mu, kT, b.b0, b.b1, st))) return s;
+    return launch_scatter(p, 0, b.b0, b.b1, d_vals_out, st);
 }
 
 extern "C" sm_status_t sm_trace_dk(sm_plan_t* p, const double* d_D, const double* d_K, double* tr_D,

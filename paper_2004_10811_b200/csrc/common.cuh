@@ -130,6 +130,15 @@ struct sm_plan {
     int lz_valid = 0;                      // lz_lo / lz_hi belong to the current call's values
     int lz_ok = 0;                         // the run did not break down: cap, bracket and quadrature may be used
     int ns_attr_set = 0, tf32_attr_set = 0;  // dynamic shared-memory opt-in done on this plan's device
+    // --- eigendecomposition path (eig.cu, option method = 1)
+    int64_t* d_eig_ptr = nullptr;          // [ngroups + 1] prefix of n_i
+    double *d_eig_lam = nullptr, *d_eig_w = nullptr;  // [sum n_i] eigenvalues, weights of Algorithm 1
+    double* d_eig_sigma = nullptr;         // [ngroups] shift of B = a_i + sigma I
+    int32_t* d_eig_order = nullptr;        // [ngroups] processing order, largest first
+    int32_t* d_eig_state = nullptr;        // [2 ngroups + 2] sweeps, flags, work counter
+    int64_t eig_total = 0;
+    int eig_bcols = 16, eig_attr_set = 0, eig_valid = 0;
+    size_t eig_smem = 0;
     // --- staging for the *_host entry points
     double *d_stage_in = nullptr, *d_stage_out = nullptr;
     // --- misc
@@ -175,6 +184,10 @@ struct EvalCtrl {
     double ne, err;    // n_elec(X_k) and its bound at the decision
 };
 sm_status_t launch_eval_ctrl(sm_plan* p, int k, int steer, double n_target, double margin, cudaStream_t st);
+// eig.cu
+sm_status_t launch_eig_decompose(sm_plan* p, const double* vals, double* buf0, double* buf1, cudaStream_t st);
+sm_status_t launch_eig_nelec(sm_plan* p, double mu, double kT, cudaStream_t st);
+sm_status_t launch_eig_density(sm_plan* p, double mu, double kT, double* buf0, const double* buf1, cudaStream_t st);
 // spectral.cu
 sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st);
 sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, double ell_abs, cudaStream_t st);
