@@ -309,6 +309,32 @@ def run_extras(args, m, B, torch, plan, info, ws, d_in, d_out, mu, hbm_peak):
                           "iter_trace": d["iter_trace"], "mu_trace": d["mu_trace"]}
     B.sm_plan_destroy(plan2)
 
+    # Algorithm 1 as written (one eigendecomposition per build, mu loop on (lambda, w))
+    plan4 = B.plan_from_matrix(m, B.default_options(method=1))
+    B.sm_set_timing(plan4, True)
+    B.sm_density_matrix(plan4, d_in, n_target, TOL_N, EPS, MU0, tmp_out, ws, st)
+    torch.cuda.synchronize()
+    k = 2
+    e0.record()
+    for _ in range(k):
+        rc, mu_e = B.sm_density_matrix(plan4, d_in, n_target, TOL_N, EPS, MU0, tmp_out, ws, st)
+    e1.record(); torch.cuda.synchronize()
+    d = st.as_dict()
+    out["algorithm1_eig"] = {"builds_per_s": k / (e0.elapsed_time(e1) * 1e-3), "ms_per_build": e0.elapsed_time(e1) / k,
+                             "status": int(rc), "mu": mu_e, "mu_steps": d["mu_steps"], "decompositions": d["tot_evaluations"],
+                             "jacobi_sweeps": [d["iter_min"], d["iter_max"]], "ms_decompose": d["ms_sign"],
+                             "max_abs_diff_vs_newton_schulz": None}
+    rc, mu_e2 = B.sm_density_matrix(plan4, d_in, n_target, TOL_N, EPS, mu, tmp_out, ws, st)  # same mu as the timed NS build
+    torch.cuda.synchronize()
+    if mu_e2 == mu:
+        out["algorithm1_eig"]["max_abs_diff_vs_newton_schulz"] = float((tmp_out - d_out).abs().max().item())
+    e0.record()
+    rc, mu_g = B.sm_density_matrix(plan4, d_in, n_target, 1e-8, EPS, MU0, tmp_out, ws, st)
+    e1.record(); torch.cuda.synchronize()
+    out["algorithm1_eig"]["guarded_tol_1e-8"] = {"status": int(rc), "mu_steps": st.mu_steps, "decompositions": st.tot_evaluations,
+                                                 "abs_g": abs(st.n_elec - n_target), "mu": mu_g, "ms": e0.elapsed_time(e1)}
+    B.sm_plan_destroy(plan4)
+
     # opt-in reduced precision (3xTF32 on tcgen05) on the same input at the accepted mu, against the FP64 result
     _, tdk64 = B.sm_trace_dk(plan, d_out, d_in)
     plan3 = B.plan_from_matrix(m, B.default_options(precision=2))
