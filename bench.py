@@ -19,8 +19,9 @@ initialisation phase (PAPER.md IV-A); its time is reported in `detail.plan_creat
 Prints ONE JSON line (rank 0).  `value` = builds/s with K~ already resident in HBM; `e2e` = the
 same through the C-ABI host-buffer call (H2D of K~ and D2H of D~ inside the timed region);
 `roofline` = the Newton-Schulz GEMM kernel against the FP64 tensor peak; `cpu_baseline` = the CPU
-oracle timed on this box's cores on a bounded sample.  N > 1: N independent replicas (the path does
-not shard in this build), weak scaling.
+oracle timed on this box's cores on a bounded sample.  N > 1: the same ONE problem sharded
+over the ranks -- contiguous chunks of submatrices balanced by sum n^3, K~ replicated, one
+scalar all-reduce per mu step, all-gather of the result columns -- i.e. strong scaling.
 """
 from __future__ import annotations
 
@@ -183,7 +184,7 @@ def run_reference(args, m, rank):
     t = sum(times) / len(times)
     line = {"impl": "reference", "metric": METRIC, "value": 1.0 / t, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(args, m), "cpu_baseline": dict(cb, value=1.0 / t),
             "e2e": {"value": 1.0 / t, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
@@ -416,8 +417,9 @@ def main():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    # replicas: rank r builds the same-size problem from seed + r
-    m = W.make_config(args.config, args.seed + rank)
+    # N > 1: ONE problem, every rank holds the whole K~ and owns a contiguous chunk of the
+    # submatrices balanced by sum n^3; strong scaling
+    m = W.make_config(args.config, args.seed)
     if args.phases:
         if rank == 0:
             run_phases(args, m, B, torch)
@@ -432,7 +434,10 @@ def main():
                  "ms_copy": pk.ms_copy, "num_sms": pk.num_sms, "clocks": smp.stop() if smp else None,
                  "how": "sm_measure_peaks: mma.sync.m8n8k4.f64 from registers, 16 warps/SM x 16 accumulators; "
                         "16-byte grid-stride copy of 1 GiB (read + write bytes); best of 5 each"}
-    plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess, mu_start=args.mu_start))
+    plan = B.plan_from_matrix(m, B.default_options(mu_guess=args.mu_guess, mu_start=args.mu_start,
+                                                   shard_rank=rank, shard_world=world))
+    if world > 1:  # one scalar all-reduce per mu step (the electron count), D~ columns by all-gather
+        B.sm_plan_set_allreduce(plan, B.make_allreduce(device=torch.device("cuda", local_rank)))
     info = B.sm_plan_query(plan)
     ws = B.alloc_workspace(plan)
     d_in = torch.from_numpy(m.values).cuda()
@@ -448,12 +453,22 @@ def main():
     def step_device():
         if flush is not None:
             flush.zero_()
-        return B.sm_density_matrix(plan, d_in, n_target, TOL_N, EPS, MU0, d_out, ws, stats)
+        r = B.sm_density_matrix(plan, d_in, n_target, TOL_N, EPS, MU0, d_out, ws, stats)
+        if world > 1:
+            B.allgather_result(d_out, info)
+        return r
 
     def step_host():
         if flush is not None:
             flush.zero_()
-        return B.sm_density_matrix_host(plan, h_in, n_target, TOL_N, EPS, MU0, h_out, ws, stats)
+        if world == 1:
+            return B.sm_density_matrix_host(plan, h_in, n_target, TOL_N, EPS, MU0, h_out, ws, stats)
+        d_in.copy_(h_in, non_blocking=True)  # every rank receives the whole K~ and returns the whole D~
+        r = B.sm_density_matrix(plan, d_in, n_target, TOL_N, EPS, MU0, d_out, ws, stats)
+        B.allgather_result(d_out, info)
+        h_out.copy_(d_out, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        return r
 
     def barrier():
         torch.cuda.synchronize()
@@ -540,13 +555,19 @@ def main():
                                   "GBps": info.index_alg_bytes / 1e6 / info.ms_index_kernels if info.ms_index_kernels > 0 else None,
                                   "frac": info.index_alg_bytes / 1e6 / info.ms_index_kernels / hbm_peak if info.ms_index_kernels > 0 else None},
                   "hbm_peak_GBps": hbm_peak, "hbm_peak_source": hbm_src, "peaks_measured_this_run": peaks}
-        if not args.no_extras:
+        if world > 1:
+            detail["sharding"] = {"rule": "contiguous chunks balanced by sum n^3, PAPER.md L235 (sm_partition_groups)",
+                                  "rank0_groups": [info.shard_group_begin, info.shard_group_end],
+                                  "collectives_per_build": "1 all-reduce of 2 doubles per sign evaluation + all-gather of D~ "
+                                                           "(one broadcast per rank of its value range)",
+                                  "note": "GEMM / launch figures of this line are rank 0's"}
+        if not args.no_extras and world == 1:
             detail.update(run_extras(args, m, B, torch, plan, info, ws, d_in, d_out, mu, hbm_peak))
-        line = {"metric": METRIC, "value": world * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+        line = {"metric": METRIC, "value": args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
-                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic", "config": workload_config(args, m), "clocks": clocks,
-                "e2e": {"value": world * k_e2e / (ms_e2e * 1e-3), "unit": UNIT, "steps": k_e2e,
+                "e2e": {"value": k_e2e / (ms_e2e * 1e-3), "unit": UNIT, "steps": k_e2e,
                         "h2d_bytes_per_step": int(info.nnz * 8), "d2h_bytes_per_step": int(info.nnz * 8)},
                 "gpu_launches": int(launches), "roofline": roofline, "detail": detail}
         if not args.no_cpu_baseline:

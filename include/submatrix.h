@@ -123,6 +123,16 @@ typedef struct {
                          /* signum of Eq.(17) replaced by the Fermi function, f(x) = 1 / (1 +          */
                          /* exp(x / kT)) for the occupation 1/2 (1 - signum(x)), reading A18); 0 =      */
                          /* zero temperature (signum)                                                  */
+    int32_t shard_rank;  /* this plan covers one contiguous chunk of the     [0]  */
+    int32_t shard_world; /* generating groups, chunk shard_rank of shard_world chunks balanced   [1]  */
+                         /* by sum n_i^3 with >= 1 group each (the greedy rule of PAPER.md L235,       */
+                         /* sm_partition_groups; contiguous chunks share blocks, L188-190).  The       */
+                         /* pattern and the values are replicated; the plan gathers, iterates and      */
+                         /* scatters only its own groups (d_vals_out: only their block columns are     */
+                         /* written), n_elec is the local partial unless sm_plan_set_allreduce has     */
+                         /* given the plan a sum over the ranks; shard_world <= 1: no sharding.        */
+                         /* The steering early-out (early_out) needs the global bound at every         */
+                         /* iteration and is switched off when shard_world > 1.                        */
 } sm_options_t;
 
 /* Plan facts (all sizes in elements unless they say bytes). */
@@ -149,6 +159,11 @@ typedef struct {
                               /* sum|S_i|*8 written                               */
     float ms_index_kernels;   /* CUDA-event time of the index-builder kernels (a2)              */
     float ms_plan_create;     /* host wall clock of the whole sm_plan_create call               */
+    int32_t shard_group_begin, shard_group_end; /* groups of the caller's numbering this plan covers   */
+    int64_t shard_val_begin, shard_val_end;     /* their result values, if those form ONE contiguous   */
+                              /* range of the value array (groups of ascending consecutive block       */
+                              /* columns), else -1, -1: the all-gather of D~ needs no index lists then */
+    int32_t ngroups_total, reserved2; /* groups of the whole problem (ngroups = those of this plan)    */
 } sm_plan_info_t;
 
 /* Filled by sm_sign_execute / sm_density_matrix (may be NULL). Times are CUDA-event ms of the
@@ -199,6 +214,27 @@ sm_status_t sm_plan_create(sm_plan_t** plan, int32_t nb, const int32_t* blk_size
                            const int64_t* colptr, const int32_t* rowidx, int32_t ngroups,
                            const int32_t* grp_ptr, const int32_t* grp_cols, const sm_options_t* opt,
                            void* cuda_stream);
+
+/*
+ * sm_partition_groups -- the load balancer of PAPER.md IV-E (L235): "a greedy algorithm to assign submatrices
+ * to ranks such that they have similar load ... one consecutive chunk of submatrices to each rank ... expected
+ * number of floating-point operations assuming that processing a submatrix takes O(n^3) FLOP and assigns
+ * submatrices to ranks as long as their load is expected to be lower than FLOP_total / #ranks.  Additionally,
+ * we make sure that each rank obtains at least one submatrix."  Reading A19: rank r takes the next submatrix
+ * while its load so far is below sum n^3 / world AND enough submatrices remain to give every later rank one;
+ * the last rank takes what is left.  Host only (no GPU needed): sub_dim[ngroups] host, first[world + 1] host
+ * out (rank r owns groups first[r] .. first[r+1] - 1).  world > ngroups is an error.
+ */
+sm_status_t sm_partition_groups(int32_t ngroups, const int32_t* sub_dim, int32_t world, int32_t* first);
+
+/*
+ * Sum over the ranks for a sharded plan (opt.shard_world > 1): fn(ctx, vals, n) must replace vals[0..n) by
+ * their sums over all ranks (host doubles; called from the calling thread after a stream synchronisation,
+ * the same number of times on every rank: once per sign evaluation / mu step).  The Python binding passes
+ * a torch.distributed all_reduce.  NULL fn: counts stay local.
+ */
+typedef void (*sm_allreduce_fn)(void* ctx, double* vals, int32_t n);
+sm_status_t sm_plan_set_allreduce(sm_plan_t* plan, sm_allreduce_fn fn, void* ctx);
 
 /* Plan facts, including the workspace size. */
 sm_status_t sm_plan_query(const sm_plan_t* plan, sm_plan_info_t* out);

@@ -232,6 +232,31 @@ def flop_model(m, idx: "Index"):
     return ops, ops_cols, (ops_cols / ops if ops else 0.0)
 
 
+def partition_groups(sub_dim, world: int):
+    """PAPER.md IV-E L235 (reading A19): consecutive chunks of submatrices; a rank is given the next submatrix
+    "as long as" its load (sum of n^3 so far) "is expected to be lower than FLOP_total / #ranks", and
+    "each rank obtains at least one submatrix" (so a rank also stops when only one submatrix per later rank
+    is left); the last rank takes the rest.  Returns first[world + 1]."""
+    n3 = [int(n) ** 3 for n in sub_dim]
+    ng = len(n3)
+    assert 1 <= world <= max(ng, 1)
+    total = sum(n3)
+    first, i = [], 0
+    for r in range(world):
+        first.append(i)
+        if r == world - 1:
+            i = ng
+            break
+        load = 0
+        taken = 0
+        while i < ng - (world - 1 - r) and (taken == 0 or load * world < total):
+            load += n3[i]
+            i += 1
+            taken += 1
+    first.append(ng)
+    return first
+
+
 def gershgorin_interval(m) -> tuple[float, float]:
     """Gershgorin interval of the whole block-sparse matrix: bracket for the mu loop (A11)."""
     cols = m.block_cols()

@@ -28,6 +28,7 @@ EXPORTS = [
     "sm_density_matrix", "sm_density_matrix_host", "sm_trace_dk", "sm_gather", "sm_sign_iterate",
     "sm_scatter", "sm_set_timing", "sm_launch_count", "sm_plan_destroy", "sm_strerror",
     "sm_last_cuda_error", "sm_measure_peaks", "sm_eig_decompose", "sm_eig_export", "sm_eig_nelec", "sm_eig_density",
+    "sm_partition_groups", "sm_plan_set_allreduce",
 ]
 
 
@@ -36,7 +37,8 @@ class sm_options_t(C.Structure):
                 ("check_every", C.c_int32), ("max_mu_steps", C.c_int32), ("bisect_iter", C.c_int32),
                 ("mu_tol", C.c_double), ("early_out", C.c_int32), ("order", C.c_int32),
                 ("overshoot", C.c_double), ("predict", C.c_int32), ("mu_guess", C.c_int32), ("rescale", C.c_int32), ("mu_start", C.c_int32),
-                ("method", C.c_int32), ("reserved1", C.c_int32), ("kT", C.c_double)]
+                ("method", C.c_int32), ("reserved1", C.c_int32), ("kT", C.c_double),
+                ("shard_rank", C.c_int32), ("shard_world", C.c_int32)]
 
 
 class sm_plan_info_t(C.Structure):
@@ -46,7 +48,12 @@ class sm_plan_info_t(C.Structure):
                 ("sum_ld2", C.c_int64), ("n_tiles", C.c_int64), ("n_buckets", C.c_int32),
                 ("reserved0", C.c_int32), ("workspace_bytes", C.c_size_t), ("sum_n3_columns", C.c_int64),
                 ("est_speedup", C.c_double), ("index_alg_bytes", C.c_int64), ("ms_index_kernels", C.c_float),
-                ("ms_plan_create", C.c_float)]
+                ("ms_plan_create", C.c_float), ("shard_group_begin", C.c_int32), ("shard_group_end", C.c_int32),
+                ("shard_val_begin", C.c_int64), ("shard_val_end", C.c_int64), ("ngroups_total", C.c_int32),
+                ("reserved2", C.c_int32)]
+
+
+ALLREDUCE_FN = C.CFUNCTYPE(None, C.c_void_p, C.POINTER(C.c_double), C.c_int32)
 
 
 class sm_peaks_t(C.Structure):
@@ -80,7 +87,7 @@ class sm_stats_t(C.Structure):
 def default_options(**kw) -> sm_options_t:
     o = sm_options_t(max_iter=100, scaling=1, precision=0, check_every=16, max_mu_steps=64, bisect_iter=0,
                      mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=1, mu_guess=1, rescale=1, mu_start=1,
-                     method=0, reserved1=0, kT=0.0)
+                     method=0, reserved1=0, kT=0.0, shard_rank=0, shard_world=1)
     for k, v in kw.items():
         setattr(o, k, v)
     return o
@@ -123,10 +130,12 @@ def lib() -> C.CDLL:
         L.sm_eig_export.argtypes = [vp, vp, vp, vp]
         L.sm_eig_nelec.argtypes = [vp, dbl, dbl, C.POINTER(dbl), vp]
         L.sm_eig_density.argtypes = [vp, dbl, dbl, vp, vp, C.c_size_t, vp]
+        L.sm_partition_groups.argtypes = [i32, vp, i32, vp]
+        L.sm_plan_set_allreduce.argtypes = [vp, ALLREDUCE_FN, vp]
         for f in ("sm_plan_create", "sm_plan_query", "sm_plan_export_index", "sm_sign_execute",
                   "sm_sign_execute_host", "sm_density_matrix", "sm_density_matrix_host", "sm_trace_dk",
                   "sm_gather", "sm_sign_iterate", "sm_scatter", "sm_set_timing", "sm_measure_peaks", "sm_eig_decompose", "sm_eig_export",
-                  "sm_eig_nelec", "sm_eig_density"):
+                  "sm_eig_nelec", "sm_eig_density", "sm_partition_groups", "sm_plan_set_allreduce"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -292,6 +301,60 @@ def sm_eig_density(plan, mu, kT, d_vals_out, d_workspace, stream=None) -> int:
                                        d_workspace.numel() * d_workspace.element_size(), _stream_ptr(stream)))
 
 
+def sm_partition_groups(sub_dim, world: int) -> np.ndarray:
+    """-> first[world + 1]: rank r owns groups first[r] .. first[r+1] - 1 (host only)."""
+    sub_dim = np.ascontiguousarray(sub_dim, dtype=np.int32)
+    first = np.zeros(world + 1, dtype=np.int32)
+    _check(lib().sm_partition_groups(len(sub_dim), _np_ptr(sub_dim), world, _np_ptr(first)))
+    return first
+
+
+_allreduce_keepalive = {}
+
+
+def make_allreduce(group=None, device=None):
+    """A C callback that sums host doubles over the ranks with torch.distributed.all_reduce (plumbing:
+    the tensor lives on `device`: CUDA for the nccl backend, CPU for gloo)."""
+    import torch
+    import torch.distributed as dist
+
+    def _fn(ctx, vals, n):
+        t = torch.tensor([vals[i] for i in range(n)], dtype=torch.float64, device=device or "cpu")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+        out = t.cpu().tolist()
+        for i in range(n):
+            vals[i] = out[i]
+
+    return ALLREDUCE_FN(_fn)
+
+
+def sm_plan_set_allreduce(plan, fn) -> int:
+    """fn: an ALLREDUCE_FN (make_allreduce) or None; kept alive as long as the plan uses it."""
+    cb = fn if fn is not None else C.cast(None, ALLREDUCE_FN)
+    _allreduce_keepalive[plan.value] = cb
+    return _check(lib().sm_plan_set_allreduce(plan, cb, None))
+
+
+def allgather_result(d_vals_out, info, group=None):
+    """D~ of a sharded build: every rank contributes the value range of its own block columns
+    (sm_plan_info_t.shard_val_begin/end) and receives the others' (plumbing over torch.distributed:
+    an all-gather of unequal contiguous slices, done as broadcasts of each rank's slice)."""
+    import torch
+    import torch.distributed as dist
+    world = dist.get_world_size(group)
+    rank = dist.get_rank(group)
+    if info.shard_val_begin < 0:
+        raise ValueError("the groups of this shard do not own one contiguous value range")
+    mine = torch.tensor([info.shard_val_begin, info.shard_val_end], dtype=torch.int64, device=d_vals_out.device)
+    ranges = [torch.zeros_like(mine) for _ in range(world)]
+    dist.all_gather(ranges, mine, group=group)
+    for r in range(world):
+        b, e = (int(x) for x in ranges[r].tolist())
+        if e > b:
+            dist.broadcast(d_vals_out[b:e], src=dist.get_global_rank(group, r) if group is not None else r, group=group)
+    return d_vals_out
+
+
 def sm_measure_peaks(stream=None) -> sm_peaks_t:
     pk = sm_peaks_t()
     _check(lib().sm_measure_peaks(C.byref(pk), _stream_ptr(stream)))
@@ -299,6 +362,7 @@ def sm_measure_peaks(stream=None) -> sm_peaks_t:
 
 
 def sm_plan_destroy(plan) -> None:
+    _allreduce_keepalive.pop(getattr(plan, "value", None), None)
     lib().sm_plan_destroy(plan)
 
 

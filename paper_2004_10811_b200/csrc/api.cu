@@ -39,6 +39,8 @@ static void default_options(sm_options_t* o) {
     o->mu_tol = 1e-6;
     o->method = 0;
     o->kT = 0.0;
+    o->shard_rank = 0;
+    o->shard_world = 1;
 }
 
 static sm_status_t validate(int32_t nb, const int32_t* bs, const int64_t* colptr, const int32_t* rowidx,
@@ -168,6 +170,46 @@ sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_si
     p->h_rowidx.assign(rowidx, rowidx + p->nnzb);
     p->h_grp_ptr.assign(grp_ptr, grp_ptr + ngroups + 1);
     p->h_grp_cols.assign(grp_cols, grp_cols + nb);
+    // keep only this rank's contiguous chunk of groups (the pattern stays whole)
+    const int world = std::max(p->opt.shard_world, 1), rank = p->opt.shard_rank;
+    const int32_t ngroups_total = ngroups;
+    if (rank < 0 || rank >= world) return SM_ERR_INVALID_ARG;
+    int shard_gb = 0, shard_ge = ngroups;
+    int64_t shard_vb = -1, shard_ve = -1;
+    if (world > 1) {
+        if (world > ngroups) return SM_ERR_INVALID_ARG;
+        std::vector<int32_t> dims(ngroups), rows;
+        for (int g = 0; g < ngroups; ++g) {  // n_i of every group: sorted union of its columns' row lists (host, plan time)
+            rows.clear();
+            for (int q = grp_ptr[g]; q < grp_ptr[g + 1]; ++q)
+                rows.insert(rows.end(), rowidx + colptr[grp_cols[q]], rowidx + colptr[grp_cols[q] + 1]);
+            std::sort(rows.begin(), rows.end());
+            rows.erase(std::unique(rows.begin(), rows.end()), rows.end());
+            int32_t n = 0;
+            for (int32_t r : rows) n += blk_size[r];
+            dims[g] = n;
+        }
+        std::vector<int32_t> first(world + 1);
+        if ((s = sm_partition_groups(ngroups, dims.data(), world, first.data()))) return s;
+        shard_gb = first[rank]; shard_ge = first[rank + 1];
+        std::vector<int32_t> gp(shard_ge - shard_gb + 1), gc(grp_cols + grp_ptr[shard_gb], grp_cols + grp_ptr[shard_ge]);
+        for (int g = shard_gb; g <= shard_ge; ++g) gp[g - shard_gb] = grp_ptr[g] - grp_ptr[shard_gb];
+        p->h_grp_ptr.swap(gp);
+        p->h_grp_cols.swap(gc);
+        p->ngroups = ngroups = shard_ge - shard_gb;
+        bool contiguous = !p->h_grp_cols.empty();
+        for (size_t k = 1; k < p->h_grp_cols.size(); ++k) contiguous = contiguous && p->h_grp_cols[k] == p->h_grp_cols[k - 1] + 1;
+        if (contiguous) {  // value offsets of the first owned column and of the one after the last
+            std::vector<int64_t> cv(nb + 1, 0);
+            for (int c = 0; c < nb; ++c) {
+                int64_t e = 0;
+                for (int64_t q = colptr[c]; q < colptr[c + 1]; ++q) e += blk_size[rowidx[q]];
+                cv[c + 1] = cv[c] + e * blk_size[c];
+            }
+            shard_vb = cv[p->h_grp_cols.front()];
+            shard_ve = cv[p->h_grp_cols.back() + 1];
+        }
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
@@ -249,6 +291,9 @@ sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_si
         while ((int64_t)ngroups * split < want_ctas && split * 8 * 4 < p->info.dim_max) ++split;
         p->gather_split = std::max(split, 1);
     }
+    p->info.shard_group_begin = shard_gb; p->info.shard_group_end = shard_ge;
+    p->info.shard_val_begin = world > 1 ? shard_vb : 0; p->info.shard_val_end = world > 1 ? shard_ve : p->nnz;
+    p->info.ngroups_total = ngroups_total;
     p->info.ms_plan_create =
         std::chrono::duration<float, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     guard.p = nullptr;
@@ -256,6 +301,37 @@ sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_si
     return SM_OK;
 }
 }  // namespace
+
+// PAPER.md L235 (reading A19): consecutive chunks, a rank takes the next submatrix while its load so far is
+// below sum n^3 / world and every later rank can still get one; the last rank takes the rest.
+extern "C" sm_status_t sm_partition_groups(int32_t ngroups, const int32_t* sub_dim, int32_t world, int32_t* first) {
+    if (ngroups < 0 || world < 1 || !first || (ngroups > 0 && !sub_dim) || world > std::max(ngroups, 1)) return SM_ERR_INVALID_ARG;
+    typedef unsigned __int128 u128;  // exact: n^3 sums of any realistic size, compared as load * world < total
+    u128 total = 0;
+    for (int i = 0; i < ngroups; ++i) total += (u128)sub_dim[i] * (u128)sub_dim[i] * (u128)sub_dim[i];
+    int i = 0;
+    for (int r = 0; r < world; ++r) {
+        first[r] = i;
+        if (r == world - 1) { i = ngroups; break; }
+        u128 load = 0;
+        const int last_allowed = ngroups - (world - 1 - r);  // leave one submatrix for every later rank
+        bool took = false;
+        while (i < last_allowed && (!took || load * (u128)world < total)) {
+            load += (u128)sub_dim[i] * (u128)sub_dim[i] * (u128)sub_dim[i];
+            ++i;
+            took = true;
+        }
+    }
+    first[world] = ngroups;
+    return SM_OK;
+}
+
+extern "C" sm_status_t sm_plan_set_allreduce(sm_plan_t* p, sm_allreduce_fn fn, void* ctx) {
+    if (!p) return SM_ERR_INVALID_ARG;
+    p->allreduce = fn;
+    p->allreduce_ctx = ctx;
+    return SM_OK;
+}
 
 extern "C" sm_status_t sm_plan_query(const sm_plan_t* p, sm_plan_info_t* out) {
     if (!p || !out) return SM_ERR_INVALID_ARG;
@@ -469,6 +545,13 @@ sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, cons
     if (p->timing) SM_CUDA(cudaEventRecord(p->ev[2], st));
     if ((s = launch_nelec(p, b.b0, reduced ? b.b0 : b.b1, st))) return s;
     if ((s = collect_stats(p, stats, not_conv, st))) return s;
+    if (p->allreduce) {  // sharded plan: global electron count and non-convergence count (same on every rank)
+        double v[2] = {p->h_pinned_d[0], (double)*not_conv};
+        p->allreduce(p->allreduce_ctx, v, 2);
+        p->h_pinned_d[0] = v[0];
+        *not_conv = (int)(v[1] + 0.5);
+        if (stats) { stats->n_elec = v[0]; stats->not_converged = *not_conv; }
+    }
     if (stats) {
         if (steer && steer->decided) stats->n_elec = steer->ne;
         stats->iterations = launched / (p->opt.order == 3 ? 3 : 2);
@@ -521,6 +604,11 @@ sm_status_t eig_decompose(sm_plan* p, const double* d_in, const Bufs& b, sm_stat
         smax = std::max(smax, state[i]);
         nc += state[ng + i] != 0;
     }
+    if (p->allreduce) {
+        double v[1] = {(double)nc};
+        p->allreduce(p->allreduce_ctx, v, 1);
+        nc = (int)(v[0] + 0.5);
+    }
     *not_conv = nc;
     if (stats) {
         stats->iter_min = ng ? smin : 0;
@@ -537,10 +625,16 @@ sm_status_t eig_decompose(sm_plan* p, const double* d_in, const Bufs& b, sm_stat
 }
 
 sm_status_t eig_count(sm_plan* p, double mu, double kT, double* ne, cudaStream_t st) {
-    if (p->eig_total == 0) { if (ne) *ne = 0.0; return SM_OK; }
+    if (p->eig_total == 0) {  // a shard without basis functions still takes part in the sum
+        double v = 0.0;
+        if (p->allreduce) p->allreduce(p->allreduce_ctx, &v, 1);
+        if (ne) *ne = v;
+        return SM_OK;
+    }
     sm_status_t s = launch_eig_nelec(p, mu, kT, st);
     if (s) return s;
     SM_CUDA(cudaStreamSynchronize(st));
+    if (p->allreduce) p->allreduce(p->allreduce_ctx, p->h_pinned_d, 1);
     if (ne) *ne = p->h_pinned_d[0];
     return SM_OK;
 }
@@ -742,7 +836,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
         acc_n3 += e.tot_sum_iter_n3; acc_sym += e.tot_sym_flop; acc_launch += e.tot_gemm_launches;
         acc_eval += 1; acc_g += e.tot_ms_gather; acc_s += e.tot_ms_sign;
     };
-    const bool early = p->opt.early_out != 0 && p->opt.precision == 0;
+    const bool early = p->opt.early_out != 0 && p->opt.precision == 0 && p->opt.shard_world <= 1;
     for (; steps < p->opt.max_mu_steps;) {
         memset(&ev, 0, sizeof(ev));
         Steer steer;

@@ -139,6 +139,9 @@ struct sm_plan {
     int64_t eig_total = 0;
     int eig_bcols = 16, eig_attr_set = 0, eig_valid = 0;
     size_t eig_smem = 0;
+    // --- sharding: the plan holds only its own chunk of groups
+    sm_allreduce_fn allreduce = nullptr;
+    void* allreduce_ctx = nullptr;
     // --- staging for the *_host entry points
     double *d_stage_in = nullptr, *d_stage_out = nullptr;
     // --- misc

@@ -318,6 +318,10 @@ k_scatter_map_build(int nb, const int32_t* __restrict__ blk_size, const int64_t*
     if (c >= nb) return;
     const int lane = threadIdx.x & 31;
     const int g = col_grp[c];
+    if (g < 0) {  // block column of another shard: an empty record, k_scatter skips it
+        if (lane == 0) col_rec[c] = make_int4(0, 0, 0, -1);
+        return;
+    }
     const int bc = blk_size[c];
     const int64_t p0 = colptr[c];
     if (lane == 0) {  // column record of k_scatter: first value, value count, group -- one 16-byte load
@@ -515,6 +519,10 @@ __global__ void k_nelec_bound(int nb, const int32_t* __restrict__ col_grp, const
     if (c >= nb || ctrl[0] != 0) return;  // evaluation already stopped: empty launch
     const int lane = threadIdx.x & 31;
     const int g = col_grp[c];
+    if (g < 0) {  // block column of another shard
+        if (lane == 0) { part[c] = 0.0; part[nb + c] = 0.0; }
+        return;
+    }
     const int di = done_iter[g];
     const int kb = (di >= 0 && di <= k) ? di : k;  // di = k + 1: predicted exit, its last update has not run yet
     const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];

@@ -220,7 +220,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     if ((s = upload(&p->d_rowidx, p->h_rowidx.data(), p->nnzb, st))) return s;
     if ((s = upload(&p->d_val_off, val_off.data(), p->nnzb + 1, st))) return s;
     if ((s = upload(&p->d_grp_ptr, p->h_grp_ptr.data(), ng + 1, st))) return s;
-    if ((s = upload(&p->d_grp_cols, p->h_grp_cols.data(), nb, st))) return s;
+    if ((s = upload(&p->d_grp_cols, p->h_grp_cols.data(), p->h_grp_cols.size(), st))) return s;
 
     // a2: index builder.  eptr = exclusive prefix of the groups' stored-block counts (every block column is
     // in exactly one group, so the scratch of pass 1 holds nnzb keys); O(nb) integers on the host.
@@ -273,6 +273,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMalloc((void**)&p->d_gen_pos, (size_t)std::max(nb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_gen_off, (size_t)std::max(nb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_col_grp, (size_t)std::max(nb, 1) * 4));
+    SM_CUDA(cudaMemsetAsync(p->d_col_grp, 0xff, (size_t)std::max(nb, 1) * 4, st));  // -1: column of another shard
     SM_CUDA(cudaMalloc((void**)&p->d_blk_pack, std::max<int64_t>(p->nnzb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_gen_width, (size_t)std::max(ng, 1) * 4));
     // pass 2
@@ -362,7 +363,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     I.workspace_bytes = 3 * buf;
     // cost model of the grouping (Eq.(14), Eq.(15)): integer sums on the host
     int64_t n3c = 0;
-    for (int c = 0; c < nb; ++c) {
+    for (int c : p->h_grp_cols) {  // the block columns of this plan's groups (all of them unless sharded)
         int64_t nc = 0;
         for (int64_t q = p->h_colptr[c]; q < p->h_colptr[c + 1]; ++q) nc += p->h_blk_size[p->h_rowidx[q]];
         n3c += nc * nc * nc;

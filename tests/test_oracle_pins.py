@@ -570,3 +570,47 @@ def test_fermi_count_is_continuous_and_bisection_meets_1e8(oracle, cfg0):
     assert abs(ne_f - m.n_occ) <= 1e-8 and len(trace) < 64
     td, _ = oracle.traces(idx, oracle.density_fermi(idx, m.values, mu, kT, nthreads=4), m.values)
     assert abs(td - ne_f) < 1e-9
+
+
+# ---------------------------------------------------------------- load balancing (IV-E L235)
+def test_partition_rule_hand_worked_and_properties(oracle):
+    """L235: greedy consecutive chunks by n^3.  Hand-worked: dims (2,2,2,2,2,2,2,2), 4 ranks: total 64,
+    target 16 -> two per rank.  dims (10,1,1,1,1,1), 3 ranks: total 1005, target 335: rank 0 stops after the
+    first (1000 >= 335), rank 1 takes while below target but must leave one: (1,1,1,1), rank 2 the last.
+    dims (1,1,1,1,1,10), 3 ranks: rank 0 would go on (load 4 < 335) but must leave two: takes four.
+    Properties on random sizes: a contiguous cover, >= 1 each, every rank but the last below
+    target + max n^3; the last at most the target when nobody was cut short by the leave-one rule."""
+    assert oracle.partition_groups([2] * 8, 4) == [0, 2, 4, 6, 8]
+    assert oracle.partition_groups([10, 1, 1, 1, 1, 1], 3) == [0, 1, 5, 6]
+    assert oracle.partition_groups([1, 1, 1, 1, 1, 10], 3) == [0, 4, 5, 6]
+    assert oracle.partition_groups([5, 7], 1) == [0, 2]
+    rng = np.random.default_rng(0)
+    for trial in range(50):
+        ng = int(rng.integers(1, 200))
+        world = int(rng.integers(1, min(ng, 16) + 1))
+        dims = rng.integers(1, 300, ng)
+        f = oracle.partition_groups(dims, world)
+        assert f[0] == 0 and f[-1] == ng and all(f[r + 1] > f[r] for r in range(world))
+        n3 = dims.astype(object) ** 3
+        total, mx = int(n3.sum()), int(n3.max())
+        loads = [int(n3[f[r]:f[r + 1]].sum()) for r in range(world)]
+        cut = [f[r + 1] == ng - (world - 1 - r) for r in range(world - 1)]
+        for r in range(world - 1):
+            assert loads[r] * world < total + mx * world
+        if not any(cut):
+            assert loads[-1] * world <= total
+
+
+def test_library_partition_equals_oracle(oracle):
+    """sm_partition_groups (host function of the C-ABI, no GPU) against the oracle's restatement."""
+    from paper_2004_10811_b200 import binding as B
+    rng = np.random.default_rng(1)
+    for trial in range(100):
+        ng = int(rng.integers(1, 300))
+        world = int(rng.integers(1, min(ng, 12) + 1))
+        dims = rng.integers(1, 2500, ng).astype(np.int32)
+        assert list(B.sm_partition_groups(dims, world)) == oracle.partition_groups(dims, world)
+    m = W.make_config(2)
+    idx = oracle.Index(m)
+    for world in (2, 3, 8):
+        assert list(B.sm_partition_groups(idx.sub_dim, world)) == oracle.partition_groups(idx.sub_dim, world)
