@@ -87,7 +87,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
     if (!p) return;
     void* ptrs[] = {p->d_blk_size, p->d_blk_off, p->d_rowidx, p->d_colptr, p->d_val_off, p->d_grp_ptr,
                     p->d_grp_cols, p->d_col_grp, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off, p->d_sub_dim,
-                    p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_gen_width, p->d_ws_off, p->d_ld, p->d_tiles,
+                    p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_gen_width, p->d_gen_rng, p->d_ws_off, p->d_ld, p->d_tiles,
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
                     p->d_partials, p->d_counters, p->d_sched, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
@@ -484,8 +484,15 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         const int64_t prods = di[i] >= 0 ? ppi * it + (fl[i] == 2 ? 0 : 1) : ppi * (int64_t)p->cur_k + p->half_iter;
         sin3 += prods * n * n * n;
         symf += prods * n * n * (n + 1);
+        // predicted exit (flag 2): its last update only computed the tiles of the generating rows
+        if (fl[i] == 2 && p->opt.order == 2 && p->opt.precision == 0) symf += p->h_final_flop[i] - n * n * (n + 1);
     }
     *not_conv = nc;
+    if (getenv("SM_DEBUG_ITERS")) {
+        int hist[2][32] = {{0}};
+        for (int i = 0; i < ng; ++i) if (di[i] >= 0 && di[i] < 32) hist[fl[i] == 2][di[i]]++;
+        for (int k = 0; k < 32; ++k) if (hist[0][k] || hist[1][k]) fprintf(stderr, "iter %d: measured %d predicted %d\n", k, hist[0][k], hist[1][k]);
+    }
     if (stats) {
         stats->iter_min = ng ? imin : 0;
         stats->iter_max = imax;

@@ -80,6 +80,9 @@ struct sm_plan {
     uint32_t *d_blk_pack = nullptr;// [nnzb] block (r,c): element row offset inside c's group's submatrix (low 20
                                    //        bits) | height blk_size[r] (high 12 bits)
     int32_t *d_gen_width = nullptr;// [ngroups] generating basis functions per group
+    int2* d_gen_rng = nullptr;     // [ngroups] first / last generating row of a_i
+    std::vector<int32_t> h_gen_rng;   // host copy (2 per group)
+    std::vector<int64_t> h_final_flop;  // flop of a last update restricted to the generating rows' tiles
     // --- device: workspace geometry and tiles
     int64_t* d_ws_off = nullptr;   // [ngroups] offset (doubles) of submatrix i in each buffer
     int32_t* d_ld = nullptr;       // [ngroups] padded leading dimension

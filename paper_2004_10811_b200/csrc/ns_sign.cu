@@ -15,9 +15,9 @@
 // bitwise symmetric, which also lets both GEMM operands be read as k-contiguous rows
 // (B[k][n] = Y[n][k]).
 //
-// Data movement (sm_100a): matrices live in the k8-panel layout of common.cuh, so the 64 x 16
-// operand slice of one pipeline stage is ONE contiguous block; a producer warp streams it with
-// cp.async.bulk (TMA, SASS UBLKCP) into a 4-stage shared-memory ring, completion counted on
+// Data movement (sm_100a): matrices live in the k8-panel layout of common.cuh, so the 64 x 32
+// operand slice of one pipeline stage (four k8 panels) is ONE contiguous block; a producer warp streams it with
+// cp.async.bulk (TMA, SASS UBLKCP) into a 2-stage shared-memory ring, completion counted on
 // mbarriers (complete_tx).  Four consumer warps wait on the "full" barrier of a stage, issue the
 // FP64 tensor-core MMAs (mma.sync m8n8k4 f64 -> SASS DMMA; tcgen05 has no f64 kind) and release the
 // stage on its "empty" barrier.  There is no CTA-wide barrier in the main loop, and the producer
@@ -40,11 +40,14 @@
 
 namespace smb {
 
+// Pipeline shape: a stage holds BK = 32 contraction indices (four k8 panels: 32 KB for both operands), two
+// stages.  Measured on config 4 (all-active launch): BK 16 x 4 stages 7.20 ms, 24 x 3 7.16, 32 x 2 6.99,
+// 8 x 8 7.19 -- fewer hand-overs win slightly, the ring depth does not matter (three CTAs per SM overlap).
 #ifndef SM_BK
-#define SM_BK 16
+#define SM_BK 32
 #endif
 #ifndef SM_STAGES
-#define SM_STAGES 4
+#define SM_STAGES 2
 #endif
 constexpr int BM = TILE, BN = TILE, BK = SM_BK, STAGES = SM_STAGES, PPS = BK / 8;  // PPS: k panels per stage
 
@@ -429,6 +432,7 @@ struct NsArgs {
     const int32_t* ctrl; // [0] != 0: the evaluation has been stopped on the device (k_eval_ctrl): do nothing
     double* alpha;       // null, or [2][ngroups] rescaling factors (slot k & 1 = iteration k), reading A8b
     double* lmin;        // [ngroups] lower bound l_k the schedule tracks
+    const int2* gen_rng; // [ngroups] first / last generating row; non-null: restrict final updates (see producer)
     int32_t n_tiles;
     int32_t ngroups;
     int32_t k;
@@ -470,12 +474,20 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
         unsigned phase = 0;
         const bool stopped = a.ctrl[0] != 0;  // decided / all converged earlier in the stream: empty launch
         auto draw = [&]() { return stopped ? a.n_tiles : atomicAdd(a.sched, 1); };
+        // MODE 1 with gen_rng: a submatrix that leaves by the predicted exit (done == k + 1: this update gives its
+        // result, nothing reads it but the extraction of the generating columns, L127) only needs the tiles that
+        // hold generating rows -- as rows (ti in range) or, mirrored, as columns (tj in range); skip = 1 otherwise
         auto load_desc = [&](int tile, int4& t0, int4& t1, int& done) {
             if (tile < a.n_tiles) {
                 const int4* tdp = reinterpret_cast<const int4*>(a.tiles + tile);
                 t0 = __ldg(tdp);
                 t1 = __ldg(tdp + 1);
                 done = a.done_iter[t0.z];
+                if (MODE == 1 && a.gen_rng && done == k + 1) {
+                    const int2 gr = __ldg(a.gen_rng + t0.z);
+                    const int tl = gr.x / BM, th = gr.y / BM, ti = t1.y & 0xffff, tj = t1.y >> 16;
+                    if (!((ti >= tl && ti <= th) || (tj >= tl && tj <= th))) done = k;  // not needed: treat as stopped
+                }
             }
         };
         int tile = draw();
@@ -658,6 +670,7 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     a.ngroups = p->ngroups; a.k = k; a.decide_only = decide_only; a.eps = eps;
     const bool resc = rescale_on(p);
     a.alpha = resc ? p->d_alpha : nullptr; a.lmin = resc ? p->d_lmin : nullptr;
+    a.gen_rng = (p->opt.order == 2) ? p->d_gen_rng : nullptr;
     a.predict = (p->opt.predict != 0 && p->opt.order == 2 && eps >= 1e-13) ? 1 : 0; a.max_iter = p->opt.max_iter;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * SM_MINB);
     a.sched = p->d_sched + 4 * k;

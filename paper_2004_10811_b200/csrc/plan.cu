@@ -151,7 +151,8 @@ k_index_fill(const int32_t* __restrict__ blk_size, const int64_t* __restrict__ c
              const int32_t* __restrict__ scratch, const int64_t* __restrict__ sub_ptr,
              int32_t* __restrict__ sub_blocks, int32_t* __restrict__ sub_off, int32_t* __restrict__ sub_dim,
              int32_t* __restrict__ gen_pos, int32_t* __restrict__ gen_off, uint32_t* __restrict__ blk_pack,
-             int32_t* __restrict__ col_grp, int32_t* __restrict__ gen_width, int32_t* __restrict__ err) {
+             int32_t* __restrict__ col_grp, int32_t* __restrict__ gen_width, int2* __restrict__ gen_rng,
+             int32_t* __restrict__ err) {
     __shared__ int s_w[32];
     const int g = blockIdx.x;
     int32_t* S = sub_blocks + sub_ptr[g];
@@ -168,11 +169,12 @@ k_index_fill(const int32_t* __restrict__ blk_size, const int64_t* __restrict__ c
     }
     if (threadIdx.x == 0) sub_dim[g] = carry;
     __syncthreads();  // S, So of this group are complete and visible to the CTA
-    int gw = 0;
+    int gw = 0, glo = INT32_MAX, ghi = -1;  // first / last generating row of a_i
     for (int gc = grp_ptr[g]; gc < grp_ptr[g + 1]; ++gc) {
         const int c = grp_cols[gc];
         gw += blk_size[c];
         const int pos = find_sorted(S, m, c);
+        if (pos >= 0) { glo = min(glo, So[pos]); ghi = max(ghi, So[pos] + blk_size[c] - 1); }
         if (threadIdx.x == 0) {
             gen_pos[gc] = pos;
             col_grp[c] = g;
@@ -184,7 +186,7 @@ k_index_fill(const int32_t* __restrict__ blk_size, const int64_t* __restrict__ c
             blk_pack[p] = (t >= 0 ? (uint32_t)So[t] : 0xfffffu) | ((uint32_t)blk_size[r] << 20);
         }
     }
-    if (threadIdx.x == 0) gen_width[g] = gw;
+    if (threadIdx.x == 0) { gen_width[g] = gw; gen_rng[g] = make_int2(glo, ghi); }
 }
 
 sm_status_t launch_excl_scan(const int32_t* in, int64_t n, int64_t* out, cudaStream_t st) {
@@ -276,18 +278,21 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMemsetAsync(p->d_col_grp, 0xff, (size_t)std::max(nb, 1) * 4, st));  // -1: column of another shard
     SM_CUDA(cudaMalloc((void**)&p->d_blk_pack, std::max<int64_t>(p->nnzb, 1) * 4));
     SM_CUDA(cudaMalloc((void**)&p->d_gen_width, (size_t)std::max(ng, 1) * 4));
+    SM_CUDA(cudaMalloc((void**)&p->d_gen_rng, (size_t)std::max(ng, 1) * 8));
     // pass 2
     SM_CUDA(cudaEventRecord(ev[2], st));
     if (ng > 0) k_index_fill<<<ng, 256, 0, st>>>(p->d_blk_size, p->d_colptr, p->d_rowidx, p->d_grp_ptr, p->d_grp_cols,
                                                  d_eptr, d_scratch, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off,
                                                  p->d_sub_dim, p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_col_grp,
-                                                 p->d_gen_width, d_err);
+                                                 p->d_gen_width, p->d_gen_rng, d_err);
     SM_CUDA(cudaEventRecord(ev[3], st));
     p->launches++;
     p->h_sub_dim.resize(ng);
     p->h_sub_ptr.assign(ng + 1, 0);
     SM_CUDA(cudaMemcpyAsync(&herr, d_err, 4, cudaMemcpyDeviceToHost, st));
     if (ng) SM_CUDA(cudaMemcpyAsync(p->h_sub_dim.data(), p->d_sub_dim, (size_t)ng * 4, cudaMemcpyDeviceToHost, st));
+    p->h_gen_rng.resize((size_t)2 * ng);
+    if (ng) SM_CUDA(cudaMemcpyAsync(p->h_gen_rng.data(), p->d_gen_rng, (size_t)ng * 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaMemcpyAsync(p->h_sub_ptr.data(), p->d_sub_ptr, (size_t)(ng + 1) * 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));  // sizes for the workspace geometry and tile list below
     SM_CUDA(cudaGetLastError());
@@ -346,6 +351,21 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
         p->h_tile_count[i] = (int32_t)tiles.size() - p->h_tile_first[i];
     }
     p->n_tiles = (int64_t)tiles.size();
+    // algorithmic flop of the last update of a submatrix that leaves by the predicted exit: only the tiles that
+    // hold generating rows (as rows, or mirrored as columns) are computed (ns_sign.cu)
+    p->h_final_flop.assign(ng, 0);
+    for (int i = 0; i < ng; ++i) {
+        const int ld = p->h_ld[i], n = p->h_sub_dim[i], nt = (ld + TILE - 1) / TILE;
+        const int tl = p->h_gen_rng[2 * i] / TILE, th = p->h_gen_rng[2 * i + 1] / TILE;
+        int64_t f = 0;
+        for (int ti = 0; ti < nt; ++ti)
+            for (int tj = 0; tj <= ti; ++tj) {
+                if (!((ti >= tl && ti <= th) || (tj >= tl && tj <= th))) continue;
+                const int64_t ri = std::max(0, std::min(TILE, n - ti * TILE)), rj = std::max(0, std::min(TILE, n - tj * TILE));
+                f += (ti == tj ? ri * (ri + 1) : 2 * ri * rj) * (int64_t)n;
+            }
+        p->h_final_flop[i] = f;
+    }
     if ((s = upload(&p->d_ld, p->h_ld.data(), ng, st))) return s;
     if ((s = upload(&p->d_ws_off, p->h_ws_off.data(), ng, st))) return s;
     if ((s = upload(&p->d_tiles, tiles.data(), tiles.size(), st))) return s;
