@@ -130,6 +130,7 @@ struct sm_plan {
     double* d_lmin = nullptr;              // [ngroups] tracked lower bound l_k of the schedule
     double* h_lz = nullptr;                // pinned [66]: lo, hi, Ritz values [32], cumulative quadrature weights [32]
     int lz_nodes = 0;
+    int lz_grid = 0;                       // CTAs of the cooperative Lanczos launch
     int lz_valid = 0;                      // lz_lo / lz_hi belong to the current call's values
     int lz_ok = 0;                         // the run did not break down: cap, bracket and quadrature may be used
     int ns_attr_set = 0, tf32_attr_set = 0;  // dynamic shared-memory opt-in done on this plan's device

@@ -570,20 +570,33 @@ sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const doub
     k_nelec_bound<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_col_grp, p->d_blk_size, p->d_gen_off, p->d_ld, p->d_ws_off,
                                                    p->d_done_iter, p->d_gersh, k, buf0, buf1, bufY, p->d_bound_part,
                                                    p->d_ctrl, rescale_on(p) ? p->d_alpha : nullptr, p->ngroups);
-    k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part, p->nb, p->d_bound + 2 * k);
-    k_sum_fixed<<<1, 1024, 0, st>>>(p->d_bound_part + p->nb, p->nb, p->d_bound + 2 * k + 1);
-    p->launches += 3;
+    p->launches += 1;  // the two sums are taken by k_eval_ctrl
     SM_CUDA(cudaGetLastError());
     return SM_OK;
 }
 
-// Device-side end of an evaluation (one thread, after k_ns_decide and k_nelec_bound of iteration k).
-__global__ void k_eval_ctrl(EvalCtrl* __restrict__ c, int k, const int32_t* __restrict__ counters,
-                            const double* __restrict__ bound, int steer, double n_target, double margin) {
-    if (threadIdx.x != 0 || blockIdx.x != 0 || c->stop != 0) return;
+// Device-side end of an evaluation (one CTA, after k_ns_decide and k_nelec_bound of iteration k): the fixed-order
+// sums of the steering partials (count of X_k and its bound; same order as k_sum_fixed), then the decision.
+__global__ void __launch_bounds__(1024)
+k_eval_ctrl(EvalCtrl* __restrict__ c, int k, const int32_t* __restrict__ counters, double* __restrict__ bound,
+            const double* __restrict__ bound_part, int nb, int steer, double n_target, double margin) {
+    __shared__ double s0[1024], s1[1024];
+    if (c->stop != 0) return;  // uniform: set by an earlier launch
+    if (steer && k >= 1) {
+        double a = 0.0, b = 0.0;
+        for (int i = threadIdx.x; i < nb; i += 1024) { a += bound_part[i]; b += bound_part[nb + i]; }
+        s0[threadIdx.x] = a; s1[threadIdx.x] = b;
+        __syncthreads();
+        for (int o = 512; o > 0; o >>= 1) {
+            if ((int)threadIdx.x < o) { s0[threadIdx.x] += s0[threadIdx.x + o]; s1[threadIdx.x] += s1[threadIdx.x + o]; }
+            __syncthreads();
+        }
+    }
+    if (threadIdx.x != 0) return;
+    if (steer && k >= 1) { bound[2 * k] = s0[0]; bound[2 * k + 1] = s1[0]; }
     if (counters[k] == 0) { c->stop = 1; c->k_stop = k; return; }
     if (steer && k >= 1) {
-        const double ne = bound[2 * k], err = bound[2 * k + 1];
+        const double ne = s0[0], err = s1[0];
         if (ne == ne && err == err && err >= 0.0) {
             const double g = ne - n_target, m = err + margin;
             if (g > m || g < -m) { c->stop = 2; c->k_stop = k; c->decided = g > 0 ? 1 : -1; c->ne = ne; c->err = err; }
@@ -592,8 +605,8 @@ __global__ void k_eval_ctrl(EvalCtrl* __restrict__ c, int k, const int32_t* __re
 }
 
 sm_status_t launch_eval_ctrl(sm_plan* p, int k, int steer, double n_target, double margin, cudaStream_t st) {
-    k_eval_ctrl<<<1, 32, 0, st>>>(reinterpret_cast<EvalCtrl*>(p->d_ctrl), k, p->d_counters, p->d_bound, steer, n_target,
-                                  margin);
+    k_eval_ctrl<<<1, 1024, 0, st>>>(reinterpret_cast<EvalCtrl*>(p->d_ctrl), k, p->d_counters, p->d_bound, p->d_bound_part,
+                                    p->nb, steer, n_target, margin);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;

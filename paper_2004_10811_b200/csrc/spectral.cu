@@ -12,6 +12,8 @@
 // of its spectral radius (largest column 2-norm of a_i - mu I, from the gather); (iii) s_i never exceeds
 // the submatrix's own Gershgorin bound.  All arithmetic runs on the device; the host only sequences
 // the launches and reads the resulting doubles.
+#include <cooperative_groups.h>
+
 #include "common.cuh"
 
 namespace smb {
@@ -53,100 +55,6 @@ __device__ __forceinline__ double lz_col(int lane, int oc, int64_t p0, int64_t p
     return dot;
 }
 
-__global__ void __launch_bounds__(256)
-k_lz_spmv(int nb, const int32_t* __restrict__ blk_size, const int32_t* __restrict__ blk_off,
-          const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx,
-          const int64_t* __restrict__ val_off, const double* __restrict__ vals, const double* __restrict__ x,
-          double* __restrict__ y, double* __restrict__ part) {
-    const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (c >= nb) return;
-    const int lane = threadIdx.x & 31;
-    const int bc = blk_size[c], oc = blk_off[c];
-    const int64_t p0 = colptr[c], p1 = colptr[c + 1];
-    double dot = 0.0;
-    switch (bc) {
-        case 1: dot = lz_col<1>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, x, y); break;
-        case 4: dot = lz_col<4>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, x, y); break;
-        case 5: dot = lz_col<5>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, x, y); break;
-        case 13: dot = lz_col<13>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, x, y); break;
-        default:
-            for (int q = 0; q < bc; ++q) {
-                double a = 0.0;
-                for (int64_t b = p0 + lane; b < p1; b += 32) {
-                    const int r = rowidx[b];
-                    const int br = blk_size[r];
-                    const double* col = vals + val_off[b] + (size_t)q * br;
-                    const double* xr = x + blk_off[r];
-                    for (int e = 0; e < br; ++e) a = fma(col[e], xr[e], a);
-                }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-                if (lane == 0) y[oc + q] = a;
-                dot = fma(a, x[oc + q], dot);
-            }
-    }
-    if (lane == 0) part[c] = dot;
-}
-
-// Deterministic 1-CTA sum; mode 0: out = sum, mode 1: out = sqrt(sum).
-__global__ void k_lz_reduce(const double* __restrict__ in, int n, double* __restrict__ out, int mode) {
-    __shared__ double s[1024];
-    double a = 0.0;
-    for (int i = threadIdx.x; i < n; i += 1024) a += in[i];
-    s[threadIdx.x] = a;
-    __syncthreads();
-    for (int o = 512; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) *out = mode ? sqrt(s[0]) : s[0];
-}
-
-// w = w - alpha v - beta_prev v_prev; part[block] = partial ||w||^2 (fixed order inside the CTA).
-__global__ void __launch_bounds__(256)
-k_lz_axpy(int64_t n, double* __restrict__ w, const double* __restrict__ v, const double* __restrict__ vprev,
-          const double* __restrict__ alpha, const double* __restrict__ beta_prev, double* __restrict__ part) {
-    __shared__ double s[256];
-    const double al = *alpha, be = beta_prev ? *beta_prev : 0.0;
-    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
-    const int64_t b = (int64_t)blockIdx.x * per, e = min(b + per, n);
-    double a = 0.0;
-    for (int64_t i = b + threadIdx.x; i < e; i += 256) {
-        const double t = w[i] - al * v[i] - be * vprev[i];
-        w[i] = t;
-        a = fma(t, t, a);
-    }
-    s[threadIdx.x] = a;
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) part[blockIdx.x] = s[0];
-}
-
-// vnext = w / beta (zero vector after a breakdown: the run then appends decoupled zeros to T,
-// which can only widen the interval).
-__global__ void k_lz_scale(int64_t n, const double* __restrict__ w, const double* __restrict__ beta,
-                           double* __restrict__ vnext) {
-    const double be = *beta;
-    const double inv = be > 1e-300 ? 1.0 / be : 0.0;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        vnext[i] = w[i] * inv;
-}
-
-// Start vector: +-1/sqrt(n) by an integer hash of the index (deterministic, not orthogonal to
-// anything in particular).
-__global__ void k_lz_start(int64_t n, double* __restrict__ v, double* __restrict__ vprev) {
-    const double a = rsqrt((double)n);
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        unsigned h = (unsigned)i * 2654435761u;
-        h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
-        v[i] = (h & 1u) ? a : -a;
-        vprev[i] = 0.0;
-    }
-}
-
 // Gauss quadrature of the k x k Lanczos tridiagonal T (diag alpha, off-diagonal beta): thread j finds
 // the j-th Ritz value by bisection on Sturm counts and its weight = squared first component of the
 // eigenvector (1 / sum_i p_i(theta)^2 with the normalised Lanczos polynomials p_i).  out[0], out[1]:
@@ -155,9 +63,8 @@ __global__ void k_lz_start(int64_t n, double* __restrict__ v, double* __restrict
 // fraction of eigenvalues of K~ below the node (used for the first interior step of the mu search,
 // DESIGN.md reading A11d); out[66] = 1.0 if the recurrence broke down (some beta_i, i < k - 1, not above
 // 1e-10 of the largest entry of T: everything after it is rounding noise), else 0.0.  One warp; k <= 32.
-__global__ void k_lz_quadrature(int k, const double* __restrict__ alpha, const double* __restrict__ beta,
-                                double margin, double* __restrict__ out) {
-    __shared__ double th[32], wt[32];
+__device__ void lz_quadrature_body(int k, const double* __restrict__ alpha, const double* __restrict__ beta,
+                                   double margin, double* __restrict__ out, double* th, double* wt) {
     const int j = threadIdx.x;
     double glo = 1e300, ghi = -1e300, tscale = 0.0;
     for (int i = 0; i < k; ++i) {
@@ -215,6 +122,114 @@ __global__ void k_lz_quadrature(int k, const double* __restrict__ alpha, const d
     }
 }
 
+// The whole Lanczos run in ONE cooperative launch (grid-wide barriers instead of ~5 launches per step):
+// start vector; per step  w = K v (block-CSC mat-vec, one warp per block column, columns dealt to the warps
+// in a fixed order), alpha = w.v, w -= alpha v + beta_prev v_prev, beta = ||w||, v_next = w / beta;
+// finally the Gauss quadrature of T.  Reductions: per-CTA partials in a fixed order, then the same fixed-order
+// sum over the CTAs in every thread that needs it -- deterministic, no floating-point atomics.
+__global__ void __launch_bounds__(256)
+k_lz_fused(int nb, int64_t n, int steps, const int32_t* __restrict__ blk_size, const int32_t* __restrict__ blk_off,
+           const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx, const int64_t* __restrict__ val_off,
+           const double* __restrict__ vals, double* __restrict__ vb0, double* __restrict__ vb1, double* __restrict__ vb2,
+           double* __restrict__ alpha, double* __restrict__ beta, double* __restrict__ part, double margin,
+           double* __restrict__ outp) {
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    __shared__ double s_red[8];
+    __shared__ double s_th[32], s_wt[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int gw = blockIdx.x * 8 + wid, nwarps = gridDim.x * 8;
+    const int64_t gtid = (int64_t)blockIdx.x * 256 + threadIdx.x, gthreads = (int64_t)gridDim.x * 256;
+    double *vprev = vb0, *v = vb1, *w = vb2;
+    {   // start vector: +-1/sqrt(n) by an integer hash of the index
+        const double a = rsqrt((double)n);
+        for (int64_t i = gtid; i < n; i += gthreads) {
+            unsigned h = (unsigned)i * 2654435761u;
+            h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
+            v[i] = (h & 1u) ? a : -a;
+            vprev[i] = 0.0;
+        }
+    }
+    grid.sync();
+    auto cta_sum = [&](double x) {  // fixed-order sum over the CTA's 8 warps; valid in thread 0
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        if (lane == 0) s_red[wid] = x;
+        __syncthreads();
+        double t = 0.0;
+        if (threadIdx.x == 0)
+            for (int q = 0; q < 8; ++q) t += s_red[q];
+        __syncthreads();
+        return t;
+    };
+    auto grid_sum = [&](const double* p) {  // the same fixed-order sum over the per-CTA partials in every warp
+        double t = 0.0;
+        for (int q = lane; q < (int)gridDim.x; q += 32) t += p[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        return t;
+    };
+    double be_prev = 0.0;
+    for (int j = 0; j < steps; ++j) {
+        // w = K v, partial of w.v
+        double dot = 0.0;
+        for (int c = gw; c < nb; c += nwarps) {
+            const int bc = blk_size[c], oc = blk_off[c];
+            const int64_t p0 = colptr[c], p1 = colptr[c + 1];
+            double d;
+            switch (bc) {
+                case 1: d = lz_col<1>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, v, w); break;
+                case 4: d = lz_col<4>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, v, w); break;
+                case 5: d = lz_col<5>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, v, w); break;
+                case 13: d = lz_col<13>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, v, w); break;
+                default:
+                    d = 0.0;
+                    for (int q = 0; q < bc; ++q) {
+                        double a = 0.0;
+                        for (int64_t b = p0 + lane; b < p1; b += 32) {
+                            const int r = rowidx[b];
+                            const int br = blk_size[r];
+                            const double* col = vals + val_off[b] + (size_t)q * br;
+                            const double* xr = v + blk_off[r];
+                            for (int e = 0; e < br; ++e) a = fma(col[e], xr[e], a);
+                        }
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                        if (lane == 0) w[oc + q] = a;
+                        d = fma(a, v[oc + q], d);
+                    }
+            }
+            dot += d;  // identical in every lane
+        }
+        {
+            const double t = cta_sum(lane == 0 ? dot : 0.0);
+            if (threadIdx.x == 0) part[blockIdx.x] = t;
+        }
+        grid.sync();
+        const double al = grid_sum(part);
+        if (gtid == 0) alpha[j] = al;
+        // w -= alpha v + beta_prev v_prev, partial of ||w||^2
+        double nrm = 0.0;
+        for (int64_t i = gtid; i < n; i += gthreads) {
+            const double t = w[i] - al * v[i] - be_prev * vprev[i];
+            w[i] = t;
+            nrm = fma(t, t, nrm);
+        }
+        {
+            const double t = cta_sum(nrm);
+            if (threadIdx.x == 0) part[gridDim.x + blockIdx.x] = t;
+        }
+        grid.sync();
+        const double be = sqrt(grid_sum(part + gridDim.x));
+        if (gtid == 0) beta[j] = be;
+        const double inv = be > 1e-300 ? 1.0 / be : 0.0;
+        for (int64_t i = gtid; i < n; i += gthreads) vprev[i] = w[i] * inv;  // v_{j+1} over v_{j-1}
+        grid.sync();
+        double* t = vprev; vprev = v; v = t;
+        be_prev = be;
+    }
+    if (blockIdx.x == 0 && threadIdx.x < 32) lz_quadrature_body(steps, alpha, beta, margin, outp, s_th, s_wt);
+}
+
 // s_g <- min(Gershgorin_g, max(cap, rho_lo_g)) / overshoot  (in place, bits of a double as written by
 // k_gather; rho_lo_g = largest column 2-norm of a_g - mu I, a rigorous lower bound of its spectral radius:
 // the estimated cap is never taken below it).
@@ -252,35 +267,28 @@ sm_status_t launch_apply_scale(sm_plan* p, double cap, double overshoot, double 
 }
 
 // Lanczos estimate of [lambda_min, lambda_max] of K~ -> p->lz_lo / p->lz_hi (host), widened by 3 %
-// of the spread.  ~5 small launches per step, LZ_STEPS steps.
+// of the spread, + the quadrature nodes.  One cooperative launch, LZ_STEPS steps.
 sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st) {
-    const int64_t n = p->info.n_basis;
-    if (n == 0 || p->nb == 0) { p->lz_lo = p->lz_hi = 0.0; return SM_OK; }
-    if (!p->d_lz) SM_CUDA(cudaMalloc((void**)&p->d_lz, (size_t)(3 * n + 2 * LZ_STEPS + 72 + std::max<int64_t>(p->nb, 1024)) * 8));
-    double* vb[3] = {p->d_lz, p->d_lz + n, p->d_lz + 2 * n};
+    int64_t n = p->info.n_basis;
+    if (n == 0 || p->nb == 0) { p->lz_lo = p->lz_hi = 0.0; p->lz_ok = 0; return SM_OK; }
+    if (!p->lz_grid) {  // as many CTAs as are co-resident (grid-wide barriers), at most 4 per SM
+        int per_sm = 0;
+        SM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_lz_fused, 256, 0));
+        if (per_sm < 1) return SM_ERR_CUDA;
+        p->lz_grid = p->num_sms * std::min(per_sm, 4);
+    }
+    if (!p->d_lz) SM_CUDA(cudaMalloc((void**)&p->d_lz, (size_t)(3 * n + 2 * LZ_STEPS + 72 + 2 * p->lz_grid) * 8));
+    double *vb0 = p->d_lz, *vb1 = p->d_lz + n, *vb2 = p->d_lz + 2 * n;
     double* alpha = p->d_lz + 3 * n;
     double* beta = alpha + LZ_STEPS;
     double* outp = beta + LZ_STEPS;
     double* part = outp + 72;
-    const int steps = (int)std::min<int64_t>(LZ_STEPS, n);
-    const int ew = (int)std::min<int64_t>((n + 255) / 256, 592);
-    const int nred = 296;
-    double *vprev = vb[0], *v = vb[1], *w = vb[2];
-    k_lz_start<<<ew, 256, 0, st>>>(n, v, vprev);
+    int steps = (int)std::min<int64_t>(LZ_STEPS, n), nb = p->nb;
+    double margin = 0.03;
+    void* args[] = {&nb, &n, &steps, &p->d_blk_size, &p->d_blk_off, &p->d_colptr, &p->d_rowidx, &p->d_val_off, &vals,
+                    &vb0, &vb1, &vb2, &alpha, &beta, &part, &margin, &outp};
+    SM_CUDA(cudaLaunchCooperativeKernel((const void*)k_lz_fused, dim3(p->lz_grid), dim3(256), args, 0, st));
     p->launches++;
-    for (int j = 0; j < steps; ++j) {
-        k_lz_spmv<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_blk_size, p->d_blk_off, p->d_colptr, p->d_rowidx,
-                                                   p->d_val_off, vals, v, w, part);
-        k_lz_reduce<<<1, 1024, 0, st>>>(part, p->nb, alpha + j, 0);
-        k_lz_axpy<<<nred, 256, 0, st>>>(n, w, v, vprev, alpha + j, j > 0 ? beta + j - 1 : nullptr, part);
-        k_lz_reduce<<<1, 1024, 0, st>>>(part, nred, beta + j, 1);
-        k_lz_scale<<<ew, 256, 0, st>>>(n, w, beta + j, vprev);
-        p->launches += 5;
-        double* t = vprev; vprev = v; v = t;  // v_{j+1} was written over v_{j-1}
-    }
-    k_lz_quadrature<<<1, 32, 0, st>>>(steps, alpha, beta, 0.03, outp);
-    p->launches++;
-    SM_CUDA(cudaGetLastError());
     SM_CUDA(cudaMemcpyAsync(p->h_lz, outp, 67 * 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));
     p->lz_lo = p->h_lz[0];
