@@ -488,19 +488,6 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         if (fl[i] == 2 && p->opt.order == 2 && p->opt.precision == 0) symf += p->h_final_flop[i] - n * n * (n + 1);
     }
     *not_conv = nc;
-    if (getenv("SM_DEBUG_RES")) {
-        for (int slot = 0; slot < 2; ++slot) {
-            std::vector<double> v(res + (size_t)slot * ng, res + (size_t)(slot + 1) * ng);
-            std::sort(v.begin(), v.end());
-            if (ng) fprintf(stderr, "res slot %d (cur_k %d): min %.3e q10 %.3e med %.3e q90 %.3e q99 %.3e max %.3e\n", slot, p->cur_k,
-                            v[0], v[ng / 10], v[ng / 2], v[ng * 9 / 10], v[ng * 99 / 100], v[ng - 1]);
-        }
-    }
-    if (getenv("SM_DEBUG_ITERS")) {
-        int hist[2][32] = {{0}};
-        for (int i = 0; i < ng; ++i) if (di[i] >= 0 && di[i] < 32) hist[fl[i] == 2][di[i]]++;
-        for (int k = 0; k < 32; ++k) if (hist[0][k] || hist[1][k]) fprintf(stderr, "iter %d: measured %d predicted %d\n", k, hist[0][k], hist[1][k]);
-    }
     if (stats) {
         stats->iter_min = ng ? imin : 0;
         stats->iter_max = imax;
