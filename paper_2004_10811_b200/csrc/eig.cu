@@ -54,9 +54,10 @@ struct EigArgs {
 // so that c^2 + s^2 = 1 to FP64 rounding: V stays orthogonal.  ~20 FP64 instructions instead of a FP64
 // division, square root and reciprocal square root (~150), which bounded the first version of this kernel.
 __device__ __forceinline__ void rotation(double a, double b, double g, double& c, double& s, double& t) {
-    const float zf = (float)(b - a) / (2.0f * (float)g);
+    // fast FP32 intrinsics (2 ulp): the tangent only has to be good to ~1e-6
+    const float zf = __fdividef((float)(b - a), 2.0f * (float)g);
     const float az = fabsf(zf);
-    float tf = az < 1e15f ? 1.0f / (az + sqrtf(fmaf(az, az, 1.0f))) : 0.5f / az;
+    float tf = az < 1e15f ? __frcp_rn(az + __fsqrt_rn(fmaf(az, az, 1.0f))) : __fdividef(0.5f, az);
     tf = zf >= 0.0f ? tf : -tf;
     t = (double)tf;
     const double x = fma(t, t, 1.0);

@@ -29,7 +29,14 @@
 
 namespace smb {
 
-constexpr int R_BM = 128, R_BN = 256, R_BK = 32, R_STAGES = 4;
+// R_CTAS = 1: one CTA per SM, 4-stage ring, two 256-column accumulators (epilogue of a tile overlaps the MMAs of
+// the next).  R_CTAS = 2: two CTAs per SM, each with a 2-stage ring and ONE 256-column accumulator: the overlap
+// comes from the other CTA, and every SM has two producers, two MMA issuers and eight epilogue warps.
+#ifndef R_CTAS
+#define R_CTAS 2
+#endif
+constexpr int R_BM = 128, R_BN = 256, R_BK = 32, R_STAGES = R_CTAS == 1 ? 4 : 2;
+constexpr int R_TBUFS = R_CTAS == 1 ? 2 : 1, R_TCOLS = R_CTAS == 1 ? 512 : 256;
 constexpr int R_STAGE_FLOATS = (R_BM + R_BN) * R_BK;  // 48 KB
 constexpr size_t R_SMEM = (size_t)R_STAGES * R_STAGE_FLOATS * sizeof(float);
 constexpr int R_THREADS = 192;
@@ -102,6 +109,17 @@ __device__ __forceinline__ float r_tf32(float x) {
     uint32_t u;
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(x));
     return __uint_as_float(u);
+}
+
+// 4 x 4 transpose inside every quad of lanes: lane 4m + i holds row i (w[0..3]) and ends with column i.
+__device__ __forceinline__ void quad_transpose(float (&w)[4], int lane) {
+    const bool o1 = lane & 1, o2 = lane & 2;
+    float s0 = o1 ? w[0] : w[1], s1 = o1 ? w[2] : w[3];
+    float r0 = __shfl_xor_sync(0xffffffffu, s0, 1), r1 = __shfl_xor_sync(0xffffffffu, s1, 1);
+    if (o1) { w[0] = r0; w[2] = r1; } else { w[1] = r0; w[3] = r1; }
+    s0 = o2 ? w[0] : w[2]; s1 = o2 ? w[1] : w[3];
+    r0 = __shfl_xor_sync(0xffffffffu, s0, 2); r1 = __shfl_xor_sync(0xffffffffu, s1, 2);
+    if (o2) { w[0] = r0; w[1] = r1; } else { w[2] = r0; w[3] = r1; }
 }
 
 // One work unit of the reduced-precision GEMMs.
@@ -199,7 +217,7 @@ struct Ns32Args {
 //            product is hi hi + hi lo + lo hi accumulated in the same FP32 TMEM tile (FP32-class
 //            accuracy, three MMAs per k step, 16-wide k slices so that a stage stays 48 KB).
 template <int MODE, int SPLIT>
-__global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
+__global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
     constexpr int BK = SPLIT ? R_BK / 2 : R_BK;     // k columns per stage
     constexpr int PL = SPLIT ? 2 : 1;               // operand planes
     constexpr int SA = R_BM * BK;                   // floats of one 128-row operand plane in a stage
@@ -213,7 +231,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (wid == 1) {  // tensor memory: all 512 columns (one CTA per SM), two 256-column accumulators
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(r_smem_u32(&s_tmem)), "n"(512));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(r_smem_u32(&s_tmem)), "n"(R_TCOLS));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -303,7 +321,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
                 }
                 r_commit(&s_tfull[buf]);        // accumulator complete
                 tphase[buf] ^= 1;
-                buf ^= 1;
+                if (R_TBUFS == 2) buf ^= 1;
             }
         }
     } else {
@@ -325,24 +343,52 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
             float* orow = a.Out + T.off32 + (size_t)row0 * ldp + (size_t)rl * 4;
             const float* xrow = a.A + T.off32 + (size_t)row0 * ldp + (size_t)rl * 4;
             double part = 0.0;
-            for (int c0 = 0; c0 < ncols; c0 += 16) {
-                uint32_t v[16];
+            // Software pipeline over the 16-column chunks: the tensor-memory load of chunk c + 1 and (MODE 1) the
+            // global loads of its X values are issued before chunk c is processed, so their latencies pass
+            // behind the arithmetic and the stores of chunk c.
+            uint32_t v[16], vn[16];
+            float4 xc[4], xn[4], xlc[4], xln[4];
+            auto tld = [&](uint32_t (&d)[16], int c0) {
                 asm volatile(
                     "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                    : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                      "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                    : "=r"(d[0]), "=r"(d[1]), "=r"(d[2]), "=r"(d[3]), "=r"(d[4]), "=r"(d[5]), "=r"(d[6]), "=r"(d[7]),
+                      "=r"(d[8]), "=r"(d[9]), "=r"(d[10]), "=r"(d[11]), "=r"(d[12]), "=r"(d[13]), "=r"(d[14]), "=r"(d[15])
                     : "r"(taddr + (uint32_t)c0));
+            };
+            auto xld = [&](float4 (&x)[4], float4 (&xl)[4], int c0) {  // MODE 1: X (and its lo plane) of this row
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int c = col0 + c0 + 4 * j;
+                    x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    xl[j] = x[j];
+                    if (rl < rows_a && c <= r) {
+                        const size_t o = (size_t)(c >> 2) * rows_a * 4;
+                        x[j] = *reinterpret_cast<const float4*>(xrow + o);
+                        if (SPLIT) xl[j] = *reinterpret_cast<const float4*>(xrow + o + a.lo_plane);
+                    }
+                }
+            };
+            tld(v, 0);
+            if (MODE == 1) xld(xc, xlc, 0);
+            for (int c0 = 0; c0 < ncols; c0 += 16) {
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (rl < rows_a) {
+                const bool more = c0 + 16 < ncols;
+                if (more) {
+                    tld(vn, c0 + 16);
+                    if (MODE == 1) xld(xn, xln, c0 + 16);
+                }
+                {
+                    const bool row_ok = rl < rows_a;
+                    const int rq = r & ~3;  // first row of this lane's quad (rows_a is a multiple of 16: quads are whole)
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         const int c = col0 + c0 + 4 * j;
-                        if (c > r) continue;  // upper triangle: the mirror image of (c, r) is stored instead
+                        const bool act = row_ok && c <= r;  // upper triangle: the mirror image of (c, r) is stored instead
                         const size_t o = (size_t)(c >> 2) * rows_a * 4;
                         float w[4] = {__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
                                       __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3])};
                         if (MODE == 0) {
-                            if (r < n) {  // residual over the n x n part; strictly-lower elements count twice
+                            if (act && r < n) {  // residual over the n x n part; strictly-lower elements count twice
                                 float p = 0.f;
 #pragma unroll
                                 for (int e = 0; e < 4; ++e) {
@@ -353,11 +399,8 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
                                 part += (double)p;
                             }
                         } else {
-                            float4 x = *reinterpret_cast<const float4*>(xrow + o);
-                            if (SPLIT) {
-                                const float4 xl = *reinterpret_cast<const float4*>(xrow + o + a.lo_plane);
-                                x.x += xl.x; x.y += xl.y; x.z += xl.z; x.w += xl.w;
-                            }
+                            float4 x = xc[j];
+                            if (SPLIT) { x.x += xlc[j].x; x.y += xlc[j].y; x.z += xlc[j].z; x.w += xlc[j].w; }
                             w[0] = 1.5f * x.x - 0.5f * w[0]; w[1] = 1.5f * x.y - 0.5f * w[1];
                             w[2] = 1.5f * x.z - 0.5f * w[2]; w[3] = 1.5f * x.w - 0.5f * w[3];
                         }
@@ -368,28 +411,51 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
                             lo[e] = w[e] - hi[e];
                         }
                         // direct elements (r, c + e), c + e <= r: one 16-byte store when the whole group is
-                        // on or below the diagonal; mirror elements (c + e, r), c + e < r: 4-byte stores.
-                        // Every stored element has exactly one writer, so X and Y stay bitwise symmetric,
-                        // which is what lets B be read as rows (and keeps the iteration stable: the
-                        // X X^T form amplifies any antisymmetric rounding noise).
-                        if (c + 3 <= r) {
-                            *reinterpret_cast<float4*>(orow + o) = make_float4(hi[0], hi[1], hi[2], hi[3]);
-                            if (SPLIT) *reinterpret_cast<float4*>(orow + o + a.lo_plane) = make_float4(lo[0], lo[1], lo[2], lo[3]);
-                        } else {
+                        // on or below the diagonal.  Every stored element has exactly one writer, so X and Y stay
+                        // bitwise symmetric, which is what lets B be read as rows (and keeps the iteration
+                        // stable: the X X^T form amplifies any antisymmetric rounding noise).
+                        if (act) {
+                            if (c + 3 <= r) {
+                                *reinterpret_cast<float4*>(orow + o) = make_float4(hi[0], hi[1], hi[2], hi[3]);
+                                if (SPLIT) *reinterpret_cast<float4*>(orow + o + a.lo_plane) = make_float4(lo[0], lo[1], lo[2], lo[3]);
+                            } else {
+#pragma unroll
+                                for (int e = 0; e < 4; ++e)
+                                    if (c + e <= r) {
+                                        orow[o + e] = hi[e];
+                                        if (SPLIT) orow[o + e + a.lo_plane] = lo[e];
+                                    }
+                            }
+                        }
+                        // mirror elements (c + e, r), c + e < r.  A quad of lanes (rows rq .. rq + 3) holds a 4 x 4
+                        // block; when it lies strictly below the diagonal it is transposed inside the quad (four
+                        // shuffles per plane, executed by every lane) and lane e stores mirror row c + e as ONE
+                        // 16-byte store; blocks touching the diagonal keep the 4-byte stores.
+                        const bool blk = row_ok && c + 3 < rq;
+                        float th[4] = {hi[0], hi[1], hi[2], hi[3]}, tl[4] = {lo[0], lo[1], lo[2], lo[3]};
+                        quad_transpose(th, lane);
+                        if (SPLIT) quad_transpose(tl, lane);
+                        if (blk) {
+                            float* mp = a.Out + T.off32 + panel32_off(c + (lane & 3), rq, ldp);
+                            *reinterpret_cast<float4*>(mp) = make_float4(th[0], th[1], th[2], th[3]);
+                            if (SPLIT) *reinterpret_cast<float4*>(mp + a.lo_plane) = make_float4(tl[0], tl[1], tl[2], tl[3]);
+                        } else if (act) {
 #pragma unroll
                             for (int e = 0; e < 4; ++e)
-                                if (c + e <= r) {
-                                    orow[o + e] = hi[e];
-                                    if (SPLIT) orow[o + e + a.lo_plane] = lo[e];
+                                if (c + e < r) {
+                                    float* mp = a.Out + T.off32 + panel32_off(c + e, r, ldp);
+                                    *mp = hi[e];
+                                    if (SPLIT) mp[a.lo_plane] = lo[e];
                                 }
                         }
+                    }
+                }
+                if (more) {
 #pragma unroll
-                        for (int e = 0; e < 4; ++e)
-                            if (c + e < r) {
-                                float* mp = a.Out + T.off32 + panel32_off(c + e, r, ldp);
-                                *mp = hi[e];
-                                if (SPLIT) mp[a.lo_plane] = lo[e];
-                            }
+                    for (int e = 0; e < 16; ++e) v[e] = vn[e];
+                    if (MODE == 1) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) { xc[j] = xn[j]; xlc[j] = xln[j]; }
                     }
                 }
             }
@@ -401,12 +467,12 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_ns_tf32(Ns32Args a) {
                 for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
                 if (lane == 0) a.partials[(size_t)T.tile * 4 + q] = part;
             }
-            buf ^= 1;
+            if (R_TBUFS == 2) buf ^= 1;
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
-    if (wid == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+    if (wid == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(R_TCOLS));
 }
 
 // Residual decision of the reduced-precision iteration: like k_ns_decide, but the residual has a
@@ -529,7 +595,7 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
     a.n_tiles = (int32_t)p->n_tiles32; a.ctrl = p->d_ctrl;
     const bool split = p->opt.precision == 2;
     a.lo_plane = split ? p->sum_ldp2 : 0;
-    const int grid = (int)std::min<int64_t>(p->n_tiles32, p->num_sms);
+    const int grid = (int)std::min<int64_t>(p->n_tiles32, (int64_t)p->num_sms * R_CTAS);
     if (which & 1) {
         a.A = X[k & 1]; a.B = X[k & 1]; a.Out = Y;
         if (split) k_ns_tf32<0, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
