@@ -92,7 +92,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_partials, p->d_counters, p->d_sched, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
                     p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_col_rec, p->d_gg, p->d_ctrl, p->d_gl_ptr, p->d_gl,
-                    p->d_alpha, p->d_lmin, p->d_eig_ptr, p->d_eig_lam, p->d_eig_w, p->d_eig_sigma, p->d_eig_order,
+                    p->d_alpha, p->d_lmin, p->d_lz_rec, p->d_eig_ptr, p->d_eig_lam, p->d_eig_w, p->d_eig_sigma, p->d_eig_order,
                     p->d_eig_state};
     for (void* q : ptrs)
         if (q) cudaFree(q);
@@ -421,6 +421,10 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
     int k = k_begin, since = 0;
     bool stopped = false;
     sm_status_t s;
+    // how far to enqueue before the first look at the control block: what the previous evaluation of this plan
+    // needed, plus two (launches behind the device-side stop are empty but not free), at most check_every
+    int batch = p->opt.check_every;
+    if (p->last_eval_iters > 0) batch = std::min(batch, p->last_eval_iters + 2);
     for (; k < k_end && k <= max_iter && !stopped; ++k) {
         const int last = k == max_iter ? 1 : 0;
         if ((s = launch_pair(p, k, eps, last, b, st, 1))) return s;
@@ -428,15 +432,17 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
         if (steer_k && (s = launch_nelec_bound(p, k, b.b0, b.b1, b.y, st))) return s;
         if ((s = launch_eval_ctrl(p, k, steer_k, steer ? steer->n_target : 0.0, margin, st))) return s;
         if (!last && (s = launch_pair(p, k, eps, 0, b, st, 2))) return s;
-        if (++since >= p->opt.check_every || last || k == k_end - 1) {
+        if (++since >= batch || last || k == k_end - 1) {
             SM_CUDA(cudaMemcpyAsync(p->h_ctrl, p->d_ctrl, sizeof(EvalCtrl), cudaMemcpyDeviceToHost, st));
             SM_CUDA(cudaStreamSynchronize(st));
             since = 0;
+            batch = std::min(p->opt.check_every, 4);  // the estimate was short: continue in small batches
             stopped = hc->stop != 0;
         }
     }
     if (stopped) {
         const int ks = hc->k_stop;
+        if (hc->stop == 1) p->last_eval_iters = ks - k_begin + 1;  // a converged evaluation: the next one will be alike
         p->cur_k = ks;
         (*launched) += (ks - k_begin + 1) + (ks - k_begin) * upd;  // launches that did work; later ones were empty
         if (hc->stop == 1) {

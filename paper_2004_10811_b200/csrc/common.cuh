@@ -104,6 +104,7 @@ struct sm_plan {
     double* h_pinned_d = nullptr;          // pinned host scalars
     double* d_gg = nullptr;                // [2 nb] per-column Gershgorin ends of k_gersh_global (allocated on first use)
     unsigned char* h_stats = nullptr;      // pinned mirror of done_iter / flag / res for collect_stats (first use)
+    int last_eval_iters = 0;               // iterations the last converged evaluation took (sizes the enqueue-ahead batch)
     int cur_k = 0;                         // completed Newton-Schulz updates of the last evaluation
     int half_iter = 0;                     // 1: MODE 0 of iteration cur_k ran, its MODE 1 did not (steering stop)
     double* d_bound = nullptr;             // [max_iter+2][2] per iteration: n_elec(X_k), its error bound
@@ -124,6 +125,7 @@ struct sm_plan {
     int4* d_col_rec = nullptr;             // [nb] scatter column records (first value lo/hi, value count, group)
     int scatter_chunks = 1;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
+    int4* d_lz_rec = nullptr;              // [nnzb] per stored block: value offset (lo, hi), blk_off of its row, its height
     double lz_lo = 0.0, lz_hi = 0.0;       // estimated [lambda_min, lambda_max] of K~ (widened)
     double* d_alpha = nullptr;             // [2][ngroups] rescaling factor alpha_k of iteration k (slot k & 1), reading A8b
     int resc_eval = 0;                     // this evaluation runs the rescaled iteration (A8b)

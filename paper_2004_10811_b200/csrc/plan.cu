@@ -221,6 +221,15 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     if ((s = upload(&p->d_colptr, p->h_colptr.data(), nb + 1, st))) return s;
     if ((s = upload(&p->d_rowidx, p->h_rowidx.data(), p->nnzb, st))) return s;
     if ((s = upload(&p->d_val_off, val_off.data(), p->nnzb + 1, st))) return s;
+    if (p->opt.scaling == 1) {  // packed block records of the Lanczos mat-vec (spectral.cu)
+        std::vector<int4> rec((size_t)p->nnzb);
+        for (int64_t q = 0; q < p->nnzb; ++q) {
+            const int r = p->h_rowidx[q];
+            rec[q] = make_int4((int)(val_off[q] & 0xffffffffll), (int)(val_off[q] >> 32), blk_off[r], p->h_blk_size[r]);
+        }
+        if ((s = upload(&p->d_lz_rec, rec.data(), (size_t)p->nnzb, st))) return s;
+        SM_CUDA(cudaStreamSynchronize(st));  // rec goes out of scope
+    }
     if ((s = upload(&p->d_grp_ptr, p->h_grp_ptr.data(), ng + 1, st))) return s;
     if ((s = upload(&p->d_grp_cols, p->h_grp_cols.data(), p->h_grp_cols.size(), st))) return s;
 

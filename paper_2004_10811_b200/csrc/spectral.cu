@@ -24,19 +24,20 @@ constexpr int LZ_STEPS = 24;  // extreme Ritz values within ~1 % of the spread (
 // column (no atomics); lane b takes every 32nd block of the column.  part[c] = y_c . x_c.
 // For the common block widths (1, 4, 5, 13: H and O in SZV / DZVP) the lane keeps the partial sums of
 // all dense columns of the block column in registers, so index and values of a block are read once.
+// rec[b] = (value offset lo, hi, first basis function of the block's row, its height): ONE 16-byte load per stored
+// block instead of a chain of four dependent index loads.
 template <int BC>
-__device__ __forceinline__ double lz_col(int lane, int oc, int64_t p0, int64_t p1, const int32_t* __restrict__ blk_size,
-                                         const int32_t* __restrict__ blk_off, const int32_t* __restrict__ rowidx,
-                                         const int64_t* __restrict__ val_off, const double* __restrict__ vals,
-                                         const double* __restrict__ x, double* __restrict__ y) {
+__device__ __forceinline__ double lz_col(int lane, int oc, int64_t p0, int64_t p1, const int4* __restrict__ rec,
+                                         const double* __restrict__ vals, const double* __restrict__ x,
+                                         double* __restrict__ y) {
     double a[BC];
 #pragma unroll
     for (int q = 0; q < BC; ++q) a[q] = 0.0;
     for (int64_t b = p0 + lane; b < p1; b += 32) {
-        const int r = __ldg(rowidx + b);
-        const int br = __ldg(blk_size + r);
-        const double* blk = vals + __ldg(val_off + b);
-        const double* xr = x + __ldg(blk_off + r);
+        const int4 rc = __ldg(rec + b);
+        const int br = rc.w;
+        const double* blk = vals + (((int64_t)rc.y << 32) | (int64_t)(uint32_t)rc.x);
+        const double* xr = x + rc.z;
         for (int e = 0; e < br; ++e) {
             const double xe = xr[e];
 #pragma unroll
@@ -129,7 +130,7 @@ __device__ void lz_quadrature_body(int k, const double* __restrict__ alpha, cons
 // sum over the CTAs in every thread that needs it -- deterministic, no floating-point atomics.
 __global__ void __launch_bounds__(256)
 k_lz_fused(int nb, int64_t n, int steps, const int32_t* __restrict__ blk_size, const int32_t* __restrict__ blk_off,
-           const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx, const int64_t* __restrict__ val_off,
+           const int64_t* __restrict__ colptr, const int4* __restrict__ rec,
            const double* __restrict__ vals, double* __restrict__ vb0, double* __restrict__ vb1, double* __restrict__ vb2,
            double* __restrict__ alpha, double* __restrict__ beta, double* __restrict__ part, double margin,
            double* __restrict__ outp) {
@@ -177,19 +178,19 @@ k_lz_fused(int nb, int64_t n, int steps, const int32_t* __restrict__ blk_size, c
             const int64_t p0 = colptr[c], p1 = colptr[c + 1];
             double d;
             switch (bc) {
-                case 1: d = lz_col<1>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, v, w); break;
-                case 4: d = lz_col<4>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, v, w); break;
-                case 5: d = lz_col<5>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, v, w); break;
-                case 13: d = lz_col<13>(lane, oc, p0, p1, blk_size, blk_off, rowidx, val_off, vals, v, w); break;
+                case 1: d = lz_col<1>(lane, oc, p0, p1, rec, vals, v, w); break;
+                case 4: d = lz_col<4>(lane, oc, p0, p1, rec, vals, v, w); break;
+                case 5: d = lz_col<5>(lane, oc, p0, p1, rec, vals, v, w); break;
+                case 13: d = lz_col<13>(lane, oc, p0, p1, rec, vals, v, w); break;
                 default:
                     d = 0.0;
                     for (int q = 0; q < bc; ++q) {
                         double a = 0.0;
                         for (int64_t b = p0 + lane; b < p1; b += 32) {
-                            const int r = rowidx[b];
-                            const int br = blk_size[r];
-                            const double* col = vals + val_off[b] + (size_t)q * br;
-                            const double* xr = v + blk_off[r];
+                            const int4 rc = __ldg(rec + b);
+                            const int br = rc.w;
+                            const double* col = vals + (((int64_t)rc.y << 32) | (int64_t)(uint32_t)rc.x) + (size_t)q * br;
+                            const double* xr = v + rc.z;
                             for (int e = 0; e < br; ++e) a = fma(col[e], xr[e], a);
                         }
 #pragma unroll
@@ -285,7 +286,7 @@ sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t s
     double* part = outp + 72;
     int steps = (int)std::min<int64_t>(LZ_STEPS, n), nb = p->nb;
     double margin = 0.03;
-    void* args[] = {&nb, &n, &steps, &p->d_blk_size, &p->d_blk_off, &p->d_colptr, &p->d_rowidx, &p->d_val_off, &vals,
+    void* args[] = {&nb, &n, &steps, &p->d_blk_size, &p->d_blk_off, &p->d_colptr, &p->d_lz_rec, &vals,
                     &vb0, &vb1, &vb2, &alpha, &beta, &part, &margin, &outp};
     SM_CUDA(cudaLaunchCooperativeKernel((const void*)k_lz_fused, dim3(p->lz_grid), dim3(256), args, 0, st));
     p->launches++;
