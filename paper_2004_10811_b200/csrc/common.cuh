@@ -96,6 +96,8 @@ struct sm_plan {
     unsigned long long* d_gersh = nullptr; // [2][ngroups] bits of the Gershgorin bound | of the largest squared column norm (atomicMax)
     double* d_partials = nullptr;          // [n_tiles][4] per-tile, per-consumer-warp residual partials
     int32_t* d_counters = nullptr;         // [max_iter+2] still-active submatrices after iteration k
+    int32_t* d_act = nullptr;              // [4][n_tiles] work lists of the GEMM launches (ns_sign.cu)
+    int32_t* d_act_cnt = nullptr;          // [2 (max_iter + 3)] their lengths
     int32_t* d_sched = nullptr;            // [2*(max_iter+2)] work counters of the persistent GEMM launches
     double* d_ne_part = nullptr;           // [ngroups] per-group electron-count partials
     double* d_scalars = nullptr;           // [8] n_elec, tr D, tr DK, gersh lo/hi

@@ -437,6 +437,15 @@ struct NsArgs {
     double* alpha;       // null, or [2][ngroups] rescaling factors (slot k & 1 = iteration k), reading A8b
     double* lmin;        // [ngroups] lower bound l_k the schedule tracks
     const int2* gen_rng; // [ngroups] first / last generating row; non-null: restrict final updates (see producer)
+    // Work lists written by k_ns_decide of iteration k (tiles of the submatrices that go on; bit 31 = "last update of a
+    // predicted exit"): a launch draws from its list instead of scanning all tiles, so a launch with few active
+    // submatrices costs what they cost.  act_list == null: every tile (MODE 0 of iteration 0).
+    const int32_t* act_list;
+    const int32_t* act_count;
+    int32_t* next_upd_list;   // k_ns_decide: list of the update (MODE 1..3) of this iteration ...
+    int32_t* next_upd_count;
+    int32_t* next_sq_list;    // ... and of the squaring (MODE 0) of the next one
+    int32_t* next_sq_count;
     int32_t n_tiles;
     int32_t ngroups;
     int32_t k;
@@ -477,16 +486,24 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
         int stage = 0;
         unsigned phase = 0;
         const bool stopped = a.ctrl[0] != 0;  // decided / all converged earlier in the stream: empty launch
-        auto draw = [&]() { return stopped ? a.n_tiles : atomicAdd(a.sched, 1); };
+        const int n_work = stopped ? 0 : (a.act_list ? *a.act_count : a.n_tiles);
+        auto draw = [&]() { return stopped ? 0x7fffffff : atomicAdd(a.sched, 1); };
         // MODE 1 with gen_rng: a submatrix that leaves by the predicted exit (done == k + 1: this update gives its
         // result, nothing reads it but the extraction of the generating columns, L127) only needs the tiles that
         // hold generating rows -- as rows (ti in range) or, mirrored, as columns (tj in range); skip = 1 otherwise
-        auto load_desc = [&](int tile, int4& t0, int4& t1, int& done) {
-            if (tile < a.n_tiles) {
+        auto load_desc = [&](int idx, int& tile, int4& t0, int4& t1, int& done) {
+            if (idx < n_work) {
+                tile = idx;
+                bool listed_final = false;
+                if (a.act_list) {
+                    const int e = a.act_list[idx];
+                    tile = e & 0x7fffffff;
+                    listed_final = e < 0;
+                }
                 const int4* tdp = reinterpret_cast<const int4*>(a.tiles + tile);
                 t0 = __ldg(tdp);
                 t1 = __ldg(tdp + 1);
-                done = a.done_iter[t0.z];
+                done = a.act_list ? (listed_final ? k + 1 : -1) : a.done_iter[t0.z];
                 if (MODE == 1 && a.gen_rng && done == k + 1) {
                     const int2 gr = __ldg(a.gen_rng + t0.z);
                     const int tl = gr.x / BM, th = gr.y / BM, ti = t1.y & 0xffff, tj = t1.y >> 16;
@@ -494,15 +511,15 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
                 }
             }
         };
-        int tile = draw();
-        int tile_n = draw();
+        int idx = draw();
+        int idx_n = draw();
         int4 t0, t1, n0, n1;
-        int done = 0, done_n = 0;
+        int done = 0, done_n = 0, tile = 0, tile_n = 0;
         t0 = t1 = n0 = n1 = make_int4(0, 0, 0, 0);
-        load_desc(tile, t0, t1, done);
-        while (tile < a.n_tiles) {
-            load_desc(tile_n, n0, n1, done_n);  // in flight while this tile streams
-            const int tile_nn = draw();
+        load_desc(idx, tile, t0, t1, done);
+        while (idx < n_work) {
+            load_desc(idx_n, tile_n, n0, n1, done_n);  // in flight while this tile streams
+            const int idx_nn = draw();
             if (done < 0 || done > k) {  // active (done > k: stops after the update of iteration k, see k_ns_decide)
                 const int g = t0.z;
                 const int64_t ws_off = ((int64_t)(unsigned)t0.x) | ((int64_t)t0.y << 32);
@@ -533,8 +550,8 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
             }
-            tile = tile_n; t0 = n0; t1 = n1; done = done_n;
-            tile_n = tile_nn;
+            idx = idx_n; tile = tile_n; t0 = n0; t1 = n1; done = done_n;
+            idx_n = idx_nn;
         }
         // end marker
         mbar_wait(&s_empty[stage], phase ^ 1);
@@ -609,6 +626,7 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
     const int lane = threadIdx.x & 31, k = a.k;
     const int cnt = 4 * tile_count[g], n = sub_dim[g];
     const double* pp = a.partials + (size_t)tile_first[g] * 4;
+    int goes_on = 0;  // lane 0: 1 = takes part in the update and in the next squaring, 2 = in the update only (predicted exit)
     double r2 = 0.0;
     for (int t = lane; t < cnt; t += 32) r2 += pp[t];
 #pragma unroll
@@ -638,6 +656,7 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
         if (stop) { a.flag[g] = conv ? 0 : 1; a.done_iter[g] = k; }
         else {
             atomicAdd(a.counters + k, 1);
+            goes_on = 1;
             // Predicted exit (reading A9): with E_k = X_k^2 - I symmetric, E_{k+1} = -3/4 E_k^2 + 1/4 E_k^3, so
             // ||E_{k+1}||_F <= 3/4 ||E_k||_F^2 + 1/4 ||E_k||_F^3.  If that bound is already a factor 10 below
             // eps, X_{k+1} is accepted without the product that would only confirm it: the submatrix takes part
@@ -649,8 +668,24 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
                     a.done_iter[g] = k + 1;
                     a.flag[g] = 2;
                     a.res[(size_t)((k + 1) & 1) * a.ngroups + g] = next;
+                    goes_on = 2;
                 }
             }
+        }
+    }
+    // work lists of the launches that follow (see NsArgs): every tile of a submatrix that goes on
+    goes_on = __shfl_sync(0xffffffffu, goes_on, 0);
+    if (goes_on && a.next_upd_list) {
+        const int tf = tile_first[g], tc = tile_count[g];
+        int base = 0;
+        if (lane == 0) base = atomicAdd(a.next_upd_count, tc);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        const int fin = goes_on == 2 ? (int)0x80000000 : 0;
+        for (int t = lane; t < tc; t += 32) a.next_upd_list[base + t] = (tf + t) | fin;
+        if (goes_on == 1) {
+            if (lane == 0) base = atomicAdd(a.next_sq_count, tc);
+            base = __shfl_sync(0xffffffffu, base, 0);
+            for (int t = lane; t < tc; t += 32) a.next_sq_list[base + t] = tf + t;
         }
     }
 }
@@ -675,15 +710,27 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     const bool resc = rescale_on(p);
     a.alpha = resc ? p->d_alpha : nullptr; a.lmin = resc ? p->d_lmin : nullptr;
     a.gen_rng = (p->opt.order == 2) ? p->d_gen_rng : nullptr;
+    // work lists: d_act = [upd 0][upd 1][sq 0][sq 1] x n_tiles entries, d_act_cnt[2 * iteration + {0: upd, 1: sq}]
+    int32_t* const L = p->d_act;
+    const size_t nt = (size_t)p->n_tiles;
+    int32_t* const C = p->d_act_cnt;
+    a.next_upd_list = L + (size_t)(k & 1) * nt;            a.next_upd_count = C + 2 * k;
+    a.next_sq_list = L + (size_t)(2 + ((k + 1) & 1)) * nt; a.next_sq_count = C + 2 * (k + 1) + 1;
+    const int32_t* sq_list = k > 0 ? L + (size_t)(2 + (k & 1)) * nt : nullptr;
+    const int32_t* sq_count = C + 2 * k + 1;
+    const int32_t* upd_list = L + (size_t)(k & 1) * nt;
+    const int32_t* upd_count = C + 2 * k;
     a.predict = (p->opt.predict != 0 && p->opt.order == 2 && eps >= 1e-13) ? 1 : 0; a.max_iter = p->opt.max_iter;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * SM_MINB);
     a.sched = p->d_sched + 4 * k;
     if (which & 1) {
+        a.act_list = sq_list; a.act_count = sq_count;
         k_ns_gemm<0><<<grid, NTHREADS, NS_SMEM, st>>>(a);
         k_ns_decide<<<(p->ngroups + 7) / 8, 256, 0, st>>>(a, p->d_tile_first, p->d_tile_count, p->d_sub_dim);
         p->launches += 2;
     }
     if ((which & 2) && !decide_only) {
+        a.act_list = upd_list; a.act_count = upd_count;
         if (p->opt.order == 3 && bufW) {  // Eq.(19): two products per update
             a.sched = p->d_sched + 4 * k + 1;
             k_ns_gemm<2><<<grid, NTHREADS, NS_SMEM, st>>>(a);
