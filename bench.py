@@ -412,10 +412,15 @@ def main():
     B.lib()  # fail loudly if the CUDA library is missing
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local_rank)
+    torch.cuda.set_device(local_rank % torch.cuda.device_count())
+    local_rank = local_rank % torch.cuda.device_count()
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        backend = os.environ.get("SM_DIST_BACKEND", "nccl")  # "gloo": functional check of the N > 1 path without N GPUs
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        else:
+            dist.init_process_group(backend)
 
     # N > 1: ONE problem, every rank holds the whole K~ and owns a contiguous chunk of the
     # submatrices balanced by sum n^3; strong scaling
