@@ -45,8 +45,8 @@ TOL_N = 0.5      # plateau acceptance (reading A11); 1e-8 is unreachab
 MU0 = -1.0       # the caller's mu, inside the occupied band (evaluated only by the literal rule, see docstring)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_ns_gemm from the committed
 # `ncu --set full` capture of the current kernel (profiles/r02_full_captures.md): all-active launch,
-# mean of MODE 0 (8.45 + 7.68 GB) and MODE 1 (17.78 + 7.75 GB).
-NS_GEMM_DRAM_BYTES_PER_LAUNCH = 20.8e9
+# mean of MODE 0 (8.40 + 7.48 GB) and MODE 1 (17.82 + 7.66 GB).
+NS_GEMM_DRAM_BYTES_PER_LAUNCH = 20.7e9
 NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # guide: B200 FP64 tensor 45 TF/s, bf16 2250 TF/s (nominal)
 
 
