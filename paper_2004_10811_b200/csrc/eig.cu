@@ -503,6 +503,7 @@ sm_status_t launch_eig_nelec(sm_plan* p, double mu, double kT, cudaStream_t st) 
 sm_status_t launch_eig_density(sm_plan* p, double mu, double kT, double* buf0, const double* buf1, cudaStream_t st) {
     if (p->ngroups == 0) return SM_OK;
     const size_t smem = (size_t)ED_QC * std::max(p->info.dim_max, 1) * 8;
+    if (smem > (size_t)200 * 1024) return SM_ERR_INVALID_ARG;  // submatrix too large for this path (n > 3200)
     if (smem > 40 * 1024) SM_CUDA(cudaFuncSetAttribute(k_eig_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_eig_density<<<p->ngroups, 256, smem, st>>>(p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_grp_ptr, p->d_grp_cols,
                                                   p->d_gen_off, p->d_blk_size, p->d_eig_ptr, p->d_eig_lam, buf1, mu, kT, buf0);

@@ -24,9 +24,11 @@ def test_struct_sizes_match_header():
     """ctypes mirrors must have the C layout (sizes and a few field offsets checked against a tiny C program)."""
     import subprocess, tempfile
     from paper_2004_10811_b200 import binding as B
-    src = ('#include <stdio.h>\n#include <stddef.h>\n#include "submatrix.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu\\n", '
+    src = ('#include <stdio.h>\n#include <stddef.h>\n#include "submatrix.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n", '
            'sizeof(sm_options_t), sizeof(sm_plan_info_t), sizeof(sm_stats_t), offsetof(sm_options_t, overshoot), '
-           'offsetof(sm_options_t, mu_guess), offsetof(sm_options_t, mu_start), offsetof(sm_stats_t, mu_guess));return 0;}\n')
+           'offsetof(sm_options_t, mu_guess), offsetof(sm_options_t, mu_start), offsetof(sm_stats_t, mu_guess), '
+           'offsetof(sm_options_t, kT), offsetof(sm_options_t, shard_world), offsetof(sm_plan_info_t, index_alg_bytes), '
+           'offsetof(sm_plan_info_t, shard_val_begin), sizeof(sm_peaks_t));return 0;}\n')
     with tempfile.TemporaryDirectory() as d:
         c = os.path.join(d, "s.c")
         open(c, "w").write(src)
@@ -36,7 +38,9 @@ def test_struct_sizes_match_header():
     assert [int(x) for x in out] == [ctypes.sizeof(B.sm_options_t), ctypes.sizeof(B.sm_plan_info_t),
                                      ctypes.sizeof(B.sm_stats_t), B.sm_options_t.overshoot.offset,
                                      B.sm_options_t.mu_guess.offset, B.sm_options_t.mu_start.offset,
-                                     B.sm_stats_t.mu_guess.offset]
+                                     B.sm_stats_t.mu_guess.offset, B.sm_options_t.kT.offset,
+                                     B.sm_options_t.shard_world.offset, B.sm_plan_info_t.index_alg_bytes.offset,
+                                     B.sm_plan_info_t.shard_val_begin.offset, ctypes.sizeof(B.sm_peaks_t)]
 
 
 def test_strerror_and_missing_library_is_loud(monkeypatch):
@@ -92,3 +96,34 @@ def test_plan_validation_is_host_logic():
     assert status(blk_size=bs) == B.SM_ERR_INVALID_ARG                    # non-positive block size
     assert status(nb=-1) == B.SM_ERR_INVALID_ARG
     assert L.sm_plan_create(None, m.nb, None, None, None, 0, None, None, None, None) == B.SM_ERR_INVALID_ARG
+
+
+def test_option_validation_is_host_logic():
+    """Bad option values (round-2 options: method, kT, shard_rank / shard_world) are rejected before any CUDA
+    call, and sm_partition_groups / sm_plan_set_allreduce validate their arguments -- all without a GPU."""
+    import numpy as np
+    from paper_2004_10811_b200 import binding as B, workloads as W
+    L = B.lib()
+    m = W.random_block_pattern(nb=12, density=0.3, max_bs=3, seed=1)
+    arrs = [np.ascontiguousarray(x) for x in (m.blk_size, m.colptr, m.rowidx, m.grp_ptr, m.grp_cols)]
+
+    def status(**kw):
+        opt = B.default_options(**kw)
+        plan = ctypes.c_void_p(0xdead)
+        st = L.sm_plan_create(ctypes.byref(plan), m.nb, arrs[0].ctypes.data, arrs[1].ctypes.data, arrs[2].ctypes.data,
+                              m.ngroups, arrs[3].ctypes.data, arrs[4].ctypes.data, ctypes.byref(opt), None)
+        assert st < 0 and not plan.value
+        return st
+
+    assert status(method=2) == B.SM_ERR_INVALID_ARG
+    assert status(method=1, kT=-1.0) == B.SM_ERR_INVALID_ARG
+    assert status(method=1, precision=2) == B.SM_ERR_INVALID_ARG          # the eigendecomposition path is FP64 only
+    assert status(shard_rank=2, shard_world=2) == B.SM_ERR_INVALID_ARG
+    assert status(shard_rank=0, shard_world=m.ngroups + 1) == B.SM_ERR_INVALID_ARG
+    dims = np.array([3, 4, 5], dtype=np.int32)
+    first = np.zeros(5, dtype=np.int32)
+    assert L.sm_partition_groups(3, dims.ctypes.data, 4, first.ctypes.data) == B.SM_ERR_INVALID_ARG  # world > ngroups
+    assert L.sm_partition_groups(3, dims.ctypes.data, 0, first.ctypes.data) == B.SM_ERR_INVALID_ARG
+    assert L.sm_partition_groups(3, dims.ctypes.data, 2, None) == B.SM_ERR_INVALID_ARG
+    assert L.sm_plan_set_allreduce(None, ctypes.cast(None, B.ALLREDUCE_FN), None) == B.SM_ERR_INVALID_ARG
+    assert L.sm_measure_peaks(None, None) == B.SM_ERR_INVALID_ARG
