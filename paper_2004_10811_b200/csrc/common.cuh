@@ -145,7 +145,7 @@ struct sm_plan {
     int32_t* d_eig_order = nullptr;        // [ngroups] processing order, largest first
     int32_t* d_eig_state = nullptr;        // [2 ngroups + 2] sweeps, flags, work counter
     int64_t eig_total = 0;
-    int eig_bcols = 16, eig_attr_set = 0, eig_valid = 0;
+    int eig_bcols = 16, eig_attr_set = 0, eig_battr_set = 0, eig_valid = 0;
     size_t eig_smem = 0;
     // --- sharding: the plan holds only its own chunk of groups
     sm_allreduce_fn allreduce = nullptr;
@@ -198,6 +198,7 @@ sm_status_t launch_eval_ctrl(sm_plan* p, int k, int steer, double n_target, doub
 // eig.cu
 sm_status_t launch_eig_decompose(sm_plan* p, const double* vals, double* buf0, double* buf1, cudaStream_t st);
 sm_status_t launch_eig_nelec(sm_plan* p, double mu, double kT, cudaStream_t st);
+sm_status_t launch_eig_bjacobi(sm_plan* p, double* G, cudaStream_t st);  // eig_block.cu
 sm_status_t launch_eig_density(sm_plan* p, double mu, double kT, double* buf0, const double* buf1, cudaStream_t st);
 // spectral.cu
 sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t st);

@@ -467,6 +467,15 @@ sm_status_t launch_eig_decompose(sm_plan* p, const double* vals, double* buf0, d
     k_eig_init<<<dim3(ng, split), 256, 0, st>>>(ng, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_gersh, buf0, buf1,
                                                  p->d_eig_sigma);
     SM_CUDA(cudaMemsetAsync(p->d_eig_state, 0, (size_t)(2 * ng + 2) * 4, st));
+#ifndef SM_EIG_BLOCK
+#define SM_EIG_BLOCK 1
+#endif
+    if (SM_EIG_BLOCK) {  // block form on the DMMA path (eig_block.cu)
+        p->launches += 1;
+        if ((s = launch_eig_bjacobi(p, buf1, st))) return s;
+        p->eig_valid = 1;
+        return SM_OK;
+    }
     if (!p->eig_attr_set) {  // static + dynamic shared memory may exceed the 48 KB default
         SM_CUDA(cudaFuncSetAttribute(k_eig_jacobi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->eig_smem));
         p->eig_attr_set = 1;
