@@ -145,8 +145,7 @@ struct sm_plan {
     int32_t* d_eig_order = nullptr;        // [ngroups] processing order, largest first
     int32_t* d_eig_state = nullptr;        // [2 ngroups + 2] sweeps, flags, work counter
     int64_t eig_total = 0;
-    int eig_bcols = 16, eig_attr_set = 0, eig_battr_set = 0, eig_valid = 0;
-    size_t eig_smem = 0;
+    int eig_battr_set = 0, eig_valid = 0;
     // --- sharding: the plan holds only its own chunk of groups
     sm_allreduce_fn allreduce = nullptr;
     void* allreduce_ctx = nullptr;

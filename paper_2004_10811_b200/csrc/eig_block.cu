@@ -1,13 +1,13 @@
-// SURVEY 8(f)1, block form of the one-sided Jacobi eigensolver of eig.cu: the O(n^3) part runs on the FP64
-// tensor-core instruction (mma.sync m8n8k4 f64, SASS DMMA).
+// SURVEY 8(f)1, the eigensolver of method = 1 (Eq.(17) first line, L246-255): block one-sided Jacobi, the
+// O(n^3) part on the FP64 tensor-core instruction (mma.sync m8n8k4 f64, SASS DMMA).
 //
-// Same mathematics as eig.cu (G = B V with B = a_i + sigma I positive definite; at convergence the columns of G are
-// mutually orthogonal, lambda_l = ||g_l|| - sigma, q_l = g_l / ||g_l||), but the columns are visited in BLOCK pairs
-// and a visit is three dense steps instead of 256 separate plane rotations:
+// Mathematics as stated in eig.cu (G = B V with B = a_i + sigma I positive definite; at convergence the columns of G
+// are mutually orthogonal, lambda_l = ||g_l|| - sigma, q_l = g_l / ||g_l||).  The columns are visited in BLOCK pairs
+// and a visit is three dense steps instead of 256 separate plane rotations of full-length columns:
 //   1. Gram matrix M = [G_I G_J]^T [G_I G_J] (32 x 32) by DMMA straight from global memory (L2-resident matrix):
 //      four column fragments per step of four rows feed the ten sub-tiles on or below the diagonal;
 //   2. M = W D W^T by a cyclic two-sided Jacobi on the 32 x 32 matrix in shared memory (one warp, 16 disjoint
-//      rotations per round, angles from M alone: rotating columns p, q of G is the congruence J^T M J on its Gram
+//      rotations per round, one sweep of 31 rounds per visit, angles from M alone: rotating columns p, q of G is the congruence J^T M J on its Gram
 //      matrix, so this IS the sequence of plane rotations of the one-sided method, applied to M instead of G);
 //   3. [G_I G_J] <- [G_I G_J] W by DMMA, W held in registers as B fragments, one 8-row strip at a time, in place.
 // One warp owns a block pair; the pairs of a tournament round are disjoint, so the warps of a CTA work on different
@@ -50,7 +50,7 @@ __device__ __forceinline__ void bj_dmma(double (&c)[2], double a, double b) {
 }
 
 // Two-sided rotation zeroing M_pq: t = tan(theta) root of t^2 + 2 zeta t - 1, zeta = (M_qq - M_pp) / (2 M_pq).
-// As in eig.cu the tangent is formed in FP32 (relative error 1e-7: the pair is then orthogonal to 1e-7 of its former
+// The tangent is formed in FP32 (relative error 1e-7: the pair is then orthogonal to 1e-7 of its former
 // inner product, which the next visit removes) and the cosine by an FP32 seed and two FP64 Newton steps, so that
 // c^2 + s^2 = 1 to FP64 rounding and W stays orthogonal -- ~25 instructions instead of FP64 division, square root
 // and reciprocal square root on the critical path of every round.
@@ -275,7 +275,7 @@ __global__ void __launch_bounds__(BJ_WARPS * 32, 1) k_eig_bjacobi(const BjArgs A
             __syncthreads();
         }
         if (threadIdx.x == 0) { A.sweeps[i] = sweep; A.eflag[i] = converged ? 0 : 1; }
-        // ---- eigenvalues, normalised eigenvectors (in place), weights of Algorithm 1 (as in eig.cu)
+        // ---- eigenvalues, normalised eigenvectors (in place), weights of Algorithm 1 (L270, L278)
         int gw = 0;
         for (int gc = A.grp_ptr[i]; gc < A.grp_ptr[i + 1]; ++gc) {
             const int c = A.grp_cols[gc], o = A.gen_off[c], b = A.blk_size[c];
