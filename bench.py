@@ -239,7 +239,7 @@ def run_phases(args, m, B, torch):
     B.sm_plan_destroy(plan)
     del ws
     out["reduced_precision"] = {}
-    for prec, name, eps in ((2, "3xTF32 (hi/lo split)", 2e-6), (1, "TF32", 1e-5)):
+    for prec, name, eps in ((2, "3xTF32 (hi/lo split)", 2e-6), (3, "BF16x2 (hi/lo split)", 1e-5), (1, "TF32", 1e-5)):
         plan = B.plan_from_matrix(m, B.default_options(precision=prec))
         ws = B.alloc_workspace(plan)
         B.sm_set_timing(plan, True)
@@ -336,23 +336,26 @@ def run_extras(args, m, B, torch, plan, info, ws, d_in, d_out, mu, hbm_peak):
                                                  "abs_g": abs(st.n_elec - n_target), "mu": mu_g, "ms": e0.elapsed_time(e1)}
     B.sm_plan_destroy(plan4)
 
-    # opt-in reduced precision (3xTF32 on tcgen05) on the same input at the accepted mu, against the FP64 result
+    # opt-in reduced precision (tcgen05: 3xTF32, and the BF16x2 rung) on the same input at the accepted mu, against
+    # the FP64 result
     _, tdk64 = B.sm_trace_dk(plan, d_out, d_in)
-    plan3 = B.plan_from_matrix(m, B.default_options(precision=2))
-    need = B.sm_plan_query(plan3).workspace_bytes
-    ws3 = ws if need <= ws.numel() * 8 else B.alloc_workspace(plan3)
-    B.sm_set_timing(plan3, True)
-    for _ in range(2):
-        rc = B.sm_sign_execute(plan3, d_in, mu, 2e-6, tmp_out, ws3, st)
-    torch.cuda.synchronize()
-    d = st.as_dict()
-    _, tdk = B.sm_trace_dk(plan3, tmp_out, d_in)
-    out["reduced_precision_3xTF32"] = {
-        "status": int(rc), "ms_sign": d["ms_sign"], "ms_total": d["ms_total"], "iter_min": d["iter_min"],
-        "iter_max": d["iter_max"], "residual_floor": d["max_residual"],
-        "max_abs_err_vs_fp64": float((tmp_out - d_out).abs().max().item()),
-        "rel_band_energy_err_vs_fp64": abs(tdk - tdk64) / abs(tdk64), "n_elec": d["n_elec"]}
-    B.sm_plan_destroy(plan3)
+    for prec, key, eps_r in ((2, "reduced_precision_3xTF32", 2e-6), (3, "reduced_precision_BF16x2", 1e-5)):
+        plan3 = B.plan_from_matrix(m, B.default_options(precision=prec))
+        need = B.sm_plan_query(plan3).workspace_bytes
+        ws3 = ws if need <= ws.numel() * 8 else B.alloc_workspace(plan3)
+        B.sm_set_timing(plan3, True)
+        for _ in range(2):
+            rc = B.sm_sign_execute(plan3, d_in, mu, eps_r, tmp_out, ws3, st)
+        torch.cuda.synchronize()
+        d = st.as_dict()
+        _, tdk = B.sm_trace_dk(plan3, tmp_out, d_in)
+        out[key] = {
+            "status": int(rc), "ms_sign": d["ms_sign"], "ms_total": d["ms_total"], "iter_min": d["iter_min"],
+            "iter_max": d["iter_max"], "residual_floor": d["max_residual"],
+            "max_abs_err_vs_fp64": float((tmp_out - d_out).abs().max().item()),
+            "rel_band_energy_err_vs_fp64": abs(tdk - tdk64) / abs(tdk64), "n_elec": d["n_elec"]}
+        B.sm_plan_destroy(plan3)
+        del ws3
     # the FP64 evaluation at the same mu, for the comparison above
     B.sm_sign_execute(plan, d_in, mu, EPS, tmp_out, ws, st)
     torch.cuda.synchronize()

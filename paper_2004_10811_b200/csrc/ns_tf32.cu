@@ -20,10 +20,16 @@
 //   warps 2..5           epilogue: tcgen05.ld of their 32 TMEM lanes, MODE 0: Y = X X and residual
 //                        partials; MODE 1: X' = 3/2 X - 1/2 X Y; two 256-column accumulators in
 //                        TMEM, so the epilogue of one tile overlaps the MMAs of the next.
+// options.precision = 2 ("3xTF32") stores hi + lo TF32 planes (8 bytes per element) and issues three products per
+// k step; options.precision = 3 ("BF16x2") stores hi + lo BF16 planes (4 bytes per element, 8 columns per 16-byte
+// chunk) and issues the same three products with kind::f16 -- the launches are HBM-bound, so halving the bytes is
+// what makes that rung faster than FP64 (Table I's ladder, L366-374, on this part's tensor pipes).
 // Work unit: (submatrix, 128-row tile, 256-column tile on or below the diagonal), static round-robin
 // over the CTAs.  Only the lower triangle is computed; every element is stored together with its
 // mirror image, so X and Y are bitwise symmetric and B can be read as k-contiguous rows.
 #include <algorithm>
+
+#include <cuda_bf16.h>
 
 #include "common.cuh"
 
@@ -45,6 +51,13 @@ __host__ __device__ __forceinline__ size_t panel32_off(int r, int c, int ldp) {
     const int t0 = r & ~127;
     const int rows_t = (ldp - t0) < 128 ? (ldp - t0) : 128;
     return (size_t)t0 * ldp + (size_t)(c >> 2) * rows_t * 4 + (size_t)((r - t0) * 4 + (c & 3));
+}
+
+// BF16 planes (precision = 3): the same layout with 8 columns per 16-byte chunk ("k8-panel/128", 2-byte elements).
+__host__ __device__ __forceinline__ size_t panel16_off(int r, int c, int ldp) {
+    const int t0 = r & ~127;
+    const int rows_t = (ldp - t0) < 128 ? (ldp - t0) : 128;
+    return (size_t)t0 * ldp + (size_t)(c >> 3) * rows_t * 8 + (size_t)((r - t0) * 8 + (c & 7));
 }
 
 __device__ __forceinline__ unsigned r_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -98,6 +111,19 @@ __device__ __forceinline__ void r_mma(uint32_t tmem_d, uint64_t da, uint64_t db,
         "}\n" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// kind::f16 with BF16 operands: A = B = BF16 ([7,10) = [10,13) = 1), K = 16 per instruction (32 bytes, as TF32's 8).
+__device__ __forceinline__ uint32_t r_idesc_bf16(int n_cols) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(n_cols >> 3) << 17) | ((unsigned)(R_BM >> 4) << 24);
+}
+__device__ __forceinline__ void r_mma_bf16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 __device__ __forceinline__ void r_commit(uint64_t* bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(r_smem_u32(bar))
                  : "memory");
@@ -121,6 +147,16 @@ __device__ __forceinline__ void quad_transpose(float (&w)[4], int lane) {
     r0 = __shfl_xor_sync(0xffffffffu, s0, 2); r1 = __shfl_xor_sync(0xffffffffu, s1, 2);
     if (o2) { w[0] = r0; w[1] = r1; } else { w[2] = r0; w[3] = r1; }
 }
+
+// x = hi + lo with hi = bf16(x), lo = bf16(x - hi): 16 mantissa bits in two BF16 numbers.
+__device__ __forceinline__ void bf_split(float x, unsigned short& hi, unsigned short& lo) {
+    const __nv_bfloat16 h = __float2bfloat16_rn(x);
+    const __nv_bfloat16 l = __float2bfloat16_rn(x - __bfloat162float(h));
+    hi = __bfloat16_as_ushort(h);
+    lo = __bfloat16_as_ushort(l);
+}
+__device__ __forceinline__ float bf_val(unsigned short b) { return __uint_as_float((unsigned)b << 16); }
+__device__ __forceinline__ unsigned bf_pack2(unsigned short a, unsigned short b) { return (unsigned)a | ((unsigned)b << 16); }
 
 // One work unit of the reduced-precision GEMMs.
 struct __align__(16) Tile32 {
@@ -200,6 +236,68 @@ k_to_f64(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __rest
     }
 }
 
+// precision = 3: FP64 k8-panel a_i - mu I  ->  BF16 hi / lo planes (k8-panel/128, 2-byte elements) of X0.
+__global__ void __launch_bounds__(256)
+k_to_bf16(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __restrict__ ldv,
+          const int64_t* __restrict__ ws_off, const int64_t* __restrict__ ws_off32,
+          const unsigned long long* __restrict__ gersh, const double* __restrict__ X64,
+          unsigned short* __restrict__ X16, int64_t lo_plane) {
+    const int g = blockIdx.x;
+    const int n = sub_dim[g], ld = ldv[g], ldp = (n + 15) & ~15;
+    double s = __longlong_as_double((long long)gersh[g]);
+    const double inv = s > 0.0 ? 1.0 / s : 1.0;
+    const double* src = X64 + ws_off[g];
+    unsigned short* dst = X16 + ws_off32[g];
+    const int chunks = ldp >> 3;
+    for (int e = blockIdx.y * blockDim.x + threadIdx.x; e < ldp * chunks; e += gridDim.y * blockDim.x) {
+        const int t = e / (128 * chunks);
+        const int rows_t = min(128, ldp - 128 * t);
+        const int w = e - t * 128 * chunks;
+        const int kc = w / rows_t, r = 128 * t + (w - kc * rows_t);
+        unsigned short hi[8], lo[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int c = 8 * kc + j;
+            const double x = (r < n && c < n) ? src[panel_off(r, c, ld)] * inv : 0.0;
+            const __nv_bfloat16 h = __float2bfloat16_rn((float)x);
+            hi[j] = __bfloat16_as_ushort(h);
+            lo[j] = __bfloat16_as_ushort(__float2bfloat16_rn((float)(x - (double)__bfloat162float(h))));
+        }
+        unsigned short* d = dst + panel16_off(r, 8 * kc, ldp);
+        *reinterpret_cast<uint4*>(d) = make_uint4(bf_pack2(hi[0], hi[1]), bf_pack2(hi[2], hi[3]), bf_pack2(hi[4], hi[5]), bf_pack2(hi[6], hi[7]));
+        *reinterpret_cast<uint4*>(d + lo_plane) = make_uint4(bf_pack2(lo[0], lo[1]), bf_pack2(lo[2], lo[3]), bf_pack2(lo[4], lo[5]), bf_pack2(lo[6], lo[7]));
+    }
+}
+
+// precision = 3: BF16 hi + lo result -> FP64 k8-panel buffer (as k_to_f64).
+__global__ void __launch_bounds__(256)
+k_from_bf16(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __restrict__ ldv,
+            const int64_t* __restrict__ ws_off, const int64_t* __restrict__ ws_off32,
+            const unsigned long long* __restrict__ gersh, const int32_t* __restrict__ done_iter, int cur_k,
+            const unsigned short* __restrict__ Xa, const unsigned short* __restrict__ Xb, double* __restrict__ X64,
+            int64_t lo_plane) {
+    const int g = blockIdx.x;
+    const int n = sub_dim[g], ld = ldv[g], ldp = (n + 15) & ~15;
+    const int di = done_iter[g];
+    const int kb = di >= 0 ? di : cur_k;
+    const unsigned short* src = ((kb & 1) ? Xb : Xa) + ws_off32[g];
+    double mul = 1.0;
+    if (kb == 0) {
+        const double s = __longlong_as_double((long long)gersh[g]);
+        mul = s > 0.0 ? s : 1.0;
+    }
+    double* dst = X64 + ws_off[g];
+    for (int e = blockIdx.y * blockDim.x + threadIdx.x; e < ld * ld; e += gridDim.y * blockDim.x) {
+        const int r = e / ld, c = e - r * ld;
+        double v = 0.0;
+        if (r < n && c < n) {
+            const size_t o = panel16_off(r, c, ldp);
+            v = ((double)bf_val(src[o]) + (double)bf_val(src[o + lo_plane])) * mul;
+        }
+        dst[panel_off(r, c, ld)] = v;
+    }
+}
+
 struct Ns32Args {
     const Tile32* tiles;
     const float* A;        // X_k
@@ -216,11 +314,17 @@ struct Ns32Args {
 // SPLIT = 1: "3xTF32": every operand is stored as hi + lo with hi = tf32(x), lo = x - hi, and a
 //            product is hi hi + hi lo + lo hi accumulated in the same FP32 TMEM tile (FP32-class
 //            accuracy, three MMAs per k step, 16-wide k slices so that a stage stays 48 KB).
+// SPLIT = 2: "BF16x2": hi = bf16(x), lo = bf16(x - hi) in two BF16 planes, the same three products with
+//            kind::f16 (K = 16 per instruction), 32-wide k slices (48 KB per stage).
 template <int MODE, int SPLIT>
 __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
-    constexpr int BK = SPLIT ? R_BK / 2 : R_BK;     // k columns per stage
+    constexpr bool BF = SPLIT == 2;                 // BF16 hi / lo planes instead of FP32 ones
+    constexpr int CW = BF ? 8 : 4;                  // columns per 16-byte chunk
+    constexpr int ES = BF ? 2 : 4;                  // bytes per element
+    constexpr int CH = SPLIT ? 4 : 8;               // chunks per stage and plane
+    constexpr int BK = CH * CW;                     // k columns per stage
     constexpr int PL = SPLIT ? 2 : 1;               // operand planes
-    constexpr int SA = R_BM * BK;                   // floats of one 128-row operand plane in a stage
+    constexpr int SA = R_BM * CH * 4;               // 4-byte units of one 128-row operand plane in a stage
     extern __shared__ __align__(128) float rsm[];
     __shared__ __align__(8) uint64_t s_full[R_STAGES], s_empty[R_STAGES], s_tfull[2], s_tempty[2];
     __shared__ uint32_t s_tmem;
@@ -252,11 +356,11 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                 const int row0 = T.ti * R_BM, rows_a = min(R_BM, ldp - row0);
                 const int col0 = T.tj * R_BN, ncols = min(R_BN, min(ldp, row0 + R_BM) - col0);  // lower triangle only
                 const int rows_b0 = min(128, ncols), rows_b1 = max(0, ncols - 128);
-                const float* Asrc = a.A + T.off32 + (size_t)row0 * ldp;
-                const float* B0 = a.B + T.off32 + (size_t)col0 * ldp;
-                const float* B1 = a.B + T.off32 + (size_t)(col0 + 128) * ldp;
+                const char* Asrc = reinterpret_cast<const char*>(a.A) + ((size_t)T.off32 + (size_t)row0 * ldp) * ES;
+                const char* B0 = reinterpret_cast<const char*>(a.B) + ((size_t)T.off32 + (size_t)col0 * ldp) * ES;
+                const char* B1 = reinterpret_cast<const char*>(a.B) + ((size_t)T.off32 + (size_t)(col0 + 128) * ldp) * ES;
                 for (int k0 = 0; k0 < ldp; k0 += BK) {
-                    const int chunks = min(BK, ldp - k0) >> 2;
+                    const int chunks = min(BK, ldp - k0) / CW;
                     r_mbar_wait(&s_empty[stage], phase ^ 1);
                     float* sa = rsm + (size_t)stage * R_STAGE_FLOATS;
                     const unsigned ba = (unsigned)(chunks * rows_a * 16), bb0 = (unsigned)(chunks * rows_b0 * 16),
@@ -264,12 +368,11 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                     r_mbar_expect_tx(&s_full[stage], PL * (ba + bb0 + bb1));
 #pragma unroll
                     for (int pl = 0; pl < PL; ++pl) {  // stage layout: [A planes][B0 planes][B1 planes]
-                        const size_t po = (size_t)pl * a.lo_plane;
-                        r_bulk_g2s(sa + pl * SA, Asrc + po + (size_t)(k0 >> 2) * rows_a * 4, ba, &s_full[stage]);
-                        r_bulk_g2s(sa + (PL + pl) * SA, B0 + po + (size_t)(k0 >> 2) * rows_b0 * 4, bb0, &s_full[stage]);
+                        const size_t po = (size_t)pl * a.lo_plane * ES, kc = (size_t)(k0 / CW) * 16;
+                        r_bulk_g2s(sa + pl * SA, Asrc + po + kc * rows_a, ba, &s_full[stage]);
+                        r_bulk_g2s(sa + (PL + pl) * SA, B0 + po + kc * rows_b0, bb0, &s_full[stage]);
                         if (rows_b1 > 0)
-                            r_bulk_g2s(sa + (2 * PL + pl) * SA, B1 + po + (size_t)(k0 >> 2) * rows_b1 * 4, bb1,
-                                       &s_full[stage]);
+                            r_bulk_g2s(sa + (2 * PL + pl) * SA, B1 + po + kc * rows_b1, bb1, &s_full[stage]);
                     }
                     if (++stage == R_STAGES) { stage = 0; phase ^= 1; }
                 }
@@ -290,9 +393,13 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                 r_mbar_wait(&s_tempty[buf], tphase[buf] ^ 1);  // epilogue has drained this accumulator
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t d0 = tmem + (uint32_t)(buf * R_BN);
-                const uint32_t id0 = r_idesc(rows_b0), id1 = r_idesc(rows_b1 > 0 ? rows_b1 : 16);
+                const uint32_t id0 = BF ? r_idesc_bf16(rows_b0) : r_idesc(rows_b0);
+                const uint32_t id1 = BF ? r_idesc_bf16(rows_b1 > 0 ? rows_b1 : 16) : r_idesc(rows_b1 > 0 ? rows_b1 : 16);
+                auto mma = [&](uint32_t d, uint64_t da, uint64_t db, uint32_t id, uint32_t acc) {
+                    if (BF) r_mma_bf16(d, da, db, id, acc); else r_mma(d, da, db, id, acc);
+                };
                 for (int k0 = 0; k0 < ldp; k0 += BK) {
-                    const int ksteps = min(BK, ldp - k0) >> 3;
+                    const int ksteps = min(BK, ldp - k0) / (2 * CW);  // two 16-byte chunks per instruction
                     r_mbar_wait(&s_full[stage], phase);
                     asm volatile("tcgen05.fence::after_thread_sync;");
                     const unsigned sa = r_smem_u32(rsm + (size_t)stage * R_STAGE_FLOATS);
@@ -303,16 +410,16 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                                        ob1 = (unsigned)(ks * 2 * rows_b1 * 16);
                         const unsigned la = (unsigned)(rows_a * 16), lb0 = (unsigned)(rows_b0 * 16), lb1 = (unsigned)(rows_b1 * 16);
                         const uint64_t da = r_desc(sa + oa, la);
-                        r_mma(d0, da, r_desc(sb0 + ob0, lb0), id0, acc);                                  // hi hi
+                        mma(d0, da, r_desc(sb0 + ob0, lb0), id0, acc);                                  // hi hi
                         if (SPLIT) {
-                            r_mma(d0, da, r_desc(sb0 + SA * 4 + ob0, lb0), id0, 1u);                      // hi lo
-                            r_mma(d0, r_desc(sa + SA * 4 + oa, la), r_desc(sb0 + ob0, lb0), id0, 1u);      // lo hi
+                            mma(d0, da, r_desc(sb0 + SA * 4 + ob0, lb0), id0, 1u);                      // hi lo
+                            mma(d0, r_desc(sa + SA * 4 + oa, la), r_desc(sb0 + ob0, lb0), id0, 1u);      // lo hi
                         }
                         if (rows_b1 > 0) {
-                            r_mma(d0 + 128, da, r_desc(sb1 + ob1, lb1), id1, acc);
+                            mma(d0 + 128, da, r_desc(sb1 + ob1, lb1), id1, acc);
                             if (SPLIT) {
-                                r_mma(d0 + 128, da, r_desc(sb1 + SA * 4 + ob1, lb1), id1, 1u);
-                                r_mma(d0 + 128, r_desc(sa + SA * 4 + oa, la), r_desc(sb1 + ob1, lb1), id1, 1u);
+                                mma(d0 + 128, da, r_desc(sb1 + SA * 4 + ob1, lb1), id1, 1u);
+                                mma(d0 + 128, r_desc(sa + SA * 4 + oa, la), r_desc(sb1 + ob1, lb1), id1, 1u);
                             }
                         }
                     }
@@ -347,7 +454,6 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
             // global loads of its X values are issued before chunk c is processed, so their latencies pass
             // behind the arithmetic and the stores of chunk c.
             uint32_t v[16], vn[16];
-            float4 xc[4], xn[4], xlc[4], xln[4];
             auto tld = [&](uint32_t (&d)[16], int c0) {
                 asm volatile(
                     "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
@@ -355,107 +461,224 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                       "=r"(d[8]), "=r"(d[9]), "=r"(d[10]), "=r"(d[11]), "=r"(d[12]), "=r"(d[13]), "=r"(d[14]), "=r"(d[15])
                     : "r"(taddr + (uint32_t)c0));
             };
-            auto xld = [&](float4 (&x)[4], float4 (&xl)[4], int c0) {  // MODE 1: X (and its lo plane) of this row
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int c = col0 + c0 + 4 * j;
-                    x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    xl[j] = x[j];
-                    if (rl < rows_a && c <= r) {
-                        const size_t o = (size_t)(c >> 2) * rows_a * 4;
-                        x[j] = *reinterpret_cast<const float4*>(xrow + o);
-                        if (SPLIT) xl[j] = *reinterpret_cast<const float4*>(xrow + o + a.lo_plane);
-                    }
-                }
-            };
-            tld(v, 0);
-            if (MODE == 1) xld(xc, xlc, 0);
-            for (int c0 = 0; c0 < ncols; c0 += 16) {
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                const bool more = c0 + 16 < ncols;
-                if (more) {
-                    tld(vn, c0 + 16);
-                    if (MODE == 1) xld(xn, xln, c0 + 16);
-                }
-                {
-                    const bool row_ok = rl < rows_a;
-                    const int rq = r & ~3;  // first row of this lane's quad (rows_a is a multiple of 16: quads are whole)
-#pragma unroll
+            if constexpr (!BF) {
+                float4 xc[4], xn[4], xlc[4], xln[4];
+                auto xld = [&](float4 (&x)[4], float4 (&xl)[4], int c0) {  // MODE 1: X (and its lo plane) of this row
+    #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         const int c = col0 + c0 + 4 * j;
-                        const bool act = row_ok && c <= r;  // upper triangle: the mirror image of (c, r) is stored instead
-                        const size_t o = (size_t)(c >> 2) * rows_a * 4;
-                        float w[4] = {__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
-                                      __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3])};
-                        if (MODE == 0) {
-                            if (act && r < n) {  // residual over the n x n part; strictly-lower elements count twice
-                                float p = 0.f;
-#pragma unroll
-                                for (int e = 0; e < 4; ++e) {
-                                    const float d = w[e] - (c + e == r ? 1.f : 0.f);
-                                    if (c + e < r) p += 2.f * d * d;
-                                    else if (c + e == r) p += d * d;
+                        x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        xl[j] = x[j];
+                        if (rl < rows_a && c <= r) {
+                            const size_t o = (size_t)(c >> 2) * rows_a * 4;
+                            x[j] = *reinterpret_cast<const float4*>(xrow + o);
+                            if (SPLIT) xl[j] = *reinterpret_cast<const float4*>(xrow + o + a.lo_plane);
+                        }
+                    }
+                };
+                tld(v, 0);
+                if (MODE == 1) xld(xc, xlc, 0);
+                for (int c0 = 0; c0 < ncols; c0 += 16) {
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    const bool more = c0 + 16 < ncols;
+                    if (more) {
+                        tld(vn, c0 + 16);
+                        if (MODE == 1) xld(xn, xln, c0 + 16);
+                    }
+                    {
+                        const bool row_ok = rl < rows_a;
+                        const int rq = r & ~3;  // first row of this lane's quad (rows_a is a multiple of 16: quads are whole)
+    #pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const int c = col0 + c0 + 4 * j;
+                            const bool act = row_ok && c <= r;  // upper triangle: the mirror image of (c, r) is stored instead
+                            const size_t o = (size_t)(c >> 2) * rows_a * 4;
+                            float w[4] = {__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
+                                          __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3])};
+                            if (MODE == 0) {
+                                if (act && r < n) {  // residual over the n x n part; strictly-lower elements count twice
+                                    float p = 0.f;
+    #pragma unroll
+                                    for (int e = 0; e < 4; ++e) {
+                                        const float d = w[e] - (c + e == r ? 1.f : 0.f);
+                                        if (c + e < r) p += 2.f * d * d;
+                                        else if (c + e == r) p += d * d;
+                                    }
+                                    part += (double)p;
                                 }
-                                part += (double)p;
-                            }
-                        } else {
-                            float4 x = xc[j];
-                            if (SPLIT) { x.x += xlc[j].x; x.y += xlc[j].y; x.z += xlc[j].z; x.w += xlc[j].w; }
-                            w[0] = 1.5f * x.x - 0.5f * w[0]; w[1] = 1.5f * x.y - 0.5f * w[1];
-                            w[2] = 1.5f * x.z - 0.5f * w[2]; w[3] = 1.5f * x.w - 0.5f * w[3];
-                        }
-                        float hi[4], lo[4];
-#pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            hi[e] = SPLIT ? r_tf32(w[e]) : w[e];
-                            lo[e] = w[e] - hi[e];
-                        }
-                        // direct elements (r, c + e), c + e <= r: one 16-byte store when the whole group is
-                        // on or below the diagonal.  Every stored element has exactly one writer, so X and Y stay
-                        // bitwise symmetric, which is what lets B be read as rows (and keeps the iteration
-                        // stable: the X X^T form amplifies any antisymmetric rounding noise).
-                        if (act) {
-                            if (c + 3 <= r) {
-                                *reinterpret_cast<float4*>(orow + o) = make_float4(hi[0], hi[1], hi[2], hi[3]);
-                                if (SPLIT) *reinterpret_cast<float4*>(orow + o + a.lo_plane) = make_float4(lo[0], lo[1], lo[2], lo[3]);
                             } else {
-#pragma unroll
+                                float4 x = xc[j];
+                                if (SPLIT) { x.x += xlc[j].x; x.y += xlc[j].y; x.z += xlc[j].z; x.w += xlc[j].w; }
+                                w[0] = 1.5f * x.x - 0.5f * w[0]; w[1] = 1.5f * x.y - 0.5f * w[1];
+                                w[2] = 1.5f * x.z - 0.5f * w[2]; w[3] = 1.5f * x.w - 0.5f * w[3];
+                            }
+                            float hi[4], lo[4];
+    #pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                hi[e] = SPLIT ? r_tf32(w[e]) : w[e];
+                                lo[e] = w[e] - hi[e];
+                            }
+                            // direct elements (r, c + e), c + e <= r: one 16-byte store when the whole group is
+                            // on or below the diagonal.  Every stored element has exactly one writer, so X and Y stay
+                            // bitwise symmetric, which is what lets B be read as rows (and keeps the iteration
+                            // stable: the X X^T form amplifies any antisymmetric rounding noise).
+                            if (act) {
+                                if (c + 3 <= r) {
+                                    *reinterpret_cast<float4*>(orow + o) = make_float4(hi[0], hi[1], hi[2], hi[3]);
+                                    if (SPLIT) *reinterpret_cast<float4*>(orow + o + a.lo_plane) = make_float4(lo[0], lo[1], lo[2], lo[3]);
+                                } else {
+    #pragma unroll
+                                    for (int e = 0; e < 4; ++e)
+                                        if (c + e <= r) {
+                                            orow[o + e] = hi[e];
+                                            if (SPLIT) orow[o + e + a.lo_plane] = lo[e];
+                                        }
+                                }
+                            }
+                            // mirror elements (c + e, r), c + e < r.  A quad of lanes (rows rq .. rq + 3) holds a 4 x 4
+                            // block; when it lies strictly below the diagonal it is transposed inside the quad (four
+                            // shuffles per plane, executed by every lane) and lane e stores mirror row c + e as ONE
+                            // 16-byte store; blocks touching the diagonal keep the 4-byte stores.
+                            const bool blk = row_ok && c + 3 < rq;
+                            float th[4] = {hi[0], hi[1], hi[2], hi[3]}, tl[4] = {lo[0], lo[1], lo[2], lo[3]};
+                            quad_transpose(th, lane);
+                            if (SPLIT) quad_transpose(tl, lane);
+                            if (blk) {
+                                float* mp = a.Out + T.off32 + panel32_off(c + (lane & 3), rq, ldp);
+                                *reinterpret_cast<float4*>(mp) = make_float4(th[0], th[1], th[2], th[3]);
+                                if (SPLIT) *reinterpret_cast<float4*>(mp + a.lo_plane) = make_float4(tl[0], tl[1], tl[2], tl[3]);
+                            } else if (act) {
+    #pragma unroll
                                 for (int e = 0; e < 4; ++e)
-                                    if (c + e <= r) {
-                                        orow[o + e] = hi[e];
-                                        if (SPLIT) orow[o + e + a.lo_plane] = lo[e];
+                                    if (c + e < r) {
+                                        float* mp = a.Out + T.off32 + panel32_off(c + e, r, ldp);
+                                        *mp = hi[e];
+                                        if (SPLIT) mp[a.lo_plane] = lo[e];
                                     }
                             }
                         }
-                        // mirror elements (c + e, r), c + e < r.  A quad of lanes (rows rq .. rq + 3) holds a 4 x 4
-                        // block; when it lies strictly below the diagonal it is transposed inside the quad (four
-                        // shuffles per plane, executed by every lane) and lane e stores mirror row c + e as ONE
-                        // 16-byte store; blocks touching the diagonal keep the 4-byte stores.
-                        const bool blk = row_ok && c + 3 < rq;
-                        float th[4] = {hi[0], hi[1], hi[2], hi[3]}, tl[4] = {lo[0], lo[1], lo[2], lo[3]};
-                        quad_transpose(th, lane);
-                        if (SPLIT) quad_transpose(tl, lane);
-                        if (blk) {
-                            float* mp = a.Out + T.off32 + panel32_off(c + (lane & 3), rq, ldp);
-                            *reinterpret_cast<float4*>(mp) = make_float4(th[0], th[1], th[2], th[3]);
-                            if (SPLIT) *reinterpret_cast<float4*>(mp + a.lo_plane) = make_float4(tl[0], tl[1], tl[2], tl[3]);
-                        } else if (act) {
-#pragma unroll
-                            for (int e = 0; e < 4; ++e)
-                                if (c + e < r) {
-                                    float* mp = a.Out + T.off32 + panel32_off(c + e, r, ldp);
-                                    *mp = hi[e];
-                                    if (SPLIT) mp[a.lo_plane] = lo[e];
-                                }
+                    }
+                    if (more) {
+    #pragma unroll
+                        for (int e = 0; e < 16; ++e) v[e] = vn[e];
+                        if (MODE == 1) {
+    #pragma unroll
+                            for (int j = 0; j < 4; ++j) { xc[j] = xn[j]; xlc[j] = xln[j]; }
                         }
                     }
                 }
-                if (more) {
+            } else {
+                // BF16 hi / lo planes: 8 columns per 16-byte chunk.  Direct elements go out as 16-byte stores per
+                // plane, mirror elements as 8-byte stores (4 x 4 blocks transposed inside the lane quads).
+                unsigned short* o16 = reinterpret_cast<unsigned short*>(a.Out) + T.off32;
+                unsigned short* orow16 = o16 + (size_t)row0 * ldp + (size_t)rl * 8;
+                const unsigned short* xrow16 =
+                    reinterpret_cast<const unsigned short*>(a.A) + T.off32 + (size_t)row0 * ldp + (size_t)rl * 8;
+                uint4 xh[2], xl[2], xhn[2], xln[2];
+                auto xld16 = [&](uint4 (&h)[2], uint4 (&l)[2], int c0) {
 #pragma unroll
-                    for (int e = 0; e < 16; ++e) v[e] = vn[e];
-                    if (MODE == 1) {
+                    for (int jj = 0; jj < 2; ++jj) {
+                        const int c = col0 + c0 + 8 * jj;
+                        h[jj] = make_uint4(0u, 0u, 0u, 0u);
+                        l[jj] = h[jj];
+                        if (rl < rows_a && c <= r) {
+                            const size_t o = (size_t)(c >> 3) * rows_a * 8;
+                            h[jj] = *reinterpret_cast<const uint4*>(xrow16 + o);
+                            l[jj] = *reinterpret_cast<const uint4*>(xrow16 + o + a.lo_plane);
+                        }
+                    }
+                };
+                tld(v, 0);
+                if (MODE == 1) xld16(xh, xl, 0);
+                for (int c0 = 0; c0 < ncols; c0 += 16) {
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    const bool more = c0 + 16 < ncols;
+                    if (more) {
+                        tld(vn, c0 + 16);
+                        if (MODE == 1) xld16(xhn, xln, c0 + 16);
+                    }
+                    const bool row_ok = rl < rows_a;
+                    const int rq = r & ~3;
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) { xc[j] = xn[j]; xlc[j] = xln[j]; }
+                    for (int jj = 0; jj < 2; ++jj) {
+                        const int c = col0 + c0 + 8 * jj;
+                        const bool act = row_ok && c <= r;
+                        const size_t o = (size_t)(c >> 3) * rows_a * 8;
+                        float w[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) w[e] = __uint_as_float(v[8 * jj + e]);
+                        if (MODE == 0) {
+                            if (act && r < n) {
+                                float pr = 0.f;
+#pragma unroll
+                                for (int e = 0; e < 8; ++e) {
+                                    const float d = w[e] - (c + e == r ? 1.f : 0.f);
+                                    if (c + e < r) pr += 2.f * d * d;
+                                    else if (c + e == r) pr += d * d;
+                                }
+                                part += (double)pr;
+                            }
+                        } else {
+                            const unsigned hw[4] = {xh[jj].x, xh[jj].y, xh[jj].z, xh[jj].w};
+                            const unsigned lw[4] = {xl[jj].x, xl[jj].y, xl[jj].z, xl[jj].w};
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                const unsigned short hb = (unsigned short)(hw[e >> 1] >> (16 * (e & 1)));
+                                const unsigned short lb = (unsigned short)(lw[e >> 1] >> (16 * (e & 1)));
+                                const float x = bf_val(hb) + bf_val(lb);
+                                w[e] = 1.5f * x - 0.5f * w[e];
+                            }
+                        }
+                        unsigned short hi[8], lo[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) bf_split(w[e], hi[e], lo[e]);
+                        if (act) {
+                            if (c + 7 <= r) {
+                                *reinterpret_cast<uint4*>(orow16 + o) = make_uint4(bf_pack2(hi[0], hi[1]), bf_pack2(hi[2], hi[3]),
+                                                                                   bf_pack2(hi[4], hi[5]), bf_pack2(hi[6], hi[7]));
+                                *reinterpret_cast<uint4*>(orow16 + o + a.lo_plane) =
+                                    make_uint4(bf_pack2(lo[0], lo[1]), bf_pack2(lo[2], lo[3]), bf_pack2(lo[4], lo[5]), bf_pack2(lo[6], lo[7]));
+                            } else {
+#pragma unroll
+                                for (int e = 0; e < 8; ++e)
+                                    if (c + e <= r) { orow16[o + e] = hi[e]; orow16[o + e + a.lo_plane] = lo[e]; }
+                            }
+                        }
+#pragma unroll
+                        for (int q4 = 0; q4 < 2; ++q4) {
+                            const int cc = c + 4 * q4;
+                            const bool blk = row_ok && cc + 3 < rq;
+                            float th[4], tl[4];
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) { th[e] = bf_val(hi[4 * q4 + e]); tl[e] = bf_val(lo[4 * q4 + e]); }
+                            quad_transpose(th, lane);
+                            quad_transpose(tl, lane);
+                            if (blk) {
+                                unsigned short* mp = o16 + panel16_off(cc + (lane & 3), rq, ldp);
+                                *reinterpret_cast<uint2*>(mp) =
+                                    make_uint2((__float_as_uint(th[0]) >> 16) | (__float_as_uint(th[1]) & 0xffff0000u),
+                                               (__float_as_uint(th[2]) >> 16) | (__float_as_uint(th[3]) & 0xffff0000u));
+                                *reinterpret_cast<uint2*>(mp + a.lo_plane) =
+                                    make_uint2((__float_as_uint(tl[0]) >> 16) | (__float_as_uint(tl[1]) & 0xffff0000u),
+                                               (__float_as_uint(tl[2]) >> 16) | (__float_as_uint(tl[3]) & 0xffff0000u));
+                            } else if (row_ok) {
+#pragma unroll
+                                for (int e = 0; e < 4; ++e)
+                                    if (cc + e < r) {
+                                        unsigned short* mp = o16 + panel16_off(cc + e, r, ldp);
+                                        *mp = hi[4 * q4 + e];
+                                        mp[a.lo_plane] = lo[4 * q4 + e];
+                                    }
+                            }
+                        }
+                    }
+                    if (more) {
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) v[e] = vn[e];
+                        if (MODE == 1) {
+#pragma unroll
+                            for (int jj = 0; jj < 2; ++jj) { xh[jj] = xhn[jj]; xl[jj] = xln[jj]; }
+                        }
                     }
                 }
             }
@@ -557,9 +780,14 @@ sm_status_t build_tf32_tables(sm_plan* p, cudaStream_t st) {
 sm_status_t launch_to_f32(sm_plan* p, const double* buf0, double* buf1, cudaStream_t st) {
     if (p->ngroups == 0) return SM_OK;
     const int split = (int)std::min<int64_t>(8, std::max<int64_t>(1, (int64_t)p->num_sms * 8 / p->ngroups));
-    k_to_f32<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
-                                                       p->d_gersh, buf0, reinterpret_cast<float*>(buf1),
-                                                       p->opt.precision == 2 ? p->sum_ldp2 : 0);
+    if (p->opt.precision == 3)
+        k_to_bf16<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
+                                                            p->d_gersh, buf0, reinterpret_cast<unsigned short*>(buf1),
+                                                            p->sum_ldp2);
+    else
+        k_to_f32<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
+                                                           p->d_gersh, buf0, reinterpret_cast<float*>(buf1),
+                                                           p->opt.precision == 2 ? p->sum_ldp2 : 0);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
@@ -568,11 +796,18 @@ sm_status_t launch_to_f32(sm_plan* p, const double* buf0, double* buf1, cudaStre
 sm_status_t launch_to_f64(sm_plan* p, double* buf0, const double* buf1, const double* bufY, cudaStream_t st) {
     if (p->ngroups == 0) return SM_OK;
     const int split = (int)std::min<int64_t>(8, std::max<int64_t>(1, (int64_t)p->num_sms * 8 / p->ngroups));
-    k_to_f64<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
-                                                       p->d_gersh, p->d_done_iter, p->cur_k,
-                                                       reinterpret_cast<const float*>(buf1),
-                                                       reinterpret_cast<const float*>(bufY), buf0,
-                                                       p->opt.precision == 2 ? p->sum_ldp2 : 0);
+    if (p->opt.precision == 3)
+        k_from_bf16<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
+                                                              p->d_gersh, p->d_done_iter, p->cur_k,
+                                                              reinterpret_cast<const unsigned short*>(buf1),
+                                                              reinterpret_cast<const unsigned short*>(bufY), buf0,
+                                                              p->sum_ldp2);
+    else
+        k_to_f64<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
+                                                           p->d_gersh, p->d_done_iter, p->cur_k,
+                                                           reinterpret_cast<const float*>(buf1),
+                                                           reinterpret_cast<const float*>(bufY), buf0,
+                                                           p->opt.precision == 2 ? p->sum_ldp2 : 0);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
@@ -586,6 +821,8 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         p->tf32_attr_set = 1;
     }
     float* X[2] = {reinterpret_cast<float*>(buf1), reinterpret_cast<float*>(bufY)};
@@ -593,12 +830,13 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
     Ns32Args a;
     a.tiles = reinterpret_cast<const Tile32*>(p->d_tiles32); a.partials = p->d_partials32; a.done_iter = p->d_done_iter;
     a.n_tiles = (int32_t)p->n_tiles32; a.ctrl = p->d_ctrl;
-    const bool split = p->opt.precision == 2;
+    const int split = p->opt.precision == 2 ? 1 : p->opt.precision == 3 ? 2 : 0;
     a.lo_plane = split ? p->sum_ldp2 : 0;
     const int grid = (int)std::min<int64_t>(p->n_tiles32, (int64_t)p->num_sms * R_CTAS);
     if (which & 1) {
         a.A = X[k & 1]; a.B = X[k & 1]; a.Out = Y;
-        if (split) k_ns_tf32<0, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        if (split == 2) k_ns_tf32<0, 2><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        else if (split == 1) k_ns_tf32<0, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
         else k_ns_tf32<0, 0><<<grid, R_THREADS, R_SMEM, st>>>(a);
         k_ns_decide32<<<(p->ngroups + 7) / 8, 256, 0, st>>>(p->ngroups, k, decide_only, eps, 0.5,
                                                             p->d_tile_first32,
@@ -608,7 +846,8 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
     }
     if ((which & 2) && !decide_only) {
         a.A = X[k & 1]; a.B = Y; a.Out = X[(k + 1) & 1];
-        if (split) k_ns_tf32<1, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        if (split == 2) k_ns_tf32<1, 2><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        else if (split == 1) k_ns_tf32<1, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
         else k_ns_tf32<1, 0><<<grid, R_THREADS, R_SMEM, st>>>(a);
         p->launches += 1;
     }
