@@ -343,19 +343,29 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tmem = s_tmem;
     const int n_tiles = a.ctrl[0] != 0 ? 0 : a.n_tiles;
+    // Tiles are dealt to the CTAs in consecutive PAIRS when there are enough of them: the 128-row units of one
+    // submatrix share operand rows (unit 1 reads the rows of unit 0 as its first B half), and back to back on one
+    // CTA the second read hits L2.
+    const bool pair = a.n_tiles >= 4 * (int)gridDim.x;
+#define R_TILES(t)                                                                     \
+    for (int t = pair ? 2 * (int)blockIdx.x : (int)blockIdx.x; t < n_tiles;            \
+         t += pair ? ((t & 1) ? 2 * (int)gridDim.x - 1 : 1) : (int)gridDim.x)
 
     if (wid == 0) {
         // ================================================================ producer (one thread)
         if (lane == 0) {
             int stage = 0;
             unsigned phase = 0;
-            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+            R_TILES(t) {
                 const Tile32 T = a.tiles[t];
                 if (a.done_iter[T.grp] >= 0) continue;
                 const int ldp = T.ldp;
                 const int row0 = T.ti * R_BM, rows_a = min(R_BM, ldp - row0);
                 const int col0 = T.tj * R_BN, ncols = min(R_BN, min(ldp, row0 + R_BM) - col0);  // lower triangle only
                 const int rows_b0 = min(128, ncols), rows_b1 = max(0, ncols - 128);
+                // Y = X X: a B half that covers the rows of A IS the A slice (X is symmetric and B is read as rows):
+                // it is loaded once and the issuer points both descriptors at it
+                const bool b0_is_a = MODE == 0 && col0 == row0, b1_is_a = MODE == 0 && rows_b1 > 0 && col0 + 128 == row0;
                 const char* Asrc = reinterpret_cast<const char*>(a.A) + ((size_t)T.off32 + (size_t)row0 * ldp) * ES;
                 const char* B0 = reinterpret_cast<const char*>(a.B) + ((size_t)T.off32 + (size_t)col0 * ldp) * ES;
                 const char* B1 = reinterpret_cast<const char*>(a.B) + ((size_t)T.off32 + (size_t)(col0 + 128) * ldp) * ES;
@@ -365,13 +375,13 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                     float* sa = rsm + (size_t)stage * R_STAGE_FLOATS;
                     const unsigned ba = (unsigned)(chunks * rows_a * 16), bb0 = (unsigned)(chunks * rows_b0 * 16),
                                    bb1 = (unsigned)(chunks * rows_b1 * 16);
-                    r_mbar_expect_tx(&s_full[stage], PL * (ba + bb0 + bb1));
+                    r_mbar_expect_tx(&s_full[stage], PL * (ba + (b0_is_a ? 0u : bb0) + (b1_is_a ? 0u : bb1)));
 #pragma unroll
                     for (int pl = 0; pl < PL; ++pl) {  // stage layout: [A planes][B0 planes][B1 planes]
                         const size_t po = (size_t)pl * a.lo_plane * ES, kc = (size_t)(k0 / CW) * 16;
                         r_bulk_g2s(sa + pl * SA, Asrc + po + kc * rows_a, ba, &s_full[stage]);
-                        r_bulk_g2s(sa + (PL + pl) * SA, B0 + po + kc * rows_b0, bb0, &s_full[stage]);
-                        if (rows_b1 > 0)
+                        if (!b0_is_a) r_bulk_g2s(sa + (PL + pl) * SA, B0 + po + kc * rows_b0, bb0, &s_full[stage]);
+                        if (rows_b1 > 0 && !b1_is_a)
                             r_bulk_g2s(sa + (2 * PL + pl) * SA, B1 + po + kc * rows_b1, bb1, &s_full[stage]);
                     }
                     if (++stage == R_STAGES) { stage = 0; phase ^= 1; }
@@ -383,13 +393,14 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
         if (lane == 0) {
             int stage = 0, buf = 0;
             unsigned phase = 0, tphase[2] = {0, 0};
-            for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+            R_TILES(t) {
                 const Tile32 T = a.tiles[t];
                 if (a.done_iter[T.grp] >= 0) continue;
                 const int ldp = T.ldp;
                 const int row0 = T.ti * R_BM, rows_a = min(R_BM, ldp - row0);
                 const int col0 = T.tj * R_BN, ncols = min(R_BN, min(ldp, row0 + R_BM) - col0);
                 const int rows_b0 = min(128, ncols), rows_b1 = max(0, ncols - 128);
+                const bool b0_is_a = MODE == 0 && col0 == row0, b1_is_a = MODE == 0 && rows_b1 > 0 && col0 + 128 == row0;
                 r_mbar_wait(&s_tempty[buf], tphase[buf] ^ 1);  // epilogue has drained this accumulator
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t d0 = tmem + (uint32_t)(buf * R_BN);
@@ -403,7 +414,7 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                     r_mbar_wait(&s_full[stage], phase);
                     asm volatile("tcgen05.fence::after_thread_sync;");
                     const unsigned sa = r_smem_u32(rsm + (size_t)stage * R_STAGE_FLOATS);
-                    const unsigned sb0 = sa + PL * SA * 4, sb1 = sa + 2 * PL * SA * 4;
+                    const unsigned sb0 = b0_is_a ? sa : sa + PL * SA * 4, sb1 = b1_is_a ? sa : sa + 2 * PL * SA * 4;
                     for (int ks = 0; ks < ksteps; ++ks) {
                         const uint32_t acc = (k0 > 0 || ks > 0) ? 1u : 0u;
                         const unsigned oa = (unsigned)(ks * 2 * rows_a * 16), ob0 = (unsigned)(ks * 2 * rows_b0 * 16),
@@ -436,7 +447,7 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
         const int q = wid & 3;  // TMEM lane quarter this warp may access
         int buf = 0;
         unsigned tphase[2] = {0, 0};
-        for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        R_TILES(t) {
             const Tile32 T = a.tiles[t];
             if (a.done_iter[T.grp] >= 0) continue;
             const int ldp = T.ldp, n = T.n;
@@ -693,6 +704,7 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
             if (R_TBUFS == 2) buf ^= 1;
         }
     }
+#undef R_TILES
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
     if (wid == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(R_TCOLS));
