@@ -75,7 +75,7 @@ typedef struct {
                          /* 3 = "BF16x2": operands stored as hi + lo BF16 pairs (16 mantissa */
                          /*     bits, 4 bytes per element), products hi hi + hi lo + lo hi   */
                          /*     on kind::f16: the rung between the two others -- error 1e-5  */
-                         /*     class at two thirds of the FP64 time (half the operand bytes) */
+                         /*     class at half the FP64 time or less (half the operand bytes)  */
                          /* 1 = FP32 storage, plain TF32 products: experimental, error 5e-4   */
                          /*     ... 2e-3, does NOT meet the 1e-3 bar in general and its      */
                          /*     n_elec is too coarse to steer the mu search on large systems */

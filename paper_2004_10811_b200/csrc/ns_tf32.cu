@@ -13,19 +13,22 @@
 // no tensor map, and the tensor core reads it as it landed.  It also makes the epilogue coalesced:
 // thread r of a warp owns TMEM lane (row) r and writes 16 B per chunk next to its neighbours.
 //
-// Kernel: persistent, one CTA per SM, warp-specialised:
-//   warp 0 (one thread)  producer: cp.async.bulk of the A / B slices into a 4-stage ring (mbarrier tx)
+// Kernel: persistent, two CTAs per SM, warp-specialised:
+//   warp 0 (one thread)  producer: cp.async.bulk of the A / B slices into a 2-stage ring (mbarrier tx)
 //   warp 1 (one thread)  issues tcgen05.mma (M = 128, N = rows of the B half, K = 8 per instruction),
 //                        tcgen05.commit releases the stage / hands the accumulator to the epilogue
-//   warps 2..5           epilogue: tcgen05.ld of their 32 TMEM lanes, MODE 0: Y = X X and residual
-//                        partials; MODE 1: X' = 3/2 X - 1/2 X Y; two 256-column accumulators in
-//                        TMEM, so the epilogue of one tile overlaps the MMAs of the next.
+//   warps 2..9           epilogue, two sets of four warps (one per TMEM lane quarter; the sets split the
+//                        16-column chunks of a tile): tcgen05.ld of their 32 TMEM lanes, MODE 0: Y = X X and
+//                        residual partials; MODE 1: X' = 3/2 X - 1/2 X Y.  Two CTAs per SM, one 256-column
+//                        accumulator each: the epilogue of a tile overlaps the MMAs of the other CTA's tile.
+//                        The launches are bound by epilogue latency, not by the tensor pipe or HBM (ncu: 15 %
+//                        tensor, 33-51 % DRAM), which is why the second warp set pays.
 // options.precision = 2 ("3xTF32") stores hi + lo TF32 planes (8 bytes per element) and issues three products per
 // k step; options.precision = 3 ("BF16x2") stores hi + lo BF16 planes (4 bytes per element, 8 columns per 16-byte
 // chunk) and issues the same three products with kind::f16 -- the launches are HBM-bound, so halving the bytes is
 // what makes that rung faster than FP64 (Table I's ladder, L366-374, on this part's tensor pipes).
-// Work unit: (submatrix, 128-row tile, 256-column tile on or below the diagonal), static round-robin
-// over the CTAs.  Only the lower triangle is computed; every element is stored together with its
+// Work unit: (submatrix, 128-row tile, 256-column tile on or below the diagonal), dealt to the CTAs in
+// consecutive pairs (the units of one submatrix share operand rows).  Only the lower triangle is computed; every element is stored together with its
 // mirror image, so X and Y are bitwise symmetric and B can be read as k-contiguous rows.
 #include <algorithm>
 
@@ -45,7 +48,8 @@ constexpr int R_BM = 128, R_BN = 256, R_BK = 32, R_STAGES = R_CTAS == 1 ? 4 : 2;
 constexpr int R_TBUFS = R_CTAS == 1 ? 2 : 1, R_TCOLS = R_CTAS == 1 ? 512 : 256;
 constexpr int R_STAGE_FLOATS = (R_BM + R_BN) * R_BK;  // 48 KB
 constexpr size_t R_SMEM = (size_t)R_STAGES * R_STAGE_FLOATS * sizeof(float);
-constexpr int R_THREADS = 192;
+constexpr int R_EPI = 2;                 // epilogue warp sets (4 warps each: one per TMEM lane quarter)
+constexpr int R_THREADS = 64 + 128 * R_EPI;
 
 __host__ __device__ __forceinline__ size_t panel32_off(int r, int c, int ldp) {
     const int t0 = r & ~127;
@@ -319,6 +323,7 @@ struct Ns32Args {
 template <int MODE, int SPLIT>
 __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
     constexpr bool BF = SPLIT == 2;                 // BF16 hi / lo planes instead of FP32 ones
+    constexpr bool PIPE = SPLIT == 0;               // software-pipelined epilogue (the split variants lack the registers)
     constexpr int CW = BF ? 8 : 4;                  // columns per 16-byte chunk
     constexpr int ES = BF ? 2 : 4;                  // bytes per element
     constexpr int CH = SPLIT ? 4 : 8;               // chunks per stage and plane
@@ -331,7 +336,7 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     if (tid == 0) {
         for (int s = 0; s < R_STAGES; ++s) { r_mbar_init(&s_full[s], 1); r_mbar_init(&s_empty[s], 1); }
-        for (int b = 0; b < 2; ++b) { r_mbar_init(&s_tfull[b], 1); r_mbar_init(&s_tempty[b], 4); }
+        for (int b = 0; b < 2; ++b) { r_mbar_init(&s_tfull[b], 1); r_mbar_init(&s_tempty[b], 4 * R_EPI); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (wid == 1) {  // tensor memory: all 512 columns (one CTA per SM), two 256-column accumulators
@@ -443,8 +448,9 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
             }
         }
     } else {
-        // ================================================================ epilogue warps 2..5
+        // ================================================================ epilogue warps 2..9
         const int q = wid & 3;  // TMEM lane quarter this warp may access
+        const int eset = (wid - 2) >> 2;  // warp set: the sets split the 16-column chunks of a tile between them
         int buf = 0;
         unsigned tphase[2] = {0, 0};
         R_TILES(t) {
@@ -461,6 +467,8 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
             float* orow = a.Out + T.off32 + (size_t)row0 * ldp + (size_t)rl * 4;
             const float* xrow = a.A + T.off32 + (size_t)row0 * ldp + (size_t)rl * 4;
             double part = 0.0;
+            const int nch = (ncols + 15) >> 4, csplit = ((nch + R_EPI - 1) / R_EPI) * 16;
+            const int cbeg = min(ncols, eset * csplit), cend = min(ncols, cbeg + csplit);
             // Software pipeline over the 16-column chunks: the tensor-memory load of chunk c + 1 and (MODE 1) the
             // global loads of its X values are issued before chunk c is processed, so their latencies pass
             // behind the arithmetic and the stores of chunk c.
@@ -487,11 +495,11 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                         }
                     }
                 };
-                tld(v, 0);
-                if (MODE == 1) xld(xc, xlc, 0);
-                for (int c0 = 0; c0 < ncols; c0 += 16) {
+                if (PIPE) { tld(v, cbeg); if (MODE == 1) xld(xc, xlc, cbeg); }
+                for (int c0 = cbeg; c0 < cend; c0 += 16) {
+                    if (!PIPE) { tld(v, c0); if (MODE == 1) xld(xc, xlc, c0); }
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                    const bool more = c0 + 16 < ncols;
+                    const bool more = PIPE && c0 + 16 < cend;
                     if (more) {
                         tld(vn, c0 + 16);
                         if (MODE == 1) xld(xn, xln, c0 + 16);
@@ -599,11 +607,11 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                         }
                     }
                 };
-                tld(v, 0);
-                if (MODE == 1) xld16(xh, xl, 0);
-                for (int c0 = 0; c0 < ncols; c0 += 16) {
+                if (PIPE) { tld(v, cbeg); if (MODE == 1) xld16(xh, xl, cbeg); }
+                for (int c0 = cbeg; c0 < cend; c0 += 16) {
+                    if (!PIPE) { tld(v, c0); if (MODE == 1) xld16(xh, xl, c0); }
                     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                    const bool more = c0 + 16 < ncols;
+                    const bool more = PIPE && c0 + 16 < cend;
                     if (more) {
                         tld(vn, c0 + 16);
                         if (MODE == 1) xld16(xhn, xln, c0 + 16);
@@ -699,7 +707,7 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
             if (MODE == 0) {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-                if (lane == 0) a.partials[(size_t)T.tile * 4 + q] = part;
+                if (lane == 0) a.partials[(size_t)T.tile * (4 * R_EPI) + 4 * eset + q] = part;
             }
             if (R_TBUFS == 2) buf ^= 1;
         }
@@ -726,8 +734,8 @@ k_ns_decide32(int ngroups, int k, int decide_only, double eps, double floor_zone
     if (g >= ngroups || ctrl[0] != 0) return;
     if (done_iter[g] >= 0) return;
     const int lane = threadIdx.x & 31;
-    const int cnt = 4 * tile_count[g], n = sub_dim[g];
-    const double* pp = partials + (size_t)tile_first[g] * 4;
+    const int cnt = 4 * R_EPI * tile_count[g], n = sub_dim[g];
+    const double* pp = partials + (size_t)tile_first[g] * (4 * R_EPI);
     double r2 = 0.0;
     for (int t = lane; t < cnt; t += 32) r2 += pp[t];
 #pragma unroll
@@ -778,7 +786,7 @@ sm_status_t build_tf32_tables(sm_plan* p, cudaStream_t st) {
     if ((s = up((void**)&p->d_tile_first32, first.data(), (size_t)ng * 4))) return s;
     if ((s = up((void**)&p->d_tile_count32, count.data(), (size_t)ng * 4))) return s;
     if ((s = up((void**)&p->d_tiles32, tiles.data(), tiles.size() * sizeof(Tile32)))) return s;
-    SM_CUDA(cudaMalloc((void**)&p->d_partials32, std::max<size_t>((size_t)tiles.size() * 32, 16)));
+    SM_CUDA(cudaMalloc((void**)&p->d_partials32, std::max<size_t>((size_t)tiles.size() * 32 * R_EPI, 16)));
     SM_CUDA(cudaStreamSynchronize(st));
     // each of the three workspace buffers must hold the FP64 matrices and the FP32 ones
     const size_t need = std::max((size_t)p->sum_ld2 * 8, (size_t)p->sum_ldp2 * 4 * planes);
