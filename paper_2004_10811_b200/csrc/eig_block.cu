@@ -21,6 +21,7 @@ namespace smb {
 constexpr int BJ_B = 16;       // columns per block
 constexpr int BJ_WARPS = 8;    // warps per CTA
 constexpr int BJ_LDM = 33;     // leading dimension of the 32 x 32 matrices in shared memory (conflict-free both ways)
+constexpr int BJ_MAXN = 1024;  // blocks per submatrix with barrier-free rounds (n <= 16384)
 constexpr int BJ_INNER = 1;    // sweeps of the 32 x 32 Jacobi per visit (the outer sweeps finish the job)
 
 struct BjArgs {
@@ -234,6 +235,7 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
 __global__ void __launch_bounds__(BJ_WARPS * 32, 1) k_eig_bjacobi(const BjArgs A) {
     extern __shared__ __align__(16) double bsm[];  // per warp: M[32 x 33], W[32 x 33], cs[32], pq[32 ints]
     __shared__ int s_next, s_rot;
+    __shared__ int s_ver[BJ_MAXN];
     __shared__ int s_genrow[1024];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     constexpr int PERW = 2 * 32 * BJ_LDM + 32 + 16;
@@ -255,19 +257,43 @@ __global__ void __launch_bounds__(BJ_WARPS * 32, 1) k_eig_bjacobi(const BjArgs A
         const int nblk = (n + BJ_B - 1) / BJ_B;
         const int N = nblk + (nblk & 1);  // >= 2: a single block is paired with an empty one
         int sweep = 0, converged = n <= 1 ? 1 : 0;
+        // Rounds are NOT separated by CTA barriers: a visit of (I, J) in round R only needs the round R - 1 visits
+        // of I and of J, so every block carries the number of rounds it has been through (s_ver) and a warp waits
+        // for its two blocks alone; warps whose visits end early (Gram matrix already diagonal) run ahead.  Every
+        // block is visited exactly once per round, rounds are processed in order by every warp: no cycle of waits.
+        const bool flow = N <= BJ_MAXN;
+        for (int b = threadIdx.x; b < N && flow; b += blockDim.x) s_ver[b] = 0;
+        __syncthreads();
+        int R = 0;
         for (; sweep < A.max_sweeps && !converged; ++sweep) {
             if (threadIdx.x == 0) s_rot = 0;
             __syncthreads();
             int my_rot = 0;
-            for (int r = 0; r < N - 1; ++r) {
+            for (int r = 0; r < N - 1; ++r, ++R) {
                 for (int q = wid; q < N / 2; q += BJ_WARPS) {
                     int I = (q == 0) ? N - 1 : (r + q) % (N - 1);
                     int J = (q == 0) ? r : (r - q + (N - 1)) % (N - 1);
                     if (I > J) { const int t = I; I = J; J = t; }
-                    if (I >= nblk) continue;  // both empty
-                    my_rot |= bj_visit(Gm, n, ld, I, J, nblk, M, W, cs, pq, tol2, lane);
+                    if (flow) {
+                        if (lane == 0) {
+                            volatile int* v = s_ver;
+                            while (v[I] < R || v[J] < R) {}
+                        }
+                        __syncwarp();
+                        __threadfence_block();
+                    }
+                    if (I < nblk) my_rot |= bj_visit(Gm, n, ld, I, J, nblk, M, W, cs, pq, tol2, lane);
+                    if (flow) {
+                        __threadfence_block();
+                        __syncwarp();
+                        if (lane == 0) {
+                            volatile int* v = s_ver;
+                            v[I] = R + 1;
+                            v[J] = R + 1;
+                        }
+                    }
                 }
-                __syncthreads();  // the next round regroups the columns
+                if (!flow) __syncthreads();  // the next round regroups the columns
             }
             if (lane == 0 && my_rot) atomicOr(&s_rot, 1);
             __syncthreads();
