@@ -19,8 +19,11 @@
 namespace smb {
 
 constexpr int BJ_B = 16;       // columns per block
-constexpr int BJ_WARPS = 8;    // warps per CTA
+constexpr int BJ_WARPS = 7;    // warps per CTA
 constexpr int BJ_LDM = 33;     // leading dimension of the 32 x 32 matrices in shared memory (conflict-free both ways)
+constexpr int BJ_LDW = 36;     // leading dimension of W (FP64): = 4 mod 16, so that the column rotations AND the reads
+                               // of its B fragments in the update are free of bank conflicts
+constexpr int BJ_PERW = 32 * BJ_LDW + 32 + 32 + 16 + 16 + 32 * BJ_LDM / 2 + 1;  // doubles of shared memory per warp
 constexpr int BJ_MAXN = 1024;  // blocks per submatrix with barrier-free rounds (n <= 16384)
 constexpr int BJ_INNER = 1;    // sweeps of the 32 x 32 Jacobi per visit (the outer sweeps finish the job)
 
@@ -55,12 +58,12 @@ __device__ __forceinline__ void bj_dmma(double (&c)[2], double a, double b) {
 // inner product, which the next visit removes) and the cosine by an FP32 seed and two FP64 Newton steps, so that
 // c^2 + s^2 = 1 to FP64 rounding and W stays orthogonal -- ~25 instructions instead of FP64 division, square root
 // and reciprocal square root on the critical path of every round.
-__device__ __forceinline__ void bj_rotation(double app, double aqq, double apq, double& c, double& s) {
+__device__ __forceinline__ void bj_rotation(double app, double aqq, double apq, double& c, double& s, double& t) {
     const float zf = __fdividef((float)(aqq - app), 2.0f * (float)apq);
     const float az = fabsf(zf);
     float tf = az < 1e15f ? __frcp_rn(az + __fsqrt_rn(fmaf(az, az, 1.0f))) : __fdividef(0.5f, az);
     tf = zf >= 0.0f ? tf : -tf;
-    const double t = (double)tf;
+    t = (double)tf;
     const double x = fma(t, t, 1.0);
     double y = (double)rsqrtf((float)x);
     y = y * fma(-0.5 * x, y * y, 1.5);
@@ -70,9 +73,16 @@ __device__ __forceinline__ void bj_rotation(double app, double aqq, double apq, 
 }
 
 // One visit of the block pair (I, J) of the n x n matrix Gm (column-major, column stride ld) by one warp.
-// M, W: this warp's 32 x 33 shared arrays; cs: 32 doubles, pq: 32 ints of shared scratch.  Returns 1 if it rotated.
-__device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, int nblk, double* __restrict__ M,
-                        double* __restrict__ W, double* __restrict__ cs, int* __restrict__ pq, double tol2, int lane) {
+// W (FP64), M (FP32: off-diagonal elements of the Gram matrix), dg (FP64: its diagonal): this warp's 32 x 33 shared
+// arrays; cs: 32 doubles, pq: 32 ints of shared scratch.  Returns 1 if it rotated.
+// Only the ANGLES come from M, so its off-diagonal elements need relative accuracy only (FP32: the rotated pair is
+// orthogonal to 1e-7 of its former inner product, removed by the next visit, whose Gram matrix is formed afresh in
+// FP64); the diagonal stays FP64 because zeta = (M_qq - M_pp) / (2 M_pq) takes a difference of nearly equal numbers
+// for close eigenvalues.  W and the columns of G never see FP32.
+__device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, int nblk, float* __restrict__ M,
+                        double* __restrict__ dg, double* __restrict__ W, double* __restrict__ cs,
+                        int* __restrict__ pq, double tol2, int lane) {
+    float* csf = reinterpret_cast<float*>(pq + 32);  // [32] (c, s) once more as floats, for the update of M
     const int lr = lane >> 2, lk = lane & 3;
     // global column of slot k of the pair (or -1): slots 0..15 block I, 16..31 block J
     auto colof = [&](int k) {
@@ -100,17 +110,18 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
 #pragma unroll
             for (int b = 0; b <= a; ++b, ++e) bj_dmma(acc[e], f[a], f[b]);
     }
-    {   // accumulator (row lr, columns 2 lk, 2 lk + 1 of sub-tile (a, b)) -> M and its mirror
+    {   // accumulator (row lr, columns 2 lk, 2 lk + 1 of sub-tile (a, b)) -> M and its mirror, diagonal -> dg
         int e = 0;
 #pragma unroll
         for (int a = 0; a < 4; ++a)
 #pragma unroll
             for (int b = 0; b <= a; ++b, ++e) {
                 const int r = 8 * a + lr, c0 = 8 * b + 2 * lk;
-                M[r * BJ_LDM + c0] = acc[e][0];
-                M[r * BJ_LDM + c0 + 1] = acc[e][1];
-                M[c0 * BJ_LDM + r] = acc[e][0];
-                M[(c0 + 1) * BJ_LDM + r] = acc[e][1];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    if (r == c0 + h) dg[r] = acc[e][h];
+                    else { M[r * BJ_LDM + c0 + h] = (float)acc[e][h]; M[(c0 + h) * BJ_LDM + r] = (float)acc[e][h]; }
+                }
             }
     }
     __syncwarp();
@@ -118,9 +129,9 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
     // sweep is enough when it is small already (the sweep squares it)
     double rmax2 = 0.0;
     {
-        const double dl = M[lane * BJ_LDM + lane];
+        const double dl = dg[lane];
         for (int k = 0; k < lane; ++k) {
-            const double v = M[lane * BJ_LDM + k], dk = M[k * BJ_LDM + k];
+            const double v = (double)M[lane * BJ_LDM + k], dk = dg[k];
             const double den = dl * dk;
             if (den > 0.0) rmax2 = fmax(rmax2, v * v / den);
         }
@@ -129,7 +140,7 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
     }
     if (!(rmax2 > tol2)) return 0;
     const int inner = rmax2 > 1e-12 ? BJ_INNER : 1;
-    for (int k = 0; k < 32; ++k) W[lane * BJ_LDM + k] = (k == lane) ? 1.0 : 0.0;
+    for (int k = 0; k < 32; ++k) W[lane * BJ_LDW + k] = (k == lane) ? 1.0 : 0.0;
     __syncwarp();
     // ---- 2. cyclic Jacobi on M (32 x 32), W accumulates the rotations
     int rotated_any = 0;
@@ -142,10 +153,17 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
             if (lane < 16) {
                 p = lane == 0 ? 31 : (rd + lane) % 31;
                 q = lane == 0 ? rd : (rd - lane + 31) % 31;
-                const double app = M[p * BJ_LDM + p], aqq = M[q * BJ_LDM + q], apq = M[p * BJ_LDM + q];
-                if (apq * apq > tol2 * app * aqq) bj_rotation(app, aqq, apq, c, s);
+                const double app = dg[p], aqq = dg[q], apq = (double)M[p * BJ_LDM + q];
+                if (apq * apq > tol2 * app * aqq) {
+                    double t;
+                    bj_rotation(app, aqq, apq, c, s, t);
+                    dg[p] = app - t * apq;  // the rotated diagonal in closed form
+                    dg[q] = aqq + t * apq;
+                }
                 cs[2 * lane] = c;
                 cs[2 * lane + 1] = s;
+                csf[2 * lane] = (float)c;
+                csf[2 * lane + 1] = (float)s;
                 pq[2 * lane] = p;
                 pq[2 * lane + 1] = q;
             }
@@ -160,7 +178,8 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
                 const int k = lane & 15, hh = lane >> 4, h16 = hh * 16;
                 const double ck = cs[2 * k], sk = cs[2 * k + 1];
                 const int pk = pq[2 * k], qk = pq[2 * k + 1];
-                double b00[8], b01[8], b10[8], b11[8];
+                const float ckf = csf[2 * k], skf = csf[2 * k + 1];
+                float b00[8], b01[8], b10[8], b11[8];
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
                     const int p2 = pq[2 * (8 * hh + j)], q2 = pq[2 * (8 * hh + j) + 1];
@@ -171,24 +190,30 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
                 }
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
-                    const double c2 = cs[2 * (8 * hh + j)], s2 = cs[2 * (8 * hh + j) + 1];
-                    if (sk == 0.0 && s2 == 0.0) continue;
-                    const int p2 = pq[2 * (8 * hh + j)], q2 = pq[2 * (8 * hh + j) + 1];
-                    const double t00 = c2 * b00[j] - s2 * b01[j], t01 = s2 * b00[j] + c2 * b01[j];
-                    const double t10 = c2 * b10[j] - s2 * b11[j], t11 = s2 * b10[j] + c2 * b11[j];
-                    M[pk * BJ_LDM + p2] = ck * t00 - sk * t10;
-                    M[pk * BJ_LDM + q2] = ck * t01 - sk * t11;
-                    M[qk * BJ_LDM + p2] = sk * t00 + ck * t10;
-                    M[qk * BJ_LDM + q2] = sk * t01 + ck * t11;
+                    const int k2 = 8 * hh + j;
+                    const float c2 = csf[2 * k2], s2 = csf[2 * k2 + 1];
+                    if (skf == 0.f && s2 == 0.f) continue;
+                    const int p2 = pq[2 * k2], q2 = pq[2 * k2 + 1];
+                    if (k2 == k) {  // the pair's own block: diagonal done in closed form, its off-diagonal element vanishes
+                        M[pk * BJ_LDM + qk] = 0.f;
+                        M[qk * BJ_LDM + pk] = 0.f;
+                        continue;
+                    }
+                    const float t00 = c2 * b00[j] - s2 * b01[j], t01 = s2 * b00[j] + c2 * b01[j];
+                    const float t10 = c2 * b10[j] - s2 * b11[j], t11 = s2 * b10[j] + c2 * b11[j];
+                    M[pk * BJ_LDM + p2] = ckf * t00 - skf * t10;
+                    M[pk * BJ_LDM + q2] = ckf * t01 - skf * t11;
+                    M[qk * BJ_LDM + p2] = skf * t00 + ckf * t10;
+                    M[qk * BJ_LDM + q2] = skf * t01 + ckf * t11;
                 }
                 if (sk != 0.0) {  // columns p, q of W
                     double x[16], y[16];
 #pragma unroll
-                    for (int r = 0; r < 16; ++r) { x[r] = W[(h16 + r) * BJ_LDM + pk]; y[r] = W[(h16 + r) * BJ_LDM + qk]; }
+                    for (int r = 0; r < 16; ++r) { x[r] = W[(h16 + r) * BJ_LDW + pk]; y[r] = W[(h16 + r) * BJ_LDW + qk]; }
 #pragma unroll
                     for (int r = 0; r < 16; ++r) {
-                        W[(h16 + r) * BJ_LDM + pk] = ck * x[r] - sk * y[r];
-                        W[(h16 + r) * BJ_LDM + qk] = sk * x[r] + ck * y[r];
+                        W[(h16 + r) * BJ_LDW + pk] = ck * x[r] - sk * y[r];
+                        W[(h16 + r) * BJ_LDW + qk] = sk * x[r] + ck * y[r];
                     }
                 }
             }
@@ -198,17 +223,15 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
         if (!rotated_sw) break;
     }
     if (!rotated_any) return 0;
-    // ---- 3. [G_I G_J] <- [G_I G_J] W: B fragments of W (k-step t = rows 4 t .. 4 t + 3, sub-tile column d) in registers
-    double wf[8][4];
-#pragma unroll
-    for (int t = 0; t < 8; ++t)
-#pragma unroll
-        for (int d = 0; d < 4; ++d) wf[t][d] = W[(4 * t + lk) * BJ_LDM + 8 * d + lr];
+    // ---- 3. [G_I G_J] <- [G_I G_J] W by DMMA, 8-row strips in place.  The B fragments of W (k-step t = rows
+    // 4 t .. 4 t + 3, sub-tile column d) are read from shared memory for every strip (conflict-free with BJ_LDW):
+    // holding all 32 of them in registers costs 64 registers and the second CTA per SM.
     int cola[8], colc[4][2];
 #pragma unroll
     for (int t = 0; t < 8; ++t) cola[t] = colof(4 * t + lk);
 #pragma unroll
     for (int d = 0; d < 4; ++d) { colc[d][0] = colof(8 * d + 2 * lk); colc[d][1] = colof(8 * d + 2 * lk + 1); }
+    const unsigned wbase = (unsigned)__cvta_generic_to_shared(W + lk * BJ_LDW + lr);
     const int strips = ld >> 3;
 #pragma unroll 2
     for (int rs = 0; rs < strips; ++rs) {
@@ -222,7 +245,11 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
 #pragma unroll
         for (int t = 0; t < 8; ++t)
 #pragma unroll
-            for (int d = 0; d < 4; ++d) bj_dmma(c4[d], af[t], wf[t][d]);
+            for (int d = 0; d < 4; ++d) {
+                double wv;  // volatile: keeps the loads inside the strip loop
+                asm volatile("ld.shared.f64 %0, [%1];" : "=d"(wv) : "r"(wbase + (unsigned)((4 * t * BJ_LDW + 8 * d) * 8)));
+                bj_dmma(c4[d], af[t], wv);
+            }
 #pragma unroll
         for (int d = 0; d < 4; ++d) {
             if (colc[d][0] >= 0) Gm[(size_t)colc[d][0] * ld + row] = c4[d][0];
@@ -232,17 +259,17 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
     return 1;
 }
 
-__global__ void __launch_bounds__(BJ_WARPS * 32, 1) k_eig_bjacobi(const BjArgs A) {
-    extern __shared__ __align__(16) double bsm[];  // per warp: M[32 x 33], W[32 x 33], cs[32], pq[32 ints]
+__global__ void __launch_bounds__(BJ_WARPS * 32, 2) k_eig_bjacobi(const BjArgs A) {
+    extern __shared__ __align__(16) double bsm[];  // per warp: W[32 x 33], dg[32], cs[32], pq[32 ints], M[32 x 33 floats]
     __shared__ int s_next, s_rot;
     __shared__ int s_ver[BJ_MAXN];
     __shared__ int s_genrow[1024];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    constexpr int PERW = 2 * 32 * BJ_LDM + 32 + 16;
-    double* M = bsm + (size_t)wid * PERW;
-    double* W = M + 32 * BJ_LDM;
-    double* cs = W + 32 * BJ_LDM;
-    int* pq = reinterpret_cast<int*>(cs + 32);
+    double* W = bsm + (size_t)wid * BJ_PERW;          // [32 x 33] doubles
+    double* dg = W + 32 * BJ_LDW;                       // [32] diagonal of the Gram matrix
+    double* cs = dg + 32;                               // [32] (c, s) of the 16 pairs of a round
+    int* pq = reinterpret_cast<int*>(cs + 32);          // [32] (p, q) of the 16 pairs
+    float* M = reinterpret_cast<float*>(pq + 64);       // [32 x 33] floats (pq + 32: the float copies of (c, s))
     for (;;) {
         if (threadIdx.x == 0) s_next = atomicAdd(A.counter, 1);
         __syncthreads();
@@ -282,7 +309,7 @@ __global__ void __launch_bounds__(BJ_WARPS * 32, 1) k_eig_bjacobi(const BjArgs A
                         __syncwarp();
                         __threadfence_block();
                     }
-                    if (I < nblk) my_rot |= bj_visit(Gm, n, ld, I, J, nblk, M, W, cs, pq, tol2, lane);
+                    if (I < nblk) my_rot |= bj_visit(Gm, n, ld, I, J, nblk, M, dg, W, cs, pq, tol2, lane);
                     if (flow) {
                         __threadfence_block();
                         __syncwarp();
@@ -340,7 +367,7 @@ __global__ void __launch_bounds__(BJ_WARPS * 32, 1) k_eig_bjacobi(const BjArgs A
 
 sm_status_t launch_eig_bjacobi(sm_plan* p, double* G, cudaStream_t st) {
     const int ng = p->ngroups;
-    constexpr size_t smem = (size_t)BJ_WARPS * (2 * 32 * BJ_LDM + 32 + 16) * sizeof(double);
+    constexpr size_t smem = (size_t)BJ_WARPS * BJ_PERW * sizeof(double);
     if (!p->eig_battr_set) {
         SM_CUDA(cudaFuncSetAttribute(k_eig_bjacobi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         p->eig_battr_set = 1;
@@ -351,7 +378,7 @@ sm_status_t launch_eig_bjacobi(sm_plan* p, double* G, cudaStream_t st) {
     a.grp_ptr = p->d_grp_ptr; a.grp_cols = p->d_grp_cols; a.gen_off = p->d_gen_off; a.blk_size = p->d_blk_size;
     a.eig_ptr = p->d_eig_ptr; a.lam = p->d_eig_lam; a.w = p->d_eig_w;
     a.ngroups = ng; a.max_sweeps = 30;
-    k_eig_bjacobi<<<std::min(ng, p->num_sms), BJ_WARPS * 32, smem, st>>>(a);
+    k_eig_bjacobi<<<std::min(ng, 2 * p->num_sms), BJ_WARPS * 32, smem, st>>>(a);
     p->launches++;
     SM_CUDA(cudaGetLastError());
     return SM_OK;
