@@ -81,7 +81,7 @@ __device__ __forceinline__ void bj_rotation(double app, double aqq, double apq, 
 // for close eigenvalues.  W and the columns of G never see FP32.
 __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, int nblk, float* __restrict__ M,
                         double* __restrict__ dg, double* __restrict__ W, double* __restrict__ cs,
-                        int* __restrict__ pq, double tol2, int lane) {
+                        int* __restrict__ pq, double tol2, int lane, bool full) {
     float* csf = reinterpret_cast<float*>(pq + 32);  // [32] (c, s) once more as floats, for the update of M
     const int lr = lane >> 2, lk = lane & 3;
     // global column of slot k of the pair (or -1): slots 0..15 block I, 16..31 block J
@@ -130,7 +130,8 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
     double rmax2 = 0.0;
     {
         const double dl = dg[lane];
-        for (int k = 0; k < lane; ++k) {
+        const int kend = full ? lane : (lane >= 16 ? 16 : 0);  // cross-only visit: the elements (J slot, I slot) alone
+        for (int k = 0; k < kend; ++k) {
             const double v = (double)M[lane * BJ_LDM + k], dk = dg[k];
             const double den = dl * dk;
             if (den > 0.0) rmax2 = fmax(rmax2, v * v / den);
@@ -146,13 +147,18 @@ __device__ int bj_visit(double* __restrict__ Gm, int n, int ld, int I, int J, in
     int rotated_any = 0;
     for (int sw = 0; sw < inner; ++sw) {
         int rotated_sw = 0;
-        for (int rd = 0; rd < 31; ++rd) {
+        for (int rd = 0; rd < (full ? 31 : 16); ++rd) {
             // pair of lane k < 16: round-robin tournament of 32 players
             int p = 0, q = 0;
             double c = 1.0, s = 0.0;
             if (lane < 16) {
-                p = lane == 0 ? 31 : (rd + lane) % 31;
-                q = lane == 0 ? rd : (rd - lane + 31) % 31;
+                if (full) {
+                    p = lane == 0 ? 31 : (rd + lane) % 31;
+                    q = lane == 0 ? rd : (rd - lane + 31) % 31;
+                } else {  // the 256 cross pairs (slot of I, slot of J) in 16 rounds
+                    p = lane;
+                    q = 16 + ((lane + rd) & 15);
+                }
                 const double app = dg[p], aqq = dg[q], apq = (double)M[p * BJ_LDM + q];
                 if (apq * apq > tol2 * app * aqq) {
                     double t;
@@ -309,7 +315,7 @@ __global__ void __launch_bounds__(BJ_WARPS * 32, 2) k_eig_bjacobi(const BjArgs A
                         __syncwarp();
                         __threadfence_block();
                     }
-                    if (I < nblk) my_rot |= bj_visit(Gm, n, ld, I, J, nblk, M, dg, W, cs, pq, tol2, lane);
+                    if (I < nblk) my_rot |= bj_visit(Gm, n, ld, I, J, nblk, M, dg, W, cs, pq, tol2, lane, r == 0);
                     if (flow) {
                         __threadfence_block();
                         __syncwarp();
