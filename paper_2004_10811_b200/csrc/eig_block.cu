@@ -6,13 +6,16 @@
 // and a visit is three dense steps instead of 256 separate plane rotations of full-length columns:
 //   1. Gram matrix M = [G_I G_J]^T [G_I G_J] (32 x 32) by DMMA straight from global memory (L2-resident matrix):
 //      four column fragments per step of four rows feed the ten sub-tiles on or below the diagonal;
-//   2. M = W D W^T by a cyclic two-sided Jacobi on the 32 x 32 matrix in shared memory (one warp, 16 disjoint
-//      rotations per round, one sweep of 31 rounds per visit, angles from M alone: rotating columns p, q of G is the congruence J^T M J on its Gram
-//      matrix, so this IS the sequence of plane rotations of the one-sided method, applied to M instead of G);
-//   3. [G_I G_J] <- [G_I G_J] W by DMMA, W held in registers as B fragments, one 8-row strip at a time, in place.
+//   2. plane rotations on M in shared memory (one warp, 16 disjoint rotations per round, angles from M alone:
+//      rotating columns p, q of G is the congruence J^T M J on its Gram matrix, so these ARE the plane rotations of
+//      the one-sided method, applied to M instead of G), accumulated in W.  M: off-diagonal elements FP32, diagonal
+//      FP64 (see bj_visit).  In the first tournament round of a sweep a visit runs all 496 pairs of its 32 columns
+//      (31 rounds; every block is in exactly one pair of that round, so pairs inside a block are covered once per
+//      sweep), afterwards only the 256 cross pairs (16 rounds);
+//   3. [G_I G_J] <- [G_I G_J] W by DMMA, one 8-row strip at a time, in place, B fragments of W from shared memory.
 // One warp owns a block pair; the pairs of a tournament round are disjoint, so the warps of a CTA work on different
-// pairs of the same submatrix and meet at a CTA barrier per round.  Pairs inside a block are covered by every visit
-// of that block (the 32 x 32 problem contains them), so there are no separate diagonal visits.
+// pairs of the same submatrix.  Rounds are not separated by CTA barriers: every block counts the rounds it has been
+// through and a warp waits for its two blocks alone.  Two CTAs (two submatrices) per SM.
 // A visit whose Gram matrix is already diagonal to the tolerance changes nothing; a sweep of such visits ends it.
 #include "common.cuh"
 
@@ -25,7 +28,7 @@ constexpr int BJ_LDW = 36;     // leading dimension of W (FP64): = 4 mod 16, so 
                                // of its B fragments in the update are free of bank conflicts
 constexpr int BJ_PERW = 32 * BJ_LDW + 32 + 32 + 16 + 16 + 32 * BJ_LDM / 2 + 1;  // doubles of shared memory per warp
 constexpr int BJ_MAXN = 1024;  // blocks per submatrix with barrier-free rounds (n <= 16384)
-constexpr int BJ_INNER = 1;    // sweeps of the 32 x 32 Jacobi per visit (the outer sweeps finish the job)
+constexpr int BJ_INNER = 1;    // passes over a visit's pair schedule (the outer sweeps finish the job)
 
 struct BjArgs {
     const int32_t* sub_dim;
