@@ -333,6 +333,26 @@ sm_status_t sm_trace_dk(sm_plan_t* plan, const double* d_D, const double* d_K, d
                         double* tr_DK, void* cuda_stream);
 
 /*
+ * sm_trace_dk_static -- the band-structure energy tr(D K) (Eq.(10)) = sum over stored elements D o K, for
+ * callers that must not allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  No plan; calls no cudaMalloc / cudaFree / allocating routine, and no synchronisation: everything is
+ * enqueued on `cuda_stream`.
+ *   nnz      number of stored values, 0 <= nnz <= SM_STATIC_MAX_NNZ; more is rejected with SM_ERR_INVALID_ARG
+ *            (text in sm_last_cuda_error); use sm_trace_dk there.
+ *   d_D, d_K DEVICE [nnz], read only (may be NULL if nnz == 0);  d_tr_DK DEVICE [1], written on the stream.
+ * Scratch: a file-scope __device__ array of 512 KB + 256 B inside the library (one partial sum per 4096 values
+ * and a ticket counter), held by every GPU that loads the library until the process exits.  ALL calls share it
+ * and it keeps the last call's contents (the call clears what must start at zero): calls on one stream are
+ * ordered and safe; calls whose kernels overlap on the GPU (other streams / threads) RACE -- serialise them.
+ * The first call on a device resolves the array's device address (cudaGetSymbolAddress, that device current);
+ * make that first call outside a graph capture.  Deterministic (fixed summation order, independent of the grid).
+ * Errors: SM_ERR_INVALID_ARG (negative / too large nnz, NULL pointer), SM_ERR_CUDA.
+ */
+#define SM_STATIC_MAX_NNZ 268435456LL
+sm_status_t sm_trace_dk_static(int64_t nnz, const double* d_D, const double* d_K, double* d_tr_DK,
+                               void* cuda_stream);
+
+/*
  * Phase entry points used by the tests and the roofline benchmark (same kernels as above):
  *   sm_gather   : workspace X buffer <- a_i - mu I (rows / columns n_i .. ld_i - 1 zero: a fixed point of
  *                 the iteration); also the Gershgorin bounds (plain Gershgorin scaling, whatever the

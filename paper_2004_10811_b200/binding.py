@@ -28,7 +28,7 @@ EXPORTS = [
     "sm_density_matrix", "sm_density_matrix_host", "sm_trace_dk", "sm_gather", "sm_sign_iterate",
     "sm_scatter", "sm_set_timing", "sm_launch_count", "sm_plan_destroy", "sm_strerror",
     "sm_last_cuda_error", "sm_measure_peaks", "sm_eig_decompose", "sm_eig_export", "sm_eig_nelec", "sm_eig_density",
-    "sm_partition_groups", "sm_plan_set_allreduce",
+    "sm_partition_groups", "sm_plan_set_allreduce", "sm_trace_dk_static",
 ]
 
 
@@ -114,6 +114,7 @@ def lib() -> C.CDLL:
                                         C.POINTER(sm_stats_t), vp]
         L.sm_density_matrix_host.argtypes = L.sm_density_matrix.argtypes
         L.sm_trace_dk.argtypes = [vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), vp]
+        L.sm_trace_dk_static.argtypes = [C.c_int64, vp, vp, vp, vp]
         L.sm_gather.argtypes = [vp, vp, dbl, vp, C.c_size_t, vp]
         L.sm_sign_iterate.argtypes = [vp, dbl, vp, C.c_size_t, C.POINTER(sm_stats_t), vp]
         L.sm_scatter.argtypes = [vp, i32, vp, vp, C.c_size_t, vp]
@@ -247,6 +248,14 @@ def sm_trace_dk(plan, d_D, d_K, stream=None):
     td, tdk = C.c_double(0), C.c_double(0)
     _check(lib().sm_trace_dk(plan, _dev_ptr(d_D), _dev_ptr(d_K), C.byref(td), C.byref(tdk), _stream_ptr(stream)))
     return td.value, tdk.value
+
+
+SM_STATIC_MAX_NNZ = 268435456
+
+
+def sm_trace_dk_static(nnz, d_D, d_K, d_out, stream=None) -> int:
+    """tr(D K) into the device double d_out[0]; allocates nothing, does not synchronise (include/submatrix.h)."""
+    return _check(lib().sm_trace_dk_static(int(nnz), _dev_ptr(d_D), _dev_ptr(d_K), _dev_ptr(d_out), _stream_ptr(stream)))
 
 
 def sm_gather(plan, d_vals_in, mu, d_workspace, stream=None) -> int:

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsubmatrix_b200.so")
-SOURCES = ["api.cu", "plan.cu", "gather_scatter.cu", "ns_sign.cu", "spectral.cu", "ns_tf32.cu", "peaks.cu", "eig.cu", "eig_block.cu"]
+SOURCES = ["api.cu", "plan.cu", "gather_scatter.cu", "ns_sign.cu", "spectral.cu", "ns_tf32.cu", "peaks.cu", "eig.cu", "eig_block.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 

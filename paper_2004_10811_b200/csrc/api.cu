@@ -17,6 +17,9 @@ void set_cuda_error(cudaError_t e, const char* where) {
     snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
     cudaGetLastError();  // clear the sticky-less error state
 }
+// A message of the library's own (argument errors that deserve more than a status code): read back through
+// sm_last_cuda_error like the CUDA ones.
+void set_error_text(const char* msg) { snprintf(g_cuda_err, sizeof(g_cuda_err), "%s", msg); }
 }  // namespace smb
 
 using namespace smb;

@@ -40,6 +40,7 @@ __host__ __device__ __forceinline__ size_t panel_off(int r, int c, int ld) {
 }
 
 void set_cuda_error(cudaError_t e, const char* where);
+void set_error_text(const char* msg);
 
 // Frees a temporary device buffer on every return path.
 struct DevTmp {
