@@ -239,7 +239,8 @@ def run_phases(args, m, B, torch):
     B.sm_plan_destroy(plan)
     del ws
     out["reduced_precision"] = {}
-    for prec, name, eps in ((2, "3xTF32 (hi/lo split)", 2e-6), (3, "BF16x2 (hi/lo split)", 1e-5), (1, "TF32", 1e-5)):
+    for prec, name, eps in ((2, "3xTF32 (hi/lo split)", 2e-6), (4, "FP16x2 (hi/lo split)", 2e-6),
+                            (3, "BF16x2 (hi/lo split)", 1e-5), (1, "TF32", 1e-5)):
         plan = B.plan_from_matrix(m, B.default_options(precision=prec))
         ws = B.alloc_workspace(plan)
         B.sm_set_timing(plan, True)
@@ -336,10 +337,11 @@ def run_extras(args, m, B, torch, plan, info, ws, d_in, d_out, mu, hbm_peak):
                                                  "abs_g": abs(st.n_elec - n_target), "mu": mu_g, "ms": e0.elapsed_time(e1)}
     B.sm_plan_destroy(plan4)
 
-    # opt-in reduced precision (tcgen05: 3xTF32, and the BF16x2 rung) on the same input at the accepted mu, against
+    # opt-in reduced precision (tcgen05: 3xTF32 and the 16-bit split rungs FP16x2 / BF16x2) on the same input at the accepted mu, against
     # the FP64 result
     _, tdk64 = B.sm_trace_dk(plan, d_out, d_in)
-    for prec, key, eps_r in ((2, "reduced_precision_3xTF32", 2e-6), (3, "reduced_precision_BF16x2", 1e-5)):
+    for prec, key, eps_r in ((2, "reduced_precision_3xTF32", 2e-6), (4, "reduced_precision_FP16x2", 2e-6),
+                             (3, "reduced_precision_BF16x2", 1e-5)):
         plan3 = B.plan_from_matrix(m, B.default_options(precision=prec))
         need = B.sm_plan_query(plan3).workspace_bytes
         ws3 = ws if need <= ws.numel() * 8 else B.alloc_workspace(plan3)

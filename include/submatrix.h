@@ -76,6 +76,9 @@ typedef struct {
                          /*     bits, 4 bytes per element), products hi hi + hi lo + lo hi   */
                          /*     on kind::f16: the rung between the two others -- error 1e-5  */
                          /*     class at half the FP64 time or less (half the operand bytes)  */
+                         /* 4 = "FP16x2": as 3 with hi + lo FP16 pairs (22 mantissa bits):    */
+                         /*     the accuracy of 2 (1e-6 class) at the cost of 3 -- the rung   */
+                         /*     to prefer on this part                                        */
                          /* 1 = FP32 storage, plain TF32 products: experimental, error 5e-4   */
                          /*     ... 2e-3, does NOT meet the 1e-3 bar in general and its      */
                          /*     n_elec is too coarse to steer the mu search on large systems */

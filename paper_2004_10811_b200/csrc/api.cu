@@ -164,7 +164,7 @@ sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_si
         if (p->opt.precision != 0) return SM_ERR_INVALID_ARG;
         p->opt.overshoot = 1.0;  // Eq.(19)'s map is increasing beyond 1: eigenvalues of X0 must not exceed 1
     }
-    if (p->opt.precision < 0 || p->opt.precision > 3 || p->opt.scaling < 0 || p->opt.scaling > 1) return SM_ERR_INVALID_ARG;
+    if (p->opt.precision < 0 || p->opt.precision > 4 || p->opt.scaling < 0 || p->opt.scaling > 1) return SM_ERR_INVALID_ARG;
     if (p->opt.method < 0 || p->opt.method > 1 || !(p->opt.kT >= 0.0)) return SM_ERR_INVALID_ARG;
     if (p->opt.method == 1 && (p->opt.precision != 0 || p->opt.order != 2)) return SM_ERR_INVALID_ARG;
     p->nb = nb; p->ngroups = ngroups; p->nnzb = nb ? colptr[nb] : 0;

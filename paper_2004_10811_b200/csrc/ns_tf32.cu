@@ -33,6 +33,7 @@
 #include <algorithm>
 
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include "common.cuh"
 
@@ -115,9 +116,10 @@ __device__ __forceinline__ void r_mma(uint32_t tmem_d, uint64_t da, uint64_t db,
         "}\n" ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
         : "memory");
 }
-// kind::f16 with BF16 operands: A = B = BF16 ([7,10) = [10,13) = 1), K = 16 per instruction (32 bytes, as TF32's 8).
-__device__ __forceinline__ uint32_t r_idesc_bf16(int n_cols) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(n_cols >> 3) << 17) | ((unsigned)(R_BM >> 4) << 24);
+// kind::f16: A and B formats in [7,10) and [10,13): 1 = BF16, 0 = FP16; K = 16 per instruction (32 bytes, as TF32's 8).
+__device__ __forceinline__ uint32_t r_idesc_bf16(int n_cols, bool fp16 = false) {
+    const unsigned fmt = fp16 ? 0u : 1u;
+    return (1u << 4) | (fmt << 7) | (fmt << 10) | ((unsigned)(n_cols >> 3) << 17) | ((unsigned)(R_BM >> 4) << 24);
 }
 __device__ __forceinline__ void r_mma_bf16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
@@ -160,6 +162,27 @@ __device__ __forceinline__ void bf_split(float x, unsigned short& hi, unsigned s
     lo = __bfloat16_as_ushort(l);
 }
 __device__ __forceinline__ float bf_val(unsigned short b) { return __uint_as_float((unsigned)b << 16); }
+// The same pair of 16-bit planes in either format.  H16: hi = fp16(x), lo = fp16(x - hi): 22 mantissa bits for
+// |x| >= 2^-3 (lo becomes subnormal below that: absolute resolution 2^-25), range 65504 -- enough here, the
+// iterates have eigenvalues in [-1, 1] and Y = al^2 X^2 <= 2.25.
+template <bool H16>
+__device__ __forceinline__ void s16_split(float x, unsigned short& hi, unsigned short& lo) {
+    if (H16) {
+        const __half h = __float2half_rn(x);
+        hi = __half_as_ushort(h);
+        lo = __half_as_ushort(__float2half_rn(x - __half2float(h)));
+    } else {
+        bf_split(x, hi, lo);
+    }
+}
+template <bool H16>
+__device__ __forceinline__ float s16_val(unsigned short b) {
+    return H16 ? __half2float(__ushort_as_half(b)) : bf_val(b);
+}
+template <bool H16>
+__device__ __forceinline__ unsigned short s16_bits(float exact) {  // exact: a value that IS representable
+    return H16 ? __half_as_ushort(__float2half_rn(exact)) : (unsigned short)(__float_as_uint(exact) >> 16);
+}
 __device__ __forceinline__ unsigned bf_pack2(unsigned short a, unsigned short b) { return (unsigned)a | ((unsigned)b << 16); }
 
 // One work unit of the reduced-precision GEMMs.
@@ -241,6 +264,7 @@ k_to_f64(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __rest
 }
 
 // precision = 3: FP64 k8-panel a_i - mu I  ->  BF16 hi / lo planes (k8-panel/128, 2-byte elements) of X0.
+template <bool H16>
 __global__ void __launch_bounds__(256)
 k_to_bf16(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __restrict__ ldv,
           const int64_t* __restrict__ ws_off, const int64_t* __restrict__ ws_off32,
@@ -263,9 +287,9 @@ k_to_bf16(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __res
         for (int j = 0; j < 8; ++j) {
             const int c = 8 * kc + j;
             const double x = (r < n && c < n) ? src[panel_off(r, c, ld)] * inv : 0.0;
-            const __nv_bfloat16 h = __float2bfloat16_rn((float)x);
-            hi[j] = __bfloat16_as_ushort(h);
-            lo[j] = __bfloat16_as_ushort(__float2bfloat16_rn((float)(x - (double)__bfloat162float(h))));
+            unsigned short d0;
+            s16_split<H16>((float)x, hi[j], d0);
+            s16_split<H16>((float)(x - (double)s16_val<H16>(hi[j])), lo[j], d0);  // lo: the FP64 remainder, rounded
         }
         unsigned short* d = dst + panel16_off(r, 8 * kc, ldp);
         *reinterpret_cast<uint4*>(d) = make_uint4(bf_pack2(hi[0], hi[1]), bf_pack2(hi[2], hi[3]), bf_pack2(hi[4], hi[5]), bf_pack2(hi[6], hi[7]));
@@ -274,6 +298,7 @@ k_to_bf16(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __res
 }
 
 // precision = 3: BF16 hi + lo result -> FP64 k8-panel buffer (as k_to_f64).
+template <bool H16>
 __global__ void __launch_bounds__(256)
 k_from_bf16(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __restrict__ ldv,
             const int64_t* __restrict__ ws_off, const int64_t* __restrict__ ws_off32,
@@ -296,7 +321,7 @@ k_from_bf16(int ngroups, const int32_t* __restrict__ sub_dim, const int32_t* __r
         double v = 0.0;
         if (r < n && c < n) {
             const size_t o = panel16_off(r, c, ldp);
-            v = ((double)bf_val(src[o]) + (double)bf_val(src[o + lo_plane])) * mul;
+            v = ((double)s16_val<H16>(src[o]) + (double)s16_val<H16>(src[o + lo_plane])) * mul;
         }
         dst[panel_off(r, c, ld)] = v;
     }
@@ -322,7 +347,8 @@ struct Ns32Args {
 //            kind::f16 (K = 16 per instruction), 32-wide k slices (48 KB per stage).
 template <int MODE, int SPLIT>
 __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
-    constexpr bool BF = SPLIT == 2;                 // BF16 hi / lo planes instead of FP32 ones
+    constexpr bool BF = SPLIT >= 2;                 // 16-bit hi / lo planes instead of FP32 ones (2: BF16, 3: FP16)
+    constexpr bool H16 = SPLIT == 3;
     constexpr bool PIPE = SPLIT == 0;               // software-pipelined epilogue (the split variants lack the registers)
     constexpr int CW = BF ? 8 : 4;                  // columns per 16-byte chunk
     constexpr int ES = BF ? 2 : 4;                  // bytes per element
@@ -409,8 +435,8 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                 r_mbar_wait(&s_tempty[buf], tphase[buf] ^ 1);  // epilogue has drained this accumulator
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t d0 = tmem + (uint32_t)(buf * R_BN);
-                const uint32_t id0 = BF ? r_idesc_bf16(rows_b0) : r_idesc(rows_b0);
-                const uint32_t id1 = BF ? r_idesc_bf16(rows_b1 > 0 ? rows_b1 : 16) : r_idesc(rows_b1 > 0 ? rows_b1 : 16);
+                const uint32_t id0 = BF ? r_idesc_bf16(rows_b0, H16) : r_idesc(rows_b0);
+                const uint32_t id1 = BF ? r_idesc_bf16(rows_b1 > 0 ? rows_b1 : 16, H16) : r_idesc(rows_b1 > 0 ? rows_b1 : 16);
                 auto mma = [&](uint32_t d, uint64_t da, uint64_t db, uint32_t id, uint32_t acc) {
                     if (BF) r_mma_bf16(d, da, db, id, acc); else r_mma(d, da, db, id, acc);
                 };
@@ -644,13 +670,13 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                             for (int e = 0; e < 8; ++e) {
                                 const unsigned short hb = (unsigned short)(hw[e >> 1] >> (16 * (e & 1)));
                                 const unsigned short lb = (unsigned short)(lw[e >> 1] >> (16 * (e & 1)));
-                                const float x = bf_val(hb) + bf_val(lb);
+                                const float x = s16_val<H16>(hb) + s16_val<H16>(lb);
                                 w[e] = 1.5f * x - 0.5f * w[e];
                             }
                         }
                         unsigned short hi[8], lo[8];
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) bf_split(w[e], hi[e], lo[e]);
+                        for (int e = 0; e < 8; ++e) s16_split<H16>(w[e], hi[e], lo[e]);
                         if (act) {
                             if (c + 7 <= r) {
                                 *reinterpret_cast<uint4*>(orow16 + o) = make_uint4(bf_pack2(hi[0], hi[1]), bf_pack2(hi[2], hi[3]),
@@ -669,17 +695,17 @@ __global__ void __launch_bounds__(R_THREADS, R_CTAS) k_ns_tf32(Ns32Args a) {
                             const bool blk = row_ok && cc + 3 < rq;
                             float th[4], tl[4];
 #pragma unroll
-                            for (int e = 0; e < 4; ++e) { th[e] = bf_val(hi[4 * q4 + e]); tl[e] = bf_val(lo[4 * q4 + e]); }
+                            for (int e = 0; e < 4; ++e) { th[e] = s16_val<H16>(hi[4 * q4 + e]); tl[e] = s16_val<H16>(lo[4 * q4 + e]); }
                             quad_transpose(th, lane);
                             quad_transpose(tl, lane);
                             if (blk) {
                                 unsigned short* mp = o16 + panel16_off(cc + (lane & 3), rq, ldp);
                                 *reinterpret_cast<uint2*>(mp) =
-                                    make_uint2((__float_as_uint(th[0]) >> 16) | (__float_as_uint(th[1]) & 0xffff0000u),
-                                               (__float_as_uint(th[2]) >> 16) | (__float_as_uint(th[3]) & 0xffff0000u));
+                                    make_uint2(bf_pack2(s16_bits<H16>(th[0]), s16_bits<H16>(th[1])),
+                                               bf_pack2(s16_bits<H16>(th[2]), s16_bits<H16>(th[3])));
                                 *reinterpret_cast<uint2*>(mp + a.lo_plane) =
-                                    make_uint2((__float_as_uint(tl[0]) >> 16) | (__float_as_uint(tl[1]) & 0xffff0000u),
-                                               (__float_as_uint(tl[2]) >> 16) | (__float_as_uint(tl[3]) & 0xffff0000u));
+                                    make_uint2(bf_pack2(s16_bits<H16>(tl[0]), s16_bits<H16>(tl[1])),
+                                               bf_pack2(s16_bits<H16>(tl[2]), s16_bits<H16>(tl[3])));
                             } else if (row_ok) {
 #pragma unroll
                                 for (int e = 0; e < 4; ++e)
@@ -801,9 +827,13 @@ sm_status_t launch_to_f32(sm_plan* p, const double* buf0, double* buf1, cudaStre
     if (p->ngroups == 0) return SM_OK;
     const int split = (int)std::min<int64_t>(8, std::max<int64_t>(1, (int64_t)p->num_sms * 8 / p->ngroups));
     if (p->opt.precision == 3)
-        k_to_bf16<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
-                                                            p->d_gersh, buf0, reinterpret_cast<unsigned short*>(buf1),
-                                                            p->sum_ldp2);
+        k_to_bf16<false><<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off,
+                                                                   p->d_ws_off32, p->d_gersh, buf0,
+                                                                   reinterpret_cast<unsigned short*>(buf1), p->sum_ldp2);
+    else if (p->opt.precision == 4)
+        k_to_bf16<true><<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off,
+                                                                  p->d_ws_off32, p->d_gersh, buf0,
+                                                                  reinterpret_cast<unsigned short*>(buf1), p->sum_ldp2);
     else
         k_to_f32<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
                                                            p->d_gersh, buf0, reinterpret_cast<float*>(buf1),
@@ -817,11 +847,17 @@ sm_status_t launch_to_f64(sm_plan* p, double* buf0, const double* buf1, const do
     if (p->ngroups == 0) return SM_OK;
     const int split = (int)std::min<int64_t>(8, std::max<int64_t>(1, (int64_t)p->num_sms * 8 / p->ngroups));
     if (p->opt.precision == 3)
-        k_from_bf16<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
-                                                              p->d_gersh, p->d_done_iter, p->cur_k,
-                                                              reinterpret_cast<const unsigned short*>(buf1),
-                                                              reinterpret_cast<const unsigned short*>(bufY), buf0,
-                                                              p->sum_ldp2);
+        k_from_bf16<false><<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off,
+                                                                     p->d_ws_off32, p->d_gersh, p->d_done_iter, p->cur_k,
+                                                                     reinterpret_cast<const unsigned short*>(buf1),
+                                                                     reinterpret_cast<const unsigned short*>(bufY), buf0,
+                                                                     p->sum_ldp2);
+    else if (p->opt.precision == 4)
+        k_from_bf16<true><<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off,
+                                                                    p->d_ws_off32, p->d_gersh, p->d_done_iter, p->cur_k,
+                                                                    reinterpret_cast<const unsigned short*>(buf1),
+                                                                    reinterpret_cast<const unsigned short*>(bufY), buf0,
+                                                                    p->sum_ldp2);
     else
         k_to_f64<<<dim3(p->ngroups, split), 256, 0, st>>>(p->ngroups, p->d_sub_dim, p->d_ld, p->d_ws_off, p->d_ws_off32,
                                                            p->d_gersh, p->d_done_iter, p->cur_k,
@@ -843,6 +879,8 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<0, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
+        SM_CUDA(cudaFuncSetAttribute(k_ns_tf32<1, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R_SMEM));
         p->tf32_attr_set = 1;
     }
     float* X[2] = {reinterpret_cast<float*>(buf1), reinterpret_cast<float*>(bufY)};
@@ -850,12 +888,13 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
     Ns32Args a;
     a.tiles = reinterpret_cast<const Tile32*>(p->d_tiles32); a.partials = p->d_partials32; a.done_iter = p->d_done_iter;
     a.n_tiles = (int32_t)p->n_tiles32; a.ctrl = p->d_ctrl;
-    const int split = p->opt.precision == 2 ? 1 : p->opt.precision == 3 ? 2 : 0;
+    const int split = p->opt.precision == 2 ? 1 : p->opt.precision == 3 ? 2 : p->opt.precision == 4 ? 3 : 0;
     a.lo_plane = split ? p->sum_ldp2 : 0;
     const int grid = (int)std::min<int64_t>(p->n_tiles32, (int64_t)p->num_sms * R_CTAS);
     if (which & 1) {
         a.A = X[k & 1]; a.B = X[k & 1]; a.Out = Y;
-        if (split == 2) k_ns_tf32<0, 2><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        if (split == 3) k_ns_tf32<0, 3><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        else if (split == 2) k_ns_tf32<0, 2><<<grid, R_THREADS, R_SMEM, st>>>(a);
         else if (split == 1) k_ns_tf32<0, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
         else k_ns_tf32<0, 0><<<grid, R_THREADS, R_SMEM, st>>>(a);
         k_ns_decide32<<<(p->ngroups + 7) / 8, 256, 0, st>>>(p->ngroups, k, decide_only, eps, 0.5,
@@ -866,7 +905,8 @@ sm_status_t launch_ns_pair_tf32(sm_plan* p, int k, double eps, int decide_only, 
     }
     if ((which & 2) && !decide_only) {
         a.A = X[k & 1]; a.B = Y; a.Out = X[(k + 1) & 1];
-        if (split == 2) k_ns_tf32<1, 2><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        if (split == 3) k_ns_tf32<1, 3><<<grid, R_THREADS, R_SMEM, st>>>(a);
+        else if (split == 2) k_ns_tf32<1, 2><<<grid, R_THREADS, R_SMEM, st>>>(a);
         else if (split == 1) k_ns_tf32<1, 1><<<grid, R_THREADS, R_SMEM, st>>>(a);
         else k_ns_tf32<1, 0><<<grid, R_THREADS, R_SMEM, st>>>(a);
         p->launches += 1;

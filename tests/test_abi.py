@@ -118,7 +118,7 @@ def test_option_validation_is_host_logic():
     assert status(method=2) == B.SM_ERR_INVALID_ARG
     assert status(method=1, kT=-1.0) == B.SM_ERR_INVALID_ARG
     assert status(method=1, precision=2) == B.SM_ERR_INVALID_ARG          # the eigendecomposition path is FP64 only
-    assert status(precision=4) == B.SM_ERR_INVALID_ARG                    # 0 FP64, 1 TF32, 2 3xTF32, 3 BF16x2
+    assert status(precision=5) == B.SM_ERR_INVALID_ARG                    # 0 FP64, 1 TF32, 2 3xTF32, 3 BF16x2, 4 FP16x2
     assert status(precision=-1) == B.SM_ERR_INVALID_ARG
     assert status(shard_rank=2, shard_world=2) == B.SM_ERR_INVALID_ARG
     assert status(shard_rank=0, shard_world=m.ngroups + 1) == B.SM_ERR_INVALID_ARG

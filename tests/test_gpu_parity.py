@@ -614,11 +614,11 @@ def test_third_order_iteration_eq19(B, oracle, cfg0):
 
 
 # ------------------------------------------------------------------------------ reduced precision
-@pytest.mark.parametrize("precision,tol_d,tol_e", [(2, 1e-4, 1e-5), (3, 5e-4, 5e-5), (1, 5e-3, 2e-3)])
+@pytest.mark.parametrize("precision,tol_d,tol_e", [(2, 1e-4, 1e-5), (4, 1e-4, 1e-5), (3, 5e-4, 5e-5), (1, 5e-3, 2e-3)])
 def test_reduced_precision_variants(B, oracle, cfg0, precision, tol_d, tol_e):
     """Opt-in tcgen05 variants (north_star: <= 1e-3 elementwise, energy error reported): precision 2
     ("3xTF32", FP32-class) must be far inside the bar, precision 3 ("BF16x2", 16 mantissa bits) inside it by more
-    than an order, precision 1 (plain TF32) is the ~2e-3 class the survey predicts (A16).  Cases: config 0; dense n = 256 (two B halves, closed form); DZVP blocks with
+    than an order, precision 4 ("FP16x2", 22 mantissa bits) held to the bar of precision 2, precision 1 (plain TF32) is the ~2e-3 class the survey predicts (A16).  Cases: config 0; dense n = 256 (two B halves, closed form); DZVP blocks with
     n > 256 (several column tiles); ragged blocks with tiny submatrices (n < 16)."""
     cases = [cfg0, W.dense_batch_as_blocks(W.haar_spectrum_batch(6, 256, seed=3)[0]),
              W.water_like(16, "DZVP", 6.0, seed=3), W.random_block_pattern(nb=30, density=0.2, max_bs=5, seed=11)]
@@ -631,7 +631,7 @@ def test_reduced_precision_variants(B, oracle, cfg0, precision, tol_d, tol_e):
             k = int(np.argmax(np.diff(srt)))
             mu = 0.5 * (srt[k] + srt[k + 1])
         d_or = oracle.density(idx, m.values, mu)
-        eps = 2e-6 if precision == 2 else 1e-5
+        eps = 2e-6 if precision in (2, 4) else 1e-5
         plan, st, d, stats, ws, vin = _run_sign(B, m, mu=mu, eps=eps, opt=B.default_options(precision=precision))
         assert st == B.SM_OK, (st, stats.not_converged, stats.max_residual)
         gap = np.abs(lam - mu).min()
@@ -702,13 +702,14 @@ def test_large_submatrix_parity_n1104(B, oracle):
     B.sm_plan_destroy(plan)
 
 
-def test_config4_reduced_precision_full_size(B, oracle):
+@pytest.mark.parametrize("precision,eps", [(2, 2e-6), (4, 2e-6), (3, 1e-5)])
+def test_config4_reduced_precision_full_size(B, oracle, precision, eps):
     """BASELINE config 4: "plus the reduced-precision tensor-core variant run on the same input".
-    precision = 2 (3xTF32 on tcgen05, THE reduced-precision variant of include/submatrix.h) at full size
-    against the ORACLE on 64 sampled groups: <= 1e-3 elementwise (north_star), its band-energy error
+    precision = 2 (3xTF32 on tcgen05, THE reduced-precision variant of include/submatrix.h), and the two 16-bit
+    split rungs (4: FP16x2, 3: BF16x2), at full size against the ORACLE on 64 sampled groups: <= 1e-3 elementwise (north_star), its band-energy error
     asserted and printed."""
     m = W.make_config(4)
-    plan, st, d_gpu, stats, ws, vin = _run_sign(B, m, eps=2e-6, opt=B.default_options(precision=2))
+    plan, st, d_gpu, stats, ws, vin = _run_sign(B, m, eps=eps, opt=B.default_options(precision=precision))
     assert st == B.SM_OK, (st, stats.not_converged, stats.max_residual)
     idx = oracle.Index(m)
     groups = _sample_groups(idx, 64, seed=2)
@@ -718,7 +719,7 @@ def test_config4_reduced_precision_full_size(B, oracle):
     td_o, tdk_o = oracle.traces(idx, d_or, m.values, cols)
     td_g, tdk_g = oracle.traces(idx, d_gpu, m.values, cols)
     e_rel = abs(tdk_g - tdk_o) / abs(tdk_o)
-    print(f"precision=2 config 4: max|D - D_oracle| = {err:.3e} on 64 groups, rel. band-energy error = {e_rel:.3e}, "
+    print(f"precision={precision} config 4: max|D - D_oracle| = {err:.3e} on 64 groups, rel. band-energy error = {e_rel:.3e}, "
           f"n_elec = {stats.n_elec:.4f}")
     assert err <= 1e-3 and e_rel <= 1e-4
     assert np.all(np.isfinite(d_gpu)) and abs(stats.n_elec - m.n_occ) < 1.0
