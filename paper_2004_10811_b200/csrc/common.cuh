@@ -191,7 +191,8 @@ struct EvalCtrl {
     int32_t stop;      // 0 running, 1 all submatrices stopped, 2 steering decision (A11c)
     int32_t k_stop;    // iteration at which it was set
     int32_t decided;   // +1 / -1: n_elec proven above / below the target
-    int32_t pad;
+    int32_t steer_off; // 1: |n_elec(X_k) - target| + bound < margin / 2 was seen: the final count is proven to lie
+                       // inside the margin, no later iteration can prove a direction -- the bound is not evaluated again
     double ne, err;    // n_elec(X_k) and its bound at the decision
 };
 sm_status_t launch_eval_ctrl(sm_plan* p, int k, int steer, double n_target, double margin, cudaStream_t st);

@@ -516,7 +516,7 @@ __global__ void k_nelec_bound(int nb, const int32_t* __restrict__ col_grp, const
                               const double* __restrict__ alpha, int ngroups) {
     // one warp per generating block column c (partials per block column: more warps in flight than one per group)
     const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (c >= nb || ctrl[0] != 0) return;  // evaluation already stopped: empty launch
+    if (c >= nb || ctrl[0] != 0 || ctrl[3] != 0) return;  // evaluation stopped, or steering proven idle (EvalCtrl::steer_off): empty launch
     const int lane = threadIdx.x & 31;
     const int g = col_grp[c];
     if (g < 0) {  // block column of another shard
@@ -582,6 +582,7 @@ k_eval_ctrl(EvalCtrl* __restrict__ c, int k, const int32_t* __restrict__ counter
             const double* __restrict__ bound_part, int nb, int steer, double n_target, double margin) {
     __shared__ double s0[1024], s1[1024];
     if (c->stop != 0) return;  // uniform: set by an earlier launch
+    if (c->steer_off != 0) steer = 0;  // uniform
     if (steer && k >= 1) {
         double a = 0.0, b = 0.0;
         for (int i = threadIdx.x; i < nb; i += 1024) { a += bound_part[i]; b += bound_part[nb + i]; }
@@ -600,6 +601,9 @@ k_eval_ctrl(EvalCtrl* __restrict__ c, int k, const int32_t* __restrict__ counter
         if (ne == ne && err == err && err >= 0.0) {
             const double g = ne - n_target, m = err + margin;
             if (g > m || g < -m) { c->stop = 2; c->k_stop = k; c->decided = g > 0 ? 1 : -1; c->ne = ne; c->err = err; }
+            // the count of the converged X lies in [ne - err, ne + err]: once that interval is inside (-m/2, m/2)
+            // around the target, no later iteration can satisfy the test above -- stop paying for the bound
+            else if (fabs(g) + err < 0.5 * m) c->steer_off = 1;
         }
     }
 }
