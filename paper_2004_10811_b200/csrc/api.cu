@@ -92,7 +92,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_grp_cols, p->d_col_grp, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off, p->d_sub_dim,
                     p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_gen_width, p->d_gen_rng, p->d_ws_off, p->d_ld, p->d_tiles,
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
-                    p->d_partials, p->d_counters, p->d_sched, p->d_act, p->d_act_cnt, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
+                    p->d_partials, p->d_counters, p->d_sched, p->d_act, p->d_act_cnt, p->d_thin_list, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
                     p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_col_rec, p->d_gg, p->d_ctrl, p->d_gl_ptr, p->d_gl,
                     p->d_alpha, p->d_lmin, p->d_lz_rec, p->d_eig_ptr, p->d_eig_lam, p->d_eig_w, p->d_eig_sigma, p->d_eig_order,
@@ -238,7 +238,8 @@ sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_si
     if (e == cudaSuccess) e = A((void**)&p->d_counters, (size_t)(p->opt.max_iter + 2) * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_sched, (size_t)(p->opt.max_iter + 2) * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_act, (size_t)std::max<int64_t>(p->n_tiles, 1) * 4 * 4);
-    if (e == cudaSuccess) e = A((void**)&p->d_act_cnt, (size_t)(p->opt.max_iter + 3) * 8);
+    if (e == cudaSuccess) e = A((void**)&p->d_act_cnt, (size_t)(p->opt.max_iter + 3) * 12);
+    if (e == cudaSuccess) e = A((void**)&p->d_thin_list, (size_t)std::max(ng, 1) * 2 * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_ne_part, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_scalars, 8 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_red, 4096 * 8);
@@ -387,7 +388,7 @@ sm_status_t reset_state(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMemsetAsync(p->d_flag, 0, (size_t)ng * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_counters, 0, (size_t)(p->opt.max_iter + 2) * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_sched, 0, (size_t)(p->opt.max_iter + 2) * 16, st));
-    SM_CUDA(cudaMemsetAsync(p->d_act_cnt, 0, (size_t)(p->opt.max_iter + 3) * 8, st));
+    SM_CUDA(cudaMemsetAsync(p->d_act_cnt, 0, (size_t)(p->opt.max_iter + 3) * 12, st));
     SM_CUDA(cudaMemsetAsync(p->d_ctrl, 0, sizeof(EvalCtrl), st));
     p->cur_k = 0;
     return SM_OK;

@@ -39,6 +39,8 @@ __host__ __device__ __forceinline__ size_t panel_off(int r, int c, int ld) {
     return (size_t)t0 * ld + (size_t)(c >> 3) * rows_t * 8 + (size_t)((r & 63) * 8 + (c & 7));
 }
 
+constexpr int THIN_MAX_ROWS = 16;  // generating-row span served by the thin last update (k_ns_thin, ns_sign.cu)
+
 void set_cuda_error(cudaError_t e, const char* where);
 void set_error_text(const char* msg);
 
@@ -98,7 +100,10 @@ struct sm_plan {
     double* d_partials = nullptr;          // [n_tiles][4] per-tile, per-consumer-warp residual partials
     int32_t* d_counters = nullptr;         // [max_iter+2] still-active submatrices after iteration k
     int32_t* d_act = nullptr;              // [4][n_tiles] work lists of the GEMM launches (ns_sign.cu)
-    int32_t* d_act_cnt = nullptr;          // [2 (max_iter + 3)] their lengths
+    int32_t* d_act_cnt = nullptr;          // [2 (max_iter + 3)] their lengths, then [max_iter + 3] lengths of the thin lists
+    int32_t* d_thin_list = nullptr;        // [2][ngroups] submatrices whose last update is the thin product (k_ns_thin)
+    size_t thin_smem = 0;                  // 8 rows of the largest submatrix; 0: thin path off (too large)
+    int thin_attr_set = 0;
     int32_t* d_sched = nullptr;            // [2*(max_iter+2)] work counters of the persistent GEMM launches
     double* d_ne_part = nullptr;           // [ngroups] per-group electron-count partials
     double* d_scalars = nullptr;           // [8] n_elec, tr D, tr DK, gersh lo/hi

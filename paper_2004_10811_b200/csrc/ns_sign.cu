@@ -446,6 +446,8 @@ struct NsArgs {
     int32_t* next_upd_count;
     int32_t* next_sq_list;    // ... and of the squaring (MODE 0) of the next one
     int32_t* next_sq_count;
+    int32_t* thin_list;       // k_ns_decide: submatrices whose LAST update is done by k_ns_thin (see there); null: none
+    int32_t* thin_count;
     int32_t n_tiles;
     int32_t ngroups;
     int32_t k;
@@ -675,6 +677,14 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
     }
     // work lists of the launches that follow (see NsArgs): every tile of a submatrix that goes on
     goes_on = __shfl_sync(0xffffffffu, goes_on, 0);
+    if (goes_on == 2 && a.thin_list && a.gen_rng) {
+        // predicted exit of a submatrix with few generating rows: its last update is the thin product of k_ns_thin
+        const int2 gr = __ldg(a.gen_rng + g);
+        if (gr.y - gr.x < THIN_MAX_ROWS) {
+            if (lane == 0) a.thin_list[atomicAdd(a.thin_count, 1)] = g;
+            return;
+        }
+    }
     if (goes_on && a.next_upd_list) {
         const int tf = tile_first[g], tc = tile_count[g];
         int base = 0;
@@ -687,6 +697,109 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
             base = __shfl_sync(0xffffffffu, base, 0);
             for (int t = lane; t < tc; t += 32) a.next_sq_list[base + t] = tf + t;
         }
+    }
+}
+
+// Last update of the submatrices that leave by the predicted exit, for groups with few generating rows.
+// Nothing reads X_{k+1} of such a submatrix but the extraction of the generating columns (PAPER.md L127 step 3) and
+// the electron count (L275): rows r0..r1 of the symmetric X_{k+1} (scatter and k_nelec_part walk rows).  So the
+// update is the THIN product  X'[r, :] = cb al (X[r, :] Y - 3 X[r, :]),  r = r0..r1 -- (r1 - r0 + 1) x n x n instead
+// of the n x n x n of a full update (or the ~40 % of it that the tile-restricted final update of k_ns_gemm<1> costs
+// at n ~ 200).  It reads all of Y once per 8 rows, i.e. it is bound by HBM, not by the FP64 pipe.
+// One CTA per submatrix and chunk of 8 rows: the rows of X staged in shared memory (A fragments), each warp takes
+// column sub-tiles j8 = w, w + 8, ..., four at a time; B fragments straight from global memory: lane (lr, lk) reads
+// Y[8 j8 + lr][8 p + 2 lk .. + 1] (Y symmetric), 512 contiguous bytes per warp load in the k8-panel layout.
+constexpr int THIN_WARPS = 8;
+struct ThinArgs {
+    const int32_t* list;
+    const int32_t* count;
+    const int32_t* sub_dim;
+    const int32_t* ldv;
+    const int64_t* ws_off;
+    const int2* gen_rng;
+    const unsigned long long* gersh;
+    const double* alpha;   // rescaling factors of this iteration (slot k & 1), or null
+    const double* X;       // X_k
+    const double* Y;       // al^2 X_k^2
+    double* Out;           // X_{k+1}
+    const int32_t* ctrl;
+    int k;
+};
+__global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin(ThinArgs a) {
+    extern __shared__ __align__(16) double sA[];  // [8][ld] rows of X, row-major
+    if (a.ctrl[0] != 0) return;
+    const int cnt = *a.count;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lr = lane >> 2, lk = lane & 3;
+    for (int i = blockIdx.x; i < cnt; i += gridDim.x) {
+        const int g = a.list[i];
+        const int ld = a.ldv[g];
+        const int2 gr = a.gen_rng[g];
+        const int64_t ws = a.ws_off[g];
+        const double* Xg = a.X + ws;
+        const double* Yg = a.Y + ws;
+        double* Og = a.Out + ws;
+        double scale = -0.5;
+        if (a.k == 0) {
+            double sg = __longlong_as_double((long long)a.gersh[g]);
+            if (!(sg > 0.0)) sg = 1.0;
+            scale /= sg;
+        }
+        if (a.alpha) scale *= a.alpha[g];
+        const int nj8 = ld >> 3;
+        for (int c0 = gr.x; c0 <= gr.y; c0 += 8) {
+            __syncthreads();  // the previous chunk's fragments have been read
+            for (int e = threadIdx.x; e < 8 * ld; e += blockDim.x) {
+                const int r = e / ld, c = e - r * ld;
+                const int row = c0 + r;
+                sA[e] = (row <= gr.y && row < ld) ? Xg[panel_off(row, c, ld)] : 0.0;
+            }
+            __syncthreads();
+            const int row = c0 + lr;
+            const bool row_ok = row <= gr.y && row < ld;
+            for (int j0 = w; j0 < nj8; j0 += 4 * THIN_WARPS) {
+                double acc[4][2];
+                const double* yp[4];
+                bool ok[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    acc[u][0] = acc[u][1] = 0.0;
+                    const int j8 = j0 + u * THIN_WARPS;
+                    ok[u] = j8 < nj8;
+                    yp[u] = Yg + panel_off(8 * (ok[u] ? j8 : 0) + lr, 2 * lk, ld);
+                }
+                // k8 panel p of row r sits at  (r's tile base) + p * rows_t * 8: advance by the panel stride
+                int pst[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int r = 8 * (ok[u] ? j0 + u * THIN_WARPS : 0) + lr;
+                    pst[u] = min(64, ld - (r & ~63)) * 8;
+                }
+                const double* ap = sA + lr * ld + 2 * lk;
+#pragma unroll 2
+                for (int p = 0; p < nj8; ++p) {
+                    const double2 af = *reinterpret_cast<const double2*>(ap + 8 * p);
+                    double2 bf[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        bf[u] = ok[u] ? *reinterpret_cast<const double2*>(yp[u] + (size_t)p * pst[u]) : make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        dmma(acc[u], af.x, bf[u].x);
+                        dmma(acc[u], af.y, bf[u].y);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int j8 = j0 + u * THIN_WARPS;
+                    if (!ok[u] || !row_ok) continue;
+                    const int col = 8 * j8 + 2 * lk;
+                    const double x0 = sA[lr * ld + col], x1 = sA[lr * ld + col + 1];
+                    *reinterpret_cast<double2*>(Og + panel_off(row, col, ld)) =
+                        make_double2(scale * fma(-3.0, x0, acc[u][0]), scale * fma(-3.0, x1, acc[u][1]));
+                }
+            }
+        }
+        __syncthreads();
     }
 }
 
@@ -721,6 +834,10 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     const int32_t* upd_list = L + (size_t)(k & 1) * nt;
     const int32_t* upd_count = C + 2 * k;
     a.predict = (p->opt.predict != 0 && p->opt.order == 2 && eps >= 1e-13) ? 1 : 0; a.max_iter = p->opt.max_iter;
+    // thin last updates (k_ns_thin): list slot k & 1, count per iteration behind the tile-list counts
+    const bool thin = a.predict && a.gen_rng && p->d_thin_list && p->thin_smem > 0;
+    a.thin_list = thin ? p->d_thin_list + (size_t)(k & 1) * std::max(p->ngroups, 1) : nullptr;
+    a.thin_count = thin ? C + 2 * (p->opt.max_iter + 3) + k : nullptr;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * SM_MINB);
     a.sched = p->d_sched + 4 * k;
     if (which & 1) {
@@ -741,6 +858,20 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
             a.sched = p->d_sched + 4 * k + 1;
             k_ns_gemm<1><<<grid, NTHREADS, NS_SMEM, st>>>(a);
             p->launches += 1;
+            if (thin) {
+                if (!p->thin_attr_set) {
+                    SM_CUDA(cudaFuncSetAttribute(k_ns_thin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->thin_smem));
+                    p->thin_attr_set = 1;
+                }
+                ThinArgs t;
+                t.list = a.thin_list; t.count = a.thin_count; t.sub_dim = p->d_sub_dim; t.ldv = p->d_ld; t.ws_off = p->d_ws_off;
+                t.gen_rng = p->d_gen_rng; t.gersh = p->d_gersh;
+                t.alpha = resc ? p->d_alpha + (size_t)(k & 1) * p->ngroups : nullptr;
+                t.X = (k & 1) ? buf1 : buf0; t.Y = bufY; t.Out = (k & 1) ? buf0 : buf1; t.ctrl = p->d_ctrl; t.k = k;
+                const int tgrid = (int)std::min<int64_t>(p->ngroups, (int64_t)p->num_sms * 8);
+                k_ns_thin<<<tgrid, THIN_WARPS * 32, p->thin_smem, st>>>(t);
+                p->launches += 1;
+            }
         }
     }
     SM_CUDA(cudaGetLastError());
