@@ -290,6 +290,35 @@ def test_large_member_count_chunked_block_map(B, oracle):
     _sampled_parity(B, oracle, m, 4)
 
 
+@pytest.mark.parametrize("per_group", [1, 3, 6, 9])
+def test_last_update_row_spans(B, oracle, per_group):
+    """The last update of a predicted exit (reading A9b) is a thin product over the generating rows when they
+    span at most 16 rows (k_ns_thin), else the tile-restricted update: groups of 1 atom (spans 4 and 1), of one
+    molecule (6: one chunk of 8 rows), of two molecules (12: two chunks) and of three (18: tile path) on the same
+    matrix must all meet the bar, and the predicted exit must actually have been taken (flag 2 is 'converged')."""
+    import dataclasses
+    base = W.water_like(48, "SZV", 6.0, seed=5)
+    nb = base.nb
+    m = dataclasses.replace(base, grp_ptr=np.arange(0, nb + 1, per_group, dtype=np.int32))
+    assert m.grp_ptr[-1] == nb
+    idx = oracle.Index(m)
+    lam, _, _, _ = oracle.eig_groups(idx, m.values)
+    srt = np.sort(lam)
+    k = int(np.argmax(np.diff(srt)))
+    mu = 0.5 * (srt[k] + srt[k + 1])  # middle of the widest hole of the union of the submatrix spectra
+    plan, st, d_gpu, stats, _, _ = _run_sign(B, m, mu=mu)
+    assert st == B.SM_OK and stats.not_converged == 0 and stats.max_residual < EPS
+    d_or = oracle.density(idx, m.values, mu)
+    assert np.abs(d_gpu - d_or).max() <= TOL_D
+    td_o, _ = oracle.traces(idx, d_or, m.values)
+    assert abs(stats.n_elec - td_o) <= 1e-9
+    # same result with the predicted exit (and with it both forms of the last update) switched off
+    plan2, st2, d_ref, stats2, _, _ = _run_sign(B, m, mu=mu, opt=B.default_options(predict=0))
+    assert st2 == B.SM_OK and np.abs(d_gpu - d_ref).max() <= 1e-12
+    assert stats.gemm_launches <= stats2.gemm_launches
+    B.sm_plan_destroy(plan); B.sm_plan_destroy(plan2)
+
+
 def test_ragged_blocks_and_scattered_groups(B, oracle):
     for seed in range(3):
         m = W.random_block_pattern(nb=30 + seed, density=0.2, max_bs=7, seed=10 + seed)
