@@ -102,9 +102,13 @@ typedef struct {
     double overshoot;    /* scaling = 1 only: s = bound / overshoot, 1 <= overshoot <= 1.5 [1.45]*/
                          /* (eigenvalues of X0 in (1, 1.5] map back into [0.56, 1); 1.45 is   */
                          /* where the top and the bottom of the water-like spectra balance)  */
-    int32_t predict;     /* 1: predicted exit (reading A9): a submatrix whose next residual  [1]  */
+    int32_t predict;     /* 1: predicted exit (reading A9b): a submatrix whose next residual [2]  */
                          /* is bounded a factor 10 below eps by ||E'|| <= 3/4||E||^2+1/4||E||^3 */
-                         /* stops after its update, without the confirming X^2 product       */
+                         /* stops after its update, without the confirming X^2 product;      */
+                         /* 2: also the two-step exit (reading A9c): the residual of X_{k+1}  */
+                         /* is certified from one product (I - Y_k)^2 without forming         */
+                         /* X_{k+1}; if it passes the test above, only the generating rows    */
+                         /* of X_{k+2} are formed (groups of <= 16 generating rows); 0: off   */
     int32_t mu_guess;    /* sm_density_matrix, scaling = 1 only: the first interior step of the   [1]  */
                          /* mu search goes to the estimate the Gauss quadrature of the Lanczos     */
                          /* run gives for the target filling (reading A11d) if that lies inside    */
@@ -202,6 +206,8 @@ typedef struct {
                               /* of K~ the interlacing bound was taken from (else 0, 0)       */
     double bracket_lo, bracket_hi; /* sm_density_matrix: the initial bisection bracket        */
     double mu_guess;          /* sm_density_matrix: the quadrature estimate (NaN if not computed) */
+    int32_t exits_predicted;  /* last evaluation: submatrices that left by the predicted exit (A9b) ... */
+    int32_t exits_two_step;   /* ... and by the two-step exit (A9c); the rest met eps on a computed residual */
 } sm_stats_t;
 
 /*

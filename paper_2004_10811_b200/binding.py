@@ -72,7 +72,8 @@ class sm_stats_t(C.Structure):
                 ("tot_gemm_launches", C.c_int32), ("tot_evaluations", C.c_int32),
                 ("tot_ms_gather", C.c_float), ("tot_ms_sign", C.c_float),
                 ("spec_lo", C.c_double), ("spec_hi", C.c_double), ("bracket_lo", C.c_double),
-                ("bracket_hi", C.c_double), ("mu_guess", C.c_double)]
+                ("bracket_hi", C.c_double), ("mu_guess", C.c_double),
+                ("exits_predicted", C.c_int32), ("exits_two_step", C.c_int32)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_ if k not in ("mu_trace", "ne_trace", "ne_err_trace", "iter_trace")}
@@ -86,7 +87,7 @@ class sm_stats_t(C.Structure):
 
 def default_options(**kw) -> sm_options_t:
     o = sm_options_t(max_iter=100, scaling=1, precision=0, check_every=16, max_mu_steps=64, bisect_iter=0,
-                     mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=1, mu_guess=1, rescale=1, mu_start=1,
+                     mu_tol=1e-6, early_out=1, overshoot=1.45, order=2, predict=2, mu_guess=1, rescale=1, mu_start=1,
                      method=0, reserved1=0, kT=0.0, shard_rank=0, shard_world=1)
     for k, v in kw.items():
         setattr(o, k, v)

@@ -31,7 +31,7 @@ static void default_options(sm_options_t* o) {
     o->early_out = 1;
     o->overshoot = 1.45;
     o->order = 2;
-    o->predict = 1;
+    o->predict = 2;
     o->mu_guess = 1;
     o->mu_start = 1;
     o->rescale = 1;
@@ -92,7 +92,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_grp_cols, p->d_col_grp, p->d_sub_ptr, p->d_sub_blocks, p->d_sub_off, p->d_sub_dim,
                     p->d_gen_pos, p->d_gen_off, p->d_blk_pack, p->d_gen_width, p->d_gen_rng, p->d_ws_off, p->d_ld, p->d_tiles,
                     p->d_tile_first, p->d_tile_count, p->d_done_iter, p->d_flag, p->d_res, p->d_gersh,
-                    p->d_partials, p->d_counters, p->d_sched, p->d_act, p->d_act_cnt, p->d_thin_list, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
+                    p->d_partials, p->d_counters, p->d_sched, p->d_act, p->d_act_cnt, p->d_thin_list, p->d_spec_tiles, p->d_spec_stat, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
                     p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_col_rec, p->d_gg, p->d_ctrl, p->d_gl_ptr, p->d_gl,
                     p->d_alpha, p->d_lmin, p->d_lz_rec, p->d_eig_ptr, p->d_eig_lam, p->d_eig_w, p->d_eig_sigma, p->d_eig_order,
@@ -238,8 +238,11 @@ sm_status_t plan_create_impl(sm_plan_t** plan, int32_t nb, const int32_t* blk_si
     if (e == cudaSuccess) e = A((void**)&p->d_counters, (size_t)(p->opt.max_iter + 2) * 4);
     if (e == cudaSuccess) e = A((void**)&p->d_sched, (size_t)(p->opt.max_iter + 2) * 16);
     if (e == cudaSuccess) e = A((void**)&p->d_act, (size_t)std::max<int64_t>(p->n_tiles, 1) * 4 * 4);
-    if (e == cudaSuccess) e = A((void**)&p->d_act_cnt, (size_t)(p->opt.max_iter + 3) * 12);
-    if (e == cudaSuccess) e = A((void**)&p->d_thin_list, (size_t)std::max(ng, 1) * 2 * 4);
+    if (e == cudaSuccess) e = A((void**)&p->d_act_cnt, (size_t)(p->opt.max_iter + 3) * 24);
+    if (e == cudaSuccess) e = A((void**)&p->d_thin_list, (size_t)std::max(ng, 1) * 4 * 4);
+    if (e == cudaSuccess) e = A((void**)&p->d_spec_tiles, (size_t)std::max<int64_t>(p->n_tiles, 1) * 4);
+    if (e == cudaSuccess) e = A((void**)&p->d_spec_stat, 8);
+    if (e == cudaSuccess) e = cudaMemset(p->d_spec_stat, 0, 8);
     if (e == cudaSuccess) e = A((void**)&p->d_ne_part, (size_t)ng * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_scalars, 8 * 8);
     if (e == cudaSuccess) e = A((void**)&p->d_red, 4096 * 8);
@@ -388,7 +391,7 @@ sm_status_t reset_state(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMemsetAsync(p->d_flag, 0, (size_t)ng * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_counters, 0, (size_t)(p->opt.max_iter + 2) * 4, st));
     SM_CUDA(cudaMemsetAsync(p->d_sched, 0, (size_t)(p->opt.max_iter + 2) * 16, st));
-    SM_CUDA(cudaMemsetAsync(p->d_act_cnt, 0, (size_t)(p->opt.max_iter + 3) * 12, st));
+    SM_CUDA(cudaMemsetAsync(p->d_act_cnt, 0, (size_t)(p->opt.max_iter + 3) * 24, st));
     SM_CUDA(cudaMemsetAsync(p->d_ctrl, 0, sizeof(EvalCtrl), st));
     p->cur_k = 0;
     return SM_OK;
@@ -479,7 +482,7 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
     }
     SM_CUDA(cudaMemcpyAsync(p->h_pinned_d, p->d_scalars, 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));
-    int imin = INT32_MAX, imax = 0, nc = 0;
+    int imin = INT32_MAX, imax = 0, nc = 0, n_pred = 0, n_two = 0;
     double rmax = 0.0;
     int64_t sin3 = 0, symf = 0;
     for (int i = 0; i < ng; ++i) {
@@ -494,11 +497,17 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         // executed symmetric products: stopped at iteration it: one X^2 per tested iterate (it + 1)
         // and one update per iteration (it); still active after cur_k launch pairs: 2 cur_k (+1 if a steering decision came between the two modes)
         const int64_t ppi = p->opt.order == 3 ? 3 : 2;  // products per iteration (Eq.(11): 2, Eq.(19): 3)
-        const int64_t prods = di[i] >= 0 ? ppi * it + (fl[i] == 2 ? 0 : 1) : ppi * (int64_t)p->cur_k + p->half_iter;
+        // flag 3 (two-step exit, reading A9c, it = k + 2): k + 1 squarings, k updates, the certificate product, and three
+        // thin products instead of the two last updates and the last squaring
+        const int64_t prods = di[i] >= 0 ? (fl[i] == 3 ? ppi * it - 2 : ppi * it + (fl[i] == 2 ? 0 : 1))
+                                         : ppi * (int64_t)p->cur_k + p->half_iter;
         sin3 += prods * n * n * n;
         symf += prods * n * n * (n + 1);
         // predicted exit (flag 2): its last update only computed the tiles of the generating rows
         if (fl[i] == 2 && p->opt.order == 2 && p->opt.precision == 0) symf += p->h_final_flop[i] - n * n * (n + 1);
+        if (fl[i] == 3) symf += 3 * p->h_final_flop[i];
+        if (fl[i] == 2) ++n_pred;
+        if (fl[i] == 3) ++n_two;
     }
     *not_conv = nc;
     if (stats) {
@@ -509,6 +518,8 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         stats->n_elec = p->h_pinned_d[0];
         stats->sum_iter_n3 = sin3;
         stats->tot_sym_flop = symf;  // per evaluation here; callers accumulate
+        stats->exits_predicted = n_pred;
+        stats->exits_two_step = n_two;
     }
     return SM_OK;
 }

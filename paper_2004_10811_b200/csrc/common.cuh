@@ -100,10 +100,14 @@ struct sm_plan {
     double* d_partials = nullptr;          // [n_tiles][4] per-tile, per-consumer-warp residual partials
     int32_t* d_counters = nullptr;         // [max_iter+2] still-active submatrices after iteration k
     int32_t* d_act = nullptr;              // [4][n_tiles] work lists of the GEMM launches (ns_sign.cu)
-    int32_t* d_act_cnt = nullptr;          // [2 (max_iter + 3)] their lengths, then [max_iter + 3] lengths of the thin lists
-    int32_t* d_thin_list = nullptr;        // [2][ngroups] submatrices whose last update is the thin product (k_ns_thin)
+    int32_t* d_act_cnt = nullptr;          // [2 (max_iter + 3)] their lengths, then 4 x [max_iter + 3]: lengths of the thin, speculation, speculation-tile and thin3 lists
+    int32_t* d_thin_list = nullptr;        // [4][ngroups]: 0, 1 submatrices whose last update is the thin product (k_ns_thin); 2 speculated, 3 certified (two-step exit)
     size_t thin_smem = 0;                  // 8 rows of the largest submatrix; 0: thin path off (too large)
     int thin_attr_set = 0;
+    int32_t* d_spec_tiles = nullptr;       // [n_tiles] work list of the MODE 4 launch (two-step exit, ns_sign.cu)
+    int32_t* d_spec_stat = nullptr;        // [2] certified / failed speculations since plan creation
+    size_t thin3_smem = 0;                 // 3 x 8 rows of the largest submatrix; 0: two-step exit off
+    int thin3_attr_set = 0;
     int32_t* d_sched = nullptr;            // [2*(max_iter+2)] work counters of the persistent GEMM launches
     double* d_ne_part = nullptr;           // [ngroups] per-group electron-count partials
     double* d_scalars = nullptr;           // [8] n_elec, tr D, tr DK, gersh lo/hi

@@ -513,7 +513,7 @@ __global__ void k_nelec_bound(int nb, const int32_t* __restrict__ col_grp, const
                               const unsigned long long* __restrict__ gersh, int k, const double* __restrict__ buf0,
                               const double* __restrict__ buf1, const double* __restrict__ bufY,
                               double* __restrict__ part, const int32_t* __restrict__ ctrl,
-                              const double* __restrict__ alpha, int ngroups) {
+                              const double* __restrict__ alpha, int ngroups, const int32_t* __restrict__ flag) {
     // one warp per generating block column c (partials per block column: more warps in flight than one per group)
     const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (c >= nb || ctrl[0] != 0 || ctrl[3] != 0) return;  // evaluation stopped, or steering proven idle (EvalCtrl::steer_off): empty launch
@@ -524,6 +524,19 @@ __global__ void k_nelec_bound(int nb, const int32_t* __restrict__ col_grp, const
         return;
     }
     const int di = done_iter[g];
+    if (di >= 0 && flag[g] == 3) {
+        // finished by the two-step exit (reading A9c): the generating rows of the result are in the buffer of parity
+        // di, X_{di-1} was never formed; the count is final, nothing is left to bound
+        const double* Xf = ((di & 1) ? buf1 : buf0) + ws_off[g];
+        const int ldf = ldv[g];
+        double af = 0.0;
+        const int of = gen_off[c], bf = blk_size[c];
+        for (int e = lane; e < bf; e += 32) af += 0.5 * (1.0 - Xf[panel_off(of + e, of + e, ldf)]);
+#pragma unroll
+        for (int w = 16; w > 0; w >>= 1) af += __shfl_xor_sync(0xffffffffu, af, w);
+        if (lane == 0) { part[c] = af; part[nb + c] = 0.0; }
+        return;
+    }
     const int kb = (di >= 0 && di <= k) ? di : k;  // di = k + 1: predicted exit, its last update has not run yet
     const double* Xg = ((kb & 1) ? buf1 : buf0) + ws_off[g];
     const double* Yg = bufY + ws_off[g];
@@ -569,7 +582,7 @@ sm_status_t launch_nelec_bound(sm_plan* p, int k, const double* buf0, const doub
     if (p->ngroups == 0 || p->nb == 0) return SM_OK;
     k_nelec_bound<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_col_grp, p->d_blk_size, p->d_gen_off, p->d_ld, p->d_ws_off,
                                                    p->d_done_iter, p->d_gersh, k, buf0, buf1, bufY, p->d_bound_part,
-                                                   p->d_ctrl, rescale_on(p) ? p->d_alpha : nullptr, p->ngroups);
+                                                   p->d_ctrl, rescale_on(p) ? p->d_alpha : nullptr, p->ngroups, p->d_flag);
     p->launches += 1;  // the two sums are taken by k_eval_ctrl
     SM_CUDA(cudaGetLastError());
     return SM_OK;

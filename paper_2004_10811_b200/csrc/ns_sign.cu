@@ -61,6 +61,8 @@ template <> struct ModeTraits<0> { static constexpr double fold = 0.0, cb = 1.0;
 template <> struct ModeTraits<1> { static constexpr double fold = -3.0, cb = -0.5; static constexpr bool scale_k0 = true; };
 template <> struct ModeTraits<2> { static constexpr double fold = -10.0 / 3.0, cb = 0.375; static constexpr bool scale_k0 = false; };
 template <> struct ModeTraits<3> { static constexpr double fold = 1.875, cb = 1.0; static constexpr bool scale_k0 = true; };
+//   MODE 4   P  = Y Y - 2 Y + I             = (I - Y)^2                    certificate of the two-step exit (A9c)
+template <> struct ModeTraits<4> { static constexpr double fold = -2.0, cb = 1.0; static constexpr bool scale_k0 = false; };
 constexpr int NCONSUMER = 128, NTHREADS = NCONSUMER + 32;
 constexpr int STAGE_DOUBLES = (BM + BN) * BK;  // A slice then B slice, dense
 constexpr size_t NS_SMEM = (size_t)STAGES * STAGE_DOUBLES * sizeof(double);
@@ -327,7 +329,7 @@ __device__ __forceinline__ void store_below(const EpiCtx& c, const double (&a)[2
     double* pm_ = c.Out + (c.base_m + sr * c.pm + sc * 64);
     pm_[0] = v0;
     pm_[8] = v1;
-    if (MODE == 0 && sr * 8 < c.rlim) {
+    if ((MODE == 0 || MODE == 4) && sr * 8 < c.rlim) {
         const double w0 = v0 * c.rinv, w1 = v1 * c.rinv;
         part = fma(2.0 * w0, w0, fma(2.0 * w1, w1, part));
     }
@@ -342,13 +344,15 @@ __device__ __forceinline__ void store_ondiag(const EpiCtx& c, const double (&a)[
     for (int q = 0; q < 2; ++q) {
         const int cq = 2 * lk + q;
         if (cq > lr) continue;  // upper triangle: its mirror image is stored
-        const double v = a[q] * c.scale;
+        double v = a[q] * c.scale;
+        if (MODE == 4 && cq == lr) v += 1.0;  // P = Y^2 - 2 Y + I
         pd_[q] = v;
         if (cq != lr) pm_[q * 8] = v;
         if (MODE == 0 && sr * 8 < c.rlim) {
             const double d = v * c.rinv - (cq == lr ? 1.0 : 0.0);
             part = fma((cq == lr ? 1.0 : 2.0) * d, d, part);
         }
+        if (MODE == 4 && sr * 8 < c.rlim) part = fma((cq == lr ? 1.0 : 2.0) * v, v, part);  // ||P||_F^2
     }
 }
 
@@ -448,6 +452,14 @@ struct NsArgs {
     int32_t* next_sq_count;
     int32_t* thin_list;       // k_ns_decide: submatrices whose LAST update is done by k_ns_thin (see there); null: none
     int32_t* thin_count;
+    // two-step exit (reading A9c): k_ns_decide lists the submatrices it speculates on and their tiles (work list of the
+    // MODE 4 launch); k_ns_spec_decide sorts them into the thin3 list (certified) or back into the update lists
+    int32_t* spec_list;
+    int32_t* spec_count;
+    int32_t* spec_tiles;
+    int32_t* spec_tile_count;
+    int32_t* thin3_list;
+    int32_t* thin3_count;
     int32_t n_tiles;
     int32_t ngroups;
     int32_t k;
@@ -476,7 +488,7 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
     __syncthreads();
 
     const double* Xk = (k & 1) ? a.buf1 : a.buf0;
-    const double* Xbase = (MODE == 2) ? a.bufY : Xk;                                  // A operand
+    const double* Xbase = (MODE == 2 || MODE == 4) ? a.bufY : Xk;                     // A operand
     const double* Bbase = (MODE == 0) ? Xk : (MODE == 3 ? a.bufW : a.bufY);           // B operand
 
     if (wid == 4) {
@@ -529,7 +541,7 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
                 const int ti = tij & 0xffff, tj = tij >> 16;
                 const int row0 = ti * BM, col0 = tj * BN;
                 const int rows_a = min(BM, ld - row0), rows_b = min(BN, ld - col0);
-                const bool b_is_a = (MODE == 0 || MODE == 2) && (ti == tj);
+                const bool b_is_a = (MODE == 0 || MODE == 2 || MODE == 4) && (ti == tj);
                 const int KP = ld >> 3;            // 8-wide k panels
                 const int KT = (KP + PPS - 1) / PPS;  // stages of PPS panels
                 const double* Asrc = Xbase + ws_off + (size_t)row0 * ld;
@@ -579,7 +591,7 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
         const int s_rows = min(8, (si.ld - row0) >> 3);  // valid 8-row sub-tile rows of this tile, 1..8
         const bool full_diag = diag && s_rows == 8;
         const int rows_a = min(BM, si.ld - row0), rows_b = min(BN, si.ld - col0);
-        const bool b_is_a = (MODE == 0 || MODE == 2) && diag;
+        const bool b_is_a = (MODE == 0 || MODE == 2 || MODE == 4) && diag;
         // work shape of this warp for this tile (see tile_var)
         int variant;
         if (full_diag) variant = 9 + wid;
@@ -606,7 +618,7 @@ __global__ void __launch_bounds__(NTHREADS, SM_MINB) k_ns_gemm(NsArgs a) {
             }
 #undef SM_TV
         }
-        if (MODE == 0) {
+        if (MODE == 0 || MODE == 4) {
             // Residual: every consumer warp publishes its partial of the tile (plain store, no fence,
             // no atomics); k_ns_decide sums them per submatrix in a fixed order after the launch.
 #pragma unroll
@@ -675,8 +687,32 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
             }
         }
     }
+    // Two-step exit (reading A9c): if X_{k+1} is likely to pass the predicted-exit test, its residual is certified
+    // WITHOUT forming it: E_{k+1} = I - X_{k+1}^2 = 3/4 Et^2 + 1/4 Et^3 with Et = I - Y_k (Y_k = al^2 X_k^2 as stored),
+    // so one product P = Et^2 (MODE 4) bounds ||E_{k+1}||_F; then only the generating rows of X_{k+2} are formed
+    // (k_ns_thin3).  The estimate here only decides whether to try: r_{k+1} ~ rt^2 with rt = ||Et||_F / sqrt(n) ~ r / 2
+    // for a rescaled step (the rescaling centres the spectrum of Et), r for a plain one.
+    if (lane == 0 && goes_on == 1 && a.spec_list && k >= 1 && k + 2 <= a.max_iter &&
+        a.gen_rng[g].y - a.gen_rng[g].x < THIN_MAX_ROWS) {
+        const double r = a.res[(size_t)(k & 1) * a.ngroups + g];
+        const double al = a.alpha ? a.alpha[(size_t)(k & 1) * a.ngroups + g] : 1.0;
+        const double rt = al != 1.0 ? 0.5 * r : r;
+        const double sn = sqrt((double)(n > 0 ? n : 1)), f = rt * rt * sn;
+        if ((0.75 * f * f + 0.25 * f * f * f) / sn < 0.1 * a.eps) goes_on = 3;
+    }
     // work lists of the launches that follow (see NsArgs): every tile of a submatrix that goes on
     goes_on = __shfl_sync(0xffffffffu, goes_on, 0);
+    if (goes_on == 3) {
+        const int tf = tile_first[g], tc = tile_count[g];
+        int base = 0;
+        if (lane == 0) {
+            a.spec_list[atomicAdd(a.spec_count, 1)] = g;
+            base = atomicAdd(a.spec_tile_count, tc);
+        }
+        base = __shfl_sync(0xffffffffu, base, 0);
+        for (int t = lane; t < tc; t += 32) a.spec_tiles[base + t] = tf + t;
+        return;
+    }
     if (goes_on == 2 && a.thin_list && a.gen_rng) {
         // predicted exit of a submatrix with few generating rows: its last update is the thin product of k_ns_thin
         const int2 gr = __ldg(a.gen_rng + g);
@@ -725,6 +761,49 @@ struct ThinArgs {
     const int32_t* ctrl;
     int k;
 };
+// One thin product for one warp: (8 rows in shared memory, sA[8][ld]) x (symmetric matrix Mg, k8-panel layout) for the
+// column sub-tiles j8 = w, w + 8, ..., four at a time; emit(j8, acc) receives this lane's two results of sub-tile j8
+// (row lr, columns 8 j8 + 2 lk, + 1).  (Reading only the blocks on or below the diagonal -- every 8 x 8 block is
+// needed twice per pass, once transposed -- was measured: the second use does not come from the L2 often enough
+// to pay for the extra loads, 76.4 against 75.6 ms per evaluation.)
+template <class Emit>
+__device__ __forceinline__ void thin_pass(const double* __restrict__ sA, const double* __restrict__ Mg, int ld, int w,
+                                          int lane, Emit&& emit) {
+    const int lr = lane >> 2, lk = lane & 3, nj8 = ld >> 3;
+    for (int j0 = w; j0 < nj8; j0 += 4 * THIN_WARPS) {
+        double acc[4][2];
+        const double* yp[4];
+        bool ok[4];
+        int pst[4];  // k8 panel p of row r sits at (r's tile base) + p * rows_t * 8
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            acc[u][0] = acc[u][1] = 0.0;
+            const int j8 = j0 + u * THIN_WARPS;
+            ok[u] = j8 < nj8;
+            const int r = 8 * (ok[u] ? j8 : 0) + lr;
+            yp[u] = Mg + panel_off(r, 2 * lk, ld);
+            pst[u] = min(64, ld - (r & ~63)) * 8;
+        }
+        const double* ap = sA + lr * ld + 2 * lk;
+#pragma unroll 2
+        for (int p = 0; p < nj8; ++p) {
+            const double2 af = *reinterpret_cast<const double2*>(ap + 8 * p);
+            double2 bf[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                bf[u] = ok[u] ? *reinterpret_cast<const double2*>(yp[u] + (size_t)p * pst[u]) : make_double2(0.0, 0.0);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                dmma(acc[u], af.x, bf[u].x);
+                dmma(acc[u], af.y, bf[u].y);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (ok[u]) emit(j0 + u * THIN_WARPS, acc[u]);
+    }
+}
+
 __global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin(ThinArgs a) {
     extern __shared__ __align__(16) double sA[];  // [8][ld] rows of X, row-major
     if (a.ctrl[0] != 0) return;
@@ -745,7 +824,6 @@ __global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin(ThinArgs a) {
             scale /= sg;
         }
         if (a.alpha) scale *= a.alpha[g];
-        const int nj8 = ld >> 3;
         for (int c0 = gr.x; c0 <= gr.y; c0 += 8) {
             __syncthreads();  // the previous chunk's fragments have been read
             for (int e = threadIdx.x; e < 8 * ld; e += blockDim.x) {
@@ -756,48 +834,153 @@ __global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin(ThinArgs a) {
             __syncthreads();
             const int row = c0 + lr;
             const bool row_ok = row <= gr.y && row < ld;
-            for (int j0 = w; j0 < nj8; j0 += 4 * THIN_WARPS) {
-                double acc[4][2];
-                const double* yp[4];
-                bool ok[4];
+            thin_pass(sA, Yg, ld, w, lane, [&](int j8, const double (&acc)[2]) {
+                if (!row_ok) return;
+                const int col = 8 * j8 + 2 * lk;
+                const double x0 = sA[lr * ld + col], x1 = sA[lr * ld + col + 1];
+                *reinterpret_cast<double2*>(Og + panel_off(row, col, ld)) =
+                    make_double2(scale * fma(-3.0, x0, acc[0]), scale * fma(-3.0, x1, acc[1]));
+            });
+        }
+        __syncthreads();
+    }
+}
+
+// ---- two-step exit (reading A9c), second half: the certificate and the generating rows of X_{k+2}
+// k_ns_spec_decide, one warp per submatrix k_ns_decide speculated on: ||P||_F from the MODE 4 partials, then
+//   ||E_{k+1}||_F <= (3/4 + 1/4 ||Et||_2) ||P||_F,   ||Et||_2 <= ||Et||_F <= (|1 - al^2| + al^2 r_k) sqrt(n)
+// (Et = I - al^2 X_k^2 = (1 - al^2) I + al^2 E_k), and the test of the predicted exit (A9b) on that bound: if
+// 3/4 f^2 + 1/4 f^3 (f = the bound) is a factor 10 below eps, X_{k+2} = 1/2 X_{k+1} (3 I - X_{k+1}^2) is accepted as the
+// result (done_iter = k + 2, flag 3) and only its generating rows are formed; otherwise the submatrix goes on as if
+// nothing had happened (its tiles join the update list of iteration k and the squaring list of k + 1): the
+// speculation cost one product.
+struct SpecArgs {
+    const int32_t* list;
+    const int32_t* count;
+    const int32_t* tile_first;
+    const int32_t* tile_count;
+    const int32_t* sub_dim;
+    const double* partials;
+    double* res;
+    const double* alpha;  // slot k & 1, or null
+    int32_t* done_iter;
+    int32_t* flag;
+    int32_t* thin3_list;
+    int32_t* thin3_count;
+    int32_t* upd_list;
+    int32_t* upd_count;
+    int32_t* sq_list;
+    int32_t* sq_count;
+    int32_t* stat;        // [0] certified, [1] failed (per plan, running totals)
+    const int32_t* ctrl;
+    int ngroups, k;
+    double eps;
+};
+__global__ void __launch_bounds__(256) k_ns_spec_decide(SpecArgs a) {
+    if (a.ctrl[0] != 0) return;
+    const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (i >= *a.count) return;
+    const int lane = threadIdx.x & 31, g = a.list[i], k = a.k;
+    const int tf = a.tile_first[g], tc = a.tile_count[g], n = a.sub_dim[g];
+    const double* pp = a.partials + (size_t)tf * 4;
+    double p2 = 0.0;
+    for (int t = lane; t < 4 * tc; t += 32) p2 += pp[t];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    acc[u][0] = acc[u][1] = 0.0;
-                    const int j8 = j0 + u * THIN_WARPS;
-                    ok[u] = j8 < nj8;
-                    yp[u] = Yg + panel_off(8 * (ok[u] ? j8 : 0) + lr, 2 * lk, ld);
-                }
-                // k8 panel p of row r sits at  (r's tile base) + p * rows_t * 8: advance by the panel stride
-                int pst[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int r = 8 * (ok[u] ? j0 + u * THIN_WARPS : 0) + lr;
-                    pst[u] = min(64, ld - (r & ~63)) * 8;
-                }
-                const double* ap = sA + lr * ld + 2 * lk;
-#pragma unroll 2
-                for (int p = 0; p < nj8; ++p) {
-                    const double2 af = *reinterpret_cast<const double2*>(ap + 8 * p);
-                    double2 bf[4];
-#pragma unroll
-                    for (int u = 0; u < 4; ++u)
-                        bf[u] = ok[u] ? *reinterpret_cast<const double2*>(yp[u] + (size_t)p * pst[u]) : make_double2(0.0, 0.0);
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        dmma(acc[u], af.x, bf[u].x);
-                        dmma(acc[u], af.y, bf[u].y);
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int j8 = j0 + u * THIN_WARPS;
-                    if (!ok[u] || !row_ok) continue;
-                    const int col = 8 * j8 + 2 * lk;
-                    const double x0 = sA[lr * ld + col], x1 = sA[lr * ld + col + 1];
-                    *reinterpret_cast<double2*>(Og + panel_off(row, col, ld)) =
-                        make_double2(scale * fma(-3.0, x0, acc[u][0]), scale * fma(-3.0, x1, acc[u][1]));
-                }
+    for (int o = 16; o > 0; o >>= 1) p2 += __shfl_xor_sync(0xffffffffu, p2, o);
+    int ok = 0;
+    if (lane == 0) {
+        const double sn = sqrt((double)(n > 0 ? n : 1));
+        const double r = a.res[(size_t)(k & 1) * a.ngroups + g];
+        const double al = a.alpha ? a.alpha[g] : 1.0;
+        const double et = (fabs(1.0 - al * al) + al * al * r) * sn;
+        const double f = (0.75 + 0.25 * et) * sqrt(p2);  // >= ||E_{k+1}||_F
+        const double next = (0.75 * f * f + 0.25 * f * f * f) / sn;
+        ok = (next < 0.1 * a.eps) ? 1 : 0;  // false for NaN
+        if (ok) {
+            a.done_iter[g] = k + 2;
+            a.flag[g] = 3;
+            a.res[(size_t)(k & 1) * a.ngroups + g] = next;  // slot (k + 2) & 1: the residual bound of the result
+            a.thin3_list[atomicAdd(a.thin3_count, 1)] = g;
+            atomicAdd(a.stat, 1);
+        } else {
+            atomicAdd(a.stat + 1, 1);
+        }
+    }
+    ok = __shfl_sync(0xffffffffu, ok, 0);
+    if (ok) return;
+    int base = 0;
+    if (lane == 0) base = atomicAdd(a.upd_count, tc);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    for (int t = lane; t < tc; t += 32) a.upd_list[base + t] = tf + t;
+    if (lane == 0) base = atomicAdd(a.sq_count, tc);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    for (int t = lane; t < tc; t += 32) a.sq_list[base + t] = tf + t;
+}
+
+// k_ns_thin3: generating rows r of X_{k+2} for the certified submatrices, three thin products per 8 rows:
+//   X_{k+1}[r, :] = 1/2 al (3 X_k[r, :] - X_k[r, :] Y)                           (Y = al^2 X_k^2, stored)
+//   Z = X_{k+1}[r, :] P,   W = Z (I - Y) = Z - Z Y                               (P = (I - Y)^2, from MODE 4)
+//   X_{k+2}[r, :] = 1/2 X_{k+1}[r, :] (3 I - X_{k+1}^2) = X_{k+1}[r, :] + 3/8 Z + 1/8 W
+// since X_{k+1}^2 = I - 3/4 P - 1/4 (I - Y) P and everything commutes.  The rows go into the buffer of X_k (parity of
+// k + 2), which nothing reads any more; P sits in the buffer X_{k+1} would have taken.
+struct Thin3Args {
+    const int32_t* list;
+    const int32_t* count;
+    const int32_t* ldv;
+    const int64_t* ws_off;
+    const int2* gen_rng;
+    const double* alpha;  // slot k & 1, or null
+    double* X;            // X_k in, rows of X_{k+2} out
+    const double* Y;
+    const double* P;
+    const int32_t* ctrl;
+};
+__global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin3(Thin3Args a) {
+    extern __shared__ __align__(16) double sm3[];  // three arrays [8][ld]
+    if (a.ctrl[0] != 0) return;
+    const int cnt = *a.count;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lr = lane >> 2, lk = lane & 3;
+    for (int i = blockIdx.x; i < cnt; i += gridDim.x) {
+        const int g = a.list[i];
+        const int ld = a.ldv[g];
+        const int2 gr = a.gen_rng[g];
+        const int64_t ws = a.ws_off[g];
+        double* Xg = a.X + ws;
+        const double* Yg = a.Y + ws;
+        const double* Pg = a.P + ws;
+        const double al = a.alpha ? a.alpha[g] : 1.0;
+        double* s0 = sm3;            // X_k rows, then Z
+        double* s1 = sm3 + 8 * ld;   // X_{k+1} rows
+        double* s2 = s1 + 8 * ld;    // Z
+        for (int c0 = gr.x; c0 <= gr.y; c0 += 8) {
+            __syncthreads();
+            for (int e = threadIdx.x; e < 8 * ld; e += blockDim.x) {
+                const int r = e / ld, c = e - r * ld;
+                const int row = c0 + r;
+                s0[e] = (row <= gr.y && row < ld) ? Xg[panel_off(row, c, ld)] : 0.0;
             }
+            __syncthreads();
+            thin_pass(s0, Yg, ld, w, lane, [&](int j8, const double (&acc)[2]) {
+                const int o = lr * ld + 8 * j8 + 2 * lk;
+                s1[o] = 0.5 * al * fma(3.0, s0[o], -acc[0]);
+                s1[o + 1] = 0.5 * al * fma(3.0, s0[o + 1], -acc[1]);
+            });
+            __syncthreads();
+            thin_pass(s1, Pg, ld, w, lane, [&](int j8, const double (&acc)[2]) {
+                const int o = lr * ld + 8 * j8 + 2 * lk;
+                s2[o] = acc[0];
+                s2[o + 1] = acc[1];
+            });
+            __syncthreads();
+            const int row = c0 + lr;
+            const bool row_ok = row <= gr.y && row < ld;
+            thin_pass(s2, Yg, ld, w, lane, [&](int j8, const double (&acc)[2]) {
+                if (!row_ok) return;
+                const int col = 8 * j8 + 2 * lk, o = lr * ld + col;
+                const double w0 = s2[o] - acc[0], w1 = s2[o + 1] - acc[1];
+                *reinterpret_cast<double2*>(Xg + panel_off(row, col, ld)) =
+                    make_double2(s1[o] + 0.375 * s2[o] + 0.125 * w0, s1[o + 1] + 0.375 * s2[o + 1] + 0.125 * w1);
+            });
         }
         __syncthreads();
     }
@@ -838,6 +1021,15 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     const bool thin = a.predict && a.gen_rng && p->d_thin_list && p->thin_smem > 0;
     a.thin_list = thin ? p->d_thin_list + (size_t)(k & 1) * std::max(p->ngroups, 1) : nullptr;
     a.thin_count = thin ? C + 2 * (p->opt.max_iter + 3) + k : nullptr;
+    // two-step exit (A9c): predict >= 2; lists: slot 2 = speculated submatrices, slot 3 = certified ones
+    const int M = p->opt.max_iter + 3;
+    const bool spec = thin && p->opt.predict >= 2 && p->thin3_smem > 0 && p->d_spec_tiles;
+    a.spec_list = spec ? p->d_thin_list + (size_t)2 * std::max(p->ngroups, 1) : nullptr;
+    a.spec_count = spec ? C + 3 * M + k : nullptr;
+    a.spec_tiles = spec ? p->d_spec_tiles : nullptr;
+    a.spec_tile_count = spec ? C + 4 * M + k : nullptr;
+    a.thin3_list = spec ? p->d_thin_list + (size_t)3 * std::max(p->ngroups, 1) : nullptr;
+    a.thin3_count = spec ? C + 5 * M + k : nullptr;
     const int grid = (int)std::min<int64_t>(p->n_tiles, (int64_t)p->num_sms * SM_MINB);
     a.sched = p->d_sched + 4 * k;
     if (which & 1) {
@@ -855,6 +1047,32 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
             k_ns_gemm<3><<<grid, NTHREADS, NS_SMEM, st>>>(a);
             p->launches += 2;
         } else {
+            if (spec) {
+                if (!p->thin3_attr_set) {
+                    SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
+                    SM_CUDA(cudaFuncSetAttribute(k_ns_thin3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->thin3_smem));
+                    p->thin3_attr_set = 1;
+                }
+                NsArgs a4 = a;  // P = (I - Y)^2 of the speculated submatrices into the buffer of X_{k+1}
+                a4.act_list = a.spec_tiles; a4.act_count = a.spec_tile_count; a4.sched = p->d_sched + 4 * k + 3;
+                k_ns_gemm<4><<<grid, NTHREADS, NS_SMEM, st>>>(a4);
+                SpecArgs sa;
+                sa.list = a.spec_list; sa.count = a.spec_count; sa.tile_first = p->d_tile_first; sa.tile_count = p->d_tile_count;
+                sa.sub_dim = p->d_sub_dim; sa.partials = p->d_partials; sa.res = p->d_res;
+                sa.alpha = resc ? p->d_alpha + (size_t)(k & 1) * p->ngroups : nullptr;
+                sa.done_iter = p->d_done_iter; sa.flag = p->d_flag; sa.thin3_list = a.thin3_list; sa.thin3_count = a.thin3_count;
+                sa.upd_list = a.next_upd_list; sa.upd_count = a.next_upd_count;
+                sa.sq_list = a.next_sq_list; sa.sq_count = a.next_sq_count;
+                sa.stat = p->d_spec_stat; sa.ctrl = p->d_ctrl; sa.ngroups = p->ngroups; sa.k = k; sa.eps = eps;
+                k_ns_spec_decide<<<(p->ngroups + 7) / 8, 256, 0, st>>>(sa);
+                Thin3Args t3;
+                t3.list = a.thin3_list; t3.count = a.thin3_count; t3.ldv = p->d_ld; t3.ws_off = p->d_ws_off;
+                t3.gen_rng = p->d_gen_rng; t3.alpha = sa.alpha;
+                t3.X = (k & 1) ? buf1 : buf0; t3.Y = bufY; t3.P = (k & 1) ? buf0 : buf1; t3.ctrl = p->d_ctrl;
+                const int tgrid3 = (int)std::min<int64_t>(p->ngroups, (int64_t)p->num_sms * 4);
+                k_ns_thin3<<<tgrid3, THIN_WARPS * 32, p->thin3_smem, st>>>(t3);
+                p->launches += 3;
+            }
             a.sched = p->d_sched + 4 * k + 1;
             k_ns_gemm<1><<<grid, NTHREADS, NS_SMEM, st>>>(a);
             p->launches += 1;

@@ -316,6 +316,17 @@ def test_last_update_row_spans(B, oracle, per_group):
     plan2, st2, d_ref, stats2, _, _ = _run_sign(B, m, mu=mu, opt=B.default_options(predict=0))
     assert st2 == B.SM_OK and np.abs(d_gpu - d_ref).max() <= 1e-12
     assert stats.gemm_launches <= stats2.gemm_launches
+    # the exits were actually taken: every group here is well conditioned; the two-step exit serves spans <= 16
+    assert stats2.exits_predicted == 0 and stats2.exits_two_step == 0
+    assert stats.exits_predicted + stats.exits_two_step >= idx.ngroups // 2
+    if per_group * 2 <= 16:
+        assert stats.exits_two_step > 0
+    else:
+        assert stats.exits_two_step == 0
+    # ... and the one-step exit alone (predict = 1) gives the same result
+    plan1, st1, d_one, stats1, _, _ = _run_sign(B, m, mu=mu, opt=B.default_options(predict=1))
+    assert st1 == B.SM_OK and stats1.exits_two_step == 0 and np.abs(d_one - d_ref).max() <= 1e-12
+    B.sm_plan_destroy(plan1)
     B.sm_plan_destroy(plan); B.sm_plan_destroy(plan2)
 
 
