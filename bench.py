@@ -496,13 +496,13 @@ def main():
         sampler.mark()
     launches0 = B.sm_launch_count(plan)
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    gemm_ms = gemm_launches = sym_flop = n3 = evals = 0.0
+    gemm_ms = gemm_launches = sym_flop = n3 = evals = gemm_only_ms = 0.0
     gather_ms = 0.0
     evs[0].record(stream)
     for i in range(args.steps):
         st, mu = step_device()
         evs[i + 1].record(stream)
-        gemm_ms += stats.tot_ms_sign; gemm_launches += stats.tot_gemm_launches
+        gemm_ms += stats.tot_ms_sign; gemm_launches += stats.tot_gemm_launches; gemm_only_ms += stats.tot_ms_gemm
         sym_flop += stats.tot_sym_flop; n3 += stats.tot_sum_iter_n3; evals += stats.tot_evaluations
         gather_ms += stats.tot_ms_gather
     barrier()
@@ -530,17 +530,19 @@ def main():
         hbm_peak, hbm_src = hbm_peak_gbps()
         # dominant kernel: k_ns_gemm<0|1>.  Algorithmic flops of one symmetric n x n product:
         # n(n+1)/2 outputs x 2n flop = n^2 (n+1); per launch = sum over the active submatrices.
-        # gemm_ms = CUDA-event time of the Newton-Schulz phases (event pairs recorded by the library on its
-        # stream around every evaluation's iteration loop): the GEMM launches plus the decision / bound /
-        # control kernels and the empty launches behind a device-side stop (~2 % of it), so `achieved` is a
-        # slight under-estimate of the GEMM kernels' own rate.
-        ach = sym_flop / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
+        # gemm_only_ms = CUDA-event time of the k_ns_gemm launches alone: the library records an event before and
+        # after every product launch on its stream (sm_stats_t.tot_ms_gemm).  gemm_ms = the whole Newton-Schulz
+        # phase (products + decision / bound / control kernels + the thin last updates, which are HBM-bound and
+        # carry almost no flop): reported as sign_phase_tflops.
+        ach = sym_flop / (gemm_only_ms * 1e-3) / 1e12 if gemm_only_ms > 0 else 0.0
+        ach_phase = sym_flop / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
         dmma = peaks["dmma_issue_tflops"]
         roofline = {"bound": "tensor", "kernel": "k_ns_gemm (FP64 DMMA Newton-Schulz, both modes)",
                     "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
                     "traffic": NS_GEMM_DRAM_BYTES_PER_LAUNCH, "peak_source": peak_src,
                     "peak_dmma_issue_measured": dmma, "frac_of_dmma_issue": ach / dmma if dmma else None,
-                    "launches_timed": int(gemm_launches), "avg_launch_ms": gemm_ms / max(gemm_launches, 1),
+                    "launches_timed": int(gemm_launches), "avg_launch_ms": gemm_only_ms / max(gemm_launches, 1),
+                    "sign_phase_tflops": ach_phase, "gemm_share_of_step": gemm_only_ms / ms if ms > 0 else None,
                     "alg_flop_per_launch": sym_flop / max(gemm_launches, 1),
                     "full_gemm_equiv_tflops": 2.0 * n3 / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0,
                     "sign_share_of_step": gemm_ms / ms if ms > 0 else None}

@@ -208,6 +208,9 @@ typedef struct {
     double mu_guess;          /* sm_density_matrix: the quadrature estimate (NaN if not computed) */
     int32_t exits_predicted;  /* last evaluation: submatrices that left by the predicted exit (A9b) ... */
     int32_t exits_two_step;   /* ... and by the two-step exit (A9c); the rest met eps on a computed residual */
+    float ms_gemm;            /* timing on: CUDA-event time of the Newton-Schulz PRODUCT launches of the last  */
+                              /* evaluation alone (k_ns_gemm; event pairs around every launch), FP64 path      */
+    float tot_ms_gemm;        /* ... summed over the evaluations of the call                                 */
 } sm_stats_t;
 
 /*

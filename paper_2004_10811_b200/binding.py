@@ -73,7 +73,8 @@ class sm_stats_t(C.Structure):
                 ("tot_ms_gather", C.c_float), ("tot_ms_sign", C.c_float),
                 ("spec_lo", C.c_double), ("spec_hi", C.c_double), ("bracket_lo", C.c_double),
                 ("bracket_hi", C.c_double), ("mu_guess", C.c_double),
-                ("exits_predicted", C.c_int32), ("exits_two_step", C.c_int32)]
+                ("exits_predicted", C.c_int32), ("exits_two_step", C.c_int32),
+                ("ms_gemm", C.c_float), ("tot_ms_gemm", C.c_float)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_ if k not in ("mu_trace", "ne_trace", "ne_err_trace", "iter_trace")}

@@ -109,6 +109,8 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
         if (e) cudaEventDestroy(e);
     for (auto& e : p->ev_iter)
         if (e) cudaEventDestroy(e);
+    for (auto& e : p->ev_gemm)
+        if (e) cudaEventDestroy(e);
     delete p;
 }
 
@@ -394,6 +396,7 @@ sm_status_t reset_state(sm_plan* p, cudaStream_t st) {
     SM_CUDA(cudaMemsetAsync(p->d_act_cnt, 0, (size_t)(p->opt.max_iter + 3) * 24, st));
     SM_CUDA(cudaMemsetAsync(p->d_ctrl, 0, sizeof(EvalCtrl), st));
     p->cur_k = 0;
+    p->ev_gemm_n = 0;
     return SM_OK;
 }
 
@@ -586,7 +589,14 @@ sm_status_t evaluate(sm_plan* p, const double* d_in, double mu, double eps, cons
         if (p->timing) {
             cudaEventElapsedTime(&stats->ms_gather, p->ev[0], p->ev[1]);
             cudaEventElapsedTime(&stats->ms_sign, p->ev[1], p->ev[2]);
+            float g = 0.f;  // the product launches alone (event pairs recorded by launch_ns_pair)
+            for (int i = 0; i + 1 < p->ev_gemm_n; i += 2) {
+                float t = 0.f;
+                if (cudaEventElapsedTime(&t, p->ev_gemm[i], p->ev_gemm[i + 1]) == cudaSuccess) g += t;
+            }
+            stats->ms_gemm = g;
         }
+        stats->tot_ms_gemm = stats->ms_gemm;
         stats->tot_sum_iter_n3 = stats->sum_iter_n3;
         stats->tot_gemm_launches = launched;
         stats->tot_evaluations = 1;
@@ -857,10 +867,10 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     sm_stats_t ev;
     int64_t acc_n3 = 0, acc_sym = 0;
     int acc_launch = 0, acc_eval = 0;
-    float acc_g = 0.f, acc_s = 0.f;
+    float acc_g = 0.f, acc_s = 0.f, acc_gemm = 0.f;
     auto accumulate = [&](const sm_stats_t& e) {
         acc_n3 += e.tot_sum_iter_n3; acc_sym += e.tot_sym_flop; acc_launch += e.tot_gemm_launches;
-        acc_eval += 1; acc_g += e.tot_ms_gather; acc_s += e.tot_ms_sign;
+        acc_eval += 1; acc_g += e.tot_ms_gather; acc_s += e.tot_ms_sign; acc_gemm += e.tot_ms_gemm;
     };
     const bool early = p->opt.early_out != 0 && p->opt.precision == 0 && p->opt.shard_world <= 1;
     for (; steps < p->opt.max_mu_steps;) {
@@ -922,7 +932,7 @@ extern "C" sm_status_t sm_density_matrix(sm_plan_t* p, const double* d_vals_in, 
     S->mu = best_mu;
     S->mu_steps = steps;
     S->tot_sum_iter_n3 = acc_n3; S->tot_sym_flop = acc_sym; S->tot_gemm_launches = acc_launch;
-    S->tot_evaluations = acc_eval; S->tot_ms_gather = acc_g; S->tot_ms_sign = acc_s;
+    S->tot_evaluations = acc_eval; S->tot_ms_gather = acc_g; S->tot_ms_sign = acc_s; S->tot_ms_gemm = acc_gemm;
     *mu_inout = best_mu;
     if (d_vals_out && (s = do_scatter(p, b, d_vals_out, S, st))) return s;
     SM_CUDA(cudaStreamSynchronize(st));

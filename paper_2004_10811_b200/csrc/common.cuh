@@ -167,6 +167,8 @@ struct sm_plan {
     int64_t launches = 0;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_iter[2] = {nullptr, nullptr};
+    std::vector<cudaEvent_t> ev_gemm;      // timing: event pairs around the Newton-Schulz GEMM launches of an evaluation
+    int ev_gemm_n = 0;
     int gather_warps = 8, gather_tile_ld = 0, gather_msb = 2, gather_split = 1;
     int gather_hash_size = 32, gather_hash_shift = 27, gather_mpad = 4, gather_mc = 2, gather_map16 = 0;
     int32_t max_col_blocks = 0;  // longest block column

@@ -997,6 +997,18 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
         SM_CUDA(cudaFuncSetAttribute(k_ns_gemm<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_SMEM));
         p->ns_attr_set = 1;
     }
+    // timing: one event before and one after every product launch (sm_stats_t.ms_gemm)
+    auto tick = [&]() -> sm_status_t {
+        if (!p->timing) return SM_OK;
+        if (p->ev_gemm_n == (int)p->ev_gemm.size()) {
+            cudaEvent_t e = nullptr;
+            SM_CUDA(cudaEventCreate(&e));
+            p->ev_gemm.push_back(e);
+        }
+        SM_CUDA(cudaEventRecord(p->ev_gemm[p->ev_gemm_n++], st));
+        return SM_OK;
+    };
+    sm_status_t ts;
     NsArgs a;
     a.tiles = p->d_tiles; a.gersh = p->d_gersh;
     a.buf0 = buf0; a.buf1 = buf1; a.bufY = bufY; a.bufW = bufW; a.partials = p->d_partials;
@@ -1034,7 +1046,9 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     a.sched = p->d_sched + 4 * k;
     if (which & 1) {
         a.act_list = sq_list; a.act_count = sq_count;
+        if ((ts = tick())) return ts;
         k_ns_gemm<0><<<grid, NTHREADS, NS_SMEM, st>>>(a);
+        if ((ts = tick())) return ts;
         k_ns_decide<<<(p->ngroups + 7) / 8, 256, 0, st>>>(a, p->d_tile_first, p->d_tile_count, p->d_sub_dim);
         p->launches += 2;
     }
@@ -1042,9 +1056,11 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
         a.act_list = upd_list; a.act_count = upd_count;
         if (p->opt.order == 3 && bufW) {  // Eq.(19): two products per update
             a.sched = p->d_sched + 4 * k + 1;
+            if ((ts = tick())) return ts;
             k_ns_gemm<2><<<grid, NTHREADS, NS_SMEM, st>>>(a);
             a.sched = p->d_sched + 4 * k + 2;
             k_ns_gemm<3><<<grid, NTHREADS, NS_SMEM, st>>>(a);
+            if ((ts = tick())) return ts;
             p->launches += 2;
         } else {
             if (spec) {
@@ -1055,7 +1071,9 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
                 }
                 NsArgs a4 = a;  // P = (I - Y)^2 of the speculated submatrices into the buffer of X_{k+1}
                 a4.act_list = a.spec_tiles; a4.act_count = a.spec_tile_count; a4.sched = p->d_sched + 4 * k + 3;
+                if ((ts = tick())) return ts;
                 k_ns_gemm<4><<<grid, NTHREADS, NS_SMEM, st>>>(a4);
+                if ((ts = tick())) return ts;
                 SpecArgs sa;
                 sa.list = a.spec_list; sa.count = a.spec_count; sa.tile_first = p->d_tile_first; sa.tile_count = p->d_tile_count;
                 sa.sub_dim = p->d_sub_dim; sa.partials = p->d_partials; sa.res = p->d_res;
@@ -1074,7 +1092,9 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
                 p->launches += 3;
             }
             a.sched = p->d_sched + 4 * k + 1;
+            if ((ts = tick())) return ts;
             k_ns_gemm<1><<<grid, NTHREADS, NS_SMEM, st>>>(a);
+            if ((ts = tick())) return ts;
             p->launches += 1;
             if (thin) {
                 if (!p->thin_attr_set) {
