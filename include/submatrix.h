@@ -108,7 +108,7 @@ typedef struct {
                          /* 2: also the two-step exit (reading A9c): the residual of X_{k+1}  */
                          /* is certified from one product (I - Y_k)^2 without forming         */
                          /* X_{k+1}; if it passes the test above, only the generating rows    */
-                         /* of X_{k+2} are formed (groups of <= 16 generating rows); 0: off   */
+                         /* of X_{k+2} are formed (generating rows spanning <= max(16, n/16)); 0: off */
     int32_t mu_guess;    /* sm_density_matrix, scaling = 1 only: the first interior step of the   [1]  */
                          /* mu search goes to the estimate the Gauss quadrature of the Lanczos     */
                          /* run gives for the target filling (reading A11d) if that lies inside    */

@@ -39,7 +39,12 @@ __host__ __device__ __forceinline__ size_t panel_off(int r, int c, int ld) {
     return (size_t)t0 * ld + (size_t)(c >> 3) * rows_t * 8 + (size_t)((r & 63) * 8 + (c & 7));
 }
 
-constexpr int THIN_MAX_ROWS = 16;  // generating-row span served by the thin last update (k_ns_thin, ns_sign.cu)
+constexpr int THIN_MAX_ROWS = 16;  // generating-row span served by the thin last update (k_ns_thin, ns_sign.cu) ...
+// ... or n / 16 if that is more: a thin product costs (span / 8) passes over n^2 values at HBM speed, a full one n^3
+// multiply-adds at the FP64 rate, so the larger the submatrix, the more generating rows the thin form can carry
+__host__ __device__ __forceinline__ bool thin_span_ok(int span, int n) {
+    return span <= (THIN_MAX_ROWS > n / 16 ? THIN_MAX_ROWS : n / 16);
+}
 
 void set_cuda_error(cudaError_t e, const char* where);
 void set_error_text(const char* msg);

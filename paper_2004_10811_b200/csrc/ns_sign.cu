@@ -693,7 +693,7 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
     // (k_ns_thin3).  The estimate here only decides whether to try: r_{k+1} ~ rt^2 with rt = ||Et||_F / sqrt(n) ~ r / 2
     // for a rescaled step (the rescaling centres the spectrum of Et), r for a plain one.
     if (lane == 0 && goes_on == 1 && a.spec_list && k >= 1 && k + 2 <= a.max_iter &&
-        a.gen_rng[g].y - a.gen_rng[g].x < THIN_MAX_ROWS) {
+        thin_span_ok(a.gen_rng[g].y - a.gen_rng[g].x + 1, n)) {
         const double r = a.res[(size_t)(k & 1) * a.ngroups + g];
         const double al = a.alpha ? a.alpha[(size_t)(k & 1) * a.ngroups + g] : 1.0;
         const double rt = al != 1.0 ? 0.5 * r : r;
@@ -716,7 +716,7 @@ __global__ void __launch_bounds__(256) k_ns_decide(NsArgs a, const int32_t* __re
     if (goes_on == 2 && a.thin_list && a.gen_rng) {
         // predicted exit of a submatrix with few generating rows: its last update is the thin product of k_ns_thin
         const int2 gr = __ldg(a.gen_rng + g);
-        if (gr.y - gr.x < THIN_MAX_ROWS) {
+        if (thin_span_ok(gr.y - gr.x + 1, n)) {
             if (lane == 0) a.thin_list[atomicAdd(a.thin_count, 1)] = g;
             return;
         }

@@ -362,7 +362,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     p->n_tiles = (int64_t)tiles.size();
     // algorithmic flop of the last update of a submatrix that leaves by the predicted exit: only the tiles that
     // hold generating rows (as rows, or mirrored as columns) are computed (ns_sign.cu)
-    // ... or, for groups whose generating rows span at most THIN_MAX_ROWS rows, the thin product of k_ns_thin: span x n x n
+    // ... or, for groups whose generating rows span at most THIN_MAX_ROWS rows (or n / 16), the thin product of k_ns_thin: span x n x n
     int max_ld = 8;
     for (int i = 0; i < ng; ++i) max_ld = std::max(max_ld, p->h_ld[i]);
     p->thin_smem = (size_t)8 * max_ld * 8 <= (size_t)200 * 1024 ? (size_t)8 * max_ld * 8 : 0;  // 8 rows of X in shared memory
@@ -372,7 +372,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
         const int ld = p->h_ld[i], n = p->h_sub_dim[i], nt = (ld + TILE - 1) / TILE;
         const int tl = p->h_gen_rng[2 * i] / TILE, th = p->h_gen_rng[2 * i + 1] / TILE;
         const int span = p->h_gen_rng[2 * i + 1] - p->h_gen_rng[2 * i] + 1;
-        if (p->thin_smem > 0 && span <= THIN_MAX_ROWS) {
+        if (p->thin_smem > 0 && thin_span_ok(span, n)) {
             p->h_final_flop[i] = 2 * (int64_t)span * n * n;
             continue;
         }
