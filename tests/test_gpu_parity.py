@@ -290,6 +290,27 @@ def test_large_member_count_chunked_block_map(B, oracle):
     _sampled_parity(B, oracle, m, 4)
 
 
+def test_timing_fields(B, cfg0):
+    """sm_set_timing: CUDA-event times of the phases of the last evaluation; the product launches alone (ms_gemm,
+    the figure bench.py's roofline entry uses) are part of the Newton-Schulz phase; all zero when timing is off."""
+    torch = _torch()
+    m = cfg0
+    plan = B.plan_from_matrix(m, B.default_options())
+    ws = B.alloc_workspace(plan)
+    vin = torch.from_numpy(m.values).cuda()
+    vout = torch.empty_like(vin)
+    st = B.sm_stats_t()
+    assert B.sm_sign_execute(plan, vin, 0.0, EPS, vout, ws, st) == B.SM_OK
+    assert st.ms_sign == 0.0 and st.ms_gemm == 0.0
+    ref = vout.clone()
+    B.sm_set_timing(plan, True)
+    assert B.sm_sign_execute(plan, vin, 0.0, EPS, vout, ws, st) == B.SM_OK
+    assert 0.0 < st.ms_gemm <= st.ms_sign <= st.ms_total and st.ms_gather > 0.0 and st.ms_scatter > 0.0
+    assert st.tot_ms_gemm == st.ms_gemm
+    assert torch.equal(vout, ref)  # timing changes nothing
+    B.sm_plan_destroy(plan)
+
+
 @pytest.mark.parametrize("per_group", [1, 3, 6, 9])
 def test_last_update_row_spans(B, oracle, per_group):
     """The last update of a predicted exit (reading A9b) is a thin product over the generating rows when they
