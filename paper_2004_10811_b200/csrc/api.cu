@@ -484,7 +484,17 @@ sm_status_t collect_stats(sm_plan* p, sm_stats_t* stats, int* not_conv, cudaStre
         SM_CUDA(cudaMemcpyAsync((void*)res, p->d_res, (size_t)ng * 16, cudaMemcpyDeviceToHost, st));
     }
     SM_CUDA(cudaMemcpyAsync(p->h_pinned_d, p->d_scalars, 8, cudaMemcpyDeviceToHost, st));
+    int32_t* h_spec = reinterpret_cast<int32_t*>(p->h_pinned_d + 6);  // two ints behind the scalars that are read back
+    if (p->d_spec_stat) SM_CUDA(cudaMemcpyAsync(h_spec, p->d_spec_stat, 8, cudaMemcpyDeviceToHost, st));
     SM_CUDA(cudaStreamSynchronize(st));
+    if (p->d_spec_stat) {
+        // two-step exit (A9c): a failed certificate costs one product.  If the last evaluation's speculations mostly
+        // failed, the estimate of k_ns_decide does not fit this input: do not try for the next 8 evaluations.
+        const int ok = h_spec[0] - p->h_spec_prev[0], fail = h_spec[1] - p->h_spec_prev[1];
+        p->h_spec_prev[0] = h_spec[0]; p->h_spec_prev[1] = h_spec[1];
+        if (p->spec_pause > 0) --p->spec_pause;
+        else if (fail > ok && fail >= 16) p->spec_pause = 8;
+    }
     int imin = INT32_MAX, imax = 0, nc = 0, n_pred = 0, n_two = 0;
     double rmax = 0.0;
     int64_t sin3 = 0, symf = 0;

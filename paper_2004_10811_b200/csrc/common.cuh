@@ -113,6 +113,8 @@ struct sm_plan {
     int32_t* d_spec_stat = nullptr;        // [2] certified / failed speculations since plan creation
     size_t thin3_smem = 0;                 // 3 x 8 rows of the largest submatrix; 0: two-step exit off
     int thin3_attr_set = 0;
+    int32_t h_spec_prev[2] = {0, 0};       // totals of d_spec_stat at the previous evaluation's end
+    int spec_pause = 0;                    // evaluations left during which the two-step exit is not tried (it kept failing)
     int32_t* d_sched = nullptr;            // [2*(max_iter+2)] work counters of the persistent GEMM launches
     double* d_ne_part = nullptr;           // [ngroups] per-group electron-count partials
     double* d_scalars = nullptr;           // [8] n_elec, tr D, tr DK, gersh lo/hi

@@ -1035,7 +1035,7 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
     a.thin_count = thin ? C + 2 * (p->opt.max_iter + 3) + k : nullptr;
     // two-step exit (A9c): predict >= 2; lists: slot 2 = speculated submatrices, slot 3 = certified ones
     const int M = p->opt.max_iter + 3;
-    const bool spec = thin && p->opt.predict >= 2 && p->thin3_smem > 0 && p->d_spec_tiles;
+    const bool spec = thin && p->opt.predict >= 2 && p->thin3_smem > 0 && p->d_spec_tiles && p->spec_pause == 0;
     a.spec_list = spec ? p->d_thin_list + (size_t)2 * std::max(p->ngroups, 1) : nullptr;
     a.spec_count = spec ? C + 3 * M + k : nullptr;
     a.spec_tiles = spec ? p->d_spec_tiles : nullptr;
