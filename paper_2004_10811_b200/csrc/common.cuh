@@ -111,7 +111,7 @@ struct sm_plan {
     int thin_attr_set = 0;
     int32_t* d_spec_tiles = nullptr;       // [n_tiles] work list of the MODE 4 launch (two-step exit, ns_sign.cu)
     int32_t* d_spec_stat = nullptr;        // [2] certified / failed speculations since plan creation
-    size_t thin3_smem = 0;                 // 3 x 8 rows of the largest submatrix; 0: two-step exit off
+    size_t thin3_smem = 0;                 // 2 x 8 rows of the largest submatrix; 0: two-step exit off
     int thin3_attr_set = 0;
     int32_t h_spec_prev[2] = {0, 0};       // totals of d_spec_stat at the previous evaluation's end
     int spec_pause = 0;                    // evaluations left during which the two-step exit is not tried (it kept failing)

@@ -785,7 +785,7 @@ __device__ __forceinline__ void thin_pass(const double* __restrict__ sA, const d
             pst[u] = min(64, ld - (r & ~63)) * 8;
         }
         const double* ap = sA + lr * ld + 2 * lk;
-#pragma unroll 2
+#pragma unroll 4
         for (int p = 0; p < nj8; ++p) {
             const double2 af = *reinterpret_cast<const double2*>(ap + 8 * p);
             double2 bf[4];
@@ -804,7 +804,7 @@ __device__ __forceinline__ void thin_pass(const double* __restrict__ sA, const d
     }
 }
 
-__global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin(ThinArgs a) {
+__global__ void __launch_bounds__(THIN_WARPS * 32, 4) k_ns_thin(ThinArgs a) {
     extern __shared__ __align__(16) double sA[];  // [8][ld] rows of X, row-major
     if (a.ctrl[0] != 0) return;
     const int cnt = *a.count;
@@ -894,7 +894,9 @@ __global__ void __launch_bounds__(256) k_ns_spec_decide(SpecArgs a) {
         const double al = a.alpha ? a.alpha[g] : 1.0;
         const double et = (fabs(1.0 - al * al) + al * al * r) * sn;
         const double f = (0.75 + 0.25 * et) * sqrt(p2);  // >= ||E_{k+1}||_F
-        const double next = (0.75 * f * f + 0.25 * f * f * f) / sn;
+        // + the term k_ns_thin3 leaves out: a perturbation of X_{k+2} of Frobenius norm <= al/16 ||P||_F^2 changes
+        // ||X^2 - I||_F by at most twice that (||X||_2 <= 1)
+        const double next = (0.75 * f * f + 0.25 * f * f * f + 0.125 * al * p2) / sn;
         ok = (next < 0.1 * a.eps) ? 1 : 0;  // false for NaN
         if (ok) {
             a.done_iter[g] = k + 2;
@@ -917,12 +919,15 @@ __global__ void __launch_bounds__(256) k_ns_spec_decide(SpecArgs a) {
     for (int t = lane; t < tc; t += 32) a.sq_list[base + t] = tf + t;
 }
 
-// k_ns_thin3: generating rows r of X_{k+2} for the certified submatrices, three thin products per 8 rows:
-//   X_{k+1}[r, :] = 1/2 al (3 X_k[r, :] - X_k[r, :] Y)                           (Y = al^2 X_k^2, stored)
-//   Z = X_{k+1}[r, :] P,   W = Z (I - Y) = Z - Z Y                               (P = (I - Y)^2, from MODE 4)
-//   X_{k+2}[r, :] = 1/2 X_{k+1}[r, :] (3 I - X_{k+1}^2) = X_{k+1}[r, :] + 3/8 Z + 1/8 W
-// since X_{k+1}^2 = I - 3/4 P - 1/4 (I - Y) P and everything commutes.  The rows go into the buffer of X_k (parity of
-// k + 2), which nothing reads any more; P sits in the buffer X_{k+1} would have taken.
+// k_ns_thin3: generating rows r of X_{k+2} for the certified submatrices.  With Et = I - Y, P = Et^2 and
+// X_{k+1} = 1/2 al X_k (2 I + Et),  X_{k+1}^2 = I - 3/4 P - 1/4 Et P  (everything commutes):
+//   X_{k+2} = 1/2 X_{k+1} (3 I - X_{k+1}^2) = 1/2 al X_k (2 I + Et + 3/4 P + 5/8 Et P + 1/8 P^2).
+// Row-wise, with A = X_k[r, :]:  U = A Et = A - A Y  (one thin pass over Y),  C = 3/4 A + 5/8 U,
+//   X_{k+2}[r, :] = 1/2 al (2 A + U + C P)  (one thin pass over P)  + 1/16 al A P^2.
+// The last term is NOT formed (it would be a third pass): ||1/16 al X_k P^2||_F <= al/16 ||P||_F^2 ~ 1e-13, and
+// k_ns_spec_decide adds its effect on the residual, 2 x that / sqrt(n), to the bound it tests and reports.
+// The rows go into the buffer of X_k (parity of k + 2), which nothing reads any more; P sits in the buffer X_{k+1}
+// would have taken.
 struct Thin3Args {
     const int32_t* list;
     const int32_t* count;
@@ -935,8 +940,8 @@ struct Thin3Args {
     const double* P;
     const int32_t* ctrl;
 };
-__global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin3(Thin3Args a) {
-    extern __shared__ __align__(16) double sm3[];  // three arrays [8][ld]
+__global__ void __launch_bounds__(THIN_WARPS * 32, 4) k_ns_thin3(Thin3Args a) {
+    extern __shared__ __align__(16) double sm3[];  // two arrays [8][ld]
     if (a.ctrl[0] != 0) return;
     const int cnt = *a.count;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lr = lane >> 2, lk = lane & 3;
@@ -949,9 +954,8 @@ __global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin3(Thin3Args a) {
         const double* Yg = a.Y + ws;
         const double* Pg = a.P + ws;
         const double al = a.alpha ? a.alpha[g] : 1.0;
-        double* s0 = sm3;            // X_k rows, then Z
-        double* s1 = sm3 + 8 * ld;   // X_{k+1} rows
-        double* s2 = s1 + 8 * ld;    // Z
+        double* s0 = sm3;            // A = X_k rows, then 2 A + U
+        double* s1 = sm3 + 8 * ld;   // A Y, then C = 3/4 A + 5/8 U
         for (int c0 = gr.x; c0 <= gr.y; c0 += 8) {
             __syncthreads();
             for (int e = threadIdx.x; e < 8 * ld; e += blockDim.x) {
@@ -962,24 +966,23 @@ __global__ void __launch_bounds__(THIN_WARPS * 32) k_ns_thin3(Thin3Args a) {
             __syncthreads();
             thin_pass(s0, Yg, ld, w, lane, [&](int j8, const double (&acc)[2]) {
                 const int o = lr * ld + 8 * j8 + 2 * lk;
-                s1[o] = 0.5 * al * fma(3.0, s0[o], -acc[0]);
-                s1[o + 1] = 0.5 * al * fma(3.0, s0[o + 1], -acc[1]);
+                s1[o] = acc[0];
+                s1[o + 1] = acc[1];
             });
             __syncthreads();
-            thin_pass(s1, Pg, ld, w, lane, [&](int j8, const double (&acc)[2]) {
-                const int o = lr * ld + 8 * j8 + 2 * lk;
-                s2[o] = acc[0];
-                s2[o + 1] = acc[1];
-            });
+            for (int e = threadIdx.x; e < 8 * ld; e += blockDim.x) {
+                const double av = s0[e], u = av - s1[e];  // U = A - A Y
+                s1[e] = fma(0.625, u, 0.75 * av);
+                s0[e] = fma(2.0, av, u);
+            }
             __syncthreads();
             const int row = c0 + lr;
             const bool row_ok = row <= gr.y && row < ld;
-            thin_pass(s2, Yg, ld, w, lane, [&](int j8, const double (&acc)[2]) {
+            thin_pass(s1, Pg, ld, w, lane, [&](int j8, const double (&acc)[2]) {
                 if (!row_ok) return;
                 const int col = 8 * j8 + 2 * lk, o = lr * ld + col;
-                const double w0 = s2[o] - acc[0], w1 = s2[o + 1] - acc[1];
                 *reinterpret_cast<double2*>(Xg + panel_off(row, col, ld)) =
-                    make_double2(s1[o] + 0.375 * s2[o] + 0.125 * w0, s1[o + 1] + 0.375 * s2[o + 1] + 0.125 * w1);
+                    make_double2(0.5 * al * (s0[o] + acc[0]), 0.5 * al * (s0[o + 1] + acc[1]));
             });
         }
         __syncthreads();
@@ -1087,7 +1090,7 @@ sm_status_t launch_ns_pair(sm_plan* p, int k, double eps, int decide_only, doubl
                 t3.list = a.thin3_list; t3.count = a.thin3_count; t3.ldv = p->d_ld; t3.ws_off = p->d_ws_off;
                 t3.gen_rng = p->d_gen_rng; t3.alpha = sa.alpha;
                 t3.X = (k & 1) ? buf1 : buf0; t3.Y = bufY; t3.P = (k & 1) ? buf0 : buf1; t3.ctrl = p->d_ctrl;
-                const int tgrid3 = (int)std::min<int64_t>(p->ngroups, (int64_t)p->num_sms * 4);
+                const int tgrid3 = (int)std::min<int64_t>(p->ngroups, (int64_t)p->num_sms * 8);
                 k_ns_thin3<<<tgrid3, THIN_WARPS * 32, p->thin3_smem, st>>>(t3);
                 p->launches += 3;
             }

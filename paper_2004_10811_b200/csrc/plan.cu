@@ -366,7 +366,7 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     int max_ld = 8;
     for (int i = 0; i < ng; ++i) max_ld = std::max(max_ld, p->h_ld[i]);
     p->thin_smem = (size_t)8 * max_ld * 8 <= (size_t)200 * 1024 ? (size_t)8 * max_ld * 8 : 0;  // 8 rows of X in shared memory
-    p->thin3_smem = (size_t)24 * max_ld * 8 <= (size_t)200 * 1024 ? (size_t)24 * max_ld * 8 : 0;  // three such arrays (k_ns_thin3)
+    p->thin3_smem = (size_t)16 * max_ld * 8 <= (size_t)200 * 1024 ? (size_t)16 * max_ld * 8 : 0;  // two such arrays (k_ns_thin3)
     p->h_final_flop.assign(ng, 0);
     for (int i = 0; i < ng; ++i) {
         const int ld = p->h_ld[i], n = p->h_sub_dim[i], nt = (ld + TILE - 1) / TILE;
