@@ -435,9 +435,9 @@ sm_status_t ns_loop(sm_plan* p, const Bufs& b, double eps, int k_end, int* all_d
     bool stopped = false;
     sm_status_t s;
     // how far to enqueue before the first look at the control block: what the previous evaluation of this plan
-    // needed, plus two (launches behind the device-side stop are empty but not free), at most check_every
+    // needed, plus one (launches behind the device-side stop are empty but not free), at most check_every
     int batch = p->opt.check_every;
-    if (p->last_eval_iters > 0) batch = std::min(batch, p->last_eval_iters + 2);
+    if (p->last_eval_iters > 0) batch = std::min(batch, p->last_eval_iters + 1);
     for (; k < k_end && k <= max_iter && !stopped; ++k) {
         const int last = k == max_iter ? 1 : 0;
         if ((s = launch_pair(p, k, eps, last, b, st, 1))) return s;
