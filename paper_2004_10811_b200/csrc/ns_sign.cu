@@ -9,6 +9,11 @@
 //   MODE 1:  X' = -1/2 (X Y - 3 X)     (iteration 0 folds the spectral scale 1/s_i into the
 //                                        coefficients, so that no scaling pass is needed)
 //   MODE 2/3: the two products of the third-order iteration Eq.(19) L348 (option order = 3).
+//   MODE 4:  P  = (I - Y)^2 + ||P||_F^2  the certificate of the two-step exit (reading A9c).
+// The end of a submatrix's iteration is not made of full products: a predicted exit (A9b) forms only the
+// generating rows of its last update (k_ns_thin), the two-step exit (A9c) certifies the residual of X_{k+1}
+// from P and forms only the generating rows of X_{k+2} (k_ns_spec_decide, k_ns_thin3) -- thin products bound by
+// HBM, further down in this file.
 // A launch issued after the evaluation was stopped on the device (EvalCtrl, common.cuh) is empty.
 // X, Y and X' are symmetric polynomials of the same matrix, so only tiles on or below the diagonal
 // are computed and every element is stored together with its mirror image: the stored matrices are
