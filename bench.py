@@ -362,7 +362,26 @@ def run_extras(args, m, B, torch, plan, info, ws, d_in, d_out, mu, hbm_peak):
     B.sm_sign_execute(plan, d_in, mu, EPS, tmp_out, ws, st)
     torch.cuda.synchronize()
     out["fp64_sign_evaluation"] = {"ms_sign": st.ms_sign, "ms_gather": st.ms_gather, "ms_scatter": st.ms_scatter,
-                                   "ms_total": st.ms_total, "iter_min": st.iter_min, "iter_max": st.iter_max}
+                                   "ms_total": st.ms_total, "iter_min": st.iter_min, "iter_max": st.iter_max,
+                                   "exits_predicted": st.exits_predicted, "exits_two_step": st.exits_two_step}
+    # the same evaluation with the exits of readings A9b / A9c switched off (predict = 1: predicted exit only; 0: every
+    # convergence confirmed by a computed residual), and how far the results are from the default's
+    d_def = tmp_out.clone()
+    out["exit_modes"] = {"predict=2 (default)": {"ms_sign": st.ms_sign, "max_residual": st.max_residual}}
+    for pr in (1, 0):
+        planp = B.plan_from_matrix(m, B.default_options(predict=pr))
+        need = B.sm_plan_query(planp).workspace_bytes
+        wsp = ws if need <= ws.numel() * 8 else B.alloc_workspace(planp)
+        B.sm_set_timing(planp, True)
+        for _ in range(2):
+            rc = B.sm_sign_execute(planp, d_in, mu, EPS, tmp_out, wsp, st)
+        torch.cuda.synchronize()
+        out["exit_modes"][f"predict={pr}"] = {
+            "status": int(rc), "ms_sign": st.ms_sign, "max_residual": st.max_residual, "iter_max": st.iter_max,
+            "exits_predicted": st.exits_predicted, "exits_two_step": st.exits_two_step,
+            "max_abs_diff_vs_default": float((tmp_out - d_def).abs().max().item())}
+        B.sm_plan_destroy(planp)
+        del wsp
     return out
 
 
