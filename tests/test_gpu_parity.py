@@ -351,6 +351,28 @@ def test_last_update_row_spans(B, oracle, per_group):
     B.sm_plan_destroy(plan); B.sm_plan_destroy(plan2)
 
 
+def test_last_update_multi_chunk_dzvp(B, oracle):
+    """DZVP molecules: 23 generating rows per group (three chunks of 8 in k_ns_thin / k_ns_thin3, allowed by the
+    n / 16 rule at n ~ 540).  Full GPU run, oracle on three groups; same result with the exits switched off."""
+    m = W.water_like(24, "DZVP", 6.0, seed=7)
+    idx = oracle.Index(m)
+    groups = np.array([0, 5, 11], dtype=np.int32)
+    lam, _, _, _ = oracle.eig_groups(idx, m.values, groups)
+    srt = np.sort(lam)
+    k = int(np.argmax(np.diff(srt)))
+    mu = 0.5 * (srt[k] + srt[k + 1])
+    assert idx.sub_dim.min() >= 23 * 16  # the thin forms serve the 23-row spans
+    plan, st, d_gpu, stats, _, _ = _run_sign(B, m, mu=mu)
+    assert st == B.SM_OK and stats.not_converged == 0 and stats.max_residual < EPS
+    assert stats.exits_two_step + stats.exits_predicted > 0
+    d_or = oracle.density(idx, m.values, mu, groups)
+    mask, _ = _column_mask(idx, m, groups)
+    assert np.abs(d_gpu - d_or)[mask].max() <= TOL_D
+    plan0, st0, d_ref, stats0, _, _ = _run_sign(B, m, mu=mu, opt=B.default_options(predict=0))
+    assert st0 == B.SM_OK and stats0.exits_two_step == 0 and np.abs(d_gpu - d_ref).max() <= 2e-12
+    B.sm_plan_destroy(plan); B.sm_plan_destroy(plan0)
+
+
 def test_ragged_blocks_and_scattered_groups(B, oracle):
     for seed in range(3):
         m = W.random_block_pattern(nb=30 + seed, density=0.2, max_bs=7, seed=10 + seed)
