@@ -26,6 +26,7 @@ constexpr int LZ_STEPS = 24;  // extreme Ritz values within ~1 % of the spread (
 // all dense columns of the block column in registers, so index and values of a block are read once.
 // rec[b] = (value offset lo, hi, first basis function of the block's row, its height): ONE 16-byte load per stored
 // block instead of a chain of four dependent index loads.
+// (Block columns of width 1, 4 and 5 take the streaming form lz_col_s below; this one serves the other widths.)
 template <int BC>
 __device__ __forceinline__ double lz_col(int lane, int oc, int64_t p0, int64_t p1, const int4* __restrict__ rec,
                                          const double* __restrict__ vals, const double* __restrict__ x,
@@ -54,6 +55,63 @@ __device__ __forceinline__ double lz_col(int lane, int oc, int64_t p0, int64_t p
         dot = fma(v, x[oc + q], dot);
     }
     return dot;
+}
+
+// Streaming form of the same product: a per-value map (x index | q << 28, built once per plan by k_lz_map) lets the
+// lanes of the warp walk the values of the block column in storage order -- coalesced 8-byte and 4-byte loads, four
+// per lane in flight -- instead of one block per lane.
+template <int BC>
+__device__ __forceinline__ double lz_col_s(int lane, int oc, int64_t v0, int64_t v1, const uint32_t* __restrict__ map,
+                                           const double* __restrict__ vals, const double* __restrict__ x,
+                                           double* __restrict__ y) {
+    double a[BC];
+#pragma unroll
+    for (int q = 0; q < BC; ++q) a[q] = 0.0;
+    for (int64_t e0 = v0 + lane; e0 < v1; e0 += 128) {
+        uint32_t m[4];
+        double v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int64_t e = e0 + 32 * u;
+            m[u] = e < v1 ? __ldcs(map + e) : 0u;
+            v[u] = e < v1 ? __ldcs(vals + e) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const double t = v[u] * x[m[u] & 0x0fffffffu];
+            const int q = (int)(m[u] >> 28);
+#pragma unroll
+            for (int qq = 0; qq < BC; ++qq) a[qq] += (BC == 1 || q == qq) ? t : 0.0;
+        }
+    }
+    double dot = 0.0;
+#pragma unroll
+    for (int q = 0; q < BC; ++q) {
+        double s = a[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) y[oc + q] = s;
+        dot = fma(s, x[oc + q], dot);
+    }
+    return dot;
+}
+
+// map[e] for every stored value e of block column c: one warp per block column, lanes over the elements of a block
+__global__ void __launch_bounds__(256)
+k_lz_map(int nb, const int32_t* __restrict__ blk_size, const int32_t* __restrict__ blk_off,
+         const int64_t* __restrict__ colptr, const int32_t* __restrict__ rowidx, const int64_t* __restrict__ val_off,
+         uint32_t* __restrict__ map) {
+    const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (c >= nb) return;
+    const int lane = threadIdx.x & 31, bc = blk_size[c];
+    for (int64_t b = colptr[c]; b < colptr[c + 1]; ++b) {
+        const int r = rowidx[b], br = blk_size[r], ro = blk_off[r];
+        const int64_t v = val_off[b];
+        for (int w = lane; w < br * bc; w += 32) {
+            const int q = w / br, el = w - q * br;
+            map[v + w] = (uint32_t)(ro + el) | ((uint32_t)q << 28);
+        }
+    }
 }
 
 // Gauss quadrature of the k x k Lanczos tridiagonal T (diag alpha, off-diagonal beta): thread j finds
@@ -128,9 +186,10 @@ __device__ void lz_quadrature_body(int k, const double* __restrict__ alpha, cons
 // in a fixed order), alpha = w.v, w -= alpha v + beta_prev v_prev, beta = ||w||, v_next = w / beta;
 // finally the Gauss quadrature of T.  Reductions: per-CTA partials in a fixed order, then the same fixed-order
 // sum over the CTAs in every thread that needs it -- deterministic, no floating-point atomics.
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 k_lz_fused(int nb, int64_t n, int steps, const int32_t* __restrict__ blk_size, const int32_t* __restrict__ blk_off,
            const int64_t* __restrict__ colptr, const int4* __restrict__ rec,
+           const uint32_t* __restrict__ vmap, const int64_t* __restrict__ val_off,
            const double* __restrict__ vals, double* __restrict__ vb0, double* __restrict__ vb1, double* __restrict__ vb2,
            double* __restrict__ alpha, double* __restrict__ beta, double* __restrict__ part, double margin,
            double* __restrict__ outp) {
@@ -177,6 +236,14 @@ k_lz_fused(int nb, int64_t n, int steps, const int32_t* __restrict__ blk_size, c
             const int bc = blk_size[c], oc = blk_off[c];
             const int64_t p0 = colptr[c], p1 = colptr[c + 1];
             double d;
+            if (vmap && (bc == 1 || bc == 4 || bc == 5)) {
+                const int64_t v0 = val_off[p0], v1 = val_off[p1];
+                if (bc == 1) d = lz_col_s<1>(lane, oc, v0, v1, vmap, vals, v, w);
+                else if (bc == 4) d = lz_col_s<4>(lane, oc, v0, v1, vmap, vals, v, w);
+                else d = lz_col_s<5>(lane, oc, v0, v1, vmap, vals, v, w);
+                dot += d;
+                continue;
+            }
             switch (bc) {
                 case 1: d = lz_col<1>(lane, oc, p0, p1, rec, vals, v, w); break;
                 case 4: d = lz_col<4>(lane, oc, p0, p1, rec, vals, v, w); break;
@@ -286,7 +353,13 @@ sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t s
     double* part = outp + 72;
     int steps = (int)std::min<int64_t>(LZ_STEPS, n), nb = p->nb;
     double margin = 0.03;
-    void* args[] = {&nb, &n, &steps, &p->d_blk_size, &p->d_blk_off, &p->d_colptr, &p->d_lz_rec, &vals,
+    if (!p->d_lz_map && n < (1 << 28)) {  // once per plan (pattern only): the map of the streaming mat-vec
+        SM_CUDA(cudaMalloc((void**)&p->d_lz_map, (size_t)std::max<int64_t>(p->nnz, 1) * 4));
+        k_lz_map<<<(p->nb + 7) / 8, 256, 0, st>>>(p->nb, p->d_blk_size, p->d_blk_off, p->d_colptr, p->d_rowidx, p->d_val_off,
+                                                p->d_lz_map);
+        p->launches++;
+    }
+    void* args[] = {&nb, &n, &steps, &p->d_blk_size, &p->d_blk_off, &p->d_colptr, &p->d_lz_rec, &p->d_lz_map, &p->d_val_off, &vals,
                     &vb0, &vb1, &vb2, &alpha, &beta, &part, &margin, &outp};
     SM_CUDA(cudaLaunchCooperativeKernel((const void*)k_lz_fused, dim3(p->lz_grid), dim3(256), args, 0, st));
     p->launches++;
