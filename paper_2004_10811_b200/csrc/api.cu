@@ -95,7 +95,7 @@ extern "C" void sm_plan_destroy(sm_plan_t* p) {
                     p->d_partials, p->d_counters, p->d_sched, p->d_act, p->d_act_cnt, p->d_thin_list, p->d_spec_tiles, p->d_spec_stat, p->d_ne_part, p->d_scalars, p->d_red, p->d_stage_in,
                     p->d_stage_out, p->d_bound, p->d_bound_part, p->d_lz, p->d_tiles32, p->d_ws_off32,
                     p->d_tile_first32, p->d_tile_count32, p->d_partials32, p->d_src_map, p->d_col_rec, p->d_gg, p->d_ctrl, p->d_gl_ptr, p->d_gl,
-                    p->d_alpha, p->d_lmin, p->d_lz_rec, p->d_lz_map, p->d_eig_ptr, p->d_eig_lam, p->d_eig_w, p->d_eig_sigma, p->d_eig_order,
+                    p->d_alpha, p->d_lmin, p->d_lz_rec, p->d_lz_map, p->d_col_val, p->d_eig_ptr, p->d_eig_lam, p->d_eig_w, p->d_eig_sigma, p->d_eig_order,
                     p->d_eig_state};
     for (void* q : ptrs)
         if (q) cudaFree(q);

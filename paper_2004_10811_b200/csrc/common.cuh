@@ -144,6 +144,7 @@ struct sm_plan {
     int4* d_col_rec = nullptr;             // [nb] scatter column records (first value lo/hi, value count, group)
     int scatter_chunks = 1;
     double* d_lz = nullptr;                // Lanczos vectors / tridiagonal (spectral.cu), lazily allocated
+    int64_t* d_col_val = nullptr;          // [nb + 1] offset of the first value of every block column
     uint32_t* d_lz_map = nullptr;          // [nnz] per stored value: index into x | dense column q << 28 (streaming mat-vec)
     int4* d_lz_rec = nullptr;              // [nnzb] per stored block: value offset (lo, hi), blk_off of its row, its height
     double lz_lo = 0.0, lz_hi = 0.0;       // estimated [lambda_min, lambda_max] of K~ (widened)

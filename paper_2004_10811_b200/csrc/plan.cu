@@ -222,6 +222,9 @@ sm_status_t build_index_device(sm_plan* p, cudaStream_t st) {
     if ((s = upload(&p->d_rowidx, p->h_rowidx.data(), p->nnzb, st))) return s;
     if ((s = upload(&p->d_val_off, val_off.data(), p->nnzb + 1, st))) return s;
     if (p->opt.scaling == 1) {  // packed block records of the Lanczos mat-vec (spectral.cu)
+        std::vector<int64_t> colval((size_t)nb + 1);  // first value of every block column: one load instead of two dependent ones
+        for (int c = 0; c <= nb; ++c) colval[c] = val_off[p->h_colptr[c]];
+        if ((s = upload(&p->d_col_val, colval.data(), (size_t)nb + 1, st))) return s;
         std::vector<int4> rec((size_t)p->nnzb);
         for (int64_t q = 0; q < p->nnzb; ++q) {
             const int r = p->h_rowidx[q];

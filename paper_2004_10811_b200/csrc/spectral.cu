@@ -234,16 +234,16 @@ k_lz_fused(int nb, int64_t n, int steps, const int32_t* __restrict__ blk_size, c
         double dot = 0.0;
         for (int c = gw; c < nb; c += nwarps) {
             const int bc = blk_size[c], oc = blk_off[c];
-            const int64_t p0 = colptr[c], p1 = colptr[c + 1];
             double d;
             if (vmap && (bc == 1 || bc == 4 || bc == 5)) {
-                const int64_t v0 = val_off[p0], v1 = val_off[p1];
+                const int64_t v0 = val_off[c], v1 = val_off[c + 1];  // val_off: first value per block COLUMN here
                 if (bc == 1) d = lz_col_s<1>(lane, oc, v0, v1, vmap, vals, v, w);
                 else if (bc == 4) d = lz_col_s<4>(lane, oc, v0, v1, vmap, vals, v, w);
                 else d = lz_col_s<5>(lane, oc, v0, v1, vmap, vals, v, w);
                 dot += d;
                 continue;
             }
+            const int64_t p0 = colptr[c], p1 = colptr[c + 1];
             switch (bc) {
                 case 1: d = lz_col<1>(lane, oc, p0, p1, rec, vals, v, w); break;
                 case 4: d = lz_col<4>(lane, oc, p0, p1, rec, vals, v, w); break;
@@ -359,7 +359,7 @@ sm_status_t launch_lanczos_bounds(sm_plan* p, const double* vals, cudaStream_t s
                                                 p->d_lz_map);
         p->launches++;
     }
-    void* args[] = {&nb, &n, &steps, &p->d_blk_size, &p->d_blk_off, &p->d_colptr, &p->d_lz_rec, &p->d_lz_map, &p->d_val_off, &vals,
+    void* args[] = {&nb, &n, &steps, &p->d_blk_size, &p->d_blk_off, &p->d_colptr, &p->d_lz_rec, &p->d_lz_map, &p->d_col_val, &vals,
                     &vb0, &vb1, &vb2, &alpha, &beta, &part, &margin, &outp};
     SM_CUDA(cudaLaunchCooperativeKernel((const void*)k_lz_fused, dim3(p->lz_grid), dim3(256), args, 0, st));
     p->launches++;
